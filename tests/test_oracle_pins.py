@@ -1,0 +1,359 @@
+"""Pins for the CPU oracle (oracle/dit_oracle.py) against things OTHER than itself: brute force in pure
+Python, closed forms, invariants, torch library routines as special cases, stored hand-computed fixtures.
+SURVEY.md §8(c) "What pins the oracle"; BASELINE.json north_star invariants.  CPU only."""
+import math
+import os
+
+import pytest
+import torch
+
+from oracle import dit_oracle as O
+from paper_2606_13501_b200 import synth
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+F64 = torch.float64
+
+
+def _rows(name):
+    with open(os.path.join(GOLD, name)) as f:
+        return [[float(t) for t in ln.split()] for ln in f if not ln.startswith("#")]
+
+
+def rnd(*shape, seed=0, name="x"):
+    return synth.normal(seed, name, shape, dtype=F64)
+
+
+# ---------------------------------------------------------------- attention
+def brute_attention(q, k, v, scale):
+    """triple loop, direct exp with NO max subtraction (pure Python floats)."""
+    Nq, H, d = q.shape
+    Nk = k.shape[0]
+    o = torch.zeros(Nq, H, d, dtype=F64)
+    lse = torch.zeros(Nq, H, dtype=F64)
+    for i in range(Nq):
+        for h in range(H):
+            e = []
+            for j in range(Nk):
+                s = 0.0
+                for c in range(d):
+                    s += float(q[i, h, c]) * float(k[j, h, c])
+                e.append(math.exp(s * scale))
+            z = sum(e)
+            lse[i, h] = math.log(z)
+            for c in range(d):
+                o[i, h, c] = sum(e[j] * float(v[j, h, c]) for j in range(Nk)) / z
+    return o, lse
+
+
+def test_attention_brute_force_tiny():
+    q, k, v = rnd(5, 2, 4, name="q"), rnd(7, 2, 4, name="k"), rnd(7, 2, 4, name="v")
+    o, lse = O.attention(q, k, v)
+    ob, lb = brute_attention(q, k, v, 1 / math.sqrt(4))
+    assert torch.allclose(o, ob, rtol=1e-12, atol=1e-13)
+    assert torch.allclose(lse, lb, rtol=1e-12, atol=1e-13)
+
+
+def test_attention_closed_form_fixture():
+    r = _rows("attention_2x2_closed_form.txt")[0]
+    q = torch.tensor(r[0:2], dtype=F64).reshape(2, 1, 1)
+    k = torch.tensor(r[2:4], dtype=F64).reshape(2, 1, 1)
+    v = torch.tensor(r[4:6], dtype=F64).reshape(2, 1, 1)
+    o, lse = O.attention(q, k, v, scale=1.0)
+    assert torch.allclose(o.reshape(-1), torch.tensor(r[6:8], dtype=F64), rtol=1e-13)
+    assert torch.allclose(lse.reshape(-1), torch.tensor(r[8:10], dtype=F64), rtol=1e-13)
+
+
+def test_attention_matches_torch_sdpa():
+    q, k, v = rnd(33, 3, 16, name="q"), rnd(50, 3, 16, name="k"), rnd(50, 3, 16, name="v")
+    o, _ = O.attention(q, k, v)
+    ref = torch.nn.functional.scaled_dot_product_attention(q.permute(1, 0, 2), k.permute(1, 0, 2), v.permute(1, 0, 2))
+    assert torch.allclose(o, ref.permute(1, 0, 2), rtol=1e-10, atol=1e-12)
+
+
+def test_softmax_rows_sum_to_one_via_ones_value():
+    # V = all ones  =>  O = sum_j p_ij = 1 exactly the row sum of the softmax
+    q, k = rnd(9, 2, 8, name="q") * 3, rnd(11, 2, 8, name="k") * 3
+    o, _ = O.attention(q, k, torch.ones(11, 2, 8, dtype=F64))
+    assert torch.allclose(o, torch.ones_like(o), rtol=0, atol=1e-14)
+
+
+def test_identical_keys_give_mean_of_v():
+    q, v = rnd(6, 2, 8, name="q"), rnd(10, 2, 8, name="v")
+    k = rnd(1, 2, 8, name="k").expand(10, 2, 8).contiguous()
+    o, lse = O.attention(q, k, v)
+    assert torch.allclose(o, v.mean(0, keepdim=True).expand_as(o), rtol=1e-13, atol=1e-14)
+    s = torch.einsum("qhd,hd->qh", q, k[0]) / math.sqrt(8)
+    assert torch.allclose(lse, s + math.log(10), rtol=1e-13)
+    o0, _ = O.attention(torch.zeros_like(q), rnd(10, 2, 8, name="k2"), v)           # q = 0 => mean of V
+    assert torch.allclose(o0, v.mean(0, keepdim=True).expand_as(o0), rtol=1e-13, atol=1e-14)
+
+
+def test_single_key_permutation_linearity_shift_peaky():
+    q, k, v = rnd(6, 2, 8, name="q"), rnd(10, 2, 8, name="k"), rnd(10, 2, 8, name="v")
+    o, lse = O.attention(q, k, v)
+    o1, _ = O.attention(q, k[:1], v[:1])
+    assert torch.allclose(o1, v[:1].expand_as(o1))                                    # Nk = 1 => v0
+    perm = torch.tensor([3, 1, 4, 0, 9, 2, 6, 5, 8, 7])
+    op, lp = O.attention(q, k[perm], v[perm])
+    assert torch.allclose(op, o, rtol=1e-12, atol=1e-14) and torch.allclose(lp, lse, rtol=1e-12)
+    o2, _ = O.attention(q, k, 2 * v)
+    assert torch.allclose(o2, 2 * o, rtol=1e-13)                                      # linear in V
+    u = rnd(1, 2, 8, name="u")
+    os_, _ = O.attention(q, k + u, v)
+    assert torch.allclose(os_, o, rtol=1e-10, atol=1e-12)                             # softmax shift invariance
+    kp = k.clone(); kp[4] = q[2] * 60.0 / (q[2] ** 2).sum(-1, keepdim=True) * math.sqrt(8)   # logit +60 for row 2
+    opk, _ = O.attention(q[2:3], kp, v)
+    assert torch.allclose(opk, v[4:5], atol=1e-9)                                     # peaky: max subtraction works
+    big = O.attention(q * 1e3, k, v)[0]
+    assert torch.isfinite(big).all()
+
+
+# ---------------------------------------------------------------- partial + merge
+@pytest.mark.parametrize("P", [1, 2, 3, 4, 8])
+def test_split_p_invariance(P):
+    q, k, v = rnd(12, 2, 8, name="q"), rnd(37, 2, 8, name="k"), rnd(37, 2, 8, name="v")
+    o, lse = O.attention(q, k, v)
+    op, lp = O.attention_split(q, k, v, P)
+    assert torch.allclose(op, o, rtol=1e-12, atol=1e-14) and torch.allclose(lp, lse, rtol=1e-12)
+
+
+def test_merge_closed_forms():
+    q, k, v = rnd(5, 2, 8, name="q"), rnd(9, 2, 8, name="k"), rnd(9, 2, 8, name="v")
+    o, lse = O.attention(q, k, v)
+    om, lm = O.merge_partials([o] * 4, [lse] * 4)                                     # P copies => O, LSE + ln P
+    assert torch.allclose(om, o, rtol=1e-13) and torch.allclose(lm, lse + math.log(4), rtol=1e-13)
+    oe, le = O.attention(q, k[:0], v[:0])                                             # empty shard: 0, -inf
+    assert (oe == 0).all() and torch.isinf(le).all() and (le < 0).all()
+    om, lm = O.merge_partials([oe, o], [le, lse])
+    assert torch.equal(om, o) and torch.equal(lm, lse)
+    om, lm = O.merge_partials([oe, oe], [le, le])
+    assert (om == 0).all() and torch.isinf(lm).all()
+    assert O.shard_bounds(10, 4) == [(0, 3), (3, 6), (6, 9), (9, 10)]
+    assert O.shard_bounds(5, 8)[-1] == (5, 5)
+    # P larger than Nk (empty tail shards) still reproduces the unsplit result
+    o8, l8 = O.attention_split(q, k[:5], v[:5], 8)
+    o1, l1 = O.attention(q, k[:5], v[:5])
+    assert torch.allclose(o8, o1, rtol=1e-12) and torch.allclose(l8, l1, rtol=1e-12)
+
+
+# ---------------------------------------------------------------- norms, activations, rope
+def test_layer_norm_properties_and_library():
+    x = rnd(7, 48, name="x") * 3 + 1.5
+    y = O.layer_norm(x, 1e-6)
+    assert torch.allclose(y.mean(-1), torch.zeros(7, dtype=F64), atol=1e-14)
+    var = x.var(-1, unbiased=False)
+    assert torch.allclose(y.var(-1, unbiased=False), var / (var + 1e-6), rtol=1e-12)
+    assert torch.allclose(y, torch.nn.functional.layer_norm(x, (48,), eps=1e-6), rtol=1e-11, atol=1e-13)
+    const = torch.full((2, 48), 3.25, dtype=F64)
+    sh, sc = rnd(48, name="sh"), rnd(48, name="sc")
+    assert torch.allclose(O.modulate(const, sh, sc, 1e-6), sh.expand(2, 48))          # constant row => y = shift
+    z = torch.zeros(48, dtype=F64)
+    assert torch.equal(O.modulate(x, z, z, 1e-6), y)                                  # zero shift/scale => plain LN
+    assert torch.allclose(O.modulate(x, sh, sc, 1e-6), y * (1 + sc) + sh)             # '1 + scale' (R3)
+
+
+def test_rms_norm_properties():
+    x = rnd(5, 3, 16, name="x") * 2
+    one = torch.ones(16, dtype=F64)
+    y = O.rms_norm_heads(x, one, 1e-6)
+    ms = (x ** 2).mean(-1)
+    assert torch.allclose((y ** 2).mean(-1).sqrt(), 1 / torch.sqrt(1 + 1e-6 / ms), rtol=1e-12)
+    assert torch.allclose(O.rms_norm_heads(7.0 * x, one, 0.0), O.rms_norm_heads(x, one, 0.0), rtol=1e-13)
+    g = rnd(16, name="g")
+    assert torch.allclose(O.rms_norm_heads(x, g, 1e-6), y * g, rtol=1e-13)
+    manual = x[2, 1] / math.sqrt(sum(float(t) ** 2 for t in x[2, 1]) / 16 + 1e-6) * g
+    assert torch.allclose(O.rms_norm_heads(x, g, 1e-6)[2, 1], manual, rtol=1e-13)
+
+
+def test_gelu_silu():
+    for z, g in _rows("gelu_tanh_points.txt"):
+        assert abs(float(O.gelu_tanh(torch.tensor(z, dtype=F64))) - g) <= 1e-15 * max(1, abs(g))
+    z = torch.linspace(-6, 6, 101, dtype=F64)
+    assert torch.allclose(O.gelu_tanh(z) - O.gelu_tanh(-z), z, atol=1e-14)            # odd-part identity
+    assert (O.gelu_tanh(z) - torch.nn.functional.gelu(z)).abs().max() < 1e-3          # close to the erf form
+    assert torch.allclose(O.gelu_tanh(z), torch.nn.functional.gelu(z, approximate="tanh"), atol=1e-14)
+    assert torch.allclose(O.silu(z), torch.nn.functional.silu(z), atol=1e-14)
+    assert float(O.silu(torch.tensor(0.0, dtype=F64))) == 0.0
+
+
+def test_rope_fixture_identity_norm_relative():
+    rows = _rows("rope_points.txt")
+    pos = torch.tensor([[0, 3, 0]])
+    ang = O.rope_angles(pos, (0, 8, 0), 10000.0)
+    x = torch.zeros(1, 1, 8, dtype=F64); x[..., 0::2] = 1.0                            # pairs (1, 0)
+    y = O.apply_rope(x, ang)
+    for j, c, s in rows:
+        assert abs(float(y[0, 0, 2 * int(j)]) - c) < 1e-15 and abs(float(y[0, 0, 2 * int(j) + 1]) - s) < 1e-15
+    # segments are laid out in axis order (f, h, w): with dims (4, 2, 2) the h axis owns elements 4..5
+    a3 = O.rope_angles(torch.tensor([[5, 7, 11]]), (4, 2, 2), 10000.0)
+    assert torch.allclose(a3, torch.tensor([[5.0, 5.0 * 10000 ** -0.5, 7.0, 11.0]], dtype=F64))
+    q = rnd(6, 2, 8, name="q"); k = rnd(6, 2, 8, name="k")
+    p0 = torch.zeros(6, 3, dtype=torch.int64)
+    assert torch.equal(O.apply_rope(q, O.rope_angles(p0, (0, 4, 4), 1e4)), q)          # pos 0 => identity
+    pos = torch.stack([torch.zeros(6, dtype=torch.int64), torch.arange(6) % 3, torch.arange(6) // 3], 1)
+    a = O.rope_angles(pos, (0, 4, 4), 1e4)
+    qr, kr = O.apply_rope(q, a), O.apply_rope(k, a)
+    assert torch.allclose((qr ** 2).sum(-1), (q ** 2).sum(-1), rtol=1e-13)            # norm preserving
+    pos2 = pos + torch.tensor([0, 5, 9])
+    a2 = O.rope_angles(pos2, (0, 4, 4), 1e4)
+    s1 = torch.einsum("qhd,khd->hqk", qr, kr)
+    s2 = torch.einsum("qhd,khd->hqk", O.apply_rope(q, a2), O.apply_rope(k, a2))
+    assert torch.allclose(s1, s2, rtol=1e-10, atol=1e-12)                             # relative-position property
+
+
+def test_token_positions_and_patchify():
+    pos = O.token_positions((2, 3, 4))
+    assert pos.shape == (24, 3) and pos[0].tolist() == [0, 0, 0] and pos[5].tolist() == [0, 1, 1]
+    assert pos[(1 * 3 + 2) * 4 + 3].tolist() == [1, 2, 3]
+    lat = rnd(3, 2, 4, 6, name="lat")
+    tok = O.patchify(lat, (1, 2, 2))
+    assert tok.shape == (2 * 2 * 3, 3 * 4)
+    # token (f'=1, h'=1, w'=2), feature (c=2, i=0, j=1, k=0)  ==  lat[2, 1, 2*1+1, 2*2+0]
+    assert tok[(1 * 2 + 1) * 3 + 2, ((2 * 1 + 0) * 2 + 1) * 2 + 0] == lat[2, 1, 3, 4]
+    assert torch.equal(O.unpatchify(tok, (1, 2, 2), lat.shape), lat)                  # round trip
+    lat3 = rnd(2, 4, 4, 4, name="lat3")
+    t3 = O.patchify(lat3, (2, 2, 2))
+    assert t3[(1 * 2 + 0) * 2 + 1, ((1 * 2 + 1) * 2 + 0) * 2 + 1] == lat3[1, 3, 0, 3]
+    assert torch.equal(O.unpatchify(t3, (2, 2, 2), lat3.shape), lat3)
+
+
+def test_timestep_embedding_closed_forms():
+    e0 = synth.timestep_embedding([0.0], 256)
+    assert torch.equal(e0[0, :128], torch.ones(128)) and torch.equal(e0[0, 128:], torch.zeros(128))
+    e = synth.timestep_embedding([500.0], 256)
+    assert abs(float(e[0, 0]) - math.cos(500.0)) < 1e-6 and abs(float(e[0, 128]) - math.sin(500.0)) < 1e-6
+    w5 = math.exp(-math.log(1e4) * 5 / 128)
+    assert abs(float(e[0, 5]) - math.cos(500 * w5)) < 1e-6
+
+
+# ---------------------------------------------------------------- step composition
+def _tiny(**kw):
+    d = dict(n_blocks=2, hidden=32, n_heads=2, head_dim=16, mlp_dim=64, latent_channels=2, temb_dim=16, cond_dim=24,
+             latent_grid=(1, 8, 8), n_cond=5, dtype="f32")
+    d.update(kw)
+    return synth.cfg1(**d)
+
+
+def _run(s, W=None, I=None, **kw):
+    W = synth.make_weights(s) if W is None else W
+    I = synth.make_inputs(s) if I is None else I
+    return O.dit_step(O.cfg_from_shape(s), W, I["latents"], I["temb"], I["cond"], **kw), W, I
+
+
+def test_zero_gates_make_blocks_identity_bit_exact():
+    s = _tiny()
+    W = synth.make_weights(s)
+    for l in range(s.n_blocks):
+        D = s.hidden
+        for lo in (2 * D, 5 * D):                                                     # gate1, gate2 chunks
+            W[f"blocks.{l}.mod.w"][lo:lo + D] = 0
+            W[f"blocks.{l}.mod.b"][lo:lo + D] = 0
+    taps = {}
+    out, _, _ = _run(s, W, taps=taps)
+    assert torch.equal(taps["b1.x_mlp"], taps["x0"])                                  # bit exact identity
+    s0 = _tiny(n_blocks=0)
+    W0 = {k: v for k, v in W.items() if not k.startswith("blocks.")}
+    out0, _, _ = _run(s0, W0)
+    assert torch.equal(out, out0)
+
+
+def test_step_split_p_invariance_and_modes():
+    for mode, rope, qkn in (("joint", (0, 0, 0), False), ("joint", (0, 8, 8), True), ("cross", (4, 6, 6), True),
+                            ("none", (0, 8, 8), False)):
+        s = _tiny(cond_mode=mode, rope_dims=rope, qk_rmsnorm=qkn)
+        out, W, I = _run(s)
+        assert out.shape == (2, 1, 8, 8) and torch.isfinite(out).all()
+        for P in (2, 4):
+            o2, _, _ = _run(s, W, I, split_p=P)
+            assert (o2 - out).norm() / out.norm() < 1e-13
+
+
+def test_joint_with_no_cond_tokens_equals_none_mode():
+    s = _tiny(cond_mode="joint", rope_dims=(0, 8, 8), qk_rmsnorm=True)
+    W, I = synth.make_weights(s), synth.make_inputs(s)
+    a = O.dit_step(O.cfg_from_shape(s), W, I["latents"], I["temb"], I["cond"][:0])
+    sn = _tiny(cond_mode="none", rope_dims=(0, 8, 8), qk_rmsnorm=True)
+    b = O.dit_step(O.cfg_from_shape(sn), W, I["latents"], I["temb"], None)
+    assert torch.allclose(a, b, rtol=1e-13, atol=1e-15)
+
+
+def test_permutation_equivariance_without_rope():
+    """patch 1x1x1, no RoPE, no cond: permuting latent pixels permutes the output identically."""
+    s = _tiny(cond_mode="none", patch=(1, 1, 1), latent_grid=(1, 4, 4))
+    out, W, I = _run(s)
+    perm = torch.randperm(16, generator=torch.Generator().manual_seed(1))
+    lat = I["latents"].reshape(2, 16)[:, perm].reshape(2, 1, 4, 4)
+    outp = O.dit_step(O.cfg_from_shape(s), W, lat, I["temb"], None)
+    assert torch.allclose(outp.reshape(2, 16), out.reshape(2, 16)[:, perm], rtol=1e-11, atol=1e-13)
+
+
+def test_patch_embed_selector_and_final_layer():
+    """With W_pe a selector and no blocks, x0 rows are raw patches (pins patch order + bias add)."""
+    s = _tiny(n_blocks=0, cond_mode="none", hidden=8, n_heads=1, head_dim=8, latent_channels=2)
+    W = synth.make_weights(s)
+    W["patch_embed.w"] = torch.eye(8); W["patch_embed.b"] = torch.zeros(8)
+    I = synth.make_inputs(s)
+    taps = {}
+    O.dit_step(O.cfg_from_shape(s), W, I["latents"], I["temb"], None, taps=taps)
+    assert torch.equal(taps["x0"], O.patchify(I["latents"].double(), (1, 2, 2)))
+    # final layer: tok = Wf (LN(x)(1 + scale_f) + shift_f) + bf, checked with torch's layer_norm
+    yf = torch.nn.functional.layer_norm(taps["x0"], (8,), eps=1e-6)
+    sc = O.silu(taps["c"])
+    modf = (W["final.mod.w"].double() @ sc + W["final.mod.b"].double()).reshape(2, 8)
+    tok = (yf * (1 + modf[1]) + modf[0]) @ W["final.w"].double().t() + W["final.b"].double()
+    assert torch.allclose(taps["tok"], tok, rtol=1e-11, atol=1e-13)
+
+
+def test_block_by_hand_one_block():
+    """One block re-derived with torch library routines (layer_norm, sdpa, gelu, silu) — an independent
+    transcription of SURVEY 8(c) step 5 that a dropped term / wrong chunk order in the oracle would fail."""
+    s = _tiny(n_blocks=1, cond_mode="none", rope_dims=(0, 0, 0), qk_rmsnorm=False)
+    W, I = synth.make_weights(s), synth.make_inputs(s)
+    taps = {}
+    O.dit_step(O.cfg_from_shape(s), W, I["latents"], I["temb"], None, taps=taps)
+    Fn = torch.nn.functional
+    Wd = {k: v.double() for k, v in W.items()}
+    D, H, d = 32, 2, 16
+    c = Fn.linear(Fn.silu(Fn.linear(I["temb"].double(), Wd["t_mlp.w1"], Wd["t_mlp.b1"])), Wd["t_mlp.w2"], Wd["t_mlp.b2"])
+    m = Fn.linear(Fn.silu(c), Wd["blocks.0.mod.w"], Wd["blocks.0.mod.b"]).reshape(6, D)
+    x = taps["x0"]
+    y = Fn.layer_norm(x, (D,), eps=1e-6) * (1 + m[1]) + m[0]
+    qkv = Fn.linear(y, Wd["blocks.0.attn.wqkv"], Wd["blocks.0.attn.bqkv"])
+    q, k, v = [t.reshape(-1, H, d).permute(1, 0, 2) for t in qkv.split(D, dim=1)]
+    o = Fn.scaled_dot_product_attention(q, k, v).permute(1, 0, 2).reshape(-1, D)
+    x = x + m[2] * Fn.linear(o, Wd["blocks.0.attn.wo"], Wd["blocks.0.attn.bo"])
+    y = Fn.layer_norm(x, (D,), eps=1e-6) * (1 + m[4]) + m[3]
+    x = x + m[5] * Fn.linear(Fn.gelu(Fn.linear(y, Wd["blocks.0.mlp.w1"], Wd["blocks.0.mlp.b1"]), approximate="tanh"),
+                             Wd["blocks.0.mlp.w2"], Wd["blocks.0.mlp.b2"])
+    assert torch.allclose(taps["b0.x_mlp"], x, rtol=1e-10, atol=1e-12)
+
+
+def test_varlen_is_per_request_and_block_rows():
+    s = _tiny(cond_mode="joint", rope_dims=(0, 8, 8), qk_rmsnorm=True)
+    W = synth.make_weights(s)
+    Is = [synth.make_inputs(s, tag=f"r{i}", t=100.0 * (i + 1)) for i in range(3)]
+    outs = O.dit_step_varlen(O.cfg_from_shape(s), W, [i["latents"] for i in Is], [i["temb"] for i in Is],
+                             [i["cond"] for i in Is])
+    for o, i in zip(outs, Is):
+        assert torch.equal(o, O.dit_step(O.cfg_from_shape(s), W, i["latents"], i["temb"], i["cond"]))
+    # teacher-forced block on sampled rows == the same rows of the full block
+    cfg = O.cfg_from_shape(s)
+    taps = {}
+    O.dit_step(cfg, W, Is[0]["latents"], Is[0]["temb"], Is[0]["cond"], taps=taps)
+    pos = torch.cat([torch.zeros(5, 3, dtype=torch.int64), O.token_positions((1, 4, 4))])
+    ang = O.rope_angles(pos, cfg["rope_dims"], cfg["rope_theta"])
+    rows = torch.tensor([0, 4, 5, 20])
+    got = O.block_rows(cfg, W, 1, taps["b0.x_mlp"], taps["mod"][1], ang, rows)
+    assert torch.allclose(got, taps["b1.x_mlp"][rows], rtol=1e-12, atol=1e-14)
+
+
+def test_cfg1_shape_facts():
+    s = synth.cfg1()
+    assert s.n_tokens == 256 and s.n_cond == 32 and s.token_grid == (1, 16, 16)
+    assert synth.cfg2().n_tokens == 4096 and synth.cfg3().n_tokens == 32760
+    assert [r.n_tokens for r in synth.cfg4_requests()] == list(synth.CFG4_TOKENS)
+    I = synth.make_inputs(s)
+    assert I["t"] == 500.0 and I["latents"].shape == (4, 1, 32, 32)
+    # generator is order independent and deterministic
+    a = synth.normal(3, "z", (1000,)); b = synth.normal(3, "z", (1000,), chunk=64)
+    assert torch.equal(a, b) and abs(float(a.mean())) < 0.15 and abs(float(a.std()) - 1) < 0.1
