@@ -1,0 +1,221 @@
+/* dit.h — C ABI of libdit_b200.so: one DiT denoising step on one B200 (sm_100a).
+ *
+ * What the library computes.  GF-DiT (arxiv/paper_2606_13501) schedules DiT requests as trajectory
+ * tasks, one task per denoising step; "denoising dominates execution time and resource consumption"
+ * (§1) and a step "performs bidirectional computation over the entire latent sequence"
+ * (§2.1).  The paper treats that step as an opaque executor call on "ordinary input and
+ * output tensors" (§5.2; §4.3) and parallelises it over the sequence with
+ * all-gather / all-to-all (§4.1).  This library IS that step on a single GPU: a stack of
+ * adaLN-Zero DiT blocks over a request's latent token sequence, plus the single-GPU analogue of the
+ * paper's SP degree (split-KV partial attention + log-sum-exp merge) and of its heterogeneous request
+ * mix (packed variable-length batching).  The mathematics is fixed in DESIGN.md §3 (readings R1-R23).
+ *
+ * Conventions (all entry points)
+ *  - "dev" pointers are device (HBM) pointers owned by the CALLER (PyTorch allocates); "host" pointers
+ *    are ordinary host memory.  The library never frees caller memory and never allocates device
+ *    memory after dit_init (its only allocation is the handle's small host struct); `workspace` is
+ *    caller-allocated with the size dit_workspace_bytes() returns and must outlive the handle, as must
+ *    every weight pointer.
+ *  - All work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = legacy default stream).
+ *    No entry point synchronises the device, except dit_init (one-time pointer-table upload) and the
+ *    *_host convenience call, which returns after enqueuing (its D2H copy is stream ordered; the caller
+ *    synchronises the stream before reading `out_host`).
+ *  - Errors: a negative dit_status is returned before anything is launched when arguments are invalid;
+ *    DIT_ERR_CUDA reports a failed launch/API call.  dit_last_error() gives a message.  Nothing throws.
+ *  - There is no CPU fallback and no alternative backend: if no sm_100 device is present every compute
+ *    entry point returns DIT_ERR_CUDA.
+ *  - dtype: DIT_F32 (all tensors fp32; SIMT FFMA kernels, no TF32) or DIT_BF16 (weights/activations
+ *    bf16, residual stream / statistics / modulation / LSE fp32; tcgen05 tensor-core kernels).
+ *  - Linear weights are [out, in] row-major, biases [out], all in the config dtype.
+ */
+#ifndef DIT_B200_H
+#define DIT_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dit_handle_s* dit_handle; /* opaque; created by dit_init, destroyed by dit_free */
+
+typedef enum {
+  DIT_OK = 0,
+  DIT_ERR_INVALID_ARG = -1,
+  DIT_ERR_UNSUPPORTED = -2,
+  DIT_ERR_WORKSPACE = -3,
+  DIT_ERR_CUDA = -4
+} dit_status;
+
+typedef enum { DIT_F32 = 0, DIT_BF16 = 1 } dit_dtype;
+typedef enum { DIT_COND_NONE = 0, DIT_COND_JOINT = 1, DIT_COND_CROSS = 2 } dit_cond_mode;
+
+/* POD configuration (all ints 32-bit).  struct_size = sizeof(dit_config) guards ABI drift. */
+typedef struct {
+  int32_t struct_size;
+  int32_t dtype;           /* dit_dtype */
+  int32_t n_blocks;        /* L >= 0 */
+  int32_t hidden;          /* D, multiple of 128, == n_heads * head_dim */
+  int32_t n_heads;         /* H */
+  int32_t head_dim;        /* d in {64, 128} */
+  int32_t mlp_dim;         /* F, multiple of 8 */
+  int32_t latent_channels; /* C */
+  int32_t patch[3];        /* {pf, ph, pw}; images: pf = 1 and latent F = 1 */
+  int32_t temb_dim;        /* width of the timestep embedding passed to dit_step */
+  int32_t cond_dim;        /* width of a conditioning token (ignored for DIT_COND_NONE) */
+  int32_t cond_mode;       /* dit_cond_mode: joint = [cond ; image] one sequence, single stream (R9);
+                              cross = extra cross-attention sub-layer per block (R10) */
+  int32_t rope_dims[3];    /* head-dim segment per axis (f, h, w), each even, sum == head_dim, or all 0
+                              for no RoPE (R6) */
+  float rope_theta;        /* 10000 */
+  float ln_eps;            /* 1e-6 (R4) */
+  float rms_eps;           /* 1e-6 (R5) */
+  int32_t qk_rmsnorm;      /* 0/1: per-head RMSNorm of q and k with gains attn.gq / attn.gk (R5) */
+  int32_t split_p;         /* split degree P used for self-attention inside a step: 1, 2, 4 or 8.
+                              P > 1 computes P split-KV partials + LSE merge (the SP analogue) */
+  int32_t max_tokens;      /* capacity: max total packed sequence rows (cond rows included in joint) */
+  int32_t max_requests;    /* capacity: max requests per dit_step_varlen call (<= 64) */
+  int32_t max_cond_tokens; /* capacity: max total conditioning tokens per call */
+} dit_config;
+
+/* One named weight tensor (device pointer, caller-owned, config dtype).  Names:
+ *   t_mlp.w1 [D,temb] t_mlp.b1 [D] t_mlp.w2 [D,D] t_mlp.b2 [D]
+ *   patch_embed.w [D, C*pf*ph*pw] patch_embed.b [D]      cond_proj.w [D,cond_dim] cond_proj.b [D]
+ *   blocks.{l}.mod.w [6D,D] .mod.b [6D]   (chunks: shift1, scale1, gate1, shift2, scale2, gate2)
+ *   blocks.{l}.attn.wqkv [3D,D] .attn.bqkv [3D] (rows: q | k | v; head h = rows h*d..)  .attn.gq [d] .attn.gk [d]
+ *   blocks.{l}.attn.wo [D,D] .attn.bo [D]   blocks.{l}.mlp.w1 [F,D] .mlp.b1 [F] .mlp.w2 [D,F] .mlp.b2 [D]
+ *   blocks.{l}.cross.wq [D,D] .bq [D] .wkv [2D,D] .bkv [2D] .gq [d] .gk [d] .wo [D,D] .bo [D]   (cross mode)
+ *   final.mod.w [2D,D] final.mod.b [2D] (shift_f, scale_f)   final.w [C*pv, D] final.b [C*pv] */
+typedef struct {
+  const char* name;
+  const void* dev_ptr;
+  int64_t numel;
+} dit_weight;
+
+/* Bytes of device workspace dit_init needs for this config (0 on an invalid config). */
+size_t dit_workspace_bytes(const dit_config* cfg);
+
+/* Validates cfg and the weight table (every required name present with the right numel; unknown names
+ * are an error), carves `workspace` (dev, 256-byte aligned), uploads pointer tables.  *out receives the
+ * handle.  Returns DIT_ERR_WORKSPACE if workspace_bytes is too small. */
+dit_status dit_init(const dit_config* cfg, const dit_weight* weights, int32_t n_weights, void* workspace,
+                    size_t workspace_bytes, dit_handle* out);
+
+/* One denoising step for one request (DESIGN.md §3 steps 1-6).
+ *   latents      dev, [C, F, H, W] in config dtype, contiguous; latent_grid = {F, H, W} (host, 3 ints)
+ *   timestep_emb dev, [temb_dim] fp32  (sinusoidal embedding of t — an input, R16)
+ *   cond_tokens  dev, [n_cond, cond_dim] config dtype (NULL / 0 allowed; ignored for DIT_COND_NONE)
+ *   out          dev, [C, F, H, W] config dtype
+ * Sequence rows used = F/pf*H/ph*W/pw (+ n_cond in joint mode) must be <= max_tokens. */
+dit_status dit_step(dit_handle h, const void* latents, const float* timestep_emb, const void* cond_tokens,
+                    int32_t n_cond, const int32_t latent_grid[3], void* out, void* stream);
+
+/* Same computation with HOST buffers (pageable or pinned): H2D copies of latents / timestep_emb / cond,
+ * the step, and the D2H copy of `out` are all enqueued on `stream`; staging lives in the workspace.
+ * This is the end-to-end call bench.py times ("e2e"). */
+dit_status dit_step_host(dit_handle h, const void* latents_host, const float* timestep_emb_host,
+                         const void* cond_tokens_host, int32_t n_cond, const int32_t latent_grid[3],
+                         void* out_host, void* stream);
+
+/* Packed variable-length batch of R heterogeneous requests (BASELINE.json north_star subsystem 6; the
+ * single-GPU analogue of the paper's heterogeneous request mix).  The result for request r
+ * is DEFINED as dit_step on request r alone (DESIGN.md §3 step 8).
+ *   latents_packed   dev: the R latents [C, F_r, H_r, W_r] back to back
+ *   timestep_emb     dev: [R, temb_dim] fp32 (per-request timesteps)
+ *   cond_packed      dev: [sum n_cond_r, cond_dim]
+ *   cu_seqlens       host [R+1]: prefix sums of the per-request sequence length
+ *                    T_r = N_r (+ n_cond_r in joint mode); validated against latent_grids / n_cond
+ *   n_cond           host [R];   latent_grids host [R][3] = {F_r, H_r, W_r}
+ *   out_packed       dev: R outputs back to back, each with its latent's shape
+ * GEMMs / norms run over the flat [sum T_r, D] sequence; modulation is indexed per request; attention is
+ * block diagonal over requests. */
+dit_status dit_step_varlen(dit_handle h, const void* latents_packed, const float* timestep_emb,
+                           const void* cond_packed, const int32_t* cu_seqlens, const int32_t* n_cond,
+                           const int32_t* latent_grids, int32_t n_requests, void* out_packed, void* stream);
+
+/* Split-KV partial attention (north_star subsystem 5; one rank's share of a P-way sequence-parallel
+ * step).  Non-causal:  for every query row i and head h over THIS call's n_k keys
+ *   s_ij = softmax_scale * q_i . k_j ;  o_i = sum_j softmax_j(s_ij) v_j (locally normalised) ;
+ *   lse_i = ln sum_j exp(s_ij)   (natural log; n_k == 0 gives o = 0, lse = -inf, R18)
+ *   q  dev [n_q, H, d] with row stride q_row_stride elements (head stride = d);  k, v dev [n_k, H, d]
+ *      with row stride kv_row_stride;  dtype = dit_dtype of q, k, v and o
+ *   o  dev [n_q, H, d] contiguous;  lse dev [n_q, H] fp32 (may be NULL)
+ * With n_k = all keys this is the full-sequence flash attention of subsystem 4. */
+dit_status dit_attn_partial(int32_t dtype, const void* q, const void* k, const void* v, int32_t n_q, int32_t n_k,
+                            int32_t n_heads, int32_t head_dim, int64_t q_row_stride, int64_t kv_row_stride,
+                            float softmax_scale, void* o, float* lse, void* stream);
+
+/* LSE merge of P partials (R18):  lse = ln sum_p e^{lse_p};  o = sum_p e^{lse_p - lse} o_p.
+ *   o_partials host array of P dev pointers [n_q, H, d] (dtype);  lses host array of P dev pointers
+ *   [n_q, H] fp32;  o dev [n_q, H, d] dtype;  lse_out dev [n_q, H] fp32 or NULL.  1 <= P <= 8.
+ * Partials with lse = -inf contribute nothing; if all are -inf the row is o = 0, lse = -inf. */
+dit_status dit_attn_merge(int32_t dtype, const void* const* o_partials, const float* const* lses, int32_t P,
+                          int32_t n_q, int32_t n_heads, int32_t head_dim, void* o, float* lse_out, void* stream);
+
+/* ---- kernel-level entry points (the building blocks of dit_step; used by the parity tests and by
+ *      bench.py's per-kernel roofline lines) ------------------------------------------------------ */
+
+typedef enum {
+  DIT_EPI_BIAS = 0,      /* out = A W^T + b                      (out in dtype) */
+  DIT_EPI_BIAS_GELU = 1, /* out = GELU_tanh(A W^T + b)           (north_star subsystem 3) */
+  DIT_EPI_BIAS_F32 = 2   /* out = A W^T + b, stored fp32         (residual-stream producers) */
+} dit_epilogue;
+
+/* out[M, N] = epilogue(A[M, K] W[N, K]^T + bias[N]).  A row stride lda, out row stride ldo (elements);
+ * W contiguous [N, K]; bias may be NULL.  bf16: tcgen05/TMEM/TMA GEMM (K % 8 == 0, lda % 8 == 0, 16-byte
+ * aligned pointers), fp32: FFMA GEMM. */
+dit_status dit_linear(int32_t dtype, int32_t epilogue, const void* A, int64_t lda, const void* W, const void* bias,
+                      void* out, int64_t ldo, int32_t M, int32_t N, int32_t K, void* stream);
+
+/* adaLN-Zero modulation kernel (north_star subsystem 2), one pass over the row:
+ *   if h != NULL:  x <- x + gate (.) h          (gate NULL = 1)       [x fp32 in/out, h dtype]
+ *   y = LN(x) (.) (1 + scale) + shift           (shift/scale NULL = 0) [y dtype]
+ * x dev [T, D] fp32; gate/shift/scale dev fp32 [R, mod_stride] rows indexed by the request of the token
+ * (cu_seqlens_dev [R+1] int32 maps row -> request; NULL means one request). */
+dit_status dit_adaln(int32_t dtype, float* x, const void* h, const float* gate, const float* shift,
+                     const float* scale, int64_t mod_stride, const int32_t* cu_seqlens_dev, int32_t n_requests,
+                     void* y, int32_t T, int32_t D, float eps, void* stream);
+
+/* out[r, n] = sum_k act(in[r, k]) W[n, k] + b[n];  in/out fp32, W/b dtype; act = SiLU if silu_input else id.
+ * The t-MLP and the adaLN modulation projection (DESIGN.md §3 steps 1-2): a weight-streaming GEMV. */
+dit_status dit_gemv(int32_t dtype, const float* in, const void* W, const void* b, float* out, int32_t R, int32_t N,
+                    int32_t K, int32_t silu_input, void* stream);
+
+/* In-place QK-RMSNorm (+ RoPE) of the q and k thirds of a packed qkv buffer [T, 3D] (R5, R6):
+ * per token per head  v <- v / sqrt(mean(v^2) + eps) * g, then pairs (2j, 2j+1) rotated by the angle whose
+ * cos/sin are rope_cos/rope_sin[T, d/2] (fp32; NULL = no RoPE).  gq/gk [d] dtype (NULL = no norm). */
+dit_status dit_qknorm_rope(int32_t dtype, void* qkv, int64_t row_stride, int32_t T, int32_t n_heads, int32_t head_dim,
+                           int32_t n_tensors /* 2: q and k; 1: q only */, const void* gq, const void* gk, float eps,
+                           const float* rope_cos, const float* rope_sin, void* stream);
+
+/* ---- debugging ---------------------------------------------------------------------------------- */
+typedef enum {
+  DIT_TAP_X = 0,   /* residual stream x   [T, D]  fp32 */
+  DIT_TAP_Y = 1,   /* last adaLN output   [T, D]  dtype */
+  DIT_TAP_QKV = 2, /* q|k|v after norm+rope [T, 3D] dtype */
+  DIT_TAP_O = 3,   /* attention output    [T, D]  dtype */
+  DIT_TAP_H = 4,   /* last out-proj / fc2 result [T, D] dtype */
+  DIT_TAP_U = 5,   /* GELU output         [T, F]  dtype */
+  DIT_TAP_C = 6,   /* c                   [R, D]  fp32 */
+  DIT_TAP_MOD = 7, /* modulation          [R, L*6*D + 2*D] fp32 */
+  DIT_TAP_TOK = 8  /* final-layer tokens  [N, C*pv] fp32 */
+} dit_tap;
+typedef enum {
+  DIT_STAGE_Y1 = 0, DIT_STAGE_QKV = 1, DIT_STAGE_ATTN = 2, DIT_STAGE_OPROJ = 3, DIT_STAGE_CROSS = 4,
+  DIT_STAGE_Y2 = 5, DIT_STAGE_FC1 = 6, DIT_STAGE_FC2 = 7
+} dit_stage;
+/* Make the next steps return right after (block, stage) so workspace buffers can be inspected;
+ * block < 0 restores normal operation. */
+dit_status dit_debug_stop_after(dit_handle h, int32_t block, int32_t stage);
+/* Copy `bytes` of a workspace buffer to dst (dev), stream ordered. */
+dit_status dit_get_tap(dit_handle h, int32_t tap, void* dst, size_t bytes, void* stream);
+
+const char* dit_last_error(dit_handle h); /* h may be NULL: last error of a handle-less entry point */
+int32_t dit_kernel_launches(void);         /* kernels launched by this library so far (this process) */
+void dit_free(dit_handle h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DIT_B200_H */

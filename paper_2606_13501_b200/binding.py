@@ -1,0 +1,281 @@
+"""Thin ctypes binding over libdit_b200.so (include/dit.h).  Argument marshalling only: every step of the
+path runs in the library's CUDA kernels; torch is used for device memory and streams.  Same names as the C
+ABI.  `load()` raises if the library is missing — there is no fallback of any kind."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libdit_b200.so")
+
+DIT_OK = 0
+DIT_F32, DIT_BF16 = 0, 1
+COND = {"none": 0, "joint": 1, "cross": 2}
+EPI_BIAS, EPI_BIAS_GELU, EPI_BIAS_F32 = 0, 1, 2
+TAP = dict(x=0, y=1, qkv=2, o=3, h=4, u=5, c=6, mod=7, tok=8)
+STAGE = dict(y1=0, qkv=1, attn=2, oproj=3, cross=4, y2=5, fc1=6, fc2=7)
+
+SYMBOLS = ["dit_workspace_bytes", "dit_init", "dit_step", "dit_step_host", "dit_step_varlen", "dit_attn_partial",
+           "dit_attn_merge", "dit_linear", "dit_adaln", "dit_gemv", "dit_qknorm_rope", "dit_debug_stop_after",
+           "dit_get_tap", "dit_last_error", "dit_kernel_launches", "dit_free"]
+
+
+class dit_config(C.Structure):
+    _fields_ = [("struct_size", C.c_int32), ("dtype", C.c_int32), ("n_blocks", C.c_int32), ("hidden", C.c_int32),
+                ("n_heads", C.c_int32), ("head_dim", C.c_int32), ("mlp_dim", C.c_int32), ("latent_channels", C.c_int32),
+                ("patch", C.c_int32 * 3), ("temb_dim", C.c_int32), ("cond_dim", C.c_int32), ("cond_mode", C.c_int32),
+                ("rope_dims", C.c_int32 * 3), ("rope_theta", C.c_float), ("ln_eps", C.c_float), ("rms_eps", C.c_float),
+                ("qk_rmsnorm", C.c_int32), ("split_p", C.c_int32), ("max_tokens", C.c_int32),
+                ("max_requests", C.c_int32), ("max_cond_tokens", C.c_int32)]
+
+
+class dit_weight(C.Structure):
+    _fields_ = [("name", C.c_char_p), ("dev_ptr", C.c_void_p), ("numel", C.c_int64)]
+
+
+class DitError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def load(path: str = LIB_PATH):
+    """dlopen the C-ABI library.  Raises (never falls back) when it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(path):
+        raise DitError(f"{path} not found: build it with `python -m paper_2606_13501_b200.build` "
+                       "(there is no CPU / PyTorch fallback)")
+    lib = C.CDLL(path)
+    lib.dit_workspace_bytes.restype = C.c_size_t
+    lib.dit_workspace_bytes.argtypes = [C.POINTER(dit_config)]
+    lib.dit_last_error.restype = C.c_char_p
+    lib.dit_last_error.argtypes = [C.c_void_p]
+    lib.dit_kernel_launches.restype = C.c_int32
+    lib.dit_free.restype = None
+    lib.dit_free.argtypes = [C.c_void_p]
+    vp, i32, i64, f32 = C.c_void_p, C.c_int32, C.c_int64, C.c_float
+    pi32 = C.POINTER(C.c_int32)
+    sig = {
+        "dit_init": [C.POINTER(dit_config), C.POINTER(dit_weight), i32, vp, C.c_size_t, C.POINTER(vp)],
+        "dit_step": [vp, vp, vp, vp, i32, pi32, vp, vp],
+        "dit_step_host": [vp, vp, vp, vp, i32, pi32, vp, vp],
+        "dit_step_varlen": [vp, vp, vp, vp, pi32, pi32, pi32, i32, vp, vp],
+        "dit_attn_partial": [i32, vp, vp, vp, i32, i32, i32, i32, i64, i64, f32, vp, vp, vp],
+        "dit_attn_merge": [i32, C.POINTER(vp), C.POINTER(vp), i32, i32, i32, i32, vp, vp, vp],
+        "dit_linear": [i32, i32, vp, i64, vp, vp, vp, i64, i32, i32, i32, vp],
+        "dit_adaln": [i32, vp, vp, vp, vp, vp, i64, vp, i32, vp, i32, i32, f32, vp],
+        "dit_gemv": [i32, vp, vp, vp, vp, i32, i32, i32, i32, vp],
+        "dit_qknorm_rope": [i32, vp, i64, i32, i32, i32, i32, vp, vp, f32, vp, vp, vp],
+        "dit_debug_stop_after": [vp, i32, i32],
+        "dit_get_tap": [vp, i32, vp, C.c_size_t, vp],
+    }
+    for name, argtypes in sig.items():
+        fn = getattr(lib, name)
+        fn.restype = C.c_int32
+        fn.argtypes = argtypes
+    _lib = lib
+    return lib
+
+
+def _check(status: int, what: str):
+    if status != DIT_OK:
+        msg = load().dit_last_error(None)
+        raise DitError(f"{what} failed with status {status}: {msg.decode() if msg else ''}")
+
+
+def _ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _stream(stream=None):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def _dt(t: torch.Tensor) -> int:
+    if t.dtype == torch.float32:
+        return DIT_F32
+    if t.dtype == torch.bfloat16:
+        return DIT_BF16
+    raise DitError(f"unsupported dtype {t.dtype}")
+
+
+def _i32arr(vals):
+    vals = [int(v) for v in vals]
+    return (C.c_int32 * len(vals))(*vals)
+
+
+def make_config(shape, split_p=1, max_tokens=None, max_requests=1, max_cond_tokens=None) -> dit_config:
+    """dit_config from a synth.DiTShape-like object (duck typed)."""
+    c = dit_config()
+    c.struct_size = C.sizeof(dit_config)
+    c.dtype = DIT_F32 if shape.dtype == "f32" else DIT_BF16
+    c.n_blocks, c.hidden, c.n_heads, c.head_dim, c.mlp_dim = shape.n_blocks, shape.hidden, shape.n_heads, shape.head_dim, shape.mlp_dim
+    c.latent_channels = shape.latent_channels
+    c.patch = (C.c_int32 * 3)(*shape.patch)
+    c.temb_dim, c.cond_dim, c.cond_mode = shape.temb_dim, shape.cond_dim, COND[shape.cond_mode]
+    c.rope_dims = (C.c_int32 * 3)(*shape.rope_dims)
+    c.rope_theta, c.ln_eps, c.rms_eps = shape.rope_theta, shape.ln_eps, shape.rms_eps
+    c.qk_rmsnorm, c.split_p = int(shape.qk_rmsnorm), split_p
+    n = shape.n_tokens + (shape.n_cond if shape.cond_mode == "joint" else 0)
+    c.max_tokens = int(max_tokens if max_tokens is not None else n)
+    c.max_requests = max_requests
+    c.max_cond_tokens = int(max_cond_tokens if max_cond_tokens is not None else (shape.n_cond if shape.cond_mode != "none" else 0))
+    return c
+
+
+class Dit:
+    """Owns a dit_handle plus the torch allocations (workspace, weights) that must outlive it."""
+
+    def __init__(self, cfg: dit_config, weights: dict, device="cuda:0"):
+        self.lib = load()
+        self.cfg = cfg
+        self.device = torch.device(device)
+        self.tdtype = torch.float32 if cfg.dtype == DIT_F32 else torch.bfloat16
+        nbytes = self.lib.dit_workspace_bytes(C.byref(cfg))
+        if nbytes == 0:
+            _check(-1, "dit_workspace_bytes")
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        self.weights = {k: v.to(self.device, self.tdtype).contiguous() for k, v in weights.items()}
+        arr = (dit_weight * len(self.weights))()
+        for i, (k, v) in enumerate(self.weights.items()):
+            arr[i].name, arr[i].dev_ptr, arr[i].numel = k.encode(), v.data_ptr(), v.numel()
+        h = C.c_void_p()
+        _check(self.lib.dit_init(C.byref(cfg), arr, len(self.weights), _ptr(self.workspace), nbytes, C.byref(h)), "dit_init")
+        self.handle = h
+
+    def __del__(self):
+        if getattr(self, "handle", None):
+            self.lib.dit_free(self.handle)
+            self.handle = None
+
+    def dit_step(self, latents, temb, cond=None, out=None, stream=None):
+        """latents [C,F,H,W] (device, config dtype), temb [temb_dim] fp32, cond [n_cond, cond_dim]."""
+        out = torch.empty_like(latents) if out is None else out
+        grid = _i32arr(latents.shape[1:])
+        n_cond = 0 if cond is None else cond.shape[0]
+        _check(self.lib.dit_step(self.handle, _ptr(latents), _ptr(temb), _ptr(cond), n_cond, grid, _ptr(out),
+                                 _stream(stream)), "dit_step")
+        return out
+
+    def dit_step_host(self, latents_host, temb_host, cond_host=None, out_host=None, stream=None):
+        out_host = torch.empty_like(latents_host) if out_host is None else out_host
+        grid = _i32arr(latents_host.shape[1:])
+        n_cond = 0 if cond_host is None else cond_host.shape[0]
+        _check(self.lib.dit_step_host(self.handle, _ptr(latents_host), _ptr(temb_host), _ptr(cond_host), n_cond, grid,
+                                      _ptr(out_host), _stream(stream)), "dit_step_host")
+        return out_host
+
+    def dit_step_varlen(self, latents_list, temb, cond_list=None, stream=None):
+        """latents_list: R tensors [C,F_r,H_r,W_r]; temb [R, temb_dim]; cond_list: R tensors or None.
+        Packs (torch.cat: memory plumbing only), calls the C ABI once, returns the R outputs (views)."""
+        R = len(latents_list)
+        packed = torch.cat([l.reshape(-1) for l in latents_list])
+        joint = self.cfg.cond_mode == COND["joint"]
+        n_cond = [0 if (cond_list is None or cond_list[r] is None) else cond_list[r].shape[0] for r in range(R)]
+        cond = torch.cat([c for c in cond_list if c is not None]) if cond_list is not None and sum(n_cond) else None
+        p = self.cfg.patch
+        cu = [0]
+        grids = []
+        for r, l in enumerate(latents_list):
+            f, h, w = l.shape[1:]
+            grids += [f, h, w]
+            cu.append(cu[-1] + (f // p[0]) * (h // p[1]) * (w // p[2]) + (n_cond[r] if joint else 0))
+        out = torch.empty_like(packed)
+        _check(self.lib.dit_step_varlen(self.handle, _ptr(packed), _ptr(temb), _ptr(cond), _i32arr(cu), _i32arr(n_cond),
+                                        _i32arr(grids), R, _ptr(out), _stream(stream)), "dit_step_varlen")
+        outs, off = [], 0
+        for l in latents_list:
+            outs.append(out[off:off + l.numel()].reshape(l.shape))
+            off += l.numel()
+        return outs
+
+    def dit_debug_stop_after(self, block, stage):
+        _check(self.lib.dit_debug_stop_after(self.handle, block, STAGE[stage] if isinstance(stage, str) else stage),
+               "dit_debug_stop_after")
+
+    def dit_get_tap(self, tap, shape, dtype, stream=None):
+        dst = torch.empty(shape, dtype=dtype, device=self.device)
+        _check(self.lib.dit_get_tap(self.handle, TAP[tap], _ptr(dst), dst.numel() * dst.element_size(), _stream(stream)),
+               "dit_get_tap")
+        return dst
+
+
+# ---- handle-less entry points -------------------------------------------------------------------
+def dit_attn_partial(q, k, v, softmax_scale=None, want_lse=True, stream=None):
+    """q [Nq,H,d], k/v [Nk,H,d] (last two dims contiguous; row stride free) -> o [Nq,H,d], lse [Nq,H] fp32."""
+    lib = load()
+    nq, H, d = q.shape
+    nk = k.shape[0]
+    assert q.stride(2) == 1 and q.stride(1) == d and k.stride(2) == 1 and k.stride(1) == d and v.stride(1) == d
+    assert nk == 0 or k.stride(0) == v.stride(0)
+    o = torch.empty((nq, H, d), dtype=q.dtype, device=q.device)
+    lse = torch.empty((nq, H), dtype=torch.float32, device=q.device) if want_lse else None
+    scale = d ** -0.5 if softmax_scale is None else softmax_scale
+    _check(lib.dit_attn_partial(_dt(q), _ptr(q), _ptr(k), _ptr(v), nq, nk, H, d, q.stride(0) if nq else H * d,
+                                k.stride(0) if nk else H * d, scale, _ptr(o), _ptr(lse), _stream(stream)),
+           "dit_attn_partial")
+    return o, lse
+
+
+def dit_attn_merge(o_parts, lse_parts, want_lse=True, stream=None):
+    lib = load()
+    P = len(o_parts)
+    nq, H, d = o_parts[0].shape
+    o = torch.empty_like(o_parts[0])
+    lse = torch.empty((nq, H), dtype=torch.float32, device=o.device) if want_lse else None
+    op = (C.c_void_p * P)(*[t.data_ptr() for t in o_parts])
+    lp = (C.c_void_p * P)(*[t.data_ptr() for t in lse_parts])
+    _check(lib.dit_attn_merge(_dt(o), op, lp, P, nq, H, d, _ptr(o), _ptr(lse), _stream(stream)), "dit_attn_merge")
+    return o, lse
+
+
+def dit_linear(A, W, bias=None, epilogue=EPI_BIAS, out=None, stream=None):
+    lib = load()
+    M, K = A.shape
+    N = W.shape[0]
+    if out is None:
+        out = torch.empty((M, N), dtype=torch.float32 if epilogue == EPI_BIAS_F32 else A.dtype, device=A.device)
+    _check(lib.dit_linear(_dt(A), epilogue, _ptr(A), A.stride(0), _ptr(W), _ptr(bias), _ptr(out), out.stride(0), M, N, K,
+                          _stream(stream)), "dit_linear")
+    return out
+
+
+def dit_adaln(x, y_dtype, h=None, gate=None, shift=None, scale=None, mod_stride=0, cu_seqlens=None, n_requests=1,
+              eps=1e-6, stream=None):
+    """x [T,D] fp32 (updated in place when h is given) -> y [T,D] in y_dtype."""
+    lib = load()
+    T, D = x.shape
+    y = torch.empty((T, D), dtype=y_dtype, device=x.device)
+    _check(lib.dit_adaln(_dt(y), _ptr(x), _ptr(h), _ptr(gate), _ptr(shift), _ptr(scale), mod_stride, _ptr(cu_seqlens),
+                         n_requests, _ptr(y), T, D, eps, _stream(stream)), "dit_adaln")
+    return y
+
+
+def dit_gemv(inp, W, b=None, silu_input=False, stream=None):
+    lib = load()
+    R, K = inp.shape
+    N = W.shape[0]
+    out = torch.empty((R, N), dtype=torch.float32, device=inp.device)
+    _check(lib.dit_gemv(_dt(W), _ptr(inp), _ptr(W), _ptr(b), _ptr(out), R, N, K, int(silu_input), _stream(stream)),
+           "dit_gemv")
+    return out
+
+
+def dit_qknorm_rope(qkv, n_heads, head_dim, n_tensors=2, gq=None, gk=None, eps=1e-6, rope_cos=None, rope_sin=None,
+                    stream=None):
+    lib = load()
+    T = qkv.shape[0]
+    _check(lib.dit_qknorm_rope(_dt(qkv), _ptr(qkv), qkv.stride(0), T, n_heads, head_dim, n_tensors, _ptr(gq), _ptr(gk),
+                               eps, _ptr(rope_cos), _ptr(rope_sin), _stream(stream)), "dit_qknorm_rope")
+    return qkv
+
+
+def dit_kernel_launches() -> int:
+    return int(load().dit_kernel_launches())

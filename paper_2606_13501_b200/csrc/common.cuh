@@ -1,0 +1,173 @@
+// common.cuh — shared device/host helpers of libdit_b200 (CUDA path only; the oracle shares nothing with it).
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/dit.h"
+
+namespace dit {
+
+typedef __nv_bfloat16 bf16;
+
+// launch accounting (dit_kernel_launches)
+extern int g_launches;
+void set_error(const char* fmt, ...);
+const char* get_error();
+
+#define DIT_CUDA_OK(expr)                                                                       \
+  do {                                                                                          \
+    cudaError_t _e = (expr);                                                                    \
+    if (_e != cudaSuccess) {                                                                    \
+      dit::set_error("%s failed: %s (%s:%d)", #expr, cudaGetErrorString(_e), __FILE__, __LINE__); \
+      return DIT_ERR_CUDA;                                                                      \
+    }                                                                                           \
+  } while (0)
+
+#define DIT_LAUNCH_CHECK()                                                                  \
+  do {                                                                                      \
+    dit::g_launches++;                                                                      \
+    cudaError_t _e = cudaPeekAtLastError();                                                 \
+    if (_e != cudaSuccess) {                                                                \
+      (void)cudaGetLastError();                                                             \
+      dit::set_error("kernel launch failed: %s (%s:%d)", cudaGetErrorString(_e), __FILE__, __LINE__); \
+      return DIT_ERR_CUDA;                                                                  \
+    }                                                                                       \
+  } while (0)
+
+#define DIT_REQUIRE(cond, status, ...) \
+  do {                                 \
+    if (!(cond)) {                     \
+      dit::set_error(__VA_ARGS__);     \
+      return status;                   \
+    }                                  \
+  } while (0)
+
+static inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
+
+// ---------------------------------------------------------------------------------------------
+// 128-bit vector access: 8 consecutive elements of T <-> 8 floats
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ float bf16lo(uint32_t u) { return __uint_as_float(u << 16); }
+__device__ __forceinline__ float bf16hi(uint32_t u) { return __uint_as_float(u & 0xffff0000u); }
+__device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
+  __nv_bfloat162 t = __floats2bfloat162_rn(a, b);
+  return *reinterpret_cast<uint32_t*>(&t);
+}
+
+template <typename T>
+__device__ __forceinline__ void ld8(const T* p, float v[8]);
+template <>
+__device__ __forceinline__ void ld8<float>(const float* p, float v[8]) {
+  float4 a = *reinterpret_cast<const float4*>(p), b = *reinterpret_cast<const float4*>(p + 4);
+  v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
+}
+template <>
+__device__ __forceinline__ void ld8<bf16>(const bf16* p, float v[8]) {
+  uint4 a = *reinterpret_cast<const uint4*>(p);
+  v[0] = bf16lo(a.x); v[1] = bf16hi(a.x); v[2] = bf16lo(a.y); v[3] = bf16hi(a.y);
+  v[4] = bf16lo(a.z); v[5] = bf16hi(a.z); v[6] = bf16lo(a.w); v[7] = bf16hi(a.w);
+}
+template <typename T>
+__device__ __forceinline__ void st8(T* p, const float v[8]);
+template <>
+__device__ __forceinline__ void st8<float>(float* p, const float v[8]) {
+  *reinterpret_cast<float4*>(p) = make_float4(v[0], v[1], v[2], v[3]);
+  *reinterpret_cast<float4*>(p + 4) = make_float4(v[4], v[5], v[6], v[7]);
+}
+template <>
+__device__ __forceinline__ void st8<bf16>(bf16* p, const float v[8]) {
+  uint4 a;
+  a.x = pack_bf16(v[0], v[1]); a.y = pack_bf16(v[2], v[3]); a.z = pack_bf16(v[4], v[5]); a.w = pack_bf16(v[6], v[7]);
+  *reinterpret_cast<uint4*>(p) = a;
+}
+
+template <typename T> __device__ __forceinline__ float to_f(T v);
+template <> __device__ __forceinline__ float to_f<float>(float v) { return v; }
+template <> __device__ __forceinline__ float to_f<bf16>(bf16 v) { return __bfloat162float(v); }
+template <typename T> __device__ __forceinline__ T from_f(float v);
+template <> __device__ __forceinline__ float from_f<float>(float v) { return v; }
+template <> __device__ __forceinline__ bf16 from_f<bf16>(float v) { return __float2bfloat16_rn(v); }
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// row -> request through cu_seqlens (R <= 64: linear scan, warp-uniform)
+__device__ __forceinline__ int find_request(const int32_t* __restrict__ cu, int R, int row) {
+  int r = 0;
+  while (r + 1 < R && row >= cu[r + 1]) ++r;
+  return r;
+}
+
+__device__ __forceinline__ float gelu_tanh_f(float z) {
+  // 0.5 z (1 + tanh(0.79788456 (z + 0.044715 z^3)))   (DESIGN.md §3 step 5); accurate tanhf, not the approx one
+  float t = tanhf(0.7978845608028654f * (z + 0.044715f * z * z * z));
+  return 0.5f * z * (1.0f + t);
+}
+__device__ __forceinline__ float silu_f(float z) { return z / (1.0f + expf(-z)); }
+
+// ---------------------------------------------------------------------------------------------
+// internal launchers (implemented across the .cu files); every one enqueues on `st`
+// ---------------------------------------------------------------------------------------------
+struct SeqMeta {        // one per request, device resident
+  int32_t seq_start;    // first row of the request in the packed sequence
+  int32_t n_cond;       // joint-mode cond rows at the head of the segment (0 otherwise)
+  int32_t gf, gh, gw;   // token grid (F', H', W')
+  int32_t lat_off_lo, lat_off_hi;  // element offset of the request's latent in the packed latents (64-bit split)
+  int32_t pad;
+};
+
+struct GemvBatch {      // one per weight matrix of a batched GEMV
+  const void* W;
+  const void* b;
+  int32_t N;
+  int32_t out_off;      // column offset inside an output row
+  int32_t row_begin;    // first flattened row index of this matrix
+  int32_t pad;
+};
+
+dit_status launch_gemv(int dtype, const float* in, const GemvBatch* batches_dev, int n_batches, int total_rows,
+                       float* out, int64_t out_stride, int R, int K, int silu_input, cudaStream_t st);
+dit_status launch_adaln(int dtype, float* x, const void* h, const float* gate, const float* shift, const float* scale,
+                        int64_t mod_stride, const int32_t* cu, int R, void* y, int T, int D, float eps, cudaStream_t st);
+dit_status launch_qknorm_rope(int dtype, void* qkv, int64_t row_stride, int T, int H, int d, int n_tensors,
+                              const void* gq, const void* gk, float eps, const float* rc, const float* rs,
+                              cudaStream_t st);
+dit_status launch_rope_table(const SeqMeta* meta, int R, int T, int d, const int32_t rope_dims[3], float theta,
+                             float* rc, float* rs, cudaStream_t st);
+dit_status launch_patchify(int dtype, const void* lat, void* patches, int C, int F, int H, int W, const int32_t patch[3],
+                           cudaStream_t st);
+dit_status launch_unpatchify(int dtype, const float* tok, void* out, int C, int F, int H, int W, const int32_t patch[3],
+                             cudaStream_t st);
+dit_status launch_merge(int dtype, const void* const* o_parts, const float* const* lses, int P, int64_t n_rows_heads,
+                        int d, void* o, float* lse_out, cudaStream_t st);
+
+// GEMM: out[M,N] = epi(A[M,K] W[N,K]^T + bias).  *_simt works for both dtypes; *_tc is the tcgen05 path (bf16).
+dit_status launch_gemm_simt(int dtype, int epi, const void* A, int64_t lda, const void* W, const void* bias, void* out,
+                            int64_t ldo, int M, int N, int K, cudaStream_t st);
+dit_status launch_gemm_tc(int epi, const void* A, int64_t lda, const void* W, const void* bias, void* out, int64_t ldo,
+                          int M, int N, int K, cudaStream_t st);
+bool gemm_tc_supported(int epi, const void* A, int64_t lda, const void* W, void* out, int64_t ldo, int M, int N, int K);
+
+// Attention over packed sequences.  q rows [cu_q[r], cu_q[r+1]) attend to k/v rows [cu_k[r], cu_k[r+1])
+// restricted to shard `shard` of `n_shards` (contiguous, size ceil(len/n_shards), R20).
+struct AttnArgs {
+  const void* q; const void* k; const void* v;
+  int64_t q_stride, kv_stride;     // row strides in elements
+  void* o; int64_t o_stride;
+  float* lse;                      // [rows, H] or nullptr
+  const int32_t* cu_q; const int32_t* cu_k;   // device, [R+1]; nullptr => single request [0, n_q) x [0, n_k)
+  const int32_t* cu_q_host; const int32_t* cu_k_host;
+  int R; int n_q; int n_k;         // totals
+  int H; int d;
+  float scale;
+  int shard, n_shards;
+};
+dit_status launch_attn_simt(int dtype, const AttnArgs& a, cudaStream_t st);
+dit_status launch_attn_tc(const AttnArgs& a, cudaStream_t st);
+bool attn_tc_supported(const AttnArgs& a);
+
+}  // namespace dit

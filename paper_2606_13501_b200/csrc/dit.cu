@@ -1,0 +1,606 @@
+// dit.cu — handle, workspace carving, step orchestration and the C ABI of libdit_b200 (include/dit.h).
+// Every stage of the step is a kernel launch on the caller's stream; no host synchronisation inside a step.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <string>
+#include <vector>
+
+#include "common.cuh"
+
+namespace dit {
+
+int g_launches = 0;
+static thread_local char g_err[512] = "";
+void set_error(const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+}
+const char* get_error() { return g_err; }
+
+static size_t esize(int dtype) { return dtype == DIT_F32 ? 4 : 2; }
+
+struct BlockW {
+  const void *mod_w, *mod_b, *wqkv, *bqkv, *gq, *gk, *wo, *bo, *w1, *b1, *w2, *b2;
+  const void *cwq, *cbq, *cwkv, *cbkv, *cgq, *cgk, *cwo, *cbo;
+};
+
+struct Workspace {
+  float* x;        // [Tm, D] residual stream fp32
+  void* y;         // [Tm, D]
+  void* qkv;       // [Tm, 3D]
+  void* o;         // [Tm, D]
+  void* h;         // [Tm, D]
+  void* u;         // [Tm, F]
+  float* c1;       // [Rm, D] first t-MLP layer
+  float* c;        // [Rm, D]
+  float* mod;      // [Rm, L*6D + 2D]
+  float* rope_c;   // [Tm, d/2]
+  float* rope_s;
+  void* patches;   // [Tm, C*pv]
+  float* tok;      // [Tm, C*pv] fp32
+  void* ctx;       // cross: [Lcm, D]
+  void* kvc;       // cross: [Lcm, 2D]
+  void* o_part;    // [P, Tm, D]   (split_p > 1)
+  float* lse_part; // [P, Tm, H]
+  int32_t* cu_dev;     // [Rm+1]
+  int32_t* cu_cond_dev;// [Rm+1]
+  SeqMeta* meta_dev;   // [Rm]
+  GemvBatch* gemv_tab; // [L + 1 + 2]
+  void* stage_in;  // host-call staging: latents | temb | cond
+  void* stage_out;
+  size_t total;
+};
+
+}  // namespace dit
+
+using namespace dit;
+
+struct dit_handle_s {
+  dit_config cfg;
+  BlockW* blocks;
+  int n_blocks;
+  const void *t_w1, *t_b1, *t_w2, *t_b2, *pe_w, *pe_b, *cp_w, *cp_b, *fm_w, *fm_b, *f_w, *f_b;
+  Workspace ws;
+  int stop_block, stop_stage;
+  // cached per-call geometry (skip rebuilding RoPE tables when unchanged)
+  std::vector<int32_t> last_geom;
+  char err[512];
+};
+
+namespace dit {
+
+static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
+
+static bool carve(const dit_config& c, char* base, Workspace* w) {
+  const size_t es = esize(c.dtype);
+  const size_t Tm = c.max_tokens, D = c.hidden, F = c.mlp_dim, Rm = c.max_requests, L = c.n_blocks;
+  const size_t pvC = (size_t)c.latent_channels * c.patch[0] * c.patch[1] * c.patch[2];
+  const size_t Lcm = c.max_cond_tokens;
+  size_t off = 0;
+  auto take = [&](size_t bytes) {
+    char* p = base ? base + off : nullptr;
+    off += align256(bytes);
+    return (void*)p;
+  };
+  w->x = (float*)take(Tm * D * 4);
+  w->y = take(Tm * D * es);
+  w->qkv = take(Tm * 3 * D * es);
+  w->o = take(Tm * D * es);
+  w->h = take(Tm * D * es);
+  w->u = take(Tm * F * es);
+  w->c1 = (float*)take(Rm * D * 4);
+  w->c = (float*)take(Rm * D * 4);
+  w->mod = (float*)take(Rm * (L * 6 * D + 2 * D) * 4);
+  w->rope_c = (float*)take(Tm * (c.head_dim / 2) * 4);
+  w->rope_s = (float*)take(Tm * (c.head_dim / 2) * 4);
+  w->patches = take(Tm * pvC * es);
+  w->tok = (float*)take(Tm * pvC * 4);
+  w->ctx = take(c.cond_mode == DIT_COND_CROSS ? Lcm * D * es : 0);
+  w->kvc = take(c.cond_mode == DIT_COND_CROSS ? Lcm * 2 * D * es : 0);
+  w->o_part = take(c.split_p > 1 ? (size_t)c.split_p * Tm * D * es : 0);
+  w->lse_part = (float*)take(c.split_p > 1 ? (size_t)c.split_p * Tm * c.n_heads * 4 : 0);
+  w->cu_dev = (int32_t*)take((Rm + 1) * 4);
+  w->cu_cond_dev = (int32_t*)take((Rm + 1) * 4);
+  w->meta_dev = (SeqMeta*)take(Rm * sizeof(SeqMeta));
+  w->gemv_tab = (GemvBatch*)take((L + 4) * sizeof(GemvBatch));
+  w->stage_in = take(Tm * pvC * es + Rm * c.temb_dim * 4 + Lcm * c.cond_dim * es + 1024);
+  w->stage_out = take(Tm * pvC * es);
+  w->total = off;
+  return true;
+}
+
+static dit_status validate(const dit_config* c) {
+  DIT_REQUIRE(c != nullptr, DIT_ERR_INVALID_ARG, "config is NULL");
+  DIT_REQUIRE(c->struct_size == (int)sizeof(dit_config), DIT_ERR_INVALID_ARG, "dit_config.struct_size %d != %d",
+              c->struct_size, (int)sizeof(dit_config));
+  DIT_REQUIRE(c->dtype == DIT_F32 || c->dtype == DIT_BF16, DIT_ERR_INVALID_ARG, "dtype %d", c->dtype);
+  DIT_REQUIRE(c->n_blocks >= 0 && c->n_blocks <= 256, DIT_ERR_INVALID_ARG, "n_blocks %d", c->n_blocks);
+  DIT_REQUIRE(c->head_dim == 64 || c->head_dim == 128, DIT_ERR_UNSUPPORTED, "head_dim %d not in {64,128}", c->head_dim);
+  DIT_REQUIRE(c->n_heads > 0 && c->hidden == c->n_heads * c->head_dim, DIT_ERR_INVALID_ARG,
+              "hidden %d != n_heads %d * head_dim %d", c->hidden, c->n_heads, c->head_dim);
+  DIT_REQUIRE(c->hidden % 256 == 0, DIT_ERR_UNSUPPORTED, "hidden %d must be a multiple of 256", c->hidden);
+  DIT_REQUIRE(c->mlp_dim > 0 && c->mlp_dim % 8 == 0, DIT_ERR_UNSUPPORTED, "mlp_dim %d must be a multiple of 8", c->mlp_dim);
+  DIT_REQUIRE(c->latent_channels > 0 && c->patch[0] > 0 && c->patch[1] > 0 && c->patch[2] > 0, DIT_ERR_INVALID_ARG,
+              "latent_channels / patch must be positive");
+  DIT_REQUIRE(c->temb_dim > 0 && c->temb_dim % 8 == 0, DIT_ERR_UNSUPPORTED, "temb_dim %d must be a multiple of 8", c->temb_dim);
+  DIT_REQUIRE(c->cond_mode >= DIT_COND_NONE && c->cond_mode <= DIT_COND_CROSS, DIT_ERR_INVALID_ARG, "cond_mode %d", c->cond_mode);
+  DIT_REQUIRE(c->cond_mode == DIT_COND_NONE || c->cond_dim > 0, DIT_ERR_INVALID_ARG, "cond_dim %d", c->cond_dim);
+  const int rs = c->rope_dims[0] + c->rope_dims[1] + c->rope_dims[2];
+  DIT_REQUIRE(rs == 0 || rs == c->head_dim, DIT_ERR_INVALID_ARG, "sum(rope_dims) = %d must be 0 or head_dim", rs);
+  for (int a = 0; a < 3; ++a)
+    DIT_REQUIRE(c->rope_dims[a] >= 0 && c->rope_dims[a] % 2 == 0, DIT_ERR_INVALID_ARG, "rope_dims[%d] = %d must be even", a, c->rope_dims[a]);
+  DIT_REQUIRE(c->split_p == 1 || c->split_p == 2 || c->split_p == 4 || c->split_p == 8, DIT_ERR_INVALID_ARG,
+              "split_p %d not in {1,2,4,8}", c->split_p);
+  DIT_REQUIRE(c->max_tokens > 0 && c->max_requests > 0 && c->max_requests <= 64 && c->max_cond_tokens >= 0,
+              DIT_ERR_INVALID_ARG, "capacities: max_tokens %d max_requests %d max_cond_tokens %d", c->max_tokens,
+              c->max_requests, c->max_cond_tokens);
+  return DIT_OK;
+}
+
+// GEMM dispatch: bf16 -> tcgen05 whenever the shape/alignment allows, else FFMA.  fp32 -> FFMA (no TF32).
+static dit_status gemm(int dtype, int epi, const void* A, int64_t lda, const void* W, const void* bias, void* out,
+                       int64_t ldo, int M, int N, int K, cudaStream_t st) {
+  if (dtype == DIT_BF16 && gemm_tc_supported(epi, A, lda, W, out, ldo, M, N, K))
+    return launch_gemm_tc(epi, A, lda, W, bias, out, ldo, M, N, K, st);
+  return launch_gemm_simt(dtype, epi, A, lda, W, bias, out, ldo, M, N, K, st);
+}
+
+static dit_status attention(int dtype, const AttnArgs& a, cudaStream_t st) {
+  if (dtype == DIT_BF16 && attn_tc_supported(a)) return launch_attn_tc(a, st);
+  return launch_attn_simt(dtype, a, st);
+}
+
+struct StepGeom {
+  int R;
+  std::vector<int32_t> cu;        // [R+1] sequence rows
+  std::vector<int32_t> cu_cond;   // [R+1] cond rows in cond_packed
+  std::vector<int32_t> ncond;     // [R]
+  std::vector<int32_t> grids;     // [R][3] latent grids
+  std::vector<int64_t> lat_off;   // [R+1] element offsets in the packed latents
+};
+
+static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents, const float* temb, const void* cond,
+                           void* out, cudaStream_t st) {
+  const dit_config& c = hd->cfg;
+  Workspace& w = hd->ws;
+  const int dt = c.dtype;
+  const size_t es = esize(dt);
+  const int D = c.hidden, F = c.mlp_dim, H = c.n_heads, d = c.head_dim, L = c.n_blocks, R = g.R;
+  const int pvC = c.latent_channels * c.patch[0] * c.patch[1] * c.patch[2];
+  const int T = g.cu[R];
+  const int64_t mod_stride = (int64_t)L * 6 * D + 2 * D;
+  const bool joint = c.cond_mode == DIT_COND_JOINT, cross = c.cond_mode == DIT_COND_CROSS;
+  const bool rope = (c.rope_dims[0] + c.rope_dims[1] + c.rope_dims[2]) > 0;
+  auto stop = [&](int blk, int stage) { return hd->stop_block == blk && hd->stop_stage == stage; };
+
+  // ---- per-call geometry to the device (pageable host memory: the driver stages it before returning)
+  std::vector<SeqMeta> meta(R);
+  std::vector<int32_t> geom;
+  for (int r = 0; r < R; ++r) {
+    meta[r].seq_start = g.cu[r];
+    meta[r].n_cond = joint ? g.ncond[r] : 0;
+    meta[r].gf = g.grids[3 * r] / c.patch[0];
+    meta[r].gh = g.grids[3 * r + 1] / c.patch[1];
+    meta[r].gw = g.grids[3 * r + 2] / c.patch[2];
+    meta[r].lat_off_lo = (int32_t)(g.lat_off[r] & 0xffffffff);
+    meta[r].lat_off_hi = (int32_t)(g.lat_off[r] >> 32);
+    meta[r].pad = 0;
+    geom.insert(geom.end(), {meta[r].seq_start, meta[r].n_cond, meta[r].gf, meta[r].gh, meta[r].gw});
+  }
+  geom.push_back(T);
+  const bool geom_changed = geom != hd->last_geom;
+  if (geom_changed) {
+    DIT_CUDA_OK(cudaMemcpyAsync(w.cu_dev, g.cu.data(), (R + 1) * 4, cudaMemcpyHostToDevice, st));
+    DIT_CUDA_OK(cudaMemcpyAsync(w.cu_cond_dev, g.cu_cond.data(), (R + 1) * 4, cudaMemcpyHostToDevice, st));
+    DIT_CUDA_OK(cudaMemcpyAsync(w.meta_dev, meta.data(), R * sizeof(SeqMeta), cudaMemcpyHostToDevice, st));
+    if (rope) {
+      dit_status s = launch_rope_table(w.meta_dev, R, T, d, c.rope_dims, c.rope_theta, w.rope_c, w.rope_s, st);
+      if (s != DIT_OK) return s;
+    }
+    hd->last_geom = geom;
+  }
+  const int32_t* cu_dev = R > 1 ? w.cu_dev : nullptr;
+  dit_status s;
+#define RUN(expr)                  \
+  do {                             \
+    s = (expr);                    \
+    if (s != DIT_OK) return s;     \
+  } while (0)
+
+  // ---- steps 1-2: c = W2 SiLU(W1 temb + b1) + b2;  mod = Wmod SiLU(c) + bmod for ALL blocks in one launch
+  RUN(launch_gemv(dt, temb, w.gemv_tab + 0, 1, D, w.c1, D, R, c.temb_dim, 0, st));
+  RUN(launch_gemv(dt, w.c1, w.gemv_tab + 1, 1, D, w.c, D, R, D, 1, st));
+  RUN(launch_gemv(dt, w.c, w.gemv_tab + 2, L + 1, L * 6 * D + 2 * D, w.mod, mod_stride, R, D, 1, st));
+
+  // ---- steps 3-4: patch-embed and cond projection write the fp32 residual stream
+  for (int r = 0; r < R; ++r) {
+    const int Fr = g.grids[3 * r], Hr = g.grids[3 * r + 1], Wr = g.grids[3 * r + 2];
+    const int Nr = (Fr / c.patch[0]) * (Hr / c.patch[1]) * (Wr / c.patch[2]);
+    const int Lc = joint ? g.ncond[r] : 0;
+    const int row0 = g.cu[r] + Lc;
+    char* pr = (char*)w.patches + (size_t)row0 * pvC * es;
+    RUN(launch_patchify(dt, (const char*)latents + g.lat_off[r] * es, pr, c.latent_channels, Fr, Hr, Wr, c.patch, st));
+    RUN(gemm(dt, DIT_EPI_BIAS_F32, pr, pvC, hd->pe_w, hd->pe_b, w.x + (size_t)row0 * D, D, Nr, D, pvC, st));
+    if (joint && Lc > 0)
+      RUN(gemm(dt, DIT_EPI_BIAS_F32, (const char*)cond + (size_t)g.cu_cond[r] * c.cond_dim * es, c.cond_dim, hd->cp_w,
+               hd->cp_b, w.x + (size_t)g.cu[r] * D, D, Lc, D, c.cond_dim, st));
+  }
+  const int Lc_total = g.cu_cond[R];
+  if (cross && Lc_total > 0)
+    RUN(gemm(dt, DIT_EPI_BIAS, cond, c.cond_dim, hd->cp_w, hd->cp_b, w.ctx, D, Lc_total, D, c.cond_dim, st));
+
+  // ---- step 5: blocks.  `pending_h` / `pending_gate` carry the gated residual into the next adaLN kernel.
+  const void* pending_h = nullptr;
+  const float* pending_gate = nullptr;
+  bool pending_has_gate = false;
+  const float scale = 1.0f / sqrtf((float)d);
+  for (int l = 0; l < L; ++l) {
+    const BlockW& b = hd->blocks[l];
+    const float* m = w.mod + (size_t)l * 6 * D;
+    RUN(launch_adaln(dt, w.x, pending_h, pending_has_gate ? pending_gate : nullptr, m + 0 * D, m + 1 * D, mod_stride,
+                     cu_dev, R, w.y, T, D, c.ln_eps, st));
+    if (stop(l, DIT_STAGE_Y1)) return DIT_OK;
+    RUN(gemm(dt, DIT_EPI_BIAS, w.y, D, b.wqkv, b.bqkv, w.qkv, 3 * D, T, 3 * D, D, st));
+    RUN(launch_qknorm_rope(dt, w.qkv, 3 * D, T, H, d, 2, c.qk_rmsnorm ? b.gq : nullptr, c.qk_rmsnorm ? b.gk : nullptr,
+                           c.rms_eps, rope ? w.rope_c : nullptr, rope ? w.rope_s : nullptr, st));
+    if (stop(l, DIT_STAGE_QKV)) return DIT_OK;
+    {
+      AttnArgs a;
+      a.q = w.qkv; a.k = (char*)w.qkv + (size_t)D * es; a.v = (char*)w.qkv + (size_t)2 * D * es;
+      a.q_stride = a.kv_stride = 3 * D;
+      a.cu_q = a.cu_k = R > 1 ? w.cu_dev : nullptr;
+      a.cu_q_host = a.cu_k_host = g.cu.data();
+      a.R = R; a.n_q = T; a.n_k = T; a.H = H; a.d = d; a.scale = scale;
+      if (c.split_p == 1) {
+        a.o = w.o; a.o_stride = D; a.lse = nullptr; a.shard = 0; a.n_shards = 1;
+        RUN(attention(dt, a, st));
+      } else {  // P split-KV partials + LSE merge (north_star subsystem 5)
+        const void* op[8];
+        const float* lp[8];
+        for (int p = 0; p < c.split_p; ++p) {
+          a.o = (char*)w.o_part + (size_t)p * c.max_tokens * D * es;
+          a.o_stride = D;
+          a.lse = w.lse_part + (size_t)p * c.max_tokens * H;
+          a.shard = p; a.n_shards = c.split_p;
+          op[p] = a.o; lp[p] = a.lse;
+          RUN(attention(dt, a, st));
+        }
+        RUN(launch_merge(dt, op, lp, c.split_p, (int64_t)T * H, d, w.o, nullptr, st));
+      }
+    }
+    if (stop(l, DIT_STAGE_ATTN)) return DIT_OK;
+    RUN(gemm(dt, DIT_EPI_BIAS, w.o, D, b.wo, b.bo, w.h, D, T, D, D, st));
+    if (stop(l, DIT_STAGE_OPROJ)) return DIT_OK;
+    if (cross) {  // R10: x <- x + gate1 h;  x <- x + Wo_c Attn(RMS(Wq_c LN(x)), RMS(Wk_c ctx), Wv_c ctx) + bo_c
+      RUN(launch_adaln(dt, w.x, w.h, m + 2 * D, nullptr, nullptr, mod_stride, cu_dev, R, w.y, T, D, c.ln_eps, st));
+      RUN(gemm(dt, DIT_EPI_BIAS, w.y, D, b.cwq, b.cbq, w.qkv, D, T, D, D, st));
+      RUN(launch_qknorm_rope(dt, w.qkv, D, T, H, d, 1, b.cgq, nullptr, c.rms_eps, nullptr, nullptr, st));
+      if (Lc_total > 0) {
+        RUN(gemm(dt, DIT_EPI_BIAS, w.ctx, D, b.cwkv, b.cbkv, w.kvc, 2 * D, Lc_total, 2 * D, D, st));
+        RUN(launch_qknorm_rope(dt, w.kvc, 2 * D, Lc_total, H, d, 1, b.cgk, nullptr, c.rms_eps, nullptr, nullptr, st));
+      }
+      AttnArgs a;
+      a.q = w.qkv; a.q_stride = D;
+      a.k = w.kvc; a.v = (char*)w.kvc + (size_t)D * es; a.kv_stride = 2 * D;
+      a.o = w.o; a.o_stride = D; a.lse = nullptr;
+      a.cu_q = R > 1 ? w.cu_dev : nullptr; a.cu_k = R > 1 ? w.cu_cond_dev : nullptr;
+      a.cu_q_host = g.cu.data(); a.cu_k_host = g.cu_cond.data();
+      a.R = R; a.n_q = T; a.n_k = Lc_total; a.H = H; a.d = d; a.scale = scale; a.shard = 0; a.n_shards = 1;
+      RUN(attention(dt, a, st));
+      RUN(gemm(dt, DIT_EPI_BIAS, w.o, D, b.cwo, b.cbo, w.h, D, T, D, D, st));
+      if (stop(l, DIT_STAGE_CROSS)) return DIT_OK;
+      RUN(launch_adaln(dt, w.x, w.h, nullptr, m + 3 * D, m + 4 * D, mod_stride, cu_dev, R, w.y, T, D, c.ln_eps, st));
+    } else {
+      RUN(launch_adaln(dt, w.x, w.h, m + 2 * D, m + 3 * D, m + 4 * D, mod_stride, cu_dev, R, w.y, T, D, c.ln_eps, st));
+    }
+    if (stop(l, DIT_STAGE_Y2)) return DIT_OK;
+    RUN(gemm(dt, DIT_EPI_BIAS_GELU, w.y, D, b.w1, b.b1, w.u, F, T, F, D, st));
+    if (stop(l, DIT_STAGE_FC1)) return DIT_OK;
+    RUN(gemm(dt, DIT_EPI_BIAS, w.u, F, b.w2, b.b2, w.h, D, T, D, F, st));
+    if (stop(l, DIT_STAGE_FC2)) return DIT_OK;
+    pending_h = w.h;
+    pending_gate = m + 5 * D;
+    pending_has_gate = true;
+  }
+  // ---- step 6: final adaLN (folds the last gated residual), Linear D -> C*pv, unpatchify (image tokens only)
+  const float* mf = w.mod + (size_t)L * 6 * D;
+  RUN(launch_adaln(dt, w.x, pending_h, pending_has_gate ? pending_gate : nullptr, mf, mf + D, mod_stride, cu_dev, R,
+                   w.y, T, D, c.ln_eps, st));
+  for (int r = 0; r < R; ++r) {
+    const int Fr = g.grids[3 * r], Hr = g.grids[3 * r + 1], Wr = g.grids[3 * r + 2];
+    const int Nr = (Fr / c.patch[0]) * (Hr / c.patch[1]) * (Wr / c.patch[2]);
+    const int row0 = g.cu[r] + (joint ? g.ncond[r] : 0);
+    float* tk = w.tok + (size_t)row0 * pvC;
+    RUN(gemm(dt, DIT_EPI_BIAS_F32, (char*)w.y + (size_t)row0 * D * es, D, hd->f_w, hd->f_b, tk, pvC, Nr, pvC, D, st));
+    RUN(launch_unpatchify(dt, tk, (char*)out + g.lat_off[r] * es, c.latent_channels, Fr, Hr, Wr, c.patch, st));
+  }
+#undef RUN
+  return DIT_OK;
+}
+
+static dit_status build_geom(dit_handle h, int R, const int32_t* cu, const int32_t* ncond, const int32_t* grids,
+                             StepGeom* g) {
+  const dit_config& c = h->cfg;
+  DIT_REQUIRE(R >= 1 && R <= c.max_requests, DIT_ERR_INVALID_ARG, "n_requests %d not in 1..%d", R, c.max_requests);
+  g->R = R;
+  g->cu.assign(R + 1, 0);
+  g->cu_cond.assign(R + 1, 0);
+  g->ncond.assign(R, 0);
+  g->grids.assign(grids, grids + 3 * R);
+  g->lat_off.assign(R + 1, 0);
+  for (int r = 0; r < R; ++r) {
+    const int Fr = grids[3 * r], Hr = grids[3 * r + 1], Wr = grids[3 * r + 2];
+    DIT_REQUIRE(Fr > 0 && Hr > 0 && Wr > 0 && Fr % c.patch[0] == 0 && Hr % c.patch[1] == 0 && Wr % c.patch[2] == 0,
+                DIT_ERR_INVALID_ARG, "request %d: latent grid {%d,%d,%d} not a positive multiple of the patch", r, Fr, Hr, Wr);
+    const int64_t Nr = (int64_t)(Fr / c.patch[0]) * (Hr / c.patch[1]) * (Wr / c.patch[2]);
+    const int nc = c.cond_mode == DIT_COND_NONE ? 0 : (ncond ? ncond[r] : 0);
+    DIT_REQUIRE(nc >= 0, DIT_ERR_INVALID_ARG, "request %d: n_cond %d < 0", r, nc);
+    g->ncond[r] = nc;
+    const int64_t Tr = Nr + (c.cond_mode == DIT_COND_JOINT ? nc : 0);
+    DIT_REQUIRE(g->cu[r] + Tr <= c.max_tokens, DIT_ERR_INVALID_ARG, "sequence rows exceed max_tokens %d", c.max_tokens);
+    g->cu[r + 1] = g->cu[r] + (int32_t)Tr;
+    g->cu_cond[r + 1] = g->cu_cond[r] + nc;
+    g->lat_off[r + 1] = g->lat_off[r] + (int64_t)c.latent_channels * Fr * Hr * Wr;
+    if (cu) DIT_REQUIRE(cu[r + 1] - cu[r] == Tr && cu[0] == 0, DIT_ERR_INVALID_ARG,
+                        "cu_seqlens[%d..%d] = %d disagrees with grid/n_cond (%lld rows)", r, r + 1, cu[r + 1] - cu[r], (long long)Tr);
+  }
+  DIT_REQUIRE(g->cu_cond[R] <= c.max_cond_tokens, DIT_ERR_INVALID_ARG, "cond tokens %d exceed max_cond_tokens %d",
+              g->cu_cond[R], c.max_cond_tokens);
+  return DIT_OK;
+}
+
+}  // namespace dit
+
+// =================================================================================================
+// C ABI
+// =================================================================================================
+extern "C" {
+
+size_t dit_workspace_bytes(const dit_config* cfg) {
+  if (validate(cfg) != DIT_OK) return 0;
+  Workspace w;
+  carve(*cfg, nullptr, &w);
+  return w.total;
+}
+
+dit_status dit_init(const dit_config* cfg, const dit_weight* weights, int32_t n_weights, void* workspace,
+                    size_t workspace_bytes, dit_handle* out) {
+  DIT_REQUIRE(out != nullptr, DIT_ERR_INVALID_ARG, "out handle pointer is NULL");
+  *out = nullptr;
+  dit_status s = validate(cfg);
+  if (s != DIT_OK) return s;
+  DIT_REQUIRE(workspace != nullptr && ((uintptr_t)workspace & 255) == 0, DIT_ERR_WORKSPACE, "workspace must be 256-byte aligned");
+  Workspace w;
+  carve(*cfg, (char*)workspace, &w);
+  DIT_REQUIRE(workspace_bytes >= w.total, DIT_ERR_WORKSPACE, "workspace too small: %zu < %zu", workspace_bytes, w.total);
+  DIT_REQUIRE(weights != nullptr || n_weights == 0, DIT_ERR_INVALID_ARG, "weights is NULL");
+
+  const int64_t D = cfg->hidden, F = cfg->mlp_dim, d = cfg->head_dim, L = cfg->n_blocks;
+  const int64_t pvC = (int64_t)cfg->latent_channels * cfg->patch[0] * cfg->patch[1] * cfg->patch[2];
+  std::map<std::string, int64_t> need;
+  need["t_mlp.w1"] = D * cfg->temb_dim; need["t_mlp.b1"] = D; need["t_mlp.w2"] = D * D; need["t_mlp.b2"] = D;
+  need["patch_embed.w"] = D * pvC; need["patch_embed.b"] = D;
+  if (cfg->cond_mode != DIT_COND_NONE) { need["cond_proj.w"] = D * cfg->cond_dim; need["cond_proj.b"] = D; }
+  for (int l = 0; l < L; ++l) {
+    std::string p = "blocks." + std::to_string(l) + ".";
+    need[p + "mod.w"] = 6 * D * D; need[p + "mod.b"] = 6 * D;
+    need[p + "attn.wqkv"] = 3 * D * D; need[p + "attn.bqkv"] = 3 * D;
+    if (cfg->qk_rmsnorm) { need[p + "attn.gq"] = d; need[p + "attn.gk"] = d; }
+    need[p + "attn.wo"] = D * D; need[p + "attn.bo"] = D;
+    need[p + "mlp.w1"] = F * D; need[p + "mlp.b1"] = F; need[p + "mlp.w2"] = D * F; need[p + "mlp.b2"] = D;
+    if (cfg->cond_mode == DIT_COND_CROSS) {
+      need[p + "cross.wq"] = D * D; need[p + "cross.bq"] = D; need[p + "cross.wkv"] = 2 * D * D; need[p + "cross.bkv"] = 2 * D;
+      need[p + "cross.gq"] = d; need[p + "cross.gk"] = d; need[p + "cross.wo"] = D * D; need[p + "cross.bo"] = D;
+    }
+  }
+  need["final.mod.w"] = 2 * D * D; need["final.mod.b"] = 2 * D; need["final.w"] = pvC * D; need["final.b"] = pvC;
+  std::map<std::string, const void*> got;
+  for (int i = 0; i < n_weights; ++i) {
+    DIT_REQUIRE(weights[i].name != nullptr, DIT_ERR_INVALID_ARG, "weight %d has no name", i);
+    auto it = need.find(weights[i].name);
+    DIT_REQUIRE(it != need.end(), DIT_ERR_INVALID_ARG, "unknown weight '%s'", weights[i].name);
+    DIT_REQUIRE(it->second == weights[i].numel, DIT_ERR_INVALID_ARG, "weight '%s': numel %lld, expected %lld",
+                weights[i].name, (long long)weights[i].numel, (long long)it->second);
+    DIT_REQUIRE(weights[i].dev_ptr != nullptr && ((uintptr_t)weights[i].dev_ptr & 15) == 0, DIT_ERR_INVALID_ARG,
+                "weight '%s': pointer must be non-NULL and 16-byte aligned", weights[i].name);
+    got[weights[i].name] = weights[i].dev_ptr;
+  }
+  for (auto& kv : need) DIT_REQUIRE(got.count(kv.first), DIT_ERR_INVALID_ARG, "missing weight '%s'", kv.first.c_str());
+
+  dit_handle h = new dit_handle_s();
+  h->cfg = *cfg;
+  h->ws = w;
+  h->n_blocks = (int)L;
+  h->blocks = new BlockW[L > 0 ? L : 1];
+  h->stop_block = -1; h->stop_stage = -1;
+  h->err[0] = 0;
+  auto G = [&](const std::string& n) -> const void* { auto it = got.find(n); return it == got.end() ? nullptr : it->second; };
+  h->t_w1 = G("t_mlp.w1"); h->t_b1 = G("t_mlp.b1"); h->t_w2 = G("t_mlp.w2"); h->t_b2 = G("t_mlp.b2");
+  h->pe_w = G("patch_embed.w"); h->pe_b = G("patch_embed.b"); h->cp_w = G("cond_proj.w"); h->cp_b = G("cond_proj.b");
+  h->fm_w = G("final.mod.w"); h->fm_b = G("final.mod.b"); h->f_w = G("final.w"); h->f_b = G("final.b");
+  std::vector<GemvBatch> tab(L + 3);
+  tab[0] = {h->t_w1, h->t_b1, (int32_t)D, 0, 0, 0};
+  tab[1] = {h->t_w2, h->t_b2, (int32_t)D, 0, 0, 0};
+  for (int l = 0; l < L; ++l) {
+    std::string p = "blocks." + std::to_string(l) + ".";
+    BlockW& b = h->blocks[l];
+    b.mod_w = G(p + "mod.w"); b.mod_b = G(p + "mod.b"); b.wqkv = G(p + "attn.wqkv"); b.bqkv = G(p + "attn.bqkv");
+    b.gq = G(p + "attn.gq"); b.gk = G(p + "attn.gk"); b.wo = G(p + "attn.wo"); b.bo = G(p + "attn.bo");
+    b.w1 = G(p + "mlp.w1"); b.b1 = G(p + "mlp.b1"); b.w2 = G(p + "mlp.w2"); b.b2 = G(p + "mlp.b2");
+    b.cwq = G(p + "cross.wq"); b.cbq = G(p + "cross.bq"); b.cwkv = G(p + "cross.wkv"); b.cbkv = G(p + "cross.bkv");
+    b.cgq = G(p + "cross.gq"); b.cgk = G(p + "cross.gk"); b.cwo = G(p + "cross.wo"); b.cbo = G(p + "cross.bo");
+    tab[2 + l] = {b.mod_w, b.mod_b, (int32_t)(6 * D), (int32_t)(l * 6 * D), (int32_t)(l * 6 * D), 0};
+  }
+  tab[2 + L] = {h->fm_w, h->fm_b, (int32_t)(2 * D), (int32_t)(L * 6 * D), (int32_t)(L * 6 * D), 0};
+  cudaError_t e = cudaMemcpy(w.gemv_tab, tab.data(), (L + 3) * sizeof(GemvBatch), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) {
+    set_error("dit_init: pointer-table upload failed: %s", cudaGetErrorString(e));
+    delete[] h->blocks;
+    delete h;
+    return DIT_ERR_CUDA;
+  }
+  *out = h;
+  return DIT_OK;
+}
+
+dit_status dit_step_varlen(dit_handle h, const void* latents_packed, const float* timestep_emb, const void* cond_packed,
+                           const int32_t* cu_seqlens, const int32_t* n_cond, const int32_t* latent_grids,
+                           int32_t n_requests, void* out_packed, void* stream) {
+  DIT_REQUIRE(h != nullptr, DIT_ERR_INVALID_ARG, "handle is NULL");
+  DIT_REQUIRE(latents_packed && timestep_emb && latent_grids && out_packed, DIT_ERR_INVALID_ARG, "NULL tensor argument");
+  StepGeom g;
+  dit_status s = build_geom(h, n_requests, cu_seqlens, n_cond, latent_grids, &g);
+  if (s != DIT_OK) return s;
+  DIT_REQUIRE(g.cu_cond[n_requests] == 0 || cond_packed != nullptr, DIT_ERR_INVALID_ARG, "cond tokens announced but cond pointer is NULL");
+  return run_step(h, g, latents_packed, timestep_emb, cond_packed, out_packed, (cudaStream_t)stream);
+}
+
+dit_status dit_step(dit_handle h, const void* latents, const float* timestep_emb, const void* cond_tokens,
+                    int32_t n_cond, const int32_t latent_grid[3], void* out, void* stream) {
+  return dit_step_varlen(h, latents, timestep_emb, cond_tokens, nullptr, &n_cond, latent_grid, 1, out, stream);
+}
+
+dit_status dit_step_host(dit_handle h, const void* latents_host, const float* timestep_emb_host,
+                         const void* cond_tokens_host, int32_t n_cond, const int32_t latent_grid[3], void* out_host,
+                         void* stream) {
+  DIT_REQUIRE(h != nullptr, DIT_ERR_INVALID_ARG, "handle is NULL");
+  DIT_REQUIRE(latents_host && timestep_emb_host && latent_grid && out_host, DIT_ERR_INVALID_ARG, "NULL tensor argument");
+  StepGeom g;
+  dit_status s = build_geom(h, 1, nullptr, &n_cond, latent_grid, &g);
+  if (s != DIT_OK) return s;
+  const dit_config& c = h->cfg;
+  const size_t es = esize(c.dtype);
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t lat_bytes = (size_t)g.lat_off[1] * es;
+  const size_t temb_bytes = (size_t)c.temb_dim * 4;
+  const size_t cond_bytes = (size_t)g.cu_cond[1] * c.cond_dim * es;
+  char* p = (char*)h->ws.stage_in;
+  char* lat_d = p;
+  char* temb_d = p + align256(lat_bytes);
+  char* cond_d = temb_d + align256(temb_bytes);
+  DIT_CUDA_OK(cudaMemcpyAsync(lat_d, latents_host, lat_bytes, cudaMemcpyHostToDevice, st));
+  DIT_CUDA_OK(cudaMemcpyAsync(temb_d, timestep_emb_host, temb_bytes, cudaMemcpyHostToDevice, st));
+  if (cond_bytes) {
+    DIT_REQUIRE(cond_tokens_host != nullptr, DIT_ERR_INVALID_ARG, "cond tokens announced but cond pointer is NULL");
+    DIT_CUDA_OK(cudaMemcpyAsync(cond_d, cond_tokens_host, cond_bytes, cudaMemcpyHostToDevice, st));
+  }
+  s = run_step(h, g, lat_d, (const float*)temb_d, cond_d, h->ws.stage_out, st);
+  if (s != DIT_OK) return s;
+  DIT_CUDA_OK(cudaMemcpyAsync(out_host, h->ws.stage_out, lat_bytes, cudaMemcpyDeviceToHost, st));
+  return DIT_OK;
+}
+
+dit_status dit_attn_partial(int32_t dtype, const void* q, const void* k, const void* v, int32_t n_q, int32_t n_k,
+                            int32_t n_heads, int32_t head_dim, int64_t q_row_stride, int64_t kv_row_stride,
+                            float softmax_scale, void* o, float* lse, void* stream) {
+  DIT_REQUIRE(dtype == DIT_F32 || dtype == DIT_BF16, DIT_ERR_INVALID_ARG, "dtype %d", dtype);
+  DIT_REQUIRE(n_q >= 0 && n_k >= 0 && n_heads > 0, DIT_ERR_INVALID_ARG, "n_q %d n_k %d n_heads %d", n_q, n_k, n_heads);
+  DIT_REQUIRE(head_dim == 64 || head_dim == 128, DIT_ERR_UNSUPPORTED, "head_dim %d not in {64,128}", head_dim);
+  DIT_REQUIRE(n_q == 0 || (q && o), DIT_ERR_INVALID_ARG, "q / o is NULL");
+  DIT_REQUIRE(n_k == 0 || (k && v), DIT_ERR_INVALID_ARG, "k / v is NULL");
+  DIT_REQUIRE(q_row_stride >= (int64_t)n_heads * head_dim && kv_row_stride >= (int64_t)n_heads * head_dim,
+              DIT_ERR_INVALID_ARG, "row strides smaller than H*d");
+  AttnArgs a;
+  a.q = q; a.k = k; a.v = v; a.q_stride = q_row_stride; a.kv_stride = kv_row_stride;
+  a.o = o; a.o_stride = (int64_t)n_heads * head_dim; a.lse = lse;
+  a.cu_q = a.cu_k = nullptr; a.cu_q_host = a.cu_k_host = nullptr;
+  a.R = 1; a.n_q = n_q; a.n_k = n_k; a.H = n_heads; a.d = head_dim; a.scale = softmax_scale; a.shard = 0; a.n_shards = 1;
+  return attention(dtype, a, (cudaStream_t)stream);
+}
+
+dit_status dit_attn_merge(int32_t dtype, const void* const* o_partials, const float* const* lses, int32_t P, int32_t n_q,
+                          int32_t n_heads, int32_t head_dim, void* o, float* lse_out, void* stream) {
+  DIT_REQUIRE(dtype == DIT_F32 || dtype == DIT_BF16, DIT_ERR_INVALID_ARG, "dtype %d", dtype);
+  DIT_REQUIRE(P >= 1 && P <= 8, DIT_ERR_INVALID_ARG, "P=%d not in 1..8", P);
+  DIT_REQUIRE(o_partials && lses && (n_q == 0 || o), DIT_ERR_INVALID_ARG, "NULL argument");
+  for (int p = 0; p < P; ++p) DIT_REQUIRE(n_q == 0 || (o_partials[p] && lses[p]), DIT_ERR_INVALID_ARG, "partial %d is NULL", p);
+  return launch_merge(dtype, o_partials, lses, P, (int64_t)n_q * n_heads, head_dim, o, lse_out, (cudaStream_t)stream);
+}
+
+dit_status dit_linear(int32_t dtype, int32_t epilogue, const void* A, int64_t lda, const void* W, const void* bias,
+                      void* out, int64_t ldo, int32_t M, int32_t N, int32_t K, void* stream) {
+  DIT_REQUIRE(dtype == DIT_F32 || dtype == DIT_BF16, DIT_ERR_INVALID_ARG, "dtype %d", dtype);
+  DIT_REQUIRE(epilogue >= DIT_EPI_BIAS && epilogue <= DIT_EPI_BIAS_F32, DIT_ERR_INVALID_ARG, "epilogue %d", epilogue);
+  DIT_REQUIRE(M >= 0 && N > 0 && K > 0 && lda >= K && ldo >= N, DIT_ERR_INVALID_ARG, "bad GEMM shape M=%d N=%d K=%d lda=%lld ldo=%lld",
+              M, N, K, (long long)lda, (long long)ldo);
+  DIT_REQUIRE(M == 0 || (A && W && out), DIT_ERR_INVALID_ARG, "NULL argument");
+  return gemm(dtype, epilogue, A, lda, W, bias, out, ldo, M, N, K, (cudaStream_t)stream);
+}
+
+dit_status dit_adaln(int32_t dtype, float* x, const void* h, const float* gate, const float* shift, const float* scale,
+                     int64_t mod_stride, const int32_t* cu_seqlens_dev, int32_t n_requests, void* y, int32_t T, int32_t D,
+                     float eps, void* stream) {
+  DIT_REQUIRE(dtype == DIT_F32 || dtype == DIT_BF16, DIT_ERR_INVALID_ARG, "dtype %d", dtype);
+  DIT_REQUIRE(T >= 0 && D > 0 && n_requests >= 1 && n_requests <= 64, DIT_ERR_INVALID_ARG, "T=%d D=%d R=%d", T, D, n_requests);
+  DIT_REQUIRE(T == 0 || (x && y), DIT_ERR_INVALID_ARG, "x / y is NULL");
+  DIT_REQUIRE(n_requests == 1 || cu_seqlens_dev, DIT_ERR_INVALID_ARG, "cu_seqlens required for n_requests > 1");
+  return launch_adaln(dtype, x, h, gate, shift, scale, mod_stride, cu_seqlens_dev, n_requests, y, T, D, eps,
+                      (cudaStream_t)stream);
+}
+
+dit_status dit_gemv(int32_t dtype, const float* in, const void* W, const void* b, float* out, int32_t R, int32_t N,
+                    int32_t K, int32_t silu_input, void* stream) {
+  DIT_REQUIRE(dtype == DIT_F32 || dtype == DIT_BF16, DIT_ERR_INVALID_ARG, "dtype %d", dtype);
+  DIT_REQUIRE(R >= 1 && N >= 1 && K >= 8 && in && W && out, DIT_ERR_INVALID_ARG, "bad GEMV arguments");
+  // the batch descriptor travels as a tiny device allocation owned by this call's stream order
+  GemvBatch tb = {W, b, N, 0, 0, 0};
+  GemvBatch* dev = nullptr;
+  DIT_CUDA_OK(cudaMallocAsync((void**)&dev, sizeof(GemvBatch), (cudaStream_t)stream));
+  DIT_CUDA_OK(cudaMemcpyAsync(dev, &tb, sizeof(tb), cudaMemcpyHostToDevice, (cudaStream_t)stream));
+  dit_status s = launch_gemv(dtype, in, dev, 1, N, out, N, R, K, silu_input, (cudaStream_t)stream);
+  cudaFreeAsync(dev, (cudaStream_t)stream);
+  return s;
+}
+
+dit_status dit_qknorm_rope(int32_t dtype, void* qkv, int64_t row_stride, int32_t T, int32_t n_heads, int32_t head_dim,
+                           int32_t n_tensors, const void* gq, const void* gk, float eps, const float* rope_cos,
+                           const float* rope_sin, void* stream) {
+  DIT_REQUIRE(dtype == DIT_F32 || dtype == DIT_BF16, DIT_ERR_INVALID_ARG, "dtype %d", dtype);
+  DIT_REQUIRE(n_tensors == 1 || n_tensors == 2, DIT_ERR_INVALID_ARG, "n_tensors %d", n_tensors);
+  DIT_REQUIRE((rope_cos == nullptr) == (rope_sin == nullptr), DIT_ERR_INVALID_ARG, "rope_cos / rope_sin must both be given");
+  DIT_REQUIRE(T == 0 || qkv, DIT_ERR_INVALID_ARG, "qkv is NULL");
+  return launch_qknorm_rope(dtype, qkv, row_stride, T, n_heads, head_dim, n_tensors, gq, gk, eps, rope_cos, rope_sin,
+                            (cudaStream_t)stream);
+}
+
+dit_status dit_debug_stop_after(dit_handle h, int32_t block, int32_t stage) {
+  DIT_REQUIRE(h != nullptr, DIT_ERR_INVALID_ARG, "handle is NULL");
+  h->stop_block = block;
+  h->stop_stage = block < 0 ? -1 : stage;
+  return DIT_OK;
+}
+
+dit_status dit_get_tap(dit_handle h, int32_t tap, void* dst, size_t bytes, void* stream) {
+  DIT_REQUIRE(h != nullptr && dst != nullptr, DIT_ERR_INVALID_ARG, "NULL argument");
+  const Workspace& w = h->ws;
+  const void* src = nullptr;
+  switch (tap) {
+    case DIT_TAP_X: src = w.x; break;
+    case DIT_TAP_Y: src = w.y; break;
+    case DIT_TAP_QKV: src = w.qkv; break;
+    case DIT_TAP_O: src = w.o; break;
+    case DIT_TAP_H: src = w.h; break;
+    case DIT_TAP_U: src = w.u; break;
+    case DIT_TAP_C: src = w.c; break;
+    case DIT_TAP_MOD: src = w.mod; break;
+    case DIT_TAP_TOK: src = w.tok; break;
+    default: DIT_REQUIRE(false, DIT_ERR_INVALID_ARG, "unknown tap %d", tap);
+  }
+  DIT_CUDA_OK(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+  return DIT_OK;
+}
+
+const char* dit_last_error(dit_handle) { return get_error(); }
+int32_t dit_kernel_launches(void) { return g_launches; }
+
+void dit_free(dit_handle h) {
+  if (!h) return;
+  delete[] h->blocks;
+  delete h;
+}
+
+}  // extern "C"

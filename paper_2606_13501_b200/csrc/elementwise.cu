@@ -1,0 +1,467 @@
+// elementwise.cu — the HBM-bound kernels of the DiT step: weight-streaming GEMV (t-MLP, modulation),
+// adaLN-Zero modulation (LayerNorm + shift/scale + gated residual), QK-RMSNorm + RoPE, RoPE tables,
+// patchify / unpatchify, LSE merge.  All 128-bit coalesced global access, warp-shuffle reductions.
+#include "common.cuh"
+
+namespace dit {
+
+// =================================================================================================
+// GEMV:  out[r, off_b + n] = sum_k act(in[r,k]) W_b[n,k] + bias_b[n]      (DESIGN.md §3 steps 1-2)
+// Roofline: HBM, weights are streamed exactly once (N*K*sizeof(T) bytes); `in` lives in shared memory.
+// A warp owns 4 weight rows at a time so every staged input fragment is reused 4x from registers
+// (keeps shared-memory traffic at R/2 bytes per weight byte) and has 4+ independent 16-byte loads in flight.
+// =================================================================================================
+template <typename T, int RMAX>
+__global__ void __launch_bounds__(256) gemv_kernel(const float* __restrict__ in, const GemvBatch* __restrict__ batches,
+                                                   int n_batches, int total_rows, float* __restrict__ out,
+                                                   int64_t out_stride, int R, int K, int silu_input) {
+  extern __shared__ float s_in[];  // [R][K]
+  for (int i = threadIdx.x; i < R * K; i += blockDim.x) {
+    float v = in[i];
+    s_in[i] = silu_input ? silu_f(v) : v;
+  }
+  __syncthreads();
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int warps_total = gridDim.x * (blockDim.x >> 5);
+  const int n_groups = (total_rows + 3) >> 2;
+  for (int g = blockIdx.x * (blockDim.x >> 5) + warp; g < n_groups; g += warps_total) {
+    const T* wrow[4];
+    bool valid[4];
+    int bidx[4], nloc[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      int row = g * 4 + j;
+      valid[j] = row < total_rows;
+      if (!valid[j]) row = total_rows - 1;
+      int b = 0;
+      while (b + 1 < n_batches && row >= batches[b + 1].row_begin) ++b;
+      bidx[j] = b;
+      nloc[j] = row - batches[b].row_begin;
+      wrow[j] = reinterpret_cast<const T*>(batches[b].W) + (int64_t)nloc[j] * K;
+    }
+    float acc[4][RMAX];
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+#pragma unroll
+      for (int r = 0; r < RMAX; ++r) acc[j][r] = 0.f;
+    for (int k0 = lane * 8; k0 < K; k0 += 256) {
+      float w[4][8];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) ld8<T>(wrow[j] + k0, w[j]);
+#pragma unroll
+      for (int r = 0; r < RMAX; ++r) {
+        if (r < R) {
+          float xin[8];
+          ld8<float>(s_in + r * K + k0, xin);
+#pragma unroll
+          for (int j = 0; j < 4; ++j)
+#pragma unroll
+            for (int e = 0; e < 8; ++e) acc[j][r] = fmaf(w[j][e], xin[e], acc[j][r]);
+        }
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+#pragma unroll
+      for (int r = 0; r < RMAX; ++r) acc[j][r] = warp_sum(acc[j][r]);
+    if (lane == 0) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        if (!valid[j]) continue;
+        const GemvBatch& B = batches[bidx[j]];
+        float bias = B.b ? to_f<T>(reinterpret_cast<const T*>(B.b)[nloc[j]]) : 0.f;
+#pragma unroll
+        for (int r = 0; r < RMAX; ++r)
+          if (r < R) out[(int64_t)r * out_stride + B.out_off + nloc[j]] = acc[j][r] + bias;
+      }
+    }
+  }
+}
+
+template <typename T>
+static dit_status launch_gemv_t(const float* in, const GemvBatch* batches, int n_batches, int total_rows, float* out,
+                                int64_t out_stride, int R, int K, int silu_input, cudaStream_t st) {
+  DIT_REQUIRE(K % 8 == 0, DIT_ERR_UNSUPPORTED, "gemv: K=%d must be a multiple of 8", K);
+  int dev = 0, sms = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  // requests are processed RMAX at a time (weights re-streamed per chunk only when R > 8)
+  for (int r0 = 0; r0 < R; r0 += 8) {
+    int rc = R - r0 < 8 ? R - r0 : 8;
+    size_t smem = (size_t)rc * K * sizeof(float);
+    int groups = (total_rows + 3) / 4;
+    int ctas = (groups + 7) / 8;
+    int per_sm = smem > 100 * 1024 ? 1 : 2;
+    if (ctas > sms * per_sm) ctas = sms * per_sm;
+    const float* inr = in + (int64_t)r0 * K;
+    float* outr = out + (int64_t)r0 * out_stride;
+#define GEMV_LAUNCH(RM)                                                                                         \
+  {                                                                                                             \
+    DIT_CUDA_OK(cudaFuncSetAttribute(gemv_kernel<T, RM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+    gemv_kernel<T, RM><<<ctas, 256, smem, st>>>(inr, batches, n_batches, total_rows, outr, out_stride, rc, K,   \
+                                                silu_input);                                                    \
+  }
+    DIT_REQUIRE(smem <= 200 * 1024, DIT_ERR_UNSUPPORTED, "gemv: R*K too large for shared memory");
+    if (rc == 1) GEMV_LAUNCH(1) else if (rc == 2) GEMV_LAUNCH(2) else if (rc <= 4) GEMV_LAUNCH(4) else GEMV_LAUNCH(8)
+#undef GEMV_LAUNCH
+    DIT_LAUNCH_CHECK();
+  }
+  return DIT_OK;
+}
+
+dit_status launch_gemv(int dtype, const float* in, const GemvBatch* batches_dev, int n_batches, int total_rows,
+                       float* out, int64_t out_stride, int R, int K, int silu_input, cudaStream_t st) {
+  if (dtype == DIT_F32)
+    return launch_gemv_t<float>(in, batches_dev, n_batches, total_rows, out, out_stride, R, K, silu_input, st);
+  return launch_gemv_t<bf16>(in, batches_dev, n_batches, total_rows, out, out_stride, R, K, silu_input, st);
+}
+
+// =================================================================================================
+// adaLN-Zero modulation (north_star subsystem 2; DESIGN.md §3 step 5):
+//   x <- x + gate (.) h   (optional);   y = LN(x) (.) (1 + scale) + shift
+// One warp per row, the whole row in registers (NC chunks of 8 elements per lane), two-pass statistics with
+// warp shuffles only.  Algorithmic bytes per token: 4D (x) + 2D (y) [+ 2D (h) + 4D (x write)].
+// =================================================================================================
+template <typename T, int NC>
+__global__ void __launch_bounds__(128) adaln_kernel(float* __restrict__ x, const T* __restrict__ h,
+                                                    const float* __restrict__ gate, const float* __restrict__ shift,
+                                                    const float* __restrict__ scale, int64_t mod_stride,
+                                                    const int32_t* __restrict__ cu, int R, T* __restrict__ y, int T_rows,
+                                                    float eps) {
+  constexpr int D = NC * 256;
+  const int lane = threadIdx.x & 31;
+  const int row = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (row >= T_rows) return;
+  const int req = (cu != nullptr && R > 1) ? find_request(cu, R, row) : 0;
+  float* xr = x + (int64_t)row * D;
+  float v[NC][8];
+#pragma unroll
+  for (int c = 0; c < NC; ++c) ld8<float>(xr + (c * 32 + lane) * 8, v[c]);
+  if (h != nullptr) {
+    const T* hr = h + (int64_t)row * D;
+    const float* g = gate ? gate + (int64_t)req * mod_stride : nullptr;
+#pragma unroll
+    for (int c = 0; c < NC; ++c) {
+      float hv[8], gv[8];
+      ld8<T>(hr + (c * 32 + lane) * 8, hv);
+      if (g) ld8<float>(g + (c * 32 + lane) * 8, gv);
+#pragma unroll
+      for (int e = 0; e < 8; ++e) v[c][e] = g ? fmaf(gv[e], hv[e], v[c][e]) : v[c][e] + hv[e];
+      st8<float>(xr + (c * 32 + lane) * 8, v[c]);
+    }
+  }
+  float s = 0.f;
+#pragma unroll
+  for (int c = 0; c < NC; ++c)
+#pragma unroll
+    for (int e = 0; e < 8; ++e) s += v[c][e];
+  const float mean = warp_sum(s) * (1.0f / D);
+  float q = 0.f;
+#pragma unroll
+  for (int c = 0; c < NC; ++c)
+#pragma unroll
+    for (int e = 0; e < 8; ++e) {
+      float dlt = v[c][e] - mean;
+      q = fmaf(dlt, dlt, q);
+    }
+  const float rstd = rsqrtf(warp_sum(q) * (1.0f / D) + eps);
+  const float* sh = shift ? shift + (int64_t)req * mod_stride : nullptr;
+  const float* sc = scale ? scale + (int64_t)req * mod_stride : nullptr;
+  T* yr = y + (int64_t)row * D;
+#pragma unroll
+  for (int c = 0; c < NC; ++c) {
+    float o[8], a[8], b[8];
+    if (sc) ld8<float>(sc + (c * 32 + lane) * 8, a);
+    if (sh) ld8<float>(sh + (c * 32 + lane) * 8, b);
+#pragma unroll
+    for (int e = 0; e < 8; ++e) {
+      float n = (v[c][e] - mean) * rstd;
+      if (sc) n = fmaf(n, a[e], n);
+      if (sh) n += b[e];
+      o[e] = n;
+    }
+    st8<T>(yr + (c * 32 + lane) * 8, o);
+  }
+}
+
+template <typename T>
+static dit_status launch_adaln_t(float* x, const T* h, const float* gate, const float* shift, const float* scale,
+                                 int64_t mod_stride, const int32_t* cu, int R, T* y, int T_rows, int D, float eps,
+                                 cudaStream_t st) {
+  if (T_rows == 0) return DIT_OK;
+  DIT_REQUIRE(D % 256 == 0 && D <= 6144, DIT_ERR_UNSUPPORTED, "adaln: D=%d must be a multiple of 256 (<= 6144)", D);
+  const int grid = cdiv(T_rows, 4);
+#define ADALN_CASE(NCV)                                                                                     \
+  case NCV:                                                                                                 \
+    adaln_kernel<T, NCV><<<grid, 128, 0, st>>>(x, h, gate, shift, scale, mod_stride, cu, R, y, T_rows, eps); \
+    break;
+  switch (D / 256) {
+    ADALN_CASE(1) ADALN_CASE(2) ADALN_CASE(3) ADALN_CASE(4) ADALN_CASE(5) ADALN_CASE(6) ADALN_CASE(8) ADALN_CASE(10)
+    ADALN_CASE(12) ADALN_CASE(16) ADALN_CASE(20) ADALN_CASE(24)
+    default:
+      DIT_REQUIRE(false, DIT_ERR_UNSUPPORTED, "adaln: D=%d has no instantiation", D);
+  }
+#undef ADALN_CASE
+  DIT_LAUNCH_CHECK();
+  return DIT_OK;
+}
+
+dit_status launch_adaln(int dtype, float* x, const void* h, const float* gate, const float* shift, const float* scale,
+                        int64_t mod_stride, const int32_t* cu, int R, void* y, int T, int D, float eps, cudaStream_t st) {
+  if (dtype == DIT_F32)
+    return launch_adaln_t<float>(x, (const float*)h, gate, shift, scale, mod_stride, cu, R, (float*)y, T, D, eps, st);
+  return launch_adaln_t<bf16>(x, (const bf16*)h, gate, shift, scale, mod_stride, cu, R, (bf16*)y, T, D, eps, st);
+}
+
+// =================================================================================================
+// QK-RMSNorm + RoPE, in place on the q and k thirds of qkv[T, 3D] (R5, R6).  d/8 lanes own one head row.
+// =================================================================================================
+template <typename T, int HD>
+__global__ void __launch_bounds__(256) qknorm_rope_kernel(T* __restrict__ qkv, int64_t row_stride, int T_rows, int H,
+                                                          int n_tensors, const T* __restrict__ gq,
+                                                          const T* __restrict__ gk, float eps,
+                                                          const float* __restrict__ rc, const float* __restrict__ rs) {
+  constexpr int LPH = HD / 8;           // lanes per head row
+  constexpr int HPW = 32 / LPH;         // head rows per warp pass
+  const int lane = threadIdx.x & 31;
+  const int sub = lane / LPH, li = lane % LPH;
+  const int D = H * HD;
+  const int64_t heads_total = (int64_t)T_rows * n_tensors * H;
+  const int64_t warp_id = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  const int64_t n_warps = (int64_t)gridDim.x * (blockDim.x >> 5);
+  for (int64_t base = warp_id * HPW; base < heads_total; base += n_warps * HPW) {
+    const int64_t item = base + sub;
+    const bool ok = item < heads_total;
+    const int64_t it = ok ? item : heads_total - 1;
+    const int head = (int)(it % H);
+    const int which = (int)((it / H) % n_tensors);
+    const int row = (int)(it / ((int64_t)H * n_tensors));
+    T* p = qkv + (int64_t)row * row_stride + (int64_t)which * D + head * HD + li * 8;
+    float v[8];
+    ld8<T>(p, v);
+    const T* g = which == 0 ? gq : gk;
+    if (g != nullptr) {
+      float ss = 0.f;
+#pragma unroll
+      for (int e = 0; e < 8; ++e) ss = fmaf(v[e], v[e], ss);
+#pragma unroll
+      for (int o = LPH / 2; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
+      const float r = rsqrtf(ss * (1.0f / HD) + eps);
+      float gv[8];
+      ld8<T>(g + li * 8, gv);
+#pragma unroll
+      for (int e = 0; e < 8; ++e) v[e] = v[e] * r * gv[e];
+    }
+    if (rc != nullptr) {
+      const float4 c = *reinterpret_cast<const float4*>(rc + (int64_t)row * (HD / 2) + li * 4);
+      const float4 s = *reinterpret_cast<const float4*>(rs + (int64_t)row * (HD / 2) + li * 4);
+      const float cc[4] = {c.x, c.y, c.z, c.w}, sn[4] = {s.x, s.y, s.z, s.w};
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const float a = v[2 * j], b = v[2 * j + 1];
+        v[2 * j] = a * cc[j] - b * sn[j];
+        v[2 * j + 1] = a * sn[j] + b * cc[j];
+      }
+    }
+    if (ok) st8<T>(p, v);
+  }
+}
+
+dit_status launch_qknorm_rope(int dtype, void* qkv, int64_t row_stride, int T, int H, int d, int n_tensors,
+                              const void* gq, const void* gk, float eps, const float* rc, const float* rs,
+                              cudaStream_t st) {
+  if (T == 0 || (gq == nullptr && gk == nullptr && rc == nullptr)) return DIT_OK;
+  DIT_REQUIRE(d == 64 || d == 128, DIT_ERR_UNSUPPORTED, "qknorm_rope: head_dim %d not in {64,128}", d);
+  int64_t heads = (int64_t)T * n_tensors * H;
+  int hpw = 32 / (d / 8);
+  int64_t warps = (heads + hpw - 1) / hpw;
+  int grid = (int)((warps + 7) / 8);
+  if (grid > 148 * 16) grid = 148 * 16;
+#define QK_LAUNCH(TT, HDV)                                                                                      \
+  qknorm_rope_kernel<TT, HDV><<<grid, 256, 0, st>>>((TT*)qkv, row_stride, T, H, n_tensors, (const TT*)gq,       \
+                                                    (const TT*)gk, eps, rc, rs)
+  if (dtype == DIT_F32) {
+    if (d == 64) QK_LAUNCH(float, 64); else QK_LAUNCH(float, 128);
+  } else {
+    if (d == 64) QK_LAUNCH(bf16, 64); else QK_LAUNCH(bf16, 128);
+  }
+#undef QK_LAUNCH
+  DIT_LAUNCH_CHECK();
+  return DIT_OK;
+}
+
+// =================================================================================================
+// RoPE tables (R6): cos/sin[t, j] for the pair j of token t; angles in double.
+// =================================================================================================
+__global__ void rope_table_kernel(const SeqMeta* __restrict__ meta, int R, int T_rows, int half, int d0, int d1, int d2,
+                                  double log2_theta, float* __restrict__ rc, float* __restrict__ rs) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (int64_t)T_rows * half) return;
+  const int t = (int)(idx / half), j = (int)(idx % half);
+  int r = 0;
+  while (r + 1 < R && t >= meta[r + 1].seq_start) ++r;
+  const SeqMeta m = meta[r];
+  const int n = t - m.seq_start - m.n_cond;
+  int pos[3] = {0, 0, 0};
+  if (n >= 0) {
+    pos[2] = n % m.gw;
+    pos[1] = (n / m.gw) % m.gh;
+    pos[0] = n / (m.gw * m.gh);
+  }
+  int axis, jj, da;
+  if (j < d0 / 2) { axis = 0; jj = j; da = d0; }
+  else if (j < (d0 + d1) / 2) { axis = 1; jj = j - d0 / 2; da = d1; }
+  else { axis = 2; jj = j - (d0 + d1) / 2; da = d2; }
+  const double omega = exp2(-2.0 * (double)jj / (double)da * log2_theta);
+  const double ang = (double)pos[axis] * omega;
+  double s, c;
+  sincos(ang, &s, &c);
+  rc[idx] = (float)c;
+  rs[idx] = (float)s;
+}
+
+dit_status launch_rope_table(const SeqMeta* meta, int R, int T, int d, const int32_t rope_dims[3], float theta,
+                             float* rc, float* rs, cudaStream_t st) {
+  if (T == 0) return DIT_OK;
+  const int half = d / 2;
+  const int64_t n = (int64_t)T * half;
+  rope_table_kernel<<<cdiv(n, 256), 256, 0, st>>>(meta, R, T, half, rope_dims[0], rope_dims[1], rope_dims[2],
+                                                 log2((double)theta), rc, rs);
+  DIT_LAUNCH_CHECK();
+  return DIT_OK;
+}
+
+// =================================================================================================
+// patchify (im2col, DESIGN.md §3 step 3 / R11) and unpatchify (step 6)
+// =================================================================================================
+template <typename T>
+__global__ void patchify_kernel(const T* __restrict__ lat, T* __restrict__ patches, int C, int F, int H, int W, int pf,
+                                int ph, int pw) {
+  const int Fp = F / pf, Hp = H / ph, Wp = W / pw, pv = pf * ph * pw;
+  const int64_t total = (int64_t)Fp * Hp * Wp * C * pv;
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= total) return;
+  const int feat = (int)(idx % (C * pv));
+  const int n = (int)(idx / (C * pv));
+  const int k = feat % pw, j = (feat / pw) % ph, i = (feat / (pw * ph)) % pf, c = feat / pv;
+  const int w_ = n % Wp, h_ = (n / Wp) % Hp, f_ = n / (Wp * Hp);
+  patches[idx] = lat[(((int64_t)c * F + f_ * pf + i) * H + h_ * ph + j) * W + w_ * pw + k];
+}
+
+template <typename T>
+__global__ void unpatchify_kernel(const float* __restrict__ tok, T* __restrict__ out, int C, int F, int H, int W,
+                                  int pf, int ph, int pw) {
+  const int Hp = H / ph, Wp = W / pw, pv = pf * ph * pw;
+  const int64_t total = (int64_t)C * F * H * W;
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= total) return;
+  const int w = (int)(idx % W), hh = (int)((idx / W) % H), f = (int)((idx / ((int64_t)W * H)) % F);
+  const int c = (int)(idx / ((int64_t)W * H * F));
+  const int n = ((f / pf) * Hp + hh / ph) * Wp + w / pw;
+  const int feat = ((c * pf + f % pf) * ph + hh % ph) * pw + w % pw;
+  out[idx] = from_f<T>(tok[(int64_t)n * (C * pv) + feat]);
+}
+
+dit_status launch_patchify(int dtype, const void* lat, void* patches, int C, int F, int H, int W, const int32_t patch[3],
+                           cudaStream_t st) {
+  const int64_t total = (int64_t)C * F * H * W;
+  if (total == 0) return DIT_OK;
+  if (dtype == DIT_F32)
+    patchify_kernel<float><<<cdiv(total, 256), 256, 0, st>>>((const float*)lat, (float*)patches, C, F, H, W, patch[0],
+                                                            patch[1], patch[2]);
+  else
+    patchify_kernel<bf16><<<cdiv(total, 256), 256, 0, st>>>((const bf16*)lat, (bf16*)patches, C, F, H, W, patch[0],
+                                                           patch[1], patch[2]);
+  DIT_LAUNCH_CHECK();
+  return DIT_OK;
+}
+
+dit_status launch_unpatchify(int dtype, const float* tok, void* out, int C, int F, int H, int W, const int32_t patch[3],
+                             cudaStream_t st) {
+  const int64_t total = (int64_t)C * F * H * W;
+  if (total == 0) return DIT_OK;
+  if (dtype == DIT_F32)
+    unpatchify_kernel<float><<<cdiv(total, 256), 256, 0, st>>>(tok, (float*)out, C, F, H, W, patch[0], patch[1], patch[2]);
+  else
+    unpatchify_kernel<bf16><<<cdiv(total, 256), 256, 0, st>>>(tok, (bf16*)out, C, F, H, W, patch[0], patch[1], patch[2]);
+  DIT_LAUNCH_CHECK();
+  return DIT_OK;
+}
+
+// =================================================================================================
+// LSE merge (north_star subsystem 5; R18):  lse = ln sum_p e^{lse_p};  o = sum_p e^{lse_p - lse} o_p
+// One thread per 8 output elements; bytes = P (rows*d*sizeof(T) + rows*4) + rows*d*sizeof(T) (+ rows*4).
+// =================================================================================================
+struct MergePtrs {
+  const void* o[8];
+  const float* lse[8];
+};
+
+template <typename T, int P>
+__global__ void __launch_bounds__(256) merge_kernel(MergePtrs ptrs, int64_t n_rh, int d, T* __restrict__ o,
+                                                    float* __restrict__ lse_out) {
+  const int cpr = d / 8;  // 8-element chunks per (row, head)
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= n_rh * cpr) return;
+  const int64_t rh = idx / cpr;
+  float l[P], m = -INFINITY;
+#pragma unroll
+  for (int p = 0; p < P; ++p) {
+    l[p] = ptrs.lse[p][rh];
+    m = fmaxf(m, l[p]);
+  }
+  const float ms = (m == -INFINITY) ? 0.f : m;
+  float z = 0.f, w[P];
+#pragma unroll
+  for (int p = 0; p < P; ++p) {
+    w[p] = expf(l[p] - ms);
+    z += w[p];
+  }
+  const float inv = z > 0.f ? 1.0f / z : 0.f;
+  float acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+#pragma unroll
+  for (int p = 0; p < P; ++p) {
+    float v[8];
+    ld8<T>(reinterpret_cast<const T*>(ptrs.o[p]) + idx * 8, v);
+    const float wp = w[p] * inv;
+#pragma unroll
+    for (int e = 0; e < 8; ++e) acc[e] = fmaf(wp, v[e], acc[e]);
+  }
+  st8<T>(o + idx * 8, acc);
+  if (lse_out != nullptr && idx % cpr == 0) lse_out[rh] = ms + logf(z);
+}
+
+template <typename T>
+static dit_status launch_merge_t(const MergePtrs& ptrs, int P, int64_t n_rh, int d, T* o, float* lse_out,
+                                 cudaStream_t st) {
+  const int64_t n = n_rh * (d / 8);
+  const int grid = cdiv(n, 256);
+  switch (P) {
+    case 1: merge_kernel<T, 1><<<grid, 256, 0, st>>>(ptrs, n_rh, d, o, lse_out); break;
+    case 2: merge_kernel<T, 2><<<grid, 256, 0, st>>>(ptrs, n_rh, d, o, lse_out); break;
+    case 3: merge_kernel<T, 3><<<grid, 256, 0, st>>>(ptrs, n_rh, d, o, lse_out); break;
+    case 4: merge_kernel<T, 4><<<grid, 256, 0, st>>>(ptrs, n_rh, d, o, lse_out); break;
+    case 5: merge_kernel<T, 5><<<grid, 256, 0, st>>>(ptrs, n_rh, d, o, lse_out); break;
+    case 6: merge_kernel<T, 6><<<grid, 256, 0, st>>>(ptrs, n_rh, d, o, lse_out); break;
+    case 7: merge_kernel<T, 7><<<grid, 256, 0, st>>>(ptrs, n_rh, d, o, lse_out); break;
+    default: merge_kernel<T, 8><<<grid, 256, 0, st>>>(ptrs, n_rh, d, o, lse_out); break;
+  }
+  DIT_LAUNCH_CHECK();
+  return DIT_OK;
+}
+
+dit_status launch_merge(int dtype, const void* const* o_parts, const float* const* lses, int P, int64_t n_rh, int d,
+                        void* o, float* lse_out, cudaStream_t st) {
+  if (n_rh == 0) return DIT_OK;
+  DIT_REQUIRE(P >= 1 && P <= 8, DIT_ERR_INVALID_ARG, "merge: P=%d not in 1..8", P);
+  DIT_REQUIRE(d % 8 == 0, DIT_ERR_UNSUPPORTED, "merge: head_dim %d must be a multiple of 8", d);
+  MergePtrs ptrs;
+  for (int p = 0; p < 8; ++p) {
+    ptrs.o[p] = o_parts[p < P ? p : 0];
+    ptrs.lse[p] = lses[p < P ? p : 0];
+  }
+  if (dtype == DIT_F32) return launch_merge_t<float>(ptrs, P, n_rh, d, (float*)o, lse_out, st);
+  return launch_merge_t<bf16>(ptrs, P, n_rh, d, (bf16*)o, lse_out, st);
+}
+
+}  // namespace dit

@@ -1,0 +1,236 @@
+"""GPU parity, kernel level: each C-ABI building block of the step against the CPU oracle on the same
+seeded inputs, element by element (sizes span several tiles and a ragged tail; edge cases included)."""
+import math
+
+import pytest
+import torch
+
+from oracle import dit_oracle as O
+from paper_2606_13501_b200 import binding as B
+from paper_2606_13501_b200 import synth
+from util import check, errors
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda:0"
+DTYPES = [torch.float32, torch.bfloat16]
+
+
+def rnd(name, shape, dtype, std=1.0, mean=0.0, seed=3):
+    return synth.normal(seed, name, shape, std=std, mean=mean, dtype=dtype, device=DEV)
+
+
+# ------------------------------------------------------------------------------ GEMV (t-MLP, modulation)
+@pytest.mark.parametrize("dtype", DTYPES)
+@pytest.mark.parametrize("R,N,K,silu", [(1, 256, 256, False), (1, 1030, 3072, True), (3, 517, 512, True),
+                                         (6, 96, 1024, True), (8, 40, 256, False)])
+def test_gemv(lib, dtype, R, N, K, silu):
+    x = rnd("in", (R, K), torch.float32)
+    W, b = rnd("W", (N, K), dtype, std=0.05), rnd("b", (N,), dtype, std=0.05)
+    got = B.dit_gemv(x, W, b, silu_input=silu)
+    xin = x.double().cpu()
+    ref = O.linear(O.silu(xin) if silu else xin, W.cpu(), b.cpu())
+    check(got, ref, torch.float32, f"gemv {dtype}", rel=2e-6, maxabs=2e-5)
+
+
+# ------------------------------------------------------------------------------ adaLN
+@pytest.mark.parametrize("dtype", DTYPES)
+@pytest.mark.parametrize("T,D", [(1, 256), (37, 256), (301, 3072), (130, 5120), (66, 1024)])
+@pytest.mark.parametrize("fused", [False, True])
+def test_adaln(lib, dtype, T, D, fused):
+    x = rnd("x", (T, D), torch.float32, std=2.0, mean=0.3)
+    mod = rnd("mod", (1, 3 * D), torch.float32, std=0.3)
+    h = rnd("h", (T, D), dtype) if fused else None
+    xg = x.clone()
+    y = B.dit_adaln(xg, dtype, h=h, gate=mod[:, 2 * D:] if fused else None, shift=mod[:, :D], scale=mod[:, D:2 * D],
+                    mod_stride=3 * D)
+    xr = x.double().cpu()
+    m = mod.double().cpu()[0]
+    if fused:
+        xr = xr + m[2 * D:] * h.double().cpu()
+        check(xg, xr, torch.float32, "adaln x update", rel=1e-6, maxabs=1e-5)
+    else:
+        assert torch.equal(xg, x)
+    ref = O.modulate(xr, m[:D], m[D:2 * D], 1e-6)
+    tol = dict(rel=2e-6, maxabs=2e-5) if dtype == torch.float32 else dict(rel=3e-3, maxabs=2e-2)
+    check(y, ref, dtype, "adaln y", **tol)
+
+
+@pytest.mark.parametrize("dtype", DTYPES)
+def test_adaln_varlen_requests_and_null_modulation(lib, dtype):
+    T, D, R = 75, 512, 3
+    cu = torch.tensor([0, 20, 21, 75], dtype=torch.int32, device=DEV)
+    x = rnd("x", (T, D), torch.float32)
+    mod = rnd("mod", (R, 2 * D), torch.float32, std=0.3)
+    y = B.dit_adaln(x, dtype, shift=mod[:, :D], scale=mod[:, D:], mod_stride=2 * D, cu_seqlens=cu, n_requests=R)
+    m = mod.double().cpu()
+    req = torch.tensor([0] * 20 + [1] + [2] * 54)
+    ref = O.layer_norm(x.double().cpu(), 1e-6) * (1 + m[req][:, D:]) + m[req][:, :D]
+    tol = dict(rel=2e-6, maxabs=2e-5) if dtype == torch.float32 else dict(rel=3e-3, maxabs=2e-2)
+    check(y, ref, dtype, "adaln varlen", **tol)
+    # NULL shift/scale = plain LN; NULL gate = 1
+    h = rnd("h", (T, D), dtype)
+    x2 = x.clone()
+    y2 = B.dit_adaln(x2, dtype, h=h)
+    xr = x.double().cpu() + h.double().cpu()
+    check(x2, xr, torch.float32, "ungated residual", rel=1e-6, maxabs=1e-5)
+    check(y2, O.layer_norm(xr, 1e-6), dtype, "plain LN", **tol)
+    # constant rows => y = shift (degenerate variance)
+    xc = torch.full((4, D), 3.25, device=DEV)
+    yc = B.dit_adaln(xc, dtype, shift=mod[:1, :D], scale=mod[:1, D:], mod_stride=2 * D)
+    check(yc, m[0, :D].expand(4, D), dtype, "constant row", **tol)
+
+
+# ------------------------------------------------------------------------------ QK-RMSNorm + RoPE
+@pytest.mark.parametrize("dtype", DTYPES)
+@pytest.mark.parametrize("T,H,d", [(33, 4, 64), (130, 24, 128), (7, 3, 128)])
+@pytest.mark.parametrize("norm,rope", [(True, True), (True, False), (False, True)])
+def test_qknorm_rope(lib, dtype, T, H, d, norm, rope):
+    D = H * d
+    qkv = rnd("qkv", (T, 3 * D), dtype)
+    gq, gk = rnd("gq", (d,), dtype, std=0.1, mean=1.0), rnd("gk", (d,), dtype, std=0.1, mean=1.0)
+    pos = torch.stack([torch.arange(T) % 3, torch.arange(T) % 5, torch.arange(T) // 5], 1)
+    dims = (d // 4, d // 4, d // 2)
+    ang = O.rope_angles(pos, dims, 10000.0)
+    rc, rs = torch.cos(ang).float().to(DEV), torch.sin(ang).float().to(DEV)
+    ref = qkv.double().cpu().reshape(T, 3, H, d)
+    q, k = ref[:, 0], ref[:, 1]
+    if norm:
+        q, k = O.rms_norm_heads(q, gq.double().cpu(), 1e-6), O.rms_norm_heads(k, gk.double().cpu(), 1e-6)
+    if rope:
+        a = torch.atan2(rs.double().cpu(), rc.double().cpu())  # the fp32 table the kernel is given
+        q, k = O.apply_rope(q, a), O.apply_rope(k, a)
+    ref = torch.stack([q, k, ref[:, 2]], 1).reshape(T, 3 * D)
+    got = qkv.clone()
+    B.dit_qknorm_rope(got, H, d, 2, gq if norm else None, gk if norm else None, 1e-6, rc if rope else None,
+                      rs if rope else None)
+    tol = dict(rel=2e-6, maxabs=2e-5) if dtype == torch.float32 else dict(rel=3e-3, maxabs=2e-2)
+    check(got, ref, dtype, "qknorm_rope", **tol)
+    assert torch.equal(got[:, 2 * D:], qkv[:, 2 * D:])          # v untouched
+
+
+# ------------------------------------------------------------------------------ Linear (GEMM + epilogues)
+GEMM_SHAPES = [(1, 64, 64), (100, 72, 16), (288, 768, 256), (257, 1024, 320), (130, 3072, 64), (515, 200, 1032),
+               (1000, 256, 4096)]
+
+
+@pytest.mark.parametrize("dtype", DTYPES)
+@pytest.mark.parametrize("M,N,K", GEMM_SHAPES)
+@pytest.mark.parametrize("epi", [B.EPI_BIAS, B.EPI_BIAS_GELU, B.EPI_BIAS_F32])
+def test_linear(lib, dtype, M, N, K, epi):
+    if dtype == torch.float32 and epi == B.EPI_BIAS_F32:
+        pytest.skip("fp32 output is the fp32 path's only output type")
+    A = rnd("A", (M, K), dtype)
+    W, b = rnd("W", (N, K), dtype, std=1.0 / math.sqrt(K)), rnd("b", (N,), dtype, std=0.5)
+    got = B.dit_linear(A, W, b, epi)
+    ref = O.linear(A.double().cpu(), W.cpu(), b.cpu())
+    if epi == B.EPI_BIAS_GELU:
+        ref = O.gelu_tanh(ref)
+    odt = torch.float32 if (epi == B.EPI_BIAS_F32 or dtype == torch.float32) else torch.bfloat16
+    assert got.dtype == odt
+    tol = dict(rel=2e-6, maxabs=3e-5) if odt == torch.float32 else dict(rel=3e-3, maxabs=2e-2)
+    check(got, ref, odt, f"linear {M}x{N}x{K} epi{epi}", **tol)
+
+
+@pytest.mark.parametrize("dtype", DTYPES)
+def test_linear_strided_views_and_no_bias(lib, dtype):
+    """A and out are column slices of wider buffers (the step's qkv / packed layouts)."""
+    M, N, K = 300, 384, 512
+    big = rnd("A", (M, 3 * K), dtype)
+    A = big[:, K:2 * K]
+    W = rnd("W", (N, K), dtype, std=1.0 / math.sqrt(K))
+    outbig = torch.zeros((M, 2 * N), dtype=dtype, device=DEV)
+    B.dit_linear(A, W, None, B.EPI_BIAS, out=outbig[:, N:])
+    ref = O.linear(A.double().cpu(), W.cpu())
+    tol = dict(rel=2e-6, maxabs=3e-5) if dtype == torch.float32 else dict(rel=3e-3, maxabs=2e-2)
+    check(outbig[:, N:], ref, dtype, "strided linear", **tol)
+    assert (outbig[:, :N] == 0).all()
+    assert B.dit_linear(A[:0], W, None).shape == (0, N)
+
+
+# ------------------------------------------------------------------------------ attention partial + merge
+def _attn_tol(dtype):
+    return dict(rel=2e-6, maxabs=3e-5) if dtype == torch.float32 else dict(rel=4e-3, maxabs=2.5e-2)
+
+
+@pytest.mark.parametrize("dtype", DTYPES)
+@pytest.mark.parametrize("nq,nk,H,d", [(1, 1, 1, 64), (77, 133, 3, 64), (288, 288, 4, 64), (300, 515, 2, 128),
+                                        (128, 1024, 2, 128), (640, 257, 3, 128)])
+def test_attn_partial(lib, dtype, nq, nk, H, d):
+    q, k, v = synth.make_attention_qkv(11, nq, nk, H, d, dtype=dtype, device=DEV)
+    o, lse = B.dit_attn_partial(q, k, v)
+    ro, rl = O.attention(q.cpu(), k.cpu(), v.cpu())
+    check(o, ro, dtype, f"attn o {nq}x{nk}", **_attn_tol(dtype))
+    assert float((lse.double().cpu() - rl).abs().max()) < (1e-5 if dtype == torch.float32 else 2e-2)
+
+
+@pytest.mark.parametrize("dtype", DTYPES)
+def test_attn_peaky_and_identical_keys(lib, dtype):
+    """x4 logits (peaky softmax, R7/§8(c) sensitivity warning) and the 'identical keys => mean of V' invariant."""
+    nq, nk, H, d = 200, 333, 2, 128
+    q, k, v = synth.make_attention_qkv(11, nq, nk, H, d, dtype=dtype, device=DEV, logit_gain=4.0)
+    o, lse = B.dit_attn_partial(q, k, v)
+    ro, rl = O.attention(q.cpu(), k.cpu(), v.cpu())
+    check(o, ro, dtype, "peaky attention", **_attn_tol(dtype))
+    k1 = k[:1].expand(nk, H, d).contiguous()
+    o1, _ = B.dit_attn_partial(q, k1, v)
+    mean_v = v.double().cpu().mean(0, keepdim=True).expand(nq, H, d)
+    check(o1, mean_v, dtype, "identical keys", **_attn_tol(dtype))
+    ones = torch.ones_like(v)
+    o2, _ = B.dit_attn_partial(q, k, ones)                      # softmax rows sum to 1
+    assert float((o2.double().cpu() - 1).abs().max()) < (1e-5 if dtype == torch.float32 else 8e-3)
+
+
+@pytest.mark.parametrize("dtype", DTYPES)
+def test_attn_strided_qkv_buffer_and_empty(lib, dtype):
+    T, H, d = 150, 3, 64
+    D = H * d
+    qkv = rnd("qkv", (T, 3 * D), dtype)
+    q, k, v = (qkv[:, i * D:(i + 1) * D].view(T, H, d) for i in range(3))
+    o, lse = B.dit_attn_partial(q, k, v)
+    ro, rl = O.attention(q.cpu(), k.cpu(), v.cpu())
+    check(o, ro, dtype, "strided attention", **_attn_tol(dtype))
+    o0, l0 = B.dit_attn_partial(q, k[:0], v[:0])                # n_k = 0: o = 0, lse = -inf (R18)
+    assert (o0 == 0).all() and torch.isinf(l0).all() and (l0 < 0).all()
+    oe, le = B.dit_attn_partial(q[:0], k, v)
+    assert oe.shape == (0, H, d)
+
+
+@pytest.mark.parametrize("dtype", DTYPES)
+@pytest.mark.parametrize("P", [1, 2, 3, 4, 8])
+def test_split_kv_merge_reproduces_unsplit(lib, dtype, P):
+    nq, nk, H, d = 260, 1000, 2, 128
+    q, k, v = synth.make_attention_qkv(11, nq, nk, H, d, dtype=dtype, device=DEV)
+    parts = [B.dit_attn_partial(q, k[a:b], v[a:b]) for a, b in O.shard_bounds(nk, P)]
+    o, lse = B.dit_attn_merge([p[0] for p in parts], [p[1] for p in parts])
+    ro, rl = O.attention(q.cpu(), k.cpu(), v.cpu())
+    check(o, ro, dtype, f"split P={P}", **_attn_tol(dtype))
+    assert float((lse.double().cpu() - rl).abs().max()) < (1e-5 if dtype == torch.float32 else 2e-2)
+    # the merge kernel alone against the oracle's merge of the SAME partials (isolates the merge)
+    mo, ml = O.merge_partials([p[0].cpu() for p in parts], [p[1].cpu() for p in parts])
+    tol = dict(rel=1e-6, maxabs=1e-5) if dtype == torch.float32 else dict(rel=3e-3, maxabs=1.6e-2)
+    check(o, mo, dtype, "merge kernel", **tol)
+    o1, _ = B.dit_attn_partial(q, k, v)
+    e_rel, _ = errors(o, o1)
+    assert e_rel < (2e-6 if dtype == torch.float32 else 3e-3)   # P-invariance on the GPU itself
+
+
+@pytest.mark.parametrize("dtype", DTYPES)
+def test_merge_closed_forms_and_empty_shards(lib, dtype):
+    nq, H, d = 70, 2, 64
+    o = rnd("o", (nq, H, d), dtype)
+    lse = rnd("lse", (nq, H), torch.float32, std=3.0)
+    mo, ml = B.dit_attn_merge([o] * 4, [lse] * 4)               # P copies => O, LSE + ln P
+    tol = dict(rel=1e-6, maxabs=1e-5) if dtype == torch.float32 else dict(rel=3e-3, maxabs=1.6e-2)
+    check(mo, o, dtype, "merge of copies", **tol)
+    assert float((ml - (lse + math.log(4))).abs().max()) < 1e-5
+    ninf = torch.full_like(lse, -math.inf)
+    z = torch.zeros_like(o)
+    mo, ml = B.dit_attn_merge([z, o], [ninf, lse])
+    assert torch.equal(mo, o) and torch.equal(ml, lse)
+    mo, ml = B.dit_attn_merge([z, z], [ninf, ninf])
+    assert (mo == 0).all() and torch.isinf(ml).all()
+    lse2 = lse.clone(); lse2[::2] = -math.inf                   # mixed: some rows have an empty shard
+    o2 = rnd("o2", (nq, H, d), dtype)
+    mo, ml = B.dit_attn_merge([o, o2], [lse, lse2])
+    ro, rl = O.merge_partials([o.cpu(), o2.cpu()], [lse.cpu(), lse2.cpu()])
+    check(mo, ro, dtype, "merge mixed -inf", **tol)

@@ -1,0 +1,194 @@
+"""GPU parity, step level: dit_step / dit_step_varlen / dit_step_host against the CPU oracle on the same
+seeded inputs — final output AND per-stage taps (SURVEY §8(c) sensitivity warning: end-to-end tolerances alone
+would pass a wrong attention kernel), split degree P, cond modes, packing invariance."""
+import pytest
+import torch
+
+from oracle import dit_oracle as O
+from paper_2606_13501_b200 import binding as B
+from paper_2606_13501_b200 import synth
+from util import check, errors
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda:0"
+
+
+def _gpu_inputs(s, I):
+    return I["latents"].to(DEV), I["temb"][0].to(DEV), None if I["cond"] is None else I["cond"].to(DEV)
+
+
+def _run_both(s, split_p=1, taps=None):
+    W, I = synth.make_weights(s), synth.make_inputs(s)
+    ref = O.dit_step(O.cfg_from_shape(s), W, I["latents"], I["temb"], I["cond"], split_p=1, taps=taps)
+    m = B.Dit(B.make_config(s, split_p=split_p), W, DEV)
+    lat, temb, cond = _gpu_inputs(s, I)
+    out = m.dit_step(lat, temb, cond)
+    torch.cuda.synchronize()
+    return out, ref, m, (lat, temb, cond)
+
+
+def _tap_checks(s, m, inputs, taps, blocks):
+    """Stop the GPU step after each stage of each block and compare the workspace buffers with the oracle."""
+    lat, temb, cond = inputs
+    D, F, dt = s.hidden, s.mlp_dim, s.torch_dtype
+    T = s.n_tokens + (s.n_cond if s.cond_mode == "joint" else 0)
+    tight = dict(rel=2e-6, maxabs=5e-5) if dt == torch.float32 else {}
+    for l in blocks:
+        for stage, tap, shape, tdt, key in (
+                ("y1", "y", (T, D), dt, f"b{l}.y1"), ("qkv", "qkv", (T, 3 * D), dt, None),
+                ("attn", "o", (T, D), dt, f"b{l}.o"), ("y2", "y", (T, D), dt, f"b{l}.y2"),
+                ("y2", "x", (T, D), torch.float32, f"b{l}.x_cross" if s.cond_mode == "cross" else f"b{l}.x_attn"),
+                ("fc1", "u", (T, F), dt, f"b{l}.u")):
+            m.dit_debug_stop_after(l, stage)
+            m.dit_step(lat, temb, cond)
+            got = m.dit_get_tap(tap, shape, tdt)
+            torch.cuda.synchronize()
+            if key is None:
+                ref = torch.cat([taps[f"b{l}.q"], taps[f"b{l}.k"], taps[f"b{l}.v"]], dim=1)
+            else:
+                ref = taps[key]
+            check(got, ref, tdt, f"tap {stage}/{tap} block {l}", **(tight if tdt == torch.float32 or dt == torch.float32 else {}))
+    m.dit_debug_stop_after(-1, 0)
+
+
+# ------------------------------------------------------------------------------ config 1 (fp32, rel-L2 1e-5)
+@pytest.mark.parametrize("P", [1, 2, 4])
+def test_cfg1_fp32_matches_oracle_for_every_split_degree(lib, P):
+    s = synth.cfg1()
+    taps = {}
+    out, ref, m, inputs = _run_both(s, split_p=P, taps=taps)
+    e = check(out, ref, torch.float32, f"cfg1 P={P}")
+    print("cfg1 P", P, e)
+    if P == 1:
+        c = m.dit_get_tap("c", (s.hidden,), torch.float32)
+        check(c, taps["c"], torch.float32, "c", rel=2e-6)
+        mod = m.dit_get_tap("mod", (s.n_blocks * 6 * s.hidden + 2 * s.hidden,), torch.float32)
+        check(mod, torch.cat([taps["mod"].reshape(-1), taps["modf"].reshape(-1)]), torch.float32, "mod", rel=2e-6)
+        _tap_checks(s, m, inputs, taps, range(s.n_blocks))
+
+
+@pytest.mark.parametrize("variant", ["cross", "rope_qknorm", "none_rope3d", "d128"])
+def test_cfg1_variants_fp32(lib, variant):
+    """R8: every code path (cross-attention, RoPE, QK-norm, no cond, head_dim 128) gets an fp32 1e-5 pin."""
+    kw = {"cross": dict(cond_mode="cross", qk_rmsnorm=True),
+          "rope_qknorm": dict(rope_dims=(0, 32, 32), qk_rmsnorm=True),
+          "none_rope3d": dict(cond_mode="none", rope_dims=(20, 22, 22), qk_rmsnorm=True, latent_grid=(3, 16, 20),
+                              patch=(1, 2, 2)),
+          "d128": dict(n_heads=2, head_dim=128, rope_dims=(0, 64, 64), qk_rmsnorm=True)}[variant]
+    s = synth.cfg1(**kw)
+    taps = {}
+    out, ref, m, inputs = _run_both(s, split_p=2 if variant == "rope_qknorm" else 1, taps=taps)
+    check(out, ref, torch.float32, f"cfg1 {variant}")
+    _tap_checks(s, m, inputs, taps, [s.n_blocks - 1])
+
+
+def test_zero_gates_identity_and_empty_cond_on_gpu(lib):
+    s = synth.cfg1()
+    W, I = synth.make_weights(s), synth.make_inputs(s)
+    D = s.hidden
+    for l in range(s.n_blocks):
+        for lo in (2 * D, 5 * D):
+            W[f"blocks.{l}.mod.w"][lo:lo + D] = 0
+            W[f"blocks.{l}.mod.b"][lo:lo + D] = 0
+    m = B.Dit(B.make_config(s), W, DEV)
+    lat, temb, cond = _gpu_inputs(s, I)
+    m.dit_debug_stop_after(0, "y1")
+    m.dit_step(lat, temb, cond)
+    x0 = m.dit_get_tap("x", (288, D), torch.float32)
+    m.dit_debug_stop_after(-1, 0)
+    m.dit_step(lat, temb, cond)
+    x1 = m.dit_get_tap("x", (288, D), torch.float32)
+    assert torch.equal(x0, x1)                                 # zero gates: blocks are the identity, bit exact
+    # joint with zero cond tokens == cond-less sequence
+    s2 = synth.cfg1()
+    W2, I2 = synth.make_weights(s2), synth.make_inputs(s2)
+    m2 = B.Dit(B.make_config(s2), W2, DEV)
+    lat, temb, _ = _gpu_inputs(s2, I2)
+    out = m2.dit_step(lat, temb, None)
+    ref = O.dit_step(O.cfg_from_shape(s2), W2, I2["latents"], I2["temb"], I2["cond"][:0])
+    check(out, ref, torch.float32, "joint, n_cond = 0")
+
+
+# ------------------------------------------------------------------------------ bf16, reduced sizes
+def _small_bf16(**kw):
+    d = dict(name="small_bf16", dtype="bf16", n_blocks=2, hidden=512, n_heads=4, head_dim=128, mlp_dim=2048,
+             latent_channels=16, cond_dim=512, rope_dims=(0, 64, 64), qk_rmsnorm=True, latent_grid=(1, 36, 44),
+             n_cond=70, extras={})
+    d.update(kw)
+    return synth.cfg1(**d)
+
+
+@pytest.mark.parametrize("mode,P", [("joint", 1), ("joint", 4), ("cross", 1), ("none", 2)])
+def test_small_bf16_step_and_taps(lib, mode, P):
+    s = _small_bf16(cond_mode=mode, rope_dims=(44, 42, 42) if mode == "cross" else (0, 64, 64),
+                    latent_grid=(3, 20, 24) if mode == "cross" else (1, 36, 44))
+    taps = {}
+    out, ref, m, inputs = _run_both(s, split_p=P, taps=taps)
+    e = check(out, ref, torch.bfloat16, f"small bf16 {mode} P={P}")
+    print("small bf16", mode, P, e)
+    if P == 1:
+        _tap_checks(s, m, inputs, taps, range(s.n_blocks))
+
+
+def test_step_host_equals_device_call(lib):
+    s = _small_bf16()
+    W, I = synth.make_weights(s), synth.make_inputs(s)
+    m = B.Dit(B.make_config(s), W, DEV)
+    lat, temb, cond = _gpu_inputs(s, I)
+    out = m.dit_step(lat, temb, cond)
+    oh = m.dit_step_host(I["latents"].pin_memory(), I["temb"][0].contiguous().pin_memory(), I["cond"].pin_memory())
+    torch.cuda.synchronize()
+    assert torch.equal(oh, out.cpu())
+    oh2 = m.dit_step_host(I["latents"], I["temb"][0].contiguous(), I["cond"])       # pageable host memory
+    torch.cuda.synchronize()
+    assert torch.equal(oh2, out.cpu())
+
+
+# ------------------------------------------------------------------------------ varlen packing
+@pytest.mark.parametrize("dtype,mode", [("f32", "joint"), ("bf16", "joint"), ("bf16", "cross")])
+def test_varlen_equals_per_request_steps(lib, dtype, mode):
+    """Packing invariance (§8(c) step 8): the packed result for request r == dit_step on request r alone, and
+    both match the oracle.  Heterogeneous grids and cond lengths, per-request timesteps."""
+    base = dict(cond_mode=mode, dtype=dtype, rope_dims=(0, 32, 32), qk_rmsnorm=True, seed=7)
+    grids = [(1, 8, 8), (1, 32, 20), (1, 16, 48), (1, 2, 2)]
+    nconds = [5, 32, 0, 17]
+    ts = [float(synth.uniform01(7, f"t{r}", 1)[0]) * 1000 for r in range(4)]
+    shapes = [synth.cfg1(latent_grid=g, n_cond=max(n, 1), **base) for g, n in zip(grids, nconds)]
+    W = synth.make_weights(shapes[0])
+    Is = [synth.make_inputs(sh, tag=f"r{r}", t=ts[r]) for r, sh in enumerate(shapes)]
+    for r, n in enumerate(nconds):
+        Is[r]["cond"] = Is[r]["cond"][:n]
+    T_total = sum(sh.n_tokens + (n if mode == "joint" else 0) for sh, n in zip(shapes, nconds))
+    cfg = B.make_config(shapes[0], max_tokens=T_total, max_requests=4, max_cond_tokens=sum(nconds))
+    m = B.Dit(cfg, W, DEV)
+    lats = [i["latents"].to(DEV) for i in Is]
+    temb = torch.cat([i["temb"] for i in Is]).to(DEV)
+    conds = [i["cond"].to(DEV) if i["cond"].shape[0] else None for i in Is]
+    outs = m.dit_step_varlen(lats, temb, conds)
+    torch.cuda.synchronize()
+    tdt = shapes[0].torch_dtype
+    for r in range(4):
+        ref = O.dit_step(O.cfg_from_shape(shapes[r]), W, Is[r]["latents"], Is[r]["temb"], Is[r]["cond"])
+        check(outs[r], ref, tdt, f"varlen request {r}")
+        single = m.dit_step(lats[r], temb[r].contiguous(), conds[r])
+        torch.cuda.synchronize()
+        e_rel, _ = errors(outs[r], single)
+        assert e_rel < (2e-6 if tdt == torch.float32 else 2e-3), f"packing changed request {r}: {e_rel}"
+
+
+def test_argument_validation_on_gpu(lib):
+    s = synth.cfg1()
+    W, I = synth.make_weights(s), synth.make_inputs(s)
+    m = B.Dit(B.make_config(s), W, DEV)
+    lat, temb, cond = _gpu_inputs(s, I)
+    n0 = B.dit_kernel_launches()
+    with pytest.raises(B.DitError):                             # too many tokens for the workspace
+        m.dit_step(torch.zeros(4, 1, 64, 64, device=DEV), temb, cond)
+    with pytest.raises(B.DitError):                             # grid not a multiple of the patch
+        m.dit_step(torch.zeros(4, 1, 31, 32, device=DEV), temb, cond)
+    assert B.dit_kernel_launches() == n0                        # rejected before any launch
+    Wbad = dict(W); Wbad.pop("final.b")
+    with pytest.raises(B.DitError):
+        B.Dit(B.make_config(s), Wbad, DEV)
+    m.dit_step(lat, temb, cond)
+    assert B.dit_kernel_launches() > n0
