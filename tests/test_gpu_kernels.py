@@ -8,7 +8,7 @@ import torch
 from oracle import dit_oracle as O
 from paper_2606_13501_b200 import binding as B
 from paper_2606_13501_b200 import synth
-from util import check, errors
+from util import check, check_rounding, errors
 
 pytestmark = pytest.mark.gpu
 DEV = "cuda:0"
@@ -51,8 +51,11 @@ def test_adaln(lib, dtype, T, D, fused):
     else:
         assert torch.equal(xg, x)
     ref = O.modulate(xr, m[:D], m[D:2 * D], 1e-6)
-    tol = dict(rel=2e-6, maxabs=2e-5) if dtype == torch.float32 else dict(rel=3e-3, maxabs=2e-2)
-    check(y, ref, dtype, "adaln y", **tol)
+    if dtype == torch.float32:
+        check(y, ref, dtype, "adaln y", rel=2e-6, maxabs=2e-5)
+    else:   # the only bf16 error is the output rounding: bound it element-wise (outliers of |y| ~ 8 RMS exist)
+        check(y, ref, dtype, "adaln y", rel=3e-3, maxabs=6e-2)
+        check_rounding(y, ref, "adaln y")
 
 
 @pytest.mark.parametrize("dtype", DTYPES)
@@ -127,8 +130,10 @@ def test_linear(lib, dtype, M, N, K, epi):
         ref = O.gelu_tanh(ref)
     odt = torch.float32 if (epi == B.EPI_BIAS_F32 or dtype == torch.float32) else torch.bfloat16
     assert got.dtype == odt
-    tol = dict(rel=2e-6, maxabs=3e-5) if odt == torch.float32 else dict(rel=3e-3, maxabs=2e-2)
+    tol = dict(rel=2e-6, maxabs=3e-5) if odt == torch.float32 else dict(rel=3e-3, maxabs=3e-2)
     check(got, ref, odt, f"linear {M}x{N}x{K} epi{epi}", **tol)
+    if odt == torch.bfloat16:       # fp32 accumulation: the only bf16 error is the output rounding
+        check_rounding(got, ref, f"linear {M}x{N}x{K} epi{epi}")
 
 
 @pytest.mark.parametrize("dtype", DTYPES)

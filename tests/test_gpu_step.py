@@ -47,7 +47,7 @@ def _tap_checks(s, m, inputs, taps, blocks):
                 ref = torch.cat([taps[f"b{l}.q"], taps[f"b{l}.k"], taps[f"b{l}.v"]], dim=1)
             else:
                 ref = taps[key]
-            check(got, ref, tdt, f"tap {stage}/{tap} block {l}", **(tight if tdt == torch.float32 or dt == torch.float32 else {}))
+            check(got, ref, dt, f"tap {stage}/{tap} block {l}", **tight)
     m.dit_debug_stop_after(-1, 0)
 
 

@@ -26,3 +26,13 @@ def check(got, ref, dtype, what="", rel=None, maxabs=None):
     assert e_rel <= rel_bar and e_max <= max_bar, (
         f"{what}: rel-L2 {e_rel:.3e} (bar {rel_bar:.1e}), max-abs/RMS {e_max:.3e} (bar {max_bar:.1e})")
     return e_rel, e_max
+
+
+def check_rounding(got, ref, what="", ulps=1.0, atol_rms=2e-3):
+    """Element-wise bound for a bf16 kernel whose only error is the final rounding (plus fp32 arithmetic noise):
+    |got - ref| <= ulps * 2^-8 |ref| + atol_rms * RMS(ref).  Tighter than max-abs/RMS for wide-range outputs."""
+    g, r = got.detach().double().cpu().reshape(-1), ref.detach().double().cpu().reshape(-1)
+    assert torch.isfinite(g).all()
+    rms = float(r.norm()) / math.sqrt(max(1, r.numel()))
+    bad = (g - r).abs() > ulps * 2.0 ** -8 * r.abs() + atol_rms * rms
+    assert not bad.any(), f"{what}: {int(bad.sum())} elements outside the bf16 rounding bound"
