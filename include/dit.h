@@ -211,6 +211,25 @@ dit_status dit_debug_stop_after(dit_handle h, int32_t block, int32_t stage);
 /* Copy `bytes` of a workspace buffer to dst (dev), stream ordered. */
 dit_status dit_get_tap(dit_handle h, int32_t tap, void* dst, size_t bytes, void* stream);
 
+/* ---- measurement (bench.py's roofline line) -------------------------------------------------------
+ * Kernel classes of the step.  dit_profile_begin(mask) makes every later launch of a class whose bit is set
+ * in `mask` be bracketed by a cudaEvent pair on the stream it is launched on (at most 16384 launches are
+ * recorded; later ones are counted but not timed).  dit_profile_end synchronises those events, writes the
+ * summed device time (ms) and the launch count per class into the two host arrays [DIT_KC_COUNT], and
+ * switches profiling off.  Process-wide; not thread safe; adds ~2 event records per profiled launch. */
+typedef enum {
+  DIT_KC_GEMM = 0,   /* block GEMMs: QKV, out-proj, fc1, fc2, cross projections (tcgen05) */
+  DIT_KC_ATTN = 1,   /* self / cross / partial attention */
+  DIT_KC_ADALN = 2,  /* LayerNorm + modulation (+ gated residual) */
+  DIT_KC_GEMV = 3,   /* t-MLP and modulation projection (weight streaming) */
+  DIT_KC_QKNORM = 4, /* QK-RMSNorm + RoPE (stand-alone form) */
+  DIT_KC_MERGE = 5,  /* LSE merge */
+  DIT_KC_MISC = 6,   /* patchify, patch-embed / cond / final GEMMs, unpatchify, RoPE table */
+  DIT_KC_COUNT = 7
+} dit_kernel_class;
+dit_status dit_profile_begin(int32_t class_mask);
+dit_status dit_profile_end(float* ms_per_class, int32_t* launches_per_class);
+
 const char* dit_last_error(dit_handle h); /* h may be NULL: last error of a handle-less entry point */
 int32_t dit_kernel_launches(void);         /* kernels launched by this library so far (this process) */
 void dit_free(dit_handle h);

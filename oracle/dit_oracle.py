@@ -119,13 +119,16 @@ def attention(q, k, v, scale=None):
         scale = 1.0 / math.sqrt(d)
     if k.shape[0] == 0:
         return torch.zeros(Nq, H, v.shape[-1], dtype=F64), torch.full((Nq, H), -math.inf, dtype=F64)
-    s = torch.einsum("qhd,khd->hqk", q, k) * scale                 # [H, Nq, Nk] full score matrix
-    m = s.max(dim=-1, keepdim=True).values
-    e = torch.exp(s - m)
-    z = e.sum(dim=-1, keepdim=True)
-    p = e / z
-    o = torch.einsum("hqk,khd->qhd", p, v)
-    lse = (m + torch.log(z)).squeeze(-1).t()
+    o = torch.empty(Nq, H, v.shape[-1], dtype=F64)
+    lse = torch.empty(Nq, H, dtype=F64)
+    for h in range(H):                                             # one head at a time (memory only)
+        s = (q[:, h, :] @ k[:, h, :].t()) * scale                  # [Nq, Nk] full score matrix of the head
+        m = s.max(dim=-1, keepdim=True).values
+        e = torch.exp(s - m)
+        z = e.sum(dim=-1, keepdim=True)
+        p = e / z
+        o[:, h, :] = p @ v[:, h, :]
+        lse[:, h] = (m + torch.log(z)).squeeze(-1)
     return o, lse
 
 

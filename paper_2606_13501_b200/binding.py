@@ -20,7 +20,7 @@ STAGE = dict(y1=0, qkv=1, attn=2, oproj=3, cross=4, y2=5, fc1=6, fc2=7)
 
 SYMBOLS = ["dit_workspace_bytes", "dit_init", "dit_step", "dit_step_host", "dit_step_varlen", "dit_attn_partial",
            "dit_attn_merge", "dit_linear", "dit_adaln", "dit_gemv", "dit_qknorm_rope", "dit_debug_stop_after",
-           "dit_get_tap", "dit_last_error", "dit_kernel_launches", "dit_free"]
+           "dit_get_tap", "dit_profile_begin", "dit_profile_end", "dit_last_error", "dit_kernel_launches", "dit_free"]
 
 
 class dit_config(C.Structure):
@@ -74,6 +74,8 @@ def load(path: str = LIB_PATH):
         "dit_qknorm_rope": [i32, vp, i64, i32, i32, i32, i32, vp, vp, f32, vp, vp, vp],
         "dit_debug_stop_after": [vp, i32, i32],
         "dit_get_tap": [vp, i32, vp, C.c_size_t, vp],
+        "dit_profile_begin": [i32],
+        "dit_profile_end": [C.POINTER(C.c_float), pi32],
     }
     for name, argtypes in sig.items():
         fn = getattr(lib, name)
@@ -275,6 +277,24 @@ def dit_qknorm_rope(qkv, n_heads, head_dim, n_tensors=2, gq=None, gk=None, eps=1
     _check(lib.dit_qknorm_rope(_dt(qkv), _ptr(qkv), qkv.stride(0), T, n_heads, head_dim, n_tensors, _ptr(gq), _ptr(gk),
                                eps, _ptr(rope_cos), _ptr(rope_sin), _stream(stream)), "dit_qknorm_rope")
     return qkv
+
+
+KC = dict(gemm=0, attn=1, adaln=2, gemv=3, qknorm=4, merge=5, misc=6)
+
+
+def dit_profile_begin(classes=tuple(KC)):
+    mask = 0
+    for c in classes:
+        mask |= 1 << KC[c]
+    _check(load().dit_profile_begin(mask), "dit_profile_begin")
+
+
+def dit_profile_end() -> dict:
+    """{class: (device ms summed over its profiled launches, launches)}"""
+    ms = (C.c_float * len(KC))()
+    n = (C.c_int32 * len(KC))()
+    _check(load().dit_profile_end(ms, n), "dit_profile_end")
+    return {k: (float(ms[i]), int(n[i])) for k, i in KC.items()}
 
 
 def dit_kernel_launches() -> int:

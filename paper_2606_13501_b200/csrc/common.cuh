@@ -45,6 +45,24 @@ const char* get_error();
 
 static inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 
+// per-class device timing (dit_profile_begin / dit_profile_end): when a class is enabled every launcher of that
+// class brackets its launch with a cudaEvent pair on the launching stream.  Off by default (zero overhead).
+extern int g_prof_mask;
+extern thread_local int g_prof_class_override;  // >= 0: launchers report this class instead of their own
+void prof_record(int cls, cudaStream_t st, bool start);
+struct ProfScope {
+  int cls;
+  cudaStream_t st;
+  bool on;
+  ProfScope(int c, cudaStream_t s) : cls(g_prof_class_override >= 0 ? g_prof_class_override : c), st(s) {
+    on = (g_prof_mask >> cls) & 1;
+    if (on) prof_record(cls, st, true);
+  }
+  ~ProfScope() {
+    if (on) prof_record(cls, st, false);
+  }
+};
+
 // ---------------------------------------------------------------------------------------------
 // 128-bit vector access: 8 consecutive elements of T <-> 8 floats
 // ---------------------------------------------------------------------------------------------

@@ -21,6 +21,36 @@ void set_error(const char* fmt, ...) {
 }
 const char* get_error() { return g_err; }
 
+// ---- per-class event timing -------------------------------------------------------------------------
+int g_prof_mask = 0;
+thread_local int g_prof_class_override = -1;
+namespace {
+struct ProfRec { cudaEvent_t a, b; int cls; };
+std::vector<ProfRec> g_prof_recs;
+std::vector<cudaEvent_t> g_prof_pool;
+int g_prof_counts[DIT_KC_COUNT];
+const size_t kProfMax = 16384;
+cudaEvent_t prof_event() {
+  if (!g_prof_pool.empty()) { cudaEvent_t e = g_prof_pool.back(); g_prof_pool.pop_back(); return e; }
+  cudaEvent_t e = nullptr;
+  cudaEventCreate(&e);
+  return e;
+}
+}  // namespace
+void prof_record(int cls, cudaStream_t st, bool start) {
+  if (start) {
+    g_prof_counts[cls]++;
+    if (g_prof_recs.size() >= kProfMax) return;
+    ProfRec r{prof_event(), prof_event(), cls};
+    cudaEventRecord(r.a, st);
+    g_prof_recs.push_back(r);
+  } else if (!g_prof_recs.empty() && g_prof_counts[cls] <= (int)kProfMax) {
+    // the matching start is the most recent record of this class (launchers do not nest within a class)
+    for (size_t i = g_prof_recs.size(); i-- > 0;)
+      if (g_prof_recs[i].cls == cls) { cudaEventRecord(g_prof_recs[i].b, st); break; }
+  }
+}
+
 static size_t esize(int dtype) { return dtype == DIT_F32 ? 4 : 2; }
 
 struct BlockW {
@@ -143,7 +173,9 @@ static dit_status validate(const dit_config* c) {
 
 // GEMM dispatch: bf16 -> tcgen05 whenever the shape/alignment allows, else FFMA.  fp32 -> FFMA (no TF32).
 static dit_status gemm(int dtype, int epi, const void* A, int64_t lda, const void* W, const void* bias, void* out,
-                       int64_t ldo, int M, int N, int K, cudaStream_t st) {
+                       int64_t ldo, int M, int N, int K, cudaStream_t st, int kc = DIT_KC_GEMM) {
+  struct Override { int prev; Override(int c) : prev(g_prof_class_override) { g_prof_class_override = c; }
+                    ~Override() { g_prof_class_override = prev; } } ov(kc == DIT_KC_GEMM ? -1 : kc);
   if (dtype == DIT_BF16 && gemm_tc_supported(epi, A, lda, W, out, ldo, M, N, K))
     return launch_gemm_tc(epi, A, lda, W, bias, out, ldo, M, N, K, st);
   return launch_gemm_simt(dtype, epi, A, lda, W, bias, out, ldo, M, N, K, st);
@@ -224,14 +256,14 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
     const int row0 = g.cu[r] + Lc;
     char* pr = (char*)w.patches + (size_t)row0 * pvC * es;
     RUN(launch_patchify(dt, (const char*)latents + g.lat_off[r] * es, pr, c.latent_channels, Fr, Hr, Wr, c.patch, st));
-    RUN(gemm(dt, DIT_EPI_BIAS_F32, pr, pvC, hd->pe_w, hd->pe_b, w.x + (size_t)row0 * D, D, Nr, D, pvC, st));
+    RUN(gemm(dt, DIT_EPI_BIAS_F32, pr, pvC, hd->pe_w, hd->pe_b, w.x + (size_t)row0 * D, D, Nr, D, pvC, st, DIT_KC_MISC));
     if (joint && Lc > 0)
       RUN(gemm(dt, DIT_EPI_BIAS_F32, (const char*)cond + (size_t)g.cu_cond[r] * c.cond_dim * es, c.cond_dim, hd->cp_w,
-               hd->cp_b, w.x + (size_t)g.cu[r] * D, D, Lc, D, c.cond_dim, st));
+               hd->cp_b, w.x + (size_t)g.cu[r] * D, D, Lc, D, c.cond_dim, st, DIT_KC_MISC));
   }
   const int Lc_total = g.cu_cond[R];
   if (cross && Lc_total > 0)
-    RUN(gemm(dt, DIT_EPI_BIAS, cond, c.cond_dim, hd->cp_w, hd->cp_b, w.ctx, D, Lc_total, D, c.cond_dim, st));
+    RUN(gemm(dt, DIT_EPI_BIAS, cond, c.cond_dim, hd->cp_w, hd->cp_b, w.ctx, D, Lc_total, D, c.cond_dim, st, DIT_KC_MISC));
 
   // ---- step 5: blocks.  `pending_h` / `pending_gate` carry the gated residual into the next adaLN kernel.
   const void* pending_h = nullptr;
@@ -315,7 +347,7 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
     const int Nr = (Fr / c.patch[0]) * (Hr / c.patch[1]) * (Wr / c.patch[2]);
     const int row0 = g.cu[r] + (joint ? g.ncond[r] : 0);
     float* tk = w.tok + (size_t)row0 * pvC;
-    RUN(gemm(dt, DIT_EPI_BIAS_F32, (char*)w.y + (size_t)row0 * D * es, D, hd->f_w, hd->f_b, tk, pvC, Nr, pvC, D, st));
+    RUN(gemm(dt, DIT_EPI_BIAS_F32, (char*)w.y + (size_t)row0 * D * es, D, hd->f_w, hd->f_b, tk, pvC, Nr, pvC, D, st, DIT_KC_MISC));
     RUN(launch_unpatchify(dt, tk, (char*)out + g.lat_off[r] * es, c.latent_channels, Fr, Hr, Wr, c.patch, st));
   }
 #undef RUN
@@ -591,6 +623,30 @@ dit_status dit_get_tap(dit_handle h, int32_t tap, void* dst, size_t bytes, void*
     default: DIT_REQUIRE(false, DIT_ERR_INVALID_ARG, "unknown tap %d", tap);
   }
   DIT_CUDA_OK(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+  return DIT_OK;
+}
+
+dit_status dit_profile_begin(int32_t class_mask) {
+  DIT_REQUIRE(class_mask >= 0 && class_mask < (1 << DIT_KC_COUNT), DIT_ERR_INVALID_ARG, "class_mask 0x%x", class_mask);
+  for (auto& r : g_prof_recs) { g_prof_pool.push_back(r.a); g_prof_pool.push_back(r.b); }
+  g_prof_recs.clear();
+  for (int i = 0; i < DIT_KC_COUNT; ++i) g_prof_counts[i] = 0;
+  g_prof_mask = class_mask;
+  return DIT_OK;
+}
+
+dit_status dit_profile_end(float* ms_per_class, int32_t* launches_per_class) {
+  DIT_REQUIRE(ms_per_class && launches_per_class, DIT_ERR_INVALID_ARG, "NULL argument");
+  g_prof_mask = 0;
+  for (int i = 0; i < DIT_KC_COUNT; ++i) { ms_per_class[i] = 0.f; launches_per_class[i] = g_prof_counts[i]; }
+  for (auto& r : g_prof_recs) {
+    DIT_CUDA_OK(cudaEventSynchronize(r.b));
+    float ms = 0.f;
+    DIT_CUDA_OK(cudaEventElapsedTime(&ms, r.a, r.b));
+    ms_per_class[r.cls] += ms;
+    g_prof_pool.push_back(r.a); g_prof_pool.push_back(r.b);
+  }
+  g_prof_recs.clear();
   return DIT_OK;
 }
 

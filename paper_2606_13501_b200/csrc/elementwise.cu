@@ -82,6 +82,7 @@ template <typename T>
 static dit_status launch_gemv_t(const float* in, const GemvBatch* batches, int n_batches, int total_rows, float* out,
                                 int64_t out_stride, int R, int K, int silu_input, cudaStream_t st) {
   DIT_REQUIRE(K % 8 == 0, DIT_ERR_UNSUPPORTED, "gemv: K=%d must be a multiple of 8", K);
+  ProfScope _prof(DIT_KC_GEMV, st);
   int dev = 0, sms = 148;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -190,6 +191,7 @@ static dit_status launch_adaln_t(float* x, const T* h, const float* gate, const 
                                  cudaStream_t st) {
   if (T_rows == 0) return DIT_OK;
   DIT_REQUIRE(D % 256 == 0 && D <= 6144, DIT_ERR_UNSUPPORTED, "adaln: D=%d must be a multiple of 256 (<= 6144)", D);
+  ProfScope _prof(DIT_KC_ADALN, st);
   const int grid = cdiv(T_rows, 4);
 #define ADALN_CASE(NCV)                                                                                     \
   case NCV:                                                                                                 \
@@ -272,6 +274,7 @@ dit_status launch_qknorm_rope(int dtype, void* qkv, int64_t row_stride, int T, i
                               cudaStream_t st) {
   if (T == 0 || (gq == nullptr && gk == nullptr && rc == nullptr)) return DIT_OK;
   DIT_REQUIRE(d == 64 || d == 128, DIT_ERR_UNSUPPORTED, "qknorm_rope: head_dim %d not in {64,128}", d);
+  ProfScope _prof(DIT_KC_QKNORM, st);
   int64_t heads = (int64_t)T * n_tensors * H;
   int hpw = 32 / (d / 8);
   int64_t warps = (heads + hpw - 1) / hpw;
@@ -324,6 +327,7 @@ dit_status launch_rope_table(const SeqMeta* meta, int R, int T, int d, const int
                              float* rc, float* rs, cudaStream_t st) {
   if (T == 0) return DIT_OK;
   const int half = d / 2;
+  ProfScope _prof(DIT_KC_MISC, st);
   const int64_t n = (int64_t)T * half;
   rope_table_kernel<<<cdiv(n, 256), 256, 0, st>>>(meta, R, T, half, rope_dims[0], rope_dims[1], rope_dims[2],
                                                  log2((double)theta), rc, rs);
@@ -366,6 +370,7 @@ dit_status launch_patchify(int dtype, const void* lat, void* patches, int C, int
                            cudaStream_t st) {
   const int64_t total = (int64_t)C * F * H * W;
   if (total == 0) return DIT_OK;
+  ProfScope _prof(DIT_KC_MISC, st);
   if (dtype == DIT_F32)
     patchify_kernel<float><<<cdiv(total, 256), 256, 0, st>>>((const float*)lat, (float*)patches, C, F, H, W, patch[0],
                                                             patch[1], patch[2]);
@@ -380,6 +385,7 @@ dit_status launch_unpatchify(int dtype, const float* tok, void* out, int C, int 
                              cudaStream_t st) {
   const int64_t total = (int64_t)C * F * H * W;
   if (total == 0) return DIT_OK;
+  ProfScope _prof(DIT_KC_MISC, st);
   if (dtype == DIT_F32)
     unpatchify_kernel<float><<<cdiv(total, 256), 256, 0, st>>>(tok, (float*)out, C, F, H, W, patch[0], patch[1], patch[2]);
   else
@@ -455,6 +461,7 @@ dit_status launch_merge(int dtype, const void* const* o_parts, const float* cons
   if (n_rh == 0) return DIT_OK;
   DIT_REQUIRE(P >= 1 && P <= 8, DIT_ERR_INVALID_ARG, "merge: P=%d not in 1..8", P);
   DIT_REQUIRE(d % 8 == 0, DIT_ERR_UNSUPPORTED, "merge: head_dim %d must be a multiple of 8", d);
+  ProfScope _prof(DIT_KC_MERGE, st);
   MergePtrs ptrs;
   for (int p = 0; p < 8; ++p) {
     ptrs.o[p] = o_parts[p < P ? p : 0];

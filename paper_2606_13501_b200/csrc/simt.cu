@@ -59,6 +59,7 @@ dit_status launch_gemm_simt(int dtype, int epi, const void* A, int64_t lda, cons
                             int64_t ldo, int M, int N, int K, cudaStream_t st) {
   if (M == 0 || N == 0) return DIT_OK;
   dim3 grid(cdiv(N, 64), cdiv(M, 64));
+  ProfScope _prof(DIT_KC_GEMM, st);
 #define GS(TT, TOO, E)                                                                                         \
   gemm_simt_kernel<TT, TOO, E><<<grid, 256, 0, st>>>((const TT*)A, lda, (const TT*)W, (const TT*)bias, (TOO*)out, \
                                                      ldo, M, N, K)
@@ -167,6 +168,7 @@ dit_status launch_attn_simt(int dtype, const AttnArgs& a, cudaStream_t st) {
     for (int r = 0; r < a.R; ++r) max_q = max(max_q, a.cu_q_host[r + 1] - a.cu_q_host[r]);
   }
   if (max_q == 0) return DIT_OK;
+  ProfScope _prof(DIT_KC_ATTN, st);
   dim3 grid(cdiv(max_q, 32), a.H, a.cu_q ? a.R : 1);
 #define AS(TT, HDV)                                                                                              \
   attn_simt_kernel<TT, HDV><<<grid, 128, 0, st>>>((const TT*)a.q, (const TT*)a.k, (const TT*)a.v, a.q_stride,    \
