@@ -168,6 +168,10 @@ dit_status launch_gemm_simt(int dtype, int epi, const void* A, int64_t lda, cons
                             int64_t ldo, int M, int N, int K, cudaStream_t st);
 dit_status launch_gemm_tc(int epi, const void* A, int64_t lda, const void* W, const void* bias, void* out, int64_t ldo,
                           int M, int N, int K, cudaStream_t st);
+// epi 3 (internal): out fp32 [M, ldo] <- out + gate[req(row)] (.) (A W^T + bias)   (gated residual fused in the epilogue)
+dit_status launch_gemm_tc_ex(int epi, const void* A, int64_t lda, const void* W, const void* bias, void* out, int64_t ldo,
+                             const float* gate, int64_t gate_stride, const int32_t* cu, int R, int M, int N, int K,
+                             cudaStream_t st);
 bool gemm_tc_supported(int epi, const void* A, int64_t lda, const void* W, void* out, int64_t ldo, int M, int N, int K);
 
 // Attention over packed sequences.  q rows [cu_q[r], cu_q[r+1]) attend to k/v rows [cu_k[r], cu_k[r+1])

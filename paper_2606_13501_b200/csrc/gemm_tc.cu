@@ -1,10 +1,291 @@
-// gemm_tc.cu — tcgen05 / TMEM / TMA GEMM (placeholder until the tensor-core kernel lands: reports unsupported so
-// the dispatcher uses the FFMA kernel).
-#include "common.cuh"
+// gemm_tc.cu — the block GEMMs of the DiT step on 5th-generation tensor cores (north_star subsystem 3):
+//   out[M, N] = epilogue(A[M, K] W[N, K]^T + bias[N]),  bf16 x bf16 -> fp32 accumulate.
+// Design (sm_100a):
+//   * persistent kernel, one CTA per SM, static round-robin over 128 x 256 output tiles (M fastest, so the CTAs
+//     of a wave share W tiles through L2);
+//   * warp 0 = TMA producer: A (128 x 64) and W (256 x 64) tiles, 128-byte swizzle, 4-stage mbarrier ring;
+//   * warp 1 = MMA issuer: one thread issues tcgen05.mma M=128 N=256 K=16, accumulator in TMEM; two
+//     accumulator stages (2 x 256 columns = all 512) so the epilogue of tile i overlaps the mainloop of i+1;
+//   * warps 2-5 = epilogue: tcgen05.ld (32 lanes x 32 columns per warp), bias / GELU-tanh / gated-residual in
+//     fp32 registers, 16-byte global stores.
+// Roofline: tensor pipe.  M=128, N=256, K=16 takes 128 cycles on one SM's tensor core = 4096 MAC/cycle/SM; the
+// shared-memory feed is 48 KB per 512 cycles = 96 B/cycle (< 128 B/cycle), so one CTA per SM can saturate it.
+#include "tc.cuh"
+
 namespace dit {
-bool gemm_tc_supported(int, const void*, int64_t, const void*, void*, int64_t, int, int, int) { return false; }
-dit_status launch_gemm_tc(int, const void*, int64_t, const void*, const void*, void*, int64_t, int, int, int, cudaStream_t) {
-  set_error("tcgen05 GEMM not built");
-  return DIT_ERR_UNSUPPORTED;
+namespace tc {
+
+EncodeTiledFn encode_tiled_fn() {
+  static EncodeTiledFn fn = []() -> EncodeTiledFn {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr) != cudaSuccess ||
+        qr != cudaDriverEntryPointSuccess) {
+      (void)cudaGetLastError();
+      return nullptr;
+    }
+    return (EncodeTiledFn)p;
+  }();
+  return fn;
 }
+
+bool make_tmap_2d_bf16(CUtensorMap* out, const void* base, uint64_t rows, uint64_t cols, uint64_t ld, uint32_t box_rows,
+                       uint32_t box_cols) {
+  EncodeTiledFn fn = encode_tiled_fn();
+  if (!fn) return false;
+  cuuint64_t dims[2] = {cols, rows};
+  cuuint64_t strides[1] = {ld * 2};
+  cuuint32_t box[2] = {box_cols, box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  return fn(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+}  // namespace tc
+
+using namespace tc;
+
+namespace {
+
+constexpr int BM = 128, BN = 256, BK = 64, STAGES = 4;
+constexpr int A_BYTES = BM * BK * 2, B_BYTES = BN * BK * 2, STAGE_BYTES = A_BYTES + B_BYTES;
+constexpr int GEMM_THREADS = 192;
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /* alignment slack */ + 256 /* barriers */;
+enum { EPI_GATE_RESID = 3 };
+
+struct EpiArgs {
+  const bf16* bias;       // [N] or nullptr
+  void* out;              // bf16 or fp32 [M, ldo]
+  int64_t ldo;
+  const float* gate;      // EPI_GATE_RESID: fp32 [R, gate_stride], nullptr = 1
+  int64_t gate_stride;
+  const int32_t* cu;      // row -> request (nullptr: one request)
+  int R;
+};
+
+__device__ __forceinline__ float gelu_tanh_fast(float z) {
+  // 0.5 z (1 + tanh(u)) = z / (1 + exp(-2u)),  u = 0.79788456 (z + 0.044715 z^3): exact identity, fast exp
+  const float u2 = 1.5957691216057308f * fmaf(0.044715f * z * z, z, z);
+  return __fdividef(z, 1.0f + __expf(-u2));
+}
+
+template <int EPI>
+__global__ void __launch_bounds__(GEMM_THREADS, 1)
+gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, EpiArgs ep, int M, int N,
+               int K) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t bar0 = smem0 + STAGES * STAGE_BYTES;
+  // barriers: full[STAGES], empty[STAGES], tfull[2], tempty[2]; then the TMEM base address word
+  auto full_bar = [&](int s) { return bar0 + 8u * s; };
+  auto empty_bar = [&](int s) { return bar0 + 8u * (STAGES + s); };
+  auto tfull_bar = [&](int s) { return bar0 + 8u * (2 * STAGES + s); };
+  auto tempty_bar = [&](int s) { return bar0 + 8u * (2 * STAGES + 2 + s); };
+  const uint32_t tmem_slot = bar0 + 8u * (2 * STAGES + 4);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int mt = (M + BM - 1) / BM, nt = (N + BN - 1) / BN, n_tiles = mt * nt;
+  const int nkb = (K + BK - 1) / BK;
+
+  if (warp == 0 && lane == 0) {
+    tma_prefetch_desc(&tmA);
+    tma_prefetch_desc(&tmB);
+  }
+  if (warp == 1 && lane == 0) {
+    for (int s = 0; s < STAGES; ++s) {
+      mbar_init(full_bar(s), 1);
+      mbar_init(empty_bar(s), 1);
+    }
+    for (int s = 0; s < 2; ++s) {
+      mbar_init(tfull_bar(s), 1);
+      mbar_init(tempty_bar(s), 4);
+    }
+    fence_barrier_init();
+  }
+  if (warp == 2) tmem_alloc<512>(tmem_slot);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+
+  if (warp == 0) {
+    // ===================================================== TMA producer
+    int s = 0;
+    uint32_t ph = 0;
+    for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+      const int m0 = (t % mt) * BM, n0 = (t / mt) * BN;
+      for (int kb = 0; kb < nkb; ++kb) {
+        mbar_wait(empty_bar(s), ph ^ 1);
+        if (lane == 0) {
+          mbar_expect_tx(full_bar(s), STAGE_BYTES);
+          tma_load_2d(smem0 + s * STAGE_BYTES, &tmA, kb * BK, m0, full_bar(s));
+          tma_load_2d(smem0 + s * STAGE_BYTES + A_BYTES, &tmB, kb * BK, n0, full_bar(s));
+        }
+        __syncwarp();
+        if (++s == STAGES) { s = 0; ph ^= 1; }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================================================== MMA issuer
+    constexpr uint32_t idesc = idesc_bf16(BM, BN, 0, 0);
+    int s = 0;
+    uint32_t ph = 0;
+    int it = 0;
+    for (int t = blockIdx.x; t < n_tiles; t += gridDim.x, ++it) {
+      const int as = it & 1;
+      const uint32_t aph = (it >> 1) & 1;
+      mbar_wait(tempty_bar(as), aph ^ 1);
+      tc_fence_after();
+      const uint32_t d_tmem = tmem_base + as * BN;
+      for (int kb = 0; kb < nkb; ++kb) {
+        mbar_wait(full_bar(s), ph);
+        tc_fence_after();
+        if (lane == 0) {
+          const uint64_t ad = desc_kmajor_sw128(smem0 + s * STAGE_BYTES);
+          const uint64_t bd = desc_kmajor_sw128(smem0 + s * STAGE_BYTES + A_BYTES);
+#pragma unroll
+          for (int k = 0; k < BK / 16; ++k) umma_ss(d_tmem, ad + 2 * k, bd + 2 * k, idesc, (kb | k) != 0);
+          umma_commit(empty_bar(s));
+          if (kb == nkb - 1) umma_commit(tfull_bar(as));
+        }
+        __syncwarp();
+        if (++s == STAGES) { s = 0; ph ^= 1; }
+      }
+    }
+  } else {
+    // ===================================================== epilogue warps (TMEM lane quadrant = warp % 4)
+    const int quad = warp & 3;
+    int it = 0;
+    for (int t = blockIdx.x; t < n_tiles; t += gridDim.x, ++it) {
+      const int as = it & 1;
+      const uint32_t aph = (it >> 1) & 1;
+      const int m0 = (t % mt) * BM, n0 = (t / mt) * BN;
+      const int row = m0 + quad * 32 + lane;
+      const bool row_ok = row < M;
+      const float* gate_row = nullptr;
+      if (EPI == EPI_GATE_RESID && ep.gate != nullptr) {
+        const int req = (ep.cu != nullptr && ep.R > 1) ? find_request(ep.cu, ep.R, row_ok ? row : M - 1) : 0;
+        gate_row = ep.gate + (int64_t)req * ep.gate_stride;
+      }
+      mbar_wait(tfull_bar(as), aph);
+      tc_fence_after();
+      const uint32_t t_addr = tmem_base + as * BN + ((uint32_t)(quad * 32) << 16);
+#pragma unroll 1
+      for (int c = 0; c < BN / 32; ++c) {
+        const int n = n0 + c * 32;
+        if (n >= N) break;  // warp-uniform
+        uint32_t r[32];
+        tmem_ld32(t_addr + c * 32, r);
+        tmem_ld_wait();
+#pragma unroll
+        for (int g = 0; g < 4; ++g) {  // groups of 8 columns
+          const int ng = n + g * 8;
+          if (ng >= N) break;  // N % 8 == 0: groups are all-or-nothing
+          float v[8];
+#pragma unroll
+          for (int e = 0; e < 8; ++e) v[e] = __uint_as_float(r[g * 8 + e]);
+          if (ep.bias != nullptr) {
+            float b[8];
+            ld8<bf16>(ep.bias + ng, b);
+#pragma unroll
+            for (int e = 0; e < 8; ++e) v[e] += b[e];
+          }
+          if (EPI == DIT_EPI_BIAS_GELU) {
+#pragma unroll
+            for (int e = 0; e < 8; ++e) v[e] = gelu_tanh_fast(v[e]);
+          }
+          if (!row_ok) continue;
+          if (EPI == DIT_EPI_BIAS || EPI == DIT_EPI_BIAS_GELU) {
+            st8<bf16>(reinterpret_cast<bf16*>(ep.out) + (int64_t)row * ep.ldo + ng, v);
+          } else if (EPI == DIT_EPI_BIAS_F32) {
+            st8<float>(reinterpret_cast<float*>(ep.out) + (int64_t)row * ep.ldo + ng, v);
+          } else {  // x <- x + gate (.) (acc + bias)
+            float* xp = reinterpret_cast<float*>(ep.out) + (int64_t)row * ep.ldo + ng;
+            float x[8];
+            ld8<float>(xp, x);
+            if (gate_row != nullptr) {
+              float gv[8];
+              ld8<float>(gate_row + ng, gv);
+#pragma unroll
+              for (int e = 0; e < 8; ++e) x[e] = fmaf(gv[e], v[e], x[e]);
+            } else {
+#pragma unroll
+              for (int e = 0; e < 8; ++e) x[e] += v[e];
+            }
+            st8<float>(xp, x);
+          }
+        }
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(tempty_bar(as));
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 2) {
+    tc_fence_after();
+    tmem_dealloc<512>(tmem_base);
+  }
+}
+
+int sm_count() {
+  static int n = []() {
+    int dev = 0, v = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev);
+    return v;
+  }();
+  return n;
+}
+
+template <int EPI>
+dit_status launch_t(const CUtensorMap& ta, const CUtensorMap& tb, const EpiArgs& ep, int M, int N, int K, cudaStream_t st) {
+  static bool attr_set = false;
+  if (!attr_set) {
+    DIT_CUDA_OK(cudaFuncSetAttribute(gemm_tc_kernel<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
+    attr_set = true;
+  }
+  const int tiles = cdiv(M, BM) * cdiv(N, BN);
+  const int grid = tiles < sm_count() ? tiles : sm_count();
+  gemm_tc_kernel<EPI><<<grid, GEMM_THREADS, SMEM_BYTES, st>>>(ta, tb, ep, M, N, K);
+  DIT_LAUNCH_CHECK();
+  return DIT_OK;
+}
+
+}  // namespace
+
+bool gemm_tc_supported(int epi, const void* A, int64_t lda, const void* W, void* out, int64_t ldo, int M, int N, int K) {
+  (void)epi;
+  if (M <= 0 || N <= 0 || K <= 0) return false;
+  if (K % 8 != 0 || lda % 8 != 0 || N % 8 != 0 || ldo % 8 != 0) return false;
+  if (((uintptr_t)A & 15) || ((uintptr_t)W & 15) || ((uintptr_t)out & 15)) return false;
+  return encode_tiled_fn() != nullptr;
+}
+
+dit_status launch_gemm_tc_ex(int epi, const void* A, int64_t lda, const void* W, const void* bias, void* out, int64_t ldo,
+                             const float* gate, int64_t gate_stride, const int32_t* cu, int R, int M, int N, int K,
+                             cudaStream_t st) {
+  if (M == 0 || N == 0) return DIT_OK;
+  CUtensorMap ta, tb;
+  DIT_REQUIRE(make_tmap_2d_bf16(&ta, A, M, K, lda, BM, BK) && make_tmap_2d_bf16(&tb, W, N, K, K, BN, BK), DIT_ERR_CUDA,
+              "gemm_tc: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d lda=%lld)", M, N, K, (long long)lda);
+  EpiArgs ep{(const bf16*)bias, out, ldo, gate, gate_stride, cu, R};
+  ProfScope _prof(DIT_KC_GEMM, st);
+  switch (epi) {
+    case DIT_EPI_BIAS: return launch_t<DIT_EPI_BIAS>(ta, tb, ep, M, N, K, st);
+    case DIT_EPI_BIAS_GELU: return launch_t<DIT_EPI_BIAS_GELU>(ta, tb, ep, M, N, K, st);
+    case DIT_EPI_BIAS_F32: return launch_t<DIT_EPI_BIAS_F32>(ta, tb, ep, M, N, K, st);
+    case EPI_GATE_RESID: return launch_t<EPI_GATE_RESID>(ta, tb, ep, M, N, K, st);
+    default: DIT_REQUIRE(false, DIT_ERR_INVALID_ARG, "gemm_tc: epilogue %d", epi);
+  }
+}
+
+dit_status launch_gemm_tc(int epi, const void* A, int64_t lda, const void* W, const void* bias, void* out, int64_t ldo,
+                          int M, int N, int K, cudaStream_t st) {
+  return launch_gemm_tc_ex(epi, A, lda, W, bias, out, ldo, nullptr, 0, nullptr, 1, M, N, K, st);
+}
+
 }  // namespace dit

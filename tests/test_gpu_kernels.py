@@ -130,7 +130,12 @@ def test_linear(lib, dtype, M, N, K, epi):
         ref = O.gelu_tanh(ref)
     odt = torch.float32 if (epi == B.EPI_BIAS_F32 or dtype == torch.float32) else torch.bfloat16
     assert got.dtype == odt
-    tol = dict(rel=2e-6, maxabs=3e-5) if odt == torch.float32 else dict(rel=3e-3, maxabs=3e-2)
+    if dtype == torch.float32:
+        tol = dict(rel=2e-6, maxabs=3e-5)
+    elif odt == torch.float32:  # tcgen05 accumulates in fp32 but aligns addends by truncation: ~sqrt(K) 2^-24 growth
+        tol = dict(rel=1e-5, maxabs=1e-4)  # (measured 4.0e-6 at K = 4096; DESIGN.md §7 tolerances)
+    else:
+        tol = dict(rel=3e-3, maxabs=3e-2)
     check(got, ref, odt, f"linear {M}x{N}x{K} epi{epi}", **tol)
     if odt == torch.bfloat16:       # fp32 accumulation: the only bf16 error is the output rounding
         check_rounding(got, ref, f"linear {M}x{N}x{K} epi{epi}")
