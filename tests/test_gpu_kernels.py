@@ -221,7 +221,9 @@ def test_split_kv_merge_reproduces_unsplit(lib, dtype, P):
     check(o, mo, dtype, "merge kernel", **tol)
     o1, _ = B.dit_attn_partial(q, k, v)
     e_rel, _ = errors(o, o1)
-    assert e_rel < (2e-6 if dtype == torch.float32 else 3e-3)   # P-invariance on the GPU itself
+    # P-invariance on the GPU itself.  bf16: both sides carry independent roundings (P and O to bf16; the split side
+    # also its bf16 partials), each ~2^-9/sqrt(3) = 1.1e-3 rel-L2 on these noise-like outputs => ~3e-3 between them
+    assert e_rel < (2e-6 if dtype == torch.float32 else 4.5e-3)
 
 
 @pytest.mark.parametrize("dtype", DTYPES)
