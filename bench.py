@@ -270,9 +270,12 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         gemm_ms, gemm_n = prof["gemm"]
         achieved = (fl["gemm"] * K) / (gemm_ms * 1e-3) / 1e12 if gemm_ms > 0 else 0.0
         traffic = None
-        tp = os.path.join(ROOT, "profiles", "traffic.json")
+        tp = os.path.join(ROOT, "profiles", "traffic.csv")   # DRAM bytes per launch from the ncu --set full capture
         if os.path.exists(tp):
-            traffic = json.load(open(tp)).get(args.workload, {}).get("gemm_dram_bytes_per_launch")
+            for ln in open(tp).read().splitlines()[1:]:
+                f = ln.split(",")
+                if len(f) >= 3 and f[0] == args.workload and f[1] == "gemm":
+                    traffic = int(f[2])
         line = {
             "metric": METRIC, "value": world * K / (ms_total * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
             "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",

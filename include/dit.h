@@ -168,6 +168,15 @@ typedef enum {
 dit_status dit_linear(int32_t dtype, int32_t epilogue, const void* A, int64_t lda, const void* W, const void* bias,
                       void* out, int64_t ldo, int32_t M, int32_t N, int32_t K, void* stream);
 
+/* Residual-stream producer with the gate fused in the GEMM epilogue (north_star subsystem 3, "gate epilogues";
+ * the out-projection and fc2 of every block):   x[M, N] <- x + gate[req(row)] (.) (A[M, K] W[N, K]^T + bias[N])
+ *   x dev fp32 [M, ldx] in/out;  A, W, bias in dtype;  gate dev fp32 [n_requests, gate_stride] (NULL = 1), row ->
+ *   request through cu_seqlens_dev [n_requests + 1] (NULL = one request).  The branch output is never rounded
+ *   to bf16 and x is read and written exactly once. */
+dit_status dit_linear_residual(int32_t dtype, const void* A, int64_t lda, const void* W, const void* bias, float* x,
+                               int64_t ldx, const float* gate, int64_t gate_stride, const int32_t* cu_seqlens_dev,
+                               int32_t n_requests, int32_t M, int32_t N, int32_t K, void* stream);
+
 /* adaLN-Zero modulation kernel (north_star subsystem 2), one pass over the row:
  *   if h != NULL:  x <- x + gate (.) h          (gate NULL = 1)       [x fp32 in/out, h dtype]
  *   y = LN(x) (.) (1 + scale) + shift           (shift/scale NULL = 0) [y dtype]
@@ -195,7 +204,6 @@ typedef enum {
   DIT_TAP_Y = 1,   /* last adaLN output   [T, D]  dtype */
   DIT_TAP_QKV = 2, /* q|k|v after norm+rope [T, 3D] dtype */
   DIT_TAP_O = 3,   /* attention output    [T, D]  dtype */
-  DIT_TAP_H = 4,   /* last out-proj / fc2 result [T, D] dtype */
   DIT_TAP_U = 5,   /* GELU output         [T, F]  dtype */
   DIT_TAP_C = 6,   /* c                   [R, D]  fp32 */
   DIT_TAP_MOD = 7, /* modulation          [R, L*6*D + 2*D] fp32 */

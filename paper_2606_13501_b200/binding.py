@@ -15,11 +15,11 @@ DIT_OK = 0
 DIT_F32, DIT_BF16 = 0, 1
 COND = {"none": 0, "joint": 1, "cross": 2}
 EPI_BIAS, EPI_BIAS_GELU, EPI_BIAS_F32 = 0, 1, 2
-TAP = dict(x=0, y=1, qkv=2, o=3, h=4, u=5, c=6, mod=7, tok=8)
+TAP = dict(x=0, y=1, qkv=2, o=3, u=5, c=6, mod=7, tok=8)
 STAGE = dict(y1=0, qkv=1, attn=2, oproj=3, cross=4, y2=5, fc1=6, fc2=7)
 
 SYMBOLS = ["dit_workspace_bytes", "dit_init", "dit_step", "dit_step_host", "dit_step_varlen", "dit_attn_partial",
-           "dit_attn_merge", "dit_linear", "dit_adaln", "dit_gemv", "dit_qknorm_rope", "dit_debug_stop_after",
+           "dit_attn_merge", "dit_linear", "dit_linear_residual", "dit_adaln", "dit_gemv", "dit_qknorm_rope", "dit_debug_stop_after",
            "dit_get_tap", "dit_profile_begin", "dit_profile_end", "dit_last_error", "dit_kernel_launches", "dit_free"]
 
 
@@ -69,6 +69,7 @@ def load(path: str = LIB_PATH):
         "dit_attn_partial": [i32, vp, vp, vp, i32, i32, i32, i32, i64, i64, f32, vp, vp, vp],
         "dit_attn_merge": [i32, C.POINTER(vp), C.POINTER(vp), i32, i32, i32, i32, vp, vp, vp],
         "dit_linear": [i32, i32, vp, i64, vp, vp, vp, i64, i32, i32, i32, vp],
+        "dit_linear_residual": [i32, vp, i64, vp, vp, vp, i64, vp, i64, vp, i32, i32, i32, i32, vp],
         "dit_adaln": [i32, vp, vp, vp, vp, vp, i64, vp, i32, vp, i32, i32, f32, vp],
         "dit_gemv": [i32, vp, vp, vp, vp, i32, i32, i32, i32, vp],
         "dit_qknorm_rope": [i32, vp, i64, i32, i32, i32, i32, vp, vp, f32, vp, vp, vp],
@@ -247,6 +248,17 @@ def dit_linear(A, W, bias=None, epilogue=EPI_BIAS, out=None, stream=None):
     _check(lib.dit_linear(_dt(A), epilogue, _ptr(A), A.stride(0), _ptr(W), _ptr(bias), _ptr(out), out.stride(0), M, N, K,
                           _stream(stream)), "dit_linear")
     return out
+
+
+def dit_linear_residual(A, W, x, bias=None, gate=None, gate_stride=0, cu_seqlens=None, n_requests=1, stream=None):
+    """x [M,N] fp32 <- x + gate[req(row)] (.) (A W^T + bias), in place."""
+    lib = load()
+    M, K = A.shape
+    N = W.shape[0]
+    _check(lib.dit_linear_residual(_dt(A), _ptr(A), A.stride(0), _ptr(W), _ptr(bias), _ptr(x), x.stride(0), _ptr(gate),
+                                   gate_stride, _ptr(cu_seqlens), n_requests, M, N, K, _stream(stream)),
+           "dit_linear_residual")
+    return x
 
 
 def dit_adaln(x, y_dtype, h=None, gate=None, shift=None, scale=None, mod_stride=0, cu_seqlens=None, n_requests=1,

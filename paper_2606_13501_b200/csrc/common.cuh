@@ -164,11 +164,13 @@ dit_status launch_merge(int dtype, const void* const* o_parts, const float* cons
                         int d, void* o, float* lse_out, cudaStream_t st);
 
 // GEMM: out[M,N] = epi(A[M,K] W[N,K]^T + bias).  *_simt works for both dtypes; *_tc is the tcgen05 path (bf16).
+// epi 3 (DIT_EPI_GATE_RESIDUAL): out fp32 [M, ldo] <- out + gate[req(row)] (.) (A W^T + bias)
 dit_status launch_gemm_simt(int dtype, int epi, const void* A, int64_t lda, const void* W, const void* bias, void* out,
-                            int64_t ldo, int M, int N, int K, cudaStream_t st);
+                            int64_t ldo, int M, int N, int K, cudaStream_t st, const float* gate = nullptr,
+                            int64_t gate_stride = 0, const int32_t* cu = nullptr, int R = 1);
 dit_status launch_gemm_tc(int epi, const void* A, int64_t lda, const void* W, const void* bias, void* out, int64_t ldo,
                           int M, int N, int K, cudaStream_t st);
-// epi 3 (internal): out fp32 [M, ldo] <- out + gate[req(row)] (.) (A W^T + bias)   (gated residual fused in the epilogue)
+// epi 3: the gated residual fused in the epilogue (gate nullptr = 1; cu nullptr = one request)
 dit_status launch_gemm_tc_ex(int epi, const void* A, int64_t lda, const void* W, const void* bias, void* out, int64_t ldo,
                              const float* gate, int64_t gate_stride, const int32_t* cu, int R, int M, int N, int K,
                              cudaStream_t st);

@@ -63,7 +63,6 @@ struct Workspace {
   void* y;         // [Tm, D]
   void* qkv;       // [Tm, 3D]
   void* o;         // [Tm, D]
-  void* h;         // [Tm, D]
   void* u;         // [Tm, F]
   float* c1;       // [Rm, D] first t-MLP layer
   float* c;        // [Rm, D]
@@ -120,7 +119,6 @@ static bool carve(const dit_config& c, char* base, Workspace* w) {
   w->y = take(Tm * D * es);
   w->qkv = take(Tm * 3 * D * es);
   w->o = take(Tm * D * es);
-  w->h = take(Tm * D * es);
   w->u = take(Tm * F * es);
   w->c1 = (float*)take(Rm * D * 4);
   w->c = (float*)take(Rm * D * 4);
@@ -179,6 +177,16 @@ static dit_status gemm(int dtype, int epi, const void* A, int64_t lda, const voi
   if (dtype == DIT_BF16 && gemm_tc_supported(epi, A, lda, W, out, ldo, M, N, K))
     return launch_gemm_tc(epi, A, lda, W, bias, out, ldo, M, N, K, st);
   return launch_gemm_simt(dtype, epi, A, lda, W, bias, out, ldo, M, N, K, st);
+}
+
+// Residual-stream producer  x <- x + gate (.) (A W^T + bias)  (out-projection, fc2).
+// The gated add runs in the GEMM's fp32 epilogue: the branch output is never rounded to bf16 and x is touched once.
+static dit_status gemm_residual(int dtype, const void* A, int64_t lda, const void* W, const void* bias, float* x,
+                                int64_t ldx, const float* gate, int64_t gate_stride, const int32_t* cu, int R, int M,
+                                int N, int K, cudaStream_t st) {
+  if (dtype == DIT_BF16 && gemm_tc_supported(3, A, lda, W, x, ldx, M, N, K))
+    return launch_gemm_tc_ex(3, A, lda, W, bias, x, ldx, gate, gate_stride, cu, R, M, N, K, st);
+  return launch_gemm_simt(dtype, 3, A, lda, W, bias, x, ldx, M, N, K, st, gate, gate_stride, cu, R);
 }
 
 static dit_status attention(int dtype, const AttnArgs& a, cudaStream_t st) {
@@ -265,16 +273,12 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
   if (cross && Lc_total > 0)
     RUN(gemm(dt, DIT_EPI_BIAS, cond, c.cond_dim, hd->cp_w, hd->cp_b, w.ctx, D, Lc_total, D, c.cond_dim, st, DIT_KC_MISC));
 
-  // ---- step 5: blocks.  `pending_h` / `pending_gate` carry the gated residual into the next adaLN kernel.
-  const void* pending_h = nullptr;
-  const float* pending_gate = nullptr;
-  bool pending_has_gate = false;
+  // ---- step 5: blocks.  Both residual branches are added to x inside their GEMM epilogues (gemm_residual).
   const float scale = 1.0f / sqrtf((float)d);
   for (int l = 0; l < L; ++l) {
     const BlockW& b = hd->blocks[l];
     const float* m = w.mod + (size_t)l * 6 * D;
-    RUN(launch_adaln(dt, w.x, pending_h, pending_has_gate ? pending_gate : nullptr, m + 0 * D, m + 1 * D, mod_stride,
-                     cu_dev, R, w.y, T, D, c.ln_eps, st));
+    RUN(launch_adaln(dt, w.x, nullptr, nullptr, m + 0 * D, m + 1 * D, mod_stride, cu_dev, R, w.y, T, D, c.ln_eps, st));
     if (stop(l, DIT_STAGE_Y1)) return DIT_OK;
     RUN(gemm(dt, DIT_EPI_BIAS, w.y, D, b.wqkv, b.bqkv, w.qkv, 3 * D, T, 3 * D, D, st));
     RUN(launch_qknorm_rope(dt, w.qkv, 3 * D, T, H, d, 2, c.qk_rmsnorm ? b.gq : nullptr, c.qk_rmsnorm ? b.gk : nullptr,
@@ -305,10 +309,10 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
       }
     }
     if (stop(l, DIT_STAGE_ATTN)) return DIT_OK;
-    RUN(gemm(dt, DIT_EPI_BIAS, w.o, D, b.wo, b.bo, w.h, D, T, D, D, st));
+    RUN(gemm_residual(dt, w.o, D, b.wo, b.bo, w.x, D, m + 2 * D, mod_stride, cu_dev, R, T, D, D, st));
     if (stop(l, DIT_STAGE_OPROJ)) return DIT_OK;
-    if (cross) {  // R10: x <- x + gate1 h;  x <- x + Wo_c Attn(RMS(Wq_c LN(x)), RMS(Wk_c ctx), Wv_c ctx) + bo_c
-      RUN(launch_adaln(dt, w.x, w.h, m + 2 * D, nullptr, nullptr, mod_stride, cu_dev, R, w.y, T, D, c.ln_eps, st));
+    if (cross) {  // R10: x <- x + Wo_c Attn(RMS(Wq_c LN(x)), RMS(Wk_c ctx), Wv_c ctx) + bo_c   (no gate, no modulation)
+      RUN(launch_adaln(dt, w.x, nullptr, nullptr, nullptr, nullptr, mod_stride, cu_dev, R, w.y, T, D, c.ln_eps, st));
       RUN(gemm(dt, DIT_EPI_BIAS, w.y, D, b.cwq, b.cbq, w.qkv, D, T, D, D, st));
       RUN(launch_qknorm_rope(dt, w.qkv, D, T, H, d, 1, b.cgq, nullptr, c.rms_eps, nullptr, nullptr, st));
       if (Lc_total > 0) {
@@ -323,25 +327,19 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
       a.cu_q_host = g.cu.data(); a.cu_k_host = g.cu_cond.data();
       a.R = R; a.n_q = T; a.n_k = Lc_total; a.H = H; a.d = d; a.scale = scale; a.shard = 0; a.n_shards = 1;
       RUN(attention(dt, a, st));
-      RUN(gemm(dt, DIT_EPI_BIAS, w.o, D, b.cwo, b.cbo, w.h, D, T, D, D, st));
+      RUN(gemm_residual(dt, w.o, D, b.cwo, b.cbo, w.x, D, nullptr, 0, cu_dev, R, T, D, D, st));
       if (stop(l, DIT_STAGE_CROSS)) return DIT_OK;
-      RUN(launch_adaln(dt, w.x, w.h, nullptr, m + 3 * D, m + 4 * D, mod_stride, cu_dev, R, w.y, T, D, c.ln_eps, st));
-    } else {
-      RUN(launch_adaln(dt, w.x, w.h, m + 2 * D, m + 3 * D, m + 4 * D, mod_stride, cu_dev, R, w.y, T, D, c.ln_eps, st));
     }
+    RUN(launch_adaln(dt, w.x, nullptr, nullptr, m + 3 * D, m + 4 * D, mod_stride, cu_dev, R, w.y, T, D, c.ln_eps, st));
     if (stop(l, DIT_STAGE_Y2)) return DIT_OK;
     RUN(gemm(dt, DIT_EPI_BIAS_GELU, w.y, D, b.w1, b.b1, w.u, F, T, F, D, st));
     if (stop(l, DIT_STAGE_FC1)) return DIT_OK;
-    RUN(gemm(dt, DIT_EPI_BIAS, w.u, F, b.w2, b.b2, w.h, D, T, D, F, st));
+    RUN(gemm_residual(dt, w.u, F, b.w2, b.b2, w.x, D, m + 5 * D, mod_stride, cu_dev, R, T, D, F, st));
     if (stop(l, DIT_STAGE_FC2)) return DIT_OK;
-    pending_h = w.h;
-    pending_gate = m + 5 * D;
-    pending_has_gate = true;
   }
   // ---- step 6: final adaLN (folds the last gated residual), Linear D -> C*pv, unpatchify (image tokens only)
   const float* mf = w.mod + (size_t)L * 6 * D;
-  RUN(launch_adaln(dt, w.x, pending_h, pending_has_gate ? pending_gate : nullptr, mf, mf + D, mod_stride, cu_dev, R,
-                   w.y, T, D, c.ln_eps, st));
+  RUN(launch_adaln(dt, w.x, nullptr, nullptr, mf, mf + D, mod_stride, cu_dev, R, w.y, T, D, c.ln_eps, st));
   for (int r = 0; r < R; ++r) {
     const int Fr = g.grids[3 * r], Hr = g.grids[3 * r + 1], Wr = g.grids[3 * r + 2];
     const int Nr = (Fr / c.patch[0]) * (Hr / c.patch[1]) * (Wr / c.patch[2]);
@@ -563,6 +561,19 @@ dit_status dit_linear(int32_t dtype, int32_t epilogue, const void* A, int64_t ld
   return gemm(dtype, epilogue, A, lda, W, bias, out, ldo, M, N, K, (cudaStream_t)stream);
 }
 
+dit_status dit_linear_residual(int32_t dtype, const void* A, int64_t lda, const void* W, const void* bias, float* x,
+                               int64_t ldx, const float* gate, int64_t gate_stride, const int32_t* cu_seqlens_dev,
+                               int32_t n_requests, int32_t M, int32_t N, int32_t K, void* stream) {
+  DIT_REQUIRE(dtype == DIT_F32 || dtype == DIT_BF16, DIT_ERR_INVALID_ARG, "dtype %d", dtype);
+  DIT_REQUIRE(M >= 0 && N > 0 && K > 0 && lda >= K && ldx >= N, DIT_ERR_INVALID_ARG, "bad GEMM shape M=%d N=%d K=%d lda=%lld ldx=%lld",
+              M, N, K, (long long)lda, (long long)ldx);
+  DIT_REQUIRE(M == 0 || (A && W && x), DIT_ERR_INVALID_ARG, "NULL argument");
+  DIT_REQUIRE(n_requests >= 1 && n_requests <= 64 && (n_requests == 1 || cu_seqlens_dev), DIT_ERR_INVALID_ARG,
+              "n_requests %d (cu_seqlens required when > 1)", n_requests);
+  return gemm_residual(dtype, A, lda, W, bias, x, ldx, gate, gate_stride, cu_seqlens_dev, n_requests, M, N, K,
+                       (cudaStream_t)stream);
+}
+
 dit_status dit_adaln(int32_t dtype, float* x, const void* h, const float* gate, const float* shift, const float* scale,
                      int64_t mod_stride, const int32_t* cu_seqlens_dev, int32_t n_requests, void* y, int32_t T, int32_t D,
                      float eps, void* stream) {
@@ -615,7 +626,6 @@ dit_status dit_get_tap(dit_handle h, int32_t tap, void* dst, size_t bytes, void*
     case DIT_TAP_Y: src = w.y; break;
     case DIT_TAP_QKV: src = w.qkv; break;
     case DIT_TAP_O: src = w.o; break;
-    case DIT_TAP_H: src = w.h; break;
     case DIT_TAP_U: src = w.u; break;
     case DIT_TAP_C: src = w.c; break;
     case DIT_TAP_MOD: src = w.mod; break;

@@ -51,7 +51,9 @@ namespace {
 constexpr int BM = 128, BN = 256, BK = 64, STAGES = 4;
 constexpr int A_BYTES = BM * BK * 2, B_BYTES = BN * BK * 2, STAGE_BYTES = A_BYTES + B_BYTES;
 constexpr int GEMM_THREADS = 192;
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /* alignment slack */ + 256 /* barriers */;
+constexpr int EPI_THREADS = 128;
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /* alignment slack */ + 256 /* barriers */ +
+                           2 * 2 * BN * 4 /* bias + gate rows of the tile, fp32, one set per accumulator stage */;
 enum { EPI_GATE_RESID = 3 };
 
 struct EpiArgs {
@@ -156,7 +158,12 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     }
   } else {
     // ===================================================== epilogue warps (TMEM lane quadrant = warp % 4)
+    // Per tile: the 128 epilogue threads first stage the tile's bias row (and, for the gated residual, the gate
+    // row of the tile's first request) in shared memory as fp32 — one global load per thread instead of one
+    // dependent global load per 8 columns — then each thread walks its accumulator row in 32-column chunks.
     const int quad = warp & 3;
+    const int et = threadIdx.x - 64;  // 0..127
+    float* const s_vec = reinterpret_cast<float*>(smem_raw + (bar0 - smem_u32(smem_raw)) + 256);
     int it = 0;
     for (int t = blockIdx.x; t < n_tiles; t += gridDim.x, ++it) {
       const int as = it & 1;
@@ -164,10 +171,41 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       const int m0 = (t % mt) * BM, n0 = (t / mt) * BN;
       const int row = m0 + quad * 32 + lane;
       const bool row_ok = row < M;
+      float* const s_bias = s_vec + as * 2 * BN;
+      float* const s_gate = s_bias + BN;
+      bool gate_smem = true;          // this thread's row takes the staged gate row
       const float* gate_row = nullptr;
       if (EPI == EPI_GATE_RESID && ep.gate != nullptr) {
-        const int req = (ep.cu != nullptr && ep.R > 1) ? find_request(ep.cu, ep.R, row_ok ? row : M - 1) : 0;
+        int req0 = 0, req = 0;
+        if (ep.cu != nullptr && ep.R > 1) {
+          req0 = find_request(ep.cu, ep.R, m0);
+          req = find_request(ep.cu, ep.R, row_ok ? row : M - 1);
+        }
+        gate_smem = req == req0;
         gate_row = ep.gate + (int64_t)req * ep.gate_stride;
+        const float* g0 = ep.gate + (int64_t)req0 * ep.gate_stride;
+#pragma unroll
+        for (int i = et; i < BN; i += EPI_THREADS) s_gate[i] = (n0 + i < N) ? g0[n0 + i] : 0.f;
+      }
+#pragma unroll
+      for (int i = et; i < BN; i += EPI_THREADS)
+        s_bias[i] = (ep.bias != nullptr && n0 + i < N) ? __bfloat162float(ep.bias[n0 + i]) : 0.f;
+      asm volatile("bar.sync 1, 128;" ::: "memory");  // staged rows visible to the 4 epilogue warps
+      float* const xrow = reinterpret_cast<float*>(ep.out) + (int64_t)(row_ok ? row : 0) * ep.ldo + n0;
+      float xc[32];
+      auto load_x = [&](int c) {  // residual-stream chunk c of this thread's row (EPI_GATE_RESID)
+#pragma unroll
+        for (int g = 0; g < 4; ++g) {
+          if (row_ok && n0 + c * 32 + g * 8 < N) ld8<float>(xrow + c * 32 + g * 8, &xc[g * 8]);
+        }
+      };
+      if (EPI == EPI_GATE_RESID) {
+        // pull this thread's 1 KB slice of the residual row into L2 while the mainloop runs (the epilogue reads it
+        // 128 bytes at a time; without this every chunk pays a DRAM round trip)
+        const int ncols = (N - n0) < BN ? (N - n0) : BN;
+        if (row_ok)
+          asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(xrow), "r"(ncols * 4) : "memory");
+        load_x(0);  // first chunk in flight while the mainloop of this tile finishes
       }
       mbar_wait(tfull_bar(as), aph);
       tc_fence_after();
@@ -179,19 +217,20 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         uint32_t r[32];
         tmem_ld32(t_addr + c * 32, r);
         tmem_ld_wait();
+        float xv[32];
+        if (EPI == EPI_GATE_RESID) {
+#pragma unroll
+          for (int e = 0; e < 32; ++e) xv[e] = xc[e];
+          if (c + 1 < BN / 32 && n + 32 < N) load_x(c + 1);  // prefetch the next chunk
+        }
 #pragma unroll
         for (int g = 0; g < 4; ++g) {  // groups of 8 columns
           const int ng = n + g * 8;
           if (ng >= N) break;  // N % 8 == 0: groups are all-or-nothing
-          float v[8];
+          float v[8], b[8];
+          ld8<float>(s_bias + c * 32 + g * 8, b);
 #pragma unroll
-          for (int e = 0; e < 8; ++e) v[e] = __uint_as_float(r[g * 8 + e]);
-          if (ep.bias != nullptr) {
-            float b[8];
-            ld8<bf16>(ep.bias + ng, b);
-#pragma unroll
-            for (int e = 0; e < 8; ++e) v[e] += b[e];
-          }
+          for (int e = 0; e < 8; ++e) v[e] = __uint_as_float(r[g * 8 + e]) + b[e];
           if (EPI == DIT_EPI_BIAS_GELU) {
 #pragma unroll
             for (int e = 0; e < 8; ++e) v[e] = gelu_tanh_fast(v[e]);
@@ -202,19 +241,20 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
           } else if (EPI == DIT_EPI_BIAS_F32) {
             st8<float>(reinterpret_cast<float*>(ep.out) + (int64_t)row * ep.ldo + ng, v);
           } else {  // x <- x + gate (.) (acc + bias)
-            float* xp = reinterpret_cast<float*>(ep.out) + (int64_t)row * ep.ldo + ng;
             float x[8];
-            ld8<float>(xp, x);
+#pragma unroll
+            for (int e = 0; e < 8; ++e) x[e] = xv[g * 8 + e];
             if (gate_row != nullptr) {
               float gv[8];
-              ld8<float>(gate_row + ng, gv);
+              if (gate_smem) ld8<float>(s_gate + c * 32 + g * 8, gv);
+              else ld8<float>(gate_row + ng, gv);
 #pragma unroll
               for (int e = 0; e < 8; ++e) x[e] = fmaf(gv[e], v[e], x[e]);
             } else {
 #pragma unroll
               for (int e = 0; e < 8; ++e) x[e] += v[e];
             }
-            st8<float>(xp, x);
+            st8<float>(xrow + c * 32 + g * 8, x);
           }
         }
       }

@@ -11,7 +11,8 @@ namespace dit {
 template <typename T, typename TO, int EPI>
 __global__ void __launch_bounds__(256) gemm_simt_kernel(const T* __restrict__ A, int64_t lda, const T* __restrict__ W,
                                                         const T* __restrict__ bias, TO* __restrict__ out, int64_t ldo,
-                                                        int M, int N, int K) {
+                                                        int M, int N, int K, const float* __restrict__ gate,
+                                                        int64_t gate_stride, const int32_t* __restrict__ cu, int R) {
   __shared__ float sA[16][64 + 4];
   __shared__ float sB[16][64 + 4];
   const int tid = threadIdx.x;
@@ -44,29 +45,39 @@ __global__ void __launch_bounds__(256) gemm_simt_kernel(const T* __restrict__ A,
   for (int i = 0; i < 4; ++i) {
     const int m = m0 + ty * 4 + i;
     if (m >= M) continue;
+    const float* grow = nullptr;
+    if (EPI == 3 && gate != nullptr) grow = gate + (int64_t)((cu != nullptr && R > 1) ? find_request(cu, R, m) : 0) * gate_stride;
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
       const int n = n0 + tx * 4 + j;
       if (n >= N) continue;
       float v = acc[i][j] + (bias ? to_f<T>(bias[n]) : 0.f);
       if (EPI == DIT_EPI_BIAS_GELU) v = gelu_tanh_f(v);
+      if (EPI == 3) {  // x <- x + gate (.) v   (TO = float)
+        const float xo = to_f<TO>(out[(int64_t)m * ldo + n]);
+        v = grow ? fmaf(grow[n], v, xo) : xo + v;
+      }
       out[(int64_t)m * ldo + n] = from_f<TO>(v);
     }
   }
 }
 
 dit_status launch_gemm_simt(int dtype, int epi, const void* A, int64_t lda, const void* W, const void* bias, void* out,
-                            int64_t ldo, int M, int N, int K, cudaStream_t st) {
+                            int64_t ldo, int M, int N, int K, cudaStream_t st, const float* gate, int64_t gate_stride,
+                            const int32_t* cu, int R) {
   if (M == 0 || N == 0) return DIT_OK;
   dim3 grid(cdiv(N, 64), cdiv(M, 64));
   ProfScope _prof(DIT_KC_GEMM, st);
 #define GS(TT, TOO, E)                                                                                         \
   gemm_simt_kernel<TT, TOO, E><<<grid, 256, 0, st>>>((const TT*)A, lda, (const TT*)W, (const TT*)bias, (TOO*)out, \
-                                                     ldo, M, N, K)
+                                                     ldo, M, N, K, gate, gate_stride, cu, R)
   if (dtype == DIT_F32) {
-    if (epi == DIT_EPI_BIAS_GELU) GS(float, float, DIT_EPI_BIAS_GELU); else GS(float, float, DIT_EPI_BIAS);
+    if (epi == DIT_EPI_BIAS_GELU) GS(float, float, DIT_EPI_BIAS_GELU);
+    else if (epi == 3) GS(float, float, 3);
+    else GS(float, float, DIT_EPI_BIAS);
   } else {
     if (epi == DIT_EPI_BIAS_GELU) GS(bf16, bf16, DIT_EPI_BIAS_GELU);
+    else if (epi == 3) GS(bf16, float, 3);
     else if (epi == DIT_EPI_BIAS_F32) GS(bf16, float, DIT_EPI_BIAS_F32);
     else GS(bf16, bf16, DIT_EPI_BIAS);
   }

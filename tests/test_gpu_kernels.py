@@ -157,6 +157,34 @@ def test_linear_strided_views_and_no_bias(lib, dtype):
     assert B.dit_linear(A[:0], W, None).shape == (0, N)
 
 
+@pytest.mark.parametrize("dtype", DTYPES)
+@pytest.mark.parametrize("M,N,K,R", [(288, 256, 256, 1), (515, 768, 1032, 3), (130, 3072, 512, 1), (1000, 264, 4096, 4)])
+@pytest.mark.parametrize("gated", [True, False])
+def test_linear_residual_gate_epilogue(lib, dtype, M, N, K, R, gated):
+    """x <- x + gate[req(row)] (.) (A W^T + b) in the GEMM epilogue (the out-projection / fc2 of every block).
+    Request boundaries fall inside 128-row tiles; N is not a multiple of the 256-column tile."""
+    A = rnd("A", (M, K), dtype)
+    W, b = rnd("W", (N, K), dtype, std=1.0 / math.sqrt(K)), rnd("b", (N,), dtype, std=0.5)
+    x0 = rnd("x", (M, N), torch.float32, std=2.0)
+    gate = rnd("gate", (R, 2 * N), torch.float32, std=0.5)[:, N:] if gated else None   # a slice: stride 2N
+    bounds = [0] + sorted(int(v) for v in (synth.uniform01(5, "cu", R - 1) * M)) + [M] if R > 1 else [0, M]
+    cu = torch.tensor(bounds, dtype=torch.int32, device=DEV)
+    x = x0.clone()
+    B.dit_linear_residual(A, W, x, b, gate, 2 * N if gated else 0, cu if R > 1 else None, R)
+    branch = O.linear(A.double().cpu(), W.cpu(), b.cpu())
+    if gated:
+        req = torch.bucketize(torch.arange(M), torch.tensor(bounds[1:-1]), right=True) if R > 1 else torch.zeros(M, dtype=torch.long)
+        branch = gate.double().cpu()[req] * branch
+    ref = x0.double().cpu() + branch
+    tol = dict(rel=2e-6, maxabs=3e-5) if dtype == torch.float32 else dict(rel=1e-5, maxabs=1e-4)
+    check(x, ref, torch.float32, f"linear_residual {M}x{N}x{K} R={R}", **tol)
+    # zero gate: x is returned bit-exact (adaLN-Zero identity, BASELINE.json north_star)
+    if gated:
+        x = x0.clone()
+        B.dit_linear_residual(A, W, x, b, torch.zeros_like(gate), N, cu if R > 1 else None, R)
+        assert torch.equal(x, x0)
+
+
 # ------------------------------------------------------------------------------ attention partial + merge
 def _attn_tol(dtype):
     return dict(rel=2e-6, maxabs=3e-5) if dtype == torch.float32 else dict(rel=4e-3, maxabs=2.5e-2)
