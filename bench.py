@@ -308,13 +308,111 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         dist.destroy_process_group()
 
 
+# --------------------------------------------------------------------------------------------------------
+# per-kernel arm: every HBM-bound kernel and the attention sweep (BASELINE.json configs[4]) timed ALONE
+# --------------------------------------------------------------------------------------------------------
+def run_kernels(args):
+    """`--workload kernels`: one JSON line with a list of per-kernel measurements.  Every kernel is launched through
+    the C ABI at the sizes it has inside cfg 2 / cfg 3 / cfg 5, timed with CUDA events on the launching stream; between
+    timed launches a 512 MB buffer is overwritten so nothing is served from the 126 MB L2.  `frac` is against
+    MEASURED_PEAKS.json: the burst figures, because each kernel is timed alone (HBM GB/s copy peak; bf16 TFLOP/s)."""
+    from paper_2606_13501_b200 import binding as B
+    B.load()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    pk = _peaks()
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
+    reps = max(3, min(args.steps, 20))
+    bf = torch.bfloat16
+
+    def timeit(fn):
+        ts = []
+        for i in range(args.warmup + reps):
+            flush.fill_(i & 0xff)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); fn(); e1.record()
+            torch.cuda.synchronize()
+            if i >= args.warmup:
+                ts.append(e0.elapsed_time(e1))
+        return statistics.median(ts), min(ts)
+
+    rows = []
+
+    def hbm(name, nbytes, fn):
+        med, best = timeit(fn)
+        gbs = nbytes / (med * 1e-3) / 1e9
+        rows.append({"kernel": name, "bound": "hbm", "bytes": nbytes, "ms": round(med, 5), "ms_best": round(best, 5),
+                     "achieved": round(gbs, 1), "unit": "GB/s", "peak": pk["hbm"], "frac": round(gbs / pk["hbm"], 4)})
+
+    def tensor(name, flops, fn):
+        med, best = timeit(fn)
+        tf = flops / (med * 1e-3) / 1e12
+        rows.append({"kernel": name, "bound": "tensor", "flops": flops, "ms": round(med, 5), "ms_best": round(best, 5),
+                     "achieved": round(tf, 1), "unit": "TFLOP/s", "peak": pk["tf_burst"], "frac": round(tf / pk["tf_burst"], 4),
+                     "frac_of_nominal_2250": round(tf / 2250.0, 4)})
+
+    rn = lambda name, shape, dt, std=1.0: synth.normal(5, name, shape, std=std, dtype=dt, device=dev)
+    # ---- adaLN (a5 / a9): 4D read + 2D write per token
+    for T, D in ((4352, 3072), (32760, 5120)):
+        x, mod = rn("x", (T, D), torch.float32), rn("mod", (1, 2 * D), torch.float32, 0.3)
+        hbm(f"adaln T={T} D={D}", T * D * 6, lambda: B.dit_adaln(x, bf, shift=mod[:, :D], scale=mod[:, D:], mod_stride=2 * D))
+        del x
+    # ---- modulation GEMV (a2): weights streamed once
+    for L, D in ((8, 3072), (4, 5120)):
+        N = L * 6 * D + 2 * D
+        Wm, bm, c = rn("Wmod", (N, D), bf, 0.02), rn("bmod", (N,), bf, 0.02), rn("c", (1, D), torch.float32)
+        hbm(f"gemv modulation N={N} K={D}", N * D * 2 + N * 2 + N * 4, lambda: B.dit_gemv(c, Wm, bm, silu_input=True))
+        del Wm
+    # ---- QK-RMSNorm + RoPE in place on q,k (read + write 2 of the 3 thirds of qkv)
+    for T, H in ((4352, 24), (32760, 40)):
+        D = H * 128
+        qkv = rn("qkv", (T, 3 * D), bf)
+        g = rn("g", (128,), bf, 0.02) + 1
+        rc, rs = rn("rc", (T, 64), torch.float32), rn("rs", (T, 64), torch.float32)
+        hbm(f"qknorm_rope T={T} H={H}", 2 * 2 * T * D * 2 + 2 * T * 64 * 4,
+            lambda: B.dit_qknorm_rope(qkv, H, 128, 2, g, g, 1e-6, rc, rs))
+        del qkv
+    # ---- LSE merge (a14)
+    for Nq, H, P in ((32768, 40, 4), (4352, 24, 2), (32768, 40, 8)):
+        op = [rn(f"o{p}", (Nq, H, 128), bf) for p in range(P)]
+        lp = [rn(f"l{p}", (Nq, H), torch.float32) for p in range(P)]
+        hbm(f"merge Nq={Nq} H={H} P={P}", P * (Nq * H * 128 * 2 + Nq * H * 4) + Nq * H * 128 * 2 + Nq * H * 4,
+            lambda: B.dit_attn_merge(op, lp))
+        del op
+    # ---- attention sweep (cfg 5): unsplit, d=128
+    for H in (24, 40):
+        for N in (1024, 2048, 4096, 8192, 16384, 32768, 65536, 131072):
+            if args.steps < 20 and N > 32768:
+                continue
+            q, k, v = synth.make_attention_qkv(11, N, N, H, 128, device=dev)
+            tensor(f"attention H={H} N={N}", 4 * N * N * 128 * H, lambda: B.dit_attn_partial(q, k, v, want_lse=True))
+            del q, k, v
+    # ---- block GEMMs at cfg 2 / cfg 3 shapes
+    for nm, M, N, K, epi in (("qkv cfg2", 4352, 9216, 3072, B.EPI_BIAS), ("fc1 cfg2", 4352, 12288, 3072, B.EPI_BIAS_GELU),
+                             ("qkv cfg3", 32760, 15360, 5120, B.EPI_BIAS), ("fc1 cfg3", 32760, 13824, 5120, B.EPI_BIAS_GELU)):
+        A, Wt, b = rn("A", (M, K), bf), rn("W", (N, K), bf, 0.02), rn("b", (N,), bf, 0.02)
+        o = torch.empty((M, N), dtype=bf, device=dev)
+        tensor(f"gemm {nm} {M}x{N}x{K}", 2 * M * N * K, lambda: B.dit_linear(A, Wt, b, epi, out=o))
+        del A, Wt, o
+    for nm, M, N, K in (("out-proj cfg2", 4352, 3072, 3072), ("fc2 cfg2", 4352, 3072, 12288), ("fc2 cfg3", 32760, 5120, 13824)):
+        A, Wt, b = rn("A", (M, K), bf), rn("W", (N, K), bf, 0.02), rn("b", (N,), bf, 0.02)
+        x, g = rn("x", (M, N), torch.float32), rn("g", (1, N), torch.float32, 0.02)
+        tensor(f"gemm+gate-residual {nm} {M}x{N}x{K}", 2 * M * N * K, lambda: B.dit_linear_residual(A, Wt, x, b, g, N))
+        del A, Wt, x
+    print(json.dumps({"metric": "per-kernel roofline", "n_gpus": 1, "reps": reps, "warmup": args.warmup,
+                      "l2": "512 MB overwritten between timed launches", "peaks": pk, "kernels": rows}), flush=True)
+
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "kernels"])
     ap.add_argument("--split-p", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -322,7 +420,10 @@ def main():
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
-    if args.impl == "reference":
+    if args.workload == "kernels":
+        if rank == 0:
+            run_kernels(args)
+    elif args.impl == "reference":
         run_reference(args, rank)
     else:
         run_ours(args, rank, local_rank, world)

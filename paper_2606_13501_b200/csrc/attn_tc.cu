@@ -4,17 +4,22 @@
 // Design (sm_100a), one CTA = one (request, head, 256 query rows) work item, 384 threads:
 //   warp 0      TMA producer: two Q tiles (128 x 128) once, then a K ring and a V ring of 128-key tiles
 //               (each tile = two 128 x 64 boxes, 128-byte swizzle);
-//   warp 1      MMA issuer (one thread): S_t = Q_t K_j^T (M=128, N=128, K=16 x 8, both operands K-major from
-//               shared memory) into TMEM, then O_t += P_t V_j with P read from TMEM (A operand in tensor memory)
-//               and V as an MN-major shared-memory operand; the two Q tiles ping-pong so the tensor pipe computes
-//               one tile's S / PV while the other tile's softmax runs;
+//   warp 1      MMA issuer (one thread).  Keys are consumed in SUB-TILES of 64: S_t,i = Q_t K_i^T (M=128, N=64,
+//               K=16 x 8) into one of TWO 64-column S buffers per Q tile, O_t += P_t,i V_i (M=128, N=128, K=16 x 4)
+//               with P read from TMEM (A operand in tensor memory) and V as an MN-major shared-memory operand.
+//               S_t,i+2 is issued right after PV_t,i (same buffer, in-order tensor pipe), so while a softmax
+//               warpgroup works on sub-tile i the scores of sub-tile i+1 are already in TMEM: neither side waits
+//               on a round trip through the other;
 //   warps 4-7   softmax warpgroup of Q tile 0, warps 8-11 of Q tile 1: one thread owns one query row — tcgen05.ld
-//               of the whole 128-wide S row, row max, exp2 with the scale folded into one FFMA, bf16 P written back
-//               over S in TMEM (tcgen05.st), fp32 row sum.  O is rescaled lazily: only when the running max grows
-//               by more than 2^8 (exact: the same max is used for P and for the sum, and divided out at the end);
+//               of the 64 scores, row max, exp2 with the scale folded into one packed FFMA2, bf16 P written back
+//               over the first 32 columns of the S buffer (tcgen05.st), fp32 row sum (packed FADD2).  A quarter of
+//               the exponentials is evaluated on the FMA pipe (round-to-nearest split + minimax cubic, rel. error
+//               7.5e-5 << bf16 rounding of P) because MUFU.EX2 (16 / clk / SM) would otherwise need exactly as many
+//               cycles as the two MMAs of the tile.  O is rescaled lazily: only when the running max grows by more
+//               than 2^8 (exact: the same max is used for P and for the sum, and divided out at the end);
 //   epilogue    the same warpgroups: O / l -> bf16 -> global, lse = ln2 * (m + log2 l).
-// TMEM: S0 | S1 | O0 | O1 = 4 x 128 fp32 columns = all 512; P_t aliases the first 64 columns of S_t.
-// Roofline: tensor pipe, co-limited by MUFU.EX2 (16 / clk / SM): 2 x 128 x 128 exps per 2048 tensor cycles.
+// TMEM: S0a S0b | S1a S1b | O0 | O1 = 4 x 128 fp32 columns = all 512; P_t,b aliases the first 32 columns of S_t,b.
+// Roofline: tensor pipe, co-limited by MUFU.EX2 and FMA issue slots.
 #include "tc.cuh"
 
 namespace dit {
@@ -24,13 +29,16 @@ namespace {
 
 constexpr int HD = 128;          // head dim
 constexpr int TQ = 128;          // query rows per tile (2 tiles per CTA)
-constexpr int TK = 128;          // keys per tile
+constexpr int TK = 128;          // keys per TMA tile
+constexpr int SK = 64;           // keys per S / P sub-tile (two sub-tiles per TMA tile)
 constexpr int KS = 2, VS = 2;    // K / V ring depths
 constexpr int TILE_BYTES = 128 * HD * 2;   // 32 KB: two [128 x 64] swizzled boxes
 constexpr int HALF_BYTES = TILE_BYTES / 2;
+constexpr int SUB_BYTES = SK * 128;        // 64 rows of a swizzled box
 constexpr int ATTN_THREADS = 384;
 constexpr int ATTN_SMEM = (2 + KS + VS) * TILE_BYTES + 1024 + 256;
 constexpr float RESCALE_THRESHOLD = 8.0f;  // log2 units
+constexpr int POLY_PAIRS = 4;              // of every 16 score pairs, this many take the FMA-pipe exp2
 
 struct AttnParams {
   bf16* o; int64_t o_stride;
@@ -43,10 +51,52 @@ struct AttnParams {
 
 __device__ __forceinline__ float ex2(float x) {
   float y;
-  asm volatile("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
-
+// packed fp32 pairs (sm_100 FFMA2 / FADD2): one issue slot for two elements
+__device__ __forceinline__ uint64_t pack2(float lo, float hi) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void unpack2(uint64_t v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+__device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+// 2^x on the FMA pipe for a packed pair, x <= ~9:  x = n + f, n = rint(x), f in [-0.5, 0.5];
+// 2^f ~ minimax cubic (rel. error 7.5e-5), 2^n by adding n to the exponent field.  x is clamped at -126 so the
+// exponent cannot wrap (masked scores are -inf): the result is then < 2^-125, i.e. zero for every purpose here.
+__device__ __forceinline__ void ex2_poly2(uint64_t x2, float& a, float& b) {
+  float xa, xb;
+  unpack2(x2, xa, xb);
+  xa = fmaxf(xa, -126.0f);
+  xb = fmaxf(xb, -126.0f);
+  const uint64_t x = pack2(xa, xb);
+  const uint64_t magic = pack2(12582912.0f, 12582912.0f);      // 1.5 * 2^23: low mantissa bits hold rint(x)
+  const uint64_t nmagic = pack2(-12582912.0f, -12582912.0f);
+  const uint64_t r = add2(x, magic);
+  const uint64_t n = add2(r, nmagic);
+  const uint64_t neg1 = pack2(-1.0f, -1.0f);
+  const uint64_t f = fma2(n, neg1, x);                          // x - n, exact
+  uint64_t p = fma2(f, pack2(0.05517132207751274f, 0.05517132207751274f), pack2(0.24261054396629333f, 0.24261054396629333f));
+  p = fma2(p, f, pack2(0.6932609677314758f, 0.6932609677314758f));
+  p = fma2(p, f, pack2(0.9999281167984009f, 0.9999281167984009f));
+  float ra, rb, pa, pb;
+  unpack2(r, ra, rb);
+  unpack2(p, pa, pb);
+  a = __int_as_float(__float_as_int(pa) + (__float_as_int(ra) << 23));
+  b = __int_as_float(__float_as_int(pb) + (__float_as_int(rb) << 23));
+}
 
 __device__ __forceinline__ void mask32(uint32_t (&s)[32], int valid) {
 #pragma unroll
@@ -63,16 +113,23 @@ __device__ __forceinline__ float max32(const uint32_t (&s)[32]) {
   }
   return fmaxf(fmaxf(m0, m1), fmaxf(m2, m3));
 }
-// p = 2^(s c + nm) for 32 scores -> 16 bf16 pairs into TMEM columns [taddr, taddr + 16); fp32 partial sums
-__device__ __forceinline__ void exp_pack_store(const uint32_t (&s)[32], float c, float nm, uint32_t taddr, float& sum0,
-                                               float& sum1) {
+// p = 2^(s c + nm) for 32 scores -> 16 bf16 pairs into TMEM columns [taddr, taddr + 16); packed fp32 partial sums
+__device__ __forceinline__ void exp_pack_store(const uint32_t (&s)[32], uint64_t c2, uint64_t nm2, uint32_t taddr,
+                                               uint64_t& sum2) {
   uint32_t pk[16];
 #pragma unroll
   for (int i = 0; i < 16; ++i) {
-    const float a = ex2(fmaf(__uint_as_float(s[2 * i]), c, nm));
-    const float b = ex2(fmaf(__uint_as_float(s[2 * i + 1]), c, nm));
-    sum0 += a;
-    sum1 += b;
+    const uint64_t x = fma2(pack2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1])), c2, nm2);
+    float a, b;
+    if (i % 4 == 3 && i / 4 < POLY_PAIRS) {   // spread over the chunk so MUFU and FMA work interleave
+      ex2_poly2(x, a, b);
+    } else {
+      float xa, xb;
+      unpack2(x, xa, xb);
+      a = ex2(xa);
+      b = ex2(xb);
+    }
+    sum2 = add2(sum2, pack2(a, b));
     pk[i] = pack_bf16(a, b);
   }
   tmem_st16(taddr, pk);
@@ -91,10 +148,12 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   auto k_empty = [&](int s) { return bar0 + 8u * (2 + KS + s); };
   auto v_full = [&](int s) { return bar0 + 8u * (2 + 2 * KS + s); };
   auto v_empty = [&](int s) { return bar0 + 8u * (2 + 2 * KS + VS + s); };
-  auto s_full = [&](int t) { return bar0 + 8u * (2 + 2 * KS + 2 * VS + t); };
-  auto p_full = [&](int t) { return bar0 + 8u * (4 + 2 * KS + 2 * VS + t); };
-  auto pv_done = [&](int t) { return bar0 + 8u * (6 + 2 * KS + 2 * VS + t); };
-  const uint32_t tmem_slot = bar0 + 8u * (8 + 2 * KS + 2 * VS);
+  constexpr int B0 = 2 + 2 * KS + 2 * VS;
+  auto s_full = [&](int t, int b) { return bar0 + 8u * (B0 + 2 * t + b); };
+  auto p_full = [&](int t, int b) { return bar0 + 8u * (B0 + 4 + 2 * t + b); };
+  // PV_t,i completes pv_done(t, i & 1): a waiter is never more than one phase behind a per-buffer barrier
+  auto pv_done = [&](int t, int b) { return bar0 + 8u * (B0 + 8 + 2 * t + b); };
+  const uint32_t tmem_slot = bar0 + 8u * (B0 + 12);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int req = blockIdx.z, head = blockIdx.y;
@@ -109,6 +168,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   if (k_hi > k_hi0) k_hi = k_hi0;
   const int kv_len = k_hi - k_lo;
   const int n_tiles = (kv_len + TK - 1) / TK;
+  const int n_sub = (kv_len + SK - 1) / SK;
 
   if (n_tiles == 0) {  // empty shard: o = 0, lse = -inf (R18)
     if (warp >= 4) {
@@ -130,9 +190,11 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   if (warp == 1 && lane == 0) {
     for (int t = 0; t < 2; ++t) {
       mbar_init(q_full(t), 1);
-      mbar_init(s_full(t), 1);
-      mbar_init(p_full(t), 128);
-      mbar_init(pv_done(t), 1);
+      for (int b = 0; b < 2; ++b) {
+        mbar_init(pv_done(t, b), 1);
+        mbar_init(s_full(t, b), 1);
+        mbar_init(p_full(t, b), 4);      // one arrival per softmax warp
+      }
     }
     for (int s = 0; s < KS; ++s) { mbar_init(k_full(s), 1); mbar_init(k_empty(s), 1); }
     for (int s = 0; s < VS; ++s) { mbar_init(v_full(s), 1); mbar_init(v_empty(s), 1); }
@@ -180,64 +242,72 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     }
   } else if (warp == 1) {
     // ===================================================== MMA issuer
-    constexpr uint32_t idesc_s = idesc_bf16(TQ, TK, 0, 0);   // S = Q K^T: A, B K-major
+    constexpr uint32_t idesc_s = idesc_bf16(TQ, SK, 0, 0);   // S = Q K^T: A, B K-major, N = 64 keys
     constexpr uint32_t idesc_o = idesc_bf16(TQ, HD, 0, 1);   // O += P V: A from TMEM, B (V) MN-major
     // V tile: two [128 keys x 64 d] boxes 16 KB apart (LBO), 8-key groups 1 KB apart (SBO); 16 keys = +2 KB
     constexpr uint64_t vdesc_hi = desc_base_sw128(HALF_BYTES >> 4, 64);
-    auto issue_s = [&](int t, int sk) {
-      const uint32_t d = tmem_base + t * 128;
-      const uint32_t qa = sQ + t * TILE_BYTES, ka = sK + sk * TILE_BYTES;
+    // sub-tile i lives in TMA tile i >> 1 (ring stage (i >> 1) % KS), rows (i & 1) * 64 ...
+    auto issue_s = [&](int t, int i) {
+      const uint32_t d = tmem_base + t * 128 + (i & 1) * SK;
+      const uint32_t qa = sQ + t * TILE_BYTES, ka = sK + ((i >> 1) % KS) * TILE_BYTES + (i & 1) * SUB_BYTES;
 #pragma unroll
       for (int k = 0; k < HD / 16; ++k) {
         const uint32_t off = (k >> 2) * HALF_BYTES + (k & 3) * 32;
         umma_ss(d, desc_kmajor_sw128(qa + off), desc_kmajor_sw128(ka + off), idesc_s, k != 0);
       }
     };
-    auto issue_pv = [&](int t, int sv, bool acc) {
+    auto issue_pv = [&](int t, int i) {
       const uint32_t d = tmem_base + 256 + t * 128;
-      const uint32_t pa = tmem_base + t * 128;  // P_t: bf16 pairs in the first 64 columns of S_t
-      const uint32_t va = sV + sv * TILE_BYTES;
+      const uint32_t pa = tmem_base + t * 128 + (i & 1) * SK;  // P_t,b: bf16 pairs in the first 32 columns of S_t,b
+      const uint32_t va = sV + ((i >> 1) % VS) * TILE_BYTES + (i & 1) * SUB_BYTES;
 #pragma unroll
-      for (int k = 0; k < TK / 16; ++k)
-        umma_ts(d, pa + 8 * k, vdesc_hi | (uint64_t)(((va + k * 2048) >> 4) & 0x3fff), idesc_o, acc || k != 0);
+      for (int k = 0; k < SK / 16; ++k)
+        umma_ts(d, pa + 8 * k, vdesc_hi | (uint64_t)(((va + k * 2048) >> 4) & 0x3fff), idesc_o, (i > 0 || k != 0) ? 1u : 0u);
     };
-    int sk = 0, sv = 0;
-    uint32_t pk = 0, pv = 0;
+    auto last_of_tile = [&](int i) { return (i & 1) == 1 || i == n_sub - 1; };
+    // prologue: S_t,0 and S_t,1 for both Q tiles
     mbar_wait(q_full(0), 0);
     mbar_wait(k_full(0), 0);
     tc_fence_after();
-    if (lane == 0) { issue_s(0, 0); umma_commit(s_full(0)); }
+    if (lane == 0) { issue_s(0, 0); umma_commit(s_full(0, 0)); }
     mbar_wait(q_full(1), 0);
     tc_fence_after();
-    if (lane == 0) { issue_s(1, 0); umma_commit(s_full(1)); umma_commit(k_empty(0)); }
+    if (lane == 0) {
+      issue_s(1, 0); umma_commit(s_full(1, 0));
+      if (n_sub > 1) {
+        issue_s(0, 1); umma_commit(s_full(0, 1));
+        issue_s(1, 1); umma_commit(s_full(1, 1));
+      }
+      umma_commit(k_empty(0));
+    }
     __syncwarp();
-    if (++sk == KS) { sk = 0; pk ^= 1; }
-    for (int j = 0; j < n_tiles; ++j) {
+    for (int i = 0; i < n_sub; ++i) {
+      const int b = i & 1;
+      const uint32_t par = (uint32_t)(i >> 1) & 1u;
       for (int t = 0; t < 2; ++t) {
-        if (t == 0) mbar_wait(v_full(sv), pv);
-        mbar_wait(p_full(t), j & 1);
+        if (t == 0 && b == 0) mbar_wait(v_full((i >> 1) % VS), (uint32_t)((i >> 1) / VS) & 1u);
+        mbar_wait(p_full(t, b), par);
         tc_fence_after();
         if (lane == 0) {
-          issue_pv(t, sv, j > 0);
-          umma_commit(pv_done(t));
-          if (t == 1) umma_commit(v_empty(sv));
+          issue_pv(t, i);
+          umma_commit(pv_done(t, b));
+          if (t == 1 && last_of_tile(i)) umma_commit(v_empty((i >> 1) % VS));
         }
         __syncwarp();
-        if (j + 1 < n_tiles) {
-          if (t == 0) {
-            mbar_wait(k_full(sk), pk);
+        const int i2 = i + 2;
+        if (i2 < n_sub) {
+          if (t == 0 && b == 0) {
+            mbar_wait(k_full((i2 >> 1) % KS), (uint32_t)((i2 >> 1) / KS) & 1u);
             tc_fence_after();
           }
           if (lane == 0) {
-            issue_s(t, sk);
-            umma_commit(s_full(t));
-            if (t == 1) umma_commit(k_empty(sk));
+            issue_s(t, i2);
+            umma_commit(s_full(t, b));
+            if (t == 1 && last_of_tile(i2)) umma_commit(k_empty((i2 >> 1) % KS));
           }
           __syncwarp();
         }
       }
-      if (++sv == VS) { sv = 0; pv ^= 1; }
-      if (j + 1 < n_tiles) { if (++sk == KS) { sk = 0; pk ^= 1; } }
     }
   }
   } else {
@@ -247,35 +317,34 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     const int quad = warp & 3;                     // TMEM lane quadrant of this warp
     const int row = q_base + t * TQ + quad * 32 + lane;
     const uint32_t lane_off = (uint32_t)(quad * 32) << 16;
-    const uint32_t s_addr = tmem_base + t * 128 + lane_off;        // S_t (fp32) and P_t (bf16 pairs, 64 columns)
+    const uint32_t s_base = tmem_base + t * 128 + lane_off;        // S_t,b (fp32, 64 cols) / P_t,b (bf16 pairs, 32 cols)
     const uint32_t o_addr = tmem_base + 256 + t * 128 + lane_off;  // O_t
     const float c = p.scale_log2;
+    const uint64_t c2 = pack2(c, c);
     float m_used = -INFINITY;   // running max in log2 units (raw score * c) that P and l are expressed against
     float l = 0.f;
-    for (int j = 0; j < n_tiles; ++j) {
-      mbar_wait(s_full(t), j & 1);
+    for (int i = 0; i < n_sub; ++i) {
+      const int b = i & 1;
+      const uint32_t s_addr = s_base + b * SK;
+      mbar_wait(s_full(t, b), (uint32_t)(i >> 1) & 1u);
       tc_fence_after();
-      uint32_t s0[32], s1[32], s2[32], s3[32];      // the thread's whole S row (four register arrays of 32)
+      uint32_t s0[32], s1[32];                     // the thread's 64 scores of this sub-tile
       tmem_ld32(s_addr + 0, s0);
       tmem_ld32(s_addr + 32, s1);
-      tmem_ld32(s_addr + 64, s2);
-      tmem_ld32(s_addr + 96, s3);
       tmem_ld_wait();
-      const int valid = kv_len - j * TK;           // keys of this tile that exist (warp-uniform)
-      if (valid < TK) {                            // -inf before the row max
+      const int valid = kv_len - i * SK;           // keys of this sub-tile that exist (warp-uniform, >= 1)
+      if (valid < SK) {                            // -inf before the row max
         mask32(s0, valid);
         mask32(s1, valid - 32);
-        mask32(s2, valid - 64);
-        mask32(s3, valid - 96);
       }
-      const float mx = fmaxf(fmaxf(max32(s0), max32(s1)), fmaxf(max32(s2), max32(s3)));
+      const float mx = fmaxf(max32(s0), max32(s1));
       const float m_new = fmaxf(m_used, mx * c);   // c > 0
-      if (j == 0) {
+      if (i == 0) {
         m_used = m_new;                            // PV_0 overwrites O: nothing to rescale
       } else {
         const bool need = (m_new - m_used) > RESCALE_THRESHOLD;
-        if (__any_sync(0xffffffffu, need)) {       // lazy rescale of O_t (rare): wait for PV_t(j-1), then O *= f
-          mbar_wait(pv_done(t), (j - 1) & 1);
+        if (__any_sync(0xffffffffu, need)) {       // lazy rescale of O_t (rare): wait for PV_t(i-1), then O *= f
+          mbar_wait(pv_done(t, (i - 1) & 1), (uint32_t)((i - 1) >> 1) & 1u);
           tc_fence_after();
           const float f = need ? ex2(m_used - m_new) : 1.0f;
 #pragma unroll 1
@@ -284,7 +353,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
             tmem_ld16(o_addr + cc * 16, o);
             tmem_ld_wait();
 #pragma unroll
-            for (int i = 0; i < 16; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * f);
+            for (int e = 0; e < 16; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * f);
             tmem_st16(o_addr + cc * 16, o);
           }
           tmem_st_wait();
@@ -292,22 +361,23 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
           if (need) m_used = m_new;
         }
       }
-      // P = 2^(s c - m_used): one FFMA + one EX2 per element; row sum in fp32; bf16 pairs back into TMEM
-      const float nm = -m_used;
-      float sum0 = 0.f, sum1 = 0.f;
-      exp_pack_store(s0, c, nm, s_addr + 0, sum0, sum1);
-      exp_pack_store(s1, c, nm, s_addr + 16, sum0, sum1);
-      exp_pack_store(s2, c, nm, s_addr + 32, sum0, sum1);
-      exp_pack_store(s3, c, nm, s_addr + 48, sum0, sum1);
-      l += sum0 + sum1;
+      // P = 2^(s c - m_used): one packed FFMA per pair, EX2 (MUFU or FMA pipe), row sum in fp32, bf16 pairs -> TMEM
+      const uint64_t nm2 = pack2(-m_used, -m_used);
+      uint64_t sum2 = pack2(0.f, 0.f);
+      exp_pack_store(s0, c2, nm2, s_addr + 0, sum2);
+      exp_pack_store(s1, c2, nm2, s_addr + 16, sum2);
+      float sa, sb;
+      unpack2(sum2, sa, sb);
+      l += sa + sb;
       tmem_st_wait();
       tc_fence_before();
-      mbar_arrive(p_full(t));
+      __syncwarp();
+      if (lane == 0) mbar_arrive(p_full(t, b));
     }
     // ---- epilogue: O_t / l -> bf16 -> global; lse = ln2 (m + log2 l)
-    mbar_wait(pv_done(t), (n_tiles - 1) & 1);
+    mbar_wait(pv_done(t, (n_sub - 1) & 1), (uint32_t)((n_sub - 1) >> 1) & 1u);
     tc_fence_after();
-    const float inv = 1.0f / l;                    // l >= 2^-8 > 0: every tile has at least one valid key
+    const float inv = 1.0f / l;                    // l >= 2^-8 > 0: every sub-tile has at least one valid key
     const bool row_ok = row < q_hi;
     bf16* orow = p.o + (int64_t)(row_ok ? row : q_lo) * p.o_stride + head * HD;
 #pragma unroll 1
