@@ -341,12 +341,16 @@ def run_kernels(args):
     rows = []
 
     def hbm(name, nbytes, fn):
+        if args.only and args.only not in name:
+            return
         med, best = timeit(fn)
         gbs = nbytes / (med * 1e-3) / 1e9
         rows.append({"kernel": name, "bound": "hbm", "bytes": nbytes, "ms": round(med, 5), "ms_best": round(best, 5),
                      "achieved": round(gbs, 1), "unit": "GB/s", "peak": pk["hbm"], "frac": round(gbs / pk["hbm"], 4)})
 
     def tensor(name, flops, fn):
+        if args.only and args.only not in name:
+            return
         med, best = timeit(fn)
         tf = flops / (med * 1e-3) / 1e12
         rows.append({"kernel": name, "bound": "tensor", "flops": flops, "ms": round(med, 5), "ms_best": round(best, 5),
@@ -415,6 +419,7 @@ def main():
     ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "kernels"])
     ap.add_argument("--split-p", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--only", default="", help="--workload kernels: time only the kernels whose name contains this")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     rank = int(os.environ.get("RANK", "0"))

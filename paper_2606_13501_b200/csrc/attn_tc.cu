@@ -213,7 +213,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   if (warp == 0) {
     // ===================================================== TMA producer
     const int c0 = head * HD;
-    if (lane == 0) {
+    if (elect_one()) {
       for (int t = 0; t < 2; ++t) {
         mbar_expect_tx(q_full(t), TILE_BYTES);
         tma_load_2d(sQ + t * TILE_BYTES, &tmQ, c0, q_base + t * TQ, q_full(t));
@@ -225,14 +225,14 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     for (int j = 0; j < n_tiles; ++j) {
       const int r0 = k_lo + j * TK;
       mbar_wait(k_empty(sk), pk ^ 1);
-      if (lane == 0) {
+      if (elect_one()) {
         mbar_expect_tx(k_full(sk), TILE_BYTES);
         tma_load_2d(sK + sk * TILE_BYTES, &tmK, c0, r0, k_full(sk));
         tma_load_2d(sK + sk * TILE_BYTES + HALF_BYTES, &tmK, c0 + 64, r0, k_full(sk));
       }
       if (++sk == KS) { sk = 0; pk ^= 1; }
       mbar_wait(v_empty(sv), pv ^ 1);
-      if (lane == 0) {
+      if (elect_one()) {
         mbar_expect_tx(v_full(sv), TILE_BYTES);
         tma_load_2d(sV + sv * TILE_BYTES, &tmV, c0, r0, v_full(sv));
         tma_load_2d(sV + sv * TILE_BYTES + HALF_BYTES, &tmV, c0 + 64, r0, v_full(sv));
@@ -269,10 +269,10 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     mbar_wait(q_full(0), 0);
     mbar_wait(k_full(0), 0);
     tc_fence_after();
-    if (lane == 0) { issue_s(0, 0); umma_commit(s_full(0, 0)); }
+    if (elect_one()) { issue_s(0, 0); umma_commit(s_full(0, 0)); }
     mbar_wait(q_full(1), 0);
     tc_fence_after();
-    if (lane == 0) {
+    if (elect_one()) {
       issue_s(1, 0); umma_commit(s_full(1, 0));
       if (n_sub > 1) {
         issue_s(0, 1); umma_commit(s_full(0, 1));
@@ -288,7 +288,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
         if (t == 0 && b == 0) mbar_wait(v_full((i >> 1) % VS), (uint32_t)((i >> 1) / VS) & 1u);
         mbar_wait(p_full(t, b), par);
         tc_fence_after();
-        if (lane == 0) {
+        if (elect_one()) {
           issue_pv(t, i);
           umma_commit(pv_done(t, b));
           if (t == 1 && last_of_tile(i)) umma_commit(v_empty((i >> 1) % VS));
@@ -300,7 +300,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
             mbar_wait(k_full((i2 >> 1) % KS), (uint32_t)((i2 >> 1) / KS) & 1u);
             tc_fence_after();
           }
-          if (lane == 0) {
+          if (elect_one()) {
             issue_s(t, i2);
             umma_commit(s_full(t, b));
             if (t == 1 && last_of_tile(i2)) umma_commit(k_empty((i2 >> 1) % KS));

@@ -120,7 +120,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       const int m0 = (t % mt) * BM, n0 = (t / mt) * BN;
       for (int kb = 0; kb < nkb; ++kb) {
         mbar_wait(empty_bar(s), ph ^ 1);
-        if (lane == 0) {
+        if (elect_one()) {
           mbar_expect_tx(full_bar(s), STAGE_BYTES);
           tma_load_2d(smem0 + s * STAGE_BYTES, &tmA, kb * BK, m0, full_bar(s));
           tma_load_2d(smem0 + s * STAGE_BYTES + A_BYTES, &tmB, kb * BK, n0, full_bar(s));
@@ -144,7 +144,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       for (int kb = 0; kb < nkb; ++kb) {
         mbar_wait(full_bar(s), ph);
         tc_fence_after();
-        if (lane == 0) {
+        if (elect_one()) {
           const uint64_t ad = desc_kmajor_sw128(smem0 + s * STAGE_BYTES);
           const uint64_t bd = desc_kmajor_sw128(smem0 + s * STAGE_BYTES + A_BYTES);
 #pragma unroll

@@ -39,6 +39,19 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   }
 }
 
+// One lane of the (fully converged) warp.  ptxas knows that code guarded by an elect.sync predicate runs in a
+// single thread, so tcgen05 / TMA operands go to uniform registers with one R2UR instead of a per-instruction
+// "waterfall" loop (ELECT + R2UR.BROADCAST + BRA.U.ANY), which `lane == 0` does not give.
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "elect.sync _|p, 0xffffffff;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(pred));
+  return pred != 0;
+}
+
 // ------------------------------------------------------------------------------------------- TMA
 __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* m) {
   asm volatile("prefetch.tensormap [%0];" ::"l"(m) : "memory");
