@@ -38,7 +38,10 @@ constexpr int SUB_BYTES = SK * 128;        // 64 rows of a swizzled box
 constexpr int ATTN_THREADS = 384;
 constexpr int ATTN_SMEM = (2 + KS + VS) * TILE_BYTES + 1024 + 256;
 constexpr float RESCALE_THRESHOLD = 8.0f;  // log2 units
-constexpr int POLY_PAIRS = 4;              // of every 16 score pairs, this many take the FMA-pipe exp2
+#ifndef DIT_ATTN_POLY_PAIRS
+#define DIT_ATTN_POLY_PAIRS 4
+#endif
+constexpr int POLY_PAIRS = DIT_ATTN_POLY_PAIRS;   // of every 16 score pairs, this many take the FMA-pipe exp2
 
 struct AttnParams {
   bf16* o; int64_t o_stride;
@@ -115,7 +118,7 @@ __device__ __forceinline__ float max32(const uint32_t (&s)[32]) {
 }
 // p = 2^(s c + nm) for 32 scores -> 16 bf16 pairs into TMEM columns [taddr, taddr + 16); packed fp32 partial sums
 __device__ __forceinline__ void exp_pack_store(const uint32_t (&s)[32], uint64_t c2, uint64_t nm2, uint32_t taddr,
-                                               uint64_t& sum2) {
+                                               uint64_t& sum2, uint64_t& sum2b) {
   uint32_t pk[16];
 #pragma unroll
   for (int i = 0; i < 16; ++i) {
@@ -129,7 +132,8 @@ __device__ __forceinline__ void exp_pack_store(const uint32_t (&s)[32], uint64_t
       a = ex2(xa);
       b = ex2(xb);
     }
-    sum2 = add2(sum2, pack2(a, b));
+    if (i & 1) sum2b = add2(sum2b, pack2(a, b));   // two independent chains
+    else sum2 = add2(sum2, pack2(a, b));
     pk[i] = pack_bf16(a, b);
   }
   tmem_st16(taddr, pk);
@@ -196,8 +200,8 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
         mbar_init(p_full(t, b), 4);      // one arrival per softmax warp
       }
     }
-    for (int s = 0; s < KS; ++s) { mbar_init(k_full(s), 1); mbar_init(k_empty(s), 1); }
-    for (int s = 0; s < VS; ++s) { mbar_init(v_full(s), 1); mbar_init(v_empty(s), 1); }
+    for (int s = 0; s < KS; ++s) { mbar_init(k_full(s), 1); mbar_init(k_empty(s), 2); }   // empty: one commit per Q tile
+    for (int s = 0; s < VS; ++s) { mbar_init(v_full(s), 1); mbar_init(v_empty(s), 2); }
     fence_barrier_init();
   }
   if (warp == 2) tmem_alloc<512>(tmem_slot);
@@ -242,20 +246,22 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     }
   } else if (warp == 1) {
     // ===================================================== MMA issuer
-    constexpr uint32_t idesc_s = idesc_bf16(TQ, SK, 0, 0);   // S = Q K^T: A, B K-major, N = 64 keys
+    constexpr uint32_t idesc_s = idesc_bf16(TQ, TK, 0, 0);   // S = Q K^T: A, B K-major, N = 128 keys (both sub-tiles)
     constexpr uint32_t idesc_o = idesc_bf16(TQ, HD, 0, 1);   // O += P V: A from TMEM, B (V) MN-major
     // V tile: two [128 keys x 64 d] boxes 16 KB apart (LBO), 8-key groups 1 KB apart (SBO); 16 keys = +2 KB
     constexpr uint64_t vdesc_hi = desc_base_sw128(HALF_BYTES >> 4, 64);
-    // sub-tile i lives in TMA tile i >> 1 (ring stage (i >> 1) % KS), rows (i & 1) * 64 ...
-    auto issue_s = [&](int t, int i) {
-      const uint32_t d = tmem_base + t * 128 + (i & 1) * SK;
-      const uint32_t qa = sQ + t * TILE_BYTES, ka = sK + ((i >> 1) % KS) * TILE_BYTES + (i & 1) * SUB_BYTES;
+    // S of key tile j for Q tile t: ONE N = 128 group fills both 64-column buffers (8 KB of shared memory per
+    // 64-cycle MMA = 128 B/clk; N = 64 groups would re-read Q for half the work and run shared-memory bound)
+    auto issue_s = [&](int t, int j) {
+      const uint32_t d = tmem_base + t * 128;
+      const uint32_t qa = sQ + t * TILE_BYTES, ka = sK + (j % KS) * TILE_BYTES;
 #pragma unroll
       for (int k = 0; k < HD / 16; ++k) {
         const uint32_t off = (k >> 2) * HALF_BYTES + (k & 3) * 32;
         umma_ss(d, desc_kmajor_sw128(qa + off), desc_kmajor_sw128(ka + off), idesc_s, k != 0);
       }
     };
+    // sub-tile i lives in TMA tile i >> 1 (ring stage (i >> 1) % VS), rows (i & 1) * 64 ...
     auto issue_pv = [&](int t, int i) {
       const uint32_t d = tmem_base + 256 + t * 128;
       const uint32_t pa = tmem_base + t * 128 + (i & 1) * SK;  // P_t,b: bf16 pairs in the first 32 columns of S_t,b
@@ -264,49 +270,50 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
       for (int k = 0; k < SK / 16; ++k)
         umma_ts(d, pa + 8 * k, vdesc_hi | (uint64_t)(((va + k * 2048) >> 4) & 0x3fff), idesc_o, (i > 0 || k != 0) ? 1u : 0u);
     };
-    auto last_of_tile = [&](int i) { return (i & 1) == 1 || i == n_sub - 1; };
-    // prologue: S_t,0 and S_t,1 for both Q tiles
+    // prologue: S of key tile 0 for both Q tiles
     mbar_wait(q_full(0), 0);
     mbar_wait(k_full(0), 0);
     tc_fence_after();
-    if (elect_one()) { issue_s(0, 0); umma_commit(s_full(0, 0)); }
+    if (elect_one()) { issue_s(0, 0); umma_commit(s_full(0, 0)); umma_commit(s_full(0, 1)); umma_commit(k_empty(0)); }
     mbar_wait(q_full(1), 0);
     tc_fence_after();
-    if (elect_one()) {
-      issue_s(1, 0); umma_commit(s_full(1, 0));
-      if (n_sub > 1) {
-        issue_s(0, 1); umma_commit(s_full(0, 1));
-        issue_s(1, 1); umma_commit(s_full(1, 1));
-      }
-      umma_commit(k_empty(0));
-    }
+    if (elect_one()) { issue_s(1, 0); umma_commit(s_full(1, 0)); umma_commit(s_full(1, 1)); umma_commit(k_empty(0)); }
     __syncwarp();
-    for (int i = 0; i < n_sub; ++i) {
-      const int b = i & 1;
-      const uint32_t par = (uint32_t)(i >> 1) & 1u;
+    // The two Q tiles advance INDEPENDENTLY: the issuer polls both tiles' p_full barriers and serves whichever
+    // softmax warpgroup has delivered its P.  (A fixed t = 0, 1 order locks the warpgroups into phase, so both run
+    // their softmax at the same time - sharing MUFU and issue slots - while the tensor pipe idles, and vice versa.)
+    // K / V stages are released by the second of the two tiles that is done with them (barrier count 2).
+    int it[2] = {0, 0};
+    while (it[0] < n_sub || it[1] < n_sub) {
+#pragma unroll
       for (int t = 0; t < 2; ++t) {
-        if (t == 0 && b == 0) mbar_wait(v_full((i >> 1) % VS), (uint32_t)((i >> 1) / VS) & 1u);
-        mbar_wait(p_full(t, b), par);
+        const int i = it[t];
+        if (i >= n_sub) continue;
+        const int b = i & 1, j = i >> 1;
+        if (!mbar_try_wait(p_full(t, b), (uint32_t)j & 1u)) continue;
+        if (b == 0) mbar_wait(v_full(j % VS), (uint32_t)(j / VS) & 1u);
         tc_fence_after();
+        const bool last_of_tile = b == 1 || i == n_sub - 1;
         if (elect_one()) {
           issue_pv(t, i);
           umma_commit(pv_done(t, b));
-          if (t == 1 && last_of_tile(i)) umma_commit(v_empty((i >> 1) % VS));
+          if (last_of_tile) umma_commit(v_empty(j % VS));
         }
         __syncwarp();
-        const int i2 = i + 2;
-        if (i2 < n_sub) {
-          if (t == 0 && b == 0) {
-            mbar_wait(k_full((i2 >> 1) % KS), (uint32_t)((i2 >> 1) / KS) & 1u);
-            tc_fence_after();
-          }
+        // both P buffers of Q tile t are consumed once PV_t of the tile's second sub-tile is queued: S of the next
+        // key tile may overwrite them (the tensor pipe executes in issue order)
+        if (b == 1 && j + 1 < n_tiles) {
+          mbar_wait(k_full((j + 1) % KS), (uint32_t)((j + 1) / KS) & 1u);
+          tc_fence_after();
           if (elect_one()) {
-            issue_s(t, i2);
-            umma_commit(s_full(t, b));
-            if (t == 1 && last_of_tile(i2)) umma_commit(k_empty((i2 >> 1) % KS));
+            issue_s(t, j + 1);
+            umma_commit(s_full(t, 0));
+            umma_commit(s_full(t, 1));
+            umma_commit(k_empty((j + 1) % KS));
           }
           __syncwarp();
         }
+        it[t] = i + 1;
       }
     }
   }
@@ -363,11 +370,11 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
       }
       // P = 2^(s c - m_used): one packed FFMA per pair, EX2 (MUFU or FMA pipe), row sum in fp32, bf16 pairs -> TMEM
       const uint64_t nm2 = pack2(-m_used, -m_used);
-      uint64_t sum2 = pack2(0.f, 0.f);
-      exp_pack_store(s0, c2, nm2, s_addr + 0, sum2);
-      exp_pack_store(s1, c2, nm2, s_addr + 16, sum2);
+      uint64_t sum2 = pack2(0.f, 0.f), sum2b = pack2(0.f, 0.f);
+      exp_pack_store(s0, c2, nm2, s_addr + 0, sum2, sum2b);
+      exp_pack_store(s1, c2, nm2, s_addr + 16, sum2, sum2b);
       float sa, sb;
-      unpack2(sum2, sa, sb);
+      unpack2(add2(sum2, sum2b), sa, sb);
       l += sa + sb;
       tmem_st_wait();
       tc_fence_before();
