@@ -35,11 +35,11 @@ constexpr int KS = 2, VS = 2;    // K / V ring depths
 constexpr int TILE_BYTES = 128 * HD * 2;   // 32 KB: two [128 x 64] swizzled boxes
 constexpr int HALF_BYTES = TILE_BYTES / 2;
 constexpr int SUB_BYTES = SK * 128;        // 64 rows of a swizzled box
-constexpr int ATTN_THREADS = 384;
-constexpr int ATTN_SMEM = (2 + KS + VS) * TILE_BYTES + 1024 + 256;
+constexpr int ATTN_THREADS = 640;         // 4 control warps + 16 softmax warps
+constexpr int ATTN_SMEM = (2 + KS + VS) * TILE_BYTES + 1024 + 256 + 6144;   // + row max / row sum exchange
 constexpr float RESCALE_THRESHOLD = 8.0f;  // log2 units
 #ifndef DIT_ATTN_POLY_PAIRS
-#define DIT_ATTN_POLY_PAIRS 4
+#define DIT_ATTN_POLY_PAIRS 2
 #endif
 constexpr int POLY_PAIRS = DIT_ATTN_POLY_PAIRS;   // of every 16 score pairs, this many take the FMA-pipe exp2
 
@@ -175,8 +175,8 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   const int n_sub = (kv_len + SK - 1) / SK;
 
   if (n_tiles == 0) {  // empty shard: o = 0, lse = -inf (R18)
-    if (warp >= 4) {
-      const int row = q_base + (warp - 4) * 32 + lane;
+    if (warp >= 4 && ((warp - 4) & 4) == 0) {   // the leader warps cover the 256 rows once
+      const int row = q_base + ((warp - 4) >> 3) * TQ + (warp & 3) * 32 + lane;
       if (row < q_hi) {
         const float z[8] = {0, 0, 0, 0, 0, 0, 0, 0};
         for (int c = 0; c < HD; c += 8) st8<bf16>(p.o + (int64_t)row * p.o_stride + head * HD + c, z);
@@ -213,7 +213,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
 
   // register budget: warpgroup 0 (TMA / MMA / idle warps) gives registers to the two softmax warpgroups
   if (warp < 4) {
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
   if (warp == 0) {
     // ===================================================== TMA producer
     const int c0 = head * HD;
@@ -279,95 +279,122 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     tc_fence_after();
     if (elect_one()) { issue_s(1, 0); umma_commit(s_full(1, 0)); umma_commit(s_full(1, 1)); umma_commit(k_empty(0)); }
     __syncwarp();
-    // The two Q tiles advance INDEPENDENTLY: the issuer polls both tiles' p_full barriers and serves whichever
-    // softmax warpgroup has delivered its P.  (A fixed t = 0, 1 order locks the warpgroups into phase, so both run
-    // their softmax at the same time - sharing MUFU and issue slots - while the tensor pipe idles, and vice versa.)
-    // K / V stages are released by the second of the two tiles that is done with them (barrier count 2).
-    int it[2] = {0, 0};
-    while (it[0] < n_sub || it[1] < n_sub) {
-#pragma unroll
+    // Per key tile j and Q tile t: PV of sub-tile a, PV of sub-tile b, then S of key tile j + 1 (both P buffers are
+    // consumed once the PVs are queued: the tensor pipe executes in issue order).  Serving t = 0 completely before
+    // t = 1 keeps the two Q tiles in anti-phase: one tile's softmax runs under the other tile's 1024 tensor cycles.
+    for (int j = 0; j < n_tiles; ++j) {
+      const uint32_t par = (uint32_t)j & 1u;
       for (int t = 0; t < 2; ++t) {
-        const int i = it[t];
-        if (i >= n_sub) continue;
-        const int b = i & 1, j = i >> 1;
-        if (!mbar_try_wait(p_full(t, b), (uint32_t)j & 1u)) continue;
-        if (b == 0) mbar_wait(v_full(j % VS), (uint32_t)(j / VS) & 1u);
+        if (t == 0) mbar_wait(v_full(j % VS), (uint32_t)(j / VS) & 1u);
+        mbar_wait(p_full(t, 0), par);
         tc_fence_after();
-        const bool last_of_tile = b == 1 || i == n_sub - 1;
         if (elect_one()) {
-          issue_pv(t, i);
-          umma_commit(pv_done(t, b));
-          if (last_of_tile) umma_commit(v_empty(j % VS));
+          issue_pv(t, 2 * j);
+          umma_commit(pv_done(t, 0));
         }
         __syncwarp();
-        // both P buffers of Q tile t are consumed once PV_t of the tile's second sub-tile is queued: S of the next
-        // key tile may overwrite them (the tensor pipe executes in issue order)
-        if (b == 1 && j + 1 < n_tiles) {
-          mbar_wait(k_full((j + 1) % KS), (uint32_t)((j + 1) / KS) & 1u);
+        if (2 * j + 1 < n_sub) {
+          mbar_wait(p_full(t, 1), par);
           tc_fence_after();
           if (elect_one()) {
+            issue_pv(t, 2 * j + 1);
+            umma_commit(pv_done(t, 1));
+          }
+          __syncwarp();
+        }
+        if (j + 1 < n_tiles && t == 0) {
+          mbar_wait(k_full((j + 1) % KS), (uint32_t)((j + 1) / KS) & 1u);
+          tc_fence_after();
+        }
+        if (elect_one()) {
+          umma_commit(v_empty(j % VS));
+          if (j + 1 < n_tiles) {
             issue_s(t, j + 1);
             umma_commit(s_full(t, 0));
             umma_commit(s_full(t, 1));
             umma_commit(k_empty((j + 1) % KS));
           }
-          __syncwarp();
         }
-        it[t] = i + 1;
+        __syncwarp();
       }
     }
   }
   } else {
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
-    // ===================================================== softmax + correction + epilogue warpgroups
-    const int t = (warp - 4) >> 2;                 // Q tile of this warpgroup
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 104;");
+    // ===================================================== softmax + correction + epilogue: 16 warps
+    // Q tile t has TWO warps per TMEM lane quadrant: the leader (h = 0) owns sub-tile a (keys 0..63 of every key
+    // tile), the follower (h = 1) sub-tile b (keys 64..127); both add into the same O_t, so they must use the same
+    // reference max.  The leader reads the whole 128-wide S row for the row max, takes the (lazy) rescale decision
+    // alone, and publishes m_used per key tile through shared memory + a named barrier (arrive / sync, 64 threads);
+    // the follower rescales its partial row sum when m_used changed.  Four softmax warps per scheduler instead of
+    // two: a single warp issues one instruction per ~3 cycles (dependent FFMA2 / MUFU chains), which made the
+    // softmax — not the tensor pipe and not MUFU — the critical path.
+    const int w = warp - 4;
+    const int t = w >> 3;                          // Q tile
+    const int h = (w >> 2) & 1;                    // 0 = leader (sub-tile a), 1 = follower (sub-tile b)
     const int quad = warp & 3;                     // TMEM lane quadrant of this warp
-    const int row = q_base + t * TQ + quad * 32 + lane;
+    const int r_in = quad * 32 + lane;             // row inside the Q tile
+    const int row = q_base + t * TQ + r_in;
     const uint32_t lane_off = (uint32_t)(quad * 32) << 16;
     const uint32_t s_base = tmem_base + t * 128 + lane_off;        // S_t,b (fp32, 64 cols) / P_t,b (bf16 pairs, 32 cols)
     const uint32_t o_addr = tmem_base + 256 + t * 128 + lane_off;  // O_t
+    float* const xch = reinterpret_cast<float*>(smem_raw + (bar0 - smem_u32(smem_raw)) + 256);
+    float* const m_sh = xch + t * 512;             // [parity][h][128 rows]: half-row maxima
+    float* const l_sh = xch + 1024 + t * 256;      // [h][128 rows]: partial row sums
+    const int bar_id = 1 + t * 4 + quad;           // named barrier of this (leader, follower) warp pair
     const float c = p.scale_log2;
     const uint64_t c2 = pack2(c, c);
     float m_used = -INFINITY;   // running max in log2 units (raw score * c) that P and l are expressed against
     float l = 0.f;
-    for (int i = 0; i < n_sub; ++i) {
-      const int b = i & 1;
-      const uint32_t s_addr = s_base + b * SK;
-      mbar_wait(s_full(t, b), (uint32_t)(i >> 1) & 1u);
-      tc_fence_after();
-      uint32_t s0[32], s1[32];                     // the thread's 64 scores of this sub-tile
-      tmem_ld32(s_addr + 0, s0);
-      tmem_ld32(s_addr + 32, s1);
-      tmem_ld_wait();
-      const int valid = kv_len - i * SK;           // keys of this sub-tile that exist (warp-uniform, >= 1)
-      if (valid < SK) {                            // -inf before the row max
-        mask32(s0, valid);
-        mask32(s1, valid - 32);
+    const uint32_t s_addr = s_base + h * SK;
+    for (int j = 0; j < n_tiles; ++j) {
+      const uint32_t par = (uint32_t)j & 1u;
+      uint32_t s0[32], s1[32];                     // the thread's 64 scores of its sub-tile
+      const int valid = kv_len - j * TK - h * SK;  // keys of this sub-tile that exist (warp-uniform; <= 0: none)
+      float mx = -INFINITY;
+      if (valid > 0) {
+        mbar_wait(s_full(t, h), par);
+        tc_fence_after();
+        tmem_ld32(s_addr + 0, s0);
+        tmem_ld32(s_addr + 32, s1);
+        tmem_ld_wait();
+        if (valid < SK) {                          // -inf before the row max
+          mask32(s0, valid);
+          mask32(s1, valid - 32);
+        }
+        mx = fmaxf(max32(s0), max32(s1));
       }
-      const float mx = fmaxf(max32(s0), max32(s1));
+      // the pair exchanges its half-row maxima: both threads then take the SAME rescale decision
+      m_sh[(par * 2 + h) * 128 + r_in] = mx;
+      asm volatile("bar.sync %0, 64;" ::"r"(bar_id) : "memory");
+      mx = fmaxf(mx, m_sh[(par * 2 + (h ^ 1)) * 128 + r_in]);
       const float m_new = fmaxf(m_used, mx * c);   // c > 0
-      if (i == 0) {
+      if (j == 0) {
         m_used = m_new;                            // PV_0 overwrites O: nothing to rescale
       } else {
         const bool need = (m_new - m_used) > RESCALE_THRESHOLD;
-        if (__any_sync(0xffffffffu, need)) {       // lazy rescale of O_t (rare): wait for PV_t(i-1), then O *= f
-          mbar_wait(pv_done(t, (i - 1) & 1), (uint32_t)((i - 1) >> 1) & 1u);
-          tc_fence_after();
+        if (__any_sync(0xffffffffu, need)) {
+          // lazy rescale (rare).  S(j) is complete, and it was issued after every PV of tile j - 1, so O_t is
+          // quiescent; PV_a(j) cannot be queued before the leader delivers P_a, and PV_b(j) is queued after PV_a(j),
+          // so the leader alone rescales O_t; both threads rescale their partial row sums.
           const float f = need ? ex2(m_used - m_new) : 1.0f;
+          if (h == 0) {
 #pragma unroll 1
-          for (int cc = 0; cc < 8; ++cc) {
-            uint32_t o[16];
-            tmem_ld16(o_addr + cc * 16, o);
-            tmem_ld_wait();
+            for (int cc = 0; cc < 8; ++cc) {
+              uint32_t o[16];
+              tmem_ld16(o_addr + cc * 16, o);
+              tmem_ld_wait();
 #pragma unroll
-            for (int e = 0; e < 16; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * f);
-            tmem_st16(o_addr + cc * 16, o);
+              for (int e = 0; e < 16; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * f);
+              tmem_st16(o_addr + cc * 16, o);
+            }
+            tmem_st_wait();
           }
-          tmem_st_wait();
           l *= f;
           if (need) m_used = m_new;
         }
       }
+      if (valid <= 0) continue;                    // ragged last tile without a sub-tile b (warp-uniform)
       // P = 2^(s c - m_used): one packed FFMA per pair, EX2 (MUFU or FMA pipe), row sum in fp32, bf16 pairs -> TMEM
       const uint64_t nm2 = pack2(-m_used, -m_used);
       uint64_t sum2 = pack2(0.f, 0.f), sum2b = pack2(0.f, 0.f);
@@ -379,18 +406,22 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
       tmem_st_wait();
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(p_full(t, b));
+      if (lane == 0) mbar_arrive(p_full(t, h));
     }
-    // ---- epilogue: O_t / l -> bf16 -> global; lse = ln2 (m + log2 l)
+    // ---- epilogue: the pair exchanges its partial row sums; leader writes columns 0..63, follower 64..127
+    // (its own barrier id, one per Q tile, 256 threads: the pair barrier may still hold the leader's last arrive)
+    l_sh[h * 128 + r_in] = l;
+    asm volatile("bar.sync %0, 256;" ::"r"(9 + t) : "memory");
+    l = l_sh[r_in] + l_sh[128 + r_in];
     mbar_wait(pv_done(t, (n_sub - 1) & 1), (uint32_t)((n_sub - 1) >> 1) & 1u);
     tc_fence_after();
-    const float inv = 1.0f / l;                    // l >= 2^-8 > 0: every sub-tile has at least one valid key
+    const float inv = 1.0f / l;                    // l >= 2^-8 > 0: every tile has at least one valid key
     const bool row_ok = row < q_hi;
-    bf16* orow = p.o + (int64_t)(row_ok ? row : q_lo) * p.o_stride + head * HD;
+    bf16* orow = p.o + (int64_t)(row_ok ? row : q_lo) * p.o_stride + head * HD + h * 64;
 #pragma unroll 1
-    for (int cc = 0; cc < 4; ++cc) {
+    for (int cc = 0; cc < 2; ++cc) {
       uint32_t o[32];
-      tmem_ld32(o_addr + cc * 32, o);
+      tmem_ld32(o_addr + h * 64 + cc * 32, o);
       tmem_ld_wait();
       if (row_ok) {
 #pragma unroll
@@ -402,7 +433,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
         }
       }
     }
-    if (row_ok && p.lse != nullptr) p.lse[(int64_t)row * p.H + head] = 0.6931471805599453f * (m_used + log2f(l));
+    if (h == 0 && row_ok && p.lse != nullptr) p.lse[(int64_t)row * p.H + head] = 0.6931471805599453f * (m_used + log2f(l));
   }
   tc_fence_before();
   __syncthreads();
