@@ -86,6 +86,20 @@ __device__ __forceinline__ void ld8<bf16>(const bf16* p, float v[8]) {
   v[0] = bf16lo(a.x); v[1] = bf16hi(a.x); v[2] = bf16lo(a.y); v[3] = bf16hi(a.y);
   v[4] = bf16lo(a.z); v[5] = bf16hi(a.z); v[6] = bf16lo(a.w); v[7] = bf16hi(a.w);
 }
+// streaming variant for data read exactly once (weights of a GEMV): bypass L1, evict-first in L2
+template <typename T>
+__device__ __forceinline__ void ld8_stream(const T* p, float v[8]);
+template <>
+__device__ __forceinline__ void ld8_stream<float>(const float* p, float v[8]) {
+  float4 a = __ldcs(reinterpret_cast<const float4*>(p)), b = __ldcs(reinterpret_cast<const float4*>(p + 4));
+  v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
+}
+template <>
+__device__ __forceinline__ void ld8_stream<bf16>(const bf16* p, float v[8]) {
+  uint4 a = __ldcs(reinterpret_cast<const uint4*>(p));
+  v[0] = bf16lo(a.x); v[1] = bf16hi(a.x); v[2] = bf16lo(a.y); v[3] = bf16hi(a.y);
+  v[4] = bf16lo(a.z); v[5] = bf16hi(a.z); v[6] = bf16lo(a.w); v[7] = bf16hi(a.w);
+}
 template <typename T>
 __device__ __forceinline__ void st8(T* p, const float v[8]);
 template <>
@@ -147,8 +161,8 @@ struct GemvBatch {      // one per weight matrix of a batched GEMV
   int32_t pad;
 };
 
-dit_status launch_gemv(int dtype, const float* in, const GemvBatch* batches_dev, int n_batches, int total_rows,
-                       float* out, int64_t out_stride, int R, int K, int silu_input, cudaStream_t st);
+dit_status launch_gemv(int dtype, const float* in, const GemvBatch* batches_dev, const GemvBatch* single, int n_batches,
+                       int total_rows, float* out, int64_t out_stride, int R, int K, int silu_input, cudaStream_t st);
 dit_status launch_adaln(int dtype, float* x, const void* h, const float* gate, const float* shift, const float* scale,
                         int64_t mod_stride, const int32_t* cu, int R, void* y, int T, int D, float eps, cudaStream_t st);
 dit_status launch_qknorm_rope(int dtype, void* qkv, int64_t row_stride, int T, int H, int d, int n_tensors,

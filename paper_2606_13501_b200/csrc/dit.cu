@@ -252,9 +252,9 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
   } while (0)
 
   // ---- steps 1-2: c = W2 SiLU(W1 temb + b1) + b2;  mod = Wmod SiLU(c) + bmod for ALL blocks in one launch
-  RUN(launch_gemv(dt, temb, w.gemv_tab + 0, 1, D, w.c1, D, R, c.temb_dim, 0, st));
-  RUN(launch_gemv(dt, w.c1, w.gemv_tab + 1, 1, D, w.c, D, R, D, 1, st));
-  RUN(launch_gemv(dt, w.c, w.gemv_tab + 2, L + 1, L * 6 * D + 2 * D, w.mod, mod_stride, R, D, 1, st));
+  RUN(launch_gemv(dt, temb, w.gemv_tab + 0, nullptr, 1, D, w.c1, D, R, c.temb_dim, 0, st));
+  RUN(launch_gemv(dt, w.c1, w.gemv_tab + 1, nullptr, 1, D, w.c, D, R, D, 1, st));
+  RUN(launch_gemv(dt, w.c, w.gemv_tab + 2, nullptr, L + 1, L * 6 * D + 2 * D, w.mod, mod_stride, R, D, 1, st));
 
   // ---- steps 3-4: patch-embed and cond projection write the fp32 residual stream
   for (int r = 0; r < R; ++r) {
@@ -589,13 +589,9 @@ dit_status dit_gemv(int32_t dtype, const float* in, const void* W, const void* b
                     int32_t K, int32_t silu_input, void* stream) {
   DIT_REQUIRE(dtype == DIT_F32 || dtype == DIT_BF16, DIT_ERR_INVALID_ARG, "dtype %d", dtype);
   DIT_REQUIRE(R >= 1 && N >= 1 && K >= 8 && in && W && out, DIT_ERR_INVALID_ARG, "bad GEMV arguments");
-  // the batch descriptor travels as a tiny device allocation owned by this call's stream order
+  // one matrix: its descriptor travels as a kernel parameter (no device allocation, no copy)
   GemvBatch tb = {W, b, N, 0, 0, 0};
-  GemvBatch* dev = nullptr;
-  DIT_CUDA_OK(cudaMallocAsync((void**)&dev, sizeof(GemvBatch), (cudaStream_t)stream));
-  DIT_CUDA_OK(cudaMemcpyAsync(dev, &tb, sizeof(tb), cudaMemcpyHostToDevice, (cudaStream_t)stream));
-  dit_status s = launch_gemv(dtype, in, dev, 1, N, out, N, R, K, silu_input, (cudaStream_t)stream);
-  cudaFreeAsync(dev, (cudaStream_t)stream);
+  dit_status s = launch_gemv(dtype, in, nullptr, &tb, 1, N, out, N, R, K, silu_input, (cudaStream_t)stream);
   return s;
 }
 

@@ -8,14 +8,21 @@ namespace dit {
 // =================================================================================================
 // GEMV:  out[r, off_b + n] = sum_k act(in[r,k]) W_b[n,k] + bias_b[n]      (DESIGN.md §3 steps 1-2)
 // Roofline: HBM, weights are streamed exactly once (N*K*sizeof(T) bytes); `in` lives in shared memory.
-// A warp owns 4 weight rows at a time so every staged input fragment is reused 4x from registers
-// (keeps shared-memory traffic at R/2 bytes per weight byte) and has 4+ independent 16-byte loads in flight.
+// A warp owns 4 weight rows at a time so every staged input fragment is reused 4x from registers (keeps
+// shared-memory traffic at R/2 bytes per weight byte); the K loop is unrolled twice, so a lane has 8 independent
+// 16-byte loads in flight and a resident SM (4 CTAs x 8 warps) about 128 KB — HBM latency x bandwidth needs ~45 KB.
+// The batch table (one entry per weight matrix) is copied to shared memory once per CTA.
 // =================================================================================================
+constexpr int GEMV_MAX_BATCHES = 264;   // n_blocks <= 256 (+ final layer)
+
 template <typename T, int RMAX>
 __global__ void __launch_bounds__(256) gemv_kernel(const float* __restrict__ in, const GemvBatch* __restrict__ batches,
-                                                   int n_batches, int total_rows, float* __restrict__ out,
-                                                   int64_t out_stride, int R, int K, int silu_input) {
-  extern __shared__ float s_in[];  // [R][K]
+                                                   const GemvBatch single, int n_batches, int total_rows,
+                                                   float* __restrict__ out, int64_t out_stride, int R, int K,
+                                                   int silu_input) {
+  extern __shared__ float s_in[];  // [R][K], then the batch table
+  GemvBatch* s_b = reinterpret_cast<GemvBatch*>(s_in + (size_t)R * K);
+  for (int i = threadIdx.x; i < n_batches; i += blockDim.x) s_b[i] = batches != nullptr ? batches[i] : single;
   for (int i = threadIdx.x; i < R * K; i += blockDim.x) {
     float v = in[i];
     s_in[i] = silu_input ? silu_f(v) : v;
@@ -23,31 +30,36 @@ __global__ void __launch_bounds__(256) gemv_kernel(const float* __restrict__ in,
   __syncthreads();
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int warps_total = gridDim.x * (blockDim.x >> 5);
-  const int n_groups = (total_rows + 3) >> 2;
-  for (int g = blockIdx.x * (blockDim.x >> 5) + warp; g < n_groups; g += warps_total) {
+  // balanced static partition: warp w streams the contiguous rows [w N / W, (w + 1) N / W) — row counts differ by
+  // at most one, so the last wave is not a quarter empty as with a strided loop over 4-row groups
+  const int wid = blockIdx.x * (blockDim.x >> 5) + warp;
+  const int r_begin = (int)((int64_t)wid * total_rows / warps_total);
+  const int r_end = (int)((int64_t)(wid + 1) * total_rows / warps_total);
+  for (int g0 = r_begin; g0 < r_end; g0 += 4) {
     const T* wrow[4];
     bool valid[4];
     int bidx[4], nloc[4];
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
-      int row = g * 4 + j;
-      valid[j] = row < total_rows;
-      if (!valid[j]) row = total_rows - 1;
+      int row = g0 + j;
+      valid[j] = row < r_end;
+      if (!valid[j]) row = r_end - 1;
       int b = 0;
-      while (b + 1 < n_batches && row >= batches[b + 1].row_begin) ++b;
+      while (b + 1 < n_batches && row >= s_b[b + 1].row_begin) ++b;
       bidx[j] = b;
-      nloc[j] = row - batches[b].row_begin;
-      wrow[j] = reinterpret_cast<const T*>(batches[b].W) + (int64_t)nloc[j] * K;
+      nloc[j] = row - s_b[b].row_begin;
+      wrow[j] = reinterpret_cast<const T*>(s_b[b].W) + (int64_t)nloc[j] * K;
     }
     float acc[4][RMAX];
 #pragma unroll
     for (int j = 0; j < 4; ++j)
 #pragma unroll
       for (int r = 0; r < RMAX; ++r) acc[j][r] = 0.f;
+#pragma unroll 2
     for (int k0 = lane * 8; k0 < K; k0 += 256) {
       float w[4][8];
 #pragma unroll
-      for (int j = 0; j < 4; ++j) ld8<T>(wrow[j] + k0, w[j]);
+      for (int j = 0; j < 4; ++j) ld8_stream<T>(wrow[j] + k0, w[j]);
 #pragma unroll
       for (int r = 0; r < RMAX; ++r) {
         if (r < R) {
@@ -68,7 +80,7 @@ __global__ void __launch_bounds__(256) gemv_kernel(const float* __restrict__ in,
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
         if (!valid[j]) continue;
-        const GemvBatch& B = batches[bidx[j]];
+        const GemvBatch& B = s_b[bidx[j]];
         float bias = B.b ? to_f<T>(reinterpret_cast<const T*>(B.b)[nloc[j]]) : 0.f;
 #pragma unroll
         for (int r = 0; r < RMAX; ++r)
@@ -79,9 +91,12 @@ __global__ void __launch_bounds__(256) gemv_kernel(const float* __restrict__ in,
 }
 
 template <typename T>
-static dit_status launch_gemv_t(const float* in, const GemvBatch* batches, int n_batches, int total_rows, float* out,
-                                int64_t out_stride, int R, int K, int silu_input, cudaStream_t st) {
+static dit_status launch_gemv_t(const float* in, const GemvBatch* batches, const GemvBatch& single, int n_batches,
+                                int total_rows, float* out, int64_t out_stride, int R, int K, int silu_input,
+                                cudaStream_t st) {
   DIT_REQUIRE(K % 8 == 0, DIT_ERR_UNSUPPORTED, "gemv: K=%d must be a multiple of 8", K);
+  DIT_REQUIRE(n_batches >= 1 && n_batches <= GEMV_MAX_BATCHES, DIT_ERR_UNSUPPORTED, "gemv: %d matrices (max %d)", n_batches,
+              GEMV_MAX_BATCHES);
   ProfScope _prof(DIT_KC_GEMV, st);
   int dev = 0, sms = 148;
   cudaGetDevice(&dev);
@@ -89,17 +104,18 @@ static dit_status launch_gemv_t(const float* in, const GemvBatch* batches, int n
   // requests are processed RMAX at a time (weights re-streamed per chunk only when R > 8)
   for (int r0 = 0; r0 < R; r0 += 8) {
     int rc = R - r0 < 8 ? R - r0 : 8;
-    size_t smem = (size_t)rc * K * sizeof(float);
-    int groups = (total_rows + 3) / 4;
-    int ctas = (groups + 7) / 8;
-    int per_sm = smem > 100 * 1024 ? 1 : 2;
-    if (ctas > sms * per_sm) ctas = sms * per_sm;
+    size_t smem = (size_t)rc * K * sizeof(float) + (size_t)n_batches * sizeof(GemvBatch);
+    int ctas = (total_rows + 63) / 64;   // at least 8 rows per warp
+    int per_sm = 1;   // exactly one resident wave: the partition is static, a partial second wave would be idle time
     const float* inr = in + (int64_t)r0 * K;
     float* outr = out + (int64_t)r0 * out_stride;
 #define GEMV_LAUNCH(RM)                                                                                         \
   {                                                                                                             \
     DIT_CUDA_OK(cudaFuncSetAttribute(gemv_kernel<T, RM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-    gemv_kernel<T, RM><<<ctas, 256, smem, st>>>(inr, batches, n_batches, total_rows, outr, out_stride, rc, K,   \
+    DIT_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gemv_kernel<T, RM>, 256, smem));          \
+    if (per_sm < 1) per_sm = 1;                                                                                 \
+    if (ctas > sms * per_sm) ctas = sms * per_sm;                                                               \
+    gemv_kernel<T, RM><<<ctas, 256, smem, st>>>(inr, batches, single, n_batches, total_rows, outr, out_stride, rc, K, \
                                                 silu_input);                                                    \
   }
     DIT_REQUIRE(smem <= 200 * 1024, DIT_ERR_UNSUPPORTED, "gemv: R*K too large for shared memory");
@@ -110,70 +126,95 @@ static dit_status launch_gemv_t(const float* in, const GemvBatch* batches, int n
   return DIT_OK;
 }
 
-dit_status launch_gemv(int dtype, const float* in, const GemvBatch* batches_dev, int n_batches, int total_rows,
-                       float* out, int64_t out_stride, int R, int K, int silu_input, cudaStream_t st) {
+// batches_dev == nullptr: one matrix, described by `single` (travels as a kernel parameter)
+dit_status launch_gemv(int dtype, const float* in, const GemvBatch* batches_dev, const GemvBatch* single, int n_batches,
+                       int total_rows, float* out, int64_t out_stride, int R, int K, int silu_input, cudaStream_t st) {
+  GemvBatch one = single ? *single : GemvBatch{nullptr, nullptr, 0, 0, 0, 0};
   if (dtype == DIT_F32)
-    return launch_gemv_t<float>(in, batches_dev, n_batches, total_rows, out, out_stride, R, K, silu_input, st);
-  return launch_gemv_t<bf16>(in, batches_dev, n_batches, total_rows, out, out_stride, R, K, silu_input, st);
+    return launch_gemv_t<float>(in, batches_dev, one, n_batches, total_rows, out, out_stride, R, K, silu_input, st);
+  return launch_gemv_t<bf16>(in, batches_dev, one, n_batches, total_rows, out, out_stride, R, K, silu_input, st);
 }
 
 // =================================================================================================
 // adaLN-Zero modulation (north_star subsystem 2; DESIGN.md §3 step 5):
 //   x <- x + gate (.) h   (optional);   y = LN(x) (.) (1 + scale) + shift
-// One warp per row, the whole row in registers (NC chunks of 8 elements per lane), two-pass statistics with
-// warp shuffles only.  Algorithmic bytes per token: 4D (x) + 2D (y) [+ 2D (h) + 4D (x write)].
+// WPR warps per row (1, 2 or 4), the whole row in registers (NCW chunks of 8 elements per lane and warp: at most 48
+// data registers, so 8+ CTAs of 128 threads stay resident and a row's 12-20 KB is in flight at once), two-pass
+// statistics: warp shuffles, then WPR partial sums through shared memory.  Algorithmic bytes per token: 4D (x) +
+// 2D (y) [+ 2D (h) + 4D (x write)].
 // =================================================================================================
-template <typename T, int NC>
+template <typename T, int NCW, int WPR>
 __global__ void __launch_bounds__(128) adaln_kernel(float* __restrict__ x, const T* __restrict__ h,
                                                     const float* __restrict__ gate, const float* __restrict__ shift,
                                                     const float* __restrict__ scale, int64_t mod_stride,
                                                     const int32_t* __restrict__ cu, int R, T* __restrict__ y, int T_rows,
                                                     float eps) {
-  constexpr int D = NC * 256;
-  const int lane = threadIdx.x & 31;
-  const int row = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-  if (row >= T_rows) return;
+  constexpr int D = NCW * WPR * 256;
+  constexpr int RPB = 4 / WPR;                       // rows per block
+  __shared__ float red[2][4];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int sub = warp % WPR;                        // which slice of the row this warp owns
+  const int row_raw = blockIdx.x * RPB + warp / WPR;
+  const bool row_ok = row_raw < T_rows;
+  const int row = row_ok ? row_raw : T_rows - 1;     // out-of-range warps redo the last row and store nothing
   const int req = (cu != nullptr && R > 1) ? find_request(cu, R, row) : 0;
-  float* xr = x + (int64_t)row * D;
-  float v[NC][8];
+  const int col0 = sub * (NCW * 256) + lane * 8;     // chunk c of this lane starts at col0 + c * 256
+  float* xr = x + (int64_t)row * D + col0;
+  float v[NCW][8];
 #pragma unroll
-  for (int c = 0; c < NC; ++c) ld8<float>(xr + (c * 32 + lane) * 8, v[c]);
+  for (int c = 0; c < NCW; ++c) ld8<float>(xr + c * 256, v[c]);
   if (h != nullptr) {
-    const T* hr = h + (int64_t)row * D;
-    const float* g = gate ? gate + (int64_t)req * mod_stride : nullptr;
+    const T* hr = h + (int64_t)row * D + col0;
+    const float* g = gate ? gate + (int64_t)req * mod_stride + col0 : nullptr;
 #pragma unroll
-    for (int c = 0; c < NC; ++c) {
+    for (int c = 0; c < NCW; ++c) {
       float hv[8], gv[8];
-      ld8<T>(hr + (c * 32 + lane) * 8, hv);
-      if (g) ld8<float>(g + (c * 32 + lane) * 8, gv);
+      ld8<T>(hr + c * 256, hv);
+      if (g) ld8<float>(g + c * 256, gv);
 #pragma unroll
       for (int e = 0; e < 8; ++e) v[c][e] = g ? fmaf(gv[e], hv[e], v[c][e]) : v[c][e] + hv[e];
-      st8<float>(xr + (c * 32 + lane) * 8, v[c]);
+      if (row_ok) st8<float>(xr + c * 256, v[c]);
     }
   }
   float s = 0.f;
 #pragma unroll
-  for (int c = 0; c < NC; ++c)
+  for (int c = 0; c < NCW; ++c)
 #pragma unroll
     for (int e = 0; e < 8; ++e) s += v[c][e];
-  const float mean = warp_sum(s) * (1.0f / D);
+  s = warp_sum(s);
+  if (WPR > 1) {
+    if (lane == 0) red[0][warp] = s;
+    __syncthreads();
+    s = 0.f;
+#pragma unroll
+    for (int i = 0; i < WPR; ++i) s += red[0][(warp / WPR) * WPR + i];
+  }
+  const float mean = s * (1.0f / D);
   float q = 0.f;
 #pragma unroll
-  for (int c = 0; c < NC; ++c)
+  for (int c = 0; c < NCW; ++c)
 #pragma unroll
     for (int e = 0; e < 8; ++e) {
       float dlt = v[c][e] - mean;
       q = fmaf(dlt, dlt, q);
     }
-  const float rstd = rsqrtf(warp_sum(q) * (1.0f / D) + eps);
-  const float* sh = shift ? shift + (int64_t)req * mod_stride : nullptr;
-  const float* sc = scale ? scale + (int64_t)req * mod_stride : nullptr;
-  T* yr = y + (int64_t)row * D;
+  q = warp_sum(q);
+  if (WPR > 1) {
+    if (lane == 0) red[1][warp] = q;
+    __syncthreads();
+    q = 0.f;
 #pragma unroll
-  for (int c = 0; c < NC; ++c) {
+    for (int i = 0; i < WPR; ++i) q += red[1][(warp / WPR) * WPR + i];
+  }
+  const float rstd = rsqrtf(q * (1.0f / D) + eps);
+  const float* sh = shift ? shift + (int64_t)req * mod_stride + col0 : nullptr;
+  const float* sc = scale ? scale + (int64_t)req * mod_stride + col0 : nullptr;
+  T* yr = y + (int64_t)row * D + col0;
+#pragma unroll
+  for (int c = 0; c < NCW; ++c) {
     float o[8], a[8], b[8];
-    if (sc) ld8<float>(sc + (c * 32 + lane) * 8, a);
-    if (sh) ld8<float>(sh + (c * 32 + lane) * 8, b);
+    if (sc) ld8<float>(sc + c * 256, a);
+    if (sh) ld8<float>(sh + c * 256, b);
 #pragma unroll
     for (int e = 0; e < 8; ++e) {
       float n = (v[c][e] - mean) * rstd;
@@ -181,7 +222,7 @@ __global__ void __launch_bounds__(128) adaln_kernel(float* __restrict__ x, const
       if (sh) n += b[e];
       o[e] = n;
     }
-    st8<T>(yr + (c * 32 + lane) * 8, o);
+    if (row_ok) st8<T>(yr + c * 256, o);
   }
 }
 
@@ -192,14 +233,15 @@ static dit_status launch_adaln_t(float* x, const T* h, const float* gate, const 
   if (T_rows == 0) return DIT_OK;
   DIT_REQUIRE(D % 256 == 0 && D <= 6144, DIT_ERR_UNSUPPORTED, "adaln: D=%d must be a multiple of 256 (<= 6144)", D);
   ProfScope _prof(DIT_KC_ADALN, st);
-  const int grid = cdiv(T_rows, 4);
-#define ADALN_CASE(NCV)                                                                                     \
+#define ADALN_CASE(NCV, NCW, WPR)                                                                           \
   case NCV:                                                                                                 \
-    adaln_kernel<T, NCV><<<grid, 128, 0, st>>>(x, h, gate, shift, scale, mod_stride, cu, R, y, T_rows, eps); \
+    adaln_kernel<T, NCW, WPR><<<cdiv(T_rows, 4 / WPR), 128, 0, st>>>(x, h, gate, shift, scale, mod_stride, cu, R, y, \
+                                                                    T_rows, eps);                           \
     break;
-  switch (D / 256) {
-    ADALN_CASE(1) ADALN_CASE(2) ADALN_CASE(3) ADALN_CASE(4) ADALN_CASE(5) ADALN_CASE(6) ADALN_CASE(8) ADALN_CASE(10)
-    ADALN_CASE(12) ADALN_CASE(16) ADALN_CASE(20) ADALN_CASE(24)
+  switch (D / 256) {   // D / 256 chunks per row = NCW per warp x WPR warps
+    ADALN_CASE(1, 1, 1) ADALN_CASE(2, 2, 1) ADALN_CASE(3, 3, 1) ADALN_CASE(4, 4, 1) ADALN_CASE(5, 5, 1)
+    ADALN_CASE(6, 3, 2) ADALN_CASE(8, 4, 2) ADALN_CASE(10, 5, 2) ADALN_CASE(12, 6, 2) ADALN_CASE(16, 4, 4)
+    ADALN_CASE(20, 5, 4) ADALN_CASE(24, 6, 4)
     default:
       DIT_REQUIRE(false, DIT_ERR_UNSUPPORTED, "adaln: D=%d has no instantiation", D);
   }
@@ -223,49 +265,69 @@ __global__ void __launch_bounds__(256) qknorm_rope_kernel(T* __restrict__ qkv, i
                                                           int n_tensors, const T* __restrict__ gq,
                                                           const T* __restrict__ gk, float eps,
                                                           const float* __restrict__ rc, const float* __restrict__ rs) {
+  // The q | k part of a row is n_tensors * D contiguous elements.  A warp pass covers UN consecutive 256-element
+  // chunks of one row (32 lanes x 8 elements = 256 / HD head rows each); every load of a pass is issued before
+  // its first use, so a lane keeps UN x (16 B data + 32 B table) in flight.
   constexpr int LPH = HD / 8;           // lanes per head row
-  constexpr int HPW = 32 / LPH;         // head rows per warp pass
+  constexpr int UN = 4;
   const int lane = threadIdx.x & 31;
-  const int sub = lane / LPH, li = lane % LPH;
   const int D = H * HD;
-  const int64_t heads_total = (int64_t)T_rows * n_tensors * H;
+  const int width = n_tensors * D;      // elements per row that are normalised
+  const int cpr = (width + 255) / 256;  // chunks per row
+  const int ppr = (cpr + UN - 1) / UN;  // passes per row
+  const int64_t n_pass = (int64_t)T_rows * ppr;
   const int64_t warp_id = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   const int64_t n_warps = (int64_t)gridDim.x * (blockDim.x >> 5);
-  for (int64_t base = warp_id * HPW; base < heads_total; base += n_warps * HPW) {
-    const int64_t item = base + sub;
-    const bool ok = item < heads_total;
-    const int64_t it = ok ? item : heads_total - 1;
-    const int head = (int)(it % H);
-    const int which = (int)((it / H) % n_tensors);
-    const int row = (int)(it / ((int64_t)H * n_tensors));
-    T* p = qkv + (int64_t)row * row_stride + (int64_t)which * D + head * HD + li * 8;
-    float v[8];
-    ld8<T>(p, v);
-    const T* g = which == 0 ? gq : gk;
-    if (g != nullptr) {
-      float ss = 0.f;
+  const int hoff = (lane % LPH) * 8;    // offset inside the head row
+  float gqv[8], gkv[8];
+  if (gq != nullptr) ld8<T>(gq + hoff, gqv);
+  if (gk != nullptr) ld8<T>(gk + hoff, gkv);
+  for (int64_t pass = warp_id; pass < n_pass; pass += n_warps) {
+    const int row = (int)(pass / ppr);
+    const int c0 = (int)(pass % ppr) * UN;
+    T* const rowp = qkv + (int64_t)row * row_stride;
+    float v[UN][8];
+    bool ok[UN];
 #pragma unroll
-      for (int e = 0; e < 8; ++e) ss = fmaf(v[e], v[e], ss);
+    for (int u = 0; u < UN; ++u) {
+      const int col = (c0 + u) * 256 + lane * 8;
+      ok[u] = col < width;
+      if (ok[u]) ld8<T>(rowp + col, v[u]);
+      else {
 #pragma unroll
-      for (int o = LPH / 2; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
-      const float r = rsqrtf(ss * (1.0f / HD) + eps);
-      float gv[8];
-      ld8<T>(g + li * 8, gv);
-#pragma unroll
-      for (int e = 0; e < 8; ++e) v[e] = v[e] * r * gv[e];
-    }
-    if (rc != nullptr) {
-      const float4 c = *reinterpret_cast<const float4*>(rc + (int64_t)row * (HD / 2) + li * 4);
-      const float4 s = *reinterpret_cast<const float4*>(rs + (int64_t)row * (HD / 2) + li * 4);
-      const float cc[4] = {c.x, c.y, c.z, c.w}, sn[4] = {s.x, s.y, s.z, s.w};
-#pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        const float a = v[2 * j], b = v[2 * j + 1];
-        v[2 * j] = a * cc[j] - b * sn[j];
-        v[2 * j + 1] = a * sn[j] + b * cc[j];
+        for (int e = 0; e < 8; ++e) v[u][e] = 0.f;
       }
     }
-    if (ok) st8<T>(p, v);
+    float4 cs, sn4;
+    if (rc != nullptr) {   // the table row depends on the token only: one load serves all UN chunks
+      cs = *reinterpret_cast<const float4*>(rc + (int64_t)row * (HD / 2) + hoff / 2);
+      sn4 = *reinterpret_cast<const float4*>(rs + (int64_t)row * (HD / 2) + hoff / 2);
+    }
+#pragma unroll
+    for (int u = 0; u < UN; ++u) {
+      const int col = (c0 + u) * 256 + lane * 8;
+      const bool is_q = col < D;                       // tensor 0 = q, tensor 1 = k
+      if ((is_q ? gq : gk) != nullptr) {
+        float ss = 0.f;
+#pragma unroll
+        for (int e = 0; e < 8; ++e) ss = fmaf(v[u][e], v[u][e], ss);
+#pragma unroll
+        for (int o = LPH / 2; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
+        const float r = rsqrtf(ss * (1.0f / HD) + eps);
+#pragma unroll
+        for (int e = 0; e < 8; ++e) v[u][e] = v[u][e] * r * (is_q ? gqv[e] : gkv[e]);
+      }
+      if (rc != nullptr) {
+        const float cc[4] = {cs.x, cs.y, cs.z, cs.w}, sn[4] = {sn4.x, sn4.y, sn4.z, sn4.w};
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const float a = v[u][2 * j], b = v[u][2 * j + 1];
+          v[u][2 * j] = a * cc[j] - b * sn[j];
+          v[u][2 * j + 1] = a * sn[j] + b * cc[j];
+        }
+      }
+      if (ok[u]) st8<T>(rowp + col, v[u]);
+    }
   }
 }
 
@@ -275,11 +337,11 @@ dit_status launch_qknorm_rope(int dtype, void* qkv, int64_t row_stride, int T, i
   if (T == 0 || (gq == nullptr && gk == nullptr && rc == nullptr)) return DIT_OK;
   DIT_REQUIRE(d == 64 || d == 128, DIT_ERR_UNSUPPORTED, "qknorm_rope: head_dim %d not in {64,128}", d);
   ProfScope _prof(DIT_KC_QKNORM, st);
-  int64_t heads = (int64_t)T * n_tensors * H;
-  int hpw = 32 / (d / 8);
-  int64_t warps = (heads + hpw - 1) / hpw;
-  int grid = (int)((warps + 7) / 8);
-  if (grid > 148 * 16) grid = 148 * 16;
+  const int cpr = (n_tensors * H * d + 255) / 256;
+  const int64_t passes = (int64_t)T * ((cpr + 3) / 4);
+  int grid = (int)((passes + 7) / 8);
+  if (grid > 148 * 8) grid = 148 * 8;
+  if (grid < 1) grid = 1;
 #define QK_LAUNCH(TT, HDV)                                                                                      \
   qknorm_rope_kernel<TT, HDV><<<grid, 256, 0, st>>>((TT*)qkv, row_stride, T, H, n_tensors, (const TT*)gq,       \
                                                     (const TT*)gk, eps, rc, rs)
