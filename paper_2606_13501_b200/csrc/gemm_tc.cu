@@ -48,12 +48,17 @@ using namespace tc;
 
 namespace {
 
-constexpr int BM = 128, BN = 256, BK = 64, STAGES = 4;
-constexpr int A_BYTES = BM * BK * 2, B_BYTES = BN * BK * 2, STAGE_BYTES = A_BYTES + B_BYTES;
+constexpr int BM = 128, BK = 64, STAGES = 4;
+constexpr int BN_MAX = 256;   // TMEM accumulator stage stride and staging-row size; the tile width BN is a template
+                              // parameter (192 / 240 / 256) picked per problem to fill the last wave (see pick_bn)
+constexpr int A_BYTES = BM * BK * 2;
+constexpr int stage_bytes(int bn) { return A_BYTES + bn * BK * 2; }
 constexpr int GEMM_THREADS = 192;
 constexpr int EPI_THREADS = 128;
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /* alignment slack */ + 256 /* barriers */ +
-                           2 * 2 * BN * 4 /* bias + gate rows of the tile, fp32, one set per accumulator stage */;
+constexpr int smem_bytes(int bn) {
+  return STAGES * stage_bytes(bn) + 1024 /* alignment slack */ + 256 /* barriers */ +
+         2 * 2 * BN_MAX * 4 /* bias + gate rows of the tile, fp32, one set per accumulator stage */;
+}
 enum { EPI_GATE_RESID = 3 };
 
 struct EpiArgs {
@@ -72,11 +77,13 @@ __device__ __forceinline__ float gelu_tanh_fast(float z) {
   return __fdividef(z, 1.0f + __expf(-u2));
 }
 
-template <int EPI>
+template <int EPI, int BN>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, EpiArgs ep, int M, int N,
                int K) {
   extern __shared__ uint8_t smem_raw[];
+  constexpr int B_BYTES = BN * BK * 2, STAGE_BYTES = A_BYTES + B_BYTES;   // both multiples of 1024 (swizzle atom)
+  static_assert(BN % 16 == 0 && BN <= BN_MAX && STAGE_BYTES % 1024 == 0, "tile width");
   const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t bar0 = smem0 + STAGES * STAGE_BYTES;
   // barriers: full[STAGES], empty[STAGES], tfull[2], tempty[2]; then the TMEM base address word
@@ -140,7 +147,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       const uint32_t aph = (it >> 1) & 1;
       mbar_wait(tempty_bar(as), aph ^ 1);
       tc_fence_after();
-      const uint32_t d_tmem = tmem_base + as * BN;
+      const uint32_t d_tmem = tmem_base + as * BN_MAX;
       for (int kb = 0; kb < nkb; ++kb) {
         mbar_wait(full_bar(s), ph);
         tc_fence_after();
@@ -171,8 +178,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       const int m0 = (t % mt) * BM, n0 = (t / mt) * BN;
       const int row = m0 + quad * 32 + lane;
       const bool row_ok = row < M;
-      float* const s_bias = s_vec + as * 2 * BN;
-      float* const s_gate = s_bias + BN;
+      float* const s_bias = s_vec + as * 2 * BN_MAX;
+      float* const s_gate = s_bias + BN_MAX;
       bool gate_smem = true;          // this thread's row takes the staged gate row
       const float* gate_row = nullptr;
       if (EPI == EPI_GATE_RESID && ep.gate != nullptr) {
@@ -196,7 +203,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       auto load_x = [&](int c) {  // residual-stream chunk c of this thread's row (EPI_GATE_RESID)
 #pragma unroll
         for (int g = 0; g < 4; ++g) {
-          if (row_ok && n0 + c * 32 + g * 8 < N) ld8<float>(xrow + c * 32 + g * 8, &xc[g * 8]);
+          if (row_ok && n0 + c * 32 + g * 8 < N && c * 32 + g * 8 < BN) ld8<float>(xrow + c * 32 + g * 8, &xc[g * 8]);
         }
       };
       if (EPI == EPI_GATE_RESID) {
@@ -209,9 +216,9 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       }
       mbar_wait(tfull_bar(as), aph);
       tc_fence_after();
-      const uint32_t t_addr = tmem_base + as * BN + ((uint32_t)(quad * 32) << 16);
+      const uint32_t t_addr = tmem_base + as * BN_MAX + ((uint32_t)(quad * 32) << 16);
 #pragma unroll 1
-      for (int c = 0; c < BN / 32; ++c) {
+      for (int c = 0; c < (BN + 31) / 32; ++c) {
         const int n = n0 + c * 32;
         if (n >= N) break;  // warp-uniform
         uint32_t r[32];
@@ -221,12 +228,12 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         if (EPI == EPI_GATE_RESID) {
 #pragma unroll
           for (int e = 0; e < 32; ++e) xv[e] = xc[e];
-          if (c + 1 < BN / 32 && n + 32 < N) load_x(c + 1);  // prefetch the next chunk
+          if (c + 1 < (BN + 31) / 32 && n + 32 < N) load_x(c + 1);  // prefetch the next chunk
         }
 #pragma unroll
         for (int g = 0; g < 4; ++g) {  // groups of 8 columns
           const int ng = n + g * 8;
-          if (ng >= N) break;  // N % 8 == 0: groups are all-or-nothing
+          if (ng >= N || c * 32 + g * 8 >= BN) break;  // N % 8 == 0, BN % 16 == 0: groups are all-or-nothing
           float v[8], b[8];
           ld8<float>(s_bias + c * 32 + g * 8, b);
 #pragma unroll
@@ -281,18 +288,44 @@ int sm_count() {
   return n;
 }
 
-template <int EPI>
+template <int EPI, int BN>
 dit_status launch_t(const CUtensorMap& ta, const CUtensorMap& tb, const EpiArgs& ep, int M, int N, int K, cudaStream_t st) {
   static bool attr_set = false;
   if (!attr_set) {
-    DIT_CUDA_OK(cudaFuncSetAttribute(gemm_tc_kernel<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
+    DIT_CUDA_OK(cudaFuncSetAttribute(gemm_tc_kernel<EPI, BN>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes(BN)));
     attr_set = true;
   }
   const int tiles = cdiv(M, BM) * cdiv(N, BN);
   const int grid = tiles < sm_count() ? tiles : sm_count();
-  gemm_tc_kernel<EPI><<<grid, GEMM_THREADS, SMEM_BYTES, st>>>(ta, tb, ep, M, N, K);
+  gemm_tc_kernel<EPI, BN><<<grid, GEMM_THREADS, smem_bytes(BN), st>>>(ta, tb, ep, M, N, K);
   DIT_LAUNCH_CHECK();
   return DIT_OK;
+}
+
+// Tile width that minimises waves x width on this many SMs (wave quantisation: M = 4352 gives 34 M-tiles, and
+// 34 x {36, 48, 12} tiles of 256 columns leave the last wave 3-27 % full; 240- or 192-wide tiles fill it).
+int pick_bn(int M, int N) {
+  const int cand[3] = {256, 240, 192};
+  int best = 256;
+  int64_t best_cost = INT64_MAX;
+  for (int i = 0; i < 3; ++i) {
+    const int bn = cand[i];
+    const int64_t tiles = (int64_t)cdiv(M, BM) * cdiv(N, bn);
+    const int64_t cost = cdiv(tiles, (int64_t)sm_count()) * bn;
+    if (cost < best_cost - best_cost / 64) {   // a narrower tile must win by > 1.5 %
+      best_cost = cost;
+      best = bn;
+    }
+  }
+  return best;
+}
+
+template <int EPI>
+dit_status launch_bn(int bn, const CUtensorMap& ta, const CUtensorMap& tb, const EpiArgs& ep, int M, int N, int K,
+                     cudaStream_t st) {
+  if (bn == 192) return launch_t<EPI, 192>(ta, tb, ep, M, N, K, st);
+  if (bn == 240) return launch_t<EPI, 240>(ta, tb, ep, M, N, K, st);
+  return launch_t<EPI, 256>(ta, tb, ep, M, N, K, st);
 }
 
 }  // namespace
@@ -310,15 +343,16 @@ dit_status launch_gemm_tc_ex(int epi, const void* A, int64_t lda, const void* W,
                              cudaStream_t st) {
   if (M == 0 || N == 0) return DIT_OK;
   CUtensorMap ta, tb;
-  DIT_REQUIRE(make_tmap_2d_bf16(&ta, A, M, K, lda, BM, BK) && make_tmap_2d_bf16(&tb, W, N, K, K, BN, BK), DIT_ERR_CUDA,
+  const int bn = pick_bn(M, N);
+  DIT_REQUIRE(make_tmap_2d_bf16(&ta, A, M, K, lda, BM, BK) && make_tmap_2d_bf16(&tb, W, N, K, K, bn, BK), DIT_ERR_CUDA,
               "gemm_tc: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d lda=%lld)", M, N, K, (long long)lda);
   EpiArgs ep{(const bf16*)bias, out, ldo, gate, gate_stride, cu, R};
   ProfScope _prof(DIT_KC_GEMM, st);
   switch (epi) {
-    case DIT_EPI_BIAS: return launch_t<DIT_EPI_BIAS>(ta, tb, ep, M, N, K, st);
-    case DIT_EPI_BIAS_GELU: return launch_t<DIT_EPI_BIAS_GELU>(ta, tb, ep, M, N, K, st);
-    case DIT_EPI_BIAS_F32: return launch_t<DIT_EPI_BIAS_F32>(ta, tb, ep, M, N, K, st);
-    case EPI_GATE_RESID: return launch_t<EPI_GATE_RESID>(ta, tb, ep, M, N, K, st);
+    case DIT_EPI_BIAS: return launch_bn<DIT_EPI_BIAS>(bn, ta, tb, ep, M, N, K, st);
+    case DIT_EPI_BIAS_GELU: return launch_bn<DIT_EPI_BIAS_GELU>(bn, ta, tb, ep, M, N, K, st);
+    case DIT_EPI_BIAS_F32: return launch_bn<DIT_EPI_BIAS_F32>(bn, ta, tb, ep, M, N, K, st);
+    case EPI_GATE_RESID: return launch_bn<EPI_GATE_RESID>(bn, ta, tb, ep, M, N, K, st);
     default: DIT_REQUIRE(false, DIT_ERR_INVALID_ARG, "gemm_tc: epilogue %d", epi);
   }
 }

@@ -112,8 +112,10 @@ def test_qknorm_rope(lib, dtype, T, H, d, norm, rope):
 
 
 # ------------------------------------------------------------------------------ Linear (GEMM + epilogues)
+# the last two pick the 240-wide tile (34 x 13 tiles = 2.99 waves of 148 SMs; ragged last N tile) and, with 20000
+# rows, several persistent rounds per CTA of the 256-wide one
 GEMM_SHAPES = [(1, 64, 64), (100, 72, 16), (288, 768, 256), (257, 1024, 320), (130, 3072, 64), (515, 200, 1032),
-               (1000, 256, 4096)]
+               (1000, 256, 4096), (4352, 3072, 128), (20000, 512, 64)]
 
 
 @pytest.mark.parametrize("dtype", DTYPES)
@@ -158,7 +160,8 @@ def test_linear_strided_views_and_no_bias(lib, dtype):
 
 
 @pytest.mark.parametrize("dtype", DTYPES)
-@pytest.mark.parametrize("M,N,K,R", [(288, 256, 256, 1), (515, 768, 1032, 3), (130, 3072, 512, 1), (1000, 264, 4096, 4)])
+@pytest.mark.parametrize("M,N,K,R", [(288, 256, 256, 1), (515, 768, 1032, 3), (130, 3072, 512, 1), (1000, 264, 4096, 4),
+                                     (4352, 3072, 64, 2)])   # the last one takes the 240-wide tile
 @pytest.mark.parametrize("gated", [True, False])
 def test_linear_residual_gate_epilogue(lib, dtype, M, N, K, R, gated):
     """x <- x + gate[req(row)] (.) (A W^T + b) in the GEMM epilogue (the out-projection / fc2 of every block).
@@ -192,7 +195,8 @@ def _attn_tol(dtype):
 
 @pytest.mark.parametrize("dtype", DTYPES)
 @pytest.mark.parametrize("nq,nk,H,d", [(1, 1, 1, 64), (77, 133, 3, 64), (288, 288, 4, 64), (300, 515, 2, 128),
-                                        (128, 1024, 2, 128), (640, 257, 3, 128)])
+                                        (128, 1024, 2, 128), (640, 257, 3, 128), (5, 64, 1, 128), (129, 65, 1, 128),
+                                        (256, 192, 2, 128), (100, 1, 2, 128)])
 def test_attn_partial(lib, dtype, nq, nk, H, d):
     q, k, v = synth.make_attention_qkv(11, nq, nk, H, d, dtype=dtype, device=DEV)
     o, lse = B.dit_attn_partial(q, k, v)
@@ -216,6 +220,22 @@ def test_attn_peaky_and_identical_keys(lib, dtype):
     ones = torch.ones_like(v)
     o2, _ = B.dit_attn_partial(q, k, ones)                      # softmax rows sum to 1
     assert float((o2.double().cpu() - 1).abs().max()) < (1e-5 if dtype == torch.float32 else 8e-3)
+
+
+@pytest.mark.parametrize("dtype", DTYPES)
+@pytest.mark.parametrize("nq,nk", [(130, 700), (257, 1100)])
+def test_attn_growing_row_maxima_force_rescale(lib, dtype, nq, nk):
+    """Keys whose norm ramps up 6x along the sequence: the running row max grows by far more than the lazy-rescale
+    threshold (2^8) from key tile to key tile, so the O / row-sum rescale path (R25; taken jointly by the
+    leader and follower softmax warps of a row) runs several times per row."""
+    H, d = 2, 128
+    q, k, v = synth.make_attention_qkv(11, nq, nk, H, d, dtype=dtype, device=DEV, logit_gain=3.0)
+    ramp = (1.0 + 5.0 * torch.arange(nk, device=DEV, dtype=torch.float32) / nk).view(nk, 1, 1)
+    k = (k.float() * ramp).to(dtype)
+    o, lse = B.dit_attn_partial(q, k, v)
+    ro, rl = O.attention(q.cpu(), k.cpu(), v.cpu())
+    check(o, ro, dtype, f"rescale attention {nq}x{nk}", **_attn_tol(dtype))
+    assert float((lse.double().cpu() - rl).abs().max()) < (1e-4 if dtype == torch.float32 else 5e-2)
 
 
 @pytest.mark.parametrize("dtype", DTYPES)
