@@ -1,0 +1,131 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (same dit_config, same
+weights recipe, whole 8- / 4-block model resident): the oracle cannot run a whole cfg 2 / cfg 3 step in seconds, so
+one block is checked teacher-forced on SAMPLED rows (oracle.block_rows: the block's input is read back from the GPU,
+keys / values cover the whole sequence, queries and everything after attention only the sampled rows), the
+attention sweep on sampled query rows, and packed batching through the property that holds at any size: the
+packed result of request r equals dit_step on request r alone."""
+import pytest
+import torch
+
+from oracle import dit_oracle as O
+from paper_2606_13501_b200 import binding as B
+from paper_2606_13501_b200 import synth
+from util import check, errors
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda:0"
+
+
+def _host_gb():
+    try:
+        import psutil
+        return psutil.virtual_memory().available / 2 ** 30
+    except Exception:
+        return 0.0
+
+
+def _block_weights_cpu(W, l):
+    """Only block l's tensors travel to the host (the full cfg 3 model is 8 GB)."""
+    return {k: v.cpu() for k, v in W.items() if k.startswith(f"blocks.{l}.")}
+
+
+def _sampled_block_check(s, l, rows, what):
+    W = synth.make_weights(s, device=DEV)
+    I = synth.make_inputs(s, device=DEV)
+    m = B.Dit(B.make_config(s), W, DEV)
+    lat, temb, cond = I["latents"], I["temb"][0].contiguous(), I["cond"]
+    D, L = s.hidden, s.n_blocks
+    joint = s.cond_mode == "joint"
+    T = s.n_tokens + (s.n_cond if joint else 0)
+    # block input (x is untouched by the y1 stage), the modulation row, the cross-attention context
+    m.dit_debug_stop_after(l, "y1")
+    m.dit_step(lat, temb, cond)
+    x_in = m.dit_get_tap("x", (T, D), torch.float32)
+    mod = m.dit_get_tap("mod", (L * 6 * D + 2 * D,), torch.float32)
+    m.dit_debug_stop_after(l, "fc2")
+    m.dit_step(lat, temb, cond)
+    x_out = m.dit_get_tap("x", (T, D), torch.float32)
+    m.dit_debug_stop_after(-1, 0)
+    torch.cuda.synchronize()
+
+    cfg = O.cfg_from_shape(s)
+    Wl = _block_weights_cpu(W, l)
+    # the modulation vectors themselves against the oracle's conditioning path (t-MLP + GEMV, whole model)
+    Wc = {k: v.cpu() for k, v in W.items() if k.startswith("t_mlp.") or ".mod." in k}
+    _, mods, modf = O.conditioning(cfg, Wc, I["temb"].cpu())
+    ref_mod = torch.cat([mm.reshape(-1) for mm in mods] + [modf.reshape(-1)])
+    check(mod, ref_mod, torch.float32, f"{what}: modulation", rel=2e-5, maxabs=2e-4)
+
+    pos = O.token_positions(s.token_grid)
+    if joint:
+        pos = torch.cat([torch.zeros(s.n_cond, 3, dtype=torch.int64), pos])
+    ang = O.rope_angles(pos, cfg["rope_dims"], cfg["rope_theta"])
+    ctx = None
+    if s.cond_mode == "cross":
+        ctx = O.linear(I["cond"].cpu().double(), W["cond_proj.w"].cpu(), W["cond_proj.b"].cpu())
+    ref = O.block_rows(cfg, Wl, l, x_in.cpu(), mods[l], ang, rows, ctx=ctx)
+    e = check(x_out[rows.to(DEV)], ref, torch.bfloat16, what)
+    print(what, "rel-L2 %.2e  max-abs/RMS %.2e" % e)
+
+
+def test_cfg2_full_size_block_on_sampled_rows(lib):
+    s = synth.cfg2()
+    T = s.n_tokens + s.n_cond
+    rows = torch.tensor([0, 1, 255, 256, 257, 300, 1023, 2048, 2049, 3071, 4000, 4095, 4096, 4350, T - 1])
+    _sampled_block_check(s, 3, rows, "cfg2 full size, block 3, sampled rows")
+
+
+def test_cfg3_full_size_block_on_sampled_rows(lib):
+    if _host_gb() < 48:
+        pytest.skip("the oracle's fp64 K/V of 32760 x 15360 need ~40 GB of host memory")
+    s = synth.cfg3()
+    rows = torch.tensor([0, 127, 128, 4097, 16380, 32000, s.n_tokens - 1])
+    _sampled_block_check(s, 1, rows, "cfg3 full size, block 1, sampled rows")
+
+
+def test_cfg4_full_size_packing_invariance(lib):
+    """configs[3]: six requests {1024, 1024, 4096, 4096, 9216, 16384} + 256 text tokens each, packed with
+    cu_seqlens, per-request timesteps (seed 7): request r of the packed step == dit_step on request r alone."""
+    shapes = synth.cfg4_requests()
+    W = synth.make_weights(shapes[0], device=DEV)
+    R = len(shapes)
+    ts = [float(synth.uniform01(7, f"t{r}", 1)[0]) * 1000 for r in range(R)]
+    Is = [synth.make_inputs(sh, device=DEV, tag=f".r{r}", t=ts[r]) for r, sh in enumerate(shapes)]
+    T_total = sum(sh.n_tokens + sh.n_cond for sh in shapes)
+    assert T_total == 37376
+    cfg = B.make_config(shapes[-1], max_tokens=T_total, max_requests=R, max_cond_tokens=sum(sh.n_cond for sh in shapes))
+    m = B.Dit(cfg, W, DEV)
+    lats = [i["latents"] for i in Is]
+    temb = torch.cat([i["temb"] for i in Is])
+    conds = [i["cond"] for i in Is]
+    outs = m.dit_step_varlen(lats, temb, conds)
+    torch.cuda.synchronize()
+    for r in (0, 2, 5):
+        single = m.dit_step(lats[r], temb[r].contiguous(), conds[r])
+        torch.cuda.synchronize()
+        e_rel, e_max = errors(outs[r], single)
+        assert torch.isfinite(outs[r].float()).all()
+        assert e_rel < 2e-3 and e_max < 3e-2, f"packing changed request {r}: rel {e_rel:.2e} max {e_max:.2e}"
+
+
+@pytest.mark.parametrize("H,N", [(24, 32768), (40, 16384)])
+def test_cfg5_full_size_attention_sampled_rows_and_split(lib, H, N):
+    """configs[4]: q, k, v ~ N(0,1), seed 11.  Sampled query rows against the plain definition over ALL keys;
+    split-KV P = 2 / 4 / 8 partials + LSE merge against the unsplit GPU result (P-invariance)."""
+    q, k, v = synth.make_attention_qkv(11, N, N, H, 128, device=DEV)
+    o, lse = B.dit_attn_partial(q, k, v)
+    rows = torch.tensor([0, 127, 128, 255, 256, 1000, N // 2 + 3, N - 129, N - 1])
+    kc, vc = k.cpu(), v.cpu()
+    ro, rl = O.attention(q[rows.to(DEV)].cpu(), kc, vc)
+    check(o[rows.to(DEV)], ro, torch.bfloat16, f"attention N={N} H={H} sampled rows", rel=4e-3, maxabs=2.5e-2)
+    assert float((lse[rows.to(DEV)].double().cpu() - rl).abs().max()) < 2e-2
+    for P in (2, 4, 8):
+        n = (N + P - 1) // P
+        parts = [B.dit_attn_partial(q, k[p * n:(p + 1) * n], v[p * n:(p + 1) * n]) for p in range(P)]
+        om, lm = B.dit_attn_merge([x[0] for x in parts], [x[1] for x in parts])
+        e_rel, e_max = errors(om, o)
+        # both sides are bf16-rounded GPU results and the partials are bf16 as well (R19): the max-abs bar is
+        # twice the GPU-vs-oracle one; the oracle comparison of the merged result follows on the sampled rows
+        assert e_rel < 4e-3 and e_max < 6e-2, f"P={P}: rel {e_rel:.2e} max {e_max:.2e}"
+        check(om[rows.to(DEV)], ro, torch.bfloat16, f"merged P={P} sampled rows")
+        assert float((lm - lse).abs().max()) < 1e-3
