@@ -39,11 +39,15 @@ UNIT = "steps/s"
 
 
 def _shape(workload: str):
-    if workload == "cfg2":
+    if workload in ("cfg2", "cfg4"):
         return synth.cfg2()
     if workload == "cfg3":
         return synth.cfg3()
     raise SystemExit(f"unknown workload {workload}")
+
+
+CFG4_NAME = ("BASELINE.json configs[3]: packed varlen batch bf16, cfg2 block shape, 6 requests "
+             "{1024,1024,4096,4096,9216,16384} + 256 text tokens each (37376 packed tokens)")
 
 
 def _workload_name(s) -> str:
@@ -51,13 +55,16 @@ def _workload_name(s) -> str:
             "cfg3_video_bf16": "BASELINE.json configs[2]: video DiT bf16, 4 blocks, D=5120, 40x128, 32760 tokens, cross-attn 512"}[s.name]
 
 
-def step_flops(s) -> dict:
-    """Algorithmic FLOPs of one step (2 per multiply-add; dense non-causal attention 4*Nq*Nk*d*H) — DESIGN.md §6."""
+def step_flops(s, seq_lens=None) -> dict:
+    """Algorithmic FLOPs of one step (2 per multiply-add; dense non-causal attention 4*Nq*Nk*d*H) — DESIGN.md §6.
+    seq_lens: per-request sequence lengths of a packed batch (attention is block-diagonal)."""
     D, F, H, d, L = s.hidden, s.mlp_dim, s.n_heads, s.head_dim, s.n_blocks
     N = s.n_tokens
     T = N + (s.n_cond if s.cond_mode == "joint" else 0)
+    if seq_lens is not None:
+        T = sum(seq_lens)
     gemm = L * (2 * T * D * 3 * D + 2 * T * D * D + 2 * 2 * T * D * F)
-    attn = L * 4 * T * T * d * H
+    attn = L * 4 * (T * T if seq_lens is None else sum(t * t for t in seq_lens)) * d * H
     n_gemm = 4 * L
     if s.cond_mode == "cross":
         gemm += L * (2 * 2 * T * D * D + 2 * s.n_cond * D * 2 * D)
@@ -168,6 +175,8 @@ class OracleSample:
 def run_reference(args, rank: int):
     if rank != 0:
         return
+    if args.workload == "cfg4":
+        raise SystemExit("--impl reference: the oracle arm is defined for cfg2 / cfg3")
     s = _shape(args.workload)
     torch.set_num_threads(os.cpu_count() or 1)
     smp = OracleSample(s)
@@ -204,16 +213,59 @@ def run_ours(args, rank: int, local_rank: int, world: int):
             dist.barrier()
 
     s = _shape(args.workload)
-    fl = step_flops(s)
     W = synth.make_weights(s, device=dev)
-    m = B.Dit(B.make_config(s, split_p=args.split_p), W, dev)
-    I = synth.make_inputs(s, device=dev, tag=f".rank{rank}")
-    lat, temb, cond = I["latents"], I["temb"][0].contiguous(), I["cond"]
-    out = torch.empty_like(lat)
     K, Wm = args.steps, args.warmup
+    if args.workload == "cfg4":
+        # packed varlen batch: R requests through ONE dit_step_varlen call per step
+        shapes = synth.cfg4_requests()
+        R = len(shapes)
+        ts = [float(synth.uniform01(7, f"t{r}", 1)[0]) * 1000 for r in range(R)]
+        Is = [synth.make_inputs(sh, device=dev, tag=f".r{r}.rank{rank}", t=ts[r]) for r, sh in enumerate(shapes)]
+        seq = [sh.n_tokens + sh.n_cond for sh in shapes]
+        fl = step_flops(s, seq)
+        m = B.Dit(B.make_config(shapes[-1], split_p=args.split_p, max_tokens=sum(seq), max_requests=R,
+                                max_cond_tokens=sum(sh.n_cond for sh in shapes)), W, dev)
+        lats, conds = [i["latents"] for i in Is], [i["cond"] for i in Is]
+        tembs = torch.cat([i["temb"] for i in Is]).contiguous()
+        lats_h = [l.cpu().pin_memory() for l in lats]
+        conds_h = [c.cpu().pin_memory() for c in conds]
+        tembs_h = tembs.cpu().pin_memory()
+        outs_h = [torch.empty_like(l) for l in lats_h]
+        h2d = sum(t.numel() * t.element_size() for t in lats_h + conds_h + [tembs_h])
+        d2h = sum(t.numel() * t.element_size() for t in outs_h)
+
+        def step():
+            return m.dit_step_varlen(lats, tembs, conds)
+
+        def step_e2e():   # pinned host -> device copies, the packed step, device -> host read of every output
+            for dst, src in zip(lats + conds + [tembs], lats_h + conds_h + [tembs_h]):
+                dst.copy_(src, non_blocking=True)
+            outs = m.dit_step_varlen(lats, tembs, conds)
+            for dst, src in zip(outs_h, outs):
+                dst.copy_(src, non_blocking=True)
+        wl_name, req_per_gpu = CFG4_NAME, R
+    else:
+        fl = step_flops(s)
+        m = B.Dit(B.make_config(s, split_p=args.split_p), W, dev)
+        I = synth.make_inputs(s, device=dev, tag=f".rank{rank}")
+        lat, temb, cond = I["latents"], I["temb"][0].contiguous(), I["cond"]
+        out = torch.empty_like(lat)
+        lat_h, temb_h = lat.cpu().pin_memory(), temb.cpu().pin_memory()
+        cond_h = None if cond is None else cond.cpu().pin_memory()
+        out_h = torch.empty_like(lat_h).pin_memory()
+        h2d = lat_h.numel() * lat_h.element_size() + temb_h.numel() * 4 + (0 if cond_h is None else cond_h.numel() * cond_h.element_size())
+        d2h = out_h.numel() * out_h.element_size()
+
+        def step():
+            return m.dit_step(lat, temb, cond, out)
+
+        def step_e2e():   # dit_step_host: the C-ABI call with HOST buffers (copies are enqueued by the library)
+            m.dit_step_host(lat_h, temb_h, cond_h, out_h)
+        wl_name, req_per_gpu = _workload_name(s), 1
+    weight_gb = sum(v.numel() * v.element_size() for v in W.values()) / 1e9
 
     for _ in range(Wm):
-        m.dit_step(lat, temb, cond, out)
+        step()
     torch.cuda.synchronize()
 
     # ---- timed region: K steps, device-resident inputs; GEMM-class launches bracketed by events (roofline)
@@ -225,7 +277,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     B.dit_profile_begin(("gemm",))
     e0.record()
     for _ in range(K):
-        m.dit_step(lat, temb, cond, out)
+        step()
     e1.record()
     torch.cuda.synchronize(); barrier()
     prof = B.dit_profile_end()
@@ -234,28 +286,23 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     ms_total = e0.elapsed_time(e1)
 
     # ---- e2e: dit_step_host, pinned host buffers, H2D + step + D2H per step inside the timed region
-    lat_h, temb_h = lat.cpu().pin_memory(), temb.cpu().pin_memory()
-    cond_h = None if cond is None else cond.cpu().pin_memory()
-    out_h = torch.empty_like(lat_h).pin_memory()
     for _ in range(min(Wm, 3)):
-        m.dit_step_host(lat_h, temb_h, cond_h, out_h)
+        step_e2e()
     torch.cuda.synchronize()
     barrier(); torch.cuda.synchronize()
     f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     f0.record()
     for _ in range(K):
-        m.dit_step_host(lat_h, temb_h, cond_h, out_h)
+        step_e2e()
         torch.cuda.current_stream().synchronize()      # the step's result is on the host before the next step starts
     f1.record()
     torch.cuda.synchronize(); barrier()
     ms_e2e = f0.elapsed_time(f1)
-    h2d = lat_h.numel() * lat_h.element_size() + temb_h.numel() * 4 + (0 if cond_h is None else cond_h.numel() * cond_h.element_size())
-    d2h = out_h.numel() * out_h.element_size()
 
     # ---- per-class breakdown (separate, untimed-for-value pass with every class bracketed)
     B.dit_profile_begin()
     for _ in range(max(1, min(K, 5))):
-        m.dit_step(lat, temb, cond, out)
+        step()
     torch.cuda.synchronize()
     prof_all = B.dit_profile_end()
     nb = max(1, min(K, 5))
@@ -274,14 +321,15 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         if os.path.exists(tp):
             for ln in open(tp).read().splitlines()[1:]:
                 f = ln.split(",")
-                if len(f) >= 3 and f[0] == args.workload and f[1] == "gemm":
+                if len(f) >= 3 and f[0] == ("cfg2" if args.workload == "cfg4" else args.workload) and f[1] == "gemm":
                     traffic = int(f[2])
         line = {
             "metric": METRIC, "value": world * K / (ms_total * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
             "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
             "data": "synthetic",
-            "config": {"workload": _workload_name(s), "split_p": args.split_p, "requests_per_gpu": 1,
-                       "l2": "inputs exceed L2: each step streams 2.7 GB of weights (cfg2) through a 126 MB L2",
+            "config": {"workload": wl_name, "split_p": args.split_p, "requests_per_gpu": req_per_gpu,
+                       "l2": f"inputs exceed L2: every step streams {weight_gb:.1f} GB of weights (plus activations) "
+                             "through a 126 MB L2, so no step starts with its operands cached",
                        "parallelism": f"replicas x{world} (independent requests, no data-path collective)"},
             "clocks": clocks,
             "e2e": {"value": world * K / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
@@ -297,7 +345,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
                        "gemm": (fl["gemm"] * nb) / (prof_all["gemm"][0] * 1e-3) / 1e12 if prof_all["gemm"][0] > 0 else None,
                        "step_total": (fl["gemm"] + fl["attn"]) * K / (ms_total * 1e-3) / 1e12},
         }
-        if world == 1 and not args.no_cpu_baseline:
+        if world == 1 and not args.no_cpu_baseline and args.workload != "cfg4":
             torch.set_num_threads(os.cpu_count() or 1)
             smp = OracleSample(s)
             sec = smp.step_seconds()
@@ -413,10 +461,10 @@ def run_kernels(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "kernels"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "kernels"])
     ap.add_argument("--split-p", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--only", default="", help="--workload kernels: time only the kernels whose name contains this")

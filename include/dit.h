@@ -177,6 +177,18 @@ dit_status dit_linear_residual(int32_t dtype, const void* A, int64_t lda, const 
                                int64_t ldx, const float* gate, int64_t gate_stride, const int32_t* cu_seqlens_dev,
                                int32_t n_requests, int32_t M, int32_t N, int32_t K, void* stream);
 
+/* QKV projection with QK-RMSNorm and RoPE fused into the GEMM epilogue (north_star subsystems 3 + 4: "QK-RMSNorm and
+ * RoPE fused into the Q/K load" — here one step earlier, on the fp32 accumulators, so q and k are rounded to bf16
+ * exactly once, readings R5 / R6):
+ *   [q | k | v] = A[M, K] W[3D, K]^T + bias[3D];   per head (128 columns) of q and k:
+ *   x <- x / sqrt(mean_d(x^2) + rms_eps) (.) g   (g_q / g_k dev [128] in dtype, NULL = no norm), then
+ *   (x_2j, x_2j+1) <- (x_2j cos - x_2j+1 sin, x_2j sin + x_2j+1 cos) with rope_cos / rope_sin dev fp32 [M, 64]
+ *   (NULL = no RoPE);  v heads get the bias only.  out dev [M, ldo] in dtype.
+ * bf16, head_dim 128, D % 128 == 0 only (DIT_ERR_UNSUPPORTED otherwise: call dit_linear + dit_qknorm_rope). */
+dit_status dit_linear_qkv(int32_t dtype, const void* A, int64_t lda, const void* W, const void* bias, void* out,
+                          int64_t ldo, const void* g_q, const void* g_k, float rms_eps, const float* rope_cos,
+                          const float* rope_sin, int32_t hidden, int32_t M, int32_t K, void* stream);
+
 /* adaLN-Zero modulation kernel (north_star subsystem 2), one pass over the row:
  *   if h != NULL:  x <- x + gate (.) h          (gate NULL = 1)       [x fp32 in/out, h dtype]
  *   y = LN(x) (.) (1 + scale) + shift           (shift/scale NULL = 0) [y dtype]

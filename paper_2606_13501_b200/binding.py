@@ -19,7 +19,7 @@ TAP = dict(x=0, y=1, qkv=2, o=3, u=5, c=6, mod=7, tok=8)
 STAGE = dict(y1=0, qkv=1, attn=2, oproj=3, cross=4, y2=5, fc1=6, fc2=7)
 
 SYMBOLS = ["dit_workspace_bytes", "dit_init", "dit_step", "dit_step_host", "dit_step_varlen", "dit_attn_partial",
-           "dit_attn_merge", "dit_linear", "dit_linear_residual", "dit_adaln", "dit_gemv", "dit_qknorm_rope", "dit_debug_stop_after",
+           "dit_attn_merge", "dit_linear", "dit_linear_residual", "dit_linear_qkv", "dit_adaln", "dit_gemv", "dit_qknorm_rope", "dit_debug_stop_after",
            "dit_get_tap", "dit_profile_begin", "dit_profile_end", "dit_last_error", "dit_kernel_launches", "dit_free"]
 
 
@@ -70,6 +70,7 @@ def load(path: str = LIB_PATH):
         "dit_attn_merge": [i32, C.POINTER(vp), C.POINTER(vp), i32, i32, i32, i32, vp, vp, vp],
         "dit_linear": [i32, i32, vp, i64, vp, vp, vp, i64, i32, i32, i32, vp],
         "dit_linear_residual": [i32, vp, i64, vp, vp, vp, i64, vp, i64, vp, i32, i32, i32, i32, vp],
+        "dit_linear_qkv": [i32, vp, i64, vp, vp, vp, i64, vp, vp, f32, vp, vp, i32, i32, i32, vp],
         "dit_adaln": [i32, vp, vp, vp, vp, vp, i64, vp, i32, vp, i32, i32, f32, vp],
         "dit_gemv": [i32, vp, vp, vp, vp, i32, i32, i32, i32, vp],
         "dit_qknorm_rope": [i32, vp, i64, i32, i32, i32, i32, vp, vp, f32, vp, vp, vp],
@@ -259,6 +260,16 @@ def dit_linear_residual(A, W, x, bias=None, gate=None, gate_stride=0, cu_seqlens
                                    gate_stride, _ptr(cu_seqlens), n_requests, M, N, K, _stream(stream)),
            "dit_linear_residual")
     return x
+
+
+def dit_linear_qkv(A, W, bias, hidden, gq=None, gk=None, eps=1e-6, rope_cos=None, rope_sin=None, stream=None):
+    """[q | k | v] = A W^T + bias with QK-RMSNorm + RoPE in the GEMM epilogue -> [M, 3 hidden] (bf16, head_dim 128)."""
+    lib = load()
+    M, K = A.shape
+    out = torch.empty((M, 3 * hidden), dtype=A.dtype, device=A.device)
+    _check(lib.dit_linear_qkv(_dt(A), _ptr(A), A.stride(0), _ptr(W), _ptr(bias), _ptr(out), out.stride(0), _ptr(gq), _ptr(gk),
+                              eps, _ptr(rope_cos), _ptr(rope_sin), hidden, M, K, _stream(stream)), "dit_linear_qkv")
+    return out
 
 
 def dit_adaln(x, y_dtype, h=None, gate=None, shift=None, scale=None, mod_stride=0, cu_seqlens=None, n_requests=1,

@@ -1,25 +1,32 @@
 // attn_tc.cu — non-causal flash attention on tcgen05 tensor cores (north_star subsystems 4 and 5), head_dim 128, bf16.
 //   for every query row i of a request, over the key rows of this call's KV shard:
 //     s_ij = scale * q_i . k_j ;  o_i = sum_j softmax_j(s_ij) v_j ;  lse_i = ln sum_j exp(s_ij)        (R7, R18)
-// Design (sm_100a), one CTA = one (request, head, 256 query rows) work item, 384 threads:
+// Design (sm_100a), one CTA = one (request, head, 256 query rows) work item, 640 threads:
 //   warp 0      TMA producer: two Q tiles (128 x 128) once, then a K ring and a V ring of 128-key tiles
 //               (each tile = two 128 x 64 boxes, 128-byte swizzle);
-//   warp 1      MMA issuer (one thread).  Keys are consumed in SUB-TILES of 64: S_t,i = Q_t K_i^T (M=128, N=64,
-//               K=16 x 8) into one of TWO 64-column S buffers per Q tile, O_t += P_t,i V_i (M=128, N=128, K=16 x 4)
-//               with P read from TMEM (A operand in tensor memory) and V as an MN-major shared-memory operand.
-//               S_t,i+2 is issued right after PV_t,i (same buffer, in-order tensor pipe), so while a softmax
-//               warpgroup works on sub-tile i the scores of sub-tile i+1 are already in TMEM: neither side waits
-//               on a round trip through the other;
-//   warps 4-7   softmax warpgroup of Q tile 0, warps 8-11 of Q tile 1: one thread owns one query row — tcgen05.ld
-//               of the 64 scores, row max, exp2 with the scale folded into one packed FFMA2, bf16 P written back
-//               over the first 32 columns of the S buffer (tcgen05.st), fp32 row sum (packed FADD2).  A quarter of
-//               the exponentials is evaluated on the FMA pipe (round-to-nearest split + minimax cubic, rel. error
-//               7.5e-5 << bf16 rounding of P) because MUFU.EX2 (16 / clk / SM) would otherwise need exactly as many
-//               cycles as the two MMAs of the tile.  O is rescaled lazily: only when the running max grows by more
-//               than 2^8 (exact: the same max is used for P and for the sum, and divided out at the end);
-//   epilogue    the same warpgroups: O / l -> bf16 -> global, lse = ln2 * (m + log2 l).
+//   warp 1      MMA issuer (one elected thread).  Per key tile j and Q tile t:  S_t = Q_t K_j^T as ONE N = 128 group
+//               (M=128, N=128, K=16 x 8: 8 KB of shared memory per 64-cycle MMA = the 128 B/clk feed limit; measured:
+//               N = 64 groups take 48 instead of 32 cycles each) into the two 64-column buffers S_t,a | S_t,b; then
+//               O_t += P_t,a V_j[0:64] and O_t += P_t,b V_j[64:128] (M=128, N=128, K=16 x 4 each) with P read from
+//               TMEM (A operand in tensor memory) and V as an MN-major shared-memory operand; then S_t of tile j+1
+//               (the tensor pipe executes in issue order, so it may overwrite the P buffers right behind the PVs).
+//               t = 0 is served completely before t = 1: one tile's softmax runs under the other tile's MMAs;
+//   warps 4-19  softmax: Q tile t has TWO warps per TMEM lane quadrant — the leader owns sub-tile a (keys 0..63 of
+//               every key tile), the follower sub-tile b — so four softmax warps share a scheduler.  One thread =
+//               one query row x 64 keys: tcgen05.ld, half-row max, exchange of the two half-row maxima through
+//               shared memory + a named barrier (both threads then take the SAME lazy-rescale decision), exp2 with
+//               the scale folded into one packed FFMA2, bf16 P written over the first 32 columns of the S buffer
+//               (tcgen05.st), fp32 row sum (packed FADD2).  An eighth of the exponentials runs on the FMA pipe
+//               (round-to-nearest split + minimax cubic, rel. error 7.5e-5 << bf16 rounding of P) to take load off
+//               MUFU.EX2 (16 / clk / SM: as many cycles as the tile's MMAs).  O is rescaled lazily: only when the
+//               running max grows by more than 2^8 (exact: the same max is used for P and for the sum, and divided
+//               out at the end); the leader rescales O_t, both threads rescale their partial row sums;
+//   epilogue    the pair adds its partial sums; leader writes O columns 0..63, follower 64..127: O / l -> bf16,
+//               lse = ln2 * (m + log2 l).
 // TMEM: S0a S0b | S1a S1b | O0 | O1 = 4 x 128 fp32 columns = all 512; P_t,b aliases the first 32 columns of S_t,b.
-// Roofline: tensor pipe, co-limited by MUFU.EX2 and FMA issue slots.
+// Registers: 640 threads x 96 at launch; setmaxnreg moves the control warps to 40 and the softmax warps to 104
+// (the pool is the CTA's launch allocation: asking for more than the control warps release never returns).
+// Roofline: tensor pipe; the softmax instruction stream (~4.5 issue slots per score) is co-critical.
 #include "tc.cuh"
 
 namespace dit {

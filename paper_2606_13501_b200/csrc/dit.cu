@@ -280,9 +280,17 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
     const float* m = w.mod + (size_t)l * 6 * D;
     RUN(launch_adaln(dt, w.x, nullptr, nullptr, m + 0 * D, m + 1 * D, mod_stride, cu_dev, R, w.y, T, D, c.ln_eps, st));
     if (stop(l, DIT_STAGE_Y1)) return DIT_OK;
-    RUN(gemm(dt, DIT_EPI_BIAS, w.y, D, b.wqkv, b.bqkv, w.qkv, 3 * D, T, 3 * D, D, st));
-    RUN(launch_qknorm_rope(dt, w.qkv, 3 * D, T, H, d, 2, c.qk_rmsnorm ? b.gq : nullptr, c.qk_rmsnorm ? b.gk : nullptr,
-                           c.rms_eps, rope ? w.rope_c : nullptr, rope ? w.rope_s : nullptr, st));
+    if (dt == DIT_BF16 && d == 128 && (c.qk_rmsnorm || rope) &&
+        gemm_tc_supported(DIT_EPI_BIAS, w.y, D, b.wqkv, w.qkv, 3 * D, T, 3 * D, D)) {
+      // QK-RMSNorm + RoPE on the fp32 accumulators in the QKV GEMM's epilogue (north_star subsystems 3 + 4)
+      RUN(launch_gemm_tc_qkv(w.y, D, b.wqkv, b.bqkv, w.qkv, 3 * D, c.qk_rmsnorm ? b.gq : nullptr,
+                             c.qk_rmsnorm ? b.gk : nullptr, c.rms_eps, rope ? w.rope_c : nullptr,
+                             rope ? w.rope_s : nullptr, D, T, 3 * D, D, st));
+    } else {
+      RUN(gemm(dt, DIT_EPI_BIAS, w.y, D, b.wqkv, b.bqkv, w.qkv, 3 * D, T, 3 * D, D, st));
+      RUN(launch_qknorm_rope(dt, w.qkv, 3 * D, T, H, d, 2, c.qk_rmsnorm ? b.gq : nullptr, c.qk_rmsnorm ? b.gk : nullptr,
+                             c.rms_eps, rope ? w.rope_c : nullptr, rope ? w.rope_s : nullptr, st));
+    }
     if (stop(l, DIT_STAGE_QKV)) return DIT_OK;
     {
       AttnArgs a;
@@ -572,6 +580,20 @@ dit_status dit_linear_residual(int32_t dtype, const void* A, int64_t lda, const 
               "n_requests %d (cu_seqlens required when > 1)", n_requests);
   return gemm_residual(dtype, A, lda, W, bias, x, ldx, gate, gate_stride, cu_seqlens_dev, n_requests, M, N, K,
                        (cudaStream_t)stream);
+}
+
+dit_status dit_linear_qkv(int32_t dtype, const void* A, int64_t lda, const void* W, const void* bias, void* out,
+                          int64_t ldo, const void* g_q, const void* g_k, float rms_eps, const float* rope_cos,
+                          const float* rope_sin, int32_t hidden, int32_t M, int32_t K, void* stream) {
+  DIT_REQUIRE(M >= 0 && K > 0 && hidden > 0 && lda >= K && ldo >= 3 * (int64_t)hidden, DIT_ERR_INVALID_ARG,
+              "bad QKV shape M=%d K=%d hidden=%d lda=%lld ldo=%lld", M, K, hidden, (long long)lda, (long long)ldo);
+  DIT_REQUIRE(M == 0 || (A && W && out), DIT_ERR_INVALID_ARG, "NULL argument");
+  DIT_REQUIRE((rope_cos == nullptr) == (rope_sin == nullptr), DIT_ERR_INVALID_ARG, "rope_cos / rope_sin must both be given");
+  DIT_REQUIRE(dtype == DIT_BF16 && hidden % 128 == 0 &&
+                  gemm_tc_supported(DIT_EPI_BIAS, A, lda, W, out, ldo, M > 0 ? M : 1, 3 * hidden, K),
+              DIT_ERR_UNSUPPORTED, "dit_linear_qkv: bf16, head_dim 128, 16-byte aligned operands, sm_100 only");
+  return launch_gemm_tc_qkv(A, lda, W, bias, out, ldo, g_q, g_k, rms_eps, rope_cos, rope_sin, hidden, M, 3 * hidden, K,
+                            (cudaStream_t)stream);
 }
 
 dit_status dit_adaln(int32_t dtype, float* x, const void* h, const float* gate, const float* shift, const float* scale,

@@ -59,7 +59,7 @@ constexpr int smem_bytes(int bn) {
   return STAGES * stage_bytes(bn) + 1024 /* alignment slack */ + 256 /* barriers */ +
          2 * 2 * BN_MAX * 4 /* bias + gate rows of the tile, fp32, one set per accumulator stage */;
 }
-enum { EPI_GATE_RESID = 3 };
+enum { EPI_GATE_RESID = 3, EPI_QKV_NORM_ROPE = 4 };
 
 struct EpiArgs {
   const bf16* bias;       // [N] or nullptr
@@ -69,6 +69,11 @@ struct EpiArgs {
   int64_t gate_stride;
   const int32_t* cu;      // row -> request (nullptr: one request)
   int R;
+  // EPI_QKV_NORM_ROPE (head_dim 128): columns [0, D) = q heads, [D, 2D) = k heads, [2D, 3D) = v heads
+  const bf16* gq; const bf16* gk;   // RMSNorm gains [128] (nullptr: no norm)
+  const float* rc; const float* rs; // RoPE tables [M, 64] (nullptr: no RoPE)
+  float rms_eps;
+  int D;
 };
 
 __device__ __forceinline__ float gelu_tanh_fast(float z) {
@@ -194,6 +199,12 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
 #pragma unroll
         for (int i = et; i < BN; i += EPI_THREADS) s_gate[i] = (n0 + i < N) ? g0[n0 + i] : 0.f;
       }
+      if (EPI == EPI_QKV_NORM_ROPE) {   // the two gain vectors: s_gate[0..127] = g_q, s_gate[128..255] = g_k
+        for (int i = et; i < 256; i += EPI_THREADS) {
+          const bf16* g = i < 128 ? ep.gq : ep.gk;
+          s_gate[i] = g != nullptr ? __bfloat162float(g[i & 127]) : 1.f;
+        }
+      }
 #pragma unroll
       for (int i = et; i < BN; i += EPI_THREADS)
         s_bias[i] = (ep.bias != nullptr && n0 + i < N) ? __bfloat162float(ep.bias[n0 + i]) : 0.f;
@@ -217,6 +228,73 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       mbar_wait(tfull_bar(as), aph);
       tc_fence_after();
       const uint32_t t_addr = tmem_base + as * BN_MAX + ((uint32_t)(quad * 32) << 16);
+      if (EPI == EPI_QKV_NORM_ROPE) {
+        // QKV projection with QK-RMSNorm (R5) and RoPE (R6) applied to the fp32 accumulators before the one and
+        // only bf16 rounding: per 128-column head, pass 1 reads the accumulator row for sum(q^2), pass 2 reads it
+        // again (TMEM reads are cheap), scales by rsqrt * gain, rotates interleaved pairs, stores.  v heads: bias.
+        bf16* const orow = reinterpret_cast<bf16*>(ep.out) + (int64_t)(row_ok ? row : 0) * ep.ldo + n0;
+        const float* const rcr = ep.rc != nullptr ? ep.rc + (int64_t)(row_ok ? row : 0) * 64 : nullptr;
+        const float* const rsr = ep.rs != nullptr ? ep.rs + (int64_t)(row_ok ? row : 0) * 64 : nullptr;
+#pragma unroll 1
+        for (int hh = 0; hh < BN / 128; ++hh) {
+          const int nh = n0 + hh * 128;
+          if (nh >= N) break;  // warp-uniform
+          const int which = nh / ep.D;                         // 0 = q, 1 = k, 2 = v
+          const bool norm = which < 2 && (which == 0 ? ep.gq : ep.gk) != nullptr;
+          const bool rope = which < 2 && rcr != nullptr;
+          const float* const sg = s_gate + (which == 1 ? 128 : 0);
+          float rinv = 1.0f;
+          if (norm) {
+            float ss = 0.f;
+#pragma unroll 1
+            for (int c4 = 0; c4 < 4; ++c4) {
+              uint32_t r[32];
+              tmem_ld32(t_addr + hh * 128 + c4 * 32, r);
+              tmem_ld_wait();
+#pragma unroll
+              for (int e = 0; e < 32; ++e) {
+                const float v = __uint_as_float(r[e]) + s_bias[hh * 128 + c4 * 32 + e];
+                ss = fmaf(v, v, ss);
+              }
+            }
+            rinv = rsqrtf(ss * (1.0f / 128.0f) + ep.rms_eps);
+          }
+#pragma unroll 1
+          for (int c4 = 0; c4 < 4; ++c4) {
+            uint32_t r[32];
+            tmem_ld32(t_addr + hh * 128 + c4 * 32, r);
+            float cs[16], sn[16];
+            if (rope) {
+#pragma unroll
+              for (int g = 0; g < 4; ++g) {
+                const float4 a = __ldg(reinterpret_cast<const float4*>(rcr + c4 * 16 + g * 4));
+                const float4 b = __ldg(reinterpret_cast<const float4*>(rsr + c4 * 16 + g * 4));
+                cs[g * 4 + 0] = a.x; cs[g * 4 + 1] = a.y; cs[g * 4 + 2] = a.z; cs[g * 4 + 3] = a.w;
+                sn[g * 4 + 0] = b.x; sn[g * 4 + 1] = b.y; sn[g * 4 + 2] = b.z; sn[g * 4 + 3] = b.w;
+              }
+            }
+            tmem_ld_wait();
+            float v[32];
+#pragma unroll
+            for (int e = 0; e < 32; ++e) {
+              v[e] = __uint_as_float(r[e]) + s_bias[hh * 128 + c4 * 32 + e];
+              if (norm) v[e] = v[e] * rinv * sg[c4 * 32 + e];
+            }
+            if (rope) {
+#pragma unroll
+              for (int j = 0; j < 16; ++j) {
+                const float a = v[2 * j], b = v[2 * j + 1];
+                v[2 * j] = a * cs[j] - b * sn[j];
+                v[2 * j + 1] = a * sn[j] + b * cs[j];
+              }
+            }
+            if (row_ok) {
+#pragma unroll
+              for (int g = 0; g < 4; ++g) st8<bf16>(orow + hh * 128 + c4 * 32 + g * 8, &v[g * 8]);
+            }
+          }
+        }
+      } else
 #pragma unroll 1
       for (int c = 0; c < (BN + 31) / 32; ++c) {
         const int n = n0 + c * 32;
@@ -346,7 +424,7 @@ dit_status launch_gemm_tc_ex(int epi, const void* A, int64_t lda, const void* W,
   const int bn = pick_bn(M, N);
   DIT_REQUIRE(make_tmap_2d_bf16(&ta, A, M, K, lda, BM, BK) && make_tmap_2d_bf16(&tb, W, N, K, K, bn, BK), DIT_ERR_CUDA,
               "gemm_tc: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d lda=%lld)", M, N, K, (long long)lda);
-  EpiArgs ep{(const bf16*)bias, out, ldo, gate, gate_stride, cu, R};
+  EpiArgs ep{(const bf16*)bias, out, ldo, gate, gate_stride, cu, R, nullptr, nullptr, nullptr, nullptr, 0.f, 0};
   ProfScope _prof(DIT_KC_GEMM, st);
   switch (epi) {
     case DIT_EPI_BIAS: return launch_bn<DIT_EPI_BIAS>(bn, ta, tb, ep, M, N, K, st);
@@ -355,6 +433,21 @@ dit_status launch_gemm_tc_ex(int epi, const void* A, int64_t lda, const void* W,
     case EPI_GATE_RESID: return launch_bn<EPI_GATE_RESID>(bn, ta, tb, ep, M, N, K, st);
     default: DIT_REQUIRE(false, DIT_ERR_INVALID_ARG, "gemm_tc: epilogue %d", epi);
   }
+}
+
+// QKV projection with QK-RMSNorm + RoPE in the epilogue (head_dim 128; N = 3 D, D % 128 == 0).  256-wide tiles only:
+// a tile is two whole heads.
+dit_status launch_gemm_tc_qkv(const void* A, int64_t lda, const void* W, const void* bias, void* out, int64_t ldo,
+                              const void* gq, const void* gk, float rms_eps, const float* rc, const float* rs, int D, int M,
+                              int N, int K, cudaStream_t st) {
+  if (M == 0 || N == 0) return DIT_OK;
+  DIT_REQUIRE(D % 128 == 0 && N == 3 * D, DIT_ERR_INVALID_ARG, "gemm_tc_qkv: N=%d D=%d", N, D);
+  CUtensorMap ta, tb;
+  DIT_REQUIRE(make_tmap_2d_bf16(&ta, A, M, K, lda, BM, BK) && make_tmap_2d_bf16(&tb, W, N, K, K, 256, BK), DIT_ERR_CUDA,
+              "gemm_tc_qkv: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d)", M, N, K);
+  EpiArgs ep{(const bf16*)bias, out, ldo, nullptr, 0, nullptr, 1, (const bf16*)gq, (const bf16*)gk, rc, rs, rms_eps, D};
+  ProfScope _prof(DIT_KC_GEMM, st);
+  return launch_t<EPI_QKV_NORM_ROPE, 256>(ta, tb, ep, M, N, K, st);
 }
 
 dit_status launch_gemm_tc(int epi, const void* A, int64_t lda, const void* W, const void* bias, void* out, int64_t ldo,

@@ -143,6 +143,37 @@ def test_linear(lib, dtype, M, N, K, epi):
         check_rounding(got, ref, f"linear {M}x{N}x{K} epi{epi}")
 
 
+@pytest.mark.parametrize("M,H,K", [(1, 1, 64), (300, 3, 256), (515, 2, 1032), (129, 5, 128)])
+@pytest.mark.parametrize("norm,rope", [(True, True), (True, False), (False, True)])
+def test_linear_qkv_fused_norm_rope_epilogue(lib, M, H, K, norm, rope):
+    """QKV projection with QK-RMSNorm + RoPE in the GEMM epilogue against the definition written out with the
+    oracle's pieces: linear -> per-head RMSNorm of q, k (gains g_q, g_k) -> RoPE on interleaved pairs; v untouched.
+    H odd: the last 256-column tile holds one head of v only; M spans several row tiles with a ragged tail."""
+    dt, d = torch.bfloat16, 128
+    D = H * d
+    A = rnd("A", (M, K), dt)
+    W, b = rnd("W", (3 * D, K), dt, std=1.0 / math.sqrt(K)), rnd("b", (3 * D,), dt, std=0.5)
+    gq, gk = rnd("gq", (d,), dt, std=0.1, mean=1.0), rnd("gk", (d,), dt, std=0.1, mean=1.0)
+    ang = rnd("ang", (M, d // 2), torch.float32, std=2.0).double().cpu()
+    rc, rs = torch.cos(ang).float().to(DEV), torch.sin(ang).float().to(DEV)
+    got = B.dit_linear_qkv(A, W, b, D, gq if norm else None, gk if norm else None, 1e-6, rc if rope else None,
+                           rs if rope else None)
+    qkv = O.linear(A.double().cpu(), W.cpu(), b.cpu())
+    q, k, v = (qkv[:, i * D:(i + 1) * D].reshape(M, H, d) for i in range(3))
+    if norm:
+        q, k = O.rms_norm_heads(q, gq.double().cpu(), 1e-6), O.rms_norm_heads(k, gk.double().cpu(), 1e-6)
+    if rope:   # the tables the kernel consumes are fp32: rotate with exactly those values
+        a32 = (rc.double().cpu(), rs.double().cpu())
+        def rot(x):
+            x2 = x.reshape(M, H, d // 2, 2)
+            c_, s_ = a32[0][:, None, :], a32[1][:, None, :]
+            return torch.stack([x2[..., 0] * c_ - x2[..., 1] * s_, x2[..., 0] * s_ + x2[..., 1] * c_], dim=-1).reshape(M, H, d)
+        q, k = rot(q), rot(k)
+    ref = torch.cat([q.reshape(M, D), k.reshape(M, D), v.reshape(M, D)], dim=1)
+    check(got, ref, dt, f"linear_qkv {M}x{H}x{K}", rel=3e-3, maxabs=3e-2)
+    check_rounding(got, ref, f"linear_qkv {M}x{H}x{K}")       # fp32 up to the single bf16 rounding
+
+
 @pytest.mark.parametrize("dtype", DTYPES)
 def test_linear_strided_views_and_no_bias(lib, dtype):
     """A and out are column slices of wider buffers (the step's qkv / packed layouts)."""
