@@ -88,7 +88,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                int K) {
   extern __shared__ uint8_t smem_raw[];
   constexpr int B_BYTES = BN * BK * 2, STAGE_BYTES = A_BYTES + B_BYTES;   // both multiples of 1024 (swizzle atom)
-  static_assert(BN % 16 == 0 && BN <= BN_MAX && STAGE_BYTES % 1024 == 0, "tile width");
+  static_assert(BN % 16 == 0 && BN <= BN_MAX && STAGE_BYTES % 1024 == 0 && (B_BYTES / 2) % 1024 == 0, "tile width");
   const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t bar0 = smem0 + STAGES * STAGE_BYTES;
   // barriers: full[STAGES], empty[STAGES], tfull[2], tempty[2]; then the TMEM base address word
@@ -99,7 +99,12 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   const uint32_t tmem_slot = bar0 + 8u * (2 * STAGES + 4);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int mt = (M + BM - 1) / BM, nt = (N + BN - 1) / BN, n_tiles = mt * nt;
+  // CTA pairs (cluster of 2): the pair works on two vertically adjacent row tiles of the same column tile and shares
+  // the W tile — each CTA fetches half of it and TMA-multicasts the half into both CTAs' shared memory, which cuts
+  // the L2 -> SM traffic of a stage from A + W to A + W/2.  Every MMA is still a 1-CTA M = 128 instruction.
+  const int rank = (int)cluster_ctarank();
+  const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
+  const int mt = (M + BM - 1) / BM, mt2 = (mt + 1) >> 1, nt = (N + BN - 1) / BN, n_tiles = mt2 * nt;   // tile PAIRS
   const int nkb = (K + BK - 1) / BK;
 
   if (warp == 0 && lane == 0) {
@@ -109,7 +114,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   if (warp == 1 && lane == 0) {
     for (int s = 0; s < STAGES; ++s) {
       mbar_init(full_bar(s), 1);
-      mbar_init(empty_bar(s), 1);
+      mbar_init(empty_bar(s), 2);   // released by this CTA's MMA warp AND the peer's (its half of W lands here too)
     }
     for (int s = 0; s < 2; ++s) {
       mbar_init(tfull_bar(s), 1);
@@ -120,6 +125,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   if (warp == 2) tmem_alloc<512>(tmem_slot);
   tc_fence_before();
   __syncthreads();
+  cluster_sync_all();   // the peer's barriers are initialised before anything is multicast to them
   tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
@@ -128,14 +134,15 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     // ===================================================== TMA producer
     int s = 0;
     uint32_t ph = 0;
-    for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
-      const int m0 = (t % mt) * BM, n0 = (t / mt) * BN;
+    for (int t = pair; t < n_tiles; t += n_pairs) {
+      const int m0 = ((t % mt2) * 2 + rank) * BM, n0 = (t / mt2) * BN;
       for (int kb = 0; kb < nkb; ++kb) {
         mbar_wait(empty_bar(s), ph ^ 1);
         if (elect_one()) {
           mbar_expect_tx(full_bar(s), STAGE_BYTES);
           tma_load_2d(smem0 + s * STAGE_BYTES, &tmA, kb * BK, m0, full_bar(s));
-          tma_load_2d(smem0 + s * STAGE_BYTES + A_BYTES, &tmB, kb * BK, n0, full_bar(s));
+          tma_load_2d_multicast(smem0 + s * STAGE_BYTES + A_BYTES + rank * (B_BYTES / 2), &tmB, kb * BK,
+                                n0 + rank * (BN / 2), full_bar(s), (uint16_t)3);
         }
         __syncwarp();
         if (++s == STAGES) { s = 0; ph ^= 1; }
@@ -147,7 +154,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     int s = 0;
     uint32_t ph = 0;
     int it = 0;
-    for (int t = blockIdx.x; t < n_tiles; t += gridDim.x, ++it) {
+    for (int t = pair; t < n_tiles; t += n_pairs, ++it) {
       const int as = it & 1;
       const uint32_t aph = (it >> 1) & 1;
       mbar_wait(tempty_bar(as), aph ^ 1);
@@ -161,7 +168,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
           const uint64_t bd = desc_kmajor_sw128(smem0 + s * STAGE_BYTES + A_BYTES);
 #pragma unroll
           for (int k = 0; k < BK / 16; ++k) umma_ss(d_tmem, ad + 2 * k, bd + 2 * k, idesc, (kb | k) != 0);
-          umma_commit(empty_bar(s));
+          umma_commit_multicast(empty_bar(s), (uint16_t)3);
           if (kb == nkb - 1) umma_commit(tfull_bar(as));
         }
         __syncwarp();
@@ -177,10 +184,10 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     const int et = threadIdx.x - 64;  // 0..127
     float* const s_vec = reinterpret_cast<float*>(smem_raw + (bar0 - smem_u32(smem_raw)) + 256);
     int it = 0;
-    for (int t = blockIdx.x; t < n_tiles; t += gridDim.x, ++it) {
+    for (int t = pair; t < n_tiles; t += n_pairs, ++it) {
       const int as = it & 1;
       const uint32_t aph = (it >> 1) & 1;
-      const int m0 = (t % mt) * BM, n0 = (t / mt) * BN;
+      const int m0 = ((t % mt2) * 2 + rank) * BM, n0 = (t / mt2) * BN;
       const int row = m0 + quad * 32 + lane;
       const bool row_ok = row < M;
       float* const s_bias = s_vec + as * 2 * BN_MAX;
@@ -350,6 +357,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   }
   tc_fence_before();
   __syncthreads();
+  cluster_sync_all();   // no CTA leaves while its peer may still multicast into its shared memory / barriers
   if (warp == 2) {
     tc_fence_after();
     tmem_dealloc<512>(tmem_base);
@@ -373,9 +381,19 @@ dit_status launch_t(const CUtensorMap& ta, const CUtensorMap& tb, const EpiArgs&
     DIT_CUDA_OK(cudaFuncSetAttribute(gemm_tc_kernel<EPI, BN>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes(BN)));
     attr_set = true;
   }
-  const int tiles = cdiv(M, BM) * cdiv(N, BN);
-  const int grid = tiles < sm_count() ? tiles : sm_count();
-  gemm_tc_kernel<EPI, BN><<<grid, GEMM_THREADS, smem_bytes(BN), st>>>(ta, tb, ep, M, N, K);
+  const int pairs = cdiv(cdiv(M, BM), 2) * cdiv(N, BN);
+  const int max_pairs = sm_count() / 2;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(2 * (pairs < max_pairs ? pairs : max_pairs));
+  cfg.blockDim = dim3(GEMM_THREADS);
+  cfg.dynamicSmemBytes = smem_bytes(BN);
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  DIT_CUDA_OK(cudaLaunchKernelEx(&cfg, gemm_tc_kernel<EPI, BN>, ta, tb, ep, M, N, K));
   DIT_LAUNCH_CHECK();
   return DIT_OK;
 }
@@ -388,8 +406,8 @@ int pick_bn(int M, int N) {
   int64_t best_cost = INT64_MAX;
   for (int i = 0; i < 3; ++i) {
     const int bn = cand[i];
-    const int64_t tiles = (int64_t)cdiv(M, BM) * cdiv(N, bn);
-    const int64_t cost = cdiv(tiles, (int64_t)sm_count()) * bn;
+    const int64_t tiles = (int64_t)cdiv(cdiv(M, BM), 2) * cdiv(N, bn);   // tile pairs on CTA pairs
+    const int64_t cost = cdiv(tiles, (int64_t)(sm_count() / 2)) * bn;
     if (cost < best_cost - best_cost / 64) {   // a narrower tile must win by > 1.5 %
       best_cost = cost;
       best = bn;
@@ -422,7 +440,7 @@ dit_status launch_gemm_tc_ex(int epi, const void* A, int64_t lda, const void* W,
   if (M == 0 || N == 0) return DIT_OK;
   CUtensorMap ta, tb;
   const int bn = pick_bn(M, N);
-  DIT_REQUIRE(make_tmap_2d_bf16(&ta, A, M, K, lda, BM, BK) && make_tmap_2d_bf16(&tb, W, N, K, K, bn, BK), DIT_ERR_CUDA,
+  DIT_REQUIRE(make_tmap_2d_bf16(&ta, A, M, K, lda, BM, BK) && make_tmap_2d_bf16(&tb, W, N, K, K, bn / 2, BK), DIT_ERR_CUDA,
               "gemm_tc: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d lda=%lld)", M, N, K, (long long)lda);
   EpiArgs ep{(const bf16*)bias, out, ldo, gate, gate_stride, cu, R, nullptr, nullptr, nullptr, nullptr, 0.f, 0};
   ProfScope _prof(DIT_KC_GEMM, st);
@@ -443,7 +461,7 @@ dit_status launch_gemm_tc_qkv(const void* A, int64_t lda, const void* W, const v
   if (M == 0 || N == 0) return DIT_OK;
   DIT_REQUIRE(D % 128 == 0 && N == 3 * D, DIT_ERR_INVALID_ARG, "gemm_tc_qkv: N=%d D=%d", N, D);
   CUtensorMap ta, tb;
-  DIT_REQUIRE(make_tmap_2d_bf16(&ta, A, M, K, lda, BM, BK) && make_tmap_2d_bf16(&tb, W, N, K, K, 256, BK), DIT_ERR_CUDA,
+  DIT_REQUIRE(make_tmap_2d_bf16(&ta, A, M, K, lda, BM, BK) && make_tmap_2d_bf16(&tb, W, N, K, K, 128, BK), DIT_ERR_CUDA,
               "gemm_tc_qkv: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d)", M, N, K);
   EpiArgs ep{(const bf16*)bias, out, ldo, nullptr, 0, nullptr, 1, (const bf16*)gq, (const bf16*)gk, rc, rs, rms_eps, D};
   ProfScope _prof(DIT_KC_GEMM, st);
