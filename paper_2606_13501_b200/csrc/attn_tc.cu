@@ -149,6 +149,7 @@ __device__ __forceinline__ void exp_pack_store(const uint32_t (&s)[32], uint64_t
 __global__ void __launch_bounds__(ATTN_THREADS, 1)
 attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                const __grid_constant__ CUtensorMap tmV, AttnParams p) {
+  pdl_trigger();
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sQ = smem0, sK = sQ + 2 * TILE_BYTES, sV = sK + KS * TILE_BYTES;
@@ -182,6 +183,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   const int n_sub = (kv_len + SK - 1) / SK;
 
   if (n_tiles == 0) {  // empty shard: o = 0, lse = -inf (R18)
+    pdl_wait();
     if (warp >= 4 && ((warp - 4) & 4) == 0) {   // the leader warps cover the 256 rows once
       const int row = q_base + ((warp - 4) >> 3) * TQ + (warp & 3) * 32 + lane;
       if (row < q_hi) {
@@ -217,6 +219,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+  pdl_wait();   // prologue done; q / k / v written by the previous kernel are read from here on
 
   // register budget: warpgroup 0 (TMA / MMA / idle warps) gives registers to the two softmax warpgroups
   if (warp < 4) {
@@ -492,7 +495,7 @@ dit_status launch_attn_tc(const AttnArgs& a, cudaStream_t st) {
   p.shard = a.shard; p.n_shards = a.n_shards;
   ProfScope _prof(DIT_KC_ATTN, st);
   dim3 grid(cdiv(max_q, 2 * TQ), a.H, a.cu_q ? a.R : 1);
-  attn_tc_kernel<<<grid, ATTN_THREADS, ATTN_SMEM, st>>>(tq, tk, tv, p);
+  DIT_CUDA_OK(launch_pdl(attn_tc_kernel, grid, dim3(ATTN_THREADS), ATTN_SMEM, st, 1, tq, tk, tv, p));
   DIT_LAUNCH_CHECK();
   return DIT_OK;
 }

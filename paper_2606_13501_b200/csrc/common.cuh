@@ -1,5 +1,6 @@
 // common.cuh — shared device/host helpers of libdit_b200 (CUDA path only; the oracle shares nothing with it).
 #pragma once
+#include <utility>
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -62,6 +63,42 @@ struct ProfScope {
     if (on) prof_record(cls, st, false);
   }
 };
+
+// ---------------------------------------------------------------------------------------------
+// Programmatic dependent launch (PDL): a kernel launched with the programmatic-stream-serialisation attribute may
+// become resident while its predecessor drains; it runs its private prologue (barrier init, TMEM allocation,
+// descriptor prefetch) and then blocks in pdl_wait() until the predecessor grid has completed and its writes are
+// visible.  Every kernel below calls pdl_trigger() first (lets ITS successor do the same) and pdl_wait() before its
+// first access to global data.  Without the launch attribute both are no-ops.  DIT_NO_PDL=1 disables the attribute.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+bool pdl_enabled();   // dit.cu
+
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, int cluster_x,
+                              Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[2];
+  int n = 0;
+  if (cluster_x > 1) {
+    attr[n].id = cudaLaunchAttributeClusterDimension;
+    attr[n].val.clusterDim.x = cluster_x; attr[n].val.clusterDim.y = 1; attr[n].val.clusterDim.z = 1;
+    ++n;
+  }
+  if (pdl_enabled()) {
+    attr[n].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[n].val.programmaticStreamSerializationAllowed = 1;
+    ++n;
+  }
+  cfg.attrs = attr;
+  cfg.numAttrs = n;
+  return cudaLaunchKernelEx(&cfg, kernel, KArgs(std::forward<Args>(args))...);
+}
 
 // ---------------------------------------------------------------------------------------------
 // 128-bit vector access: 8 consecutive elements of T <-> 8 floats

@@ -1,5 +1,6 @@
 // dit.cu — handle, workspace carving, step orchestration and the C ABI of libdit_b200 (include/dit.h).
 // Every stage of the step is a kernel launch on the caller's stream; no host synchronisation inside a step.
+#include <cstdlib>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
@@ -167,6 +168,14 @@ static dit_status validate(const dit_config* c) {
               DIT_ERR_INVALID_ARG, "capacities: max_tokens %d max_requests %d max_cond_tokens %d", c->max_tokens,
               c->max_requests, c->max_cond_tokens);
   return DIT_OK;
+}
+
+bool pdl_enabled() {
+  static const bool on = []() {
+    const char* e = getenv("DIT_NO_PDL");
+    return !(e != nullptr && e[0] == '1');
+  }();
+  return on;
 }
 
 // GEMM dispatch: bf16 -> tcgen05 whenever the shape/alignment allows, else FFMA.  fp32 -> FFMA (no TF32).

@@ -20,6 +20,8 @@ __global__ void __launch_bounds__(256) gemv_kernel(const float* __restrict__ in,
                                                    const GemvBatch single, int n_batches, int total_rows,
                                                    float* __restrict__ out, int64_t out_stride, int R, int K,
                                                    int silu_input) {
+  pdl_trigger();
+  pdl_wait();
   extern __shared__ float s_in[];  // [R][K], then the batch table
   GemvBatch* s_b = reinterpret_cast<GemvBatch*>(s_in + (size_t)R * K);
   for (int i = threadIdx.x; i < n_batches; i += blockDim.x) s_b[i] = batches != nullptr ? batches[i] : single;
@@ -115,8 +117,8 @@ static dit_status launch_gemv_t(const float* in, const GemvBatch* batches, const
     DIT_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gemv_kernel<T, RM>, 256, smem));          \
     if (per_sm < 1) per_sm = 1;                                                                                 \
     if (ctas > sms * per_sm) ctas = sms * per_sm;                                                               \
-    gemv_kernel<T, RM><<<ctas, 256, smem, st>>>(inr, batches, single, n_batches, total_rows, outr, out_stride, rc, K, \
-                                                silu_input);                                                    \
+    DIT_CUDA_OK(launch_pdl(gemv_kernel<T, RM>, dim3(ctas), dim3(256), smem, st, 1, inr, batches, single, n_batches,     \
+                           total_rows, outr, out_stride, rc, K, silu_input));                                   \
   }
     DIT_REQUIRE(smem <= 200 * 1024, DIT_ERR_UNSUPPORTED, "gemv: R*K too large for shared memory");
     if (rc == 1) GEMV_LAUNCH(1) else if (rc == 2) GEMV_LAUNCH(2) else if (rc <= 4) GEMV_LAUNCH(4) else GEMV_LAUNCH(8)
@@ -149,6 +151,8 @@ __global__ void __launch_bounds__(128) adaln_kernel(float* __restrict__ x, const
                                                     const float* __restrict__ scale, int64_t mod_stride,
                                                     const int32_t* __restrict__ cu, int R, T* __restrict__ y, int T_rows,
                                                     float eps) {
+  pdl_trigger();
+  pdl_wait();
   constexpr int D = NCW * WPR * 256;
   constexpr int RPB = 4 / WPR;                       // rows per block
   __shared__ float red[2][4];
@@ -235,8 +239,8 @@ static dit_status launch_adaln_t(float* x, const T* h, const float* gate, const 
   ProfScope _prof(DIT_KC_ADALN, st);
 #define ADALN_CASE(NCV, NCW, WPR)                                                                           \
   case NCV:                                                                                                 \
-    adaln_kernel<T, NCW, WPR><<<cdiv(T_rows, 4 / WPR), 128, 0, st>>>(x, h, gate, shift, scale, mod_stride, cu, R, y, \
-                                                                    T_rows, eps);                           \
+    DIT_CUDA_OK(launch_pdl(adaln_kernel<T, NCW, WPR>, dim3(cdiv(T_rows, 4 / WPR)), dim3(128), 0, st, 1, x, h, gate, \
+                           shift, scale, mod_stride, cu, R, y, T_rows, eps));                                \
     break;
   switch (D / 256) {   // D / 256 chunks per row = NCW per warp x WPR warps
     ADALN_CASE(1, 1, 1) ADALN_CASE(2, 2, 1) ADALN_CASE(3, 3, 1) ADALN_CASE(4, 4, 1) ADALN_CASE(5, 5, 1)
@@ -468,6 +472,8 @@ struct MergePtrs {
 template <typename T, int P>
 __global__ void __launch_bounds__(256) merge_kernel(MergePtrs ptrs, int64_t n_rh, int d, T* __restrict__ o,
                                                     float* __restrict__ lse_out) {
+  pdl_trigger();
+  pdl_wait();
   const int cpr = d / 8;  // 8-element chunks per (row, head)
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= n_rh * cpr) return;
@@ -505,14 +511,14 @@ static dit_status launch_merge_t(const MergePtrs& ptrs, int P, int64_t n_rh, int
   const int64_t n = n_rh * (d / 8);
   const int grid = cdiv(n, 256);
   switch (P) {
-    case 1: merge_kernel<T, 1><<<grid, 256, 0, st>>>(ptrs, n_rh, d, o, lse_out); break;
-    case 2: merge_kernel<T, 2><<<grid, 256, 0, st>>>(ptrs, n_rh, d, o, lse_out); break;
-    case 3: merge_kernel<T, 3><<<grid, 256, 0, st>>>(ptrs, n_rh, d, o, lse_out); break;
-    case 4: merge_kernel<T, 4><<<grid, 256, 0, st>>>(ptrs, n_rh, d, o, lse_out); break;
-    case 5: merge_kernel<T, 5><<<grid, 256, 0, st>>>(ptrs, n_rh, d, o, lse_out); break;
-    case 6: merge_kernel<T, 6><<<grid, 256, 0, st>>>(ptrs, n_rh, d, o, lse_out); break;
-    case 7: merge_kernel<T, 7><<<grid, 256, 0, st>>>(ptrs, n_rh, d, o, lse_out); break;
-    default: merge_kernel<T, 8><<<grid, 256, 0, st>>>(ptrs, n_rh, d, o, lse_out); break;
+    case 1: DIT_CUDA_OK(launch_pdl(merge_kernel<T, 1>, dim3(grid), dim3(256), 0, st, 1, ptrs, n_rh, d, o, lse_out)); break;
+    case 2: DIT_CUDA_OK(launch_pdl(merge_kernel<T, 2>, dim3(grid), dim3(256), 0, st, 1, ptrs, n_rh, d, o, lse_out)); break;
+    case 3: DIT_CUDA_OK(launch_pdl(merge_kernel<T, 3>, dim3(grid), dim3(256), 0, st, 1, ptrs, n_rh, d, o, lse_out)); break;
+    case 4: DIT_CUDA_OK(launch_pdl(merge_kernel<T, 4>, dim3(grid), dim3(256), 0, st, 1, ptrs, n_rh, d, o, lse_out)); break;
+    case 5: DIT_CUDA_OK(launch_pdl(merge_kernel<T, 5>, dim3(grid), dim3(256), 0, st, 1, ptrs, n_rh, d, o, lse_out)); break;
+    case 6: DIT_CUDA_OK(launch_pdl(merge_kernel<T, 6>, dim3(grid), dim3(256), 0, st, 1, ptrs, n_rh, d, o, lse_out)); break;
+    case 7: DIT_CUDA_OK(launch_pdl(merge_kernel<T, 7>, dim3(grid), dim3(256), 0, st, 1, ptrs, n_rh, d, o, lse_out)); break;
+    default: DIT_CUDA_OK(launch_pdl(merge_kernel<T, 8>, dim3(grid), dim3(256), 0, st, 1, ptrs, n_rh, d, o, lse_out)); break;
   }
   DIT_LAUNCH_CHECK();
   return DIT_OK;

@@ -86,6 +86,7 @@ template <int EPI, int BN>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, EpiArgs ep, int M, int N,
                int K) {
+  pdl_trigger();
   extern __shared__ uint8_t smem_raw[];
   constexpr int B_BYTES = BN * BK * 2, STAGE_BYTES = A_BYTES + B_BYTES;   // both multiples of 1024 (swizzle atom)
   static_assert(BN % 16 == 0 && BN <= BN_MAX && STAGE_BYTES % 1024 == 0 && (B_BYTES / 2) % 1024 == 0, "tile width");
@@ -127,6 +128,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   __syncthreads();
   cluster_sync_all();   // the peer's barriers are initialised before anything is multicast to them
   tc_fence_after();
+  pdl_wait();           // prologue done; from here on global memory written by the previous kernel is read
   uint32_t tmem_base;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
@@ -383,17 +385,8 @@ dit_status launch_t(const CUtensorMap& ta, const CUtensorMap& tb, const EpiArgs&
   }
   const int pairs = cdiv(cdiv(M, BM), 2) * cdiv(N, BN);
   const int max_pairs = sm_count() / 2;
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(2 * (pairs < max_pairs ? pairs : max_pairs));
-  cfg.blockDim = dim3(GEMM_THREADS);
-  cfg.dynamicSmemBytes = smem_bytes(BN);
-  cfg.stream = st;
-  cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeClusterDimension;
-  attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-  cfg.attrs = attr;
-  cfg.numAttrs = 1;
-  DIT_CUDA_OK(cudaLaunchKernelEx(&cfg, gemm_tc_kernel<EPI, BN>, ta, tb, ep, M, N, K));
+  DIT_CUDA_OK(launch_pdl(gemm_tc_kernel<EPI, BN>, dim3(2 * (pairs < max_pairs ? pairs : max_pairs)), dim3(GEMM_THREADS),
+                         smem_bytes(BN), st, 2, ta, tb, ep, M, N, K));
   DIT_LAUNCH_CHECK();
   return DIT_OK;
 }
