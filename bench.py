@@ -130,6 +130,22 @@ def _gpu_index(local_rank: int) -> int:
     return local_rank
 
 
+def max_over_ranks(values, world: int, device="cpu"):
+    """Per-rank device times -> the job's times: MAX over ranks (the slowest rank defines the step; contract:
+    "time on the device, max over ranks").  One all_reduce on the default process group (nccl on GPUs, gloo in
+    the CPU test of this function)."""
+    t = torch.tensor([float(v) for v in values], dtype=torch.float64, device=device)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def job_throughput(world: int, steps: int, ms_max: float) -> float:
+    """Whole-job steps/s of `world` independent replicas that each ran `steps` steps: world * steps / slowest rank."""
+    return world * steps / (ms_max * 1e-3)
+
+
 def _peaks() -> dict:
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -307,10 +323,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     prof_all = B.dit_profile_end()
     nb = max(1, min(K, 5))
 
-    t = torch.tensor([ms_total, ms_e2e], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_total, ms_e2e = float(t[0]), float(t[1])
+    ms_total, ms_e2e = max_over_ranks([ms_total, ms_e2e], world, dev)
 
     if rank == 0:
         pk = _peaks()
@@ -324,7 +337,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
                 if len(f) >= 3 and f[0] == ("cfg2" if args.workload == "cfg4" else args.workload) and f[1] == "gemm":
                     traffic = int(f[2])
         line = {
-            "metric": METRIC, "value": world * K / (ms_total * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+            "metric": METRIC, "value": job_throughput(world, K, ms_total), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
             "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
             "data": "synthetic",
             "config": {"workload": wl_name, "split_p": args.split_p, "requests_per_gpu": req_per_gpu,
@@ -332,7 +345,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
                              "through a 126 MB L2, so no step starts with its operands cached",
                        "parallelism": f"replicas x{world} (independent requests, no data-path collective)"},
             "clocks": clocks,
-            "e2e": {"value": world * K / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+            "e2e": {"value": job_throughput(world, K, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
             "gpu_launches": launches,
             "roofline": {"bound": "tensor", "kernel": "block GEMMs (QKV, out-proj, fc1, fc2)", "achieved": achieved,
                          "peak": pk["tf_sust"], "unit": "TFLOP/s", "frac": achieved / pk["tf_sust"],
