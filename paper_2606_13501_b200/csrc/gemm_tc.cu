@@ -1,15 +1,23 @@
 // gemm_tc.cu — the block GEMMs of the DiT step on 5th-generation tensor cores (north_star subsystem 3):
 //   out[M, N] = epilogue(A[M, K] W[N, K]^T + bias[N]),  bf16 x bf16 -> fp32 accumulate.
 // Design (sm_100a):
-//   * persistent kernel, one CTA per SM, static round-robin over 128 x 256 output tiles (M fastest, so the CTAs
-//     of a wave share W tiles through L2);
-//   * warp 0 = TMA producer: A (128 x 64) and W (256 x 64) tiles, 128-byte swizzle, 4-stage mbarrier ring;
-//   * warp 1 = MMA issuer: one thread issues tcgen05.mma M=128 N=256 K=16, accumulator in TMEM; two
-//     accumulator stages (2 x 256 columns = all 512) so the epilogue of tile i overlaps the mainloop of i+1;
-//   * warps 2-5 = epilogue: tcgen05.ld (32 lanes x 32 columns per warp), bias / GELU-tanh / gated-residual in
-//     fp32 registers, 16-byte global stores.
-// Roofline: tensor pipe.  M=128, N=256, K=16 takes 128 cycles on one SM's tensor core = 4096 MAC/cycle/SM; the
-// shared-memory feed is 48 KB per 512 cycles = 96 B/cycle (< 128 B/cycle), so one CTA per SM can saturate it.
+//   * persistent kernel on CTA PAIRS (cluster of 2, one CTA per SM): the pair walks a static round-robin list of
+//     256 x BN output tiles (row-tile pairs fastest, so the pairs of a wave share W tiles through L2); BN is 256,
+//     240 or 192, whichever fills the last wave best (pick_bn);
+//   * warp 0 of each CTA = TMA producer: its own A rows (128 x 64) and its own HALF of the W tile (BN/2 x 64),
+//     128-byte swizzle, 6-stage ring; both CTAs' boxes complete on the leader CTA's full barrier (cta_group::2
+//     form of cp.async.bulk.tensor);
+//   * warp 1 of the LEADER CTA = MMA issuer: one elected thread issues tcgen05.mma.cta_group::2 M=256 N=BN K=16 —
+//     each SM's tensor core reads its own A and its own half of W and the halves are exchanged inside the pair —
+//     accumulators (128 rows per CTA) in TMEM; two accumulator stages (2 x 256 columns = all 512) so the epilogue
+//     of tile i overlaps the mainloop of i+1; tcgen05.commit.cta_group::2 is multicast to both CTAs' barriers;
+//   * warps 2-5 of each CTA = epilogue of its own 128 rows: tcgen05.ld (32 lanes x 32 columns per warp), bias /
+//     GELU-tanh / gated-residual / QK-RMSNorm + RoPE in fp32 registers, 16-byte global stores; the peer CTA's
+//     epilogue warps release the accumulator stage with a remote mbarrier arrive on the leader's barrier.
+// Roofline: tensor pipe.  M=256 (pair), N=256, K=16 takes 128 cycles on both tensor cores = 4096 MAC/cycle/SM
+// (measured, clock64 loop).  Per SM a stage is A + W/2 = 32 KB, written once by TMA and read once by the MMAs per
+// 512 tensor cycles: 128 B/cycle of shared-memory traffic in total — the port's limit; a 1-CTA 128 x 256 tile needs
+// 192 B/cycle and stalled at ~80 % tensor-pipe utilisation.
 #include "tc.cuh"
 
 namespace dit {
@@ -48,11 +56,11 @@ using namespace tc;
 
 namespace {
 
-constexpr int BM = 128, BK = 64, STAGES = 4;
+constexpr int BM = 128, BK = 64, STAGES = 6;
 constexpr int BN_MAX = 256;   // TMEM accumulator stage stride and staging-row size; the tile width BN is a template
                               // parameter (192 / 240 / 256) picked per problem to fill the last wave (see pick_bn)
 constexpr int A_BYTES = BM * BK * 2;
-constexpr int stage_bytes(int bn) { return A_BYTES + bn * BK * 2; }
+constexpr int stage_bytes(int bn) { return A_BYTES + (bn / 2) * BK * 2; }   // own A rows + own HALF of the W tile
 constexpr int GEMM_THREADS = 192;
 constexpr int EPI_THREADS = 128;
 constexpr int smem_bytes(int bn) {
@@ -88,8 +96,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                int K) {
   pdl_trigger();
   extern __shared__ uint8_t smem_raw[];
-  constexpr int B_BYTES = BN * BK * 2, STAGE_BYTES = A_BYTES + B_BYTES;   // both multiples of 1024 (swizzle atom)
-  static_assert(BN % 16 == 0 && BN <= BN_MAX && STAGE_BYTES % 1024 == 0 && (B_BYTES / 2) % 1024 == 0, "tile width");
+  constexpr int BH_BYTES = (BN / 2) * BK * 2, STAGE_BYTES = A_BYTES + BH_BYTES;   // multiples of 1024 (swizzle atom)
+  static_assert(BN % 16 == 0 && BN <= BN_MAX && STAGE_BYTES % 1024 == 0, "tile width");
   const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t bar0 = smem0 + STAGES * STAGE_BYTES;
   // barriers: full[STAGES], empty[STAGES], tfull[2], tempty[2]; then the TMEM base address word
@@ -100,9 +108,11 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   const uint32_t tmem_slot = bar0 + 8u * (2 * STAGES + 4);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  // CTA pairs (cluster of 2): the pair works on two vertically adjacent row tiles of the same column tile and shares
-  // the W tile — each CTA fetches half of it and TMA-multicasts the half into both CTAs' shared memory, which cuts
-  // the L2 -> SM traffic of a stage from A + W to A + W/2.  Every MMA is still a 1-CTA M = 128 instruction.
+  // CTA pairs (cluster of 2, cta_group::2): the pair computes a 256 x BN tile with ONE M = 256 MMA stream issued by
+  // the leader CTA (rank 0).  Each CTA holds its own 128 rows of A and HALF of the W tile (rows rank * BN/2 ...) in
+  // shared memory and its own 128 accumulator rows in TMEM: per CTA a stage is A + W/2 bytes — written once by TMA
+  // and read once by the tensor core — instead of A + W, which is what a 1-CTA tile cannot feed through a
+  // 128 B/clk shared-memory port.
   const int rank = (int)cluster_ctarank();
   const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
   const int mt = (M + BM - 1) / BM, mt2 = (mt + 1) >> 1, nt = (N + BN - 1) / BN, n_tiles = mt2 * nt;   // tile PAIRS
@@ -114,64 +124,68 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   }
   if (warp == 1 && lane == 0) {
     for (int s = 0; s < STAGES; ++s) {
-      mbar_init(full_bar(s), 1);
-      mbar_init(empty_bar(s), 2);   // released by this CTA's MMA warp AND the peer's (its half of W lands here too)
+      mbar_init(full_bar(s), 1);        // (leader only) the TMA bytes of BOTH CTAs' halves of the stage
+      mbar_init(empty_bar(s), 1);       // the leader's commit, multicast to both CTAs
     }
     for (int s = 0; s < 2; ++s) {
-      mbar_init(tfull_bar(s), 1);
-      mbar_init(tempty_bar(s), 4);
+      mbar_init(tfull_bar(s), 1);       // the leader's commit, multicast
+      mbar_init(tempty_bar(s), 8);      // (leader only) 4 epilogue warps of each CTA
     }
     fence_barrier_init();
   }
-  if (warp == 2) tmem_alloc<512>(tmem_slot);
+  if (warp == 2) tmem_alloc_pair<512>(tmem_slot);
   tc_fence_before();
   __syncthreads();
-  cluster_sync_all();   // the peer's barriers are initialised before anything is multicast to them
+  cluster_sync_all();   // the peer's barriers are initialised before anything arrives on them
   tc_fence_after();
   pdl_wait();           // prologue done; from here on global memory written by the previous kernel is read
   uint32_t tmem_base;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
   if (warp == 0) {
-    // ===================================================== TMA producer
+    // ===================================================== TMA producer (both CTAs: own A rows, own half of W)
+    // Both CTAs' boxes complete on the LEADER's full barrier (cta_group::2 form of the TMA load), which expects the
+    // bytes of both stages; a CTA refills a stage when the leader's commit has arrived on its own empty barrier.
     int s = 0;
     uint32_t ph = 0;
     for (int t = pair; t < n_tiles; t += n_pairs) {
-      const int m0 = ((t % mt2) * 2 + rank) * BM, n0 = (t / mt2) * BN;
+      const int m0 = ((t % mt2) * 2 + rank) * BM, n0 = (t / mt2) * BN + rank * (BN / 2);
       for (int kb = 0; kb < nkb; ++kb) {
-        mbar_wait(empty_bar(s), ph ^ 1);
+        mbar_wait_poll(empty_bar(s), ph ^ 1);
         if (elect_one()) {
-          mbar_expect_tx(full_bar(s), STAGE_BYTES);
-          tma_load_2d(smem0 + s * STAGE_BYTES, &tmA, kb * BK, m0, full_bar(s));
-          tma_load_2d_multicast(smem0 + s * STAGE_BYTES + A_BYTES + rank * (B_BYTES / 2), &tmB, kb * BK,
-                                n0 + rank * (BN / 2), full_bar(s), (uint16_t)3);
+          const uint32_t fb = mapa_cluster(full_bar(s), 0);
+          if (rank == 0) mbar_expect_tx(full_bar(s), 2 * STAGE_BYTES);
+          tma_load_2d_pair(smem0 + s * STAGE_BYTES, &tmA, kb * BK, m0, fb);
+          tma_load_2d_pair(smem0 + s * STAGE_BYTES + A_BYTES, &tmB, kb * BK, n0, fb);
         }
         __syncwarp();
         if (++s == STAGES) { s = 0; ph ^= 1; }
       }
     }
+  } else if (warp == 1 && rank != 0) {
+    // the peer CTA's warp 1 has nothing to issue: the leader drives both tensor cores
   } else if (warp == 1) {
-    // ===================================================== MMA issuer
-    constexpr uint32_t idesc = idesc_bf16(BM, BN, 0, 0);
+    // ===================================================== leader CTA: MMA issuer for the pair
+    constexpr uint32_t idesc = idesc_bf16(2 * BM, BN, 0, 0);
     int s = 0;
     uint32_t ph = 0;
     int it = 0;
     for (int t = pair; t < n_tiles; t += n_pairs, ++it) {
       const int as = it & 1;
       const uint32_t aph = (it >> 1) & 1;
-      mbar_wait(tempty_bar(as), aph ^ 1);
+      mbar_wait_poll(tempty_bar(as), aph ^ 1);
       tc_fence_after();
       const uint32_t d_tmem = tmem_base + as * BN_MAX;
       for (int kb = 0; kb < nkb; ++kb) {
-        mbar_wait(full_bar(s), ph);
+        mbar_wait_poll(full_bar(s), ph);
         tc_fence_after();
         if (elect_one()) {
           const uint64_t ad = desc_kmajor_sw128(smem0 + s * STAGE_BYTES);
           const uint64_t bd = desc_kmajor_sw128(smem0 + s * STAGE_BYTES + A_BYTES);
 #pragma unroll
-          for (int k = 0; k < BK / 16; ++k) umma_ss(d_tmem, ad + 2 * k, bd + 2 * k, idesc, (kb | k) != 0);
-          umma_commit_multicast(empty_bar(s), (uint16_t)3);
-          if (kb == nkb - 1) umma_commit(tfull_bar(as));
+          for (int k = 0; k < BK / 16; ++k) umma_ss_pair(d_tmem, ad + 2 * k, bd + 2 * k, idesc, (kb | k) != 0);
+          umma_commit_pair(empty_bar(s), (uint16_t)3);
+          if (kb == nkb - 1) umma_commit_pair(tfull_bar(as), (uint16_t)3);
         }
         __syncwarp();
         if (++s == STAGES) { s = 0; ph ^= 1; }
@@ -234,7 +248,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
           asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(xrow), "r"(ncols * 4) : "memory");
         load_x(0);  // first chunk in flight while the mainloop of this tile finishes
       }
-      mbar_wait(tfull_bar(as), aph);
+      mbar_wait_poll(tfull_bar(as), aph);
       tc_fence_after();
       const uint32_t t_addr = tmem_base + as * BN_MAX + ((uint32_t)(quad * 32) << 16);
       if (EPI == EPI_QKV_NORM_ROPE) {
@@ -354,7 +368,10 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       }
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(tempty_bar(as));
+      if (lane == 0) {   // the accumulator stage is drained: tell the leader's MMA warp
+        if (rank == 0) mbar_arrive(tempty_bar(as));
+        else mbar_arrive_remote(tempty_bar(as), 0);
+      }
     }
   }
   tc_fence_before();
@@ -362,7 +379,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   cluster_sync_all();   // no CTA leaves while its peer may still multicast into its shared memory / barriers
   if (warp == 2) {
     tc_fence_after();
-    tmem_dealloc<512>(tmem_base);
+    tmem_dealloc_pair<512>(tmem_base);
   }
 }
 
