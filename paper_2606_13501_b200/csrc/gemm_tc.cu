@@ -50,24 +50,41 @@ bool make_tmap_2d_bf16(CUtensorMap* out, const void* base, uint64_t rows, uint64
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+bool make_tmap_2d_f32(CUtensorMap* out, const void* base, uint64_t rows, uint64_t cols, uint64_t ld, uint32_t box_rows) {
+  EncodeTiledFn fn = encode_tiled_fn();
+  if (!fn) return false;
+  cuuint64_t dims[2] = {cols, rows};
+  cuuint64_t strides[1] = {ld * 4};
+  cuuint32_t box[2] = {32, box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  return fn(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void*>(base), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 }  // namespace tc
 
 using namespace tc;
 
 namespace {
 
-constexpr int BM = 128, BK = 64, STAGES = 6;
+constexpr int BM = 128, BK = 64;
 constexpr int BN_MAX = 256;   // TMEM accumulator stage stride and staging-row size; the tile width BN is a template
                               // parameter (192 / 240 / 256) picked per problem to fill the last wave (see pick_bn)
 constexpr int A_BYTES = BM * BK * 2;
 constexpr int stage_bytes(int bn) { return A_BYTES + (bn / 2) * BK * 2; }   // own A rows + own HALF of the W tile
 constexpr int GEMM_THREADS = 192;
 constexpr int EPI_THREADS = 128;
-constexpr int smem_bytes(int bn) {
-  return STAGES * stage_bytes(bn) + 1024 /* alignment slack */ + 256 /* barriers */ +
+enum { EPI_GATE_RESID = 3, EPI_QKV_NORM_ROPE = 4 };
+// The gated-residual epilogue stages its fp32 tile chunks in shared memory for TMA reduce-add (two 32 x 32 fp32
+// buffers per epilogue warp = 32 KB) and gives up one ring stage for them.
+constexpr int STG_WARP_BYTES = 2 * 32 * 128;
+constexpr int stages_for(int epi) { return epi == EPI_GATE_RESID ? 5 : 6; }
+constexpr int staging_bytes(int epi) { return epi == EPI_GATE_RESID ? 4 * STG_WARP_BYTES : 0; }
+constexpr int smem_bytes(int bn, int epi) {
+  return stages_for(epi) * stage_bytes(bn) + staging_bytes(epi) + 1024 /* alignment slack */ + 256 /* barriers */ +
          2 * 2 * BN_MAX * 4 /* bias + gate rows of the tile, fp32, one set per accumulator stage */;
 }
-enum { EPI_GATE_RESID = 3, EPI_QKV_NORM_ROPE = 4 };
 
 struct EpiArgs {
   const bf16* bias;       // [N] or nullptr
@@ -92,14 +109,16 @@ __device__ __forceinline__ float gelu_tanh_fast(float z) {
 
 template <int EPI, int BN>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
-gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, EpiArgs ep, int M, int N,
-               int K) {
+gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
+               const __grid_constant__ CUtensorMap tmX, EpiArgs ep, int M, int N, int K) {
   pdl_trigger();
+  constexpr int STAGES = stages_for(EPI);
   extern __shared__ uint8_t smem_raw[];
   constexpr int BH_BYTES = (BN / 2) * BK * 2, STAGE_BYTES = A_BYTES + BH_BYTES;   // multiples of 1024 (swizzle atom)
   static_assert(BN % 16 == 0 && BN <= BN_MAX && STAGE_BYTES % 1024 == 0, "tile width");
   const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t bar0 = smem0 + STAGES * STAGE_BYTES;
+  const uint32_t stg0 = smem0 + STAGES * STAGE_BYTES;          // TMA reduce staging (gated residual only), 1024-aligned
+  const uint32_t bar0 = stg0 + staging_bytes(EPI);
   // barriers: full[STAGES], empty[STAGES], tfull[2], tempty[2]; then the TMEM base address word
   auto full_bar = [&](int s) { return bar0 + 8u * s; };
   auto empty_bar = [&](int s) { return bar0 + 8u * (STAGES + s); };
@@ -121,6 +140,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&tmA);
     tma_prefetch_desc(&tmB);
+    if (EPI == EPI_GATE_RESID) tma_prefetch_desc(&tmX);
   }
   if (warp == 1 && lane == 0) {
     for (int s = 0; s < STAGES; ++s) {
@@ -232,22 +252,11 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       for (int i = et; i < BN; i += EPI_THREADS)
         s_bias[i] = (ep.bias != nullptr && n0 + i < N) ? __bfloat162float(ep.bias[n0 + i]) : 0.f;
       asm volatile("bar.sync 1, 128;" ::: "memory");  // staged rows visible to the 4 epilogue warps
-      float* const xrow = reinterpret_cast<float*>(ep.out) + (int64_t)(row_ok ? row : 0) * ep.ldo + n0;
-      float xc[32];
-      auto load_x = [&](int c) {  // residual-stream chunk c of this thread's row (EPI_GATE_RESID)
-#pragma unroll
-        for (int g = 0; g < 4; ++g) {
-          if (row_ok && n0 + c * 32 + g * 8 < N && c * 32 + g * 8 < BN) ld8<float>(xrow + c * 32 + g * 8, &xc[g * 8]);
-        }
-      };
-      if (EPI == EPI_GATE_RESID) {
-        // pull this thread's 1 KB slice of the residual row into L2 while the mainloop runs (the epilogue reads it
-        // 128 bytes at a time; without this every chunk pays a DRAM round trip)
-        const int ncols = (N - n0) < BN ? (N - n0) : BN;
-        if (row_ok)
-          asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(xrow), "r"(ncols * 4) : "memory");
-        load_x(0);  // first chunk in flight while the mainloop of this tile finishes
-      }
+      // Gated residual (x <- x + gate (.) (acc + bias)): the thread's 32-column chunk of gate (.) (acc + bias) goes to
+      // a swizzled shared-memory buffer of its warp (32 rows x 128 bytes) and ONE TMA reduce-add per warp and chunk
+      // adds it to x in L2: x is never read into the SM, and the global traffic is full 128-byte rows instead of
+      // 32 scattered 16-byte pieces per load / store instruction (which made this epilogue 40 k cycles per tile).
+      const uint32_t stg = stg0 + (uint32_t)quad * STG_WARP_BYTES;
       mbar_wait_poll(tfull_bar(as), aph);
       tc_fence_after();
       const uint32_t t_addr = tmem_base + as * BN_MAX + ((uint32_t)(quad * 32) << 16);
@@ -325,11 +334,38 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         uint32_t r[32];
         tmem_ld32(t_addr + c * 32, r);
         tmem_ld_wait();
-        float xv[32];
         if (EPI == EPI_GATE_RESID) {
+          const uint32_t buf = stg + (uint32_t)(c & 1) * (STG_WARP_BYTES / 2);
+          if (lane == 0) tma_store_wait_read<1>();   // the reduce issued from this buffer two chunks ago has read it
+          __syncwarp();
 #pragma unroll
-          for (int e = 0; e < 32; ++e) xv[e] = xc[e];
-          if (c + 1 < (BN + 31) / 32 && n + 32 < N) load_x(c + 1);  // prefetch the next chunk
+          for (int g = 0; g < 4; ++g) {
+            const int ng = n + g * 8;
+            float v[8], b[8], gv[8];
+            ld8<float>(s_bias + c * 32 + g * 8, b);
+            const bool live = ng < N && c * 32 + g * 8 < BN;   // columns past the tile belong to the next tile: add 0
+            if (gate_row != nullptr && live) {
+              if (gate_smem) ld8<float>(s_gate + c * 32 + g * 8, gv);
+              else ld8<float>(gate_row + ng, gv);
+            } else {
+#pragma unroll
+              for (int e = 0; e < 8; ++e) gv[e] = 1.0f;
+            }
+#pragma unroll
+            for (int e = 0; e < 8; ++e) v[e] = live ? gv[e] * (__uint_as_float(r[g * 8 + e]) + b[e]) : 0.f;
+            // 128-byte swizzle of the TMA box: 16-byte chunk j of row `lane` sits at chunk j ^ (lane & 7)
+            const uint32_t a0 = buf + (uint32_t)lane * 128u + (uint32_t)(((2 * g) ^ (lane & 7)) << 4);
+            const uint32_t a1 = buf + (uint32_t)lane * 128u + (uint32_t)(((2 * g + 1) ^ (lane & 7)) << 4);
+            asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(a0), "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]) : "memory");
+            asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(a1), "f"(v[4]), "f"(v[5]), "f"(v[6]), "f"(v[7]) : "memory");
+          }
+          fence_proxy_async();   // the generic-proxy stores above are visible to the TMA engine
+          __syncwarp();
+          if (lane == 0) {
+            tma_reduce_add_2d(&tmX, buf, n, m0 + quad * 32);   // rows >= M and columns >= N are clipped by the map
+            tma_store_commit();
+          }
+          continue;
         }
 #pragma unroll
         for (int g = 0; g < 4; ++g) {  // groups of 8 columns
@@ -348,21 +384,6 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
             st8<bf16>(reinterpret_cast<bf16*>(ep.out) + (int64_t)row * ep.ldo + ng, v);
           } else if (EPI == DIT_EPI_BIAS_F32) {
             st8<float>(reinterpret_cast<float*>(ep.out) + (int64_t)row * ep.ldo + ng, v);
-          } else {  // x <- x + gate (.) (acc + bias)
-            float x[8];
-#pragma unroll
-            for (int e = 0; e < 8; ++e) x[e] = xv[g * 8 + e];
-            if (gate_row != nullptr) {
-              float gv[8];
-              if (gate_smem) ld8<float>(s_gate + c * 32 + g * 8, gv);
-              else ld8<float>(gate_row + ng, gv);
-#pragma unroll
-              for (int e = 0; e < 8; ++e) x[e] = fmaf(gv[e], v[e], x[e]);
-            } else {
-#pragma unroll
-              for (int e = 0; e < 8; ++e) x[e] += v[e];
-            }
-            st8<float>(xrow + c * 32 + g * 8, x);
           }
         }
       }
@@ -374,9 +395,10 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       }
     }
   }
+  if (EPI == EPI_GATE_RESID && warp >= 2 && lane == 0) tma_store_wait<0>();   // every reduce-add has been performed
   tc_fence_before();
   __syncthreads();
-  cluster_sync_all();   // no CTA leaves while its peer may still multicast into its shared memory / barriers
+  cluster_sync_all();   // no CTA leaves while its peer may still signal its barriers
   if (warp == 2) {
     tc_fence_after();
     tmem_dealloc_pair<512>(tmem_base);
@@ -394,16 +416,18 @@ int sm_count() {
 }
 
 template <int EPI, int BN>
-dit_status launch_t(const CUtensorMap& ta, const CUtensorMap& tb, const EpiArgs& ep, int M, int N, int K, cudaStream_t st) {
+dit_status launch_t(const CUtensorMap& ta, const CUtensorMap& tb, const CUtensorMap& tx, const EpiArgs& ep, int M, int N, int K,
+                    cudaStream_t st) {
   static bool attr_set = false;
   if (!attr_set) {
-    DIT_CUDA_OK(cudaFuncSetAttribute(gemm_tc_kernel<EPI, BN>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes(BN)));
+    DIT_CUDA_OK(cudaFuncSetAttribute(gemm_tc_kernel<EPI, BN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     smem_bytes(BN, EPI)));
     attr_set = true;
   }
   const int pairs = cdiv(cdiv(M, BM), 2) * cdiv(N, BN);
   const int max_pairs = sm_count() / 2;
   DIT_CUDA_OK(launch_pdl(gemm_tc_kernel<EPI, BN>, dim3(2 * (pairs < max_pairs ? pairs : max_pairs)), dim3(GEMM_THREADS),
-                         smem_bytes(BN), st, 2, ta, tb, ep, M, N, K));
+                         smem_bytes(BN, EPI), st, 2, ta, tb, tx, ep, M, N, K));
   DIT_LAUNCH_CHECK();
   return DIT_OK;
 }
@@ -427,11 +451,11 @@ int pick_bn(int M, int N) {
 }
 
 template <int EPI>
-dit_status launch_bn(int bn, const CUtensorMap& ta, const CUtensorMap& tb, const EpiArgs& ep, int M, int N, int K,
-                     cudaStream_t st) {
-  if (bn == 192) return launch_t<EPI, 192>(ta, tb, ep, M, N, K, st);
-  if (bn == 240) return launch_t<EPI, 240>(ta, tb, ep, M, N, K, st);
-  return launch_t<EPI, 256>(ta, tb, ep, M, N, K, st);
+dit_status launch_bn(int bn, const CUtensorMap& ta, const CUtensorMap& tb, const CUtensorMap& tx, const EpiArgs& ep, int M,
+                     int N, int K, cudaStream_t st) {
+  if (bn == 192) return launch_t<EPI, 192>(ta, tb, tx, ep, M, N, K, st);
+  if (bn == 240) return launch_t<EPI, 240>(ta, tb, tx, ep, M, N, K, st);
+  return launch_t<EPI, 256>(ta, tb, tx, ep, M, N, K, st);
 }
 
 }  // namespace
@@ -455,10 +479,14 @@ dit_status launch_gemm_tc_ex(int epi, const void* A, int64_t lda, const void* W,
   EpiArgs ep{(const bf16*)bias, out, ldo, gate, gate_stride, cu, R, nullptr, nullptr, nullptr, nullptr, 0.f, 0};
   ProfScope _prof(DIT_KC_GEMM, st);
   switch (epi) {
-    case DIT_EPI_BIAS: return launch_bn<DIT_EPI_BIAS>(bn, ta, tb, ep, M, N, K, st);
-    case DIT_EPI_BIAS_GELU: return launch_bn<DIT_EPI_BIAS_GELU>(bn, ta, tb, ep, M, N, K, st);
-    case DIT_EPI_BIAS_F32: return launch_bn<DIT_EPI_BIAS_F32>(bn, ta, tb, ep, M, N, K, st);
-    case EPI_GATE_RESID: return launch_bn<EPI_GATE_RESID>(bn, ta, tb, ep, M, N, K, st);
+    case DIT_EPI_BIAS: return launch_bn<DIT_EPI_BIAS>(bn, ta, tb, ta, ep, M, N, K, st);
+    case DIT_EPI_BIAS_GELU: return launch_bn<DIT_EPI_BIAS_GELU>(bn, ta, tb, ta, ep, M, N, K, st);
+    case DIT_EPI_BIAS_F32: return launch_bn<DIT_EPI_BIAS_F32>(bn, ta, tb, ta, ep, M, N, K, st);
+    case EPI_GATE_RESID: {
+      CUtensorMap tx;   // the fp32 residual stream as the target of the epilogue's TMA reduce-add
+      DIT_REQUIRE(make_tmap_2d_f32(&tx, out, M, N, ldo, 32), DIT_ERR_CUDA, "gemm_tc: cuTensorMapEncodeTiled (x) failed");
+      return launch_bn<EPI_GATE_RESID>(bn, ta, tb, tx, ep, M, N, K, st);
+    }
     default: DIT_REQUIRE(false, DIT_ERR_INVALID_ARG, "gemm_tc: epilogue %d", epi);
   }
 }
@@ -475,7 +503,7 @@ dit_status launch_gemm_tc_qkv(const void* A, int64_t lda, const void* W, const v
               "gemm_tc_qkv: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d)", M, N, K);
   EpiArgs ep{(const bf16*)bias, out, ldo, nullptr, 0, nullptr, 1, (const bf16*)gq, (const bf16*)gk, rc, rs, rms_eps, D};
   ProfScope _prof(DIT_KC_GEMM, st);
-  return launch_t<EPI_QKV_NORM_ROPE, 256>(ta, tb, ep, M, N, K, st);
+  return launch_t<EPI_QKV_NORM_ROPE, 256>(ta, tb, ta, ep, M, N, K, st);
 }
 
 dit_status launch_gemm_tc(int epi, const void* A, int64_t lda, const void* W, const void* bias, void* out, int64_t ldo,

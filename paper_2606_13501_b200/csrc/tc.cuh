@@ -98,6 +98,12 @@ __device__ __forceinline__ void tma_store_2d(const CUtensorMap* m, uint32_t src,
                "r"(c1)
                : "memory");
 }
+// global[box at (c0, c1)] += shared[box], element type of the map (fp32), performed in L2; bulk-group completion
+__device__ __forceinline__ void tma_reduce_add_2d(const CUtensorMap* m, uint32_t src, int c0, int c1) {
+  asm volatile("cp.reduce.async.bulk.tensor.2d.global.shared::cta.add.tile.bulk_group [%0, {%2, %3}], [%1];" ::"l"(m),
+               "r"(src), "r"(c0), "r"(c1)
+               : "memory");
+}
 __device__ __forceinline__ void tma_store_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void tma_store_wait_read() {
@@ -293,6 +299,8 @@ EncodeTiledFn encode_tiled_fn();  // resolved once through cudaGetDriverEntryPoi
 // bf16 [rows, cols] row-major (row stride ld elements) -> map with box {box_cols, box_rows}, 128-byte swizzle
 bool make_tmap_2d_bf16(CUtensorMap* out, const void* base, uint64_t rows, uint64_t cols, uint64_t ld, uint32_t box_rows,
                        uint32_t box_cols);
+// fp32 [rows, cols] row-major -> map with box {32 columns = 128 bytes, box_rows}, 128-byte swizzle (TMA reduce-add target)
+bool make_tmap_2d_f32(CUtensorMap* out, const void* base, uint64_t rows, uint64_t cols, uint64_t ld, uint32_t box_rows);
 
 }  // namespace tc
 }  // namespace dit
