@@ -365,8 +365,10 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
       if (valid > 0) {
         mbar_wait(s_full(t, h), par);
         tc_fence_after();
-        tmem_ld32(s_addr + 0, s0);
+        // pass 1: the second 32 scores only for the row max (re-read after the exchange: a TMEM read is cheaper
+        // than 32 live registers, which made ptxas recompute every address inside the loop); the first 32 stay
         tmem_ld32(s_addr + 32, s1);
+        tmem_ld32(s_addr + 0, s0);
         tmem_ld_wait();
         if (valid < SK) {                          // -inf before the row max
           mask32(s0, valid);
@@ -408,7 +410,10 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
       // P = 2^(s c - m_used): one packed FFMA per pair, EX2 (MUFU or FMA pipe), row sum in fp32, bf16 pairs -> TMEM
       const uint64_t nm2 = pack2(-m_used, -m_used);
       uint64_t sum2 = pack2(0.f, 0.f), sum2b = pack2(0.f, 0.f);
-      exp_pack_store(s0, c2, nm2, s_addr + 0, sum2, sum2b);
+      tmem_ld32(s_addr + 32, s1);                  // pass 2 of the second half: S columns 32..63 are still intact
+      exp_pack_store(s0, c2, nm2, s_addr + 0, sum2, sum2b);     // P columns 0..15 overwrite S columns 0..15 (consumed)
+      tmem_ld_wait();
+      if (valid < SK) mask32(s1, valid - 32);
       exp_pack_store(s1, c2, nm2, s_addr + 16, sum2, sum2b);
       float sa, sb;
       unpack2(add2(sum2, sum2b), sa, sb);
