@@ -345,6 +345,9 @@ def run_ours(args, rank: int, local_rank: int, world: int):
                              "through a 126 MB L2, so no step starts with its operands cached",
                        "parallelism": f"replicas x{world} (independent requests, no data-path collective)"},
             "clocks": clocks,
+            "device": {"name": torch.cuda.get_device_name(dev), "sms": torch.cuda.get_device_properties(dev).multi_processor_count,
+                       "torch": torch.__version__, "cuda": torch.version.cuda, "peaks": pk,
+                       "timing": f"{K} back-to-back steps after {Wm} warm-ups (sustained clocks), CUDA events"},
             "e2e": {"value": job_throughput(world, K, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
             "gpu_launches": launches,
             "roofline": {"bound": "tensor", "kernel": "block GEMMs (QKV, out-proj, fc1, fc2)", "achieved": achieved,

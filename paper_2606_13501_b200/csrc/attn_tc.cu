@@ -27,6 +27,8 @@
 // Registers: 640 threads x 96 at launch; setmaxnreg moves the control warps to 40 and the softmax warps to 104
 // (the pool is the CTA's launch allocation: asking for more than the control warps release never returns).
 // Roofline: tensor pipe; the softmax instruction stream (~4.5 issue slots per score) is co-critical.
+#include <algorithm>
+
 #include "tc.cuh"
 
 namespace dit {
@@ -57,6 +59,7 @@ struct AttnParams {
   int n_q, n_k, H;
   float scale_log2;   // softmax scale * log2(e)
   int shard, n_shards;
+  uint8_t order[64];  // blockIdx.z -> request, longest key sequence first: the last wave is made of short items
 };
 
 __device__ __forceinline__ float ex2(float x) {
@@ -168,7 +171,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   const uint32_t tmem_slot = bar0 + 8u * (B0 + 12);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int req = blockIdx.z, head = blockIdx.y;
+  const int req = p.cu_q ? p.order[blockIdx.z] : 0, head = blockIdx.y;
   const int q_lo = p.cu_q ? p.cu_q[req] : 0, q_hi = p.cu_q ? p.cu_q[req + 1] : p.n_q;
   const int q_base = q_lo + blockIdx.x * (2 * TQ);
   if (q_base >= q_hi) return;  // CTA-uniform
@@ -498,6 +501,11 @@ dit_status launch_attn_tc(const AttnArgs& a, cudaStream_t st) {
   p.n_q = a.n_q; p.n_k = a.n_k; p.H = a.H;
   p.scale_log2 = a.scale * 1.4426950408889634f;
   p.shard = a.shard; p.n_shards = a.n_shards;
+  for (int r = 0; r < 64; ++r) p.order[r] = (uint8_t)(r < a.R ? r : 0);
+  if (a.cu_q && a.cu_k_host && a.R > 1 && a.R <= 64)   // work per CTA is proportional to the request's key count
+    std::stable_sort(p.order, p.order + a.R, [&](uint8_t x, uint8_t y) {
+      return a.cu_k_host[x + 1] - a.cu_k_host[x] > a.cu_k_host[y + 1] - a.cu_k_host[y];
+    });
   ProfScope _prof(DIT_KC_ATTN, st);
   dim3 grid(cdiv(max_q, 2 * TQ), a.H, a.cu_q ? a.R : 1);
   DIT_CUDA_OK(launch_pdl(attn_tc_kernel, grid, dim3(ATTN_THREADS), ATTN_SMEM, st, 1, tq, tk, tv, p));
