@@ -244,7 +244,7 @@ static dit_status launch_adaln_t(float* x, const T* h, const float* gate, const 
     break;
   switch (D / 256) {   // D / 256 chunks per row = NCW per warp x WPR warps
     ADALN_CASE(1, 1, 1) ADALN_CASE(2, 2, 1) ADALN_CASE(3, 3, 1) ADALN_CASE(4, 4, 1) ADALN_CASE(5, 5, 1)
-    ADALN_CASE(6, 3, 2) ADALN_CASE(8, 4, 2) ADALN_CASE(10, 5, 2) ADALN_CASE(12, 6, 2) ADALN_CASE(16, 4, 4)
+    ADALN_CASE(6, 3, 2) ADALN_CASE(8, 4, 2) ADALN_CASE(10, 5, 2) ADALN_CASE(12, 3, 4) ADALN_CASE(16, 4, 4)
     ADALN_CASE(20, 5, 4) ADALN_CASE(24, 6, 4)
     default:
       DIT_REQUIRE(false, DIT_ERR_UNSUPPORTED, "adaln: D=%d has no instantiation", D);
