@@ -110,7 +110,7 @@ __device__ __forceinline__ float gelu_tanh_fast(float z) {
 template <int EPI, int BN>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
-               const __grid_constant__ CUtensorMap tmX, EpiArgs ep, int M, int N, int K) {
+               const __grid_constant__ CUtensorMap tmX, EpiArgs ep, int M, int N, int K, int GM) {
   pdl_trigger();
   constexpr int STAGES = stages_for(EPI);
   extern __shared__ uint8_t smem_raw[];
@@ -136,6 +136,17 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
   const int mt = (M + BM - 1) / BM, mt2 = (mt + 1) >> 1, nt = (N + BN - 1) / BN, n_tiles = mt2 * nt;   // tile PAIRS
   const int nkb = (K + BK - 1) / BK;
+  // Tile order: groups of GM row-tile pairs; inside a group the column tile is the slow index.  A wave of 74 CTA
+  // pairs then covers ~74 / GM column tiles of the same GM row-tile pairs, whose A panels (GM x 256 x K) are sized
+  // by the host to stay in L2 while the group sweeps over all column tiles: A is read from DRAM about once instead
+  // of once per column tile (cfg 3: 335 MB of A x 60 column tiles = 20 GB per QKV GEMM with the plain order).
+  auto tile_mn = [&](int t, int& mp, int& n) {
+    const int per_group = GM * nt;
+    const int g = t / per_group, r = t - g * per_group;
+    const int gsize = (mt2 - g * GM) < GM ? (mt2 - g * GM) : GM;
+    n = r / gsize;
+    mp = g * GM + (r - n * gsize);
+  };
 
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&tmA);
@@ -169,7 +180,9 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     int s = 0;
     uint32_t ph = 0;
     for (int t = pair; t < n_tiles; t += n_pairs) {
-      const int m0 = ((t % mt2) * 2 + rank) * BM, n0 = (t / mt2) * BN + rank * (BN / 2);
+      int mp, nn;
+      tile_mn(t, mp, nn);
+      const int m0 = (mp * 2 + rank) * BM, n0 = nn * BN + rank * (BN / 2);
       for (int kb = 0; kb < nkb; ++kb) {
         mbar_wait_poll(empty_bar(s), ph ^ 1);
         if (elect_one()) {
@@ -223,7 +236,9 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     for (int t = pair; t < n_tiles; t += n_pairs, ++it) {
       const int as = it & 1;
       const uint32_t aph = (it >> 1) & 1;
-      const int m0 = ((t % mt2) * 2 + rank) * BM, n0 = (t / mt2) * BN;
+      int mp, nn;
+      tile_mn(t, mp, nn);
+      const int m0 = (mp * 2 + rank) * BM, n0 = nn * BN;
       const int row = m0 + quad * 32 + lane;
       const bool row_ok = row < M;
       float* const s_bias = s_vec + as * 2 * BN_MAX;
@@ -405,6 +420,15 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   }
 }
 
+// Row-tile pairs per raster group: their A panels (256 rows x K bf16 each) should take about 48 MB of the 126 MB L2.
+int group_rows(int M, int K) {
+  const int mt2 = cdiv(cdiv(M, BM), 2);
+  int gm = (int)(48.0e6 / (512.0 * K) + 0.5);
+  if (gm < 4) gm = 4;
+  if (gm > mt2) gm = mt2;
+  return gm;
+}
+
 int sm_count() {
   static int n = []() {
     int dev = 0, v = 148;
@@ -427,7 +451,7 @@ dit_status launch_t(const CUtensorMap& ta, const CUtensorMap& tb, const CUtensor
   const int pairs = cdiv(cdiv(M, BM), 2) * cdiv(N, BN);
   const int max_pairs = sm_count() / 2;
   DIT_CUDA_OK(launch_pdl(gemm_tc_kernel<EPI, BN>, dim3(2 * (pairs < max_pairs ? pairs : max_pairs)), dim3(GEMM_THREADS),
-                         smem_bytes(BN, EPI), st, 2, ta, tb, tx, ep, M, N, K));
+                         smem_bytes(BN, EPI), st, 2, ta, tb, tx, ep, M, N, K, group_rows(M, K)));
   DIT_LAUNCH_CHECK();
   return DIT_OK;
 }
