@@ -18,6 +18,8 @@
 // (measured, clock64 loop).  Per SM a stage is A + W/2 = 32 KB, written once by TMA and read once by the MMAs per
 // 512 tensor cycles: 128 B/cycle of shared-memory traffic in total — the port's limit; a 1-CTA 128 x 256 tile needs
 // 192 B/cycle and stalled at ~80 % tensor-pipe utilisation.
+#include <cstdlib>
+
 #include "tc.cuh"
 
 namespace dit {
@@ -423,7 +425,11 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
 // Row-tile pairs per raster group: their A panels (256 rows x K bf16 each) should take about 48 MB of the 126 MB L2.
 int group_rows(int M, int K) {
   const int mt2 = cdiv(cdiv(M, BM), 2);
-  int gm = (int)(48.0e6 / (512.0 * K) + 0.5);
+  static const double budget = []() {   // DIT_GEMM_L2_MB overrides the 48 MB default (tuning knob)
+    const char* e = getenv("DIT_GEMM_L2_MB");
+    return (e != nullptr && atof(e) > 0 ? atof(e) : 48.0) * 1.0e6;
+  }();
+  int gm = (int)(budget / (512.0 * K) + 0.5);
   if (gm < 4) gm = 4;
   if (gm > mt2) gm = mt2;
   return gm;
