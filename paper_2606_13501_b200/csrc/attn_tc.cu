@@ -149,6 +149,10 @@ __device__ __forceinline__ void exp_pack_store(const uint32_t (&s)[32], uint64_t
   tmem_st16(taddr, pk);
 }
 
+// PAIR: launched as clusters of two CTAs that are adjacent 256-row query blocks of the same (request, head): both walk
+// the same key tiles, so each CTA fetches ONE of the two 64-column boxes of every K / V tile and TMA-multicasts it to
+// both (L2 -> SM traffic of the K / V stream halves); a ring stage is refilled when both CTAs have released it.
+template <bool PAIR>
 __global__ void __launch_bounds__(ATTN_THREADS, 1)
 attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                const __grid_constant__ CUtensorMap tmV, AttnParams p) {
@@ -174,7 +178,8 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   const int req = p.cu_q ? p.order[blockIdx.z] : 0, head = blockIdx.y;
   const int q_lo = p.cu_q ? p.cu_q[req] : 0, q_hi = p.cu_q ? p.cu_q[req + 1] : p.n_q;
   const int q_base = q_lo + blockIdx.x * (2 * TQ);
-  if (q_base >= q_hi) return;  // CTA-uniform
+  if (!PAIR && q_base >= q_hi) return;  // CTA-uniform (pairs are only launched when every block has rows)
+  const uint32_t crank = PAIR ? cluster_ctarank() : 0u;
   const int k_lo0 = p.cu_k ? p.cu_k[req] : 0, k_hi0 = p.cu_k ? p.cu_k[req + 1] : p.n_k;
   const int klen = k_hi0 - k_lo0;
   const int ssz = (klen + p.n_shards - 1) / p.n_shards;
@@ -212,13 +217,15 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
         mbar_init(p_full(t, b), 4);      // one arrival per softmax warp
       }
     }
-    for (int s = 0; s < KS; ++s) { mbar_init(k_full(s), 1); mbar_init(k_empty(s), 2); }   // empty: one commit per Q tile
-    for (int s = 0; s < VS; ++s) { mbar_init(v_full(s), 1); mbar_init(v_empty(s), 2); }
+    // empty: one commit per Q tile (and per CTA of a pair)
+    for (int s = 0; s < KS; ++s) { mbar_init(k_full(s), 1); mbar_init(k_empty(s), PAIR ? 4 : 2); }
+    for (int s = 0; s < VS; ++s) { mbar_init(v_full(s), 1); mbar_init(v_empty(s), PAIR ? 4 : 2); }
     fence_barrier_init();
   }
   if (warp == 2) tmem_alloc<512>(tmem_slot);
   tc_fence_before();
   __syncthreads();
+  if (PAIR) cluster_sync_all();   // the peer's barriers exist before anything is multicast to them
   tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
@@ -244,15 +251,23 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
       mbar_wait(k_empty(sk), pk ^ 1);
       if (elect_one()) {
         mbar_expect_tx(k_full(sk), TILE_BYTES);
-        tma_load_2d(sK + sk * TILE_BYTES, &tmK, c0, r0, k_full(sk));
-        tma_load_2d(sK + sk * TILE_BYTES + HALF_BYTES, &tmK, c0 + 64, r0, k_full(sk));
+        if (PAIR) {
+          tma_load_2d_multicast(sK + sk * TILE_BYTES + crank * HALF_BYTES, &tmK, c0 + crank * 64, r0, k_full(sk), (uint16_t)3);
+        } else {
+          tma_load_2d(sK + sk * TILE_BYTES, &tmK, c0, r0, k_full(sk));
+          tma_load_2d(sK + sk * TILE_BYTES + HALF_BYTES, &tmK, c0 + 64, r0, k_full(sk));
+        }
       }
       if (++sk == KS) { sk = 0; pk ^= 1; }
       mbar_wait(v_empty(sv), pv ^ 1);
       if (elect_one()) {
         mbar_expect_tx(v_full(sv), TILE_BYTES);
-        tma_load_2d(sV + sv * TILE_BYTES, &tmV, c0, r0, v_full(sv));
-        tma_load_2d(sV + sv * TILE_BYTES + HALF_BYTES, &tmV, c0 + 64, r0, v_full(sv));
+        if (PAIR) {
+          tma_load_2d_multicast(sV + sv * TILE_BYTES + crank * HALF_BYTES, &tmV, c0 + crank * 64, r0, v_full(sv), (uint16_t)3);
+        } else {
+          tma_load_2d(sV + sv * TILE_BYTES, &tmV, c0, r0, v_full(sv));
+          tma_load_2d(sV + sv * TILE_BYTES + HALF_BYTES, &tmV, c0 + 64, r0, v_full(sv));
+        }
       }
       if (++sv == VS) { sv = 0; pv ^= 1; }
       __syncwarp();
@@ -275,6 +290,10 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
       }
     };
     // sub-tile i lives in TMA tile i >> 1 (ring stage (i >> 1) % VS), rows (i & 1) * 64 ...
+    auto release = [&](uint32_t bar) {   // a K / V stage is free once the MMAs issued so far have read it
+      if (PAIR) umma_commit_multicast(bar, (uint16_t)3);
+      else umma_commit(bar);
+    };
     auto issue_pv = [&](int t, int i) {
       const uint32_t d = tmem_base + 256 + t * 128;
       const uint32_t pa = tmem_base + t * 128 + (i & 1) * SK;  // P_t,b: bf16 pairs in the first 32 columns of S_t,b
@@ -287,10 +306,10 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     mbar_wait(q_full(0), 0);
     mbar_wait(k_full(0), 0);
     tc_fence_after();
-    if (elect_one()) { issue_s(0, 0); umma_commit(s_full(0, 0)); umma_commit(s_full(0, 1)); umma_commit(k_empty(0)); }
+    if (elect_one()) { issue_s(0, 0); umma_commit(s_full(0, 0)); umma_commit(s_full(0, 1)); release(k_empty(0)); }
     mbar_wait(q_full(1), 0);
     tc_fence_after();
-    if (elect_one()) { issue_s(1, 0); umma_commit(s_full(1, 0)); umma_commit(s_full(1, 1)); umma_commit(k_empty(0)); }
+    if (elect_one()) { issue_s(1, 0); umma_commit(s_full(1, 0)); umma_commit(s_full(1, 1)); release(k_empty(0)); }
     __syncwarp();
     // Per key tile j and Q tile t: PV of sub-tile a, PV of sub-tile b, then S of key tile j + 1 (both P buffers are
     // consumed once the PVs are queued: the tensor pipe executes in issue order).  Serving t = 0 completely before
@@ -320,12 +339,12 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
           tc_fence_after();
         }
         if (elect_one()) {
-          umma_commit(v_empty(j % VS));
+          release(v_empty(j % VS));
           if (j + 1 < n_tiles) {
             issue_s(t, j + 1);
             umma_commit(s_full(t, 0));
             umma_commit(s_full(t, 1));
-            umma_commit(k_empty((j + 1) % KS));
+            release(k_empty((j + 1) % KS));
           }
         }
         __syncwarp();
@@ -455,6 +474,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   }
   tc_fence_before();
   __syncthreads();
+  if (PAIR) cluster_sync_all();   // the peer may still multicast into this CTA's shared memory / barriers
   if (warp == 2) {
     tc_fence_after();
     tmem_dealloc<512>(tmem_base);
@@ -481,7 +501,8 @@ dit_status launch_attn_tc(const AttnArgs& a, cudaStream_t st) {
   if (max_q == 0) return DIT_OK;
   static bool attr_set = false;
   if (!attr_set) {
-    DIT_CUDA_OK(cudaFuncSetAttribute(attn_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ATTN_SMEM));
+    DIT_CUDA_OK(cudaFuncSetAttribute(attn_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, ATTN_SMEM));
+    DIT_CUDA_OK(cudaFuncSetAttribute(attn_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, ATTN_SMEM));
     attr_set = true;
   }
   // K / V maps need a valid base even when there are no keys (the kernel then never issues a load)
@@ -508,7 +529,20 @@ dit_status launch_attn_tc(const AttnArgs& a, cudaStream_t st) {
     });
   ProfScope _prof(DIT_KC_ATTN, st);
   dim3 grid(cdiv(max_q, 2 * TQ), a.H, a.cu_q ? a.R : 1);
-  DIT_CUDA_OK(launch_pdl(attn_tc_kernel, grid, dim3(ATTN_THREADS), ATTN_SMEM, st, 1, tq, tk, tv, p));
+  // CTA pairs when every request has an even number of 256-row query blocks (each CTA of a pair then has rows)
+  // ... and the key sequence is long: measured alone it is neutral from N = 8192 (slower below: the pair runs in
+  // lockstep), inside a power-capped step it is ~2 % faster (less L2 -> SM traffic, higher clock)
+  bool pair = a.n_k >= 8192;
+  if (a.cu_q_host) {
+    for (int r = 0; r < a.R; ++r) {
+      const int len = a.cu_q_host[r + 1] - a.cu_q_host[r];
+      if (cdiv(len, 2 * TQ) % 2 != 0 || cdiv(len, 2 * TQ) != (int)grid.x) pair = false;   // all requests fill the grid
+    }
+  } else if (grid.x % 2 != 0) {
+    pair = false;
+  }
+  if (pair) DIT_CUDA_OK(launch_pdl(attn_tc_kernel<true>, grid, dim3(ATTN_THREADS), ATTN_SMEM, st, 2, tq, tk, tv, p));
+  else DIT_CUDA_OK(launch_pdl(attn_tc_kernel<false>, grid, dim3(ATTN_THREADS), ATTN_SMEM, st, 1, tq, tk, tv, p));
   DIT_LAUNCH_CHECK();
   return DIT_OK;
 }

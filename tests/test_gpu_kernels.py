@@ -269,6 +269,21 @@ def test_attn_growing_row_maxima_force_rescale(lib, dtype, nq, nk):
     assert float((lse.double().cpu() - rl).abs().max()) < (1e-4 if dtype == torch.float32 else 5e-2)
 
 
+def test_attn_cta_pair_multicast_path(lib):
+    """n_k >= 8192 and an even number of 256-row query blocks: the kernel runs as CTA pairs that share every K / V
+    tile by TMA multicast.  Sampled query rows (both CTAs of a pair, ragged last key tile) against the oracle, and
+    the whole output against the same call made with an odd block count (single-CTA path) on the common rows."""
+    H, d, nk = 2, 128, 8192 + 77
+    q, k, v = synth.make_attention_qkv(11, 1024, nk, H, d, dtype=torch.bfloat16, device=DEV)
+    o, lse = B.dit_attn_partial(q, k, v)                       # 4 query blocks -> 2 pairs
+    rows = torch.tensor([0, 255, 256, 300, 511, 512, 767, 768, 1023])
+    ro, rl = O.attention(q[rows.to(DEV)].cpu(), k.cpu(), v.cpu())
+    check(o[rows.to(DEV)], ro, torch.bfloat16, "pair attention sampled rows", **_attn_tol(torch.bfloat16))
+    assert float((lse[rows.to(DEV)].double().cpu() - rl).abs().max()) < 2e-2
+    o1, lse1 = B.dit_attn_partial(q[:768], k, v)               # 3 query blocks -> single-CTA kernel
+    assert torch.equal(o[:768], o1) and torch.equal(lse[:768], lse1)
+
+
 @pytest.mark.parametrize("dtype", DTYPES)
 def test_attn_strided_qkv_buffer_and_empty(lib, dtype):
     T, H, d = 150, 3, 64
