@@ -19,7 +19,8 @@ Pins (tests/test_oracle_pins.py, `-m "not gpu"`): brute-force attention in pure 
 softmax rows sum to 1; identical keys -> mean of V; zero gates -> identity (bit exact); split-P
 invariance; merge closed forms; LN / RMSNorm / RoPE / GELU / patchify invariants; torch library routines
 (layer_norm, scaled_dot_product_attention, gelu(tanh), silu) as special cases; stored hand-computed
-fixtures under tests/golden/.
+fixtures under tests/golden/; the trajectory (`dit_sample`): constant-velocity closed form, guidance special cases,
+semigroup property.
 PARITY UNPINNED: the *composition order* of the block (R1, R9, R10, R12: which sub-layer follows which,
 single-stream joint attention, cross-attention placement, final layer) is a definition this repo makes
 — the paper prints nothing it could be checked against beyond the invariants above.
@@ -282,6 +283,27 @@ def dit_step(cfg, W, latents, temb, cond=None, split_p=1, taps=None):
 def dit_step_varlen(cfg, W, latents_list, temb_list, cond_list, split_p=1):
     """§8(c) step 8: packing is DEFINED as running every request on its own."""
     return [dit_step(cfg, W, lat, te, co, split_p) for lat, te, co in zip(latents_list, temb_list, cond_list)]
+
+
+def dit_sample(cfg, W, latents, tembs, sigmas, cond=None, uncond=None, guidance_scale=1.0, split_p=1):
+    """One request's denoising trajectory (§3.1: a request is a chain of trajectory tasks, one per
+    denoising step; DESIGN.md §3 step 9, readings R30-R32).  tembs [n_steps, temb_dim],
+    sigmas n_steps + 1 numbers.  Step i:  v = dit_step(x_i, tembs[i], cond); with `uncond` given (classifier-free
+    guidance)  v = v_u + guidance_scale (v - v_u),  v_u = dit_step(x_i, tembs[i], uncond);  flow-matching Euler update
+    x_{i+1} = x_i + (sigmas[i+1] - sigmas[i]) v.  Returns x_{n_steps} (float64).
+    Pins: closed form for a constant velocity field, guidance special cases (scale 0 / 1, cond == uncond), the
+    semigroup property (a trajectory equals the chained single-step trajectories)."""
+    x = _d(latents).clone()
+    n_steps = len(sigmas) - 1
+    assert tembs.shape[0] == n_steps
+    for i in range(n_steps):
+        te = tembs[i:i + 1]
+        v = dit_step(cfg, W, x, te, cond, split_p)
+        if uncond is not None:
+            vu = dit_step(cfg, W, x, te, uncond, split_p)
+            v = vu + float(guidance_scale) * (v - vu)
+        x = x + (float(sigmas[i + 1]) - float(sigmas[i])) * v
+    return x
 
 
 def block_rows(cfg, W, l, x_in, mods_l, ang, rows, ctx=None):

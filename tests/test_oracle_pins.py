@@ -347,6 +347,72 @@ def test_varlen_is_per_request_and_block_rows():
     assert torch.allclose(got, taps["b1.x_mlp"][rows], rtol=1e-12, atol=1e-14)
 
 
+# ---------------------------------------------------------------- trajectory (dit_sample)
+def _traj_inputs(s, n_steps, seed_tag=""):
+    I = synth.make_inputs(s)
+    ts = [900.0 - 250.0 * i for i in range(n_steps)]
+    tembs = synth.timestep_embedding(ts, s.temb_dim)
+    sigmas = [1.0 - (i / n_steps) ** 1.5 for i in range(n_steps + 1)]      # uneven spacing, decreasing to 0
+    unc = synth.normal(s.seed, "uncond" + seed_tag, (3, s.cond_dim), dtype=s.torch_dtype)
+    return I, tembs, sigmas, unc
+
+
+def test_sample_constant_velocity_closed_form():
+    """final.w = 0 makes v = unpatchify(final.b) whatever x and t are: x_n = x_0 + (sigma_n - sigma_0) v exactly
+    (wrong sign of the step, a dropped step or an accumulated-vs-overwritten state all fail this)."""
+    s = _tiny()
+    W = synth.make_weights(s)
+    W["final.w"] = torch.zeros_like(W["final.w"])
+    I, tembs, sigmas, _ = _traj_inputs(s, 3)
+    cfg = O.cfg_from_shape(s)
+    C_, (F_, H_, W_) = s.latent_channels, s.latent_grid
+    n_tok = (F_ // s.patch[0]) * (H_ // s.patch[1]) * (W_ // s.patch[2])
+    v = O.unpatchify(W["final.b"].double().repeat(n_tok, 1), s.patch, (C_, F_, H_, W_))
+    out = O.dit_sample(cfg, W, I["latents"], tembs, sigmas, I["cond"])
+    want = I["latents"].double() + (sigmas[-1] - sigmas[0]) * v
+    assert torch.allclose(out, want, rtol=0, atol=1e-12)
+    assert sigmas[-1] - sigmas[0] == -1.0 and float((out - I["latents"].double() + v).abs().max()) < 1e-12
+
+
+def test_sample_semigroup_and_single_step():
+    """A 3-step trajectory equals three chained 1-step trajectories with the sliced tembs / sigmas (catches a wrong
+    temb or sigma index), and one step equals x + dsigma * dit_step."""
+    s = _tiny(rope_dims=(0, 8, 8), qk_rmsnorm=True)
+    W = synth.make_weights(s)
+    I, tembs, sigmas, _ = _traj_inputs(s, 3)
+    cfg = O.cfg_from_shape(s)
+    full = O.dit_sample(cfg, W, I["latents"], tembs, sigmas, I["cond"])
+    x = I["latents"].double()
+    for i in range(3):
+        x1 = O.dit_sample(cfg, W, x, tembs[i:i + 1], sigmas[i:i + 2], I["cond"])
+        v = O.dit_step(cfg, W, x, tembs[i:i + 1], I["cond"])
+        assert torch.allclose(x1, x + (sigmas[i + 1] - sigmas[i]) * v, rtol=0, atol=1e-13)
+        x = x1
+    assert torch.equal(full, x)
+    # the steps really differ (tembs and sigmas are not interchangeable): permuting tembs changes the result
+    perm = O.dit_sample(cfg, W, I["latents"], tembs.flip(0), sigmas, I["cond"])
+    assert float((perm - full).abs().max()) > 1e-6
+
+
+def test_sample_guidance_special_cases():
+    s = _tiny()
+    W = synth.make_weights(s)
+    I, tembs, sigmas, unc = _traj_inputs(s, 2)
+    cfg = O.cfg_from_shape(s)
+    lat, cond = I["latents"], I["cond"]
+    only_c = O.dit_sample(cfg, W, lat, tembs, sigmas, cond)
+    only_u = O.dit_sample(cfg, W, lat, tembs, sigmas, unc)
+    assert torch.allclose(O.dit_sample(cfg, W, lat, tembs, sigmas, cond, unc, 1.0), only_c, rtol=0, atol=1e-13)
+    assert torch.allclose(O.dit_sample(cfg, W, lat, tembs, sigmas, cond, unc, 0.0), only_u, rtol=0, atol=1e-13)
+    assert torch.allclose(O.dit_sample(cfg, W, lat, tembs, sigmas, cond, cond, 7.5), only_c, rtol=0, atol=1e-12)
+    # one step: the guided update is affine in the scale, x(g) = x(0) + g (x(1) - x(0))
+    g1 = O.dit_sample(cfg, W, lat, tembs[:1], sigmas[:2], cond, unc, 3.0)
+    c1 = O.dit_sample(cfg, W, lat, tembs[:1], sigmas[:2], cond)
+    u1 = O.dit_sample(cfg, W, lat, tembs[:1], sigmas[:2], unc)
+    assert torch.allclose(g1, u1 + 3.0 * (c1 - u1), rtol=0, atol=1e-13)
+    assert float((only_c - only_u).abs().max()) > 1e-6
+
+
 def test_cfg1_shape_facts():
     s = synth.cfg1()
     assert s.n_tokens == 256 and s.n_cond == 32 and s.token_grid == (1, 16, 16)
