@@ -111,6 +111,26 @@ dit_status dit_init(const dit_config* cfg, const dit_weight* weights, int32_t n_
 dit_status dit_step(dit_handle h, const void* latents, const float* timestep_emb, const void* cond_tokens,
                     int32_t n_cond, const int32_t latent_grid[3], void* out, void* stream);
 
+/* One request's denoising TRAJECTORY: n_steps denoising steps chained by the sampler update (PAPER.md:133 — a request
+ * is a chain of trajectory tasks, one per denoising step; DESIGN.md §3 step 9, readings R30-R32):
+ *     x_0 = latents;   for i = 0 .. n_steps-1:
+ *         v_c = dit_step(x_i, timestep_embs[i], cond_tokens)
+ *         v   = uncond_tokens ? v_u + guidance_scale * (v_c - v_u),  v_u = dit_step(x_i, timestep_embs[i], uncond_tokens)
+ *                             : v_c                                   (classifier-free guidance, two passes per step)
+ *         x_{i+1} = x_i + (sigmas[i+1] - sigmas[i]) * v               (flow-matching Euler update)
+ *     out = x_{n_steps}
+ *   latents       dev, [C, F, H, W] config dtype            out  dev, same shape and dtype (may not alias latents)
+ *   timestep_embs dev, [n_steps, temb_dim] fp32             sigmas  HOST, [n_steps + 1] fp32
+ *   cond_tokens / uncond_tokens  dev, [n_cond | n_uncond, cond_dim] config dtype; uncond_tokens NULL = no guidance
+ * The state x_i is carried in fp32 inside the workspace; every step reads x_i rounded to the config dtype (it is staged
+ * in `out`) and v is the fp32 result of the final Linear — the update is fused into the unpatchify kernel.
+ * use_graph != 0: the whole trajectory is captured once into a CUDA graph (cached in the handle, keyed by every
+ * argument) and replayed with one launch; identical results.  n_steps == 0 copies latents to out. */
+dit_status dit_sample(dit_handle h, const void* latents, const float* timestep_embs, const float* sigmas_host,
+                      const void* cond_tokens, int32_t n_cond, const void* uncond_tokens, int32_t n_uncond,
+                      float guidance_scale, const int32_t latent_grid[3], int32_t n_steps, int32_t use_graph, void* out,
+                      void* stream);
+
 /* Same computation with HOST buffers (pageable or pinned): H2D copies of latents / timestep_emb / cond,
  * the step, and the D2H copy of `out` are all enqueued on `stream`; staging lives in the workspace.
  * This is the end-to-end call bench.py times ("e2e"). */

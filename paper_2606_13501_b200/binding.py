@@ -18,7 +18,7 @@ EPI_BIAS, EPI_BIAS_GELU, EPI_BIAS_F32 = 0, 1, 2
 TAP = dict(x=0, y=1, qkv=2, o=3, u=5, c=6, mod=7, tok=8)
 STAGE = dict(y1=0, qkv=1, attn=2, oproj=3, cross=4, y2=5, fc1=6, fc2=7)
 
-SYMBOLS = ["dit_workspace_bytes", "dit_init", "dit_step", "dit_step_host", "dit_step_varlen", "dit_attn_partial",
+SYMBOLS = ["dit_workspace_bytes", "dit_init", "dit_step", "dit_step_host", "dit_step_varlen", "dit_sample", "dit_attn_partial",
            "dit_attn_merge", "dit_linear", "dit_linear_residual", "dit_linear_qkv", "dit_adaln", "dit_gemv", "dit_qknorm_rope", "dit_debug_stop_after",
            "dit_get_tap", "dit_profile_begin", "dit_profile_end", "dit_last_error", "dit_kernel_launches", "dit_free"]
 
@@ -66,6 +66,7 @@ def load(path: str = LIB_PATH):
         "dit_step": [vp, vp, vp, vp, i32, pi32, vp, vp],
         "dit_step_host": [vp, vp, vp, vp, i32, pi32, vp, vp],
         "dit_step_varlen": [vp, vp, vp, vp, pi32, pi32, pi32, i32, vp, vp],
+        "dit_sample": [vp, vp, vp, C.POINTER(C.c_float), vp, i32, vp, i32, f32, pi32, i32, i32, vp, vp],
         "dit_attn_partial": [i32, vp, vp, vp, i32, i32, i32, i32, i64, i64, f32, vp, vp, vp],
         "dit_attn_merge": [i32, C.POINTER(vp), C.POINTER(vp), i32, i32, i32, i32, vp, vp, vp],
         "dit_linear": [i32, i32, vp, i64, vp, vp, vp, i64, i32, i32, i32, vp],
@@ -166,6 +167,22 @@ class Dit:
         n_cond = 0 if cond is None else cond.shape[0]
         _check(self.lib.dit_step(self.handle, _ptr(latents), _ptr(temb), _ptr(cond), n_cond, grid, _ptr(out),
                                  _stream(stream)), "dit_step")
+        return out
+
+    def dit_sample(self, latents, tembs, sigmas, cond=None, uncond=None, guidance_scale=1.0, use_graph=False, out=None,
+                   stream=None):
+        """n_steps = tembs.shape[0] denoising steps chained by the Euler update; tembs [n_steps, temb_dim] fp32 (device),
+        sigmas: n_steps + 1 host floats; uncond given = classifier-free guidance (two passes per step)."""
+        out = torch.empty_like(latents) if out is None else out
+        n_steps = int(tembs.shape[0])
+        assert len(sigmas) == n_steps + 1
+        sig = (C.c_float * (n_steps + 1))(*[float(x) for x in sigmas])
+        grid = _i32arr(latents.shape[1:])
+        n_cond = 0 if cond is None else cond.shape[0]
+        n_unc = 0 if uncond is None else uncond.shape[0]
+        _check(self.lib.dit_sample(self.handle, _ptr(latents), _ptr(tembs), sig, _ptr(cond), n_cond, _ptr(uncond), n_unc,
+                                   float(guidance_scale), grid, n_steps, int(bool(use_graph)), _ptr(out), _stream(stream)),
+               "dit_sample")
         return out
 
     def dit_step_host(self, latents_host, temb_host, cond_host=None, out_host=None, stream=None):

@@ -209,8 +209,18 @@ dit_status launch_rope_table(const SeqMeta* meta, int R, int T, int d, const int
                              float* rc, float* rs, cudaStream_t st);
 dit_status launch_patchify(int dtype, const void* lat, void* patches, int C, int F, int H, int W, const int32_t patch[3],
                            cudaStream_t st);
+// Sampler epilogue of the unpatchify kernel (dit_sample).  mode 0: out = v.  mode 1: v_hold = v (fp32, no out).
+// mode 2: v' = v_hold ? v_hold + guidance (v - v_hold) : v;  state += dsigma v';  out = state.
+struct SampleEpi {
+  int mode;
+  float* state;
+  float* v_hold;
+  float dsigma, guidance;
+};
 dit_status launch_unpatchify(int dtype, const float* tok, void* out, int C, int F, int H, int W, const int32_t patch[3],
-                             cudaStream_t st);
+                             cudaStream_t st, const SampleEpi* epi = nullptr);
+dit_status launch_sample_init(int dtype, const void* lat, float* state, int64_t n, cudaStream_t st);
+dit_status launch_sample_final(int dtype, const float* state, void* out, int64_t n, cudaStream_t st);
 dit_status launch_merge(int dtype, const void* const* o_parts, const float* const* lses, int P, int64_t n_rows_heads,
                         int d, void* o, float* lse_out, cudaStream_t st);
 

@@ -82,6 +82,8 @@ struct Workspace {
   GemvBatch* gemv_tab; // [L + 1 + 2]
   void* stage_in;  // host-call staging: latents | temb | cond
   void* stage_out;
+  float* sample_x; // dit_sample: fp32 trajectory state [Tm * C*pv]
+  float* sample_v; // dit_sample: unconditional velocity of a guided step, fp32
   size_t total;
 };
 
@@ -98,6 +100,10 @@ struct dit_handle_s {
   int stop_block, stop_stage;
   // cached per-call geometry (skip rebuilding RoPE tables when unchanged)
   std::vector<int32_t> last_geom;
+  // dit_sample: one cached trajectory graph, valid while every argument (and sigma) it was captured with is unchanged
+  cudaGraphExec_t graph_exec = nullptr;
+  cudaStream_t cap_stream = nullptr;   // capture happens here (the caller's stream may be the legacy default stream)
+  std::vector<uint64_t> graph_key;
   char err[512];
 };
 
@@ -138,6 +144,8 @@ static bool carve(const dit_config& c, char* base, Workspace* w) {
   w->gemv_tab = (GemvBatch*)take((L + 4) * sizeof(GemvBatch));
   w->stage_in = take(Tm * pvC * es + Rm * c.temb_dim * 4 + Lcm * c.cond_dim * es + 1024);
   w->stage_out = take(Tm * pvC * es);
+  w->sample_x = (float*)take(Tm * pvC * 4);
+  w->sample_v = (float*)take(Tm * pvC * 4);
   w->total = off;
   return true;
 }
@@ -212,21 +220,14 @@ struct StepGeom {
   std::vector<int64_t> lat_off;   // [R+1] element offsets in the packed latents
 };
 
-static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents, const float* temb, const void* cond,
-                           void* out, cudaStream_t st) {
+// Per-call geometry to the device (pageable host memory: the driver stages it before returning) and the RoPE tables;
+// skipped when the geometry is the one already resident.  Not capturable: dit_sample calls it before it begins a capture.
+static dit_status upload_geom(dit_handle hd, const StepGeom& g, cudaStream_t st) {
   const dit_config& c = hd->cfg;
   Workspace& w = hd->ws;
-  const int dt = c.dtype;
-  const size_t es = esize(dt);
-  const int D = c.hidden, F = c.mlp_dim, H = c.n_heads, d = c.head_dim, L = c.n_blocks, R = g.R;
-  const int pvC = c.latent_channels * c.patch[0] * c.patch[1] * c.patch[2];
-  const int T = g.cu[R];
-  const int64_t mod_stride = (int64_t)L * 6 * D + 2 * D;
-  const bool joint = c.cond_mode == DIT_COND_JOINT, cross = c.cond_mode == DIT_COND_CROSS;
+  const int R = g.R, T = g.cu[R], d = c.head_dim;
+  const bool joint = c.cond_mode == DIT_COND_JOINT;
   const bool rope = (c.rope_dims[0] + c.rope_dims[1] + c.rope_dims[2]) > 0;
-  auto stop = [&](int blk, int stage) { return hd->stop_block == blk && hd->stop_stage == stage; };
-
-  // ---- per-call geometry to the device (pageable host memory: the driver stages it before returning)
   std::vector<SeqMeta> meta(R);
   std::vector<int32_t> geom;
   for (int r = 0; r < R; ++r) {
@@ -241,16 +242,34 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
     geom.insert(geom.end(), {meta[r].seq_start, meta[r].n_cond, meta[r].gf, meta[r].gh, meta[r].gw});
   }
   geom.push_back(T);
-  const bool geom_changed = geom != hd->last_geom;
-  if (geom_changed) {
-    DIT_CUDA_OK(cudaMemcpyAsync(w.cu_dev, g.cu.data(), (R + 1) * 4, cudaMemcpyHostToDevice, st));
-    DIT_CUDA_OK(cudaMemcpyAsync(w.cu_cond_dev, g.cu_cond.data(), (R + 1) * 4, cudaMemcpyHostToDevice, st));
-    DIT_CUDA_OK(cudaMemcpyAsync(w.meta_dev, meta.data(), R * sizeof(SeqMeta), cudaMemcpyHostToDevice, st));
-    if (rope) {
-      dit_status s = launch_rope_table(w.meta_dev, R, T, d, c.rope_dims, c.rope_theta, w.rope_c, w.rope_s, st);
-      if (s != DIT_OK) return s;
-    }
-    hd->last_geom = geom;
+  if (geom == hd->last_geom) return DIT_OK;
+  DIT_CUDA_OK(cudaMemcpyAsync(w.cu_dev, g.cu.data(), (R + 1) * 4, cudaMemcpyHostToDevice, st));
+  DIT_CUDA_OK(cudaMemcpyAsync(w.cu_cond_dev, g.cu_cond.data(), (R + 1) * 4, cudaMemcpyHostToDevice, st));
+  DIT_CUDA_OK(cudaMemcpyAsync(w.meta_dev, meta.data(), R * sizeof(SeqMeta), cudaMemcpyHostToDevice, st));
+  if (rope) {
+    dit_status s = launch_rope_table(w.meta_dev, R, T, d, c.rope_dims, c.rope_theta, w.rope_c, w.rope_s, st);
+    if (s != DIT_OK) return s;
+  }
+  hd->last_geom = geom;
+  return DIT_OK;
+}
+
+static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents, const float* temb, const void* cond,
+                           void* out, cudaStream_t st, const SampleEpi* epi = nullptr) {
+  const dit_config& c = hd->cfg;
+  Workspace& w = hd->ws;
+  const int dt = c.dtype;
+  const size_t es = esize(dt);
+  const int D = c.hidden, F = c.mlp_dim, H = c.n_heads, d = c.head_dim, L = c.n_blocks, R = g.R;
+  const int pvC = c.latent_channels * c.patch[0] * c.patch[1] * c.patch[2];
+  const int T = g.cu[R];
+  const int64_t mod_stride = (int64_t)L * 6 * D + 2 * D;
+  const bool joint = c.cond_mode == DIT_COND_JOINT, cross = c.cond_mode == DIT_COND_CROSS;
+  const bool rope = (c.rope_dims[0] + c.rope_dims[1] + c.rope_dims[2]) > 0;
+  auto stop = [&](int blk, int stage) { return hd->stop_block == blk && hd->stop_stage == stage; };
+  {
+    dit_status gs = upload_geom(hd, g, st);
+    if (gs != DIT_OK) return gs;
   }
   const int32_t* cu_dev = R > 1 ? w.cu_dev : nullptr;
   dit_status s;
@@ -363,7 +382,7 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
     const int row0 = g.cu[r] + (joint ? g.ncond[r] : 0);
     float* tk = w.tok + (size_t)row0 * pvC;
     RUN(gemm(dt, DIT_EPI_BIAS_F32, (char*)w.y + (size_t)row0 * D * es, D, hd->f_w, hd->f_b, tk, pvC, Nr, pvC, D, st, DIT_KC_MISC));
-    RUN(launch_unpatchify(dt, tk, (char*)out + g.lat_off[r] * es, c.latent_channels, Fr, Hr, Wr, c.patch, st));
+    RUN(launch_unpatchify(dt, tk, (char*)out + g.lat_off[r] * es, c.latent_channels, Fr, Hr, Wr, c.patch, st, epi));
   }
 #undef RUN
   return DIT_OK;
@@ -541,6 +560,78 @@ dit_status dit_step_host(dit_handle h, const void* latents_host, const float* ti
   return DIT_OK;
 }
 
+dit_status dit_sample(dit_handle h, const void* latents, const float* timestep_embs, const float* sigmas_host,
+                      const void* cond_tokens, int32_t n_cond, const void* uncond_tokens, int32_t n_uncond,
+                      float guidance_scale, const int32_t latent_grid[3], int32_t n_steps, int32_t use_graph, void* out,
+                      void* stream) {
+  DIT_REQUIRE(h != nullptr, DIT_ERR_INVALID_ARG, "handle is NULL");
+  DIT_REQUIRE(latents && latent_grid && out && n_steps >= 0, DIT_ERR_INVALID_ARG, "NULL tensor argument or n_steps < 0");
+  DIT_REQUIRE(n_steps == 0 || (timestep_embs && sigmas_host), DIT_ERR_INVALID_ARG, "timestep_embs / sigmas is NULL");
+  DIT_REQUIRE(latents != out, DIT_ERR_INVALID_ARG, "out may not alias latents");
+  const dit_config& c = h->cfg;
+  cudaStream_t st = (cudaStream_t)stream;
+  const bool guided = uncond_tokens != nullptr;
+  StepGeom gc, gu;
+  dit_status s = build_geom(h, 1, nullptr, &n_cond, latent_grid, &gc);
+  if (s != DIT_OK) return s;
+  DIT_REQUIRE(gc.cu_cond[1] == 0 || cond_tokens != nullptr, DIT_ERR_INVALID_ARG, "cond tokens announced but cond pointer is NULL");
+  if (guided) {
+    s = build_geom(h, 1, nullptr, &n_uncond, latent_grid, &gu);
+    if (s != DIT_OK) return s;
+  }
+  const int64_t n = gc.lat_off[1];
+  Workspace& w = h->ws;
+  // cond and uncond token counts may differ: in joint mode that changes the sequence geometry (rows, RoPE table), which is
+  // uploaded outside a capture; a guided trajectory with n_cond != n_uncond in joint mode therefore runs without a graph
+  const bool same_geom = !guided || gu.cu == gc.cu;
+  auto enqueue = [&](cudaStream_t st) -> dit_status {
+    dit_status e = launch_sample_init(c.dtype, latents, w.sample_x, n, st);
+    if (e != DIT_OK) return e;
+    for (int i = 0; i < n_steps; ++i) {
+      const void* x_in = i == 0 ? latents : out;   // x_i rounded to the config dtype was staged in `out` by step i - 1
+      const float* temb = timestep_embs + (size_t)i * c.temb_dim;
+      SampleEpi epi{2, w.sample_x, nullptr, sigmas_host[i + 1] - sigmas_host[i], guidance_scale};
+      if (guided) {
+        SampleEpi hold{1, nullptr, w.sample_v, 0.f, 0.f};
+        e = run_step(h, gu, x_in, temb, uncond_tokens, out, st, &hold);
+        if (e != DIT_OK) return e;
+        epi.v_hold = w.sample_v;
+      }
+      e = run_step(h, gc, x_in, temb, cond_tokens, out, st, &epi);
+      if (e != DIT_OK) return e;
+    }
+    if (n_steps == 0) return launch_sample_final(c.dtype, w.sample_x, out, n, st);
+    return DIT_OK;
+  };
+  if (!use_graph || n_steps == 0 || !same_geom || g_prof_mask != 0) return enqueue(st);
+
+  std::vector<uint64_t> key = {(uint64_t)(uintptr_t)latents, (uint64_t)(uintptr_t)timestep_embs, (uint64_t)(uintptr_t)cond_tokens,
+                               (uint64_t)(uintptr_t)uncond_tokens, (uint64_t)(uintptr_t)out, (uint64_t)n_cond, (uint64_t)n_uncond,
+                               (uint64_t)n_steps, (uint64_t)latent_grid[0], (uint64_t)latent_grid[1], (uint64_t)latent_grid[2]};
+  uint32_t gbits;
+  memcpy(&gbits, &guidance_scale, 4);
+  key.push_back(gbits);
+  for (int i = 0; i <= n_steps; ++i) { uint32_t b; memcpy(&b, &sigmas_host[i], 4); key.push_back(b); }
+  if (h->graph_exec == nullptr || key != h->graph_key) {
+    if (h->graph_exec) { cudaGraphExecDestroy(h->graph_exec); h->graph_exec = nullptr; }
+    s = upload_geom(h, gc, st);   // host -> device geometry copies and the RoPE table are enqueued outside the capture
+    if (s != DIT_OK) return s;
+    if (h->cap_stream == nullptr) DIT_CUDA_OK(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
+    DIT_CUDA_OK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeRelaxed));
+    s = enqueue(h->cap_stream);
+    cudaGraph_t graph = nullptr;
+    cudaError_t ce = cudaStreamEndCapture(h->cap_stream, &graph);
+    if (s != DIT_OK) { if (graph) cudaGraphDestroy(graph); return s; }
+    DIT_REQUIRE(ce == cudaSuccess && graph != nullptr, DIT_ERR_CUDA, "dit_sample: stream capture failed: %s", cudaGetErrorString(ce));
+    ce = cudaGraphInstantiate(&h->graph_exec, graph, 0);
+    cudaGraphDestroy(graph);
+    DIT_REQUIRE(ce == cudaSuccess, DIT_ERR_CUDA, "dit_sample: cudaGraphInstantiate failed: %s", cudaGetErrorString(ce));
+    h->graph_key = key;
+  }
+  DIT_CUDA_OK(cudaGraphLaunch(h->graph_exec, st));
+  return DIT_OK;
+}
+
 dit_status dit_attn_partial(int32_t dtype, const void* q, const void* k, const void* v, int32_t n_q, int32_t n_k,
                             int32_t n_heads, int32_t head_dim, int64_t q_row_stride, int64_t kv_row_stride,
                             float softmax_scale, void* o, float* lse, void* stream) {
@@ -692,6 +783,8 @@ int32_t dit_kernel_launches(void) { return g_launches; }
 
 void dit_free(dit_handle h) {
   if (!h) return;
+  if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
+  if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
   delete[] h->blocks;
   delete h;
 }

@@ -420,7 +420,7 @@ __global__ void patchify_kernel(const T* __restrict__ lat, T* __restrict__ patch
 
 template <typename T>
 __global__ void unpatchify_kernel(const float* __restrict__ tok, T* __restrict__ out, int C, int F, int H, int W,
-                                  int pf, int ph, int pw) {
+                                  int pf, int ph, int pw, SampleEpi epi) {
   const int Hp = H / ph, Wp = W / pw, pv = pf * ph * pw;
   const int64_t total = (int64_t)C * F * H * W;
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -429,7 +429,31 @@ __global__ void unpatchify_kernel(const float* __restrict__ tok, T* __restrict__
   const int c = (int)(idx / ((int64_t)W * H * F));
   const int n = ((f / pf) * Hp + hh / ph) * Wp + w / pw;
   const int feat = ((c * pf + f % pf) * ph + hh % ph) * pw + w % pw;
-  out[idx] = from_f<T>(tok[(int64_t)n * (C * pv) + feat]);
+  float v = tok[(int64_t)n * (C * pv) + feat];
+  if (epi.mode == 1) {          // unconditional pass of a guided step: keep v_u in fp32
+    epi.v_hold[idx] = v;
+    return;
+  }
+  if (epi.mode == 2) {          // Euler update on the fp32 state (dit_sample)
+    if (epi.v_hold != nullptr) {
+      const float vu = epi.v_hold[idx];
+      v = vu + epi.guidance * (v - vu);
+    }
+    v = epi.state[idx] + epi.dsigma * v;
+    epi.state[idx] = v;
+  }
+  out[idx] = from_f<T>(v);
+}
+
+template <typename T>
+__global__ void sample_init_kernel(const T* __restrict__ lat, float* __restrict__ state, int64_t n) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx < n) state[idx] = to_f(lat[idx]);
+}
+template <typename T>
+__global__ void sample_final_kernel(const float* __restrict__ state, T* __restrict__ out, int64_t n) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx < n) out[idx] = from_f<T>(state[idx]);
 }
 
 dit_status launch_patchify(int dtype, const void* lat, void* patches, int C, int F, int H, int W, const int32_t patch[3],
@@ -448,14 +472,33 @@ dit_status launch_patchify(int dtype, const void* lat, void* patches, int C, int
 }
 
 dit_status launch_unpatchify(int dtype, const float* tok, void* out, int C, int F, int H, int W, const int32_t patch[3],
-                             cudaStream_t st) {
+                             cudaStream_t st, const SampleEpi* epi) {
   const int64_t total = (int64_t)C * F * H * W;
   if (total == 0) return DIT_OK;
+  const SampleEpi e = epi ? *epi : SampleEpi{0, nullptr, nullptr, 0.f, 0.f};
   ProfScope _prof(DIT_KC_MISC, st);
   if (dtype == DIT_F32)
-    unpatchify_kernel<float><<<cdiv(total, 256), 256, 0, st>>>(tok, (float*)out, C, F, H, W, patch[0], patch[1], patch[2]);
+    unpatchify_kernel<float><<<cdiv(total, 256), 256, 0, st>>>(tok, (float*)out, C, F, H, W, patch[0], patch[1], patch[2], e);
   else
-    unpatchify_kernel<bf16><<<cdiv(total, 256), 256, 0, st>>>(tok, (bf16*)out, C, F, H, W, patch[0], patch[1], patch[2]);
+    unpatchify_kernel<bf16><<<cdiv(total, 256), 256, 0, st>>>(tok, (bf16*)out, C, F, H, W, patch[0], patch[1], patch[2], e);
+  DIT_LAUNCH_CHECK();
+  return DIT_OK;
+}
+
+dit_status launch_sample_init(int dtype, const void* lat, float* state, int64_t n, cudaStream_t st) {
+  if (n == 0) return DIT_OK;
+  ProfScope _prof(DIT_KC_MISC, st);
+  if (dtype == DIT_F32) sample_init_kernel<float><<<cdiv(n, 256), 256, 0, st>>>((const float*)lat, state, n);
+  else sample_init_kernel<bf16><<<cdiv(n, 256), 256, 0, st>>>((const bf16*)lat, state, n);
+  DIT_LAUNCH_CHECK();
+  return DIT_OK;
+}
+
+dit_status launch_sample_final(int dtype, const float* state, void* out, int64_t n, cudaStream_t st) {
+  if (n == 0) return DIT_OK;
+  ProfScope _prof(DIT_KC_MISC, st);
+  if (dtype == DIT_F32) sample_final_kernel<float><<<cdiv(n, 256), 256, 0, st>>>(state, (float*)out, n);
+  else sample_final_kernel<bf16><<<cdiv(n, 256), 256, 0, st>>>(state, (bf16*)out, n);
   DIT_LAUNCH_CHECK();
   return DIT_OK;
 }

@@ -1,0 +1,116 @@
+"""GPU parity of dit_sample (a request's denoising trajectory: steps chained by the Euler update, optional
+classifier-free guidance, optional CUDA-graph replay) against the CPU oracle's dit_sample on the same seeded inputs."""
+import pytest
+import torch
+
+from oracle import dit_oracle as O
+from paper_2606_13501_b200 import binding as B
+from paper_2606_13501_b200 import synth
+from util import check, errors
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda:0"
+
+
+def _traj(s, n_steps, n_unc=None):
+    I = synth.make_inputs(s)
+    ts = [900.0 - 700.0 * i / max(1, n_steps) for i in range(n_steps)]
+    tembs = synth.timestep_embedding(ts, s.temb_dim) if n_steps else torch.zeros(0, s.temb_dim)
+    sigmas = [1.0 - (i / max(1, n_steps)) ** 1.5 for i in range(n_steps + 1)]
+    unc = None
+    if n_unc is not None and s.cond_mode != "none":
+        unc = synth.normal(s.seed, "uncond", (n_unc, s.cond_dim), dtype=s.torch_dtype)
+    return I, tembs, sigmas, unc
+
+
+def _both(s, n_steps, n_unc=None, g=1.0, use_graph=False, split_p=1):
+    W = synth.make_weights(s)
+    I, tembs, sigmas, unc = _traj(s, n_steps, n_unc)
+    ref = O.dit_sample(O.cfg_from_shape(s), W, I["latents"], tembs, sigmas, I["cond"], unc, g)
+    m = B.Dit(B.make_config(s, split_p=split_p), W, DEV)
+    dev = lambda t: None if t is None else t.to(DEV)
+    args = (dev(I["latents"]), dev(tembs), sigmas, dev(I["cond"]), dev(unc), g)
+    out = m.dit_sample(*args, use_graph=use_graph)
+    torch.cuda.synchronize()
+    return out, ref, m, args, I
+
+
+def _check_traj(out, ref, I, dt, what, disp_rel):
+    check(out, ref, dt, what)
+    x0 = I["latents"].double()
+    e_rel, _ = errors(out.double().cpu() - x0, ref - x0)      # the displacement: x_0 does not mask the velocity error
+    assert e_rel <= disp_rel, f"{what}: displacement rel-L2 {e_rel:.3e} > {disp_rel:.1e}"
+
+
+@pytest.mark.parametrize("use_graph", [False, True])
+def test_cfg1_fp32_trajectory(lib, use_graph):
+    s = synth.cfg1()
+    out, ref, *_, I = _both(s, 3, use_graph=use_graph)
+    _check_traj(out, ref, I, torch.float32, "cfg1 3 steps", 2e-5)
+
+
+@pytest.mark.parametrize("mode,n_unc,use_graph", [("joint", 16, False), ("joint", 32, True), ("cross", 16, True)])
+def test_fp32_guided_trajectory(lib, mode, n_unc, use_graph):
+    """Joint mode with n_uncond != n_cond changes the sequence geometry between the two passes (no graph)."""
+    s = synth.cfg1(cond_mode=mode, rope_dims=(0, 32, 32), qk_rmsnorm=True)
+    out, ref, *_, I = _both(s, 2, n_unc=n_unc, g=4.0, use_graph=use_graph, split_p=2)
+    _check_traj(out, ref, I, torch.float32, f"cfg1 guided {mode}", 5e-5)
+
+
+@pytest.mark.parametrize("use_graph", [False, True])
+def test_bf16_guided_trajectory(lib, use_graph):
+    s = synth.cfg1(name="traj_bf16", dtype="bf16", hidden=512, n_heads=4, head_dim=128, mlp_dim=2048, cond_dim=512,
+                   latent_channels=16, rope_dims=(0, 64, 64), qk_rmsnorm=True, n_blocks=3)
+    out, ref, *_, I = _both(s, 4, n_unc=32, g=3.0, use_graph=use_graph)
+    _check_traj(out, ref, I, torch.bfloat16, "bf16 guided 4 steps", 2e-2)
+
+
+def test_graph_replay_is_bit_identical_and_recaptures_on_change(lib):
+    s = synth.cfg1(name="traj_bf16", dtype="bf16", hidden=512, n_heads=4, head_dim=128, mlp_dim=2048, cond_dim=512,
+                   latent_channels=16, rope_dims=(0, 64, 64), qk_rmsnorm=True)
+    out_e, ref, m, args, I = _both(s, 3, n_unc=32, g=2.0, use_graph=False)
+    lat, tembs, sigmas, cond, unc, g = args
+    out_g = torch.empty_like(lat)
+    for _ in range(3):                                   # capture, then two replays of the cached graph
+        out_g.zero_()
+        m.dit_sample(lat, tembs, sigmas, cond, unc, g, use_graph=True, out=out_g)
+        torch.cuda.synchronize()
+        assert torch.equal(out_g, out_e)
+    sig2 = [x * 0.5 for x in sigmas]                     # a changed schedule must not replay the stale graph
+    m.dit_sample(lat, tembs, sig2, cond, unc, g, use_graph=True, out=out_g)
+    want = m.dit_sample(lat, tembs, sig2, cond, unc, g, use_graph=False)
+    torch.cuda.synchronize()
+    assert torch.equal(out_g, want) and not torch.equal(out_g, out_e)
+    # the plain step still works after a trajectory (geometry cache, workspace) and matches a fresh run
+    v = m.dit_step(lat, tembs[0], cond)
+    v2 = B.Dit(B.make_config(s), synth.make_weights(s), DEV).dit_step(lat, tembs[0], cond)
+    torch.cuda.synchronize()
+    assert torch.equal(v, v2)
+
+
+def test_zero_steps_and_argument_errors(lib):
+    s = synth.cfg1()
+    W = synth.make_weights(s)
+    I, tembs, sigmas, _ = _traj(s, 0)
+    m = B.Dit(B.make_config(s), W, DEV)
+    lat = I["latents"].to(DEV)
+    out = m.dit_sample(lat, tembs.to(DEV), sigmas, I["cond"].to(DEV))
+    torch.cuda.synchronize()
+    assert torch.equal(out, lat)
+    I, tembs, sigmas, _ = _traj(s, 2)
+    with pytest.raises(B.DitError):
+        m.dit_sample(lat, tembs.to(DEV), sigmas, I["cond"].to(DEV), out=lat)          # out aliases latents
+
+
+def test_one_step_equals_step_plus_update(lib):
+    """dit_sample with one step against dit_step on the same handle: out = x + dsigma v up to the bf16 rounding of v."""
+    s = synth.cfg1()
+    W = synth.make_weights(s)
+    I, tembs, sigmas, _ = _traj(s, 1)
+    m = B.Dit(B.make_config(s), W, DEV)
+    lat, cond, te = I["latents"].to(DEV), I["cond"].to(DEV), tembs.to(DEV)
+    out = m.dit_sample(lat, te, sigmas, cond)
+    v = m.dit_step(lat, te[0], cond)
+    torch.cuda.synchronize()
+    want = lat.double() + (sigmas[1] - sigmas[0]) * v.double()
+    assert float((out.double() - want).abs().max()) <= 1e-6
