@@ -373,6 +373,56 @@ def run_ours(args, rank: int, local_rank: int, world: int):
 
 
 # --------------------------------------------------------------------------------------------------------
+# trajectory arm: dit_sample over a whole request, stream launches vs one CUDA-graph launch
+# --------------------------------------------------------------------------------------------------------
+def run_traj(args):
+    """`--workload traj`: one request of cfg 2 shape through `dit_sample` (n denoising steps chained by the Euler
+    update on the device, no host round trip between steps).  Reports denoising steps/s of the trajectory when its
+    kernels are launched one by one on the stream and when the captured CUDA graph is replayed with one launch, plus a
+    classifier-free-guided trajectory (two passes per step).  `--steps` = trajectories timed, `--traj-steps` = n."""
+    from paper_2606_13501_b200 import binding as B
+    B.load()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    s = _shape("cfg2")
+    n = args.traj_steps
+    W = synth.make_weights(s, device=dev)
+    m = B.Dit(B.make_config(s, split_p=args.split_p), W, dev)
+    I = synth.make_inputs(s, device=dev)
+    lat, cond = I["latents"], I["cond"]
+    unc = synth.normal(s.seed, "uncond", tuple(cond.shape), dtype=s.torch_dtype, device=dev)
+    tembs = synth.timestep_embedding([1000.0 * (1 - i / n) for i in range(n)], s.temb_dim, device=dev).contiguous()
+    sigmas = [1.0 - i / n for i in range(n + 1)]
+    out = torch.empty_like(lat)
+    K, Wm = max(1, min(args.steps, 10)), max(1, min(args.warmup, 3))
+    rows = []
+    for name, u, graph in (("stream launches", None, False), ("cuda graph", None, True),
+                           ("guided (2 passes/step), cuda graph", unc, True)):
+        for _ in range(Wm):
+            m.dit_sample(lat, tembs, sigmas, cond, u, 4.0, use_graph=graph, out=out)
+        torch.cuda.synchronize()
+        n0 = B.dit_kernel_launches()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0 = time.perf_counter()
+        e0.record()
+        for _ in range(K):
+            m.dit_sample(lat, tembs, sigmas, cond, u, 4.0, use_graph=graph, out=out)
+        t_enq = time.perf_counter() - t0
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / K
+        rows.append({"mode": name, "ms_per_trajectory": ms, "denoising_steps_per_s": n / (ms * 1e-3),
+                     "model_passes_per_s": (2 if u is not None else 1) * n / (ms * 1e-3),
+                     "host_enqueue_ms_per_trajectory": t_enq / K * 1e3,
+                     "library_launch_calls_per_trajectory": (B.dit_kernel_launches() - n0) / K})
+    print(json.dumps({"metric": "trajectory denoising steps/s", "unit": UNIT, "n_gpus": 1, "trajectories": K, "warmup": Wm,
+                      "config": {"workload": _workload_name(s), "traj_steps": n, "split_p": args.split_p}, "dtype": "bf16",
+                      "data": "synthetic", "rows": rows}), flush=True)
+
+
+# --------------------------------------------------------------------------------------------------------
 # per-kernel arm: every HBM-bound kernel and the attention sweep (BASELINE.json configs[4]) timed ALONE
 # --------------------------------------------------------------------------------------------------------
 def run_kernels(args):
@@ -480,7 +530,8 @@ def main():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "kernels"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "kernels", "traj"])
+    ap.add_argument("--traj-steps", type=int, default=20, help="--workload traj: denoising steps per trajectory")
     ap.add_argument("--split-p", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--only", default="", help="--workload kernels: time only the kernels whose name contains this")
@@ -492,6 +543,9 @@ def main():
     if args.workload == "kernels":
         if rank == 0:
             run_kernels(args)
+    elif args.workload == "traj":
+        if rank == 0:
+            run_traj(args)
     elif args.impl == "reference":
         run_reference(args, rank)
     else:
