@@ -50,6 +50,10 @@ constexpr float RESCALE_THRESHOLD = 8.0f;  // log2 units
 #ifndef DIT_ATTN_POLY_PAIRS
 #define DIT_ATTN_POLY_PAIRS 2
 #endif
+#ifndef DIT_ATTN_OPTIMISTIC
+#define DIT_ATTN_OPTIMISTIC 1
+#endif
+constexpr bool OPTIMISTIC = DIT_ATTN_OPTIMISTIC != 0;   // 0: every key tile takes the exact path (row max per tile)
 constexpr int POLY_PAIRS = DIT_ATTN_POLY_PAIRS;   // of every 16 score pairs, this many take the FMA-pipe exp2
 
 struct AttnParams {
@@ -173,6 +177,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   // PV_t,i completes pv_done(t, i & 1): a waiter is never more than one phase behind a per-buffer barrier
   auto pv_done = [&](int t, int b) { return bar0 + 8u * (B0 + 8 + 2 * t + b); };
   const uint32_t tmem_slot = bar0 + 8u * (B0 + 12);
+  const uint32_t panic_addr = bar0 + 8u * (B0 + 13);   // set by a softmax warp whose optimistic pass overflowed
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int req = p.cu_q ? p.order[blockIdx.z] : 0, head = blockIdx.y;
@@ -220,6 +225,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     // empty: one commit per Q tile (and per CTA of a pair)
     for (int s = 0; s < KS; ++s) { mbar_init(k_full(s), 1); mbar_init(k_empty(s), PAIR ? 4 : 2); }
     for (int s = 0; s < VS; ++s) { mbar_init(v_full(s), 1); mbar_init(v_empty(s), PAIR ? 4 : 2); }
+    asm volatile("st.shared.u32 [%0], %1;" ::"r"(panic_addr), "r"(0u) : "memory");
     fence_barrier_init();
   }
   if (warp == 2) tmem_alloc<512>(tmem_slot);
@@ -232,20 +238,44 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   pdl_wait();   // prologue done; q / k / v written by the previous kernel are read from here on
 
   // register budget: warpgroup 0 (TMA / MMA / idle warps) gives registers to the two softmax warpgroups
+
+  // Pass 0 is OPTIMISTIC (no row max after the first key tile, see the softmax warps); it is exact unless a row's
+  // scores outgrow the reference by ~2^60 inside one key tile, which a thread notices from its row sum.  Then the
+  // whole CTA (the whole pair) runs pass 1, the exact algorithm with a row max per tile, over the same keys: every
+  // ring stage / barrier phase simply continues (tile counter g = pass * n_tiles + j).
+  const int cnt_b1 = n_sub - n_tiles;   // key tiles per pass that have a sub-tile b (the ragged last one may not)
+  // pass boundary: does the optimistic result stand?  (CTA-wide; a pair decides together — its CTAs share every K / V
+  // stage, so both repeat or neither does.)  Called by every thread of the CTA, from either register-budget branch.
+  auto repeat_exact = [&]() -> bool {
+    tc_fence_before();
+    if (PAIR) cluster_sync_all(); else __syncthreads();
+    tc_fence_after();
+    uint32_t redo;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(redo) : "r"(panic_addr) : "memory");
+    if (PAIR) {
+      uint32_t peer;
+      asm volatile("ld.shared::cluster.u32 %0, [%1];" : "=r"(peer) : "r"(mapa_cluster(panic_addr, crank ^ 1u)) : "memory");
+      redo |= peer;
+    }
+    return redo != 0;
+  };
   if (warp < 4) {
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+  asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+  int sk = 0, sv = 0;                   // TMA producer ring state, runs on across passes
+  uint32_t pk = 0, pv = 0;
+  for (int pass = 0;; ++pass) {
+    const bool exact = !OPTIMISTIC || pass == 1;
+    const int gb = pass * n_tiles;      // global index of this pass's first key tile
   if (warp == 0) {
     // ===================================================== TMA producer
     const int c0 = head * HD;
-    if (elect_one()) {
+    if (pass == 0 && elect_one()) {
       for (int t = 0; t < 2; ++t) {
         mbar_expect_tx(q_full(t), TILE_BYTES);
         tma_load_2d(sQ + t * TILE_BYTES, &tmQ, c0, q_base + t * TQ, q_full(t));
         tma_load_2d(sQ + t * TILE_BYTES + HALF_BYTES, &tmQ, c0 + 64, q_base + t * TQ, q_full(t));
       }
     }
-    int sk = 0, sv = 0;
-    uint32_t pk = 0, pv = 0;
     for (int j = 0; j < n_tiles; ++j) {
       const int r0 = k_lo + j * TK;
       mbar_wait(k_empty(sk), pk ^ 1);
@@ -278,89 +308,100 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     constexpr uint32_t idesc_o = idesc_bf16(TQ, HD, 0, 1);   // O += P V: A from TMEM, B (V) MN-major
     // V tile: two [128 keys x 64 d] boxes 16 KB apart (LBO), 8-key groups 1 KB apart (SBO); 16 keys = +2 KB
     constexpr uint64_t vdesc_hi = desc_base_sw128(HALF_BYTES >> 4, 64);
-    // S of key tile j for Q tile t: ONE N = 128 group fills both 64-column buffers (8 KB of shared memory per
+    // S of key tile g for Q tile t: ONE N = 128 group fills both 64-column buffers (8 KB of shared memory per
     // 64-cycle MMA = 128 B/clk; N = 64 groups would re-read Q for half the work and run shared-memory bound)
-    auto issue_s = [&](int t, int j) {
+    auto issue_s = [&](int t, int g) {
       const uint32_t d = tmem_base + t * 128;
-      const uint32_t qa = sQ + t * TILE_BYTES, ka = sK + (j % KS) * TILE_BYTES;
+      const uint32_t qa = sQ + t * TILE_BYTES, ka = sK + (g % KS) * TILE_BYTES;
 #pragma unroll
       for (int k = 0; k < HD / 16; ++k) {
         const uint32_t off = (k >> 2) * HALF_BYTES + (k & 3) * 32;
         umma_ss(d, desc_kmajor_sw128(qa + off), desc_kmajor_sw128(ka + off), idesc_s, k != 0);
       }
     };
-    // sub-tile i lives in TMA tile i >> 1 (ring stage (i >> 1) % VS), rows (i & 1) * 64 ...
     auto release = [&](uint32_t bar) {   // a K / V stage is free once the MMAs issued so far have read it
       if (PAIR) umma_commit_multicast(bar, (uint16_t)3);
       else umma_commit(bar);
     };
-    auto issue_pv = [&](int t, int i) {
+    // sub-tile b (0 / 1) of key tile g (ring stage g % VS, rows b * 64 ...); `first` = first PV of this pass
+    auto issue_pv = [&](int t, int g, int b, bool first) {
       const uint32_t d = tmem_base + 256 + t * 128;
-      const uint32_t pa = tmem_base + t * 128 + (i & 1) * SK;  // P_t,b: bf16 pairs in the first 32 columns of S_t,b
-      const uint32_t va = sV + ((i >> 1) % VS) * TILE_BYTES + (i & 1) * SUB_BYTES;
+      const uint32_t pa = tmem_base + t * 128 + b * SK;  // P_t,b: bf16 pairs in the first 32 columns of S_t,b
+      const uint32_t va = sV + (g % VS) * TILE_BYTES + b * SUB_BYTES;
 #pragma unroll
       for (int k = 0; k < SK / 16; ++k)
-        umma_ts(d, pa + 8 * k, vdesc_hi | (uint64_t)(((va + k * 2048) >> 4) & 0x3fff), idesc_o, (i > 0 || k != 0) ? 1u : 0u);
+        umma_ts(d, pa + 8 * k, vdesc_hi | (uint64_t)(((va + k * 2048) >> 4) & 0x3fff), idesc_o, (!first || k != 0) ? 1u : 0u);
     };
     // prologue: S of key tile 0 for both Q tiles
     mbar_wait(q_full(0), 0);
-    mbar_wait(k_full(0), 0);
+    mbar_wait(k_full(gb % KS), (uint32_t)(gb / KS) & 1u);
     tc_fence_after();
-    if (elect_one()) { issue_s(0, 0); umma_commit(s_full(0, 0)); umma_commit(s_full(0, 1)); release(k_empty(0)); }
+    if (elect_one()) { issue_s(0, gb); umma_commit(s_full(0, 0)); umma_commit(s_full(0, 1)); release(k_empty(gb % KS)); }
     mbar_wait(q_full(1), 0);
     tc_fence_after();
-    if (elect_one()) { issue_s(1, 0); umma_commit(s_full(1, 0)); umma_commit(s_full(1, 1)); release(k_empty(0)); }
+    if (elect_one()) { issue_s(1, gb); umma_commit(s_full(1, 0)); umma_commit(s_full(1, 1)); release(k_empty(gb % KS)); }
     __syncwarp();
     // Per key tile j and Q tile t: PV of sub-tile a, PV of sub-tile b, then S of key tile j + 1 (both P buffers are
     // consumed once the PVs are queued: the tensor pipe executes in issue order).  Serving t = 0 completely before
     // t = 1 keeps the two Q tiles in anti-phase: one tile's softmax runs under the other tile's 1024 tensor cycles.
     for (int j = 0; j < n_tiles; ++j) {
-      const uint32_t par = (uint32_t)j & 1u;
+      const int g = gb + j;
+      const bool has_b = 2 * j + 1 < n_sub;
       for (int t = 0; t < 2; ++t) {
-        if (t == 0) mbar_wait(v_full(j % VS), (uint32_t)(j / VS) & 1u);
-        mbar_wait(p_full(t, 0), par);
+        if (t == 0) mbar_wait(v_full(g % VS), (uint32_t)(g / VS) & 1u);
+        mbar_wait(p_full(t, 0), (uint32_t)g & 1u);
         tc_fence_after();
         if (elect_one()) {
-          issue_pv(t, 2 * j);
+          issue_pv(t, g, 0, j == 0);
           umma_commit(pv_done(t, 0));
         }
         __syncwarp();
-        if (2 * j + 1 < n_sub) {
-          mbar_wait(p_full(t, 1), par);
+        if (has_b) {
+          mbar_wait(p_full(t, 1), (uint32_t)(pass * cnt_b1 + j) & 1u);
           tc_fence_after();
           if (elect_one()) {
-            issue_pv(t, 2 * j + 1);
+            issue_pv(t, g, 1, false);
             umma_commit(pv_done(t, 1));
           }
           __syncwarp();
         }
         if (j + 1 < n_tiles && t == 0) {
-          mbar_wait(k_full((j + 1) % KS), (uint32_t)((j + 1) / KS) & 1u);
+          mbar_wait(k_full((g + 1) % KS), (uint32_t)((g + 1) / KS) & 1u);
           tc_fence_after();
         }
         if (elect_one()) {
-          release(v_empty(j % VS));
+          release(v_empty(g % VS));
           if (j + 1 < n_tiles) {
-            issue_s(t, j + 1);
+            issue_s(t, g + 1);
             umma_commit(s_full(t, 0));
             umma_commit(s_full(t, 1));
-            release(k_empty((j + 1) % KS));
+            release(k_empty((g + 1) % KS));
           }
         }
         __syncwarp();
       }
     }
   }
+    if (exact || !repeat_exact()) break;
+  }
   } else {
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 104;");
+  asm volatile("setmaxnreg.inc.sync.aligned.u32 104;");
+  for (int pass = 0;; ++pass) {
+    const bool exact = !OPTIMISTIC || pass == 1;
+    const int gb = pass * n_tiles;
     // ===================================================== softmax + correction + epilogue: 16 warps
     // Q tile t has TWO warps per TMEM lane quadrant: the leader (h = 0) owns sub-tile a (keys 0..63 of every key
     // tile), the follower (h = 1) sub-tile b (keys 64..127); both add into the same O_t, so they must use the same
-    // reference max.  The leader reads the whole 128-wide S row for the row max, takes the (lazy) rescale decision
-    // alone, and publishes m_used per key tile through shared memory + a named barrier (arrive / sync, 64 threads);
-    // the follower rescales its partial row sum when m_used changed.  Four softmax warps per scheduler instead of
-    // two: a single warp issues one instruction per ~3 cycles (dependent FFMA2 / MUFU chains), which made the
-    // softmax — not the tensor pipe and not MUFU — the critical path.
+    // reference max.  Four softmax warps per scheduler instead of two: a single warp issues one instruction per ~3
+    // cycles (dependent FFMA2 / MUFU chains), which made the softmax — not the tensor pipe and not MUFU — the
+    // critical path.
+    //   exact tile (every tile of pass 1, the first tile of pass 0): the pair exchanges its half-row maxima through
+    //   shared memory + a named barrier (arrive / sync, 64 threads) and takes the same lazy-rescale decision (R25);
+    //   optimistic tile (pass 0, j > 0): no row max at all.  Any reference is exact as long as nothing overflows
+    //   (P, the row sum and O are all expressed against m_used, which is divided out at the end), so the reference
+    //   only moves when the PREVIOUS tile's row sum shows that the scores have grown by 2^30: the pair exchanges
+    //   last tile's partial sums BEFORE it waits for S(j) — off the S -> P -> PV chain.  A tile sum above 2^60
+    //   (or infinite) raises the CTA's panic flag and the result of this pass is discarded (R33).
     const int w = warp - 4;
     const int t = w >> 3;                          // Q tile
     const int h = (w >> 2) & 1;                    // 0 = leader (sub-tile a), 1 = follower (sub-tile b)
@@ -371,18 +412,73 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     const uint32_t s_base = tmem_base + t * 128 + lane_off;        // S_t,b (fp32, 64 cols) / P_t,b (bf16 pairs, 32 cols)
     const uint32_t o_addr = tmem_base + 256 + t * 128 + lane_off;  // O_t
     float* const xch = reinterpret_cast<float*>(smem_raw + (bar0 - smem_u32(smem_raw)) + 256);
-    float* const m_sh = xch + t * 512;             // [parity][h][128 rows]: half-row maxima
+    float* const m_sh = xch + t * 512;             // [parity][h][128 rows]: half-row maxima / last tile's partial sums
     float* const l_sh = xch + 1024 + t * 256;      // [h][128 rows]: partial row sums
     const int bar_id = 1 + t * 4 + quad;           // named barrier of this (leader, follower) warp pair
     const float c = p.scale_log2;
     const uint64_t c2 = pack2(c, c);
-    float m_used = -INFINITY;   // running max in log2 units (raw score * c) that P and l are expressed against
+    float m_used = -INFINITY;   // reference (log2 units, raw score * c) that P and l are expressed against
     float l = 0.f;
+    float tile_prev = 0.f;      // this thread's partial row sum of the previous key tile
+    float tile_worst = 0.f;     // largest partial tile sum of this pass (panic test)
     const uint32_t s_addr = s_base + h * SK;
+    auto rescale_o = [&](float f) {   // O_t *= f (leader only; O_t quiescent: S(j) complete and issued behind every PV)
+#pragma unroll 1
+      for (int cc = 0; cc < 8; ++cc) {
+        uint32_t o[16];
+        tmem_ld16(o_addr + cc * 16, o);
+        tmem_ld_wait();
+#pragma unroll
+        for (int e = 0; e < 16; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * f);
+        tmem_st16(o_addr + cc * 16, o);
+      }
+      tmem_st_wait();
+    };
     for (int j = 0; j < n_tiles; ++j) {
-      const uint32_t par = (uint32_t)j & 1u;
+      const uint32_t par = (uint32_t)(gb + j) & 1u;
       uint32_t s0[32], s1[32];                     // the thread's 64 scores of its sub-tile
       const int valid = kv_len - j * TK - h * SK;  // keys of this sub-tile that exist (warp-uniform; <= 0: none)
+      if (!exact && j > 0) {
+        // ---------------------------------------- optimistic tile
+        m_sh[(par * 2 + h) * 128 + r_in] = tile_prev;
+        asm volatile("bar.sync %0, 64;" ::"r"(bar_id) : "memory");
+        const float tot = tile_prev + m_sh[(par * 2 + (h ^ 1)) * 128 + r_in];   // same value in both threads of the row
+        const bool need = tot > 1073741824.0f;     // 2^30
+        if (valid > 0) {
+          mbar_wait(s_full(t, h), par);
+          tc_fence_after();
+          tmem_ld32(s_addr + 0, s0);
+        }
+        if (__any_sync(0xffffffffu, need)) {       // rare: move the reference up by floor(log2 tot)
+          if (valid <= 0) { mbar_wait(s_full(t, 0), par); tc_fence_after(); }
+          const float e = need ? (float)(((__float_as_int(tot) >> 23) & 0xff) - 127) : 0.f;
+          const float f = ex2(-e);
+          if (h == 0) rescale_o(f);
+          l *= f;
+          m_used += e;
+        }
+        if (valid <= 0) { tile_prev = 0.f; continue; }   // ragged last tile without a sub-tile b (warp-uniform)
+        const uint64_t nm2 = pack2(-m_used, -m_used);
+        uint64_t sum2 = pack2(0.f, 0.f), sum2b = pack2(0.f, 0.f);
+        tmem_ld_wait();
+        tmem_ld32(s_addr + 32, s1);
+        if (valid < SK) mask32(s0, valid);         // -inf -> P = 0
+        exp_pack_store(s0, c2, nm2, s_addr + 0, sum2, sum2b);
+        tmem_ld_wait();
+        if (valid < SK) mask32(s1, valid - 32);
+        exp_pack_store(s1, c2, nm2, s_addr + 16, sum2, sum2b);
+        float sa, sb;
+        unpack2(add2(sum2, sum2b), sa, sb);
+        tile_prev = sa + sb;
+        tile_worst = fmaxf(tile_worst, tile_prev);
+        l += tile_prev;
+        tmem_st_wait();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(p_full(t, h));
+        continue;
+      }
+      // ------------------------------------------ exact tile
       float mx = -INFINITY;
       if (valid > 0) {
         mbar_wait(s_full(t, h), par);
@@ -412,23 +508,12 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
           // quiescent; PV_a(j) cannot be queued before the leader delivers P_a, and PV_b(j) is queued after PV_a(j),
           // so the leader alone rescales O_t; both threads rescale their partial row sums.
           const float f = need ? ex2(m_used - m_new) : 1.0f;
-          if (h == 0) {
-#pragma unroll 1
-            for (int cc = 0; cc < 8; ++cc) {
-              uint32_t o[16];
-              tmem_ld16(o_addr + cc * 16, o);
-              tmem_ld_wait();
-#pragma unroll
-              for (int e = 0; e < 16; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * f);
-              tmem_st16(o_addr + cc * 16, o);
-            }
-            tmem_st_wait();
-          }
+          if (h == 0) rescale_o(f);
           l *= f;
           if (need) m_used = m_new;
         }
       }
-      if (valid <= 0) continue;                    // ragged last tile without a sub-tile b (warp-uniform)
+      if (valid <= 0) { tile_prev = 0.f; continue; }   // ragged last tile without a sub-tile b (warp-uniform)
       // P = 2^(s c - m_used): one packed FFMA per pair, EX2 (MUFU or FMA pipe), row sum in fp32, bf16 pairs -> TMEM
       const uint64_t nm2 = pack2(-m_used, -m_used);
       uint64_t sum2 = pack2(0.f, 0.f), sum2b = pack2(0.f, 0.f);
@@ -439,20 +524,28 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
       exp_pack_store(s1, c2, nm2, s_addr + 16, sum2, sum2b);
       float sa, sb;
       unpack2(add2(sum2, sum2b), sa, sb);
-      l += sa + sb;
+      tile_prev = sa + sb;
+      l += tile_prev;
       tmem_st_wait();
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(p_full(t, h));
     }
+    if (!exact && __any_sync(0xffffffffu, !(tile_worst < 1.152921504606847e18f)) && lane == 0)   // 2^60, inf
+      asm volatile("st.shared.u32 [%0], %1;" ::"r"(panic_addr), "r"(1u) : "memory");
     // ---- epilogue: the pair exchanges its partial row sums; leader writes columns 0..63, follower 64..127
-    // (its own barrier id, one per Q tile, 256 threads: the pair barrier may still hold the leader's last arrive)
+    // (its own barrier id, one per Q tile, 256 threads: the pair barrier may still hold the leader's last arrive).
+    // After an optimistic pass it runs before the CTA knows whether the pass stands: pass 1 overwrites the output.
     l_sh[h * 128 + r_in] = l;
     asm volatile("bar.sync %0, 256;" ::"r"(9 + t) : "memory");
     l = l_sh[r_in] + l_sh[128 + r_in];
-    mbar_wait(pv_done(t, (n_sub - 1) & 1), (uint32_t)((n_sub - 1) >> 1) & 1u);
+    {
+      const int lb = (n_sub - 1) & 1;              // barrier of the last PV; completions so far, all passes
+      const int done = (pass + 1) * (lb == 0 ? n_tiles : cnt_b1);
+      mbar_wait(pv_done(t, lb), (uint32_t)(done - 1) & 1u);
+    }
     tc_fence_after();
-    const float inv = 1.0f / l;                    // l >= 2^-8 > 0: every tile has at least one valid key
+    const float inv = 1.0f / l;                    // l > 0: every tile has at least one valid key
     const bool row_ok = row < q_hi;
     bf16* orow = p.o + (int64_t)(row_ok ? row : q_lo) * p.o_stride + head * HD + h * 64;
 #pragma unroll 1
@@ -471,6 +564,8 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
       }
     }
     if (h == 0 && row_ok && p.lse != nullptr) p.lse[(int64_t)row * p.H + head] = 0.6931471805599453f * (m_used + log2f(l));
+    if (exact || !repeat_exact()) break;
+  }
   }
   tc_fence_before();
   __syncthreads();

@@ -269,6 +269,27 @@ def test_attn_growing_row_maxima_force_rescale(lib, dtype, nq, nk):
     assert float((lse.double().cpu() - rl).abs().max()) < (1e-4 if dtype == torch.float32 else 5e-2)
 
 
+@pytest.mark.parametrize("nq,nk,jump_at", [(300, 1000, 700), (130, 300, 140), (512, 8192, 5000)])
+def test_attn_score_jump_repeats_the_pass_exactly(lib, nq, nk, jump_at):
+    """One key far down the sequence is 12 x a query row: that row's score jumps ~190 log2 units above everything seen
+    before, inside one key tile.  The optimistic pass of the tensor-core kernel (no row max after the first key tile,
+    DESIGN.md R33) overflows there, raises the CTA's panic flag and the CTA (for n_k >= 8192: the CTA pair) repeats the
+    keys with the exact per-tile row max; rows of other CTAs keep their optimistic result.  Both must match the oracle."""
+    H, d = 2, 128
+    q, k, v = synth.make_attention_qkv(11, nq, nk, H, d, dtype=torch.bfloat16, device=DEV)
+    k[jump_at] = (12.0 * q[5].float()).to(torch.bfloat16)
+    o, lse = B.dit_attn_partial(q, k, v)
+    torch.cuda.synchronize()
+    assert torch.isfinite(o.float()).all() and torch.isfinite(lse).all()
+    ro, rl = O.attention(q.cpu(), k.cpu(), v.cpu())
+    # row 5 returns v[jump_at] itself (|v| up to ~4 against RMS(o) ~ 0.1): its bf16 output rounding alone exceeds the
+    # max-abs / RMS bar, so the element-wise rounding bound is used next to the rel-L2 bar
+    assert errors(o, ro)[0] <= 4e-3
+    check_rounding(o, ro, f"score jump {nq}x{nk}", ulps=1.0, atol_rms=2.5e-2)
+    assert float((lse.double().cpu() - rl).abs().max()) < 5e-2
+    assert float((o[5].float().cpu() - v[jump_at].float().cpu()).abs().max()) < 2e-2       # row 5 sees only that key
+
+
 def test_attn_cta_pair_multicast_path(lib):
     """n_k >= 8192 and an even number of 256-row query blocks: the kernel runs as CTA pairs that share every K / V
     tile by TMA multicast.  Sampled query rows (both CTAs of a pair, ragged last key tile) against the oracle, and
