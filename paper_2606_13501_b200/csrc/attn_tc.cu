@@ -53,6 +53,10 @@ constexpr float RESCALE_THRESHOLD = 8.0f;  // log2 units
 #ifndef DIT_ATTN_OPTIMISTIC
 #define DIT_ATTN_OPTIMISTIC 1
 #endif
+#ifndef DIT_ATTN_OPT_PERIOD
+#define DIT_ATTN_OPT_PERIOD 4
+#endif
+constexpr int OPT_PERIOD = DIT_ATTN_OPT_PERIOD;   // optimistic tiles between two looks at the row sums (power of 2)
 constexpr bool OPTIMISTIC = DIT_ATTN_OPTIMISTIC != 0;   // 0: every key tile takes the exact path (row max per tile)
 constexpr int POLY_PAIRS = DIT_ATTN_POLY_PAIRS;   // of every 16 score pairs, this many take the FMA-pipe exp2
 
@@ -419,7 +423,8 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     const uint64_t c2 = pack2(c, c);
     float m_used = -INFINITY;   // reference (log2 units, raw score * c) that P and l are expressed against
     float l = 0.f;
-    float tile_prev = 0.f;      // this thread's partial row sum of the previous key tile
+    float tile_prev = 0.f;      // this thread's largest partial tile sum since the pair last looked
+    uint32_t xs = 0;            // exchange slot: consecutive exchanges of a pair alternate between two buffers
     float tile_worst = 0.f;     // largest partial tile sum of this pass (panic test)
     const uint32_t s_addr = s_base + h * SK;
     auto rescale_o = [&](float f) {   // O_t *= f (leader only; O_t quiescent: S(j) complete and issued behind every PV)
@@ -440,9 +445,14 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
       const int valid = kv_len - j * TK - h * SK;  // keys of this sub-tile that exist (warp-uniform; <= 0: none)
       if (!exact && j > 0) {
         // ---------------------------------------- optimistic tile
-        m_sh[(par * 2 + h) * 128 + r_in] = tile_prev;
-        asm volatile("bar.sync %0, 64;" ::"r"(bar_id) : "memory");
-        const float tot = tile_prev + m_sh[(par * 2 + (h ^ 1)) * 128 + r_in];   // same value in both threads of the row
+        float tot = 0.f;
+        if ((j & (OPT_PERIOD - 1)) == 0) {         // every OPT_PERIOD-th tile: largest partial sum since the last look
+          m_sh[(xs * 2 + h) * 128 + r_in] = tile_prev;
+          asm volatile("bar.sync %0, 64;" ::"r"(bar_id) : "memory");
+          tot = tile_prev + m_sh[(xs * 2 + (h ^ 1)) * 128 + r_in];   // same value in both threads of the row
+          xs ^= 1u;
+          tile_prev = 0.f;
+        }
         const bool need = tot > 1073741824.0f;     // 2^30
         if (valid > 0) {
           mbar_wait(s_full(t, h), par);
@@ -469,9 +479,9 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
         exp_pack_store(s1, c2, nm2, s_addr + 16, sum2, sum2b);
         float sa, sb;
         unpack2(add2(sum2, sum2b), sa, sb);
-        tile_prev = sa + sb;
-        tile_worst = fmaxf(tile_worst, tile_prev);
-        l += tile_prev;
+        tile_prev = fmaxf(tile_prev, sa + sb);
+        tile_worst = fmaxf(tile_worst, sa + sb);
+        l += sa + sb;
         tmem_st_wait();
         tc_fence_before();
         __syncwarp();
@@ -495,9 +505,10 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
         mx = fmaxf(max32(s0), max32(s1));
       }
       // the pair exchanges its half-row maxima: both threads then take the SAME rescale decision
-      m_sh[(par * 2 + h) * 128 + r_in] = mx;
+      m_sh[(xs * 2 + h) * 128 + r_in] = mx;
       asm volatile("bar.sync %0, 64;" ::"r"(bar_id) : "memory");
-      mx = fmaxf(mx, m_sh[(par * 2 + (h ^ 1)) * 128 + r_in]);
+      mx = fmaxf(mx, m_sh[(xs * 2 + (h ^ 1)) * 128 + r_in]);
+      xs ^= 1u;
       const float m_new = fmaxf(m_used, mx * c);   // c > 0
       if (j == 0) {
         m_used = m_new;                            // PV_0 overwrites O: nothing to rescale
