@@ -612,10 +612,12 @@ dit_status dit_sample(dit_handle h, const void* latents, const float* timestep_e
   memcpy(&gbits, &guidance_scale, 4);
   key.push_back(gbits);
   for (int i = 0; i <= n_steps; ++i) { uint32_t b; memcpy(&b, &sigmas_host[i], 4); key.push_back(b); }
+  // host -> device geometry copies and the RoPE table are not part of the graph: they are enqueued here, ahead of the
+  // capture or the replay, whenever another call has left a different geometry on the device (else a no-op)
+  s = upload_geom(h, gc, st);
+  if (s != DIT_OK) return s;
   if (h->graph_exec == nullptr || key != h->graph_key) {
     if (h->graph_exec) { cudaGraphExecDestroy(h->graph_exec); h->graph_exec = nullptr; }
-    s = upload_geom(h, gc, st);   // host -> device geometry copies and the RoPE table are enqueued outside the capture
-    if (s != DIT_OK) return s;
     if (h->cap_stream == nullptr) DIT_CUDA_OK(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
     DIT_CUDA_OK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeRelaxed));
     s = enqueue(h->cap_stream);

@@ -81,6 +81,13 @@ def test_graph_replay_is_bit_identical_and_recaptures_on_change(lib):
     want = m.dit_sample(lat, tembs, sig2, cond, unc, g, use_graph=False)
     torch.cuda.synchronize()
     assert torch.equal(out_g, want) and not torch.equal(out_g, out_e)
+    # another call with a different latent grid in between leaves its geometry (cu_seqlens, RoPE table) on the device:
+    # the replay must restore its own
+    small = lat[:, :, :16, :16].contiguous()
+    m.dit_step(small, tembs[0], cond)
+    m.dit_sample(lat, tembs, sig2, cond, unc, g, use_graph=True, out=out_g)
+    torch.cuda.synchronize()
+    assert torch.equal(out_g, want)
     # the plain step still works after a trajectory (geometry cache, workspace) and matches a fresh run
     v = m.dit_step(lat, tembs[0], cond)
     v2 = B.Dit(B.make_config(s), synth.make_weights(s), DEV).dit_step(lat, tembs[0], cond)
