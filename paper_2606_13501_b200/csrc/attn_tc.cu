@@ -21,12 +21,18 @@
 //               MUFU.EX2 (16 / clk / SM: as many cycles as the tile's MMAs).  O is rescaled lazily: only when the
 //               running max grows by more than 2^8 (exact: the same max is used for P and for the sum, and divided
 //               out at the end); the leader rescales O_t, both threads rescale their partial row sums;
+//               That is the EXACT tile.  Pass 0 of a CTA is optimistic (R33): only its first key tile is exact;
+//               the others compute no row max (any reference is exact while nothing overflows), the pair only looks at
+//               its recent row sums every 4th tile — before it waits for S, off the S -> P -> PV chain — and moves the
+//               reference when they have grown by 2^30.  A tile sum above 2^60 raises the CTA's panic flag and the
+//               CTA (CTA pair) repeats all key tiles as pass 1 with exact tiles only;
 //   epilogue    the pair adds its partial sums; leader writes O columns 0..63, follower 64..127: O / l -> bf16,
 //               lse = ln2 * (m + log2 l).
 // TMEM: S0a S0b | S1a S1b | O0 | O1 = 4 x 128 fp32 columns = all 512; P_t,b aliases the first 32 columns of S_t,b.
 // Registers: 640 threads x 96 at launch; setmaxnreg moves the control warps to 40 and the softmax warps to 104
 // (the pool is the CTA's launch allocation: asking for more than the control warps release never returns).
-// Roofline: tensor pipe; the softmax instruction stream (~4.5 issue slots per score) is co-critical.
+// Roofline: tensor pipe; the softmax instruction stream (312 instructions per 64 scores in an optimistic tile, 379 in
+// an exact one; MUFU.EX2 at 16 / clk / SM) is co-critical.
 #include <algorithm>
 
 #include "tc.cuh"
