@@ -54,6 +54,13 @@ def test_workspace_bytes_and_validation_without_gpu(lib):
     h = C.c_void_p()
     st = lib.dit_init(C.byref(binding.make_config(synth.cfg1())), None, 0, None, 0, C.byref(h))
     assert st == -3 and b"workspace" in lib.dit_last_error(None)
+    # every step / trajectory entry point rejects a NULL handle before touching the device
+    grid = (C.c_int32 * 3)(1, 8, 8)
+    sig = (C.c_float * 2)(1.0, 0.0)
+    assert lib.dit_step(None, None, None, None, 0, grid, None, None) == -1
+    assert lib.dit_step_host(None, None, None, None, 0, grid, None, None) == -1
+    assert lib.dit_sample(None, None, None, sig, None, 0, None, 0, 1.0, grid, 1, 0, None, None) == -1
+    assert b"handle" in lib.dit_last_error(None)
     assert lib.dit_kernel_launches() == 0
 
 
