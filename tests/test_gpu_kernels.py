@@ -288,6 +288,15 @@ def test_attn_score_jump_repeats_the_pass_exactly(lib, nq, nk, jump_at):
     check_rounding(o, ro, f"score jump {nq}x{nk}", ulps=1.0, atol_rms=2.5e-2)
     assert float((lse.double().cpu() - rl).abs().max()) < 5e-2
     assert float((o[5].float().cpu() - v[jump_at].float().cpu()).abs().max()) < 2e-2       # row 5 sees only that key
+    # the repeated pass is deterministic, and the split-KV form (the jump sits in one of P = 2 shards; the other shard's
+    # partial keeps its optimistic result) merges to the same answer
+    o2, lse2 = B.dit_attn_partial(q, k, v)
+    assert torch.equal(o, o2) and torch.equal(lse, lse2)
+    half = (nk + 1) // 2
+    parts = [B.dit_attn_partial(q, k[a:b], v[a:b]) for a, b in ((0, half), (half, nk))]
+    om, lm = B.dit_attn_merge([x[0] for x in parts], [x[1] for x in parts])
+    torch.cuda.synchronize()
+    assert errors(om, ro)[0] <= 5e-3 and float((lm.double().cpu() - rl).abs().max()) < 5e-2
 
 
 def test_attn_cta_pair_multicast_path(lib):
