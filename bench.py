@@ -379,7 +379,8 @@ def run_traj(args):
     """`--workload traj`: one request of cfg 2 shape through `dit_sample` (n denoising steps chained by the Euler
     update on the device, no host round trip between steps).  Reports denoising steps/s of the trajectory when its
     kernels are launched one by one on the stream and when the captured CUDA graph is replayed with one launch, plus a
-    classifier-free-guided trajectory (two passes per step).  `--steps` = trajectories timed, `--traj-steps` = n."""
+    classifier-free-guided trajectory as two passes per step and as ONE packed pass of two requests per step (a handle with
+    room for both).  `--steps` = trajectories timed, `--traj-steps` = n."""
     from paper_2606_13501_b200 import binding as B
     B.load()
     if not torch.cuda.is_available():
@@ -389,7 +390,9 @@ def run_traj(args):
     s = _shape("cfg2")
     n = args.traj_steps
     W = synth.make_weights(s, device=dev)
-    m = B.Dit(B.make_config(s, split_p=args.split_p), W, dev)
+    m1 = B.Dit(B.make_config(s, split_p=args.split_p), W, dev)
+    m2 = B.Dit(B.make_config(s, split_p=args.split_p, max_requests=2, max_tokens=2 * (s.n_tokens + s.n_cond),
+                             max_cond_tokens=2 * s.n_cond), W, dev)
     I = synth.make_inputs(s, device=dev)
     lat, cond = I["latents"], I["cond"]
     unc = synth.normal(s.seed, "uncond", tuple(cond.shape), dtype=s.torch_dtype, device=dev)
@@ -398,8 +401,9 @@ def run_traj(args):
     out = torch.empty_like(lat)
     K, Wm = max(1, min(args.steps, 10)), max(1, min(args.warmup, 3))
     rows = []
-    for name, u, graph in (("stream launches", None, False), ("cuda graph", None, True),
-                           ("guided (2 passes/step), cuda graph", unc, True)):
+    for name, m, u, graph in (("stream launches", m1, None, False), ("cuda graph", m1, None, True),
+                              ("guided (2 passes/step), cuda graph", m1, unc, True),
+                              ("guided (1 packed pass of 2 requests/step), cuda graph", m2, unc, True)):
         for _ in range(Wm):
             m.dit_sample(lat, tembs, sigmas, cond, u, 4.0, use_graph=graph, out=out)
         torch.cuda.synchronize()

@@ -116,7 +116,7 @@ dit_status dit_step(dit_handle h, const void* latents, const float* timestep_emb
  *     x_0 = latents;   for i = 0 .. n_steps-1:
  *         v_c = dit_step(x_i, timestep_embs[i], cond_tokens)
  *         v   = uncond_tokens ? v_u + guidance_scale * (v_c - v_u),  v_u = dit_step(x_i, timestep_embs[i], uncond_tokens)
- *                             : v_c                                   (classifier-free guidance, two passes per step)
+ *                             : v_c                                   (classifier-free guidance)
  *         x_{i+1} = x_i + (sigmas[i+1] - sigmas[i]) * v               (flow-matching Euler update)
  *     out = x_{n_steps}
  *   latents       dev, [C, F, H, W] config dtype            out  dev, same shape and dtype (may not alias latents)
@@ -124,6 +124,9 @@ dit_status dit_step(dit_handle h, const void* latents, const float* timestep_emb
  *   cond_tokens / uncond_tokens  dev, [n_cond | n_uncond, cond_dim] config dtype; uncond_tokens NULL = no guidance
  * The state x_i is carried in fp32 inside the workspace; every step reads x_i rounded to the config dtype (it is staged
  * in `out`) and v is the fp32 result of the final Linear — the update is fused into the unpatchify kernel.
+ * Guidance runs as ONE packed pass of two requests per step (unconditional + conditional over the same x_i, the varlen
+ * path of dit_step_varlen: every weight is streamed once) when the handle has room for both — max_requests >= 2, both
+ * sequences within max_tokens, n_cond + n_uncond <= max_cond_tokens — and as two passes per step otherwise.
  * use_graph != 0: the whole trajectory is captured once into a CUDA graph (cached in the handle, keyed by every
  * argument) and replayed with one launch; identical results.  n_steps == 0 copies latents to out. */
 dit_status dit_sample(dit_handle h, const void* latents, const float* timestep_embs, const float* sigmas_host,

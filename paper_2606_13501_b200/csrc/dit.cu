@@ -254,8 +254,12 @@ static dit_status upload_geom(dit_handle hd, const StepGeom& g, cudaStream_t st)
   return DIT_OK;
 }
 
+// `pair` (dit_sample, guided step as ONE packed pass): the R = 2 requests are the unconditional and the conditional pass
+// of the same latents at the same timestep — one t-MLP / modulation row serves both (row stride 0), each request has its
+// own cond pointer and its own unpatchify epilogue.
+struct GuidedPair { const void* cond[2]; const SampleEpi* epi[2]; };
 static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents, const float* temb, const void* cond,
-                           void* out, cudaStream_t st, const SampleEpi* epi = nullptr) {
+                           void* out, cudaStream_t st, const SampleEpi* epi = nullptr, const GuidedPair* pair = nullptr) {
   const dit_config& c = hd->cfg;
   Workspace& w = hd->ws;
   const int dt = c.dtype;
@@ -263,7 +267,12 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
   const int D = c.hidden, F = c.mlp_dim, H = c.n_heads, d = c.head_dim, L = c.n_blocks, R = g.R;
   const int pvC = c.latent_channels * c.patch[0] * c.patch[1] * c.patch[2];
   const int T = g.cu[R];
-  const int64_t mod_stride = (int64_t)L * 6 * D + 2 * D;
+  const int64_t mod_len = (int64_t)L * 6 * D + 2 * D;
+  const int Rt = pair ? 1 : R;                      // timestep rows
+  const int64_t mod_stride = pair ? 0 : mod_len;    // modulation row of request r = mod + r * mod_stride
+  auto cond_of = [&](int r) -> const char* {
+    return pair ? (const char*)pair->cond[r] : (const char*)cond + (size_t)g.cu_cond[r] * c.cond_dim * esize(c.dtype);
+  };
   const bool joint = c.cond_mode == DIT_COND_JOINT, cross = c.cond_mode == DIT_COND_CROSS;
   const bool rope = (c.rope_dims[0] + c.rope_dims[1] + c.rope_dims[2]) > 0;
   auto stop = [&](int blk, int stage) { return hd->stop_block == blk && hd->stop_stage == stage; };
@@ -280,9 +289,9 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
   } while (0)
 
   // ---- steps 1-2: c = W2 SiLU(W1 temb + b1) + b2;  mod = Wmod SiLU(c) + bmod for ALL blocks in one launch
-  RUN(launch_gemv(dt, temb, w.gemv_tab + 0, nullptr, 1, D, w.c1, D, R, c.temb_dim, 0, st));
-  RUN(launch_gemv(dt, w.c1, w.gemv_tab + 1, nullptr, 1, D, w.c, D, R, D, 1, st));
-  RUN(launch_gemv(dt, w.c, w.gemv_tab + 2, nullptr, L + 1, L * 6 * D + 2 * D, w.mod, mod_stride, R, D, 1, st));
+  RUN(launch_gemv(dt, temb, w.gemv_tab + 0, nullptr, 1, D, w.c1, D, Rt, c.temb_dim, 0, st));
+  RUN(launch_gemv(dt, w.c1, w.gemv_tab + 1, nullptr, 1, D, w.c, D, Rt, D, 1, st));
+  RUN(launch_gemv(dt, w.c, w.gemv_tab + 2, nullptr, L + 1, L * 6 * D + 2 * D, w.mod, mod_len, Rt, D, 1, st));
 
   // ---- steps 3-4: patch-embed and cond projection write the fp32 residual stream
   for (int r = 0; r < R; ++r) {
@@ -294,12 +303,20 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
     RUN(launch_patchify(dt, (const char*)latents + g.lat_off[r] * es, pr, c.latent_channels, Fr, Hr, Wr, c.patch, st));
     RUN(gemm(dt, DIT_EPI_BIAS_F32, pr, pvC, hd->pe_w, hd->pe_b, w.x + (size_t)row0 * D, D, Nr, D, pvC, st, DIT_KC_MISC));
     if (joint && Lc > 0)
-      RUN(gemm(dt, DIT_EPI_BIAS_F32, (const char*)cond + (size_t)g.cu_cond[r] * c.cond_dim * es, c.cond_dim, hd->cp_w,
-               hd->cp_b, w.x + (size_t)g.cu[r] * D, D, Lc, D, c.cond_dim, st, DIT_KC_MISC));
+      RUN(gemm(dt, DIT_EPI_BIAS_F32, cond_of(r), c.cond_dim, hd->cp_w, hd->cp_b, w.x + (size_t)g.cu[r] * D, D, Lc, D,
+               c.cond_dim, st, DIT_KC_MISC));
   }
   const int Lc_total = g.cu_cond[R];
-  if (cross && Lc_total > 0)
-    RUN(gemm(dt, DIT_EPI_BIAS, cond, c.cond_dim, hd->cp_w, hd->cp_b, w.ctx, D, Lc_total, D, c.cond_dim, st, DIT_KC_MISC));
+  if (cross && Lc_total > 0) {
+    if (!pair) {
+      RUN(gemm(dt, DIT_EPI_BIAS, cond, c.cond_dim, hd->cp_w, hd->cp_b, w.ctx, D, Lc_total, D, c.cond_dim, st, DIT_KC_MISC));
+    } else {
+      for (int r = 0; r < R; ++r)
+        if (g.ncond[r] > 0)
+          RUN(gemm(dt, DIT_EPI_BIAS, cond_of(r), c.cond_dim, hd->cp_w, hd->cp_b, (char*)w.ctx + (size_t)g.cu_cond[r] * D * es, D,
+                   g.ncond[r], D, c.cond_dim, st, DIT_KC_MISC));
+    }
+  }
 
   // ---- step 5: blocks.  Both residual branches are added to x inside their GEMM epilogues (gemm_residual).
   const float scale = 1.0f / sqrtf((float)d);
@@ -382,7 +399,8 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
     const int row0 = g.cu[r] + (joint ? g.ncond[r] : 0);
     float* tk = w.tok + (size_t)row0 * pvC;
     RUN(gemm(dt, DIT_EPI_BIAS_F32, (char*)w.y + (size_t)row0 * D * es, D, hd->f_w, hd->f_b, tk, pvC, Nr, pvC, D, st, DIT_KC_MISC));
-    RUN(launch_unpatchify(dt, tk, (char*)out + g.lat_off[r] * es, c.latent_channels, Fr, Hr, Wr, c.patch, st, epi));
+    RUN(launch_unpatchify(dt, tk, (char*)out + g.lat_off[r] * es, c.latent_channels, Fr, Hr, Wr, c.patch, st,
+                          pair ? pair->epi[r] : epi));
   }
 #undef RUN
   return DIT_OK;
@@ -581,9 +599,23 @@ dit_status dit_sample(dit_handle h, const void* latents, const float* timestep_e
   }
   const int64_t n = gc.lat_off[1];
   Workspace& w = h->ws;
+  // Guided step as ONE packed pass (R = 2: the unconditional and the conditional request over the same latents, varlen
+  // path) when the handle's capacities allow it — max_requests >= 2, both sequences within max_tokens, both cond sets
+  // within max_cond_tokens; else two passes per step.  Every weight is then streamed once per step instead of twice.
+  StepGeom g2;
+  bool packed = false;
+  if (guided && c.max_requests >= 2 && (int64_t)gu.cu[1] + gc.cu[1] <= c.max_tokens &&
+      (int64_t)gu.cu_cond[1] + gc.cu_cond[1] <= c.max_cond_tokens) {
+    const int32_t nc2[2] = {n_uncond, n_cond};
+    const int32_t grid2[6] = {latent_grid[0], latent_grid[1], latent_grid[2], latent_grid[0], latent_grid[1], latent_grid[2]};
+    s = build_geom(h, 2, nullptr, nc2, grid2, &g2);
+    if (s != DIT_OK) return s;
+    g2.lat_off.assign(3, 0);   // both requests read the same latents; the conditional one writes `out`
+    packed = true;
+  }
   // cond and uncond token counts may differ: in joint mode that changes the sequence geometry (rows, RoPE table), which is
   // uploaded outside a capture; a guided trajectory with n_cond != n_uncond in joint mode therefore runs without a graph
-  const bool same_geom = !guided || gu.cu == gc.cu;
+  const bool same_geom = !guided || packed || gu.cu == gc.cu;
   auto enqueue = [&](cudaStream_t st) -> dit_status {
     dit_status e = launch_sample_init(c.dtype, latents, w.sample_x, n, st);
     if (e != DIT_OK) return e;
@@ -591,6 +623,14 @@ dit_status dit_sample(dit_handle h, const void* latents, const float* timestep_e
       const void* x_in = i == 0 ? latents : out;   // x_i rounded to the config dtype was staged in `out` by step i - 1
       const float* temb = timestep_embs + (size_t)i * c.temb_dim;
       SampleEpi epi{2, w.sample_x, nullptr, sigmas_host[i + 1] - sigmas_host[i], guidance_scale};
+      if (packed) {
+        SampleEpi hold{1, nullptr, w.sample_v, 0.f, 0.f};
+        epi.v_hold = w.sample_v;
+        GuidedPair gp{{uncond_tokens, cond_tokens}, {&hold, &epi}};
+        e = run_step(h, g2, x_in, temb, nullptr, out, st, nullptr, &gp);
+        if (e != DIT_OK) return e;
+        continue;
+      }
       if (guided) {
         SampleEpi hold{1, nullptr, w.sample_v, 0.f, 0.f};
         e = run_step(h, gu, x_in, temb, uncond_tokens, out, st, &hold);
@@ -614,7 +654,7 @@ dit_status dit_sample(dit_handle h, const void* latents, const float* timestep_e
   for (int i = 0; i <= n_steps; ++i) { uint32_t b; memcpy(&b, &sigmas_host[i], 4); key.push_back(b); }
   // host -> device geometry copies and the RoPE table are not part of the graph: they are enqueued here, ahead of the
   // capture or the replay, whenever another call has left a different geometry on the device (else a no-op)
-  s = upload_geom(h, gc, st);
+  s = upload_geom(h, packed ? g2 : gc, st);
   if (s != DIT_OK) return s;
   if (h->graph_exec == nullptr || key != h->graph_key) {
     if (h->graph_exec) { cudaGraphExecDestroy(h->graph_exec); h->graph_exec = nullptr; }

@@ -23,11 +23,17 @@ def _traj(s, n_steps, n_unc=None):
     return I, tembs, sigmas, unc
 
 
-def _both(s, n_steps, n_unc=None, g=1.0, use_graph=False, split_p=1):
+def _packed_caps(s, n_unc):
+    """Handle capacities that let dit_sample run a guided step as ONE packed pass of two requests (include/dit.h)."""
+    joint = s.cond_mode == "joint"
+    return dict(max_requests=2, max_tokens=2 * s.n_tokens + (s.n_cond + n_unc if joint else 0), max_cond_tokens=s.n_cond + n_unc)
+
+
+def _both(s, n_steps, n_unc=None, g=1.0, use_graph=False, split_p=1, packed=False):
     W = synth.make_weights(s)
     I, tembs, sigmas, unc = _traj(s, n_steps, n_unc)
     ref = O.dit_sample(O.cfg_from_shape(s), W, I["latents"], tembs, sigmas, I["cond"], unc, g)
-    m = B.Dit(B.make_config(s, split_p=split_p), W, DEV)
+    m = B.Dit(B.make_config(s, split_p=split_p, **(_packed_caps(s, n_unc) if packed else {})), W, DEV)
     dev = lambda t: None if t is None else t.to(DEV)
     args = (dev(I["latents"]), dev(tembs), sigmas, dev(I["cond"]), dev(unc), g)
     out = m.dit_sample(*args, use_graph=use_graph)
@@ -49,20 +55,37 @@ def test_cfg1_fp32_trajectory(lib, use_graph):
     _check_traj(out, ref, I, torch.float32, "cfg1 3 steps", 2e-5)
 
 
+@pytest.mark.parametrize("packed", [False, True])
 @pytest.mark.parametrize("mode,n_unc,use_graph", [("joint", 16, False), ("joint", 32, True), ("cross", 16, True)])
-def test_fp32_guided_trajectory(lib, mode, n_unc, use_graph):
-    """Joint mode with n_uncond != n_cond changes the sequence geometry between the two passes (no graph)."""
+def test_fp32_guided_trajectory(lib, mode, n_unc, use_graph, packed):
+    """Two passes per step: joint mode with n_uncond != n_cond changes the sequence geometry between the passes (no
+    graph).  packed: the handle has room for both requests, the step is ONE varlen pass of two requests."""
     s = synth.cfg1(cond_mode=mode, rope_dims=(0, 32, 32), qk_rmsnorm=True)
-    out, ref, *_, I = _both(s, 2, n_unc=n_unc, g=4.0, use_graph=use_graph, split_p=2)
-    _check_traj(out, ref, I, torch.float32, f"cfg1 guided {mode}", 5e-5)
+    out, ref, *_, I = _both(s, 2, n_unc=n_unc, g=4.0, use_graph=use_graph or packed, split_p=2, packed=packed)
+    _check_traj(out, ref, I, torch.float32, f"cfg1 guided {mode} packed={packed}", 5e-5)
 
 
+@pytest.mark.parametrize("packed", [False, True])
 @pytest.mark.parametrize("use_graph", [False, True])
-def test_bf16_guided_trajectory(lib, use_graph):
+def test_bf16_guided_trajectory(lib, use_graph, packed):
     s = synth.cfg1(name="traj_bf16", dtype="bf16", hidden=512, n_heads=4, head_dim=128, mlp_dim=2048, cond_dim=512,
                    latent_channels=16, rope_dims=(0, 64, 64), qk_rmsnorm=True, n_blocks=3)
-    out, ref, *_, I = _both(s, 4, n_unc=32, g=3.0, use_graph=use_graph)
-    _check_traj(out, ref, I, torch.bfloat16, "bf16 guided 4 steps", 2e-2)
+    out, ref, *_, I = _both(s, 4, n_unc=32, g=3.0, use_graph=use_graph, packed=packed)
+    _check_traj(out, ref, I, torch.bfloat16, f"bf16 guided 4 steps packed={packed}", 2e-2)
+
+
+def test_packed_guidance_needs_room_for_both_requests(lib):
+    """One request short of room in max_tokens: the same call falls back to two passes per step and still matches."""
+    s = synth.cfg1(cond_mode="joint", rope_dims=(0, 32, 32), qk_rmsnorm=True)
+    W = synth.make_weights(s)
+    I, tembs, sigmas, unc = _traj(s, 2, 16)
+    ref = O.dit_sample(O.cfg_from_shape(s), W, I["latents"], tembs, sigmas, I["cond"], unc, 2.5)
+    caps = _packed_caps(s, 16)
+    caps["max_tokens"] -= 1
+    m = B.Dit(B.make_config(s, **caps), W, DEV)
+    out = m.dit_sample(I["latents"].to(DEV), tembs.to(DEV), sigmas, I["cond"].to(DEV), unc.to(DEV), 2.5, use_graph=False)
+    torch.cuda.synchronize()
+    _check_traj(out, ref, I, torch.float32, "guided, capacity one row short", 5e-5)
 
 
 def test_graph_replay_is_bit_identical_and_recaptures_on_change(lib):
