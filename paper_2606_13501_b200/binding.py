@@ -172,7 +172,9 @@ class Dit:
     def dit_sample(self, latents, tembs, sigmas, cond=None, uncond=None, guidance_scale=1.0, use_graph=False, out=None,
                    stream=None):
         """n_steps = tembs.shape[0] denoising steps chained by the Euler update; tembs [n_steps, temb_dim] fp32 (device),
-        sigmas: n_steps + 1 host floats; uncond given = classifier-free guidance (two passes per step)."""
+        sigmas: n_steps + 1 host floats; uncond given = classifier-free guidance (one packed pass of two requests per step when
+        the handle has room for both — make_config(max_requests=2, max_tokens=2T, max_cond_tokens=n_cond + n_uncond) — else
+        two passes per step)."""
         out = torch.empty_like(latents) if out is None else out
         n_steps = int(tembs.shape[0])
         assert len(sigmas) == n_steps + 1
