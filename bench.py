@@ -188,6 +188,9 @@ class OracleSample:
         return self.t0 + self.s.n_blocks * max(t1 - self.t0, 0.0)
 
 
+REF_BUDGET_S = 240.0
+
+
 def run_reference(args, rank: int):
     if rank != 0:
         return
@@ -196,13 +199,24 @@ def run_reference(args, rank: int):
     s = _shape(args.workload)
     torch.set_num_threads(os.cpu_count() or 1)
     smp = OracleSample(s)
-    for _ in range(args.warmup):
+    # K + W samples of ~3-10 s each; a wall-clock bound keeps a large --steps within a few minutes on any host: once
+    # REF_BUDGET_S are spent, no further sample is run and the line says how many were timed
+    t_start = time.perf_counter()
+    for i in range(args.warmup):
+        if i > 0 and time.perf_counter() - t_start > REF_BUDGET_S / 4:
+            break
         smp.step_seconds()
-    times = [smp.step_seconds() for _ in range(args.steps)]
+    times = []
+    for _ in range(args.steps):
+        if times and time.perf_counter() - t_start > REF_BUDGET_S:
+            break
+        times.append(smp.step_seconds())
     sec = sum(times) / len(times)
     val = 1.0 / sec
     cores = torch.get_num_threads()
-    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+    if len(times) < args.steps:
+        smp.sample += f"; {len(times)} of {args.steps} steps timed ({REF_BUDGET_S:.0f} s wall-clock bound)"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": len(times),
             "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic", "config": {"workload": _workload_name(s)},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": smp.sample},
