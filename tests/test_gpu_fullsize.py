@@ -129,3 +129,32 @@ def test_cfg5_full_size_attention_sampled_rows_and_split(lib, H, N):
         assert e_rel < 4e-3 and e_max < 6e-2, f"P={P}: rel {e_rel:.2e} max {e_max:.2e}"
         check(om[rows.to(DEV)], ro, torch.bfloat16, f"merged P={P} sampled rows")
         assert float((lm - lse).abs().max()) < 1e-3
+
+
+def test_cfg2_full_size_guided_step_packed_vs_two_passes(lib):
+    """configs[1] shape, one guided Euler step of dit_sample: on a handle with room for both requests the step runs as
+    ONE packed pass of two requests (include/dit.h), on a handle without it as two passes.  Both combine fp32 velocities
+    and round x_1 once, so they agree to a bf16 rounding flip here and there — the property that holds at any size (the
+    oracle checks both forms at small sizes).  A second, looser look against two plain dit_step calls, whose bf16-rounded
+    velocities the guidance scale amplifies."""
+    s = synth.cfg2()
+    W = synth.make_weights(s, device=DEV)
+    I = synth.make_inputs(s, device=DEV)
+    lat, temb, cond = I["latents"], I["temb"][0].contiguous(), I["cond"]
+    unc = synth.normal(s.seed, "uncond", (192, s.cond_dim), dtype=s.torch_dtype, device=DEV)   # n_uncond != n_cond
+    g, sig = 3.5, [1.0, 0.75]
+    m1 = B.Dit(B.make_config(s), W, DEV)
+    two = m1.dit_sample(lat, temb.reshape(1, -1), sig, cond, unc, g, use_graph=False)
+    v_c = m1.dit_step(lat, temb, cond).float()
+    v_u = m1.dit_step(lat, temb, unc).float()
+    loose = lat.float() + (sig[1] - sig[0]) * (v_u + g * (v_c - v_u))
+    T2 = 2 * s.n_tokens + s.n_cond + 192
+    m2 = B.Dit(B.make_config(s, max_requests=2, max_tokens=T2, max_cond_tokens=s.n_cond + 192), W, DEV)
+    for use_graph in (False, True):
+        got = m2.dit_sample(lat, temb.reshape(1, -1), sig, cond, unc, g, use_graph=use_graph)
+        torch.cuda.synchronize()
+        assert torch.isfinite(got.float()).all()
+        e_rel, e_max = errors(got.float() - lat.float(), two.float() - lat.float())
+        assert e_rel < 2e-3 and e_max < 3e-2, f"packed vs two passes (graph={use_graph}): rel {e_rel:.2e} max {e_max:.2e}"
+        l_rel, _ = errors(got.float() - lat.float(), loose - lat.float())
+        assert l_rel < 2e-2, f"packed vs two dit_step calls (graph={use_graph}): rel {l_rel:.2e}"
