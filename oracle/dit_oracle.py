@@ -20,10 +20,14 @@ softmax rows sum to 1; identical keys -> mean of V; zero gates -> identity (bit 
 invariance; merge closed forms; LN / RMSNorm / RoPE / GELU / patchify invariants; torch library routines
 (layer_norm, scaled_dot_product_attention, gelu(tanh), silu) as special cases; stored hand-computed
 fixtures under tests/golden/; the trajectory (`dit_sample`): constant-velocity closed form, guidance special cases,
-semigroup property.
+semigroup property; the block in all three modes re-derived with torch library routines and a by-hand RoPE
+(`test_block_by_hand_one_block`, `test_joint_block_by_hand_rmsnorm_then_rope`: [ctx ; x] order, cond position 0,
+RMSNorm BEFORE RoPE, interleaved pairs; `test_cross_block_by_hand`: wkv rows [k | v], ungated / unmodulated / un-roped
+cross branch, also for `block_rows` in cross mode).  Mutants of each of those lines fail the CPU suite.
 PARITY UNPINNED: the *composition order* of the block (R1, R9, R10, R12: which sub-layer follows which,
 single-stream joint attention, cross-attention placement, final layer) is a definition this repo makes
-— the paper prints nothing it could be checked against beyond the invariants above.
+— the paper prints nothing it could be checked against; the transcriptions above pin the oracle to DESIGN.md §3's
+sentences, not to the paper.
 """
 from __future__ import annotations
 

@@ -328,6 +328,147 @@ def test_block_by_hand_one_block():
     assert torch.allclose(taps["b0.x_mlp"], x, rtol=1e-10, atol=1e-12)
 
 
+def _hand_rope(t, pos, rope_dims, theta):
+    """Interleaved-pair RoPE written out element by element (R6), independent of O.rope_angles / O.apply_rope:
+    head dim cut into per-axis segments (f, h, w); pair j of a d_a-wide segment = elements (2j, 2j+1) of the segment,
+    angle pos_a * theta^(-2j/d_a); (a, b) -> (a cos - b sin, a sin + b cos).  t: [T, H, d]."""
+    out = t.clone()
+    T, H, d = t.shape
+    for n in range(T):
+        base = 0
+        for a, d_a in enumerate(rope_dims):
+            for j in range(d_a // 2):
+                th = float(pos[n][a]) * theta ** (-2.0 * j / d_a)
+                c, s_ = math.cos(th), math.sin(th)
+                e, o = t[n, :, base + 2 * j], t[n, :, base + 2 * j + 1]
+                out[n, :, base + 2 * j] = e * c - o * s_
+                out[n, :, base + 2 * j + 1] = e * s_ + o * c
+            base += d_a
+    return out
+
+
+def _wide_gains(W, s):
+    """QK-norm gains with std 0.3 (not the near-one gains of R14) so that norm-then-RoPE and RoPE-then-norm differ
+    by far more than rounding: a gain is per ELEMENT, RoPE mixes the two elements of a pair."""
+    for name in list(W):
+        if name.endswith(".gq") or name.endswith(".gk"):
+            W[name] = (1.0 + 0.3 * synth.normal(5, "wide:" + name, W[name].shape, dtype=F64)).to(W[name].dtype)
+    return W
+
+
+def test_joint_block_by_hand_rmsnorm_then_rope():
+    """One JOINT block with QK-RMSNorm and 2D RoPE, re-derived with torch library routines and a by-hand rotation:
+    sequence [ctx ; x] (R9), cond tokens at position 0 (R6), per-head RMSNorm FIRST, RoPE SECOND (R5), then SDPA.
+    Fails if the oracle rotates before normalising, swaps cos/sin, uses half-split instead of interleaved pairs,
+    puts ctx after x, or gives cond tokens a non-zero position."""
+    s = _tiny(n_blocks=1, cond_mode="joint", rope_dims=(0, 8, 8), qk_rmsnorm=True)
+    W, I = _wide_gains(synth.make_weights(s), s), synth.make_inputs(s)
+    taps = {}
+    O.dit_step(O.cfg_from_shape(s), W, I["latents"], I["temb"], I["cond"], taps=taps)
+    Fn = torch.nn.functional
+    Wd = {k: v.double() for k, v in W.items()}
+    D, H, d, Lc = 32, 2, 16, 5
+    c = Fn.linear(Fn.silu(Fn.linear(I["temb"].double(), Wd["t_mlp.w1"], Wd["t_mlp.b1"])), Wd["t_mlp.w2"], Wd["t_mlp.b2"])
+    m = Fn.linear(Fn.silu(c), Wd["blocks.0.mod.w"], Wd["blocks.0.mod.b"]).reshape(6, D)
+    lat = I["latents"].double()                                            # [2, 1, 8, 8], patch (1, 2, 2) -> 4 x 4 tokens
+    patches = torch.stack([lat[:, 0, 2 * hh:2 * hh + 2, 2 * ww:2 * ww + 2].reshape(-1) for hh in range(4) for ww in range(4)])
+    ximg = Fn.linear(patches, Wd["patch_embed.w"], Wd["patch_embed.b"])
+    ctx = Fn.linear(I["cond"].double(), Wd["cond_proj.w"], Wd["cond_proj.b"])
+    x = torch.cat([ctx, ximg], 0)
+    assert torch.allclose(taps["x0"], x, rtol=1e-12, atol=1e-14)
+    pos = [(0, 0, 0)] * Lc + [(0, hh, ww) for hh in range(4) for ww in range(4)]
+    y = Fn.layer_norm(x, (D,), eps=1e-6) * (1 + m[1]) + m[0]
+    qkv = Fn.linear(y, Wd["blocks.0.attn.wqkv"], Wd["blocks.0.attn.bqkv"])
+    q, k, v = [t.reshape(-1, H, d) for t in qkv.split(D, dim=1)]
+    q = Fn.rms_norm(q, (d,), weight=Wd["blocks.0.attn.gq"], eps=1e-6)
+    k = Fn.rms_norm(k, (d,), weight=Wd["blocks.0.attn.gk"], eps=1e-6)
+    q, k = _hand_rope(q, pos, (0, 8, 8), 10000.0), _hand_rope(k, pos, (0, 8, 8), 10000.0)
+    assert torch.allclose(taps["b0.q"], q.reshape(-1, D), rtol=1e-11, atol=1e-13)
+    assert torch.allclose(taps["b0.k"], k.reshape(-1, D), rtol=1e-11, atol=1e-13)
+    o = Fn.scaled_dot_product_attention(q.permute(1, 0, 2), k.permute(1, 0, 2), v.permute(1, 0, 2)).permute(1, 0, 2)
+    x = x + m[2] * Fn.linear(o.reshape(-1, D), Wd["blocks.0.attn.wo"], Wd["blocks.0.attn.bo"])
+    y = Fn.layer_norm(x, (D,), eps=1e-6) * (1 + m[4]) + m[3]
+    x = x + m[5] * Fn.linear(Fn.gelu(Fn.linear(y, Wd["blocks.0.mlp.w1"], Wd["blocks.0.mlp.b1"]), approximate="tanh"),
+                             Wd["blocks.0.mlp.w2"], Wd["blocks.0.mlp.b2"])
+    assert torch.allclose(taps["b0.x_mlp"], x, rtol=1e-10, atol=1e-12)
+    # the order matters at these gains: rotating first and normalising second is a different function
+    q2 = Fn.rms_norm(_hand_rope(qkv[:, :D].reshape(-1, H, d), pos, (0, 8, 8), 10000.0), (d,),
+                     weight=Wd["blocks.0.attn.gq"], eps=1e-6)
+    assert float((q2 - q).abs().max()) > 1e-2
+
+
+def _cross_block_by_hand(s, W, I, x_in, m, pos):
+    """R10 transcribed with torch library routines: self-attention (norm -> RoPE), gated residual, then the cross
+    sub-layer x += Wo_c SDPA(RMS(Wq_c LN(x) + bq), RMS(Wk ctx + bk), Wv ctx + bv) + bo_c with wkv rows [k | v], NO
+    gate, NO modulation, NO RoPE; then the MLP.  Returns (x after cross, x after MLP)."""
+    Fn = torch.nn.functional
+    Wd = {k: v.double() for k, v in W.items()}
+    D, H, d = s.hidden, s.n_heads, s.head_dim
+    ctx = Fn.linear(I["cond"].double(), Wd["cond_proj.w"], Wd["cond_proj.b"])
+    y = Fn.layer_norm(x_in, (D,), eps=1e-6) * (1 + m[1]) + m[0]
+    qkv = Fn.linear(y, Wd["blocks.0.attn.wqkv"], Wd["blocks.0.attn.bqkv"])
+    q, k, v = [t.reshape(-1, H, d) for t in qkv.split(D, dim=1)]
+    q = _hand_rope(Fn.rms_norm(q, (d,), weight=Wd["blocks.0.attn.gq"], eps=1e-6), pos, s.rope_dims, 10000.0)
+    k = _hand_rope(Fn.rms_norm(k, (d,), weight=Wd["blocks.0.attn.gk"], eps=1e-6), pos, s.rope_dims, 10000.0)
+    o = Fn.scaled_dot_product_attention(q.permute(1, 0, 2), k.permute(1, 0, 2), v.permute(1, 0, 2)).permute(1, 0, 2)
+    x = x_in + m[2] * Fn.linear(o.reshape(-1, D), Wd["blocks.0.attn.wo"], Wd["blocks.0.attn.bo"])
+    qc = Fn.linear(Fn.layer_norm(x, (D,), eps=1e-6), Wd["blocks.0.cross.wq"], Wd["blocks.0.cross.bq"]).reshape(-1, H, d)
+    kc = Fn.linear(ctx, Wd["blocks.0.cross.wkv"][:D], Wd["blocks.0.cross.bkv"][:D]).reshape(-1, H, d)   # K = first half
+    vc = Fn.linear(ctx, Wd["blocks.0.cross.wkv"][D:], Wd["blocks.0.cross.bkv"][D:]).reshape(-1, H, d)   # V = second half
+    qc = Fn.rms_norm(qc, (d,), weight=Wd["blocks.0.cross.gq"], eps=1e-6)
+    kc = Fn.rms_norm(kc, (d,), weight=Wd["blocks.0.cross.gk"], eps=1e-6)
+    oc = Fn.scaled_dot_product_attention(qc.permute(1, 0, 2), kc.permute(1, 0, 2), vc.permute(1, 0, 2)).permute(1, 0, 2)
+    xc = x + Fn.linear(oc.reshape(-1, D), Wd["blocks.0.cross.wo"], Wd["blocks.0.cross.bo"])
+    y = Fn.layer_norm(xc, (D,), eps=1e-6) * (1 + m[4]) + m[3]
+    xm = xc + m[5] * Fn.linear(Fn.gelu(Fn.linear(y, Wd["blocks.0.mlp.w1"], Wd["blocks.0.mlp.b1"]), approximate="tanh"),
+                               Wd["blocks.0.mlp.w2"], Wd["blocks.0.mlp.b2"])
+    return xc, xm
+
+
+def test_cross_block_by_hand():
+    """One CROSS block (cfg 3's topology, R10) against an independent torch-library transcription; also pins
+    block_rows in cross mode (the whole oracle side of the full-size cfg 3 test) to the same transcription.
+    Fails if the K / V halves of wkv are swapped, the cross branch is gated or modulated, RoPE is applied to the
+    cross q / k, the cross sub-layer is placed after the MLP, or its RMSNorm gains are dropped."""
+    s = _tiny(n_blocks=1, cond_mode="cross", rope_dims=(4, 6, 6), qk_rmsnorm=True, latent_grid=(2, 8, 8), n_cond=7)
+    W, I = _wide_gains(synth.make_weights(s), s), synth.make_inputs(s)
+    cfg = O.cfg_from_shape(s)
+    taps = {}
+    O.dit_step(cfg, W, I["latents"], I["temb"], I["cond"], taps=taps)
+    Fn = torch.nn.functional
+    Wd = {k: v.double() for k, v in W.items()}
+    c = Fn.linear(Fn.silu(Fn.linear(I["temb"].double(), Wd["t_mlp.w1"], Wd["t_mlp.b1"])), Wd["t_mlp.w2"], Wd["t_mlp.b2"])
+    m = Fn.linear(Fn.silu(c), Wd["blocks.0.mod.w"], Wd["blocks.0.mod.b"]).reshape(6, s.hidden)
+    pos = [(f, hh, ww) for f in range(2) for hh in range(4) for ww in range(4)]        # token n = (f H' + h) W' + w
+    assert taps["x0"].shape[0] == len(pos)                                             # cross mode: sequence = x only
+    xc, xm = _cross_block_by_hand(s, W, I, taps["x0"], m, pos)
+    assert torch.allclose(taps["b0.x_cross"], xc, rtol=1e-10, atol=1e-12)
+    assert torch.allclose(taps["b0.x_mlp"], xm, rtol=1e-10, atol=1e-12)
+    # the cross branch is not negligible here, so the comparison really sees it
+    assert float((taps["b0.x_cross"] - taps["b0.x_attn"]).norm() / taps["b0.x_attn"].norm()) > 1e-3
+    # block_rows, cross mode, against the hand transcription (not against dit_step)
+    ang = O.rope_angles(torch.tensor(pos), cfg["rope_dims"], cfg["rope_theta"])
+    ctx = Fn.linear(I["cond"].double(), Wd["cond_proj.w"], Wd["cond_proj.b"])
+    rows = torch.tensor([0, 3, 17, 31])
+    got = O.block_rows(cfg, W, 0, taps["x0"], taps["mod"][0], ang, rows, ctx=ctx)
+    assert torch.allclose(got, xm[rows], rtol=1e-10, atol=1e-12)
+
+
+def test_block_rows_cross_equals_step_rows():
+    """block_rows(..., ctx) in cross mode == the same rows of dit_step's second block (teacher forcing changes nothing
+    when the forced input is the oracle's own)."""
+    s = _tiny(n_blocks=2, cond_mode="cross", rope_dims=(4, 6, 6), qk_rmsnorm=True, latent_grid=(2, 8, 8), n_cond=7)
+    W, I = _wide_gains(synth.make_weights(s), s), synth.make_inputs(s)
+    cfg = O.cfg_from_shape(s)
+    taps = {}
+    O.dit_step(cfg, W, I["latents"], I["temb"], I["cond"], taps=taps)
+    ang = O.rope_angles(O.token_positions((2, 4, 4)), cfg["rope_dims"], cfg["rope_theta"])
+    ctx = O.linear(I["cond"].double(), W["cond_proj.w"], W["cond_proj.b"])
+    rows = torch.tensor([1, 2, 16, 30])
+    got = O.block_rows(cfg, W, 1, taps["b0.x_mlp"], taps["mod"][1], ang, rows, ctx=ctx)
+    assert torch.allclose(got, taps["b1.x_mlp"][rows], rtol=1e-12, atol=1e-14)
+
+
 def test_varlen_is_per_request_and_block_rows():
     s = _tiny(cond_mode="joint", rope_dims=(0, 8, 8), qk_rmsnorm=True)
     W = synth.make_weights(s)
