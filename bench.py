@@ -11,14 +11,18 @@ C ABI.  Workload at N=1: BASELINE.json configs[1] (image DiT bf16: 8 blocks, D=3
 256 text tokens, joint).  N>1: every rank runs the same step on its own request (independent requests shard
 with no data-path collective: weak scaling) and the value is N*K / max-over-ranks time.
 
-Prints ONE JSON line (rank 0).  `value` = steps/s with inputs resident in HBM; `e2e` = the same through
-`dit_step_host` (pinned HOST buffers in, host buffer out, copies inside the timed region).
+Prints ONE JSON line (rank 0).  `value` = steps/s with inputs resident in HBM, timed with no per-launch
+instrumentation; `e2e` = the same through `dit_step_host` / `dit_step_varlen_host` (pinned HOST buffers in, host
+buffer out, copies inside the timed region); `roofline` (block GEMMs) and `roofline_attention` come from a second
+region of the same K steps with those launches bracketed by CUDA events, against the measured peak that matches
+the SM clock sampled during that region.
 `--impl reference` times the CPU oracle (oracle/dit_oracle.py, as it stands) on the host cores instead.
 """
 from __future__ import annotations
 
 import argparse
 import json
+import math
 import os
 import statistics
 import subprocess
@@ -53,6 +57,15 @@ CFG4_NAME = ("BASELINE.json configs[3]: packed varlen batch bf16, cfg2 block sha
 def _workload_name(s) -> str:
     return {"cfg2_image_bf16": "BASELINE.json configs[1]: image DiT bf16, 8 blocks, D=3072, 24x128, 4096+256 joint tokens",
             "cfg3_video_bf16": "BASELINE.json configs[2]: video DiT bf16, 4 blocks, D=5120, 40x128, 32760 tokens, cross-attn 512"}[s.name]
+
+
+def bench_config(s, wl_name: str, split_p: int, req_per_gpu: int, world: int) -> dict:
+    """The `config` object of the JSON line — the same for both arms (`--impl ours` and `--impl reference`)."""
+    weight_gb = sum(math.prod(shp) for shp in synth.weight_shapes(s).values()) * (4 if s.dtype == "f32" else 2) / 1e9
+    return {"workload": wl_name, "split_p": split_p, "requests_per_gpu": req_per_gpu,
+            "l2": f"inputs exceed L2: every step streams {weight_gb:.1f} GB of weights (plus activations) "
+                  "through a 126 MB L2, so no step starts with its operands cached",
+            "parallelism": f"replicas x{world} (independent requests, no data-path collective)"}
 
 
 def step_flops(s, seq_lens=None) -> dict:
@@ -218,7 +231,7 @@ def run_reference(args, rank: int):
         smp.sample += f"; {len(times)} of {args.steps} steps timed ({REF_BUDGET_S:.0f} s wall-clock bound)"
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": len(times),
             "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic", "config": {"workload": _workload_name(s)},
+            "dtype": "f64", "data": "synthetic", "config": bench_config(s, _workload_name(s), args.split_p, 1, args.gpus),
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": smp.sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -257,22 +270,19 @@ def run_ours(args, rank: int, local_rank: int, world: int):
                                 max_cond_tokens=sum(sh.n_cond for sh in shapes)), W, dev)
         lats, conds = [i["latents"] for i in Is], [i["cond"] for i in Is]
         tembs = torch.cat([i["temb"] for i in Is]).contiguous()
-        lats_h = [l.cpu().pin_memory() for l in lats]
-        conds_h = [c.cpu().pin_memory() for c in conds]
+        packed_h = torch.cat([l.reshape(-1) for l in lats]).cpu().pin_memory()
+        cond_h = torch.cat(conds).cpu().pin_memory()
         tembs_h = tembs.cpu().pin_memory()
-        outs_h = [torch.empty_like(l) for l in lats_h]
-        h2d = sum(t.numel() * t.element_size() for t in lats_h + conds_h + [tembs_h])
-        d2h = sum(t.numel() * t.element_size() for t in outs_h)
+        out_h = torch.empty_like(packed_h).pin_memory()
+        lat_shapes, n_conds = [tuple(l.shape) for l in lats], [int(c.shape[0]) for c in conds]
+        h2d = sum(t.numel() * t.element_size() for t in (packed_h, cond_h, tembs_h))
+        d2h = out_h.numel() * out_h.element_size()
 
         def step():
             return m.dit_step_varlen(lats, tembs, conds)
 
-        def step_e2e():   # pinned host -> device copies, the packed step, device -> host read of every output
-            for dst, src in zip(lats + conds + [tembs], lats_h + conds_h + [tembs_h]):
-                dst.copy_(src, non_blocking=True)
-            outs = m.dit_step_varlen(lats, tembs, conds)
-            for dst, src in zip(outs_h, outs):
-                dst.copy_(src, non_blocking=True)
+        def step_e2e():   # dit_step_varlen_host: ONE C-ABI call with HOST buffers (the library enqueues H2D, step, D2H)
+            m.dit_step_varlen_host(packed_h, lat_shapes, tembs_h, cond_h, n_conds, out_h)
         wl_name, req_per_gpu = CFG4_NAME, R
     else:
         fl = step_flops(s)
@@ -292,30 +302,43 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         def step_e2e():   # dit_step_host: the C-ABI call with HOST buffers (copies are enqueued by the library)
             m.dit_step_host(lat_h, temb_h, cond_h, out_h)
         wl_name, req_per_gpu = _workload_name(s), 1
-    weight_gb = sum(v.numel() * v.element_size() for v in W.values()) / 1e9
 
     for _ in range(Wm):
         step()
     torch.cuda.synchronize()
 
-    # ---- timed region: K steps, device-resident inputs; GEMM-class launches bracketed by events (roofline)
+    # ---- timed region: K steps, device-resident inputs, NO per-launch instrumentation (this is `value`)
     sampler = ClockSampler(_gpu_index(local_rank))
     time.sleep(0.25)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier(); torch.cuda.synchronize()
     n0 = B.dit_kernel_launches()
-    B.dit_profile_begin(("gemm",))
     e0.record()
     for _ in range(K):
         step()
     e1.record()
     torch.cuda.synchronize(); barrier()
-    prof = B.dit_profile_end()
     launches = B.dit_kernel_launches() - n0
     clocks = sampler.stop()
     ms_total = e0.elapsed_time(e1)
 
-    # ---- e2e: dit_step_host, pinned host buffers, H2D + step + D2H per step inside the timed region
+    # ---- roofline region: the same K back-to-back steps again with every block-GEMM and attention launch bracketed by a
+    # CUDA-event pair on the launching stream (dit_profile_begin).  Kept apart from the region above: the event pairs
+    # (2 x 40 per cfg 2 step) stop PDL overlap between neighbours and would perturb `value`.
+    sampler_r = ClockSampler(_gpu_index(local_rank))
+    torch.cuda.synchronize()
+    r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    B.dit_profile_begin(("gemm", "attn"))
+    r0.record()
+    for _ in range(K):
+        step()
+    r1.record()
+    torch.cuda.synchronize()
+    prof = B.dit_profile_end()
+    clocks_r = sampler_r.stop()
+    ms_roof = r0.elapsed_time(r1)
+
+    # ---- e2e: dit_step_host / dit_step_varlen_host, pinned host buffers, H2D + step + D2H per step inside the timed region
     for _ in range(min(Wm, 3)):
         step_e2e()
     torch.cuda.synchronize()
@@ -341,35 +364,46 @@ def run_ours(args, rank: int, local_rank: int, world: int):
 
     if rank == 0:
         pk = _peaks()
-        gemm_ms, gemm_n = prof["gemm"]
-        achieved = (fl["gemm"] * K) / (gemm_ms * 1e-3) / 1e12 if gemm_ms > 0 else 0.0
-        traffic = None
-        tp = os.path.join(ROOT, "profiles", "traffic.csv")   # DRAM bytes per launch from the ncu --set full capture
-        if os.path.exists(tp):
-            for ln in open(tp).read().splitlines()[1:]:
-                f = ln.split(",")
-                if len(f) >= 3 and f[0] == ("cfg2" if args.workload == "cfg4" else args.workload) and f[1] == "gemm":
-                    traffic = int(f[2])
+
+        def roof(cls, flops_per_step, kernel, wl_key):
+            ms, n = prof[cls]
+            ach = (flops_per_step * K) / (ms * 1e-3) / 1e12 if ms > 0 else 0.0
+            # which measured peak applies is decided by the SM clock sampled DURING this region: at >= 0.9 of the maximum
+            # the part is in its burst regime (MEASURED_PEAKS.json bf16_tflops), below it under the power cap (sustained)
+            sm, mx = clocks_r.get("sm_mhz"), clocks_r.get("sm_max_mhz")
+            burst = bool(sm and mx and sm >= 0.9 * mx)
+            peak = pk["tf_burst"] if burst else pk["tf_sust"]
+            traffic = None
+            tp = os.path.join(ROOT, "profiles", "traffic.csv")   # DRAM bytes per launch from the ncu --set full capture
+            if os.path.exists(tp):
+                for ln in open(tp).read().splitlines()[1:]:
+                    f = ln.split(",")
+                    if len(f) >= 3 and f[0] == ("cfg2" if args.workload == "cfg4" else args.workload) and f[1] == wl_key:
+                        traffic = int(f[2])
+            return {"bound": "tensor", "kernel": kernel, "achieved": ach, "peak": peak, "unit": "TFLOP/s",
+                    "frac": ach / peak, "peak_source": pk["src"] + (" bf16_tflops (burst: " if burst else " bf16_tflops_sustained (") +
+                    f"SM clock {sm} of {mx} MHz sampled during the region)",
+                    "frac_burst": ach / pk["tf_burst"], "frac_sustained": ach / pk["tf_sust"], "frac_of_nominal_2250": ach / 2250.0,
+                    "launches": n, "avg_launch_ms": ms / max(1, min(n, 16384)), "share_of_step": ms / ms_roof,
+                    "flops_per_step": flops_per_step, "traffic": traffic,
+                    "timed": f"CUDA events around every launch of the class over {K} back-to-back steps (a second region; "
+                             "`value` is timed without them)"}
+
         line = {
             "metric": METRIC, "value": job_throughput(world, K, ms_total), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
             "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
             "data": "synthetic",
-            "config": {"workload": wl_name, "split_p": args.split_p, "requests_per_gpu": req_per_gpu,
-                       "l2": f"inputs exceed L2: every step streams {weight_gb:.1f} GB of weights (plus activations) "
-                             "through a 126 MB L2, so no step starts with its operands cached",
-                       "parallelism": f"replicas x{world} (independent requests, no data-path collective)"},
+            "config": bench_config(s, wl_name, args.split_p, req_per_gpu, world),
             "clocks": clocks,
             "device": {"name": torch.cuda.get_device_name(dev), "sms": torch.cuda.get_device_properties(dev).multi_processor_count,
                        "torch": torch.__version__, "cuda": torch.version.cuda, "peaks": pk,
-                       "timing": f"{K} back-to-back steps after {Wm} warm-ups (sustained clocks), CUDA events"},
-            "e2e": {"value": job_throughput(world, K, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
-            "gpu_launches": launches,
-            "roofline": {"bound": "tensor", "kernel": "block GEMMs (QKV, out-proj, fc1, fc2)", "achieved": achieved,
-                         "peak": pk["tf_sust"], "unit": "TFLOP/s", "frac": achieved / pk["tf_sust"],
-                         "peak_source": pk["src"] + " bf16_tflops_sustained (kernel timed inside a long step)",
-                         "frac_of_nominal_2250": achieved / 2250.0, "launches": gemm_n,
-                         "avg_launch_ms": gemm_ms / max(1, min(gemm_n, 16384)), "share_of_step": gemm_ms / ms_total,
-                         "flops_per_step": fl["gemm"], "traffic": traffic},
+                       "timing": f"{K} back-to-back steps after {Wm} warm-ups, CUDA events, no per-launch instrumentation"},
+            "e2e": {"value": job_throughput(world, K, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "call": "dit_step_varlen_host" if args.workload == "cfg4" else "dit_step_host"},
+            "gpu_launches": launches, "fallback_launches": B.dit_fallback_launches(),
+            "roofline": roof("gemm", fl["gemm"], "block GEMMs (QKV, out-proj, fc1, fc2" + (", cross projections)" if s.cond_mode == "cross" else ")"), "gemm"),
+            "roofline_attention": roof("attn", fl["attn"], "attention (self" + (" + cross)" if s.cond_mode == "cross" else ")"), "attn"),
+            "clocks_roofline_region": clocks_r,
             "breakdown_ms_per_step": {k: round(v[0] / nb, 4) for k, v in prof_all.items()},
             "tflops": {"attention": (fl["attn"] * nb) / (prof_all["attn"][0] * 1e-3) / 1e12 if prof_all["attn"][0] > 0 else None,
                        "gemm": (fl["gemm"] * nb) / (prof_all["gemm"][0] * 1e-3) / 1e12 if prof_all["gemm"][0] > 0 else None,

@@ -23,7 +23,15 @@
  *  - Errors: a negative dit_status is returned before anything is launched when arguments are invalid;
  *    DIT_ERR_CUDA reports a failed launch/API call.  dit_last_error() gives a message.  Nothing throws.
  *  - There is no CPU fallback and no alternative backend: if no sm_100 device is present every compute
- *    entry point returns DIT_ERR_CUDA.
+ *    entry point returns DIT_ERR_CUDA.  A DIT_BF16 handle runs its step on the tcgen05 kernels ONLY: dit_init
+ *    returns DIT_ERR_UNSUPPORTED for a bf16 config they cannot serve (head_dim != 128, C*pv or cond_dim not a
+ *    multiple of 8) and a step returns DIT_ERR_UNSUPPORTED rather than substitute the fp32 FFMA kernels.  The
+ *    kernel-level entry points below do run bf16 shapes outside those limits on the FFMA kernels; each such
+ *    launch is counted by dit_fallback_launches().
+ *  - Threads and streams: a handle owns ONE workspace, so calls on the same handle must be ordered by the caller
+ *    (one stream at a time, or explicit events between streams); different handles are independent and may be
+ *    driven from different host threads.  dit_last_error is per host thread.  The measurement calls
+ *    (dit_profile_begin / dit_profile_end) are process wide.
  *  - dtype: DIT_F32 (all tensors fp32; SIMT FFMA kernels, no TF32) or DIT_BF16 (weights/activations
  *    bf16, residual stream / statistics / modulation / LSE fp32; tcgen05 tensor-core kernels).
  *  - Linear weights are [out, in] row-major, biases [out], all in the config dtype.
@@ -141,6 +149,13 @@ dit_status dit_step_host(dit_handle h, const void* latents_host, const float* ti
                          const void* cond_tokens_host, int32_t n_cond, const int32_t latent_grid[3],
                          void* out_host, void* stream);
 
+/* dit_step_varlen with HOST buffers (pageable or pinned): latents_packed / timestep_emb / cond_packed are copied to the
+ * workspace's staging area, the packed step runs, and out_packed is copied back, all enqueued on `stream`; the caller
+ * synchronises the stream before reading out_packed_host.  Arguments as dit_step_varlen below. */
+dit_status dit_step_varlen_host(dit_handle h, const void* latents_packed_host, const float* timestep_emb_host,
+                                const void* cond_packed_host, const int32_t* cu_seqlens, const int32_t* n_cond,
+                                const int32_t* latent_grids, int32_t n_requests, void* out_packed_host, void* stream);
+
 /* Packed variable-length batch of R heterogeneous requests (BASELINE.json north_star subsystem 6; the
  * single-GPU analogue of the paper's heterogeneous request mix).  The result for request r
  * is DEFINED as dit_step on request r alone (DESIGN.md §3 step 8).
@@ -152,7 +167,10 @@ dit_status dit_step_host(dit_handle h, const void* latents_host, const float* ti
  *   n_cond           host [R];   latent_grids host [R][3] = {F_r, H_r, W_r}
  *   out_packed       dev: R outputs back to back, each with its latent's shape
  * GEMMs / norms run over the flat [sum T_r, D] sequence; modulation is indexed per request; attention is
- * block diagonal over requests. */
+ * block diagonal over requests.
+ * (SURVEY.md §8(b) sketched this call with a host AND a device copy of cu_seqlens; the library uploads its own device
+ * copy — a few hundred bytes, skipped when the geometry is already resident — so the caller passes host arrays only:
+ * DESIGN.md reading R35.) */
 dit_status dit_step_varlen(dit_handle h, const void* latents_packed, const float* timestep_emb,
                            const void* cond_packed, const int32_t* cu_seqlens, const int32_t* n_cond,
                            const int32_t* latent_grids, int32_t n_requests, void* out_packed, void* stream);
@@ -164,7 +182,11 @@ dit_status dit_step_varlen(dit_handle h, const void* latents_packed, const float
  *   q  dev [n_q, H, d] with row stride q_row_stride elements (head stride = d);  k, v dev [n_k, H, d]
  *      with row stride kv_row_stride;  dtype = dit_dtype of q, k, v and o
  *   o  dev [n_q, H, d] contiguous;  lse dev [n_q, H] fp32 (may be NULL)
- * With n_k = all keys this is the full-sequence flash attention of subsystem 4. */
+ * With n_k = all keys this is the full-sequence flash attention of subsystem 4.
+ * q and k are taken AS GIVEN: QK-RMSNorm and RoPE (north_star subsystem 4, "fused into the Q/K load") are applied one
+ * kernel earlier, on the fp32 accumulators of the QKV projection (dit_linear_qkv below), not on the attention kernel's
+ * loads; SURVEY.md §8(b)'s optional `dit_attn_opts` (norm / RoPE on load) is therefore not part of this ABI.  Why, with
+ * the measurements: DESIGN.md reading R34.  Callers with raw q / k use dit_linear_qkv or dit_qknorm_rope first. */
 dit_status dit_attn_partial(int32_t dtype, const void* q, const void* k, const void* v, int32_t n_q, int32_t n_k,
                             int32_t n_heads, int32_t head_dim, int64_t q_row_stride, int64_t kv_row_stride,
                             float softmax_scale, void* o, float* lse, void* stream);
@@ -275,6 +297,9 @@ dit_status dit_profile_end(float* ms_per_class, int32_t* launches_per_class);
 
 const char* dit_last_error(dit_handle h); /* h may be NULL: last error of a handle-less entry point */
 int32_t dit_kernel_launches(void);         /* kernels launched by this library so far (this process) */
+int32_t dit_fallback_launches(void);       /* of those: bf16 GEMM / attention launches that ran on the fp32-path FFMA kernels
+                                              because the shape is outside the tcgen05 kernels' limits (kernel-level entry
+                                              points only; a step never does).  0 in every BASELINE.json config. */
 void dit_free(dit_handle h);
 
 #ifdef __cplusplus

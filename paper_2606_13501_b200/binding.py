@@ -18,9 +18,10 @@ EPI_BIAS, EPI_BIAS_GELU, EPI_BIAS_F32 = 0, 1, 2
 TAP = dict(x=0, y=1, qkv=2, o=3, u=5, c=6, mod=7, tok=8)
 STAGE = dict(y1=0, qkv=1, attn=2, oproj=3, cross=4, y2=5, fc1=6, fc2=7)
 
-SYMBOLS = ["dit_workspace_bytes", "dit_init", "dit_step", "dit_step_host", "dit_step_varlen", "dit_sample", "dit_attn_partial",
+SYMBOLS = ["dit_workspace_bytes", "dit_init", "dit_step", "dit_step_host", "dit_step_varlen", "dit_step_varlen_host", "dit_sample", "dit_attn_partial",
            "dit_attn_merge", "dit_linear", "dit_linear_residual", "dit_linear_qkv", "dit_adaln", "dit_gemv", "dit_qknorm_rope", "dit_debug_stop_after",
-           "dit_get_tap", "dit_profile_begin", "dit_profile_end", "dit_last_error", "dit_kernel_launches", "dit_free"]
+           "dit_get_tap", "dit_profile_begin", "dit_profile_end", "dit_last_error", "dit_kernel_launches", "dit_fallback_launches",
+           "dit_free"]
 
 
 class dit_config(C.Structure):
@@ -57,6 +58,7 @@ def load(path: str = LIB_PATH):
     lib.dit_last_error.restype = C.c_char_p
     lib.dit_last_error.argtypes = [C.c_void_p]
     lib.dit_kernel_launches.restype = C.c_int32
+    lib.dit_fallback_launches.restype = C.c_int32
     lib.dit_free.restype = None
     lib.dit_free.argtypes = [C.c_void_p]
     vp, i32, i64, f32 = C.c_void_p, C.c_int32, C.c_int64, C.c_float
@@ -66,6 +68,7 @@ def load(path: str = LIB_PATH):
         "dit_step": [vp, vp, vp, vp, i32, pi32, vp, vp],
         "dit_step_host": [vp, vp, vp, vp, i32, pi32, vp, vp],
         "dit_step_varlen": [vp, vp, vp, vp, pi32, pi32, pi32, i32, vp, vp],
+        "dit_step_varlen_host": [vp, vp, vp, vp, pi32, pi32, pi32, i32, vp, vp],
         "dit_sample": [vp, vp, vp, C.POINTER(C.c_float), vp, i32, vp, i32, f32, pi32, i32, i32, vp, vp],
         "dit_attn_partial": [i32, vp, vp, vp, i32, i32, i32, i32, i64, i64, f32, vp, vp, vp],
         "dit_attn_merge": [i32, C.POINTER(vp), C.POINTER(vp), i32, i32, i32, i32, vp, vp, vp],
@@ -195,21 +198,24 @@ class Dit:
                                       _ptr(out_host), _stream(stream)), "dit_step_host")
         return out_host
 
+    def _varlen_geom(self, shapes, n_cond):
+        joint = self.cfg.cond_mode == COND["joint"]
+        p = self.cfg.patch
+        cu, grids = [0], []
+        for r, shp in enumerate(shapes):
+            f, h, w = shp[1:]
+            grids += [f, h, w]
+            cu.append(cu[-1] + (f // p[0]) * (h // p[1]) * (w // p[2]) + (n_cond[r] if joint else 0))
+        return cu, grids
+
     def dit_step_varlen(self, latents_list, temb, cond_list=None, stream=None):
         """latents_list: R tensors [C,F_r,H_r,W_r]; temb [R, temb_dim]; cond_list: R tensors or None.
         Packs (torch.cat: memory plumbing only), calls the C ABI once, returns the R outputs (views)."""
         R = len(latents_list)
         packed = torch.cat([l.reshape(-1) for l in latents_list])
-        joint = self.cfg.cond_mode == COND["joint"]
         n_cond = [0 if (cond_list is None or cond_list[r] is None) else cond_list[r].shape[0] for r in range(R)]
         cond = torch.cat([c for c in cond_list if c is not None]) if cond_list is not None and sum(n_cond) else None
-        p = self.cfg.patch
-        cu = [0]
-        grids = []
-        for r, l in enumerate(latents_list):
-            f, h, w = l.shape[1:]
-            grids += [f, h, w]
-            cu.append(cu[-1] + (f // p[0]) * (h // p[1]) * (w // p[2]) + (n_cond[r] if joint else 0))
+        cu, grids = self._varlen_geom([l.shape for l in latents_list], n_cond)
         out = torch.empty_like(packed)
         _check(self.lib.dit_step_varlen(self.handle, _ptr(packed), _ptr(temb), _ptr(cond), _i32arr(cu), _i32arr(n_cond),
                                         _i32arr(grids), R, _ptr(out), _stream(stream)), "dit_step_varlen")
@@ -218,6 +224,16 @@ class Dit:
             outs.append(out[off:off + l.numel()].reshape(l.shape))
             off += l.numel()
         return outs
+
+    def dit_step_varlen_host(self, packed_host, shapes, temb_host, cond_host, n_cond, out_host, stream=None):
+        """HOST buffers, already packed by the caller: packed_host = the R latents back to back (1-D), shapes = their
+        [C,F_r,H_r,W_r] shapes, temb_host [R, temb_dim] fp32, cond_host [sum n_cond, cond_dim] or None, out_host like
+        packed_host.  One C-ABI call: H2D copies, the packed step and the D2H copy are enqueued by the library."""
+        cu, grids = self._varlen_geom(shapes, n_cond)
+        _check(self.lib.dit_step_varlen_host(self.handle, _ptr(packed_host), _ptr(temb_host), _ptr(cond_host), _i32arr(cu),
+                                             _i32arr(n_cond), _i32arr(grids), len(shapes), _ptr(out_host), _stream(stream)),
+               "dit_step_varlen_host")
+        return out_host
 
     def dit_debug_stop_after(self, block, stage):
         _check(self.lib.dit_debug_stop_after(self.handle, block, STAGE[stage] if isinstance(stage, str) else stage),
@@ -341,3 +357,8 @@ def dit_profile_end() -> dict:
 
 def dit_kernel_launches() -> int:
     return int(load().dit_kernel_launches())
+
+
+def dit_fallback_launches() -> int:
+    """bf16 GEMM / attention launches that ran on the FFMA (fp32-path) kernels; 0 for every BASELINE.json config."""
+    return int(load().dit_fallback_launches())

@@ -611,7 +611,7 @@ dit_status launch_attn_tc(const AttnArgs& a, cudaStream_t st) {
     for (int r = 0; r < a.R; ++r) max_q = max(max_q, a.cu_q_host[r + 1] - a.cu_q_host[r]);
   }
   if (max_q == 0) return DIT_OK;
-  static bool attr_set = false;
+  static std::atomic<bool> attr_set{false};
   if (!attr_set) {
     DIT_CUDA_OK(cudaFuncSetAttribute(attn_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, ATTN_SMEM));
     DIT_CUDA_OK(cudaFuncSetAttribute(attn_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, ATTN_SMEM));

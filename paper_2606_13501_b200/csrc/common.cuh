@@ -1,5 +1,6 @@
 // common.cuh — shared device/host helpers of libdit_b200 (CUDA path only; the oracle shares nothing with it).
 #pragma once
+#include <atomic>
 #include <utility>
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
@@ -11,8 +12,10 @@ namespace dit {
 
 typedef __nv_bfloat16 bf16;
 
-// launch accounting (dit_kernel_launches)
-extern int g_launches;
+// launch accounting (dit_kernel_launches); g_fallback_launches counts bf16 GEMM / attention launches that did NOT take
+// the tcgen05 path (dit_fallback_launches): the FFMA kernels are the fp32 path, never a silent substitute for bf16
+extern std::atomic<int> g_launches;
+extern std::atomic<int> g_fallback_launches;
 void set_error(const char* fmt, ...);
 const char* get_error();
 
@@ -48,7 +51,7 @@ static inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 
 // per-class device timing (dit_profile_begin / dit_profile_end): when a class is enabled every launcher of that
 // class brackets its launch with a cudaEvent pair on the launching stream.  Off by default (zero overhead).
-extern int g_prof_mask;
+extern std::atomic<int> g_prof_mask;
 extern thread_local int g_prof_class_override;  // >= 0: launchers report this class instead of their own
 void prof_record(int cls, cudaStream_t st, bool start);
 struct ProfScope {
@@ -56,7 +59,7 @@ struct ProfScope {
   cudaStream_t st;
   bool on;
   ProfScope(int c, cudaStream_t s) : cls(g_prof_class_override >= 0 ? g_prof_class_override : c), st(s) {
-    on = (g_prof_mask >> cls) & 1;
+    on = (g_prof_mask.load(std::memory_order_relaxed) >> cls) & 1;
     if (on) prof_record(cls, st, true);
   }
   ~ProfScope() {

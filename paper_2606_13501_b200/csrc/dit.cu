@@ -4,7 +4,9 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <atomic>
 #include <map>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -12,7 +14,8 @@
 
 namespace dit {
 
-int g_launches = 0;
+std::atomic<int> g_launches{0};
+std::atomic<int> g_fallback_launches{0};
 static thread_local char g_err[512] = "";
 void set_error(const char* fmt, ...) {
   va_list ap;
@@ -23,10 +26,11 @@ void set_error(const char* fmt, ...) {
 const char* get_error() { return g_err; }
 
 // ---- per-class event timing -------------------------------------------------------------------------
-int g_prof_mask = 0;
+std::atomic<int> g_prof_mask{0};
 thread_local int g_prof_class_override = -1;
 namespace {
-struct ProfRec { cudaEvent_t a, b; int cls; };
+std::mutex g_prof_mu;   // guards the record list, the event pool and the counts (launchers of several host threads)
+struct ProfRec { cudaEvent_t a, b; int cls; bool open; };
 std::vector<ProfRec> g_prof_recs;
 std::vector<cudaEvent_t> g_prof_pool;
 int g_prof_counts[DIT_KC_COUNT];
@@ -39,16 +43,21 @@ cudaEvent_t prof_event() {
 }
 }  // namespace
 void prof_record(int cls, cudaStream_t st, bool start) {
+  std::lock_guard<std::mutex> lk(g_prof_mu);
   if (start) {
     g_prof_counts[cls]++;
-    if (g_prof_recs.size() >= kProfMax) return;
-    ProfRec r{prof_event(), prof_event(), cls};
+    if (g_prof_recs.size() >= kProfMax) return;   // counted, not timed
+    ProfRec r{prof_event(), prof_event(), cls, true};
     cudaEventRecord(r.a, st);
     g_prof_recs.push_back(r);
-  } else if (!g_prof_recs.empty() && g_prof_counts[cls] <= (int)kProfMax) {
-    // the matching start is the most recent record of this class (launchers do not nest within a class)
+  } else {
+    // the matching start is the most recent OPEN record of this class (launchers do not nest within a class); a
+    // launch that was counted but not recorded (list full) has no open record and its end is dropped
     for (size_t i = g_prof_recs.size(); i-- > 0;)
-      if (g_prof_recs[i].cls == cls) { cudaEventRecord(g_prof_recs[i].b, st); break; }
+      if (g_prof_recs[i].cls == cls) {
+        if (g_prof_recs[i].open) { cudaEventRecord(g_prof_recs[i].b, st); g_prof_recs[i].open = false; }
+        break;
+      }
   }
 }
 
@@ -98,8 +107,10 @@ struct dit_handle_s {
   const void *t_w1, *t_b1, *t_w2, *t_b2, *pe_w, *pe_b, *cp_w, *cp_b, *fm_w, *fm_b, *f_w, *f_b;
   Workspace ws;
   int stop_block, stop_stage;
-  // cached per-call geometry (skip rebuilding RoPE tables when unchanged)
+  // geometry resident on the device (cu_seqlens, cond offsets, per-request meta, RoPE tables): uploads are skipped
+  // when a call's geometry equals it in EVERY field
   std::vector<int32_t> last_geom;
+  bool capturing = false;              // inside dit_sample's stream capture: no host -> device copy may be enqueued
   // dit_sample: one cached trajectory graph, valid while every argument (and sigma) it was captured with is unchanged
   cudaGraphExec_t graph_exec = nullptr;
   cudaStream_t cap_stream = nullptr;   // capture happens here (the caller's stream may be the legacy default stream)
@@ -160,6 +171,19 @@ static dit_status validate(const dit_config* c) {
   DIT_REQUIRE(c->n_heads > 0 && c->hidden == c->n_heads * c->head_dim, DIT_ERR_INVALID_ARG,
               "hidden %d != n_heads %d * head_dim %d", c->hidden, c->n_heads, c->head_dim);
   DIT_REQUIRE(c->hidden % 256 == 0, DIT_ERR_UNSUPPORTED, "hidden %d must be a multiple of 256", c->hidden);
+  {  // the adaLN kernel is instantiated for these row widths (elementwise.cu, launch_adaln_t)
+    const int nc = c->hidden / 256;
+    const bool ok = nc == 1 || nc == 2 || nc == 3 || nc == 4 || nc == 5 || nc == 6 || nc == 8 || nc == 10 || nc == 12 ||
+                    nc == 16 || nc == 20 || nc == 24;
+    DIT_REQUIRE(ok, DIT_ERR_UNSUPPORTED, "hidden %d: hidden / 256 must be one of 1,2,3,4,5,6,8,10,12,16,20,24", c->hidden);
+  }
+  if (c->dtype == DIT_BF16) {   // a bf16 step runs on the tcgen05 kernels only (no FFMA substitute inside a step)
+    const int pvC = c->latent_channels * c->patch[0] * c->patch[1] * c->patch[2];
+    DIT_REQUIRE(c->head_dim == 128, DIT_ERR_UNSUPPORTED, "bf16 configs need head_dim 128 (tcgen05 attention); got %d", c->head_dim);
+    DIT_REQUIRE(pvC % 8 == 0, DIT_ERR_UNSUPPORTED, "bf16 configs need latent_channels * patch volume (%d) to be a multiple of 8", pvC);
+    DIT_REQUIRE(c->cond_mode == DIT_COND_NONE || c->cond_dim % 8 == 0, DIT_ERR_UNSUPPORTED,
+                "bf16 configs need cond_dim (%d) to be a multiple of 8", c->cond_dim);
+  }
   DIT_REQUIRE(c->mlp_dim > 0 && c->mlp_dim % 8 == 0, DIT_ERR_UNSUPPORTED, "mlp_dim %d must be a multiple of 8", c->mlp_dim);
   DIT_REQUIRE(c->latent_channels > 0 && c->patch[0] > 0 && c->patch[1] > 0 && c->patch[2] > 0, DIT_ERR_INVALID_ARG,
               "latent_channels / patch must be positive");
@@ -186,6 +210,15 @@ bool pdl_enabled() {
   return on;
 }
 
+// Inside a denoising step (run_step) a bf16 config must run on the tcgen05 kernels: the FFMA kernels are the fp32 path,
+// ~100x slower, and never a silent substitute (north_star: "no multi-backend dispatch").  The kernel-level entry points
+// (dit_linear, dit_attn_partial, ...) still accept shapes the tensor-core kernels do not (head_dim 64, K % 8 != 0) and
+// run them on the FFMA kernels; every such launch is counted in dit_fallback_launches().
+static thread_local bool g_strict_tc = false;
+#define DIT_STRICT_TC(what)                                                                                    \
+  DIT_REQUIRE(!g_strict_tc, DIT_ERR_UNSUPPORTED, "bf16 step: %s does not meet the tcgen05 kernels' requirements " \
+              "(head_dim 128, K / N / strides multiples of 8, 16-byte aligned pointers)", what)
+
 // GEMM dispatch: bf16 -> tcgen05 whenever the shape/alignment allows, else FFMA.  fp32 -> FFMA (no TF32).
 static dit_status gemm(int dtype, int epi, const void* A, int64_t lda, const void* W, const void* bias, void* out,
                        int64_t ldo, int M, int N, int K, cudaStream_t st, int kc = DIT_KC_GEMM) {
@@ -193,6 +226,10 @@ static dit_status gemm(int dtype, int epi, const void* A, int64_t lda, const voi
                     ~Override() { g_prof_class_override = prev; } } ov(kc == DIT_KC_GEMM ? -1 : kc);
   if (dtype == DIT_BF16 && gemm_tc_supported(epi, A, lda, W, out, ldo, M, N, K))
     return launch_gemm_tc(epi, A, lda, W, bias, out, ldo, M, N, K, st);
+  if (dtype == DIT_BF16 && M > 0) {
+    DIT_STRICT_TC("a GEMM");
+    g_fallback_launches++;   // visible through dit_fallback_launches()
+  }
   return launch_gemm_simt(dtype, epi, A, lda, W, bias, out, ldo, M, N, K, st);
 }
 
@@ -203,11 +240,19 @@ static dit_status gemm_residual(int dtype, const void* A, int64_t lda, const voi
                                 int N, int K, cudaStream_t st) {
   if (dtype == DIT_BF16 && gemm_tc_supported(3, A, lda, W, x, ldx, M, N, K))
     return launch_gemm_tc_ex(3, A, lda, W, bias, x, ldx, gate, gate_stride, cu, R, M, N, K, st);
+  if (dtype == DIT_BF16 && M > 0) {
+    DIT_STRICT_TC("a residual GEMM");
+    g_fallback_launches++;
+  }
   return launch_gemm_simt(dtype, 3, A, lda, W, bias, x, ldx, M, N, K, st, gate, gate_stride, cu, R);
 }
 
 static dit_status attention(int dtype, const AttnArgs& a, cudaStream_t st) {
   if (dtype == DIT_BF16 && attn_tc_supported(a)) return launch_attn_tc(a, st);
+  if (dtype == DIT_BF16 && a.n_q > 0) {
+    DIT_STRICT_TC("attention");
+    g_fallback_launches++;
+  }
   return launch_attn_simt(dtype, a, st);
 }
 
@@ -222,6 +267,8 @@ struct StepGeom {
 
 // Per-call geometry to the device (pageable host memory: the driver stages it before returning) and the RoPE tables;
 // skipped when the geometry is the one already resident.  Not capturable: dit_sample calls it before it begins a capture.
+// A handle's workspace (and this geometry) is shared by all its calls: calls on one handle must be stream ordered by the
+// caller (include/dit.h, conventions).
 static dit_status upload_geom(dit_handle hd, const StepGeom& g, cudaStream_t st) {
   const dit_config& c = hd->cfg;
   Workspace& w = hd->ws;
@@ -229,6 +276,9 @@ static dit_status upload_geom(dit_handle hd, const StepGeom& g, cudaStream_t st)
   const bool joint = c.cond_mode == DIT_COND_JOINT;
   const bool rope = (c.rope_dims[0] + c.rope_dims[1] + c.rope_dims[2]) > 0;
   std::vector<SeqMeta> meta(R);
+  // The key holds everything the device copies are made from: sequence starts, the cond-token offsets of EVERY mode
+  // (cross-attention reads cu_cond_dev: same latent grids with other prompt lengths is the normal serving case), the
+  // token grids, the latent offsets and the total row count.
   std::vector<int32_t> geom;
   for (int r = 0; r < R; ++r) {
     meta[r].seq_start = g.cu[r];
@@ -239,10 +289,13 @@ static dit_status upload_geom(dit_handle hd, const StepGeom& g, cudaStream_t st)
     meta[r].lat_off_lo = (int32_t)(g.lat_off[r] & 0xffffffff);
     meta[r].lat_off_hi = (int32_t)(g.lat_off[r] >> 32);
     meta[r].pad = 0;
-    geom.insert(geom.end(), {meta[r].seq_start, meta[r].n_cond, meta[r].gf, meta[r].gh, meta[r].gw});
+    geom.insert(geom.end(), {meta[r].seq_start, g.ncond[r], g.cu_cond[r + 1], meta[r].gf, meta[r].gh, meta[r].gw,
+                             meta[r].lat_off_lo, meta[r].lat_off_hi});
   }
   geom.push_back(T);
+  geom.push_back(R);
   if (geom == hd->last_geom) return DIT_OK;
+  DIT_REQUIRE(!hd->capturing, DIT_ERR_CUDA, "geometry changed inside a stream capture");
   DIT_CUDA_OK(cudaMemcpyAsync(w.cu_dev, g.cu.data(), (R + 1) * 4, cudaMemcpyHostToDevice, st));
   DIT_CUDA_OK(cudaMemcpyAsync(w.cu_cond_dev, g.cu_cond.data(), (R + 1) * 4, cudaMemcpyHostToDevice, st));
   DIT_CUDA_OK(cudaMemcpyAsync(w.meta_dev, meta.data(), R * sizeof(SeqMeta), cudaMemcpyHostToDevice, st));
@@ -280,6 +333,8 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
     dit_status gs = upload_geom(hd, g, st);
     if (gs != DIT_OK) return gs;
   }
+  struct Strict { bool prev; Strict(bool on) : prev(g_strict_tc) { g_strict_tc = on; } ~Strict() { g_strict_tc = prev; } }
+      strict(dt == DIT_BF16);
   const int32_t* cu_dev = R > 1 ? w.cu_dev : nullptr;
   dit_status s;
 #define RUN(expr)                  \
@@ -578,6 +633,39 @@ dit_status dit_step_host(dit_handle h, const void* latents_host, const float* ti
   return DIT_OK;
 }
 
+dit_status dit_step_varlen_host(dit_handle h, const void* latents_packed_host, const float* timestep_emb_host,
+                                const void* cond_packed_host, const int32_t* cu_seqlens, const int32_t* n_cond,
+                                const int32_t* latent_grids, int32_t n_requests, void* out_packed_host, void* stream) {
+  DIT_REQUIRE(h != nullptr, DIT_ERR_INVALID_ARG, "handle is NULL");
+  DIT_REQUIRE(latents_packed_host && timestep_emb_host && latent_grids && out_packed_host, DIT_ERR_INVALID_ARG, "NULL tensor argument");
+  StepGeom g;
+  dit_status s = build_geom(h, n_requests, cu_seqlens, n_cond, latent_grids, &g);
+  if (s != DIT_OK) return s;
+  const dit_config& c = h->cfg;
+  const size_t es = esize(c.dtype);
+  cudaStream_t st = (cudaStream_t)stream;
+  const int64_t pvC = (int64_t)c.latent_channels * c.patch[0] * c.patch[1] * c.patch[2];
+  const size_t lat_bytes = (size_t)g.lat_off[n_requests] * es;
+  const size_t temb_bytes = (size_t)n_requests * c.temb_dim * 4;
+  const size_t cond_bytes = (size_t)g.cu_cond[n_requests] * c.cond_dim * es;
+  // the staging area holds max_tokens patches: image tokens of all requests (a latent has exactly N_r * C * pv elements)
+  DIT_REQUIRE(lat_bytes <= (size_t)c.max_tokens * pvC * es, DIT_ERR_WORKSPACE, "packed latents exceed the staging area");
+  char* p = (char*)h->ws.stage_in;
+  char* lat_d = p;
+  char* temb_d = p + align256((size_t)c.max_tokens * pvC * es);
+  char* cond_d = temb_d + align256((size_t)c.max_requests * c.temb_dim * 4);
+  DIT_CUDA_OK(cudaMemcpyAsync(lat_d, latents_packed_host, lat_bytes, cudaMemcpyHostToDevice, st));
+  DIT_CUDA_OK(cudaMemcpyAsync(temb_d, timestep_emb_host, temb_bytes, cudaMemcpyHostToDevice, st));
+  if (cond_bytes) {
+    DIT_REQUIRE(cond_packed_host != nullptr, DIT_ERR_INVALID_ARG, "cond tokens announced but cond pointer is NULL");
+    DIT_CUDA_OK(cudaMemcpyAsync(cond_d, cond_packed_host, cond_bytes, cudaMemcpyHostToDevice, st));
+  }
+  s = run_step(h, g, lat_d, (const float*)temb_d, cond_d, h->ws.stage_out, st);
+  if (s != DIT_OK) return s;
+  DIT_CUDA_OK(cudaMemcpyAsync(out_packed_host, h->ws.stage_out, lat_bytes, cudaMemcpyDeviceToHost, st));
+  return DIT_OK;
+}
+
 dit_status dit_sample(dit_handle h, const void* latents, const float* timestep_embs, const float* sigmas_host,
                       const void* cond_tokens, int32_t n_cond, const void* uncond_tokens, int32_t n_uncond,
                       float guidance_scale, const int32_t latent_grid[3], int32_t n_steps, int32_t use_graph, void* out,
@@ -643,7 +731,8 @@ dit_status dit_sample(dit_handle h, const void* latents, const float* timestep_e
     if (n_steps == 0) return launch_sample_final(c.dtype, w.sample_x, out, n, st);
     return DIT_OK;
   };
-  if (!use_graph || n_steps == 0 || !same_geom || g_prof_mask != 0) return enqueue(st);
+  // no graph while per-class profiling is on (event records are not captured) or a debug stop is set
+  if (!use_graph || n_steps == 0 || !same_geom || g_prof_mask.load() != 0 || h->stop_block >= 0) return enqueue(st);
 
   std::vector<uint64_t> key = {(uint64_t)(uintptr_t)latents, (uint64_t)(uintptr_t)timestep_embs, (uint64_t)(uintptr_t)cond_tokens,
                                (uint64_t)(uintptr_t)uncond_tokens, (uint64_t)(uintptr_t)out, (uint64_t)n_cond, (uint64_t)n_uncond,
@@ -660,7 +749,9 @@ dit_status dit_sample(dit_handle h, const void* latents, const float* timestep_e
     if (h->graph_exec) { cudaGraphExecDestroy(h->graph_exec); h->graph_exec = nullptr; }
     if (h->cap_stream == nullptr) DIT_CUDA_OK(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
     DIT_CUDA_OK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeRelaxed));
+    h->capturing = true;
     s = enqueue(h->cap_stream);
+    h->capturing = false;
     cudaGraph_t graph = nullptr;
     cudaError_t ce = cudaStreamEndCapture(h->cap_stream, &graph);
     if (s != DIT_OK) { if (graph) cudaGraphDestroy(graph); return s; }
@@ -798,6 +889,7 @@ dit_status dit_get_tap(dit_handle h, int32_t tap, void* dst, size_t bytes, void*
 
 dit_status dit_profile_begin(int32_t class_mask) {
   DIT_REQUIRE(class_mask >= 0 && class_mask < (1 << DIT_KC_COUNT), DIT_ERR_INVALID_ARG, "class_mask 0x%x", class_mask);
+  std::lock_guard<std::mutex> lk(g_prof_mu);
   for (auto& r : g_prof_recs) { g_prof_pool.push_back(r.a); g_prof_pool.push_back(r.b); }
   g_prof_recs.clear();
   for (int i = 0; i < DIT_KC_COUNT; ++i) g_prof_counts[i] = 0;
@@ -808,8 +900,10 @@ dit_status dit_profile_begin(int32_t class_mask) {
 dit_status dit_profile_end(float* ms_per_class, int32_t* launches_per_class) {
   DIT_REQUIRE(ms_per_class && launches_per_class, DIT_ERR_INVALID_ARG, "NULL argument");
   g_prof_mask = 0;
+  std::lock_guard<std::mutex> lk(g_prof_mu);
   for (int i = 0; i < DIT_KC_COUNT; ++i) { ms_per_class[i] = 0.f; launches_per_class[i] = g_prof_counts[i]; }
   for (auto& r : g_prof_recs) {
+    if (r.open) { g_prof_pool.push_back(r.a); g_prof_pool.push_back(r.b); continue; }   // a launch that failed mid-way
     DIT_CUDA_OK(cudaEventSynchronize(r.b));
     float ms = 0.f;
     DIT_CUDA_OK(cudaEventElapsedTime(&ms, r.a, r.b));
@@ -821,7 +915,8 @@ dit_status dit_profile_end(float* ms_per_class, int32_t* launches_per_class) {
 }
 
 const char* dit_last_error(dit_handle) { return get_error(); }
-int32_t dit_kernel_launches(void) { return g_launches; }
+int32_t dit_kernel_launches(void) { return g_launches.load(); }
+int32_t dit_fallback_launches(void) { return g_fallback_launches.load(); }
 
 void dit_free(dit_handle h) {
   if (!h) return;

@@ -448,7 +448,7 @@ int sm_count() {
 template <int EPI, int BN>
 dit_status launch_t(const CUtensorMap& ta, const CUtensorMap& tb, const CUtensorMap& tx, const EpiArgs& ep, int M, int N, int K,
                     cudaStream_t st) {
-  static bool attr_set = false;
+  static std::atomic<bool> attr_set{false};
   if (!attr_set) {
     DIT_CUDA_OK(cudaFuncSetAttribute(gemm_tc_kernel<EPI, BN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                      smem_bytes(BN, EPI)));

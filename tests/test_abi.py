@@ -59,9 +59,16 @@ def test_workspace_bytes_and_validation_without_gpu(lib):
     sig = (C.c_float * 2)(1.0, 0.0)
     assert lib.dit_step(None, None, None, None, 0, grid, None, None) == -1
     assert lib.dit_step_host(None, None, None, None, 0, grid, None, None) == -1
+    assert lib.dit_step_varlen_host(None, None, None, None, None, None, grid, 1, None, None) == -1
     assert lib.dit_sample(None, None, None, sig, None, 0, None, 0, 1.0, grid, 1, 0, None, None) == -1
     assert b"handle" in lib.dit_last_error(None)
-    assert lib.dit_kernel_launches() == 0
+    assert lib.dit_kernel_launches() == 0 and lib.dit_fallback_launches() == 0
+    # a bf16 config the tcgen05 kernels cannot serve is refused (no FFMA substitute inside a step), so is a row width
+    # the adaLN kernel is not instantiated for
+    assert lib.dit_workspace_bytes(C.byref(binding.make_config(synth.cfg1(dtype="bf16")))) == 0      # head_dim 64
+    assert b"head_dim 128" in lib.dit_last_error(None)
+    assert lib.dit_workspace_bytes(C.byref(binding.make_config(synth.cfg1(hidden=1792, n_heads=28)))) == 0
+    assert lib.dit_workspace_bytes(C.byref(binding.make_config(synth.cfg2(latent_channels=3)))) == 0  # C*pv = 12
 
 
 def test_missing_library_fails_loudly(tmp_path, monkeypatch):

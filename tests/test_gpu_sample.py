@@ -118,6 +118,21 @@ def test_graph_replay_is_bit_identical_and_recaptures_on_change(lib):
     assert torch.equal(v, v2)
 
 
+def test_packed_guided_cross_graph_with_changing_uncond_count(lib):
+    """Cross-attention, packed guided step (R = 2), CUDA-graph replay: a second trajectory on the SAME handle with the
+    same latents but another number of unconditional tokens changes only the cond-token offsets (cu_cond) — the resident
+    geometry must be refreshed and the graph re-captured, each call matching the oracle."""
+    s = synth.cfg1(cond_mode="cross", rope_dims=(0, 32, 32), qk_rmsnorm=True)
+    W = synth.make_weights(s)
+    m = B.Dit(B.make_config(s, max_requests=2, max_tokens=2 * s.n_tokens, max_cond_tokens=s.n_cond + 32), W, DEV)
+    for n_unc in (16, 32, 8, 16):
+        I, tembs, sigmas, unc = _traj(s, 2, n_unc)
+        ref = O.dit_sample(O.cfg_from_shape(s), W, I["latents"], tembs, sigmas, I["cond"], unc, 3.0)
+        out = m.dit_sample(I["latents"].to(DEV), tembs.to(DEV), sigmas, I["cond"].to(DEV), unc.to(DEV), 3.0, use_graph=True)
+        torch.cuda.synchronize()
+        _check_traj(out, ref, I, torch.float32, f"packed guided cross, n_uncond={n_unc}", 5e-5)
+
+
 def test_zero_steps_and_argument_errors(lib):
     s = synth.cfg1()
     W = synth.make_weights(s)

@@ -176,6 +176,72 @@ def test_varlen_equals_per_request_steps(lib, dtype, mode):
         assert e_rel < (2e-6 if tdt == torch.float32 else 2e-3), f"packing changed request {r}: {e_rel}"
 
 
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+def test_same_handle_cross_mode_changing_cond_counts(lib, dtype):
+    """The geometry resident on the device (cu_seqlens of the cond tokens included) is keyed by EVERY field: a second
+    packed cross-attention call on the same handle with the same latent grids but PERMUTED / changed cond counts
+    (fixed image size, other prompt lengths — the normal serving case) must attend to its own context rows."""
+    base = dict(cond_mode="cross", dtype=dtype, rope_dims=(0, 32, 32), qk_rmsnorm=True, seed=3)
+    if dtype == "bf16":
+        base.update(hidden=512, n_heads=4, head_dim=128, mlp_dim=1024, cond_dim=512, latent_channels=16, rope_dims=(0, 64, 64))
+    grids = [(1, 16, 16), (1, 16, 16)]
+    W = None
+    m = None
+    for nconds in ((5, 7), (7, 5), (20, 20), (10, 10)):
+        shapes = [synth.cfg1(latent_grid=g, n_cond=n, **base) for g, n in zip(grids, nconds)]
+        if W is None:
+            W = synth.make_weights(shapes[0])
+            cfg = B.make_config(shapes[0], max_tokens=sum(sh.n_tokens for sh in shapes), max_requests=2, max_cond_tokens=64)
+            m = B.Dit(cfg, W, DEV)
+        Is = [synth.make_inputs(sh, tag=f"r{r}", t=300.0 + 200 * r) for r, sh in enumerate(shapes)]
+        lats = [i["latents"].to(DEV) for i in Is]
+        temb = torch.cat([i["temb"] for i in Is]).to(DEV)
+        conds = [i["cond"].to(DEV) for i in Is]
+        outs = m.dit_step_varlen(lats, temb, conds)
+        torch.cuda.synchronize()
+        for r in range(2):
+            ref = O.dit_step(O.cfg_from_shape(shapes[r]), W, Is[r]["latents"], Is[r]["temb"], Is[r]["cond"])
+            check(outs[r], ref, shapes[0].torch_dtype, f"n_cond {nconds}, request {r}")
+    assert dtype == "f32" or B.dit_fallback_launches() == 0
+
+
+def test_varlen_host_equals_device_call(lib):
+    """dit_step_varlen_host (host buffers, copies enqueued by the library) == dit_step_varlen, bit for bit."""
+    shapes = [_small_bf16(latent_grid=g, n_cond=n) for g, n in (((1, 12, 20), 9), ((1, 36, 44), 70), ((1, 4, 4), 33))]
+    W = synth.make_weights(shapes[0])
+    Is = [synth.make_inputs(sh, tag=f"h{r}", t=100.0 + 300 * r) for r, sh in enumerate(shapes)]
+    T_total = sum(sh.n_tokens + sh.n_cond for sh in shapes)
+    m = B.Dit(B.make_config(shapes[0], max_tokens=T_total, max_requests=3, max_cond_tokens=sum(sh.n_cond for sh in shapes)), W, DEV)
+    lats = [i["latents"].to(DEV) for i in Is]
+    temb = torch.cat([i["temb"] for i in Is])
+    conds = [i["cond"].to(DEV) for i in Is]
+    outs = m.dit_step_varlen(lats, temb.to(DEV), conds)
+    packed_h = torch.cat([i["latents"].reshape(-1) for i in Is]).pin_memory()
+    cond_h = torch.cat([i["cond"] for i in Is]).pin_memory()
+    out_h = torch.empty_like(packed_h).pin_memory()
+    m.dit_step_varlen_host(packed_h, [i["latents"].shape for i in Is], temb.contiguous().pin_memory(), cond_h,
+                           [sh.n_cond for sh in shapes], out_h)
+    torch.cuda.synchronize()
+    assert torch.equal(out_h, torch.cat([o.reshape(-1) for o in outs]).cpu())
+    assert B.dit_fallback_launches() == 0
+
+
+def test_bf16_step_never_substitutes_the_ffma_kernels(lib):
+    """A bf16 config the tcgen05 kernels cannot serve is refused at dit_init (DIT_ERR_UNSUPPORTED), not run ~100x slower
+    on the fp32-path kernels; the kernel-level entry points do run such shapes and count them."""
+    s = synth.cfg1(dtype="bf16")                                  # head_dim 64
+    with pytest.raises(B.DitError, match="head_dim 128"):
+        B.Dit(B.make_config(s), synth.make_weights(s), DEV)
+    n0 = B.dit_fallback_launches()
+    q, k, v = synth.make_attention_qkv(1, 40, 50, 2, 64, device=DEV)
+    B.dit_attn_partial(q, k, v)
+    A = synth.normal(1, "A", (33, 20), dtype=torch.bfloat16, device=DEV)     # K % 8 != 0
+    Wt = synth.normal(1, "W", (16, 20), dtype=torch.bfloat16, device=DEV)
+    B.dit_linear(A, Wt)
+    torch.cuda.synchronize()
+    assert B.dit_fallback_launches() == n0 + 2
+
+
 def test_argument_validation_on_gpu(lib):
     s = synth.cfg1()
     W, I = synth.make_weights(s), synth.make_inputs(s)
