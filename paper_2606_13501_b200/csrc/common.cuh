@@ -238,10 +238,11 @@ dit_status launch_gemm_tc(int epi, const void* A, int64_t lda, const void* W, co
 dit_status launch_gemm_tc_ex(int epi, const void* A, int64_t lda, const void* W, const void* bias, void* out, int64_t ldo,
                              const float* gate, int64_t gate_stride, const int32_t* cu, int R, int M, int N, int K,
                              cudaStream_t st);
-// QKV projection + QK-RMSNorm + RoPE in one kernel (bf16, head_dim 128): out [M, 3D] holds normalised, rotated q | k and v
+// Projection + QK-RMSNorm + RoPE in one kernel (bf16, head_dim 128): out [M, N] holds normalised, rotated q heads in columns
+// [0, q_end), k heads in [q_end, k_end), plain v heads behind them (self-attention: D, 2D, N = 3D)
 dit_status launch_gemm_tc_qkv(const void* A, int64_t lda, const void* W, const void* bias, void* out, int64_t ldo,
-                              const void* gq, const void* gk, float rms_eps, const float* rc, const float* rs, int D, int M,
-                              int N, int K, cudaStream_t st);
+                              const void* gq, const void* gk, float rms_eps, const float* rc, const float* rs, int q_end,
+                              int k_end, int M, int N, int K, cudaStream_t st);
 bool gemm_tc_supported(int epi, const void* A, int64_t lda, const void* W, void* out, int64_t ldo, int M, int N, int K);
 
 // Attention over packed sequences.  q rows [cu_q[r], cu_q[r+1]) attend to k/v rows [cu_k[r], cu_k[r+1])

@@ -289,8 +289,11 @@ static dit_status upload_geom(dit_handle hd, const StepGeom& g, cudaStream_t st)
     meta[r].lat_off_lo = (int32_t)(g.lat_off[r] & 0xffffffff);
     meta[r].lat_off_hi = (int32_t)(g.lat_off[r] >> 32);
     meta[r].pad = 0;
-    geom.insert(geom.end(), {meta[r].seq_start, g.ncond[r], g.cu_cond[r + 1], meta[r].gf, meta[r].gh, meta[r].gw,
-                             meta[r].lat_off_lo, meta[r].lat_off_hi});
+    // (one cross / cond-less request: no kernel reads the cond offsets, so the two passes of an unpacked guided step
+    // with different prompt lengths share one resident geometry and stay capturable)
+    const bool cond_used = joint || R > 1;
+    geom.insert(geom.end(), {meta[r].seq_start, cond_used ? g.ncond[r] : 0, cond_used ? g.cu_cond[r + 1] : 0, meta[r].gf,
+                             meta[r].gh, meta[r].gw, meta[r].lat_off_lo, meta[r].lat_off_hi});
   }
   geom.push_back(T);
   geom.push_back(R);
@@ -385,7 +388,7 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
       // QK-RMSNorm + RoPE on the fp32 accumulators in the QKV GEMM's epilogue (north_star subsystems 3 + 4)
       RUN(launch_gemm_tc_qkv(w.y, D, b.wqkv, b.bqkv, w.qkv, 3 * D, c.qk_rmsnorm ? b.gq : nullptr,
                              c.qk_rmsnorm ? b.gk : nullptr, c.rms_eps, rope ? w.rope_c : nullptr,
-                             rope ? w.rope_s : nullptr, D, T, 3 * D, D, st));
+                             rope ? w.rope_s : nullptr, D, 2 * D, T, 3 * D, D, st));
     } else {
       RUN(gemm(dt, DIT_EPI_BIAS, w.y, D, b.wqkv, b.bqkv, w.qkv, 3 * D, T, 3 * D, D, st));
       RUN(launch_qknorm_rope(dt, w.qkv, 3 * D, T, H, d, 2, c.qk_rmsnorm ? b.gq : nullptr, c.qk_rmsnorm ? b.gk : nullptr,
@@ -421,11 +424,23 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
     if (stop(l, DIT_STAGE_OPROJ)) return DIT_OK;
     if (cross) {  // R10: x <- x + Wo_c Attn(RMS(Wq_c LN(x)), RMS(Wk_c ctx), Wv_c ctx) + bo_c   (no gate, no modulation)
       RUN(launch_adaln(dt, w.x, nullptr, nullptr, nullptr, nullptr, mod_stride, cu_dev, R, w.y, T, D, c.ln_eps, st));
-      RUN(gemm(dt, DIT_EPI_BIAS, w.y, D, b.cwq, b.cbq, w.qkv, D, T, D, D, st));
-      RUN(launch_qknorm_rope(dt, w.qkv, D, T, H, d, 1, b.cgq, nullptr, c.rms_eps, nullptr, nullptr, st));
+      // bf16: the per-head RMSNorm of the cross q / k runs on the fp32 accumulators of their projections (one bf16
+      // rounding instead of two, and no stand-alone pass over [T, D]); fp32 path: stand-alone kernel
+      const bool fused = dt == DIT_BF16 && d == 128 && gemm_tc_supported(DIT_EPI_BIAS, w.y, D, b.cwq, w.qkv, D, T, D, D);
+      if (fused) {
+        RUN(launch_gemm_tc_qkv(w.y, D, b.cwq, b.cbq, w.qkv, D, b.cgq, nullptr, c.rms_eps, nullptr, nullptr, D, D, T, D, D, st));
+      } else {
+        RUN(gemm(dt, DIT_EPI_BIAS, w.y, D, b.cwq, b.cbq, w.qkv, D, T, D, D, st));
+        RUN(launch_qknorm_rope(dt, w.qkv, D, T, H, d, 1, b.cgq, nullptr, c.rms_eps, nullptr, nullptr, st));
+      }
       if (Lc_total > 0) {
-        RUN(gemm(dt, DIT_EPI_BIAS, w.ctx, D, b.cwkv, b.cbkv, w.kvc, 2 * D, Lc_total, 2 * D, D, st));
-        RUN(launch_qknorm_rope(dt, w.kvc, 2 * D, Lc_total, H, d, 1, b.cgk, nullptr, c.rms_eps, nullptr, nullptr, st));
+        if (fused) {
+          RUN(launch_gemm_tc_qkv(w.ctx, D, b.cwkv, b.cbkv, w.kvc, 2 * D, nullptr, b.cgk, c.rms_eps, nullptr, nullptr, 0, D,
+                                 Lc_total, 2 * D, D, st));
+        } else {
+          RUN(gemm(dt, DIT_EPI_BIAS, w.ctx, D, b.cwkv, b.cbkv, w.kvc, 2 * D, Lc_total, 2 * D, D, st));
+          RUN(launch_qknorm_rope(dt, w.kvc, 2 * D, Lc_total, H, d, 1, b.cgk, nullptr, c.rms_eps, nullptr, nullptr, st));
+        }
       }
       AttnArgs a;
       a.q = w.qkv; a.q_stride = D;
@@ -825,8 +840,8 @@ dit_status dit_linear_qkv(int32_t dtype, const void* A, int64_t lda, const void*
   DIT_REQUIRE(dtype == DIT_BF16 && hidden % 128 == 0 &&
                   gemm_tc_supported(DIT_EPI_BIAS, A, lda, W, out, ldo, M > 0 ? M : 1, 3 * hidden, K),
               DIT_ERR_UNSUPPORTED, "dit_linear_qkv: bf16, head_dim 128, 16-byte aligned operands, sm_100 only");
-  return launch_gemm_tc_qkv(A, lda, W, bias, out, ldo, g_q, g_k, rms_eps, rope_cos, rope_sin, hidden, M, 3 * hidden, K,
-                            (cudaStream_t)stream);
+  return launch_gemm_tc_qkv(A, lda, W, bias, out, ldo, g_q, g_k, rms_eps, rope_cos, rope_sin, hidden, 2 * hidden, M,
+                            3 * hidden, K, (cudaStream_t)stream);
 }
 
 dit_status dit_adaln(int32_t dtype, float* x, const void* h, const float* gate, const float* shift, const float* scale,

@@ -96,11 +96,13 @@ struct EpiArgs {
   int64_t gate_stride;
   const int32_t* cu;      // row -> request (nullptr: one request)
   int R;
-  // EPI_QKV_NORM_ROPE (head_dim 128): columns [0, D) = q heads, [D, 2D) = k heads, [2D, 3D) = v heads
+  // EPI_QKV_NORM_ROPE (head_dim 128): columns [0, q_end) = q heads, [q_end, k_end) = k heads, [k_end, N) = v heads
+  // (self-attention: q_end = D, k_end = 2D; cross-attention q projection: q_end = k_end = N; cross k | v: q_end = 0,
+  // k_end = D)
   const bf16* gq; const bf16* gk;   // RMSNorm gains [128] (nullptr: no norm)
   const float* rc; const float* rs; // RoPE tables [M, 64] (nullptr: no RoPE)
   float rms_eps;
-  int D;
+  int q_end, k_end;
 };
 
 __device__ __forceinline__ float gelu_tanh_fast(float z) {
@@ -288,7 +290,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         for (int hh = 0; hh < BN / 128; ++hh) {
           const int nh = n0 + hh * 128;
           if (nh >= N) break;  // warp-uniform
-          const int which = nh / ep.D;                         // 0 = q, 1 = k, 2 = v
+          const int which = nh < ep.q_end ? 0 : (nh < ep.k_end ? 1 : 2);   // 0 = q, 1 = k, 2 = v
           const bool norm = which < 2 && (which == 0 ? ep.gq : ep.gk) != nullptr;
           const bool rope = which < 2 && rcr != nullptr;
           const float* const sg = s_gate + (which == 1 ? 128 : 0);
@@ -506,7 +508,7 @@ dit_status launch_gemm_tc_ex(int epi, const void* A, int64_t lda, const void* W,
   const int bn = pick_bn(M, N);
   DIT_REQUIRE(make_tmap_2d_bf16(&ta, A, M, K, lda, BM, BK) && make_tmap_2d_bf16(&tb, W, N, K, K, bn / 2, BK), DIT_ERR_CUDA,
               "gemm_tc: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d lda=%lld)", M, N, K, (long long)lda);
-  EpiArgs ep{(const bf16*)bias, out, ldo, gate, gate_stride, cu, R, nullptr, nullptr, nullptr, nullptr, 0.f, 0};
+  EpiArgs ep{(const bf16*)bias, out, ldo, gate, gate_stride, cu, R, nullptr, nullptr, nullptr, nullptr, 0.f, 0, 0};
   ProfScope _prof(DIT_KC_GEMM, st);
   switch (epi) {
     case DIT_EPI_BIAS: return launch_bn<DIT_EPI_BIAS>(bn, ta, tb, ta, ep, M, N, K, st);
@@ -521,17 +523,19 @@ dit_status launch_gemm_tc_ex(int epi, const void* A, int64_t lda, const void* W,
   }
 }
 
-// QKV projection with QK-RMSNorm + RoPE in the epilogue (head_dim 128; N = 3 D, D % 128 == 0).  256-wide tiles only:
-// a tile is two whole heads.
+// Projection with QK-RMSNorm + RoPE in the epilogue (head_dim 128): columns [0, q_end) are q heads (gain gq), [q_end, k_end)
+// k heads (gain gk), the rest v heads (bias only); q_end, k_end, N multiples of 128.  256-wide tiles only: a tile is two
+// whole heads.  Self-attention QKV: (D, 2D, N = 3D); cross-attention q: (D, D, N = D); cross-attention k | v: (0, D, N = 2D).
 dit_status launch_gemm_tc_qkv(const void* A, int64_t lda, const void* W, const void* bias, void* out, int64_t ldo,
-                              const void* gq, const void* gk, float rms_eps, const float* rc, const float* rs, int D, int M,
-                              int N, int K, cudaStream_t st) {
+                              const void* gq, const void* gk, float rms_eps, const float* rc, const float* rs, int q_end,
+                              int k_end, int M, int N, int K, cudaStream_t st) {
   if (M == 0 || N == 0) return DIT_OK;
-  DIT_REQUIRE(D % 128 == 0 && N == 3 * D, DIT_ERR_INVALID_ARG, "gemm_tc_qkv: N=%d D=%d", N, D);
+  DIT_REQUIRE(q_end % 128 == 0 && k_end % 128 == 0 && N % 128 == 0 && 0 <= q_end && q_end <= k_end && k_end <= N,
+              DIT_ERR_INVALID_ARG, "gemm_tc_qkv: N=%d q_end=%d k_end=%d", N, q_end, k_end);
   CUtensorMap ta, tb;
   DIT_REQUIRE(make_tmap_2d_bf16(&ta, A, M, K, lda, BM, BK) && make_tmap_2d_bf16(&tb, W, N, K, K, 128, BK), DIT_ERR_CUDA,
               "gemm_tc_qkv: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d)", M, N, K);
-  EpiArgs ep{(const bf16*)bias, out, ldo, nullptr, 0, nullptr, 1, (const bf16*)gq, (const bf16*)gk, rc, rs, rms_eps, D};
+  EpiArgs ep{(const bf16*)bias, out, ldo, nullptr, 0, nullptr, 1, (const bf16*)gq, (const bf16*)gk, rc, rs, rms_eps, q_end, k_end};
   ProfScope _prof(DIT_KC_GEMM, st);
   return launch_t<EPI_QKV_NORM_ROPE, 256>(ta, tb, ta, ep, M, N, K, st);
 }

@@ -150,6 +150,8 @@ def test_varlen_equals_per_request_steps(lib, dtype, mode):
     """Packing invariance (§8(c) step 8): the packed result for request r == dit_step on request r alone, and
     both match the oracle.  Heterogeneous grids and cond lengths, per-request timesteps."""
     base = dict(cond_mode=mode, dtype=dtype, rope_dims=(0, 32, 32), qk_rmsnorm=True, seed=7)
+    if dtype == "bf16":   # a bf16 step runs on the tcgen05 kernels only: head_dim 128
+        base.update(hidden=512, n_heads=4, head_dim=128, mlp_dim=1024, cond_dim=512, latent_channels=16, rope_dims=(0, 64, 64))
     grids = [(1, 8, 8), (1, 32, 20), (1, 16, 48), (1, 2, 2)]
     nconds = [5, 32, 0, 17]
     ts = [float(synth.uniform01(7, f"t{r}", 1)[0]) * 1000 for r in range(4)]
@@ -187,6 +189,7 @@ def test_same_handle_cross_mode_changing_cond_counts(lib, dtype):
     grids = [(1, 16, 16), (1, 16, 16)]
     W = None
     m = None
+    n0 = B.dit_fallback_launches()
     for nconds in ((5, 7), (7, 5), (20, 20), (10, 10)):
         shapes = [synth.cfg1(latent_grid=g, n_cond=n, **base) for g, n in zip(grids, nconds)]
         if W is None:
@@ -202,7 +205,7 @@ def test_same_handle_cross_mode_changing_cond_counts(lib, dtype):
         for r in range(2):
             ref = O.dit_step(O.cfg_from_shape(shapes[r]), W, Is[r]["latents"], Is[r]["temb"], Is[r]["cond"])
             check(outs[r], ref, shapes[0].torch_dtype, f"n_cond {nconds}, request {r}")
-    assert dtype == "f32" or B.dit_fallback_launches() == 0
+    assert B.dit_fallback_launches() == n0
 
 
 def test_varlen_host_equals_device_call(lib):
@@ -212,6 +215,7 @@ def test_varlen_host_equals_device_call(lib):
     Is = [synth.make_inputs(sh, tag=f"h{r}", t=100.0 + 300 * r) for r, sh in enumerate(shapes)]
     T_total = sum(sh.n_tokens + sh.n_cond for sh in shapes)
     m = B.Dit(B.make_config(shapes[0], max_tokens=T_total, max_requests=3, max_cond_tokens=sum(sh.n_cond for sh in shapes)), W, DEV)
+    n0 = B.dit_fallback_launches()
     lats = [i["latents"].to(DEV) for i in Is]
     temb = torch.cat([i["temb"] for i in Is])
     conds = [i["cond"].to(DEV) for i in Is]
@@ -223,7 +227,7 @@ def test_varlen_host_equals_device_call(lib):
                            [sh.n_cond for sh in shapes], out_h)
     torch.cuda.synchronize()
     assert torch.equal(out_h, torch.cat([o.reshape(-1) for o in outs]).cpu())
-    assert B.dit_fallback_launches() == 0
+    assert B.dit_fallback_launches() == n0
 
 
 def test_bf16_step_never_substitutes_the_ffma_kernels(lib):
