@@ -34,6 +34,7 @@
 // Roofline: tensor pipe; the softmax instruction stream (312 instructions per 64 scores in an optimistic tile, 379 in
 // an exact one; MUFU.EX2 at 16 / clk / SM) is co-critical.
 #include <algorithm>
+#include <cstdlib>
 
 #include "tc.cuh"
 
@@ -593,6 +594,445 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   }
 }
 
+
+// =====================================================================================================================
+// attn_pair_kernel — the same attention on CTA PAIRS (cta_group::2), ONE 256-row Q tile per pair, S and P in separate
+// tensor-memory buffers.
+//
+// Why.  In attn_tc_kernel a CTA holds two Q tiles and TMEM is full with S0 S1 O0 O1; P(j) overwrites S(j), so S(j+1) of
+// a tile cannot be queued before PV(j) of the same tile: the chain S -> softmax -> PV of a tile is hidden only by the
+// other tile's 1024 tensor cycles.  Measured: the softmax warps wait for S 41 % of the time, tensor pipe 56-62 % busy.
+// Here a CTA owns 128 Q rows only and TMEM is  S[0] S[1] | P[0] P[1] | O  (2 x 128 + 2 x 64 + 128 columns):
+//   * an S buffer is free again as soon as the softmax warps have READ it (a few hundred cycles into the tile), not when
+//     PV has consumed P: the issuer queues S(j+2) long before P(j) exists, and no softmax warp ever waits for S;
+//   * P(j) is handed over at the end of the tile; PV(j) then has a whole tile time before P(j+2) needs the buffer.
+// (A first version with three S buffers and P aliased over S — S(0) S(1) S(2) | PV(0) S(3) | ... — ran at 71 % tensor
+//  utilisation: each buffer cycles through S, softmax, hand-off, PV, and three buffers per 4300-cycle cycle give one
+//  tile per 1440 cycles; profiles/r02_ncu_attn_pair.md.)
+// A single CTA cannot feed this from shared memory (S alone reads A + B = 8 KB per 64-cycle MMA = the whole 128 B/clk
+// port, and the K / V stream is written on top); on a pair each CTA supplies its own 128 Q rows and HALF of every K / V
+// tile (S: 64 keys; PV: 64 of the 128 d columns): 96 / 32 B/clk of operand reads + 32 B/clk of TMA writes.
+//   warp 0      K producer (+ Q once): this CTA's 64 keys of every key tile (two [64 x 64] boxes), 5-deep ring
+//   warp 2      V producer: this CTA's 64 d-columns of every key tile (one [128 x 64] box), 4-deep ring; TMEM allocation
+//               (every box of both CTAs completes on the LEADER's full barrier; a stage is refilled when the leader's
+//               commit, multicast to both CTAs, says the MMAs have read it)
+//   warp 1      (leader CTA) one elected thread issues every MMA for both tensor cores, in the order the events arrive:
+//               S(0) S(1) | S(2) PV(0) | S(3) PV(1) | ...   S(j) = Q K_j^T, M = 256, N = 128 keys, K = 16 x 8, into
+//               S[j & 1] once the softmax has read S(j-2);  O += P(j) V_j, M = 256, N = 128 (d), K = 16 x 8, P[j & 1]
+//               from tensor memory, V MN-major
+//   warps 4-19  softmax, two groups of 8 warps in anti-phase: group g owns key tiles j = g (mod 2), S[g] and P[g]; the
+//               leader warp of a TMEM lane quadrant takes keys 0..63 of the tile, the follower keys 64..127 (one thread =
+//               one query row x 64 keys).  Events of BOTH CTAs are counted by the leader's barriers (relaxed remote
+//               arrive from the peer, ~210 cycles, off the issuing warp).
+// Reference (R33, simplified): P, the row sum and O are expressed against ONE reference m per row for the whole pass
+// (divided out at the end: any m is exact while nothing overflows).  Pass 0 takes m = row max of the first key tile and
+// never moves it; a tile sum above 2^60 (a score ~2^60 above m) raises the pair's panic flag, and the pair then runs
+// pass 1 = row max over ALL key tiles (S MMAs only) and pass 2 = pass 0's loop with the true max as reference (the
+// textbook two-pass softmax; cannot overflow).  O is never rescaled inside a pass.
+// =====================================================================================================================
+constexpr int PKS = 5, PVS = 4;                 // K / V ring depths
+constexpr int PQ_BYTES = TQ * HD * 2;           // this CTA's 128 Q rows: two [128 x 64] boxes
+constexpr int PQ_HALF = PQ_BYTES / 2;
+constexpr int PKV_BYTES = 64 * HD * 2;          // a K stage (64 keys x 128 d: two [64 x 64] boxes) or a V stage ([128 keys x 64 d])
+constexpr int PK_HALF = PKV_BYTES / 2;
+constexpr int PAIR_BAR_BYTES = 512;
+constexpr int PAIR_XCH_FLOATS = 2 * 128 + 128 + 4 * 128;   // pair max exchange | published reference | 4-way reduce
+constexpr int PAIR_SMEM = PQ_BYTES + (PKS + PVS) * PKV_BYTES + 1024 + PAIR_BAR_BYTES + PAIR_XCH_FLOATS * 4;
+constexpr uint32_t TM_S = 0, TM_P = 256, TM_O = 384;       // TMEM columns: S[g] = g * 128, P[g] = 256 + g * 64, O = 384
+#ifndef DIT_ATTN_RELAXED_ARRIVE
+#define DIT_ATTN_RELAXED_ARRIVE 1
+#endif
+
+// p = 2^(s c + nm) for 32 scores -> 16 packed bf16 pairs in pk; packed fp32 partial sums
+__device__ __forceinline__ void exp_pack(const uint32_t (&s)[32], uint64_t c2, uint64_t nm2, uint32_t (&pk)[16],
+                                         uint64_t& sum2, uint64_t& sum2b) {
+#pragma unroll
+  for (int i = 0; i < 16; ++i) {
+    const uint64_t x = fma2(pack2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1])), c2, nm2);
+    float a, b;
+    if (i % 4 == 3 && i / 4 < POLY_PAIRS) {   // spread over the chunk so MUFU and FMA work interleave
+      ex2_poly2(x, a, b);
+    } else {
+      float xa, xb;
+      unpack2(x, xa, xb);
+      a = ex2(xa);
+      b = ex2(xb);
+    }
+    if (i & 1) sum2b = add2(sum2b, pack2(a, b));   // two independent chains
+    else sum2 = add2(sum2, pack2(a, b));
+    pk[i] = pack_bf16(a, b);
+  }
+}
+
+__global__ void __launch_bounds__(ATTN_THREADS, 1)
+attn_pair_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
+                 const __grid_constant__ CUtensorMap tmV, AttnParams p) {
+  pdl_trigger();
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t sQ = smem0, sK = sQ + PQ_BYTES, sV = sK + PKS * PKV_BYTES;
+  const uint32_t bar0 = sV + PVS * PKV_BYTES;
+  auto q_full = [&]() { return bar0; };
+  auto k_full = [&](int s) { return bar0 + 8u * (1 + s); };
+  auto k_empty = [&](int s) { return bar0 + 8u * (1 + PKS + s); };
+  auto v_full = [&](int s) { return bar0 + 8u * (1 + 2 * PKS + s); };
+  auto v_empty = [&](int s) { return bar0 + 8u * (1 + 2 * PKS + PVS + s); };
+  constexpr int B0 = 1 + 2 * PKS + 2 * PVS;
+  auto s_full = [&](int g) { return bar0 + 8u * (B0 + g); };        // S[g] complete (leader's commit, both CTAs)
+  auto s_free = [&](int g) { return bar0 + 8u * (B0 + 2 + g); };    // S[g] read by all its softmax warps (leader CTA only)
+  auto p_full = [&](int g) { return bar0 + 8u * (B0 + 4 + g); };    // P[g] written by all its softmax warps (leader CTA only)
+  auto pv_done = [&](int g) { return bar0 + 8u * (B0 + 6 + g); };   // the PV that read P[g] has completed (both CTAs)
+  auto o_done = [&]() { return bar0 + 8u * (B0 + 8); };
+  const uint32_t tmem_slot = bar0 + 8u * (B0 + 9);
+  const uint32_t panic_addr = bar0 + 8u * (B0 + 10);
+  static_assert(8 * (B0 + 11) <= PAIR_BAR_BYTES, "barrier area");
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t crank = cluster_ctarank();
+  const bool leader_cta = crank == 0;
+  const int req = p.cu_q ? p.order[blockIdx.z] : 0, head = blockIdx.y;
+  const int q_lo = p.cu_q ? p.cu_q[req] : 0, q_hi = p.cu_q ? p.cu_q[req + 1] : p.n_q;
+  const int q_pair = q_lo + (int)(blockIdx.x >> 1) * (2 * TQ);   // first row of the pair's 256-row block
+  if (q_pair >= q_hi) return;                                    // pair-uniform: before any cluster-wide step
+  const int q_base = q_pair + (int)crank * TQ;                   // this CTA's 128 rows (may lie past q_hi: nothing stored)
+  const int k_lo0 = p.cu_k ? p.cu_k[req] : 0, k_hi0 = p.cu_k ? p.cu_k[req + 1] : p.n_k;
+  const int klen = k_hi0 - k_lo0;
+  const int ssz = (klen + p.n_shards - 1) / p.n_shards;
+  int k_lo = k_lo0 + p.shard * ssz, k_hi = k_lo0 + (p.shard + 1) * ssz;
+  if (k_lo > k_hi0) k_lo = k_hi0;
+  if (k_hi > k_hi0) k_hi = k_hi0;
+  const int kv_len = k_hi - k_lo;
+  const int n_tiles = (kv_len + TK - 1) / TK;
+
+  if (n_tiles == 0) {  // empty shard: o = 0, lse = -inf (R18)
+    pdl_wait();
+    if (warp >= 4 && warp < 8) {
+      const int row = q_base + (warp & 3) * 32 + lane;
+      if (row < q_hi) {
+        const float z[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        for (int c = 0; c < HD; c += 8) st8<bf16>(p.o + (int64_t)row * p.o_stride + head * HD + c, z);
+        if (p.lse) p.lse[(int64_t)row * p.H + head] = -INFINITY;
+      }
+    }
+    return;
+  }
+
+  if (warp == 0 && lane == 0) {
+    tma_prefetch_desc(&tmQ);
+    tma_prefetch_desc(&tmK);
+    tma_prefetch_desc(&tmV);
+  }
+  if (warp == 1 && lane == 0) {
+    mbar_init(q_full(), 1);
+    for (int s = 0; s < PKS; ++s) { mbar_init(k_full(s), 1); mbar_init(k_empty(s), 1); }
+    for (int s = 0; s < PVS; ++s) { mbar_init(v_full(s), 1); mbar_init(v_empty(s), 1); }
+    for (int g = 0; g < 2; ++g) {
+      mbar_init(s_full(g), 1);
+      mbar_init(s_free(g), 16);          // 8 warps of the owning group in each CTA
+      mbar_init(p_full(g), 16);
+      mbar_init(pv_done(g), 1);
+    }
+    mbar_init(o_done(), 1);
+    asm volatile("st.shared.u32 [%0], %1;" ::"r"(panic_addr), "r"(0u) : "memory");
+    fence_barrier_init();
+  }
+  if (warp == 2) tmem_alloc_pair<512>(tmem_slot);
+  tc_fence_before();
+  __syncthreads();
+  cluster_sync_all();   // the peer's barriers exist before anything arrives on them
+  tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+  pdl_wait();           // prologue done; q / k / v written by the previous kernel are read from here on
+
+  // Does pass 0 stand?  Every thread of both CTAs calls this at the end of pass 0.
+  auto pair_panicked = [&]() -> bool {
+    tc_fence_before();
+    cluster_sync_all();
+    tc_fence_after();
+    uint32_t mine, peer;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(mine) : "r"(panic_addr) : "memory");
+    asm volatile("ld.shared::cluster.u32 %0, [%1];" : "=r"(peer) : "r"(mapa_cluster(panic_addr, crank ^ 1u)) : "memory");
+    return (mine | peer) != 0;
+  };
+  // pass 0: reference = row max of key tile 0;  pass 1 (after a panic): row max over all key tiles, S only;  pass 2: as
+  // pass 0 with the reference given.  Use counters of rings, buffers and barriers run on across passes.
+  const int c0 = head * HD;
+  if (warp < 4) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");   // 128 x 56 + 512 x 104 <= 640 x 96
+    int kc = 0, vc = 0;            // K / V tiles produced or consumed so far (all passes)
+    int su0 = 0, su1 = 0;          // S tiles issued into S[0] / S[1] so far
+    int pu0 = 0, pu1 = 0;          // PVs issued from P[0] / P[1] so far
+    for (int pass = 0;; ++pass) {
+      const bool with_pv = pass != 1;
+      if (warp == 0) {
+        // ===================================================== K producer (+ Q once)
+        const uint32_t lead_q = mapa_cluster(q_full(), 0);
+        if (pass == 0 && elect_one()) {
+          if (leader_cta) mbar_expect_tx(q_full(), 2 * PQ_BYTES);
+          tma_load_2d_pair(sQ, &tmQ, c0, q_base, lead_q);
+          tma_load_2d_pair(sQ + PQ_HALF, &tmQ, c0 + 64, q_base, lead_q);
+        }
+        for (int j = 0; j < n_tiles; ++j, ++kc) {
+          const int s = kc % PKS;
+          mbar_wait_poll(k_empty(s), (uint32_t)((kc / PKS) & 1) ^ 1u);
+          if (elect_one()) {
+            const uint32_t fb = mapa_cluster(k_full(s), 0);
+            if (leader_cta) mbar_expect_tx(k_full(s), 2 * PKV_BYTES);
+            const int r0 = k_lo + j * TK + (int)crank * 64;      // this CTA's 64 keys of the tile
+            tma_load_2d_pair(sK + s * PKV_BYTES, &tmK, c0, r0, fb);
+            tma_load_2d_pair(sK + s * PKV_BYTES + PK_HALF, &tmK, c0 + 64, r0, fb);
+          }
+          __syncwarp();
+        }
+      } else if (warp == 2) {
+        // ===================================================== V producer
+        if (with_pv) {
+          for (int j = 0; j < n_tiles; ++j, ++vc) {
+            const int s = vc % PVS;
+            mbar_wait_poll(v_empty(s), (uint32_t)((vc / PVS) & 1) ^ 1u);
+            if (elect_one()) {
+              const uint32_t fb = mapa_cluster(v_full(s), 0);
+              if (leader_cta) mbar_expect_tx(v_full(s), 2 * PKV_BYTES);
+              tma_load_2d_pair(sV + s * PKV_BYTES, &tmV, c0 + (int)crank * 64, k_lo + j * TK, fb);   // 64 of the 128 d columns
+            }
+            __syncwarp();
+          }
+        }
+      } else if (warp == 1 && leader_cta) {
+        // ===================================================== MMA issuer for the pair
+        constexpr uint32_t idesc_s = idesc_bf16(2 * TQ, TK, 0, 0);   // S = Q K^T: M = 256, N = 128 keys
+        constexpr uint32_t idesc_o = idesc_bf16(2 * TQ, HD, 0, 1);   // O += P V: A from TMEM, B (V) MN-major, N = 128 (d)
+        constexpr uint64_t vdesc_hi = desc_base_sw128(1, 64);        // one 128-byte atom wide (64 d), 8-key groups 1 KB apart
+        // S of the next key tile into S[g]; the buffer's previous contents have been read (s_free)
+        auto issue_s = [&](int g) {
+          const int su = g ? su1 : su0;
+          if (su > 0) mbar_wait_poll(s_free(g), (uint32_t)(su - 1) & 1u);
+          const int s = kc % PKS;
+          mbar_wait_poll(k_full(s), (uint32_t)(kc / PKS) & 1u);
+          tc_fence_after();
+          if (elect_one()) {
+            const uint32_t d = tmem_base + TM_S + g * 128;
+            const uint32_t ka = sK + s * PKV_BYTES;
+#pragma unroll
+            for (int k = 0; k < HD / 16; ++k)
+              umma_ss_pair(d, desc_kmajor_sw128(sQ + (k >> 2) * PQ_HALF + (k & 3) * 32),
+                           desc_kmajor_sw128(ka + (k >> 2) * PK_HALF + (k & 3) * 32), idesc_s, k != 0);
+            umma_commit_pair(s_full(g), (uint16_t)3);
+            umma_commit_pair(k_empty(s), (uint16_t)3);
+          }
+          __syncwarp();
+          ++kc;
+          if (g) ++su1; else ++su0;
+        };
+        // O (+)= P(j) V_j from P[j & 1]
+        auto issue_pv = [&](int j) {
+          const int g = j & 1;
+          const int pu = g ? pu1 : pu0;
+          const int vs = vc % PVS;
+          const int nk16 = kv_len - j * TK > SK ? 8 : 4;           // a ragged last tile may have no keys 64..127
+          mbar_wait_poll(v_full(vs), (uint32_t)(vc / PVS) & 1u);
+          mbar_wait_poll(p_full(g), (uint32_t)pu & 1u);
+          tc_fence_after();
+          if (elect_one()) {
+            const uint32_t d = tmem_base + TM_O;
+            const uint32_t pa = tmem_base + TM_P + g * 64;         // bf16 pairs: keys 0..63 in columns 0..31, 64..127 in 32..63
+            const uint32_t va = sV + vs * PKV_BYTES;
+#pragma unroll
+            for (int k = 0; k < 8; ++k)
+              if (k < nk16)
+                umma_ts_pair(d, pa + 8 * k, vdesc_hi | (uint64_t)(((va + k * 2048) >> 4) & 0x3fff), idesc_o, (j != 0 || k != 0) ? 1u : 0u);
+            umma_commit_pair(v_empty(vs), (uint16_t)3);
+            umma_commit_pair(pv_done(g), (uint16_t)3);
+            if (j == n_tiles - 1) umma_commit_pair(o_done(), (uint16_t)3);
+          }
+          __syncwarp();
+          ++vc;
+          if (g) ++pu1; else ++pu0;
+        };
+        if (pass == 0) { mbar_wait_poll(q_full(), 0); tc_fence_after(); }
+        // order = the order the events arrive in: S(j + 2) as soon as S(j) has been read (early in tile j's softmax),
+        // PV(j - 1) when P(j - 1) is complete (the other group, half a period earlier)
+        for (int i = 0; i < 2 && i < n_tiles; ++i) issue_s(i);
+        for (int j = 0; j < n_tiles; ++j) {
+          if (j + 2 < n_tiles) issue_s(j & 1);
+          if (with_pv && j >= 1) issue_pv(j - 1);
+        }
+        if (with_pv) issue_pv(n_tiles - 1);
+      }
+      if (pass == 2) break;
+      if (pass == 0 && !pair_panicked()) break;
+      if (pass == 1) { tc_fence_before(); cluster_sync_all(); tc_fence_after(); }   // pass 1 -> 2 boundary (see the softmax warps)
+    }
+  } else {
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 104;");
+    const int w = warp - 4;
+    const int grp = w >> 3;                        // owns key tiles j = grp (mod 2), S[grp], P[grp]
+    const int h = (w >> 2) & 1;                    // 0: keys 0..63 of the tile (leader), 1: keys 64..127 (follower)
+    const int quad = warp & 3;                     // TMEM lane quadrant of this warp
+    const int r_in = quad * 32 + lane;             // row inside this CTA's Q tile
+    const int row = q_base + r_in;
+    const uint32_t lane_off = (uint32_t)(quad * 32) << 16;
+    const uint32_t s_addr = tmem_base + TM_S + grp * 128 + h * SK + lane_off;    // this thread's 64 scores
+    const uint32_t p_addr = tmem_base + TM_P + grp * 64 + h * 32 + lane_off;     // ... and its 32 columns of P
+    const uint32_t o_addr = tmem_base + TM_O + lane_off;
+    float* const xch = reinterpret_cast<float*>(smem_raw + (bar0 - smem_u32(smem_raw)) + PAIR_BAR_BYTES);
+    float* const m_sh = xch;                       // [h][128]: half-row maxima of key tile 0 (group 0)
+    float* const m_row = xch + 256;                // [128]: the row's reference (log2 units)
+    float* const red = xch + 384;                  // [grp * 2 + h][128]: 4-way reductions (row max of pass 1, row sums)
+    const float c = p.scale_log2;
+    const uint64_t c2 = pack2(c, c);
+    auto arrive = [&](uint32_t bar) {              // one arrival per warp on a barrier of the leader CTA
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) {
+        if (leader_cta) mbar_arrive(bar);
+#if DIT_ATTN_RELAXED_ARRIVE
+        else mbar_arrive_remote_relaxed(bar, 0);
+#else
+        else mbar_arrive_remote(bar, 0);
+#endif
+      }
+    };
+    int us = 0, up = 0;                            // S tiles read / P tiles written by this group so far (all passes)
+    float m_used = 0.f;
+    for (int pass = 0;; ++pass) {
+      if (pass == 1) {
+        // ------------------------------------------ row max over all key tiles (after a panic)
+        float mx = -INFINITY;
+        for (int j = grp; j < n_tiles; j += 2, ++us) {
+          const int valid = kv_len - j * TK - h * SK;
+          if (valid > 0) {
+            uint32_t s0[32], s1[32];
+            mbar_wait(s_full(grp), (uint32_t)us & 1u);
+            tc_fence_after();
+            tmem_ld32(s_addr + 0, s0);
+            tmem_ld32(s_addr + 32, s1);
+            tmem_ld_wait();
+            if (valid < SK) { mask32(s0, valid); mask32(s1, valid - 32); }
+            mx = fmaxf(mx, fmaxf(max32(s0), max32(s1)));
+          }
+          arrive(s_free(grp));
+        }
+        red[(grp * 2 + h) * 128 + r_in] = mx;
+        asm volatile("bar.sync %0, 128;" ::"r"(9 + quad) : "memory");
+        mx = fmaxf(fmaxf(red[r_in], red[128 + r_in]), fmaxf(red[256 + r_in], red[384 + r_in]));
+        m_used = mx * c;                           // c > 0; every row has at least one key
+        asm volatile("bar.sync %0, 128;" ::"r"(9 + quad) : "memory");   // `red` is reused for the row sums
+        tc_fence_before(); cluster_sync_all(); tc_fence_after();        // pass 1 -> 2 boundary
+        continue;
+      }
+      // -------------------------------------------- pass 0 / 2: P, row sums, PV against one reference per row
+      float l = 0.f, tile_worst = 0.f;
+      if (pass == 0 && grp == 1) {                 // the reference comes from group 0's first tile
+        asm volatile("bar.sync %0, 128;" ::"r"(5 + quad) : "memory");
+        m_used = m_row[r_in];
+      }
+      for (int j = grp; j < n_tiles; j += 2, ++us, ++up) {
+        const int valid = kv_len - j * TK - h * SK;    // keys of this half that exist (warp-uniform; <= 0: none)
+        uint32_t s0[32], s1[32];
+        if (pass == 0 && j == 0) {
+          // first key tile: its row max is the reference of the whole pass (group 0 only)
+          float mx = -INFINITY;
+          if (valid > 0) {
+            mbar_wait(s_full(grp), (uint32_t)us & 1u);
+            tc_fence_after();
+            // the second 32 scores only for the row max (re-read after the exchange: a TMEM read is cheaper than 32 more
+            // live registers); the first 32 stay
+            tmem_ld32(s_addr + 32, s1);
+            tmem_ld32(s_addr + 0, s0);
+            tmem_ld_wait();
+            if (valid < SK) { mask32(s0, valid); mask32(s1, valid - 32); }   // -inf before the row max
+            mx = fmaxf(max32(s0), max32(s1));
+          }
+          m_sh[h * 128 + r_in] = mx;
+          asm volatile("bar.sync %0, 64;" ::"r"(1 + quad) : "memory");
+          mx = fmaxf(mx, m_sh[(h ^ 1) * 128 + r_in]);
+          m_used = mx * c;
+          if (h == 0) m_row[r_in] = m_used;
+          __threadfence_block();
+          asm volatile("bar.arrive %0, 128;" ::"r"(5 + quad) : "memory");     // group 1 may read m_row
+          if (valid > 0) {
+            tmem_ld32(s_addr + 32, s1);
+            tmem_ld_wait();
+          }
+          arrive(s_free(grp));
+        } else {
+          if (valid > 0) {
+            mbar_wait(s_full(grp), (uint32_t)us & 1u);
+            tc_fence_after();
+            tmem_ld32(s_addr + 0, s0);
+            tmem_ld32(s_addr + 32, s1);
+            tmem_ld_wait();
+          }
+          arrive(s_free(grp));                     // S[grp] may be overwritten by S(j + 2) from here on
+          if (valid > 0 && valid < SK) mask32(s0, valid);   // -inf -> P = 0
+        }
+        if (valid > 0) {
+          const uint64_t nm2 = pack2(-m_used, -m_used);
+          uint64_t sum2 = pack2(0.f, 0.f), sum2b = pack2(0.f, 0.f);
+          {
+            uint32_t pk[16];
+            exp_pack(s0, c2, nm2, pk, sum2, sum2b);
+            // PV(j - 2) has read P[grp]: it was issued when this group finished tile j - 2, i.e. about half a tile ago
+            if (up > 0) { mbar_wait(pv_done(grp), (uint32_t)(up - 1) & 1u); tc_fence_after(); }
+            tmem_st16(p_addr + 0, pk);
+          }
+          if (valid < SK) mask32(s1, valid - 32);
+          {
+            uint32_t pk[16];
+            exp_pack(s1, c2, nm2, pk, sum2, sum2b);
+            tmem_st16(p_addr + 16, pk);
+          }
+          float sa, sb;
+          unpack2(add2(sum2, sum2b), sa, sb);
+          tile_worst = fmaxf(tile_worst, sa + sb);
+          l += sa + sb;
+          tmem_st_wait();
+        }
+        arrive(p_full(grp));
+      }
+      if (pass == 0 && __any_sync(0xffffffffu, !(tile_worst < 1.152921504606847e18f)) && lane == 0)   // 2^60, inf, NaN
+        asm volatile("st.shared.u32 [%0], %1;" ::"r"(panic_addr), "r"(1u) : "memory");
+      // ---- epilogue: the row's four threads add their partial sums; thread (grp, h) writes d columns (grp * 2 + h) * 32 ..
+      red[(grp * 2 + h) * 128 + r_in] = l;
+      asm volatile("bar.sync %0, 128;" ::"r"(9 + quad) : "memory");
+      l = (red[r_in] + red[128 + r_in]) + (red[256 + r_in] + red[384 + r_in]);
+      mbar_wait(o_done(), pass == 0 ? 0u : 1u);
+      tc_fence_after();
+      const float inv = 1.0f / l;                  // l > 0: the first tile has at least one key
+      const bool row_ok = row < q_hi;
+      {
+        const int cq = (grp * 2 + h) * 32;
+        uint32_t o[32];
+        tmem_ld32(o_addr + cq, o);
+        tmem_ld_wait();
+        if (row_ok) {
+          bf16* orow = p.o + (int64_t)row * p.o_stride + head * HD + cq;
+#pragma unroll
+          for (int g = 0; g < 4; ++g) {
+            float v[8];
+#pragma unroll
+            for (int e = 0; e < 8; ++e) v[e] = __uint_as_float(o[g * 8 + e]) * inv;
+            st8<bf16>(orow + g * 8, v);
+          }
+        }
+      }
+      if (grp == 0 && h == 0 && row_ok && p.lse != nullptr)
+        p.lse[(int64_t)row * p.H + head] = 0.6931471805599453f * (m_used + log2f(l));
+      if (pass == 2) break;
+      if (!pair_panicked()) break;
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  cluster_sync_all();   // no CTA leaves while its peer may still signal its barriers or read its shared memory
+  if (warp == 2) {
+    tc_fence_after();
+    tmem_dealloc_pair<512>(tmem_base);
+  }
+}
+
 }  // namespace
 
 bool attn_tc_supported(const AttnArgs& a) {
@@ -615,8 +1055,13 @@ dit_status launch_attn_tc(const AttnArgs& a, cudaStream_t st) {
   if (!attr_set) {
     DIT_CUDA_OK(cudaFuncSetAttribute(attn_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, ATTN_SMEM));
     DIT_CUDA_OK(cudaFuncSetAttribute(attn_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, ATTN_SMEM));
+    DIT_CUDA_OK(cudaFuncSetAttribute(attn_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, PAIR_SMEM));
     attr_set = true;
   }
+  static const bool use_pair = []() {   // DIT_ATTN_KERNEL=two-tile selects the previous kernel (A / B measurements)
+    const char* e = getenv("DIT_ATTN_KERNEL");
+    return !(e != nullptr && e[0] == 't');
+  }();
   // K / V maps need a valid base even when there are no keys (the kernel then never issues a load)
   const void* kb = a.n_k > 0 ? a.k : a.q;
   const void* vb = a.n_k > 0 ? a.v : a.q;
@@ -625,7 +1070,7 @@ dit_status launch_attn_tc(const AttnArgs& a, cudaStream_t st) {
   CUtensorMap tq, tk, tv;
   const uint64_t cols = (uint64_t)a.H * HD;
   DIT_REQUIRE(make_tmap_2d_bf16(&tq, a.q, a.n_q, cols, a.q_stride, TQ, 64) &&
-                  make_tmap_2d_bf16(&tk, kb, nk_rows, cols, kv_ld, TK, 64) &&
+                  make_tmap_2d_bf16(&tk, kb, nk_rows, cols, kv_ld, use_pair ? 64 : TK, 64) &&
                   make_tmap_2d_bf16(&tv, vb, nk_rows, cols, kv_ld, TK, 64),
               DIT_ERR_CUDA, "attn_tc: cuTensorMapEncodeTiled failed (n_q=%d n_k=%d H=%d)", a.n_q, a.n_k, a.H);
   AttnParams p;
@@ -640,6 +1085,12 @@ dit_status launch_attn_tc(const AttnArgs& a, cudaStream_t st) {
       return a.cu_k_host[x + 1] - a.cu_k_host[x] > a.cu_k_host[y + 1] - a.cu_k_host[y];
     });
   ProfScope _prof(DIT_KC_ATTN, st);
+  if (use_pair) {   // one CTA pair per (256-row query block, head, request)
+    dim3 pgrid(2 * cdiv(max_q, 2 * TQ), a.H, a.cu_q ? a.R : 1);
+    DIT_CUDA_OK(launch_pdl(attn_pair_kernel, pgrid, dim3(ATTN_THREADS), PAIR_SMEM, st, 2, tq, tk, tv, p));
+    DIT_LAUNCH_CHECK();
+    return DIT_OK;
+  }
   dim3 grid(cdiv(max_q, 2 * TQ), a.H, a.cu_q ? a.R : 1);
   // CTA pairs when every request has an even number of 256-row query blocks (each CTA of a pair then has rows)
   // ... and the key sequence is long: measured alone it is neutral from N = 8192 (slower below: the pair runs in

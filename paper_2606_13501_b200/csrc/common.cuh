@@ -203,8 +203,10 @@ struct GemvBatch {      // one per weight matrix of a batched GEMV
 
 dit_status launch_gemv(int dtype, const float* in, const GemvBatch* batches_dev, const GemvBatch* single, int n_batches,
                        int total_rows, float* out, int64_t out_stride, int R, int K, int silu_input, cudaStream_t st);
+// split != 0 (bf16 only): y is [T, 2D] = [hi | lo], y = hi + lo to ~16 bits (the final layer's input, R36)
 dit_status launch_adaln(int dtype, float* x, const void* h, const float* gate, const float* shift, const float* scale,
-                        int64_t mod_stride, const int32_t* cu, int R, void* y, int T, int D, float eps, cudaStream_t st);
+                        int64_t mod_stride, const int32_t* cu, int R, void* y, int T, int D, float eps, cudaStream_t st,
+                        int split = 0);
 dit_status launch_qknorm_rope(int dtype, void* qkv, int64_t row_stride, int T, int H, int d, int n_tensors,
                               const void* gq, const void* gk, float eps, const float* rc, const float* rs,
                               cudaStream_t st);
@@ -232,17 +234,18 @@ dit_status launch_merge(int dtype, const void* const* o_parts, const float* cons
 dit_status launch_gemm_simt(int dtype, int epi, const void* A, int64_t lda, const void* W, const void* bias, void* out,
                             int64_t ldo, int M, int N, int K, cudaStream_t st, const float* gate = nullptr,
                             int64_t gate_stride = 0, const int32_t* cu = nullptr, int R = 1);
+// epi 5 (split): out bf16 [M, 2N] = [hi | lo] of A W^T + bias.  a_split != 0: A is such a [hi | lo] pair, [M, 2K]
 dit_status launch_gemm_tc(int epi, const void* A, int64_t lda, const void* W, const void* bias, void* out, int64_t ldo,
-                          int M, int N, int K, cudaStream_t st);
+                          int M, int N, int K, cudaStream_t st, int a_split = 0);
 // epi 3: the gated residual fused in the epilogue (gate nullptr = 1; cu nullptr = one request)
 dit_status launch_gemm_tc_ex(int epi, const void* A, int64_t lda, const void* W, const void* bias, void* out, int64_t ldo,
                              const float* gate, int64_t gate_stride, const int32_t* cu, int R, int M, int N, int K,
-                             cudaStream_t st);
+                             cudaStream_t st, int a_split = 0);
 // Projection + QK-RMSNorm + RoPE in one kernel (bf16, head_dim 128): out [M, N] holds normalised, rotated q heads in columns
 // [0, q_end), k heads in [q_end, k_end), plain v heads behind them (self-attention: D, 2D, N = 3D)
 dit_status launch_gemm_tc_qkv(const void* A, int64_t lda, const void* W, const void* bias, void* out, int64_t ldo,
                               const void* gq, const void* gk, float rms_eps, const float* rc, const float* rs, int q_end,
-                              int k_end, int M, int N, int K, cudaStream_t st);
+                              int k_end, int M, int N, int K, cudaStream_t st, int a_split = 0);
 bool gemm_tc_supported(int epi, const void* A, int64_t lda, const void* W, void* out, int64_t ldo, int M, int N, int K);
 
 // Attention over packed sequences.  q rows [cu_q[r], cu_q[r+1]) attend to k/v rows [cu_k[r], cu_k[r+1])

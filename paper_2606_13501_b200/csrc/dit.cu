@@ -134,7 +134,7 @@ static bool carve(const dit_config& c, char* base, Workspace* w) {
     return (void*)p;
   };
   w->x = (float*)take(Tm * D * 4);
-  w->y = take(Tm * D * es);
+  w->y = take(Tm * 2 * D * es);   // [Tm, D]; the final adaLN writes [Tm, 2D] = [hi | lo] (bf16, R36)
   w->qkv = take(Tm * 3 * D * es);
   w->o = take(Tm * D * es);
   w->u = take(Tm * F * es);
@@ -145,7 +145,7 @@ static bool carve(const dit_config& c, char* base, Workspace* w) {
   w->rope_s = (float*)take(Tm * (c.head_dim / 2) * 4);
   w->patches = take(Tm * pvC * es);
   w->tok = (float*)take(Tm * pvC * 4);
-  w->ctx = take(c.cond_mode == DIT_COND_CROSS ? Lcm * D * es : 0);
+  w->ctx = take(c.cond_mode == DIT_COND_CROSS ? Lcm * 2 * D * es : 0);   // bf16: [Lcm, 2D] = [hi | lo] (R36)
   w->kvc = take(c.cond_mode == DIT_COND_CROSS ? Lcm * 2 * D * es : 0);
   w->o_part = take(c.split_p > 1 ? (size_t)c.split_p * Tm * D * es : 0);
   w->lse_part = (float*)take(c.split_p > 1 ? (size_t)c.split_p * Tm * c.n_heads * 4 : 0);
@@ -221,11 +221,12 @@ static thread_local bool g_strict_tc = false;
 
 // GEMM dispatch: bf16 -> tcgen05 whenever the shape/alignment allows, else FFMA.  fp32 -> FFMA (no TF32).
 static dit_status gemm(int dtype, int epi, const void* A, int64_t lda, const void* W, const void* bias, void* out,
-                       int64_t ldo, int M, int N, int K, cudaStream_t st, int kc = DIT_KC_GEMM) {
+                       int64_t ldo, int M, int N, int K, cudaStream_t st, int kc = DIT_KC_GEMM, int a_split = 0) {
   struct Override { int prev; Override(int c) : prev(g_prof_class_override) { g_prof_class_override = c; }
                     ~Override() { g_prof_class_override = prev; } } ov(kc == DIT_KC_GEMM ? -1 : kc);
   if (dtype == DIT_BF16 && gemm_tc_supported(epi, A, lda, W, out, ldo, M, N, K))
-    return launch_gemm_tc(epi, A, lda, W, bias, out, ldo, M, N, K, st);
+    return launch_gemm_tc(epi, A, lda, W, bias, out, ldo, M, N, K, st, a_split);
+  DIT_REQUIRE(!a_split && epi <= DIT_EPI_BIAS_F32, DIT_ERR_UNSUPPORTED, "split-bf16 operands exist on the tcgen05 path only");
   if (dtype == DIT_BF16 && M > 0) {
     DIT_STRICT_TC("a GEMM");
     g_fallback_launches++;   // visible through dit_fallback_launches()
@@ -365,13 +366,19 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
                c.cond_dim, st, DIT_KC_MISC));
   }
   const int Lc_total = g.cu_cond[R];
+  // R36: in a bf16 step the cross-attention context and the final layer's input are kept as an unevaluated sum of two
+  // bf16 numbers [hi | lo] (~16 significand bits); their consumer GEMMs read both parts as one A operand of width 2K
+  // against W wrapped along K.  These operands are small (Lc rows; one N = C*pv GEMM), their rounding is not.
+  const bool split = dt == DIT_BF16;
+  const int ctx_ld = split ? 2 * D : D;
   if (cross && Lc_total > 0) {
+    const int cepi = split ? 5 /* EPI_BIAS_SPLIT */ : DIT_EPI_BIAS;
     if (!pair) {
-      RUN(gemm(dt, DIT_EPI_BIAS, cond, c.cond_dim, hd->cp_w, hd->cp_b, w.ctx, D, Lc_total, D, c.cond_dim, st, DIT_KC_MISC));
+      RUN(gemm(dt, cepi, cond, c.cond_dim, hd->cp_w, hd->cp_b, w.ctx, ctx_ld, Lc_total, D, c.cond_dim, st, DIT_KC_MISC));
     } else {
       for (int r = 0; r < R; ++r)
         if (g.ncond[r] > 0)
-          RUN(gemm(dt, DIT_EPI_BIAS, cond_of(r), c.cond_dim, hd->cp_w, hd->cp_b, (char*)w.ctx + (size_t)g.cu_cond[r] * D * es, D,
+          RUN(gemm(dt, cepi, cond_of(r), c.cond_dim, hd->cp_w, hd->cp_b, (char*)w.ctx + (size_t)g.cu_cond[r] * ctx_ld * es, ctx_ld,
                    g.ncond[r], D, c.cond_dim, st, DIT_KC_MISC));
     }
   }
@@ -435,10 +442,10 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
       }
       if (Lc_total > 0) {
         if (fused) {
-          RUN(launch_gemm_tc_qkv(w.ctx, D, b.cwkv, b.cbkv, w.kvc, 2 * D, nullptr, b.cgk, c.rms_eps, nullptr, nullptr, 0, D,
-                                 Lc_total, 2 * D, D, st));
+          RUN(launch_gemm_tc_qkv(w.ctx, ctx_ld, b.cwkv, b.cbkv, w.kvc, 2 * D, nullptr, b.cgk, c.rms_eps, nullptr, nullptr, 0, D,
+                                 Lc_total, 2 * D, D, st, split ? 1 : 0));
         } else {
-          RUN(gemm(dt, DIT_EPI_BIAS, w.ctx, D, b.cwkv, b.cbkv, w.kvc, 2 * D, Lc_total, 2 * D, D, st));
+          RUN(gemm(dt, DIT_EPI_BIAS, w.ctx, ctx_ld, b.cwkv, b.cbkv, w.kvc, 2 * D, Lc_total, 2 * D, D, st, DIT_KC_GEMM, split ? 1 : 0));
           RUN(launch_qknorm_rope(dt, w.kvc, 2 * D, Lc_total, H, d, 1, b.cgk, nullptr, c.rms_eps, nullptr, nullptr, st));
         }
       }
@@ -462,13 +469,15 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
   }
   // ---- step 6: final adaLN (folds the last gated residual), Linear D -> C*pv, unpatchify (image tokens only)
   const float* mf = w.mod + (size_t)L * 6 * D;
-  RUN(launch_adaln(dt, w.x, nullptr, nullptr, mf, mf + D, mod_stride, cu_dev, R, w.y, T, D, c.ln_eps, st));
+  RUN(launch_adaln(dt, w.x, nullptr, nullptr, mf, mf + D, mod_stride, cu_dev, R, w.y, T, D, c.ln_eps, st, split ? 1 : 0));
+  const int y_ld = split ? 2 * D : D;
   for (int r = 0; r < R; ++r) {
     const int Fr = g.grids[3 * r], Hr = g.grids[3 * r + 1], Wr = g.grids[3 * r + 2];
     const int Nr = (Fr / c.patch[0]) * (Hr / c.patch[1]) * (Wr / c.patch[2]);
     const int row0 = g.cu[r] + (joint ? g.ncond[r] : 0);
     float* tk = w.tok + (size_t)row0 * pvC;
-    RUN(gemm(dt, DIT_EPI_BIAS_F32, (char*)w.y + (size_t)row0 * D * es, D, hd->f_w, hd->f_b, tk, pvC, Nr, pvC, D, st, DIT_KC_MISC));
+    RUN(gemm(dt, DIT_EPI_BIAS_F32, (char*)w.y + (size_t)row0 * y_ld * es, y_ld, hd->f_w, hd->f_b, tk, pvC, Nr, pvC, D, st, DIT_KC_MISC,
+             split ? 1 : 0));
     RUN(launch_unpatchify(dt, tk, (char*)out + g.lat_off[r] * es, c.latent_channels, Fr, Hr, Wr, c.patch, st,
                           pair ? pair->epi[r] : epi));
   }

@@ -150,7 +150,7 @@ __global__ void __launch_bounds__(128) adaln_kernel(float* __restrict__ x, const
                                                     const float* __restrict__ gate, const float* __restrict__ shift,
                                                     const float* __restrict__ scale, int64_t mod_stride,
                                                     const int32_t* __restrict__ cu, int R, T* __restrict__ y, int T_rows,
-                                                    float eps) {
+                                                    float eps, int split) {
   pdl_trigger();
   pdl_wait();
   constexpr int D = NCW * WPR * 256;
@@ -213,7 +213,7 @@ __global__ void __launch_bounds__(128) adaln_kernel(float* __restrict__ x, const
   const float rstd = rsqrtf(q * (1.0f / D) + eps);
   const float* sh = shift ? shift + (int64_t)req * mod_stride + col0 : nullptr;
   const float* sc = scale ? scale + (int64_t)req * mod_stride + col0 : nullptr;
-  T* yr = y + (int64_t)row * D + col0;
+  T* yr = y + (int64_t)row * (split ? 2 * D : D) + col0;   // split: row = [hi (D) | lo (D)]
 #pragma unroll
   for (int c = 0; c < NCW; ++c) {
     float o[8], a[8], b[8];
@@ -227,20 +227,26 @@ __global__ void __launch_bounds__(128) adaln_kernel(float* __restrict__ x, const
       o[e] = n;
     }
     if (row_ok) st8<T>(yr + c * 256, o);
+    if (split && row_ok) {   // lo = y - hi, exact in fp32, rounded to T once more
+      float lo[8];
+#pragma unroll
+      for (int e = 0; e < 8; ++e) lo[e] = o[e] - to_f<T>(from_f<T>(o[e]));
+      st8<T>(yr + D + c * 256, lo);
+    }
   }
 }
 
 template <typename T>
 static dit_status launch_adaln_t(float* x, const T* h, const float* gate, const float* shift, const float* scale,
                                  int64_t mod_stride, const int32_t* cu, int R, T* y, int T_rows, int D, float eps,
-                                 cudaStream_t st) {
+                                 cudaStream_t st, int split) {
   if (T_rows == 0) return DIT_OK;
   DIT_REQUIRE(D % 256 == 0 && D <= 6144, DIT_ERR_UNSUPPORTED, "adaln: D=%d must be a multiple of 256 (<= 6144)", D);
   ProfScope _prof(DIT_KC_ADALN, st);
 #define ADALN_CASE(NCV, NCW, WPR)                                                                           \
   case NCV:                                                                                                 \
     DIT_CUDA_OK(launch_pdl(adaln_kernel<T, NCW, WPR>, dim3(cdiv(T_rows, 4 / WPR)), dim3(128), 0, st, 1, x, h, gate, \
-                           shift, scale, mod_stride, cu, R, y, T_rows, eps));                                \
+                           shift, scale, mod_stride, cu, R, y, T_rows, eps, split));                         \
     break;
   switch (D / 256) {   // D / 256 chunks per row = NCW per warp x WPR warps
     ADALN_CASE(1, 1, 1) ADALN_CASE(2, 2, 1) ADALN_CASE(3, 3, 1) ADALN_CASE(4, 4, 1) ADALN_CASE(5, 5, 1)
@@ -255,10 +261,11 @@ static dit_status launch_adaln_t(float* x, const T* h, const float* gate, const 
 }
 
 dit_status launch_adaln(int dtype, float* x, const void* h, const float* gate, const float* shift, const float* scale,
-                        int64_t mod_stride, const int32_t* cu, int R, void* y, int T, int D, float eps, cudaStream_t st) {
+                        int64_t mod_stride, const int32_t* cu, int R, void* y, int T, int D, float eps, cudaStream_t st,
+                        int split) {
   if (dtype == DIT_F32)
-    return launch_adaln_t<float>(x, (const float*)h, gate, shift, scale, mod_stride, cu, R, (float*)y, T, D, eps, st);
-  return launch_adaln_t<bf16>(x, (const bf16*)h, gate, shift, scale, mod_stride, cu, R, (bf16*)y, T, D, eps, st);
+    return launch_adaln_t<float>(x, (const float*)h, gate, shift, scale, mod_stride, cu, R, (float*)y, T, D, eps, st, 0);
+  return launch_adaln_t<bf16>(x, (const bf16*)h, gate, shift, scale, mod_stride, cu, R, (bf16*)y, T, D, eps, st, split);
 }
 
 // =================================================================================================

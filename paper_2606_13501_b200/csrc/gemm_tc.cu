@@ -77,7 +77,11 @@ constexpr int A_BYTES = BM * BK * 2;
 constexpr int stage_bytes(int bn) { return A_BYTES + (bn / 2) * BK * 2; }   // own A rows + own HALF of the W tile
 constexpr int GEMM_THREADS = 192;
 constexpr int EPI_THREADS = 128;
-enum { EPI_GATE_RESID = 3, EPI_QKV_NORM_ROPE = 4 };
+enum { EPI_GATE_RESID = 3, EPI_QKV_NORM_ROPE = 4, EPI_BIAS_SPLIT = 5 };
+// EPI_BIAS_SPLIT: out[row, n] = hi = bf16(acc + bias), out[row, N + n] = lo = bf16((acc + bias) - hi): the result as an
+// unevaluated sum of two bf16 numbers (~16 significand bits).  A consumer GEMM reads [hi | lo] as ONE A operand of
+// width 2N against W wrapped along K (k_wrap): hi W^T + lo W^T in the fp32 accumulator — for the small operands whose
+// bf16 rounding would otherwise sit on the critical error path (the cross-attention context, R36).
 // The gated-residual epilogue stages its fp32 tile chunks in shared memory for TMA reduce-add (two 32 x 32 fp32
 // buffers per epilogue warp = 32 KB) and gives up one ring stage for them.
 constexpr int STG_WARP_BYTES = 2 * 32 * 128;
@@ -114,7 +118,7 @@ __device__ __forceinline__ float gelu_tanh_fast(float z) {
 template <int EPI, int BN>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
-               const __grid_constant__ CUtensorMap tmX, EpiArgs ep, int M, int N, int K, int GM) {
+               const __grid_constant__ CUtensorMap tmX, EpiArgs ep, int M, int N, int K, int GM, int k_wrap) {
   pdl_trigger();
   constexpr int STAGES = stages_for(EPI);
   extern __shared__ uint8_t smem_raw[];
@@ -193,7 +197,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
           const uint32_t fb = mapa_cluster(full_bar(s), 0);
           if (rank == 0) mbar_expect_tx(full_bar(s), 2 * STAGE_BYTES);
           tma_load_2d_pair(smem0 + s * STAGE_BYTES, &tmA, kb * BK, m0, fb);
-          tma_load_2d_pair(smem0 + s * STAGE_BYTES + A_BYTES, &tmB, kb * BK, n0, fb);
+          // k_wrap > 0: A is [hi | lo] (two bf16 parts side by side) and W repeats along K every k_wrap blocks
+          tma_load_2d_pair(smem0 + s * STAGE_BYTES + A_BYTES, &tmB, (k_wrap > 0 ? kb % k_wrap : kb) * BK, n0, fb);
         }
         __syncwarp();
         if (++s == STAGES) { s = 0; ph ^= 1; }
@@ -399,7 +404,14 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
             for (int e = 0; e < 8; ++e) v[e] = gelu_tanh_fast(v[e]);
           }
           if (!row_ok) continue;
-          if (EPI == DIT_EPI_BIAS || EPI == DIT_EPI_BIAS_GELU) {
+          if (EPI == EPI_BIAS_SPLIT) {
+            bf16* const o = reinterpret_cast<bf16*>(ep.out) + (int64_t)row * ep.ldo + ng;
+            float lo[8];
+#pragma unroll
+            for (int e = 0; e < 8; ++e) lo[e] = v[e] - __bfloat162float(__float2bfloat16_rn(v[e]));
+            st8<bf16>(o, v);
+            st8<bf16>(o + N, lo);
+          } else if (EPI == DIT_EPI_BIAS || EPI == DIT_EPI_BIAS_GELU) {
             st8<bf16>(reinterpret_cast<bf16*>(ep.out) + (int64_t)row * ep.ldo + ng, v);
           } else if (EPI == DIT_EPI_BIAS_F32) {
             st8<float>(reinterpret_cast<float*>(ep.out) + (int64_t)row * ep.ldo + ng, v);
@@ -449,7 +461,7 @@ int sm_count() {
 
 template <int EPI, int BN>
 dit_status launch_t(const CUtensorMap& ta, const CUtensorMap& tb, const CUtensorMap& tx, const EpiArgs& ep, int M, int N, int K,
-                    cudaStream_t st) {
+                    cudaStream_t st, int k_wrap = 0) {
   static std::atomic<bool> attr_set{false};
   if (!attr_set) {
     DIT_CUDA_OK(cudaFuncSetAttribute(gemm_tc_kernel<EPI, BN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -459,7 +471,7 @@ dit_status launch_t(const CUtensorMap& ta, const CUtensorMap& tb, const CUtensor
   const int pairs = cdiv(cdiv(M, BM), 2) * cdiv(N, BN);
   const int max_pairs = sm_count() / 2;
   DIT_CUDA_OK(launch_pdl(gemm_tc_kernel<EPI, BN>, dim3(2 * (pairs < max_pairs ? pairs : max_pairs)), dim3(GEMM_THREADS),
-                         smem_bytes(BN, EPI), st, 2, ta, tb, tx, ep, M, N, K, group_rows(M, K)));
+                         smem_bytes(BN, EPI), st, 2, ta, tb, tx, ep, M, N, K, group_rows(M, K), k_wrap));
   DIT_LAUNCH_CHECK();
   return DIT_OK;
 }
@@ -484,10 +496,10 @@ int pick_bn(int M, int N) {
 
 template <int EPI>
 dit_status launch_bn(int bn, const CUtensorMap& ta, const CUtensorMap& tb, const CUtensorMap& tx, const EpiArgs& ep, int M,
-                     int N, int K, cudaStream_t st) {
-  if (bn == 192) return launch_t<EPI, 192>(ta, tb, tx, ep, M, N, K, st);
-  if (bn == 240) return launch_t<EPI, 240>(ta, tb, tx, ep, M, N, K, st);
-  return launch_t<EPI, 256>(ta, tb, tx, ep, M, N, K, st);
+                     int N, int K, cudaStream_t st, int k_wrap = 0) {
+  if (bn == 192) return launch_t<EPI, 192>(ta, tb, tx, ep, M, N, K, st, k_wrap);
+  if (bn == 240) return launch_t<EPI, 240>(ta, tb, tx, ep, M, N, K, st, k_wrap);
+  return launch_t<EPI, 256>(ta, tb, tx, ep, M, N, K, st, k_wrap);
 }
 
 }  // namespace
@@ -502,22 +514,27 @@ bool gemm_tc_supported(int epi, const void* A, int64_t lda, const void* W, void*
 
 dit_status launch_gemm_tc_ex(int epi, const void* A, int64_t lda, const void* W, const void* bias, void* out, int64_t ldo,
                              const float* gate, int64_t gate_stride, const int32_t* cu, int R, int M, int N, int K,
-                             cudaStream_t st) {
+                             cudaStream_t st, int a_split) {
   if (M == 0 || N == 0) return DIT_OK;
   CUtensorMap ta, tb;
   const int bn = pick_bn(M, N);
-  DIT_REQUIRE(make_tmap_2d_bf16(&ta, A, M, K, lda, BM, BK) && make_tmap_2d_bf16(&tb, W, N, K, K, bn / 2, BK), DIT_ERR_CUDA,
+  // a_split: A is [hi | lo], 2K columns; W [N, K] is walked twice along K (k_wrap blocks of 64)
+  DIT_REQUIRE(!a_split || K % BK == 0, DIT_ERR_INVALID_ARG, "gemm_tc: split A needs K %% 64 == 0 (K=%d)", K);
+  const int k_wrap = a_split ? K / BK : 0;
+  const int Ka = a_split ? 2 * K : K;
+  DIT_REQUIRE(make_tmap_2d_bf16(&ta, A, M, Ka, lda, BM, BK) && make_tmap_2d_bf16(&tb, W, N, K, K, bn / 2, BK), DIT_ERR_CUDA,
               "gemm_tc: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d lda=%lld)", M, N, K, (long long)lda);
   EpiArgs ep{(const bf16*)bias, out, ldo, gate, gate_stride, cu, R, nullptr, nullptr, nullptr, nullptr, 0.f, 0, 0};
   ProfScope _prof(DIT_KC_GEMM, st);
   switch (epi) {
-    case DIT_EPI_BIAS: return launch_bn<DIT_EPI_BIAS>(bn, ta, tb, ta, ep, M, N, K, st);
-    case DIT_EPI_BIAS_GELU: return launch_bn<DIT_EPI_BIAS_GELU>(bn, ta, tb, ta, ep, M, N, K, st);
-    case DIT_EPI_BIAS_F32: return launch_bn<DIT_EPI_BIAS_F32>(bn, ta, tb, ta, ep, M, N, K, st);
+    case DIT_EPI_BIAS: return launch_bn<DIT_EPI_BIAS>(bn, ta, tb, ta, ep, M, N, Ka, st, k_wrap);
+    case DIT_EPI_BIAS_GELU: return launch_bn<DIT_EPI_BIAS_GELU>(bn, ta, tb, ta, ep, M, N, Ka, st, k_wrap);
+    case DIT_EPI_BIAS_F32: return launch_bn<DIT_EPI_BIAS_F32>(bn, ta, tb, ta, ep, M, N, Ka, st, k_wrap);
+    case EPI_BIAS_SPLIT: return launch_bn<EPI_BIAS_SPLIT>(bn, ta, tb, ta, ep, M, N, Ka, st, k_wrap);
     case EPI_GATE_RESID: {
       CUtensorMap tx;   // the fp32 residual stream as the target of the epilogue's TMA reduce-add
       DIT_REQUIRE(make_tmap_2d_f32(&tx, out, M, N, ldo, 32), DIT_ERR_CUDA, "gemm_tc: cuTensorMapEncodeTiled (x) failed");
-      return launch_bn<EPI_GATE_RESID>(bn, ta, tb, tx, ep, M, N, K, st);
+      return launch_bn<EPI_GATE_RESID>(bn, ta, tb, tx, ep, M, N, Ka, st, k_wrap);
     }
     default: DIT_REQUIRE(false, DIT_ERR_INVALID_ARG, "gemm_tc: epilogue %d", epi);
   }
@@ -528,21 +545,24 @@ dit_status launch_gemm_tc_ex(int epi, const void* A, int64_t lda, const void* W,
 // whole heads.  Self-attention QKV: (D, 2D, N = 3D); cross-attention q: (D, D, N = D); cross-attention k | v: (0, D, N = 2D).
 dit_status launch_gemm_tc_qkv(const void* A, int64_t lda, const void* W, const void* bias, void* out, int64_t ldo,
                               const void* gq, const void* gk, float rms_eps, const float* rc, const float* rs, int q_end,
-                              int k_end, int M, int N, int K, cudaStream_t st) {
+                              int k_end, int M, int N, int K, cudaStream_t st, int a_split) {
   if (M == 0 || N == 0) return DIT_OK;
+  DIT_REQUIRE(!a_split || K % BK == 0, DIT_ERR_INVALID_ARG, "gemm_tc_qkv: split A needs K %% 64 == 0 (K=%d)", K);
+  const int k_wrap = a_split ? K / BK : 0;
+  const int Ka = a_split ? 2 * K : K;
   DIT_REQUIRE(q_end % 128 == 0 && k_end % 128 == 0 && N % 128 == 0 && 0 <= q_end && q_end <= k_end && k_end <= N,
               DIT_ERR_INVALID_ARG, "gemm_tc_qkv: N=%d q_end=%d k_end=%d", N, q_end, k_end);
   CUtensorMap ta, tb;
-  DIT_REQUIRE(make_tmap_2d_bf16(&ta, A, M, K, lda, BM, BK) && make_tmap_2d_bf16(&tb, W, N, K, K, 128, BK), DIT_ERR_CUDA,
+  DIT_REQUIRE(make_tmap_2d_bf16(&ta, A, M, Ka, lda, BM, BK) && make_tmap_2d_bf16(&tb, W, N, K, K, 128, BK), DIT_ERR_CUDA,
               "gemm_tc_qkv: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d)", M, N, K);
   EpiArgs ep{(const bf16*)bias, out, ldo, nullptr, 0, nullptr, 1, (const bf16*)gq, (const bf16*)gk, rc, rs, rms_eps, q_end, k_end};
   ProfScope _prof(DIT_KC_GEMM, st);
-  return launch_t<EPI_QKV_NORM_ROPE, 256>(ta, tb, ta, ep, M, N, K, st);
+  return launch_t<EPI_QKV_NORM_ROPE, 256>(ta, tb, ta, ep, M, N, Ka, st, k_wrap);
 }
 
 dit_status launch_gemm_tc(int epi, const void* A, int64_t lda, const void* W, const void* bias, void* out, int64_t ldo,
-                          int M, int N, int K, cudaStream_t st) {
-  return launch_gemm_tc_ex(epi, A, lda, W, bias, out, ldo, nullptr, 0, nullptr, 1, M, N, K, st);
+                          int M, int N, int K, cudaStream_t st, int a_split) {
+  return launch_gemm_tc_ex(epi, A, lda, W, bias, out, ldo, nullptr, 0, nullptr, 1, M, N, K, st, a_split);
 }
 
 }  // namespace dit

@@ -1,8 +1,9 @@
 """Writes tests/golden/cfg3_oracle_rows.pt: sampled rows of ONE FULL END-TO-END oracle step at BASELINE.json's full
 size, for the configuration whose whole-step oracle is too slow to run inside `pytest -m gpu` (cfg 3: 168 TFLOP of fp64
-CPU work, ~20-30 minutes and ~50 GB of host memory on 8 cores).
+CPU work and ~65 GB of host memory: the oracle materialises the 32760 x 32760 fp64 score matrix of a head, as the plain
+definition says).
 
-    python tests/golden/make_fullsize_oracle.py --cfg 3        # this container (no GPU needed)
+    python tests/golden/make_fullsize_oracle.py --cfg 3 [--out FILE]     # CPU only; needs a host with > 70 GB of RAM
 
 It calls ONLY `oracle/dit_oracle.py` (as it stands) and the seeded input generator `paper_2606_13501_b200/synth.py`
 (which holds none of the method's arithmetic).  No value comes from the CUDA path.  The GPU test
@@ -91,11 +92,12 @@ def main():
     ap.add_argument("--n-tok", type=int, default=2048)
     ap.add_argument("--n-x", type=int, default=24)
     ap.add_argument("--smoke", action="store_true", help="tiny cfg3-like shape, writes to /tmp (checks this script only)")
+    ap.add_argument("--out", default=os.path.join(HERE, "cfg3_oracle_rows.pt"))
     args = ap.parse_args()
     if args.smoke:
         run_cfg3("/tmp/cfg3_oracle_rows_smoke.pt", 64, 8, smoke=True)
     else:
-        run_cfg3(os.path.join(HERE, "cfg3_oracle_rows.pt"), args.n_tok, args.n_x)
+        run_cfg3(args.out, args.n_tok, args.n_x)
 
 
 if __name__ == "__main__":
