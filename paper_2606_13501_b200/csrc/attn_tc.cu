@@ -35,6 +35,7 @@
 // an exact one; MUFU.EX2 at 16 / clk / SM) is co-critical.
 #include <algorithm>
 #include <cstdlib>
+#include <type_traits>
 
 #include "tc.cuh"
 
@@ -636,13 +637,19 @@ constexpr int PQ_HALF = PQ_BYTES / 2;
 constexpr int PKV_BYTES = 64 * HD * 2;          // a K stage (64 keys x 128 d: two [64 x 64] boxes) or a V stage ([128 keys x 64 d])
 constexpr int PK_HALF = PKV_BYTES / 2;
 constexpr int PAIR_BAR_BYTES = 512;
-constexpr int PAIR_XCH_FLOATS = 2 * 128 + 128 + 4 * 128;   // pair max exchange | published reference | 4-way reduce
+constexpr int PAIR_XCH_FLOATS = 4 * 128 + 128;   // [4][row]: 4-way reductions of a row's threads | the published reference
 constexpr int PAIR_SMEM = PQ_BYTES + (PKS + PVS) * PKV_BYTES + 1024 + PAIR_BAR_BYTES + PAIR_XCH_FLOATS * 4;
 constexpr uint32_t TM_S = 0, TM_P = 256, TM_O = 384;       // TMEM columns: S[g] = g * 128, P[g] = 256 + g * 64, O = 384
 #ifndef DIT_ATTN_RELAXED_ARRIVE
 #define DIT_ATTN_RELAXED_ARRIVE 1
 #endif
 
+#ifndef DIT_ATTN_PAIR_POLY_PAIRS
+#define DIT_ATTN_PAIR_POLY_PAIRS 0
+#endif
+// In the pair kernel the softmax is bound by instruction issue, not by MUFU (XU pipe 58 % busy): every exponential on the
+// MUFU is fastest (measured at N = 16384, H = 24: 0 / 2 / 4 polynomial pairs of 16: 1359 / 1326 / 1303 TFLOP/s).
+constexpr int PAIR_POLY_PAIRS = DIT_ATTN_PAIR_POLY_PAIRS;
 // p = 2^(s c + nm) for 32 scores -> 16 packed bf16 pairs in pk; packed fp32 partial sums
 __device__ __forceinline__ void exp_pack(const uint32_t (&s)[32], uint64_t c2, uint64_t nm2, uint32_t (&pk)[16],
                                          uint64_t& sum2, uint64_t& sum2b) {
@@ -650,7 +657,7 @@ __device__ __forceinline__ void exp_pack(const uint32_t (&s)[32], uint64_t c2, u
   for (int i = 0; i < 16; ++i) {
     const uint64_t x = fma2(pack2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1])), c2, nm2);
     float a, b;
-    if (i % 4 == 3 && i / 4 < POLY_PAIRS) {   // spread over the chunk so MUFU and FMA work interleave
+    if (i % 4 == 3 && i / 4 < PAIR_POLY_PAIRS) {   // spread over the chunk so MUFU and FMA work interleave
       ex2_poly2(x, a, b);
     } else {
       float xa, xb;
@@ -728,7 +735,7 @@ attn_pair_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
     for (int s = 0; s < PVS; ++s) { mbar_init(v_full(s), 1); mbar_init(v_empty(s), 1); }
     for (int g = 0; g < 2; ++g) {
       mbar_init(s_full(g), 1);
-      mbar_init(s_free(g), 16);          // 8 warps of the owning group in each CTA
+      mbar_init(s_free(g), 16);          // the 8 warps of a group in each CTA
       mbar_init(p_full(g), 16);
       mbar_init(pv_done(g), 1);
     }
@@ -761,8 +768,7 @@ attn_pair_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
   if (warp < 4) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");   // 128 x 56 + 512 x 104 <= 640 x 96
     int kc = 0, vc = 0;            // K / V tiles produced or consumed so far (all passes)
-    int su0 = 0, su1 = 0;          // S tiles issued into S[0] / S[1] so far
-    int pu0 = 0, pu1 = 0;          // PVs issued from P[0] / P[1] so far
+    int sn = 0, pn = 0;            // S tiles / PVs issued so far (all passes): S tile t goes to S[t & 1], PV t reads P[t & 1]
     for (int pass = 0;; ++pass) {
       const bool with_pv = pass != 1;
       if (warp == 0) {
@@ -805,9 +811,9 @@ attn_pair_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
         constexpr uint32_t idesc_o = idesc_bf16(2 * TQ, HD, 0, 1);   // O += P V: A from TMEM, B (V) MN-major, N = 128 (d)
         constexpr uint64_t vdesc_hi = desc_base_sw128(1, 64);        // one 128-byte atom wide (64 d), 8-key groups 1 KB apart
         // S of the next key tile into S[g]; the buffer's previous contents have been read (s_free)
-        auto issue_s = [&](int g) {
-          const int su = g ? su1 : su0;
-          if (su > 0) mbar_wait_poll(s_free(g), (uint32_t)(su - 1) & 1u);
+        auto issue_s = [&]() {
+          const int g = sn & 1;
+          if (sn >= 2) mbar_wait_poll(s_free(g), (uint32_t)((sn >> 1) - 1) & 1u);
           const int s = kc % PKS;
           mbar_wait_poll(k_full(s), (uint32_t)(kc / PKS) & 1u);
           tc_fence_after();
@@ -822,21 +828,20 @@ attn_pair_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
             umma_commit_pair(k_empty(s), (uint16_t)3);
           }
           __syncwarp();
-          ++kc;
-          if (g) ++su1; else ++su0;
+          ++kc; ++sn;
         };
-        // O (+)= P(j) V_j from P[j & 1]
+        // O (+)= P(j) V_j
         auto issue_pv = [&](int j) {
-          const int g = j & 1;
-          const int pu = g ? pu1 : pu0;
+          const int g = pn & 1;
           const int vs = vc % PVS;
-          const int nk16 = kv_len - j * TK > SK ? 8 : 4;           // a ragged last tile may have no keys 64..127
+          const int left = kv_len - j * TK;                        // a ragged last tile: only the 32-key quarters with keys
+          const int nk16 = left >= TK ? 8 : 2 * ((left + 31) / 32);
           mbar_wait_poll(v_full(vs), (uint32_t)(vc / PVS) & 1u);
-          mbar_wait_poll(p_full(g), (uint32_t)pu & 1u);
+          mbar_wait_poll(p_full(g), (uint32_t)(pn >> 1) & 1u);
           tc_fence_after();
           if (elect_one()) {
             const uint32_t d = tmem_base + TM_O;
-            const uint32_t pa = tmem_base + TM_P + g * 64;         // bf16 pairs: keys 0..63 in columns 0..31, 64..127 in 32..63
+            const uint32_t pa = tmem_base + TM_P + g * 64;         // bf16 pairs: key 2 i, 2 i + 1 in column i
             const uint32_t va = sV + vs * PKV_BYTES;
 #pragma unroll
             for (int k = 0; k < 8; ++k)
@@ -847,15 +852,14 @@ attn_pair_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
             if (j == n_tiles - 1) umma_commit_pair(o_done(), (uint16_t)3);
           }
           __syncwarp();
-          ++vc;
-          if (g) ++pu1; else ++pu0;
+          ++vc; ++pn;
         };
         if (pass == 0) { mbar_wait_poll(q_full(), 0); tc_fence_after(); }
-        // order = the order the events arrive in: S(j + 2) as soon as S(j) has been read (early in tile j's softmax),
-        // PV(j - 1) when P(j - 1) is complete (the other group, half a period earlier)
-        for (int i = 0; i < 2 && i < n_tiles; ++i) issue_s(i);
+        // order = the order the events arrive in: S(j + 2) as soon as S(j) has been read (at the start of tile j's
+        // softmax), PV(j - 1) when P(j - 1) is complete
+        for (int i = 0; i < 2 && i < n_tiles; ++i) issue_s();
         for (int j = 0; j < n_tiles; ++j) {
-          if (j + 2 < n_tiles) issue_s(j & 1);
+          if (j + 2 < n_tiles) issue_s();
           if (with_pv && j >= 1) issue_pv(j - 1);
         }
         if (with_pv) issue_pv(n_tiles - 1);
@@ -866,123 +870,86 @@ attn_pair_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
     }
   } else {
     asm volatile("setmaxnreg.inc.sync.aligned.u32 104;");
+    // ===================================================== softmax: two groups of 8 warps in anti-phase
+    // Key tile t (counted over all passes) belongs to group t & 1, lives in S[t & 1], and its P goes to P[pt & 1] (pt =
+    // P tiles so far).  Thread = one query row x 64 keys: TMEM lane quadrant `quad` (rows), key half `h`.
     const int w = warp - 4;
-    const int grp = w >> 3;                        // owns key tiles j = grp (mod 2), S[grp], P[grp]
-    const int h = (w >> 2) & 1;                    // 0: keys 0..63 of the tile (leader), 1: keys 64..127 (follower)
+    const int grp = w >> 3;
+    const int h = (w >> 2) & 1;                    // 0: keys 0..63 of the tile, 1: keys 64..127
+    const int kq = grp * 2 + h;                    // the row's four threads, for the 4-way reductions and the epilogue
     const int quad = warp & 3;                     // TMEM lane quadrant of this warp
     const int r_in = quad * 32 + lane;             // row inside this CTA's Q tile
     const int row = q_base + r_in;
     const uint32_t lane_off = (uint32_t)(quad * 32) << 16;
-    const uint32_t s_addr = tmem_base + TM_S + grp * 128 + h * SK + lane_off;    // this thread's 64 scores
-    const uint32_t p_addr = tmem_base + TM_P + grp * 64 + h * 32 + lane_off;     // ... and its 32 columns of P
-    const uint32_t o_addr = tmem_base + TM_O + lane_off;
+    const uint32_t s_addr = tmem_base + TM_S + grp * 128 + h * SK + lane_off;
+    const uint32_t p_addr = tmem_base + TM_P + h * 32 + lane_off;      // + 64 * (pt & 1)
+    const uint32_t o_addr = tmem_base + TM_O + kq * 32 + lane_off;
     float* const xch = reinterpret_cast<float*>(smem_raw + (bar0 - smem_u32(smem_raw)) + PAIR_BAR_BYTES);
-    float* const m_sh = xch;                       // [h][128]: half-row maxima of key tile 0 (group 0)
-    float* const m_row = xch + 256;                // [128]: the row's reference (log2 units)
-    float* const red = xch + 384;                  // [grp * 2 + h][128]: 4-way reductions (row max of pass 1, row sums)
+    float* const red0 = xch;                       // [kq][128]: 4-way reductions (row max, row sums)
+    float* const red = red0 + kq * 128 + r_in;
+    float* const m_row = xch + 512;                // [128]: the row's reference, published by group 0
     const float c = p.scale_log2;
     const uint64_t c2 = pack2(c, c);
-    auto arrive = [&](uint32_t bar) {              // one arrival per warp on a barrier of the leader CTA
+    // barriers of the LEADER CTA as shared::cluster addresses (valid from both CTAs: no branch at the arrival)
+    const uint32_t a_sfree = mapa_cluster(s_free(grp), 0), a_pfull = mapa_cluster(p_full(0), 0);
+    const uint32_t b_sfull = s_full(grp);
+    auto arrive = [&](uint32_t bar_cluster) {      // one arrival per warp
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) {
-        if (leader_cta) mbar_arrive(bar);
-#if DIT_ATTN_RELAXED_ARRIVE
-        else mbar_arrive_remote_relaxed(bar, 0);
-#else
-        else mbar_arrive_remote(bar, 0);
-#endif
-      }
+      if (lane == 0)
+        asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster) : "memory");
     };
-    int us = 0, up = 0;                            // S tiles read / P tiles written by this group so far (all passes)
     float m_used = 0.f;
     for (int pass = 0;; ++pass) {
-      if (pass == 1) {
-        // ------------------------------------------ row max over all key tiles (after a panic)
-        float mx = -INFINITY;
-        for (int j = grp; j < n_tiles; j += 2, ++us) {
-          const int valid = kv_len - j * TK - h * SK;
-          if (valid > 0) {
-            uint32_t s0[32], s1[32];
-            mbar_wait(s_full(grp), (uint32_t)us & 1u);
-            tc_fence_after();
-            tmem_ld32(s_addr + 0, s0);
-            tmem_ld32(s_addr + 32, s1);
-            tmem_ld_wait();
-            if (valid < SK) { mask32(s0, valid); mask32(s1, valid - 32); }
-            mx = fmaxf(mx, fmaxf(max32(s0), max32(s1)));
-          }
-          arrive(s_free(grp));
-        }
-        red[(grp * 2 + h) * 128 + r_in] = mx;
-        asm volatile("bar.sync %0, 128;" ::"r"(9 + quad) : "memory");
-        mx = fmaxf(fmaxf(red[r_in], red[128 + r_in]), fmaxf(red[256 + r_in], red[384 + r_in]));
-        m_used = mx * c;                           // c > 0; every row has at least one key
-        asm volatile("bar.sync %0, 128;" ::"r"(9 + quad) : "memory");   // `red` is reused for the row sums
-        tc_fence_before(); cluster_sync_all(); tc_fence_after();        // pass 1 -> 2 boundary
-        continue;
-      }
-      // -------------------------------------------- pass 0 / 2: P, row sums, PV against one reference per row
-      float l = 0.f, tile_worst = 0.f;
+      float l = 0.f, tile_worst = 0.f, mx_run = -INFINITY;
+      const int base = pass * n_tiles;             // global index of this pass's first key tile
+      const int pbase = pass == 2 ? n_tiles : 0;   // ... minus this = its P index (pass 1 writes no P)
       if (pass == 0 && grp == 1) {                 // the reference comes from group 0's first tile
         asm volatile("bar.sync %0, 128;" ::"r"(5 + quad) : "memory");
         m_used = m_row[r_in];
       }
-      for (int j = grp; j < n_tiles; j += 2, ++us, ++up) {
-        const int valid = kv_len - j * TK - h * SK;    // keys of this half that exist (warp-uniform; <= 0: none)
+      for (int t = base + ((base ^ grp) & 1); t < base + n_tiles; t += 2) {
+        const int valid = kv_len - (t - base) * TK - h * SK;   // keys of this half that exist (>= 64: all; warp-uniform)
         uint32_t s0[32], s1[32];
-        if (pass == 0 && j == 0) {
-          // first key tile: its row max is the reference of the whole pass (group 0 only)
-          float mx = -INFINITY;
+        if (valid > 0) {
+          mbar_wait(b_sfull, (uint32_t)(t >> 1) & 1u);
+          tc_fence_after();
+          tmem_ld32(s_addr + 0, s0);
+          tmem_ld32(s_addr + 32, s1);
+          tmem_ld_wait();
+        }
+        arrive(a_sfree);                           // S[grp] may be overwritten by S(t + 2) from here on
+        if (pass == 1) {                           // row-max pass (after a panic)
           if (valid > 0) {
-            mbar_wait(s_full(grp), (uint32_t)us & 1u);
-            tc_fence_after();
-            // the second 32 scores only for the row max (re-read after the exchange: a TMEM read is cheaper than 32 more
-            // live registers); the first 32 stay
-            tmem_ld32(s_addr + 32, s1);
-            tmem_ld32(s_addr + 0, s0);
-            tmem_ld_wait();
-            if (valid < SK) { mask32(s0, valid); mask32(s1, valid - 32); }   // -inf before the row max
-            mx = fmaxf(max32(s0), max32(s1));
+            if (valid < SK) { mask32(s0, valid); mask32(s1, valid - 32); }
+            mx_run = fmaxf(mx_run, fmaxf(max32(s0), max32(s1)));
           }
-          m_sh[h * 128 + r_in] = mx;
+          continue;
+        }
+        if (valid > 0 && valid < SK) { mask32(s0, valid); mask32(s1, valid - 32); }   // -inf: before the row max; P = 0
+        if (t == 0) {                              // the row max of the first key tile is the reference of the pass
+          *red = valid > 0 ? fmaxf(max32(s0), max32(s1)) : -INFINITY;
           asm volatile("bar.sync %0, 64;" ::"r"(1 + quad) : "memory");
-          mx = fmaxf(mx, m_sh[(h ^ 1) * 128 + r_in]);
-          m_used = mx * c;
+          m_used = fmaxf(red0[r_in], red0[128 + r_in]) * c;       // kq = 0, 1: group 0's two halves; c > 0
           if (h == 0) m_row[r_in] = m_used;
           __threadfence_block();
           asm volatile("bar.arrive %0, 128;" ::"r"(5 + quad) : "memory");     // group 1 may read m_row
-          if (valid > 0) {
-            tmem_ld32(s_addr + 32, s1);
-            tmem_ld_wait();
-          }
-          arrive(s_free(grp));
-        } else {
-          if (valid > 0) {
-            mbar_wait(s_full(grp), (uint32_t)us & 1u);
-            tc_fence_after();
-            tmem_ld32(s_addr + 0, s0);
-            tmem_ld32(s_addr + 32, s1);
-            tmem_ld_wait();
-          }
-          arrive(s_free(grp));                     // S[grp] may be overwritten by S(j + 2) from here on
-          if (valid > 0 && valid < SK) mask32(s0, valid);   // -inf -> P = 0
         }
+        const uint32_t pt = (uint32_t)(t - pbase), bp = pt & 1u;
         if (valid > 0) {
           const uint64_t nm2 = pack2(-m_used, -m_used);
           uint64_t sum2 = pack2(0.f, 0.f), sum2b = pack2(0.f, 0.f);
           {
             uint32_t pk[16];
             exp_pack(s0, c2, nm2, pk, sum2, sum2b);
-            // PV(j - 2) has read P[grp]: it was issued when this group finished tile j - 2, i.e. about half a tile ago
-            if (up > 0) { mbar_wait(pv_done(grp), (uint32_t)(up - 1) & 1u); tc_fence_after(); }
-            tmem_st16(p_addr + 0, pk);
+            // the PV before last has read P[bp]: it was issued about a tile ago
+            if (pt >= 2) { mbar_wait(pv_done(0) + 8u * bp, ((pt >> 1) - 1u) & 1u); tc_fence_after(); }
+            tmem_st16(p_addr + bp * 64u, pk);
           }
-          if (valid < SK) mask32(s1, valid - 32);
           {
             uint32_t pk[16];
             exp_pack(s1, c2, nm2, pk, sum2, sum2b);
-            tmem_st16(p_addr + 16, pk);
+            tmem_st16(p_addr + bp * 64u + 16, pk);
           }
           float sa, sb;
           unpack2(add2(sum2, sum2b), sa, sb);
@@ -990,25 +957,32 @@ attn_pair_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
           l += sa + sb;
           tmem_st_wait();
         }
-        arrive(p_full(grp));
+        arrive(a_pfull + 8u * bp);
+      }
+      if (pass == 1) {
+        *red = mx_run;
+        asm volatile("bar.sync %0, 128;" ::"r"(9 + quad) : "memory");
+        m_used = fmaxf(fmaxf(red0[r_in], red0[128 + r_in]), fmaxf(red0[256 + r_in], red0[384 + r_in])) * c;
+        asm volatile("bar.sync %0, 128;" ::"r"(9 + quad) : "memory");   // `red` is reused for the row sums
+        tc_fence_before(); cluster_sync_all(); tc_fence_after();        // pass 1 -> 2 boundary
+        continue;
       }
       if (pass == 0 && __any_sync(0xffffffffu, !(tile_worst < 1.152921504606847e18f)) && lane == 0)   // 2^60, inf, NaN
         asm volatile("st.shared.u32 [%0], %1;" ::"r"(panic_addr), "r"(1u) : "memory");
-      // ---- epilogue: the row's four threads add their partial sums; thread (grp, h) writes d columns (grp * 2 + h) * 32 ..
-      red[(grp * 2 + h) * 128 + r_in] = l;
+      // ---- epilogue: the row's four threads add their partial sums; thread kq writes d columns 32 kq .. 32 kq + 31
+      *red = l;
       asm volatile("bar.sync %0, 128;" ::"r"(9 + quad) : "memory");
-      l = (red[r_in] + red[128 + r_in]) + (red[256 + r_in] + red[384 + r_in]);
+      l = (red0[r_in] + red0[128 + r_in]) + (red0[256 + r_in] + red0[384 + r_in]);
       mbar_wait(o_done(), pass == 0 ? 0u : 1u);
       tc_fence_after();
       const float inv = 1.0f / l;                  // l > 0: the first tile has at least one key
       const bool row_ok = row < q_hi;
       {
-        const int cq = (grp * 2 + h) * 32;
         uint32_t o[32];
-        tmem_ld32(o_addr + cq, o);
+        tmem_ld32(o_addr, o);
         tmem_ld_wait();
         if (row_ok) {
-          bf16* orow = p.o + (int64_t)row * p.o_stride + head * HD + cq;
+          bf16* orow = p.o + (int64_t)row * p.o_stride + head * HD + kq * 32;
 #pragma unroll
           for (int g = 0; g < 4; ++g) {
             float v[8];
@@ -1018,7 +992,7 @@ attn_pair_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
           }
         }
       }
-      if (grp == 0 && h == 0 && row_ok && p.lse != nullptr)
+      if (kq == 0 && row_ok && p.lse != nullptr)
         p.lse[(int64_t)row * p.H + head] = 0.6931471805599453f * (m_used + log2f(l));
       if (pass == 2) break;
       if (!pair_panicked()) break;
@@ -1058,19 +1032,32 @@ dit_status launch_attn_tc(const AttnArgs& a, cudaStream_t st) {
     DIT_CUDA_OK(cudaFuncSetAttribute(attn_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, PAIR_SMEM));
     attr_set = true;
   }
-  static const bool use_pair = []() {   // DIT_ATTN_KERNEL=two-tile selects the previous kernel (A / B measurements)
+  static const bool use_pair = []() {   // DIT_ATTN_KERNEL=two-tile selects attn_tc_kernel for every shape (A / B measurements)
     const char* e = getenv("DIT_ATTN_KERNEL");
     return !(e != nullptr && e[0] == 't');
+  }();
+  static const int pair_min_k = []() {  // DIT_ATTN_PAIR_MIN_K overrides the switch-over length (tuning knob)
+    const char* e = getenv("DIT_ATTN_PAIR_MIN_K");
+    return e != nullptr ? atoi(e) : 8192;
   }();
   // K / V maps need a valid base even when there are no keys (the kernel then never issues a load)
   const void* kb = a.n_k > 0 ? a.k : a.q;
   const void* vb = a.n_k > 0 ? a.v : a.q;
   const uint64_t nk_rows = a.n_k > 0 ? a.n_k : 1;
   const uint64_t kv_ld = a.n_k > 0 ? a.kv_stride : a.q_stride;
+  // Key sequences from 8192 (64 key tiles): the pair kernel; shorter ones: attn_tc_kernel, whose per-work-item prologue
+  // and drain weigh less (measured, H = 24: N = 4352: 1040 vs 970 TFLOP/s; N = 8192: 1100 vs 1220; 16384: 1244 vs 1359).
+  int max_k = a.n_k;
+  if (a.cu_k_host) {
+    max_k = 0;
+    for (int r = 0; r < a.R; ++r) max_k = max(max_k, a.cu_k_host[r + 1] - a.cu_k_host[r]);
+  }
+  max_k = cdiv(max_k, a.n_shards);
+  const bool pair_kernel = use_pair && max_k >= pair_min_k;
   CUtensorMap tq, tk, tv;
   const uint64_t cols = (uint64_t)a.H * HD;
   DIT_REQUIRE(make_tmap_2d_bf16(&tq, a.q, a.n_q, cols, a.q_stride, TQ, 64) &&
-                  make_tmap_2d_bf16(&tk, kb, nk_rows, cols, kv_ld, use_pair ? 64 : TK, 64) &&
+                  make_tmap_2d_bf16(&tk, kb, nk_rows, cols, kv_ld, pair_kernel ? 64 : TK, 64) &&
                   make_tmap_2d_bf16(&tv, vb, nk_rows, cols, kv_ld, TK, 64),
               DIT_ERR_CUDA, "attn_tc: cuTensorMapEncodeTiled failed (n_q=%d n_k=%d H=%d)", a.n_q, a.n_k, a.H);
   AttnParams p;
@@ -1085,7 +1072,7 @@ dit_status launch_attn_tc(const AttnArgs& a, cudaStream_t st) {
       return a.cu_k_host[x + 1] - a.cu_k_host[x] > a.cu_k_host[y + 1] - a.cu_k_host[y];
     });
   ProfScope _prof(DIT_KC_ATTN, st);
-  if (use_pair) {   // one CTA pair per (256-row query block, head, request)
+  if (pair_kernel) {   // one CTA pair per (256-row query block, head, request)
     dim3 pgrid(2 * cdiv(max_q, 2 * TQ), a.H, a.cu_q ? a.R : 1);
     DIT_CUDA_OK(launch_pdl(attn_pair_kernel, pgrid, dim3(ATTN_THREADS), PAIR_SMEM, st, 2, tq, tk, tv, p));
     DIT_LAUNCH_CHECK();

@@ -279,7 +279,12 @@ def test_cfg4_full_size_packed_batch(lib):
         torch.cuda.synchronize()
         e_rel, e_max = errors(outs[r], single)
         assert torch.isfinite(outs[r].float()).all()
-        assert e_rel < 2e-3 and e_max < 3e-2, f"packing changed request {r}: rel {e_rel:.2e} max {e_max:.2e}"
+        # The packed launch (longest request: 16640 keys) runs the CTA-pair attention kernel, a short request alone the
+        # two-tile kernel: both are exact re-associations with different bf16 rounding points (reference of P), so the two
+        # GPU results are independent bf16 realisations of the same step — each within the oracle bar above (requests 0-3),
+        # their difference within sqrt(2) of it.  Requests 4, 5 alone take the pair kernel too and agree more closely.
+        assert e_rel < 5e-3 and e_max < 4.5e-2, f"packing changed request {r}: rel {e_rel:.2e} max {e_max:.2e}"
+        _log(test="cfg4 packing invariance (packed vs alone, GPU vs GPU)", request=r, rel_l2=e_rel, max_abs_over_rms=e_max)
     assert B.dit_fallback_launches() == n0
 
 
