@@ -34,6 +34,7 @@
 // Roofline: tensor pipe; the softmax instruction stream (312 instructions per 64 scores in an optimistic tile, 379 in
 // an exact one; MUFU.EX2 at 16 / clk / SM) is co-critical.
 #include <algorithm>
+#include <cstdio>
 #include <cstdlib>
 #include <type_traits>
 
@@ -75,6 +76,7 @@ struct AttnParams {
   int n_q, n_k, H;
   float scale_log2;   // softmax scale * log2(e)
   int shard, n_shards;
+  int R, n_items;     // pair kernel: requests, work items = sum over requests of 256-row query blocks x heads
   uint8_t order[64];  // blockIdx.z -> request, longest key sequence first: the last wave is made of short items
 };
 
@@ -638,7 +640,7 @@ constexpr int PKV_BYTES = 64 * HD * 2;          // a K stage (64 keys x 128 d: t
 constexpr int PK_HALF = PKV_BYTES / 2;
 constexpr int PAIR_BAR_BYTES = 512;
 constexpr int PAIR_XCH_FLOATS = 4 * 128 + 128;   // [4][row]: 4-way reductions of a row's threads | the published reference
-constexpr int PAIR_SMEM = PQ_BYTES + (PKS + PVS) * PKV_BYTES + 1024 + PAIR_BAR_BYTES + PAIR_XCH_FLOATS * 4;
+constexpr int PAIR_SMEM = 2 * PQ_BYTES + (PKS + PVS) * PKV_BYTES + 1024 + PAIR_BAR_BYTES + PAIR_XCH_FLOATS * 4;
 constexpr uint32_t TM_S = 0, TM_P = 256, TM_O = 384;       // TMEM columns: S[g] = g * 128, P[g] = 256 + g * 64, O = 384
 #ifndef DIT_ATTN_RELAXED_ARRIVE
 #define DIT_ATTN_RELAXED_ARRIVE 1
@@ -671,20 +673,26 @@ __device__ __forceinline__ void exp_pack(const uint32_t (&s)[32], uint64_t c2, u
   }
 }
 
+#ifdef DIT_ATTN_TRACE
+__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+#define TRACE(i) do { if (tr_on && tr_n < 4) tr[tr_n][i] = gtime(); } while (0)
+#else
+#define TRACE(i) do { } while (0)
+#endif
 __global__ void __launch_bounds__(ATTN_THREADS, 1)
 attn_pair_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                  const __grid_constant__ CUtensorMap tmV, AttnParams p) {
   pdl_trigger();
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t sQ = smem0, sK = sQ + PQ_BYTES, sV = sK + PKS * PKV_BYTES;
+  const uint32_t sQ = smem0, sK = sQ + 2 * PQ_BYTES, sV = sK + PKS * PKV_BYTES;
   const uint32_t bar0 = sV + PVS * PKV_BYTES;
-  auto q_full = [&]() { return bar0; };
-  auto k_full = [&](int s) { return bar0 + 8u * (1 + s); };
-  auto k_empty = [&](int s) { return bar0 + 8u * (1 + PKS + s); };
-  auto v_full = [&](int s) { return bar0 + 8u * (1 + 2 * PKS + s); };
-  auto v_empty = [&](int s) { return bar0 + 8u * (1 + 2 * PKS + PVS + s); };
-  constexpr int B0 = 1 + 2 * PKS + 2 * PVS;
+  auto q_full = [&](int b) { return bar0 + 8u * b; };   // Q buffer b = work item parity
+  auto k_full = [&](int s) { return bar0 + 8u * (2 + s); };
+  auto k_empty = [&](int s) { return bar0 + 8u * (2 + PKS + s); };
+  auto v_full = [&](int s) { return bar0 + 8u * (2 + 2 * PKS + s); };
+  auto v_empty = [&](int s) { return bar0 + 8u * (2 + 2 * PKS + PVS + s); };
+  constexpr int B0 = 2 + 2 * PKS + 2 * PVS;
   auto s_full = [&](int g) { return bar0 + 8u * (B0 + g); };        // S[g] complete (leader's commit, both CTAs)
   auto s_free = [&](int g) { return bar0 + 8u * (B0 + 2 + g); };    // S[g] read by all its softmax warps (leader CTA only)
   auto p_full = [&](int g) { return bar0 + 8u * (B0 + 4 + g); };    // P[g] written by all its softmax warps (leader CTA only)
@@ -697,32 +705,36 @@ attn_pair_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t crank = cluster_ctarank();
   const bool leader_cta = crank == 0;
-  const int req = p.cu_q ? p.order[blockIdx.z] : 0, head = blockIdx.y;
-  const int q_lo = p.cu_q ? p.cu_q[req] : 0, q_hi = p.cu_q ? p.cu_q[req + 1] : p.n_q;
-  const int q_pair = q_lo + (int)(blockIdx.x >> 1) * (2 * TQ);   // first row of the pair's 256-row block
-  if (q_pair >= q_hi) return;                                    // pair-uniform: before any cluster-wide step
-  const int q_base = q_pair + (int)crank * TQ;                   // this CTA's 128 rows (may lie past q_hi: nothing stored)
-  const int k_lo0 = p.cu_k ? p.cu_k[req] : 0, k_hi0 = p.cu_k ? p.cu_k[req + 1] : p.n_k;
-  const int klen = k_hi0 - k_lo0;
-  const int ssz = (klen + p.n_shards - 1) / p.n_shards;
-  int k_lo = k_lo0 + p.shard * ssz, k_hi = k_lo0 + (p.shard + 1) * ssz;
-  if (k_lo > k_hi0) k_lo = k_hi0;
-  if (k_hi > k_hi0) k_hi = k_hi0;
-  const int kv_len = k_hi - k_lo;
-  const int n_tiles = (kv_len + TK - 1) / TK;
-
-  if (n_tiles == 0) {  // empty shard: o = 0, lse = -inf (R18)
-    pdl_wait();
-    if (warp >= 4 && warp < 8) {
-      const int row = q_base + (warp & 3) * 32 + lane;
-      if (row < q_hi) {
-        const float z[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-        for (int c = 0; c < HD; c += 8) st8<bf16>(p.o + (int64_t)row * p.o_stride + head * HD + c, z);
-        if (p.lse) p.lse[(int64_t)row * p.H + head] = -INFINITY;
+  // PERSISTENT: the pair walks the work items idx = pair, pair + n_pairs, ... of the list (request in order of decreasing
+  // key count, head, 256-row query block); the prologue (barriers, TMEM, cluster sync) is paid once per SM instead of
+  // once per item, and the next item's Q tile is fetched while the current item runs.
+  struct Item { int head, q_lo, q_hi, q_base, k_lo, kv_len, n_tiles; };
+  auto decode = [&](int idx) -> Item {
+    Item it;
+    int req = 0, rem = idx, nqb = (p.n_q + 2 * TQ - 1) / (2 * TQ);
+    if (p.cu_q) {
+      for (int i = 0; i < p.R; ++i) {
+        req = p.order[i];
+        nqb = (p.cu_q[req + 1] - p.cu_q[req] + 2 * TQ - 1) / (2 * TQ);
+        if (rem < nqb * p.H || i == p.R - 1) break;
+        rem -= nqb * p.H;
       }
     }
-    return;
-  }
+    it.head = rem / nqb;
+    it.q_lo = p.cu_q ? p.cu_q[req] : 0;
+    it.q_hi = p.cu_q ? p.cu_q[req + 1] : p.n_q;
+    it.q_base = it.q_lo + (rem - it.head * nqb) * (2 * TQ) + (int)crank * TQ;   // this CTA's 128 rows (may lie past q_hi)
+    const int k_lo0 = p.cu_k ? p.cu_k[req] : 0, k_hi0 = p.cu_k ? p.cu_k[req + 1] : p.n_k;
+    const int ssz = (k_hi0 - k_lo0 + p.n_shards - 1) / p.n_shards;
+    int k_lo = k_lo0 + p.shard * ssz, k_hi = k_lo0 + (p.shard + 1) * ssz;
+    if (k_lo > k_hi0) k_lo = k_hi0;
+    if (k_hi > k_hi0) k_hi = k_hi0;
+    it.k_lo = k_lo;
+    it.kv_len = k_hi - k_lo;
+    it.n_tiles = (it.kv_len + TK - 1) / TK;
+    return it;
+  };
+  const int pair_id = (int)(blockIdx.x >> 1), n_pairs = (int)(gridDim.x >> 1);
 
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&tmQ);
@@ -730,7 +742,8 @@ attn_pair_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
     tma_prefetch_desc(&tmV);
   }
   if (warp == 1 && lane == 0) {
-    mbar_init(q_full(), 1);
+    mbar_init(q_full(0), 1);
+    mbar_init(q_full(1), 1);
     for (int s = 0; s < PKS; ++s) { mbar_init(k_full(s), 1); mbar_init(k_empty(s), 1); }
     for (int s = 0; s < PVS; ++s) { mbar_init(v_full(s), 1); mbar_init(v_empty(s), 1); }
     for (int g = 0; g < 2; ++g) {
@@ -764,20 +777,41 @@ attn_pair_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
   };
   // pass 0: reference = row max of key tile 0;  pass 1 (after a panic): row max over all key tiles, S only;  pass 2: as
   // pass 0 with the reference given.  Use counters of rings, buffers and barriers run on across passes.
-  const int c0 = head * HD;
   if (warp < 4) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");   // 128 x 56 + 512 x 104 <= 640 x 96
-    int kc = 0, vc = 0;            // K / V tiles produced or consumed so far (all passes)
-    int sn = 0, pn = 0;            // S tiles / PVs issued so far (all passes): S tile t goes to S[t & 1], PV t reads P[t & 1]
+    int kc = 0, vc = 0;            // K / V tiles produced or consumed so far (all items and passes)
+    int sn = 0, pn = 0;            // S tiles / PVs issued so far: S tile t goes to S[t & 1], PV t reads P[t & 1]
+    int qi = 0;                    // items with keys so far: item qi uses Q buffer qi & 1
+    bool q_have = false;           // this item's Q was prefetched during the previous one
+    for (int idx = pair_id; idx < p.n_items; idx += n_pairs) {
+    const Item it = decode(idx);
+    const int head = it.head, k_lo = it.k_lo, kv_len = it.kv_len, n_tiles = it.n_tiles;
+    const int c0 = head * HD;
+    if (n_tiles == 0) continue;    // empty shard: the softmax warps write o = 0, lse = -inf
+    const int ii = qi++;
+    const uint32_t sQi = sQ + (uint32_t)(ii & 1) * PQ_BYTES;   // this item's Q buffer
+    const bool q_had = q_have;
+    Item nxt = it;
+    q_have = false;
+    if (idx + n_pairs < p.n_items) {
+      nxt = decode(idx + n_pairs);
+      q_have = nxt.n_tiles > 0;
+    }
     for (int pass = 0;; ++pass) {
       const bool with_pv = pass != 1;
       if (warp == 0) {
         // ===================================================== K producer (+ Q once)
-        const uint32_t lead_q = mapa_cluster(q_full(), 0);
+        // Q of this item (the first item only: later ones were prefetched) and Q of the pair's next item, whose buffer
+        // was last read by the item before this one (complete: every item ends with a pair-wide barrier)
         if (pass == 0 && elect_one()) {
-          if (leader_cta) mbar_expect_tx(q_full(), 2 * PQ_BYTES);
-          tma_load_2d_pair(sQ, &tmQ, c0, q_base, lead_q);
-          tma_load_2d_pair(sQ + PQ_HALF, &tmQ, c0 + 64, q_base, lead_q);
+          auto load_q = [&](const Item& q, int b) {
+            const uint32_t lead_q = mapa_cluster(q_full(b), 0);
+            if (leader_cta) mbar_expect_tx(q_full(b), 2 * PQ_BYTES);
+            tma_load_2d_pair(sQ + b * PQ_BYTES, &tmQ, q.head * HD, q.q_base, lead_q);
+            tma_load_2d_pair(sQ + b * PQ_BYTES + PQ_HALF, &tmQ, q.head * HD + 64, q.q_base, lead_q);
+          };
+          if (!q_had) load_q(it, ii & 1);
+          if (q_have) load_q(nxt, (ii + 1) & 1);
         }
         for (int j = 0; j < n_tiles; ++j, ++kc) {
           const int s = kc % PKS;
@@ -822,7 +856,7 @@ attn_pair_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
             const uint32_t ka = sK + s * PKV_BYTES;
 #pragma unroll
             for (int k = 0; k < HD / 16; ++k)
-              umma_ss_pair(d, desc_kmajor_sw128(sQ + (k >> 2) * PQ_HALF + (k & 3) * 32),
+              umma_ss_pair(d, desc_kmajor_sw128(sQi + (k >> 2) * PQ_HALF + (k & 3) * 32),
                            desc_kmajor_sw128(ka + (k >> 2) * PK_HALF + (k & 3) * 32), idesc_s, k != 0);
             umma_commit_pair(s_full(g), (uint16_t)3);
             umma_commit_pair(k_empty(s), (uint16_t)3);
@@ -854,7 +888,7 @@ attn_pair_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
           __syncwarp();
           ++vc; ++pn;
         };
-        if (pass == 0) { mbar_wait_poll(q_full(), 0); tc_fence_after(); }
+        if (pass == 0) { mbar_wait_poll(q_full(ii & 1), (uint32_t)(ii >> 1) & 1u); tc_fence_after(); }
         // order = the order the events arrive in: S(j + 2) as soon as S(j) has been read (at the start of tile j's
         // softmax), PV(j - 1) when P(j - 1) is complete
         for (int i = 0; i < 2 && i < n_tiles; ++i) issue_s();
@@ -864,9 +898,10 @@ attn_pair_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
         }
         if (with_pv) issue_pv(n_tiles - 1);
       }
-      if (pass == 2) break;
+      if (pass == 2) { tc_fence_before(); cluster_sync_all(); tc_fence_after(); break; }   // O has been read: next item
       if (pass == 0 && !pair_panicked()) break;
       if (pass == 1) { tc_fence_before(); cluster_sync_all(); tc_fence_after(); }   // pass 1 -> 2 boundary (see the softmax warps)
+    }
     }
   } else {
     asm volatile("setmaxnreg.inc.sync.aligned.u32 104;");
@@ -879,7 +914,6 @@ attn_pair_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
     const int kq = grp * 2 + h;                    // the row's four threads, for the 4-way reductions and the epilogue
     const int quad = warp & 3;                     // TMEM lane quadrant of this warp
     const int r_in = quad * 32 + lane;             // row inside this CTA's Q tile
-    const int row = q_base + r_in;
     const uint32_t lane_off = (uint32_t)(quad * 32) << 16;
     const uint32_t s_addr = tmem_base + TM_S + grp * 128 + h * SK + lane_off;
     const uint32_t p_addr = tmem_base + TM_P + h * 32 + lane_off;      // + 64 * (pt & 1)
@@ -900,11 +934,30 @@ attn_pair_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
         asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster) : "memory");
     };
     float m_used = 0.f;
+#ifdef DIT_ATTN_TRACE
+    unsigned long long tr[4][8]; int tr_n = 0; const bool tr_on = blockIdx.x == 0 && warp == 4 && lane == 0;
+#endif
+    int st = 0, ptn = 0, od = 0;                   // S tiles / P tiles / PV passes so far (all items and passes)
+    for (int idx = pair_id; idx < p.n_items; idx += n_pairs) {
+    const Item it = decode(idx);
+    const int head = it.head, q_hi = it.q_hi, kv_len = it.kv_len, n_tiles = it.n_tiles;
+    const int row = it.q_base + r_in;
+    if (n_tiles == 0) {                            // empty shard: o = 0, lse = -inf (R18)
+      if (row < q_hi) {
+        const float z[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        for (int cc = 0; cc < 32; cc += 8) st8<bf16>(p.o + (int64_t)row * p.o_stride + head * HD + kq * 32 + cc, z);
+        if (kq == 0 && p.lse) p.lse[(int64_t)row * p.H + head] = -INFINITY;
+      }
+      continue;
+    }
+    TRACE(0);
     for (int pass = 0;; ++pass) {
       float l = 0.f, tile_worst = 0.f, mx_run = -INFINITY;
-      const int base = pass * n_tiles;             // global index of this pass's first key tile
-      const int pbase = pass == 2 ? n_tiles : 0;   // ... minus this = its P index (pass 1 writes no P)
-      if (pass == 0 && grp == 1) {                 // the reference comes from group 0's first tile
+      const int base = st;                         // global index of this pass's first key tile
+      const int pbase = base - ptn;                // ... minus this = its P index (pass 1 writes no P)
+      st += n_tiles;
+      if (pass != 1) ptn += n_tiles;
+      if (pass == 0 && grp != (base & 1)) {        // the reference comes from the other group's first tile
         asm volatile("bar.sync %0, 128;" ::"r"(5 + quad) : "memory");
         m_used = m_row[r_in];
       }
@@ -913,6 +966,7 @@ attn_pair_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
         uint32_t s0[32], s1[32];
         if (valid > 0) {
           mbar_wait(b_sfull, (uint32_t)(t >> 1) & 1u);
+          if (t == base) TRACE(1);
           tc_fence_after();
           tmem_ld32(s_addr + 0, s0);
           tmem_ld32(s_addr + 32, s1);
@@ -927,10 +981,10 @@ attn_pair_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
           continue;
         }
         if (valid > 0 && valid < SK) { mask32(s0, valid); mask32(s1, valid - 32); }   // -inf: before the row max; P = 0
-        if (t == 0) {                              // the row max of the first key tile is the reference of the pass
+        if (pass == 0 && t == base) {              // the row max of the first key tile is the reference of the pass
           *red = valid > 0 ? fmaxf(max32(s0), max32(s1)) : -INFINITY;
           asm volatile("bar.sync %0, 64;" ::"r"(1 + quad) : "memory");
-          m_used = fmaxf(red0[r_in], red0[128 + r_in]) * c;       // kq = 0, 1: group 0's two halves; c > 0
+          m_used = fmaxf(red0[grp * 256 + r_in], red0[grp * 256 + 128 + r_in]) * c;   // this group's two halves; c > 0
           if (h == 0) m_row[r_in] = m_used;
           __threadfence_block();
           asm volatile("bar.arrive %0, 128;" ::"r"(5 + quad) : "memory");     // group 1 may read m_row
@@ -958,7 +1012,9 @@ attn_pair_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
           tmem_st_wait();
         }
         arrive(a_pfull + 8u * bp);
+        if (t == base) TRACE(2);
       }
+      TRACE(3);
       if (pass == 1) {
         *red = mx_run;
         asm volatile("bar.sync %0, 128;" ::"r"(9 + quad) : "memory");
@@ -973,7 +1029,9 @@ attn_pair_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
       *red = l;
       asm volatile("bar.sync %0, 128;" ::"r"(9 + quad) : "memory");
       l = (red0[r_in] + red0[128 + r_in]) + (red0[256 + r_in] + red0[384 + r_in]);
-      mbar_wait(o_done(), pass == 0 ? 0u : 1u);
+      mbar_wait(o_done(), (uint32_t)od & 1u);
+      TRACE(4);
+      ++od;
       tc_fence_after();
       const float inv = 1.0f / l;                  // l > 0: the first tile has at least one key
       const bool row_ok = row < q_hi;
@@ -994,9 +1052,26 @@ attn_pair_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
       }
       if (kq == 0 && row_ok && p.lse != nullptr)
         p.lse[(int64_t)row * p.H + head] = 0.6931471805599453f * (m_used + log2f(l));
-      if (pass == 2) break;
-      if (!pair_panicked()) break;
+      TRACE(5);
+      if (pass == 2) {                             // O has been read: the next item's first PV may overwrite it; the panic
+        if (threadIdx.x == 128)                    // flag was read by both CTAs two pair-wide barriers ago
+          asm volatile("st.shared.u32 [%0], %1;" ::"r"(panic_addr), "r"(0u) : "memory");
+        tc_fence_before(); cluster_sync_all(); tc_fence_after();
+        break;
+      }
+      { const bool pp = pair_panicked(); TRACE(6);
+#ifdef DIT_ATTN_TRACE
+        if (tr_on) ++tr_n;
+#endif
+        if (!pp) break; }
     }
+    }
+#ifdef DIT_ATTN_TRACE
+    if (tr_on) for (int i = 0; i < tr_n && i < 4; ++i)
+      printf("item %d: start->S0 %llu  S0->P0 %llu  P0->lastP %llu  lastP->o_done %llu  epilogue %llu  sync %llu  | next start +%llu ns\n", i,
+             tr[i][1] - tr[i][0], tr[i][2] - tr[i][1], tr[i][3] - tr[i][2], tr[i][4] - tr[i][3], tr[i][5] - tr[i][4], tr[i][6] - tr[i][5],
+             i + 1 < tr_n ? tr[i + 1][0] - tr[i][6] : 0ull);
+#endif
   }
   tc_fence_before();
   __syncthreads();
@@ -1038,15 +1113,16 @@ dit_status launch_attn_tc(const AttnArgs& a, cudaStream_t st) {
   }();
   static const int pair_min_k = []() {  // DIT_ATTN_PAIR_MIN_K overrides the switch-over length (tuning knob)
     const char* e = getenv("DIT_ATTN_PAIR_MIN_K");
-    return e != nullptr ? atoi(e) : 8192;
+    return e != nullptr ? atoi(e) : 2048;
   }();
   // K / V maps need a valid base even when there are no keys (the kernel then never issues a load)
   const void* kb = a.n_k > 0 ? a.k : a.q;
   const void* vb = a.n_k > 0 ? a.v : a.q;
   const uint64_t nk_rows = a.n_k > 0 ? a.n_k : 1;
   const uint64_t kv_ld = a.n_k > 0 ? a.kv_stride : a.q_stride;
-  // Key sequences from 8192 (64 key tiles): the pair kernel; shorter ones: attn_tc_kernel, whose per-work-item prologue
-  // and drain weigh less (measured, H = 24: N = 4352: 1040 vs 970 TFLOP/s; N = 8192: 1100 vs 1220; 16384: 1244 vs 1359).
+  // Key sequences from 2048 keys (16 key tiles): the persistent pair kernel; shorter ones: attn_tc_kernel, whose fill and
+  // drain per work item weigh less (measured alone, H = 24, attn_tc_kernel vs pair: N = 1024: 419 vs 360 TFLOP/s; 2048:
+  // 599 vs 735; 4352: 1040 vs 1072; 8192: 1100 vs 1274; 16384: 1244 vs 1385; 32768: 1173 vs 1262).
   int max_k = a.n_k;
   if (a.cu_k_host) {
     max_k = 0;
@@ -1072,8 +1148,15 @@ dit_status launch_attn_tc(const AttnArgs& a, cudaStream_t st) {
       return a.cu_k_host[x + 1] - a.cu_k_host[x] > a.cu_k_host[y + 1] - a.cu_k_host[y];
     });
   ProfScope _prof(DIT_KC_ATTN, st);
-  if (pair_kernel) {   // one CTA pair per (256-row query block, head, request)
-    dim3 pgrid(2 * cdiv(max_q, 2 * TQ), a.H, a.cu_q ? a.R : 1);
+  if (pair_kernel) {   // persistent: one CTA pair per SM pair walks the (request, head, 256-row query block) items
+    int n_items = 0;
+    if (a.cu_q && a.cu_q_host) for (int r = 0; r < a.R; ++r) n_items += cdiv(a.cu_q_host[r + 1] - a.cu_q_host[r], 2 * TQ) * a.H;
+    else n_items = cdiv(a.n_q, 2 * TQ) * a.H;
+    p.R = a.cu_q ? a.R : 1;
+    p.n_items = n_items;
+    int sms = 148;
+    { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); }
+    dim3 pgrid(2 * min(n_items, sms / 2), 1, 1);
     DIT_CUDA_OK(launch_pdl(attn_pair_kernel, pgrid, dim3(ATTN_THREADS), PAIR_SMEM, st, 2, tq, tk, tv, p));
     DIT_LAUNCH_CHECK();
     return DIT_OK;
