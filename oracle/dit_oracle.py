@@ -21,7 +21,8 @@ invariance; merge closed forms; LN / RMSNorm / RoPE / GELU / patchify invariants
 (layer_norm, scaled_dot_product_attention, gelu(tanh), silu) as special cases; stored hand-computed
 fixtures under tests/golden/; the trajectory (`dit_sample`): constant-velocity closed form, guidance special cases,
 semigroup property; the block in all three modes re-derived with torch library routines and a by-hand RoPE
-(`test_block_by_hand_one_block`, `test_joint_block_by_hand_rmsnorm_then_rope`: [ctx ; x] order, cond position 0,
+(`test_dual_stream_*`: the dual-stream block against a torch-library transcription and against the single-stream block
+with the same weights in both streams; `test_block_by_hand_one_block`, `test_joint_block_by_hand_rmsnorm_then_rope`: [ctx ; x] order, cond position 0,
 RMSNorm BEFORE RoPE, interleaved pairs; `test_cross_block_by_hand`: wkv rows [k | v], ungated / unmodulated / un-roped
 cross branch, also for `block_rows` in cross mode).  Mutants of each of those lines fail the CPU suite.
 PARITY UNPINNED: the *composition order* of the block (R1, R9, R10, R12: which sub-layer follows which,
@@ -198,6 +199,52 @@ def conditioning(cfg, W, temb):
     return c.reshape(-1), mods, modf
 
 
+def conditioning_txt(cfg, W, c):
+    """Dual-stream blocks (R37): the text stream's own modulation, mod_txt_l = Wmod_txt_l SiLU(c) + bmod_txt_l (6 chunks
+    in the same order as the image stream's)."""
+    sc = silu(_d(c).reshape(1, -1))
+    return [linear(sc, W[f"blocks.{l}.txt.mod.w"], W[f"blocks.{l}.txt.mod.b"]).reshape(6, -1) for l in range(cfg["n_blocks"])]
+
+
+def dual_stream_block(cfg, W, l, x, Lc, m_img, m_txt, ang, split_p, taps):
+    """One DUAL-STREAM joint block (reading R37 — the MMDiT form of the models the paper
+    serves): the text rows x[:Lc] and the image rows x[Lc:] each have their OWN modulation, QKV projection
+    (and QK-RMSNorm gains), out-projection and MLP (`blocks.l.txt.*` / `blocks.l.*`); ONE attention runs over the joint
+    sequence [txt ; img] (RoPE as in the single-stream block: text rows at position 0).  Everything else is step 5."""
+    D, H, d, eps = cfg["hidden"], cfg["n_heads"], cfg["head_dim"], cfg["ln_eps"]
+    parts = (("txt", f"blocks.{l}.txt.", x[:Lc], m_txt), ("img", f"blocks.{l}.", x[Lc:], m_img))
+    qs, ks, vs = [], [], []
+    for name, pre, xs, m in parts:
+        y1 = modulate(xs, m[0], m[1], eps)
+        qkv = linear(y1, W[pre + "attn.wqkv"], W[pre + "attn.bqkv"])
+        q, k, v = (qkv[:, i * D:(i + 1) * D].reshape(-1, H, d) for i in range(3))
+        if cfg["qk_rmsnorm"]:
+            q = rms_norm_heads(q, _d(W[pre + "attn.gq"]), cfg["rms_eps"])
+            k = rms_norm_heads(k, _d(W[pre + "attn.gk"]), cfg["rms_eps"])
+        qs.append(q); ks.append(k); vs.append(v)
+        if taps is not None:
+            taps[f"b{l}.{name}.y1"] = y1
+    q, k, v = torch.cat(qs, 0), torch.cat(ks, 0), torch.cat(vs, 0)               # [txt ; img]
+    if ang is not None:
+        q, k = apply_rope(q, ang), apply_rope(k, ang)
+    o, _ = attention_split(q, k, v, split_p)
+    o = o.reshape(-1, D)
+    if taps is not None:
+        taps[f"b{l}.q"], taps[f"b{l}.k"], taps[f"b{l}.v"], taps[f"b{l}.o"] = q.reshape(-1, D), k.reshape(-1, D), v.reshape(-1, D), o
+    outs = []
+    for (name, pre, xs, m), os_ in zip(parts, (o[:Lc], o[Lc:])):
+        xa = xs + m[2] * linear(os_, W[pre + "attn.wo"], W[pre + "attn.bo"])
+        y2 = modulate(xa, m[3], m[4], eps)
+        u = gelu_tanh(linear(y2, W[pre + "mlp.w1"], W[pre + "mlp.b1"]))
+        outs.append(xa + m[5] * linear(u, W[pre + "mlp.w2"], W[pre + "mlp.b2"]))
+        if taps is not None:
+            taps[f"b{l}.{name}.x_attn"], taps[f"b{l}.{name}.y2"], taps[f"b{l}.{name}.u"] = xa, y2, u
+    x = torch.cat(outs, 0)
+    if taps is not None:
+        taps[f"b{l}.x_mlp"] = x.clone()
+    return x
+
+
 def self_attention_block(cfg, W, l, y, ang, split_p, taps, rows=None):
     """§8(c) step 5, attention half: q,k,v = split(Wqkv y + b); QK-RMSNorm (R5); RoPE (R6); softmax(QK^T/sqrt d)V.
     `rows` (optional index tensor) restricts the QUERY rows (sampled-row checks at large sizes);
@@ -239,9 +286,10 @@ def dit_step(cfg, W, latents, temb, cond=None, split_p=1, taps=None):
     Lc = 0
     if mode != "none":
         ctx = linear(_d(cond), W["cond_proj.w"], W["cond_proj.b"])                               # step 4
-    if mode == "joint":
+    if mode in ("joint", "joint2"):
         Lc = ctx.shape[0]
         x = torch.cat([ctx, x], dim=0)                                                            # [ctx ; x] (R9)
+    mods_txt = conditioning_txt(cfg, W, c) if mode == "joint2" else None
     ang = None
     if sum(cfg["rope_dims"]) > 0:
         pos = token_positions(grid)
@@ -253,6 +301,9 @@ def dit_step(cfg, W, latents, temb, cond=None, split_p=1, taps=None):
         taps["mod"] = torch.stack(mods, 0) if mods else torch.zeros(0, 6, D, dtype=F64)
         taps["modf"] = modf
     for l in range(cfg["n_blocks"]):
+        if mode == "joint2":                                                                      # dual-stream block (R37)
+            x = dual_stream_block(cfg, W, l, x, Lc, mods[l], mods_txt[l], ang, split_p, taps)
+            continue
         sh1, sc1, g1, sh2, sc2, g2 = mods[l]                                                      # step 2 order
         y1 = modulate(x, sh1, sc1, eps)
         o, _ = self_attention_block(cfg, W, l, y1, ang, split_p, taps)

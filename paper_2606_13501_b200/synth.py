@@ -92,7 +92,7 @@ class DiTShape:
     patch: tuple                # (pf, ph, pw)
     temb_dim: int
     cond_dim: int
-    cond_mode: str              # "none" | "joint" | "cross"
+    cond_mode: str              # "none" | "joint" | "cross" | "joint2" (dual-stream joint blocks)
     rope_dims: tuple            # per axis (f, h, w); all zero = no RoPE
     qk_rmsnorm: bool
     latent_grid: tuple          # (F, H, W) of the latent (before patching)
@@ -189,6 +189,9 @@ def weight_shapes(s: DiTShape) -> dict:
             w[p + "cross.wo"] = (D, D); w[p + "cross.bo"] = (D,)
         w[p + "mlp.w1"] = (F, D); w[p + "mlp.b1"] = (F,)
         w[p + "mlp.w2"] = (D, F); w[p + "mlp.b2"] = (D,)
+        if s.cond_mode == "joint2":      # dual-stream blocks: the text stream's own copy of every per-block tensor
+            for k in [k for k in w if k.startswith(p) and not k.startswith(p + "txt.")]:
+                w[p + "txt." + k[len(p):]] = w[k]
     w["final.mod.w"] = (2 * D, D); w["final.mod.b"] = (2 * D,)
     w["final.w"] = (pvC, D); w["final.b"] = (pvC,)
     return w

@@ -469,6 +469,72 @@ def test_block_rows_cross_equals_step_rows():
     assert torch.allclose(got, taps["b1.x_mlp"][rows], rtol=1e-12, atol=1e-14)
 
 
+def test_dual_stream_equals_single_stream_when_both_streams_share_weights():
+    """Dual-stream joint blocks (R37) with the text stream's tensors set equal to the image stream's ARE the single-stream
+    joint blocks (R9): same rows, same order, one attention over [ctx ; x]."""
+    s2 = _tiny(cond_mode="joint2", rope_dims=(0, 8, 8), qk_rmsnorm=True)
+    s1 = _tiny(cond_mode="joint", rope_dims=(0, 8, 8), qk_rmsnorm=True)
+    W1 = _wide_gains(synth.make_weights(s1), s1)
+    W2 = dict(W1)
+    for k, v in W1.items():
+        if k.startswith("blocks."):
+            l, rest = k.split(".", 2)[1:]
+            W2[f"blocks.{l}.txt.{rest}"] = v
+    assert set(W2) == set(synth.weight_shapes(s2))
+    I = synth.make_inputs(s1)
+    a = O.dit_step(O.cfg_from_shape(s1), W1, I["latents"], I["temb"], I["cond"])
+    b = O.dit_step(O.cfg_from_shape(s2), W2, I["latents"], I["temb"], I["cond"])
+    assert torch.allclose(a, b, rtol=1e-12, atol=1e-14)
+    b4 = O.dit_step(O.cfg_from_shape(s2), W2, I["latents"], I["temb"], I["cond"], split_p=4)
+    assert torch.allclose(a, b4, rtol=1e-11, atol=1e-13)
+
+
+def test_dual_stream_block_by_hand():
+    """One dual-stream block with DIFFERENT weights per stream, re-derived with torch library routines: per-stream adaLN
+    (own modulation), QKV, QK-RMSNorm (own gains), by-hand RoPE, ONE SDPA over [txt ; img], per-stream gated out-projection
+    and MLP.  Fails if the streams' weights are swapped, the text rows do not attend to the image rows, the text stream
+    takes the image stream's modulation / gains, or the text rows are placed after the image rows."""
+    s = _tiny(n_blocks=1, cond_mode="joint2", rope_dims=(0, 8, 8), qk_rmsnorm=True)
+    W, I = _wide_gains(synth.make_weights(s), s), synth.make_inputs(s)
+    taps = {}
+    O.dit_step(O.cfg_from_shape(s), W, I["latents"], I["temb"], I["cond"], taps=taps)
+    Fn = torch.nn.functional
+    Wd = {k: v.double() for k, v in W.items()}
+    D, H, d, Lc = 32, 2, 16, 5
+    c = Fn.linear(Fn.silu(Fn.linear(I["temb"].double(), Wd["t_mlp.w1"], Wd["t_mlp.b1"])), Wd["t_mlp.w2"], Wd["t_mlp.b2"])
+    x = taps["x0"]
+    pos = [(0, 0, 0)] * Lc + [(0, hh, ww) for hh in range(4) for ww in range(4)]
+    streams = (("blocks.0.txt.", slice(0, Lc)), ("blocks.0.", slice(Lc, None)))
+    mods, qkvs = {}, {}
+    for pre, rows in streams:
+        m = Fn.linear(Fn.silu(c), Wd[pre + "mod.w"], Wd[pre + "mod.b"]).reshape(6, D)
+        y = Fn.layer_norm(x[rows], (D,), eps=1e-6) * (1 + m[1]) + m[0]
+        q, k, v = [t.reshape(-1, H, d) for t in Fn.linear(y, Wd[pre + "attn.wqkv"], Wd[pre + "attn.bqkv"]).split(D, dim=1)]
+        q = Fn.rms_norm(q, (d,), weight=Wd[pre + "attn.gq"], eps=1e-6)
+        k = Fn.rms_norm(k, (d,), weight=Wd[pre + "attn.gk"], eps=1e-6)
+        mods[pre], qkvs[pre] = m, (q, k, v)
+    q, k, v = [torch.cat([qkvs["blocks.0.txt."][i], qkvs["blocks.0."][i]], 0) for i in range(3)]
+    q, k = _hand_rope(q, pos, (0, 8, 8), 10000.0), _hand_rope(k, pos, (0, 8, 8), 10000.0)
+    o = Fn.scaled_dot_product_attention(q.permute(1, 0, 2), k.permute(1, 0, 2), v.permute(1, 0, 2)).permute(1, 0, 2).reshape(-1, D)
+    outs = []
+    for pre, rows in streams:
+        m = mods[pre]
+        xa = x[rows] + m[2] * Fn.linear(o[rows], Wd[pre + "attn.wo"], Wd[pre + "attn.bo"])
+        y = Fn.layer_norm(xa, (D,), eps=1e-6) * (1 + m[4]) + m[3]
+        outs.append(xa + m[5] * Fn.linear(Fn.gelu(Fn.linear(y, Wd[pre + "mlp.w1"], Wd[pre + "mlp.b1"]), approximate="tanh"),
+                                          Wd[pre + "mlp.w2"], Wd[pre + "mlp.b2"]))
+    want = torch.cat(outs, 0)
+    assert torch.allclose(taps["b0.x_mlp"], want, rtol=1e-10, atol=1e-12)
+    # the streams really differ: giving the text rows the image stream's weights changes the text rows
+    Wsw = dict(W)
+    for kk in list(W):
+        if kk.startswith("blocks.0.txt."):
+            Wsw[kk] = W["blocks.0." + kk[len("blocks.0.txt."):]]
+    t2 = {}
+    O.dit_step(O.cfg_from_shape(s), Wsw, I["latents"], I["temb"], I["cond"], taps=t2)
+    assert float((t2["b0.x_mlp"][:Lc] - want[:Lc]).abs().max()) > 1e-3
+
+
 def test_varlen_is_per_request_and_block_rows():
     s = _tiny(cond_mode="joint", rope_dims=(0, 8, 8), qk_rmsnorm=True)
     W = synth.make_weights(s)
