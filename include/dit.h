@@ -57,7 +57,7 @@ typedef enum {
 } dit_status;
 
 typedef enum { DIT_F32 = 0, DIT_BF16 = 1 } dit_dtype;
-typedef enum { DIT_COND_NONE = 0, DIT_COND_JOINT = 1, DIT_COND_CROSS = 2 } dit_cond_mode;
+typedef enum { DIT_COND_NONE = 0, DIT_COND_JOINT = 1, DIT_COND_CROSS = 2, DIT_COND_JOINT2 = 3 } dit_cond_mode;
 
 /* POD configuration (all ints 32-bit).  struct_size = sizeof(dit_config) guards ABI drift. */
 typedef struct {
@@ -73,7 +73,9 @@ typedef struct {
   int32_t temb_dim;        /* width of the timestep embedding passed to dit_step */
   int32_t cond_dim;        /* width of a conditioning token (ignored for DIT_COND_NONE) */
   int32_t cond_mode;       /* dit_cond_mode: joint = [cond ; image] one sequence, single stream (R9);
-                              cross = extra cross-attention sub-layer per block (R10) */
+                              cross = extra cross-attention sub-layer per block (R10); joint2 = DUAL-STREAM joint
+                              blocks (R37): one sequence [cond ; image] and one attention, but
+                              the cond rows have their own per-block weights `blocks.{l}.txt.*` */
   int32_t rope_dims[3];    /* head-dim segment per axis (f, h, w), each even, sum == head_dim, or all 0
                               for no RoPE (R6) */
   float rope_theta;        /* 10000 */
@@ -94,6 +96,8 @@ typedef struct {
  *   blocks.{l}.attn.wqkv [3D,D] .attn.bqkv [3D] (rows: q | k | v; head h = rows h*d..)  .attn.gq [d] .attn.gk [d]
  *   blocks.{l}.attn.wo [D,D] .attn.bo [D]   blocks.{l}.mlp.w1 [F,D] .mlp.b1 [F] .mlp.w2 [D,F] .mlp.b2 [D]
  *   blocks.{l}.cross.wq [D,D] .bq [D] .wkv [2D,D] .bkv [2D] .gq [d] .gk [d] .wo [D,D] .bo [D]   (cross mode)
+ *   blocks.{l}.txt.{mod.w, mod.b, attn.wqkv, attn.bqkv, attn.gq, attn.gk, attn.wo, attn.bo, mlp.w1, mlp.b1, mlp.w2, mlp.b2}
+ *        (joint2 mode: the text stream's copy, same shapes as the image stream's blocks.{l}.*)
  *   final.mod.w [2D,D] final.mod.b [2D] (shift_f, scale_f)   final.w [C*pv, D] final.b [C*pv] */
 typedef struct {
   const char* name;

@@ -13,7 +13,7 @@ LIB_PATH = os.path.join(HERE, "libdit_b200.so")
 
 DIT_OK = 0
 DIT_F32, DIT_BF16 = 0, 1
-COND = {"none": 0, "joint": 1, "cross": 2}
+COND = {"none": 0, "joint": 1, "cross": 2, "joint2": 3}
 EPI_BIAS, EPI_BIAS_GELU, EPI_BIAS_F32 = 0, 1, 2
 TAP = dict(x=0, y=1, qkv=2, o=3, u=5, c=6, mod=7, tok=8)
 STAGE = dict(y1=0, qkv=1, attn=2, oproj=3, cross=4, y2=5, fc1=6, fc2=7)
@@ -131,7 +131,7 @@ def make_config(shape, split_p=1, max_tokens=None, max_requests=1, max_cond_toke
     c.rope_dims = (C.c_int32 * 3)(*shape.rope_dims)
     c.rope_theta, c.ln_eps, c.rms_eps = shape.rope_theta, shape.ln_eps, shape.rms_eps
     c.qk_rmsnorm, c.split_p = int(shape.qk_rmsnorm), split_p
-    n = shape.n_tokens + (shape.n_cond if shape.cond_mode == "joint" else 0)
+    n = shape.n_tokens + (shape.n_cond if shape.cond_mode in ("joint", "joint2") else 0)
     c.max_tokens = int(max_tokens if max_tokens is not None else n)
     c.max_requests = max_requests
     c.max_cond_tokens = int(max_cond_tokens if max_cond_tokens is not None else (shape.n_cond if shape.cond_mode != "none" else 0))
@@ -199,7 +199,7 @@ class Dit:
         return out_host
 
     def _varlen_geom(self, shapes, n_cond):
-        joint = self.cfg.cond_mode == COND["joint"]
+        joint = self.cfg.cond_mode in (COND["joint"], COND["joint2"])
         p = self.cfg.patch
         cu, grids = [0], []
         for r, shp in enumerate(shapes):

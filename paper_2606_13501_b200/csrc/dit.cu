@@ -66,6 +66,8 @@ static size_t esize(int dtype) { return dtype == DIT_F32 ? 4 : 2; }
 struct BlockW {
   const void *mod_w, *mod_b, *wqkv, *bqkv, *gq, *gk, *wo, *bo, *w1, *b1, *w2, *b2;
   const void *cwq, *cbq, *cwkv, *cbkv, *cgq, *cgk, *cwo, *cbo;
+  // dual-stream joint blocks (DIT_COND_JOINT2, R37): the text stream's own copy of the per-block tensors
+  const void *t_mod_w, *t_mod_b, *t_wqkv, *t_bqkv, *t_gq, *t_gk, *t_wo, *t_bo, *t_w1, *t_b1, *t_w2, *t_b2;
 };
 
 struct Workspace {
@@ -140,7 +142,7 @@ static bool carve(const dit_config& c, char* base, Workspace* w) {
   w->u = take(Tm * F * es);
   w->c1 = (float*)take(Rm * D * 4);
   w->c = (float*)take(Rm * D * 4);
-  w->mod = (float*)take(Rm * (L * 6 * D + 2 * D) * 4);
+  w->mod = (float*)take(Rm * (L * (c.cond_mode == DIT_COND_JOINT2 ? 12 : 6) * D + 2 * D) * 4);   // [img blocks | final | txt blocks]
   w->rope_c = (float*)take(Tm * (c.head_dim / 2) * 4);
   w->rope_s = (float*)take(Tm * (c.head_dim / 2) * 4);
   w->patches = take(Tm * pvC * es);
@@ -152,7 +154,7 @@ static bool carve(const dit_config& c, char* base, Workspace* w) {
   w->cu_dev = (int32_t*)take((Rm + 1) * 4);
   w->cu_cond_dev = (int32_t*)take((Rm + 1) * 4);
   w->meta_dev = (SeqMeta*)take(Rm * sizeof(SeqMeta));
-  w->gemv_tab = (GemvBatch*)take((L + 4) * sizeof(GemvBatch));
+  w->gemv_tab = (GemvBatch*)take((2 * L + 4) * sizeof(GemvBatch));
   w->stage_in = take(Tm * pvC * es + Rm * c.temb_dim * 4 + Lcm * c.cond_dim * es + 1024);
   w->stage_out = take(Tm * pvC * es);
   w->sample_x = (float*)take(Tm * pvC * 4);
@@ -188,8 +190,10 @@ static dit_status validate(const dit_config* c) {
   DIT_REQUIRE(c->latent_channels > 0 && c->patch[0] > 0 && c->patch[1] > 0 && c->patch[2] > 0, DIT_ERR_INVALID_ARG,
               "latent_channels / patch must be positive");
   DIT_REQUIRE(c->temb_dim > 0 && c->temb_dim % 8 == 0, DIT_ERR_UNSUPPORTED, "temb_dim %d must be a multiple of 8", c->temb_dim);
-  DIT_REQUIRE(c->cond_mode >= DIT_COND_NONE && c->cond_mode <= DIT_COND_CROSS, DIT_ERR_INVALID_ARG, "cond_mode %d", c->cond_mode);
+  DIT_REQUIRE(c->cond_mode >= DIT_COND_NONE && c->cond_mode <= DIT_COND_JOINT2, DIT_ERR_INVALID_ARG, "cond_mode %d", c->cond_mode);
   DIT_REQUIRE(c->cond_mode == DIT_COND_NONE || c->cond_dim > 0, DIT_ERR_INVALID_ARG, "cond_dim %d", c->cond_dim);
+  DIT_REQUIRE(c->cond_mode != DIT_COND_JOINT2 || c->n_blocks <= 128, DIT_ERR_UNSUPPORTED,
+              "dual-stream blocks: n_blocks %d > 128 (one modulation launch covers 2 L + 1 matrices)", c->n_blocks);
   const int rs = c->rope_dims[0] + c->rope_dims[1] + c->rope_dims[2];
   DIT_REQUIRE(rs == 0 || rs == c->head_dim, DIT_ERR_INVALID_ARG, "sum(rope_dims) = %d must be 0 or head_dim", rs);
   for (int a = 0; a < 3; ++a)
@@ -274,7 +278,7 @@ static dit_status upload_geom(dit_handle hd, const StepGeom& g, cudaStream_t st)
   const dit_config& c = hd->cfg;
   Workspace& w = hd->ws;
   const int R = g.R, T = g.cu[R], d = c.head_dim;
-  const bool joint = c.cond_mode == DIT_COND_JOINT;
+  const bool joint = c.cond_mode == DIT_COND_JOINT || c.cond_mode == DIT_COND_JOINT2;
   const bool rope = (c.rope_dims[0] + c.rope_dims[1] + c.rope_dims[2]) > 0;
   std::vector<SeqMeta> meta(R);
   // The key holds everything the device copies are made from: sequence starts, the cond-token offsets of EVERY mode
@@ -324,13 +328,15 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
   const int D = c.hidden, F = c.mlp_dim, H = c.n_heads, d = c.head_dim, L = c.n_blocks, R = g.R;
   const int pvC = c.latent_channels * c.patch[0] * c.patch[1] * c.patch[2];
   const int T = g.cu[R];
-  const int64_t mod_len = (int64_t)L * 6 * D + 2 * D;
+  const bool dual = c.cond_mode == DIT_COND_JOINT2;
+  const int64_t mod_img = (int64_t)L * 6 * D + 2 * D;                 // image-stream blocks + final layer
+  const int64_t mod_len = mod_img + (dual ? (int64_t)L * 6 * D : 0);   // ... + text-stream blocks (dual-stream, R37)
   const int Rt = pair ? 1 : R;                      // timestep rows
   const int64_t mod_stride = pair ? 0 : mod_len;    // modulation row of request r = mod + r * mod_stride
   auto cond_of = [&](int r) -> const char* {
     return pair ? (const char*)pair->cond[r] : (const char*)cond + (size_t)g.cu_cond[r] * c.cond_dim * esize(c.dtype);
   };
-  const bool joint = c.cond_mode == DIT_COND_JOINT, cross = c.cond_mode == DIT_COND_CROSS;
+  const bool joint = c.cond_mode == DIT_COND_JOINT || dual, cross = c.cond_mode == DIT_COND_CROSS;
   const bool rope = (c.rope_dims[0] + c.rope_dims[1] + c.rope_dims[2]) > 0;
   auto stop = [&](int blk, int stage) { return hd->stop_block == blk && hd->stop_stage == stage; };
   {
@@ -350,7 +356,7 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
   // ---- steps 1-2: c = W2 SiLU(W1 temb + b1) + b2;  mod = Wmod SiLU(c) + bmod for ALL blocks in one launch
   RUN(launch_gemv(dt, temb, w.gemv_tab + 0, nullptr, 1, D, w.c1, D, Rt, c.temb_dim, 0, st));
   RUN(launch_gemv(dt, w.c1, w.gemv_tab + 1, nullptr, 1, D, w.c, D, Rt, D, 1, st));
-  RUN(launch_gemv(dt, w.c, w.gemv_tab + 2, nullptr, L + 1, L * 6 * D + 2 * D, w.mod, mod_len, Rt, D, 1, st));
+  RUN(launch_gemv(dt, w.c, w.gemv_tab + 2, nullptr, dual ? 2 * L + 1 : L + 1, (int)mod_len, w.mod, mod_len, Rt, D, 1, st));
 
   // ---- steps 3-4: patch-embed and cond projection write the fp32 residual stream
   for (int r = 0; r < R; ++r) {
@@ -385,8 +391,91 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
 
   // ---- step 5: blocks.  Both residual branches are added to x inside their GEMM epilogues (gemm_residual).
   const float scale = 1.0f / sqrtf((float)d);
+  // dual-stream blocks: every request is two row segments (its text rows, its image rows) with their own weights and
+  // modulation; per-row kernels and GEMMs run once per segment, attention once over the joint sequence
+  struct Seg { int row0, rows, r; bool txt; };
+  std::vector<Seg> segs;
+  if (dual)
+    for (int r = 0; r < R; ++r) {
+      const int Lc = g.ncond[r];
+      if (Lc > 0) segs.push_back({g.cu[r], Lc, r, true});
+      if (g.cu[r + 1] - g.cu[r] - Lc > 0) segs.push_back({g.cu[r] + Lc, g.cu[r + 1] - g.cu[r] - Lc, r, false});
+    }
   for (int l = 0; l < L; ++l) {
     const BlockW& b = hd->blocks[l];
+    if (dual) {
+      struct SW { const void *wqkv, *bqkv, *gq, *gk, *wo, *bo, *w1, *b1, *w2, *b2; };
+      const SW sw_img{b.wqkv, b.bqkv, b.gq, b.gk, b.wo, b.bo, b.w1, b.b1, b.w2, b.b2};
+      const SW sw_txt{b.t_wqkv, b.t_bqkv, b.t_gq, b.t_gk, b.t_wo, b.t_bo, b.t_w1, b.t_b1, b.t_w2, b.t_b2};
+      auto mod_of = [&](const Seg& sg) { return w.mod + (size_t)sg.r * mod_stride + (sg.txt ? mod_img : 0) + (size_t)l * 6 * D; };
+      auto rows_of = [&](void* base, const Seg& sg, int64_t ld) { return (void*)((char*)base + (size_t)sg.row0 * ld * es); };
+      for (const Seg& sg : segs)
+        RUN(launch_adaln(dt, w.x + (size_t)sg.row0 * D, nullptr, nullptr, mod_of(sg), mod_of(sg) + D, 0, nullptr, 1, rows_of(w.y, sg, D),
+                         sg.rows, D, c.ln_eps, st));
+      if (stop(l, DIT_STAGE_Y1)) return DIT_OK;
+      for (const Seg& sg : segs) {
+        const SW& sw = sg.txt ? sw_txt : sw_img;
+        const float* rc = rope ? w.rope_c + (size_t)sg.row0 * (d / 2) : nullptr;
+        const float* rs = rope ? w.rope_s + (size_t)sg.row0 * (d / 2) : nullptr;
+        const void* gq = c.qk_rmsnorm ? sw.gq : nullptr;
+        const void* gk = c.qk_rmsnorm ? sw.gk : nullptr;
+        if (dt == DIT_BF16 && (c.qk_rmsnorm || rope)) {
+          RUN(launch_gemm_tc_qkv(rows_of(w.y, sg, D), D, sw.wqkv, sw.bqkv, rows_of(w.qkv, sg, 3 * D), 3 * D, gq, gk, c.rms_eps, rc, rs, D,
+                                 2 * D, sg.rows, 3 * D, D, st));
+        } else {
+          RUN(gemm(dt, DIT_EPI_BIAS, rows_of(w.y, sg, D), D, sw.wqkv, sw.bqkv, rows_of(w.qkv, sg, 3 * D), 3 * D, sg.rows, 3 * D, D, st));
+          RUN(launch_qknorm_rope(dt, rows_of(w.qkv, sg, 3 * D), 3 * D, sg.rows, H, d, 2, gq, gk, c.rms_eps, rc, rs, st));
+        }
+      }
+      if (stop(l, DIT_STAGE_QKV)) return DIT_OK;
+      {
+        AttnArgs a;
+        a.q = w.qkv; a.k = (char*)w.qkv + (size_t)D * es; a.v = (char*)w.qkv + (size_t)2 * D * es;
+        a.q_stride = a.kv_stride = 3 * D;
+        a.cu_q = a.cu_k = R > 1 ? w.cu_dev : nullptr;
+        a.cu_q_host = a.cu_k_host = g.cu.data();
+        a.R = R; a.n_q = T; a.n_k = T; a.H = H; a.d = d; a.scale = 1.0f / sqrtf((float)d);
+        if (c.split_p == 1) {
+          a.o = w.o; a.o_stride = D; a.lse = nullptr; a.shard = 0; a.n_shards = 1;
+          RUN(attention(dt, a, st));
+        } else {
+          const void* op[8];
+          const float* lp[8];
+          for (int p = 0; p < c.split_p; ++p) {
+            a.o = (char*)w.o_part + (size_t)p * c.max_tokens * D * es;
+            a.o_stride = D;
+            a.lse = w.lse_part + (size_t)p * c.max_tokens * H;
+            a.shard = p; a.n_shards = c.split_p;
+            op[p] = a.o; lp[p] = a.lse;
+            RUN(attention(dt, a, st));
+          }
+          RUN(launch_merge(dt, op, lp, c.split_p, (int64_t)T * H, d, w.o, nullptr, st));
+        }
+      }
+      if (stop(l, DIT_STAGE_ATTN)) return DIT_OK;
+      for (const Seg& sg : segs) {
+        const SW& sw = sg.txt ? sw_txt : sw_img;
+        RUN(gemm_residual(dt, rows_of(w.o, sg, D), D, sw.wo, sw.bo, w.x + (size_t)sg.row0 * D, D, mod_of(sg) + 2 * D, 0, nullptr, 1,
+                          sg.rows, D, D, st));
+      }
+      if (stop(l, DIT_STAGE_OPROJ)) return DIT_OK;
+      for (const Seg& sg : segs)
+        RUN(launch_adaln(dt, w.x + (size_t)sg.row0 * D, nullptr, nullptr, mod_of(sg) + 3 * D, mod_of(sg) + 4 * D, 0, nullptr, 1,
+                         rows_of(w.y, sg, D), sg.rows, D, c.ln_eps, st));
+      if (stop(l, DIT_STAGE_Y2)) return DIT_OK;
+      for (const Seg& sg : segs) {
+        const SW& sw = sg.txt ? sw_txt : sw_img;
+        RUN(gemm(dt, DIT_EPI_BIAS_GELU, rows_of(w.y, sg, D), D, sw.w1, sw.b1, rows_of(w.u, sg, F), F, sg.rows, F, D, st));
+      }
+      if (stop(l, DIT_STAGE_FC1)) return DIT_OK;
+      for (const Seg& sg : segs) {
+        const SW& sw = sg.txt ? sw_txt : sw_img;
+        RUN(gemm_residual(dt, rows_of(w.u, sg, F), F, sw.w2, sw.b2, w.x + (size_t)sg.row0 * D, D, mod_of(sg) + 5 * D, 0, nullptr, 1,
+                          sg.rows, D, F, st));
+      }
+      if (stop(l, DIT_STAGE_FC2)) return DIT_OK;
+      continue;
+    }
     const float* m = w.mod + (size_t)l * 6 * D;
     RUN(launch_adaln(dt, w.x, nullptr, nullptr, m + 0 * D, m + 1 * D, mod_stride, cu_dev, R, w.y, T, D, c.ln_eps, st));
     if (stop(l, DIT_STAGE_Y1)) return DIT_OK;
@@ -503,7 +592,7 @@ static dit_status build_geom(dit_handle h, int R, const int32_t* cu, const int32
     const int nc = c.cond_mode == DIT_COND_NONE ? 0 : (ncond ? ncond[r] : 0);
     DIT_REQUIRE(nc >= 0, DIT_ERR_INVALID_ARG, "request %d: n_cond %d < 0", r, nc);
     g->ncond[r] = nc;
-    const int64_t Tr = Nr + (c.cond_mode == DIT_COND_JOINT ? nc : 0);
+    const int64_t Tr = Nr + (c.cond_mode == DIT_COND_JOINT || c.cond_mode == DIT_COND_JOINT2 ? nc : 0);
     DIT_REQUIRE(g->cu[r] + Tr <= c.max_tokens, DIT_ERR_INVALID_ARG, "sequence rows exceed max_tokens %d", c.max_tokens);
     g->cu[r + 1] = g->cu[r] + (int32_t)Tr;
     g->cu_cond[r + 1] = g->cu_cond[r] + nc;
@@ -555,6 +644,13 @@ dit_status dit_init(const dit_config* cfg, const dit_weight* weights, int32_t n_
     if (cfg->qk_rmsnorm) { need[p + "attn.gq"] = d; need[p + "attn.gk"] = d; }
     need[p + "attn.wo"] = D * D; need[p + "attn.bo"] = D;
     need[p + "mlp.w1"] = F * D; need[p + "mlp.b1"] = F; need[p + "mlp.w2"] = D * F; need[p + "mlp.b2"] = D;
+    if (cfg->cond_mode == DIT_COND_JOINT2) {
+      need[p + "txt.mod.w"] = 6 * D * D; need[p + "txt.mod.b"] = 6 * D;
+      need[p + "txt.attn.wqkv"] = 3 * D * D; need[p + "txt.attn.bqkv"] = 3 * D;
+      if (cfg->qk_rmsnorm) { need[p + "txt.attn.gq"] = d; need[p + "txt.attn.gk"] = d; }
+      need[p + "txt.attn.wo"] = D * D; need[p + "txt.attn.bo"] = D;
+      need[p + "txt.mlp.w1"] = F * D; need[p + "txt.mlp.b1"] = F; need[p + "txt.mlp.w2"] = D * F; need[p + "txt.mlp.b2"] = D;
+    }
     if (cfg->cond_mode == DIT_COND_CROSS) {
       need[p + "cross.wq"] = D * D; need[p + "cross.bq"] = D; need[p + "cross.wkv"] = 2 * D * D; need[p + "cross.bkv"] = 2 * D;
       need[p + "cross.gq"] = d; need[p + "cross.gk"] = d; need[p + "cross.wo"] = D * D; need[p + "cross.bo"] = D;
@@ -585,7 +681,8 @@ dit_status dit_init(const dit_config* cfg, const dit_weight* weights, int32_t n_
   h->t_w1 = G("t_mlp.w1"); h->t_b1 = G("t_mlp.b1"); h->t_w2 = G("t_mlp.w2"); h->t_b2 = G("t_mlp.b2");
   h->pe_w = G("patch_embed.w"); h->pe_b = G("patch_embed.b"); h->cp_w = G("cond_proj.w"); h->cp_b = G("cond_proj.b");
   h->fm_w = G("final.mod.w"); h->fm_b = G("final.mod.b"); h->f_w = G("final.w"); h->f_b = G("final.b");
-  std::vector<GemvBatch> tab(L + 3);
+  const bool dual = cfg->cond_mode == DIT_COND_JOINT2;
+  std::vector<GemvBatch> tab((dual ? 2 * L : L) + 3);
   tab[0] = {h->t_w1, h->t_b1, (int32_t)D, 0, 0, 0};
   tab[1] = {h->t_w2, h->t_b2, (int32_t)D, 0, 0, 0};
   for (int l = 0; l < L; ++l) {
@@ -596,10 +693,17 @@ dit_status dit_init(const dit_config* cfg, const dit_weight* weights, int32_t n_
     b.w1 = G(p + "mlp.w1"); b.b1 = G(p + "mlp.b1"); b.w2 = G(p + "mlp.w2"); b.b2 = G(p + "mlp.b2");
     b.cwq = G(p + "cross.wq"); b.cbq = G(p + "cross.bq"); b.cwkv = G(p + "cross.wkv"); b.cbkv = G(p + "cross.bkv");
     b.cgq = G(p + "cross.gq"); b.cgk = G(p + "cross.gk"); b.cwo = G(p + "cross.wo"); b.cbo = G(p + "cross.bo");
+    b.t_mod_w = G(p + "txt.mod.w"); b.t_mod_b = G(p + "txt.mod.b"); b.t_wqkv = G(p + "txt.attn.wqkv"); b.t_bqkv = G(p + "txt.attn.bqkv");
+    b.t_gq = G(p + "txt.attn.gq"); b.t_gk = G(p + "txt.attn.gk"); b.t_wo = G(p + "txt.attn.wo"); b.t_bo = G(p + "txt.attn.bo");
+    b.t_w1 = G(p + "txt.mlp.w1"); b.t_b1 = G(p + "txt.mlp.b1"); b.t_w2 = G(p + "txt.mlp.w2"); b.t_b2 = G(p + "txt.mlp.b2");
     tab[2 + l] = {b.mod_w, b.mod_b, (int32_t)(6 * D), (int32_t)(l * 6 * D), (int32_t)(l * 6 * D), 0};
+    if (dual) {   // text-stream modulation rows follow the image blocks and the final layer
+      const int32_t off = (int32_t)(L * 6 * D + 2 * D + l * 6 * D);
+      tab[3 + L + l] = {b.t_mod_w, b.t_mod_b, (int32_t)(6 * D), off, off, 0};
+    }
   }
   tab[2 + L] = {h->fm_w, h->fm_b, (int32_t)(2 * D), (int32_t)(L * 6 * D), (int32_t)(L * 6 * D), 0};
-  cudaError_t e = cudaMemcpy(w.gemv_tab, tab.data(), (L + 3) * sizeof(GemvBatch), cudaMemcpyHostToDevice);
+  cudaError_t e = cudaMemcpy(w.gemv_tab, tab.data(), tab.size() * sizeof(GemvBatch), cudaMemcpyHostToDevice);
   if (e != cudaSuccess) {
     set_error("dit_init: pointer-table upload failed: %s", cudaGetErrorString(e));
     delete[] h->blocks;

@@ -246,6 +246,54 @@ def test_bf16_step_never_substitutes_the_ffma_kernels(lib):
     assert B.dit_fallback_launches() == n0 + 2
 
 
+# ------------------------------------------------------------------------------ dual-stream joint blocks (R37)
+@pytest.mark.parametrize("dtype,P", [("f32", 1), ("f32", 2), ("bf16", 1), ("bf16", 4)])
+def test_dual_stream_step_and_taps(lib, dtype, P):
+    """cond_mode joint2: text and image rows have their own per-block weights, one attention over [txt ; img].  Output,
+    the residual stream after every block and the attention output of the last block against the oracle."""
+    if dtype == "f32":
+        s = synth.cfg1(cond_mode="joint2", rope_dims=(0, 32, 32), qk_rmsnorm=True)
+    else:
+        s = _small_bf16(cond_mode="joint2")
+    taps = {}
+    out, ref, m, (lat, temb, cond) = _run_both(s, split_p=P, taps=taps)
+    dt = s.torch_dtype
+    check(out, ref, dt, f"dual-stream {dtype} P={P}")
+    T, D = s.n_tokens + s.n_cond, s.hidden
+    tight = dict(rel=2e-6, maxabs=5e-5) if dt == torch.float32 else {}
+    for l in range(s.n_blocks):
+        m.dit_debug_stop_after(l, "fc2")
+        m.dit_step(lat, temb, cond)
+        check(m.dit_get_tap("x", (T, D), torch.float32), taps[f"b{l}.x_mlp"], dt, f"dual-stream x after block {l}", **tight)
+    m.dit_debug_stop_after(s.n_blocks - 1, "attn")
+    m.dit_step(lat, temb, cond)
+    check(m.dit_get_tap("o", (T, D), dt), taps[f"b{s.n_blocks - 1}.o"], dt, "dual-stream attention output", **tight)
+    m.dit_debug_stop_after(-1, 0)
+
+
+def test_dual_stream_varlen_and_empty_text(lib):
+    """Packed dual-stream batch: heterogeneous grids and text lengths (one request without text), per-request timesteps;
+    each request against the oracle's step on that request alone."""
+    grids, nconds = [(1, 12, 20), (1, 36, 44), (1, 4, 4)], [9, 70, 0]
+    shapes = [_small_bf16(cond_mode="joint2", latent_grid=g, n_cond=max(n, 1)) for g, n in zip(grids, nconds)]
+    W = synth.make_weights(shapes[0])
+    Is = [synth.make_inputs(sh, tag=f"d{r}", t=150.0 + 250 * r) for r, sh in enumerate(shapes)]
+    for r, n in enumerate(nconds):
+        Is[r]["cond"] = Is[r]["cond"][:n]
+    T_total = sum(sh.n_tokens + n for sh, n in zip(shapes, nconds))
+    m = B.Dit(B.make_config(shapes[0], max_tokens=T_total, max_requests=3, max_cond_tokens=sum(nconds)), W, DEV)
+    lats = [i["latents"].to(DEV) for i in Is]
+    temb = torch.cat([i["temb"] for i in Is]).to(DEV)
+    conds = [i["cond"].to(DEV) if i["cond"].shape[0] else None for i in Is]
+    n0 = B.dit_fallback_launches()
+    outs = m.dit_step_varlen(lats, temb, conds)
+    torch.cuda.synchronize()
+    for r in range(3):
+        ref = O.dit_step(O.cfg_from_shape(shapes[r]), W, Is[r]["latents"], Is[r]["temb"], Is[r]["cond"])
+        check(outs[r], ref, torch.bfloat16, f"dual-stream varlen request {r}")
+    assert B.dit_fallback_launches() == n0
+
+
 def test_argument_validation_on_gpu(lib):
     s = synth.cfg1()
     W, I = synth.make_weights(s), synth.make_inputs(s)
