@@ -551,6 +551,13 @@ def run_kernels(args):
         hbm(f"merge Nq={Nq} H={H} P={P}", P * (Nq * H * 128 * 2 + Nq * H * 4) + Nq * H * 128 * 2 + Nq * H * 4,
             lambda: B.dit_attn_merge(op, lp))
         del op
+    # ---- re-layout P -> P' of the residual stream: reads and writes the artifact once
+    for T, D, ps, pd in ((32760, 5120, 4, 8), (4352, 3072, 2, 4)):
+        full = rn("relayout", (T, D), torch.float32)
+        sz = -(-T // ps)
+        src = [full[p * sz:min((p + 1) * sz, T)].contiguous() for p in range(ps)]
+        hbm(f"relayout T={T} D={D} P={ps}->{pd}", 2 * T * D * 4, lambda: B.dit_relayout(src, pd))
+        del full, src
     # ---- attention sweep (cfg 5): unsplit, d=128
     for H in (24, 40):
         for N in (1024, 2048, 4096, 8192, 16384, 32768, 65536, 131072):

@@ -202,6 +202,27 @@ dit_status dit_attn_partial(int32_t dtype, const void* q, const void* k, const v
 dit_status dit_attn_merge(int32_t dtype, const void* const* o_partials, const float* const* lses, int32_t P,
                           int32_t n_q, int32_t n_heads, int32_t head_dim, void* o, float* lse_out, void* stream);
 
+/* ---- re-layout between split degrees (§5.3 "Layout-Aware Artifact Migration") --
+ * A row-sharded artifact (latent tokens, residual stream, per-token embeddings: "latent states and embeddings")
+ * of n_rows rows lives as P contiguous shards (shard p = rows [p ceil(n/P), (p+1) ceil(n/P)) clipped to n: reading R20).
+ * When the next trajectory task runs at another degree P', the planner intersects every source-owned slice with every
+ * destination-required slice; every non-empty intersection is ONE transfer entry. */
+typedef struct {
+  int32_t src_rank, dst_rank; /* source shard p, destination shard q */
+  int64_t src_row, dst_row;   /* first row of the range INSIDE the source / destination shard */
+  int64_t n_rows;             /* rows in the range (> 0) */
+} dit_transfer;
+/* Host only.  Writes the plan (destination-major, source ranks ascending) to entries[0 .. min(count, max_entries)) and
+ * returns `count`, the number of entries the plan has (<= p_src + p_dst - 1); negative dit_status on bad arguments
+ * (1 <= p_src, p_dst <= 32).  n_rows = 0 gives 0 entries. */
+int32_t dit_relayout_plan(int64_t n_rows, int32_t p_src, int32_t p_dst, dit_transfer* entries, int32_t max_entries);
+/* Executes a plan on the device: ONE copy kernel packs every source range and installs it in its destination shard
+ * (HBM-bound: reads and writes the artifact once).  entries host [n_entries <= 64]; src_shards / dst_shards HOST arrays
+ * of device pointers indexed by rank, each shard [rows_of_shard, row_bytes] contiguous; row_bytes = bytes per row.
+ * 128-bit accesses when every range is 16-byte aligned, narrower otherwise. */
+dit_status dit_relayout(const dit_transfer* entries, int32_t n_entries, const void* const* src_shards,
+                        void* const* dst_shards, int64_t row_bytes, void* stream);
+
 /* ---- kernel-level entry points (the building blocks of dit_step; used by the parity tests and by
  *      bench.py's per-kernel roofline lines) ------------------------------------------------------ */
 

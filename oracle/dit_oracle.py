@@ -159,6 +159,14 @@ def shard_bounds(n, P):
     return [(min(p * sz, n), min((p + 1) * sz, n)) for p in range(P)]
 
 
+def relayout(shards, p_dst):
+    """Re-layout of a row-sharded artifact between split degrees (§5.3): the P
+    source shards are the R20 row ranges of ONE logical tensor, the result is its P' R20 row ranges — the plain
+    definition: put the rows back together, cut them again."""
+    full = torch.cat(list(shards), dim=0)
+    return [full[a:b] for a, b in shard_bounds(full.shape[0], p_dst)]
+
+
 def attention_split(q, k, v, P, scale=None):
     """§8(c) step 7: P independent partials over contiguous KV shards, then merge.  P = 1 == attention()."""
     parts = [attention(q, k[a:b], v[a:b], scale) for a, b in shard_bounds(k.shape[0], P)]

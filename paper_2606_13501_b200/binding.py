@@ -19,7 +19,7 @@ TAP = dict(x=0, y=1, qkv=2, o=3, u=5, c=6, mod=7, tok=8)
 STAGE = dict(y1=0, qkv=1, attn=2, oproj=3, cross=4, y2=5, fc1=6, fc2=7)
 
 SYMBOLS = ["dit_workspace_bytes", "dit_init", "dit_step", "dit_step_host", "dit_step_varlen", "dit_step_varlen_host", "dit_sample", "dit_attn_partial",
-           "dit_attn_merge", "dit_linear", "dit_linear_residual", "dit_linear_qkv", "dit_adaln", "dit_gemv", "dit_qknorm_rope", "dit_debug_stop_after",
+           "dit_attn_merge", "dit_relayout_plan", "dit_relayout", "dit_linear", "dit_linear_residual", "dit_linear_qkv", "dit_adaln", "dit_gemv", "dit_qknorm_rope", "dit_debug_stop_after",
            "dit_get_tap", "dit_profile_begin", "dit_profile_end", "dit_last_error", "dit_kernel_launches", "dit_fallback_launches",
            "dit_free"]
 
@@ -35,6 +35,11 @@ class dit_config(C.Structure):
 
 class dit_weight(C.Structure):
     _fields_ = [("name", C.c_char_p), ("dev_ptr", C.c_void_p), ("numel", C.c_int64)]
+
+
+class dit_transfer(C.Structure):
+    _fields_ = [("src_rank", C.c_int32), ("dst_rank", C.c_int32), ("src_row", C.c_int64), ("dst_row", C.c_int64),
+                ("n_rows", C.c_int64)]
 
 
 class DitError(RuntimeError):
@@ -59,6 +64,7 @@ def load(path: str = LIB_PATH):
     lib.dit_last_error.argtypes = [C.c_void_p]
     lib.dit_kernel_launches.restype = C.c_int32
     lib.dit_fallback_launches.restype = C.c_int32
+    lib.dit_relayout_plan.restype = C.c_int32
     lib.dit_free.restype = None
     lib.dit_free.argtypes = [C.c_void_p]
     vp, i32, i64, f32 = C.c_void_p, C.c_int32, C.c_int64, C.c_float
@@ -72,6 +78,8 @@ def load(path: str = LIB_PATH):
         "dit_sample": [vp, vp, vp, C.POINTER(C.c_float), vp, i32, vp, i32, f32, pi32, i32, i32, vp, vp],
         "dit_attn_partial": [i32, vp, vp, vp, i32, i32, i32, i32, i64, i64, f32, vp, vp, vp],
         "dit_attn_merge": [i32, C.POINTER(vp), C.POINTER(vp), i32, i32, i32, i32, vp, vp, vp],
+        "dit_relayout_plan": [i64, i32, i32, C.POINTER(dit_transfer), i32],
+        "dit_relayout": [C.POINTER(dit_transfer), i32, C.POINTER(vp), C.POINTER(vp), i64, vp],
         "dit_linear": [i32, i32, vp, i64, vp, vp, vp, i64, i32, i32, i32, vp],
         "dit_linear_residual": [i32, vp, i64, vp, vp, vp, i64, vp, i64, vp, i32, i32, i32, i32, vp],
         "dit_linear_qkv": [i32, vp, i64, vp, vp, vp, i64, vp, vp, f32, vp, vp, i32, i32, i32, vp],
@@ -273,6 +281,40 @@ def dit_attn_merge(o_parts, lse_parts, want_lse=True, stream=None):
     lp = (C.c_void_p * P)(*[t.data_ptr() for t in lse_parts])
     _check(lib.dit_attn_merge(_dt(o), op, lp, P, nq, H, d, _ptr(o), _ptr(lse), _stream(stream)), "dit_attn_merge")
     return o, lse
+
+
+def dit_relayout_plan(n_rows: int, p_src: int, p_dst: int):
+    """The transfer entries of a P -> P' re-layout of an n_rows-row artifact: list of (src_rank, dst_rank, src_row, dst_row,
+    n_rows) tuples (host only, no GPU needed)."""
+    lib = load()
+    arr = (dit_transfer * 64)()
+    n = lib.dit_relayout_plan(n_rows, p_src, p_dst, arr, 64)
+    if n < 0:
+        _check(n, "dit_relayout_plan")
+    return [(arr[i].src_rank, arr[i].dst_rank, arr[i].src_row, arr[i].dst_row, arr[i].n_rows) for i in range(n)]
+
+
+def dit_relayout(src_shards, p_dst: int, stream=None):
+    """src_shards: P tensors [rows_p, ...] (the R20 shards of one artifact) -> the P' destination shards (new tensors)."""
+    lib = load()
+    n_rows = sum(int(t.shape[0]) for t in src_shards)
+    P = len(src_shards)
+    ref = src_shards[0]
+    row_shape = tuple(ref.shape[1:])
+    row_bytes = ref.element_size()
+    for d in row_shape:
+        row_bytes *= int(d)
+    sz = -(-n_rows // p_dst) if n_rows else 0
+    dst = [torch.empty((max(0, min((q + 1) * sz, n_rows) - min(q * sz, n_rows)),) + row_shape, dtype=ref.dtype, device=ref.device)
+           for q in range(p_dst)]
+    arr = (dit_transfer * 64)()
+    n = lib.dit_relayout_plan(n_rows, P, p_dst, arr, 64)
+    if n < 0:
+        _check(n, "dit_relayout_plan")
+    sp = (C.c_void_p * P)(*[t.data_ptr() if t.numel() else None for t in src_shards])
+    dp = (C.c_void_p * p_dst)(*[t.data_ptr() if t.numel() else None for t in dst])
+    _check(lib.dit_relayout(arr, n, sp, dp, row_bytes, _stream(stream)), "dit_relayout")
+    return dst
 
 
 def dit_linear(A, W, bias=None, epilogue=EPI_BIAS, out=None, stream=None):
