@@ -583,13 +583,81 @@ def run_kernels(args):
 
 
 
+# --------------------------------------------------------------------------------------------------------
+# policy-simulator arm: measured step times -> cost model -> FCFS / SRTF / EDF on a synthetic trace
+# --------------------------------------------------------------------------------------------------------
+def run_sim(args):
+    """`--workload sim`: times `dit_step` (cfg 2 block shape, 8 blocks) at the paper's three image request shapes
+    (512^2 / 1024^2 / 1536^2 -> 1024 / 4096 / 9216 image tokens + 256 text tokens) on this GPU, builds the cost
+    table cost(shape, P) for P = 1, 2, 4, 8 — P = 1 measured; P > 1 modelled as per-row work / P plus one all-gather of the
+    block's K | V shards per block at the measured NVLink peer bandwidth (B200_PROFILING.md: 770 GB/s per direction) — and
+    replays one seeded Poisson trace (S : M : L = 5 : 3 : 2, 20 steps per request, the paper's Qwen-Image SLO multipliers
+    1.5 / 2.0 / 6.0 + 1 s) through `dit_sim_run` for the three policies of PAPER.md:299-303 on 8 ranks."""
+    from paper_2606_13501_b200 import binding as B
+    B.load()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    base = synth.cfg2()
+    W = synth.make_weights(base, device=dev)
+    sides = (64, 128, 192)                                   # latent side; patch 2 -> 1024 / 4096 / 9216 tokens
+    m = B.Dit(B.make_config(synth.cfg2(latent_grid=(1, sides[-1], sides[-1]))), W, dev)
+    step_s, tokens = [], []
+    for side in sides:
+        sh = synth.cfg2(latent_grid=(1, side, side))
+        I = synth.make_inputs(sh, device=dev)
+        lat, temb, cond = I["latents"], I["temb"][0].contiguous(), I["cond"]
+        out = torch.empty_like(lat)
+        for _ in range(3):
+            m.dit_step(lat, temb, cond, out)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        K = max(5, min(args.steps, 20))
+        e0.record()
+        for _ in range(K):
+            m.dit_step(lat, temb, cond, out)
+        e1.record()
+        torch.cuda.synchronize()
+        step_s.append(e0.elapsed_time(e1) / K * 1e-3)
+        tokens.append(sh.n_tokens + sh.n_cond)
+    D, L, nvlink = base.hidden, base.n_blocks, 770e9
+    table = {}
+    for c, (t1, T) in enumerate(zip(step_s, tokens)):
+        for P in (1, 2, 4, 8):
+            gather = 0.0 if P == 1 else L * (2 * T * D * 2) * (P - 1) / P / nvlink      # K | V of the other P - 1 shards, per block
+            table[(c, P)] = t1 / P + gather
+    n_req, n_steps, rate = 400, 20, 0.9 / (sum(w * t for w, t in zip((0.5, 0.3, 0.2), step_s)) * 20 / 8)   # ~90 % load of 8 ranks at P = 1
+    u = synth.uniform01(17, "sim.trace", 2 * n_req).tolist()
+    t, reqs = 0.0, []
+    alpha = (1.5, 2.0, 6.0)
+    for i in range(n_req):
+        t += -math.log(u[2 * i]) / rate
+        c = 0 if u[2 * i + 1] < 0.5 else (1 if u[2 * i + 1] < 0.8 else 2)
+        reqs.append(dict(shape_class=c, n_steps=n_steps, arrival_s=t, deadline_s=t + alpha[c] * n_steps * step_s[c] + 1.0))
+    state_mb = [(T * 64 * 2 + 256 * D * 2) / 1e6 for T in tokens]                       # latents + text embeddings (PAPER.md:49)
+    rows = []
+    for pol, grp in (("fcfs", 1), ("fcfs", 4), ("srtf", 1), ("edf", 1)):
+        cfg = dict(policy=pol, n_ranks=8, fcfs_group=grp, state_mb=state_mb, relayout_gbps=nvlink / 1e9, timeout_s=1500.0)
+        t0 = time.perf_counter()
+        _, summ = B.dit_sim_run(cfg, table, reqs)
+        wall = time.perf_counter() - t0
+        rows.append(dict(policy=pol + (f"-SP{grp}" if pol == "fcfs" else ""), **{k: round(v, 6) if isinstance(v, float) else v for k, v in summ.items()},
+                         sim_wall_ms=round(wall * 1e3, 3), events_per_s=round(summ["n_events"] / wall) if wall > 0 else None))
+    print(json.dumps({"metric": "policy simulation on measured step times", "n_gpus": 1, "data": "synthetic",
+                      "config": {"workload": "cfg2 block shape at 512^2 / 1024^2 / 1536^2 (+256 text tokens), 20-step requests, 8 simulated ranks",
+                                 "trace": f"{n_req} requests, Poisson rate {rate:.2f}/s, S:M:L = 5:3:2, deadline = a + alpha T + 1 s"},
+                      "measured_step_s_P1": step_s, "cost_table": {f"{c},{P}": round(v, 6) for (c, P), v in sorted(table.items())},
+                      "policies": rows}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "kernels", "traj"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "kernels", "traj", "sim"])
     ap.add_argument("--traj-steps", type=int, default=20, help="--workload traj: denoising steps per trajectory")
     ap.add_argument("--split-p", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -605,6 +673,9 @@ def main():
     elif args.workload == "traj":
         if rank == 0:
             run_traj(args)
+    elif args.workload == "sim":
+        if rank == 0:
+            run_sim(args)
     elif args.impl == "reference":
         run_reference(args, rank)
     else:

@@ -20,7 +20,7 @@ STAGE = dict(y1=0, qkv=1, attn=2, oproj=3, cross=4, y2=5, fc1=6, fc2=7)
 
 SYMBOLS = ["dit_workspace_bytes", "dit_init", "dit_step", "dit_step_host", "dit_step_varlen", "dit_step_varlen_host", "dit_sample", "dit_attn_partial",
            "dit_attn_merge", "dit_relayout_plan", "dit_relayout", "dit_linear", "dit_linear_residual", "dit_linear_qkv", "dit_adaln", "dit_gemv", "dit_qknorm_rope", "dit_debug_stop_after",
-           "dit_get_tap", "dit_profile_begin", "dit_profile_end", "dit_last_error", "dit_kernel_launches", "dit_fallback_launches",
+           "dit_get_tap", "dit_profile_begin", "dit_profile_end", "dit_last_error", "dit_kernel_launches", "dit_fallback_launches", "dit_sim_run",
            "dit_free"]
 
 
@@ -40,6 +40,32 @@ class dit_weight(C.Structure):
 class dit_transfer(C.Structure):
     _fields_ = [("src_rank", C.c_int32), ("dst_rank", C.c_int32), ("src_row", C.c_int64), ("dst_row", C.c_int64),
                 ("n_rows", C.c_int64)]
+
+
+class dit_cost_entry(C.Structure):
+    _fields_ = [("shape_class", C.c_int32), ("degree", C.c_int32), ("step_s", C.c_double)]
+
+
+class dit_sim_request(C.Structure):
+    _fields_ = [("shape_class", C.c_int32), ("n_steps", C.c_int32), ("arrival_s", C.c_double), ("deadline_s", C.c_double)]
+
+
+class dit_sim_config(C.Structure):
+    _fields_ = [("struct_size", C.c_int32), ("policy", C.c_int32), ("n_ranks", C.c_int32), ("fcfs_group", C.c_int32),
+                ("n_classes", C.c_int32), ("state_mb", C.c_double * 16), ("relayout_gbps", C.c_double), ("timeout_s", C.c_double)]
+
+
+class dit_sim_result(C.Structure):
+    _fields_ = [("finish_s", C.c_double), ("busy_rank_s", C.c_double), ("n_migrations", C.c_int32), ("max_degree", C.c_int32),
+                ("met_deadline", C.c_int32), ("failed", C.c_int32)]
+
+
+class dit_sim_summary(C.Structure):
+    _fields_ = [("makespan_s", C.c_double), ("throughput_rps", C.c_double), ("mean_latency_s", C.c_double),
+                ("p95_latency_s", C.c_double), ("slo_attainment", C.c_double), ("utilisation", C.c_double), ("n_events", C.c_int64)]
+
+
+POLICY = {"fcfs": 0, "srtf": 1, "edf": 2}
 
 
 class DitError(RuntimeError):
@@ -90,6 +116,8 @@ def load(path: str = LIB_PATH):
         "dit_get_tap": [vp, i32, vp, C.c_size_t, vp],
         "dit_profile_begin": [i32],
         "dit_profile_end": [C.POINTER(C.c_float), pi32],
+        "dit_sim_run": [C.POINTER(dit_sim_config), C.POINTER(dit_cost_entry), i32, C.POINTER(dit_sim_request), i32,
+                        C.POINTER(dit_sim_result), C.POINTER(dit_sim_summary)],
     }
     for name, argtypes in sig.items():
         fn = getattr(lib, name)
@@ -404,3 +432,34 @@ def dit_kernel_launches() -> int:
 def dit_fallback_launches() -> int:
     """bf16 GEMM / attention launches that ran on the FFMA (fp32-path) kernels; 0 for every BASELINE.json config."""
     return int(load().dit_fallback_launches())
+
+
+def dit_sim_run(cfg: dict, table: dict, requests: list):
+    """Scheduling-policy simulator (include/dit_sim.h; host only).  cfg: policy ("fcfs" | "srtf" | "edf" or its number), n_ranks,
+    fcfs_group, state_mb (list per class), relayout_gbps, timeout_s.  table: {(shape_class, degree): step seconds}.  requests:
+    dicts with shape_class, n_steps, arrival_s, deadline_s.  Returns (list of result dicts, summary dict)."""
+    lib = load()
+    c = dit_sim_config()
+    c.struct_size = C.sizeof(dit_sim_config)
+    pol = cfg["policy"]
+    c.policy = POLICY[pol] if isinstance(pol, str) else int(pol)
+    c.n_ranks, c.fcfs_group = int(cfg["n_ranks"]), int(cfg.get("fcfs_group", 1))
+    smb = list(cfg.get("state_mb", [0.0]))
+    c.n_classes = max(len(smb), 1 + max([k[0] for k in table] + [q["shape_class"] for q in requests] + [0]))
+    for i, v in enumerate(smb):
+        c.state_mb[i] = float(v)
+    c.relayout_gbps, c.timeout_s = float(cfg.get("relayout_gbps", 0.0)), float(cfg.get("timeout_s", 0.0))
+    tab = (dit_cost_entry * max(1, len(table)))()
+    for i, ((cls, deg), sec) in enumerate(sorted(table.items())):
+        tab[i].shape_class, tab[i].degree, tab[i].step_s = int(cls), int(deg), float(sec)
+    n = len(requests)
+    rq = (dit_sim_request * max(1, n))()
+    for i, q in enumerate(requests):
+        rq[i].shape_class, rq[i].n_steps, rq[i].arrival_s, rq[i].deadline_s = int(q["shape_class"]), int(q["n_steps"]), float(q["arrival_s"]), float(q["deadline_s"])
+    res = (dit_sim_result * max(1, n))()
+    summ = dit_sim_summary()
+    _check(lib.dit_sim_run(C.byref(c), tab, len(table), rq, n, res, C.byref(summ)), "dit_sim_run")
+    results = [dict(finish_s=res[i].finish_s, busy_rank_s=res[i].busy_rank_s, n_migrations=res[i].n_migrations,
+                    max_degree=res[i].max_degree, met_deadline=res[i].met_deadline, failed=res[i].failed) for i in range(n)]
+    summary = {k: getattr(summ, k) for k, _ in dit_sim_summary._fields_}
+    return results, summary
