@@ -87,6 +87,8 @@ typedef struct {
   int32_t max_tokens;      /* capacity: max total packed sequence rows (cond rows included in joint) */
   int32_t max_requests;    /* capacity: max requests per dit_step_varlen call (<= 64) */
   int32_t max_cond_tokens; /* capacity: max total conditioning tokens per call */
+  int32_t mlp_gated;       /* 0: MLP = W2 GELU_tanh(W1 y + b1) + b2 (R3).  1: gated MLP (SwiGLU; SURVEY.md §8(f) item 2,
+                              DESIGN.md R40): W2 (SiLU(W1 y + b1) (.) (W3 y + b3)) + b2 with extra weights mlp.w3, mlp.b3 */
 } dit_config;
 
 /* One named weight tensor (device pointer, caller-owned, config dtype).  Names:
@@ -95,6 +97,7 @@ typedef struct {
  *   blocks.{l}.mod.w [6D,D] .mod.b [6D]   (chunks: shift1, scale1, gate1, shift2, scale2, gate2)
  *   blocks.{l}.attn.wqkv [3D,D] .attn.bqkv [3D] (rows: q | k | v; head h = rows h*d..)  .attn.gq [d] .attn.gk [d]
  *   blocks.{l}.attn.wo [D,D] .attn.bo [D]   blocks.{l}.mlp.w1 [F,D] .mlp.b1 [F] .mlp.w2 [D,F] .mlp.b2 [D]
+ *   blocks.{l}.mlp.w3 [F,D] .mlp.b3 [F]   (mlp_gated only; joint2 also blocks.{l}.txt.mlp.w3 / .b3)
  *   blocks.{l}.cross.wq [D,D] .bq [D] .wkv [2D,D] .bkv [2D] .gq [d] .gk [d] .wo [D,D] .bo [D]   (cross mode)
  *   blocks.{l}.txt.{mod.w, mod.b, attn.wqkv, attn.bqkv, attn.gq, attn.gk, attn.wo, attn.bo, mlp.w1, mlp.b1, mlp.w2, mlp.b2}
  *        (joint2 mode: the text stream's copy, same shapes as the image stream's blocks.{l}.*)

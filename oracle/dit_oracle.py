@@ -56,6 +56,17 @@ def gelu_tanh(z):
     return 0.5 * z * (1.0 + torch.tanh(0.7978845608028654 * (z + 0.044715 * z ** 3)))
 
 
+def mlp(cfg, W, pre, y):
+    """The block's MLP branch before the gated residual (§8(c) step 5).  Default: W2 GELU_tanh(W1 y + b1) + b2.
+    `mlp_gated` (SURVEY.md §8(f) item 2 "gated-MLP variants", reading R40): the SwiGLU form
+    W2 (SiLU(W1 y + b1) (.) (W3 y + b3)) + b2.  Returns (u, W2 u + b2)."""
+    if cfg.get("mlp_gated"):
+        u = silu(linear(y, W[pre + "mlp.w1"], W[pre + "mlp.b1"])) * linear(y, W[pre + "mlp.w3"], W[pre + "mlp.b3"])
+    else:
+        u = gelu_tanh(linear(y, W[pre + "mlp.w1"], W[pre + "mlp.b1"]))
+    return u, linear(u, W[pre + "mlp.w2"], W[pre + "mlp.b2"])
+
+
 def layer_norm(x, eps):
     """LN(x) = (x - mu) / sqrt(var + eps), biased variance over the last dim, no affine (R4)."""
     mu = x.mean(dim=-1, keepdim=True)
@@ -243,8 +254,8 @@ def dual_stream_block(cfg, W, l, x, Lc, m_img, m_txt, ang, split_p, taps):
     for (name, pre, xs, m), os_ in zip(parts, (o[:Lc], o[Lc:])):
         xa = xs + m[2] * linear(os_, W[pre + "attn.wo"], W[pre + "attn.bo"])
         y2 = modulate(xa, m[3], m[4], eps)
-        u = gelu_tanh(linear(y2, W[pre + "mlp.w1"], W[pre + "mlp.b1"]))
-        outs.append(xa + m[5] * linear(u, W[pre + "mlp.w2"], W[pre + "mlp.b2"]))
+        u, hm = mlp(cfg, W, pre, y2)
+        outs.append(xa + m[5] * hm)
         if taps is not None:
             taps[f"b{l}.{name}.x_attn"], taps[f"b{l}.{name}.y2"], taps[f"b{l}.{name}.u"] = xa, y2, u
     x = torch.cat(outs, 0)
@@ -331,8 +342,8 @@ def dit_step(cfg, W, latents, temb, cond=None, split_p=1, taps=None):
             if taps is not None:
                 taps[f"b{l}.oc"], taps[f"b{l}.x_cross"] = oc.reshape(-1, D), x.clone()
         y2 = modulate(x, sh2, sc2, eps)
-        u = gelu_tanh(linear(y2, W[f"blocks.{l}.mlp.w1"], W[f"blocks.{l}.mlp.b1"]))
-        x = x + g2 * linear(u, W[f"blocks.{l}.mlp.w2"], W[f"blocks.{l}.mlp.b2"])
+        u, hm = mlp(cfg, W, f"blocks.{l}.", y2)
+        x = x + g2 * hm
         if taps is not None:
             taps[f"b{l}.y2"], taps[f"b{l}.u"], taps[f"b{l}.x_mlp"] = y2, u, x.clone()
     xi = x[Lc:]                                                                                   # image tokens only
@@ -389,12 +400,11 @@ def block_rows(cfg, W, l, x_in, mods_l, ang, rows, ctx=None):
         oc, _ = attention(qc, kc, vc)
         x = x + linear(oc.reshape(-1, D), W[p + "wo"], W[p + "bo"])
     y2 = modulate(x, sh2, sc2, eps)
-    u = gelu_tanh(linear(y2, W[f"blocks.{l}.mlp.w1"], W[f"blocks.{l}.mlp.b1"]))
-    return x + g2 * linear(u, W[f"blocks.{l}.mlp.w2"], W[f"blocks.{l}.mlp.b2"])
+    return x + g2 * mlp(cfg, W, f"blocks.{l}.", y2)[1]
 
 
 def cfg_from_shape(s):
     """Plain dict view of a synth.DiTShape (duck-typed; the oracle does not import the package)."""
     return dict(n_blocks=s.n_blocks, hidden=s.hidden, n_heads=s.n_heads, head_dim=s.head_dim, mlp_dim=s.mlp_dim,
                 patch=tuple(s.patch), cond_mode=s.cond_mode, rope_dims=tuple(s.rope_dims), rope_theta=s.rope_theta,
-                ln_eps=s.ln_eps, rms_eps=s.rms_eps, qk_rmsnorm=bool(s.qk_rmsnorm))
+                ln_eps=s.ln_eps, rms_eps=s.rms_eps, qk_rmsnorm=bool(s.qk_rmsnorm), mlp_gated=bool(s.extras.get("mlp_gated", False)))

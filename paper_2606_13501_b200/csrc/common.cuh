@@ -246,6 +246,10 @@ dit_status launch_gemm_tc_ex(int epi, const void* A, int64_t lda, const void* W,
 dit_status launch_gemm_tc_qkv(const void* A, int64_t lda, const void* W, const void* bias, void* out, int64_t ldo,
                               const void* gq, const void* gk, float rms_eps, const float* rc, const float* rs, int q_end,
                               int k_end, int M, int N, int K, cudaStream_t st, int a_split = 0);
+// Gated-MLP up-projection (R40): out bf16 [M, ldo] <- SiLU(A W1^T + b1) (.) (A W3^T + b3), one kernel (tcgen05)
+dit_status launch_gemm_tc_swiglu(const void* A, int64_t lda, const void* W1, const void* b1, const void* W3, const void* b3,
+                                 void* out, int64_t ldo, int M, int N, int K, cudaStream_t st);
+dit_status launch_silu_mul(int dtype, void* u, const void* u3, int64_t n, cudaStream_t st);   // u <- SiLU(u) (.) u3 (FFMA path)
 bool gemm_tc_supported(int epi, const void* A, int64_t lda, const void* W, void* out, int64_t ldo, int M, int N, int K);
 
 // Attention over packed sequences.  q rows [cu_q[r], cu_q[r+1]) attend to k/v rows [cu_k[r], cu_k[r+1])

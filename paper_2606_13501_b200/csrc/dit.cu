@@ -65,6 +65,7 @@ static size_t esize(int dtype) { return dtype == DIT_F32 ? 4 : 2; }
 
 struct BlockW {
   const void *mod_w, *mod_b, *wqkv, *bqkv, *gq, *gk, *wo, *bo, *w1, *b1, *w2, *b2;
+  const void *w3, *b3, *t_w3, *t_b3;   // gated MLP (mlp_gated, R40): the second up-projection (image / text stream)
   const void *cwq, *cbq, *cwkv, *cbkv, *cgq, *cgk, *cwo, *cbo;
   // dual-stream joint blocks (DIT_COND_JOINT2, R37): the text stream's own copy of the per-block tensors
   const void *t_mod_w, *t_mod_b, *t_wqkv, *t_bqkv, *t_gq, *t_gk, *t_wo, *t_bo, *t_w1, *t_b1, *t_w2, *t_b2;
@@ -76,6 +77,7 @@ struct Workspace {
   void* qkv;       // [Tm, 3D]
   void* o;         // [Tm, D]
   void* u;         // [Tm, F]
+  void* u3;        // [Tm, F]: gated MLP on the FFMA path only (the W3 product before the elementwise gate)
   float* c1;       // [Rm, D] first t-MLP layer
   float* c;        // [Rm, D]
   float* mod;      // [Rm, L*6D + 2D]
@@ -140,6 +142,7 @@ static bool carve(const dit_config& c, char* base, Workspace* w) {
   w->qkv = take(Tm * 3 * D * es);
   w->o = take(Tm * D * es);
   w->u = take(Tm * F * es);
+  w->u3 = take(c.mlp_gated && c.dtype == DIT_F32 ? Tm * F * es : 0);
   w->c1 = (float*)take(Rm * D * 4);
   w->c = (float*)take(Rm * D * 4);
   w->mod = (float*)take(Rm * (L * (c.cond_mode == DIT_COND_JOINT2 ? 12 : 6) * D + 2 * D) * 4);   // [img blocks | final | txt blocks]
@@ -187,6 +190,7 @@ static dit_status validate(const dit_config* c) {
                 "bf16 configs need cond_dim (%d) to be a multiple of 8", c->cond_dim);
   }
   DIT_REQUIRE(c->mlp_dim > 0 && c->mlp_dim % 8 == 0, DIT_ERR_UNSUPPORTED, "mlp_dim %d must be a multiple of 8", c->mlp_dim);
+  DIT_REQUIRE(c->mlp_gated == 0 || c->mlp_gated == 1, DIT_ERR_INVALID_ARG, "mlp_gated %d not in {0,1}", c->mlp_gated);
   DIT_REQUIRE(c->latent_channels > 0 && c->patch[0] > 0 && c->patch[1] > 0 && c->patch[2] > 0, DIT_ERR_INVALID_ARG,
               "latent_channels / patch must be positive");
   DIT_REQUIRE(c->temb_dim > 0 && c->temb_dim % 8 == 0, DIT_ERR_UNSUPPORTED, "temb_dim %d must be a multiple of 8", c->temb_dim);
@@ -236,6 +240,26 @@ static dit_status gemm(int dtype, int epi, const void* A, int64_t lda, const voi
     g_fallback_launches++;   // visible through dit_fallback_launches()
   }
   return launch_gemm_simt(dtype, epi, A, lda, W, bias, out, ldo, M, N, K, st);
+}
+
+// MLP up-projection  u <- act(y W1^T + b1)  (§8(a) a10): GELU(tanh), or with `w3` the gated form SiLU(.) (.) (y W3^T + b3)
+// (R40) — one tcgen05 kernel on the bf16 path, two FFMA GEMMs and an elementwise product on the fp32 path.
+static dit_status gemm_mlp_up(int dtype, const void* y, const void* w1, const void* b1, const void* w3, const void* b3,
+                              void* u, void* u3, int M, int F, int D, cudaStream_t st) {
+  if (w3 == nullptr) return gemm(dtype, DIT_EPI_BIAS_GELU, y, D, w1, b1, u, F, M, F, D, st);
+  if (M == 0) return DIT_OK;
+  if (dtype == DIT_BF16) {
+    if (!gemm_tc_supported(DIT_EPI_BIAS, y, D, w1, u, F, M, F, D) || ((uintptr_t)w3 & 15)) DIT_STRICT_TC("the gated MLP up-projection");
+    DIT_REQUIRE(gemm_tc_supported(DIT_EPI_BIAS, y, D, w1, u, F, M, F, D) && !((uintptr_t)w3 & 15), DIT_ERR_UNSUPPORTED,
+                "gated MLP (bf16) runs on the tcgen05 kernel only");
+    return launch_gemm_tc_swiglu(y, D, w1, b1, w3, b3, u, F, M, F, D, st);
+  }
+  DIT_REQUIRE(u3 != nullptr, DIT_ERR_WORKSPACE, "gated MLP: no workspace for the second up-projection");
+  dit_status s = gemm(dtype, DIT_EPI_BIAS, y, D, w1, b1, u, F, M, F, D, st);
+  if (s != DIT_OK) return s;
+  s = gemm(dtype, DIT_EPI_BIAS, y, D, w3, b3, u3, F, M, F, D, st);
+  if (s != DIT_OK) return s;
+  return launch_silu_mul(dtype, u, u3, (int64_t)M * F, st);
 }
 
 // Residual-stream producer  x <- x + gate (.) (A W^T + bias)  (out-projection, fc2).
@@ -404,9 +428,9 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
   for (int l = 0; l < L; ++l) {
     const BlockW& b = hd->blocks[l];
     if (dual) {
-      struct SW { const void *wqkv, *bqkv, *gq, *gk, *wo, *bo, *w1, *b1, *w2, *b2; };
-      const SW sw_img{b.wqkv, b.bqkv, b.gq, b.gk, b.wo, b.bo, b.w1, b.b1, b.w2, b.b2};
-      const SW sw_txt{b.t_wqkv, b.t_bqkv, b.t_gq, b.t_gk, b.t_wo, b.t_bo, b.t_w1, b.t_b1, b.t_w2, b.t_b2};
+      struct SW { const void *wqkv, *bqkv, *gq, *gk, *wo, *bo, *w1, *b1, *w2, *b2, *w3, *b3; };
+      const SW sw_img{b.wqkv, b.bqkv, b.gq, b.gk, b.wo, b.bo, b.w1, b.b1, b.w2, b.b2, b.w3, b.b3};
+      const SW sw_txt{b.t_wqkv, b.t_bqkv, b.t_gq, b.t_gk, b.t_wo, b.t_bo, b.t_w1, b.t_b1, b.t_w2, b.t_b2, b.t_w3, b.t_b3};
       auto mod_of = [&](const Seg& sg) { return w.mod + (size_t)sg.r * mod_stride + (sg.txt ? mod_img : 0) + (size_t)l * 6 * D; };
       auto rows_of = [&](void* base, const Seg& sg, int64_t ld) { return (void*)((char*)base + (size_t)sg.row0 * ld * es); };
       for (const Seg& sg : segs)
@@ -465,7 +489,8 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
       if (stop(l, DIT_STAGE_Y2)) return DIT_OK;
       for (const Seg& sg : segs) {
         const SW& sw = sg.txt ? sw_txt : sw_img;
-        RUN(gemm(dt, DIT_EPI_BIAS_GELU, rows_of(w.y, sg, D), D, sw.w1, sw.b1, rows_of(w.u, sg, F), F, sg.rows, F, D, st));
+        RUN(gemm_mlp_up(dt, rows_of(w.y, sg, D), sw.w1, sw.b1, sw.w3, sw.b3, rows_of(w.u, sg, F),
+                        w.u3 != nullptr ? rows_of(w.u3, sg, F) : nullptr, sg.rows, F, D, st));
       }
       if (stop(l, DIT_STAGE_FC1)) return DIT_OK;
       for (const Seg& sg : segs) {
@@ -551,7 +576,7 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
     }
     RUN(launch_adaln(dt, w.x, nullptr, nullptr, m + 3 * D, m + 4 * D, mod_stride, cu_dev, R, w.y, T, D, c.ln_eps, st));
     if (stop(l, DIT_STAGE_Y2)) return DIT_OK;
-    RUN(gemm(dt, DIT_EPI_BIAS_GELU, w.y, D, b.w1, b.b1, w.u, F, T, F, D, st));
+    RUN(gemm_mlp_up(dt, w.y, b.w1, b.b1, b.w3, b.b3, w.u, w.u3, T, F, D, st));
     if (stop(l, DIT_STAGE_FC1)) return DIT_OK;
     RUN(gemm_residual(dt, w.u, F, b.w2, b.b2, w.x, D, m + 5 * D, mod_stride, cu_dev, R, T, D, F, st));
     if (stop(l, DIT_STAGE_FC2)) return DIT_OK;
@@ -644,6 +669,10 @@ dit_status dit_init(const dit_config* cfg, const dit_weight* weights, int32_t n_
     if (cfg->qk_rmsnorm) { need[p + "attn.gq"] = d; need[p + "attn.gk"] = d; }
     need[p + "attn.wo"] = D * D; need[p + "attn.bo"] = D;
     need[p + "mlp.w1"] = F * D; need[p + "mlp.b1"] = F; need[p + "mlp.w2"] = D * F; need[p + "mlp.b2"] = D;
+    if (cfg->mlp_gated) {
+      need[p + "mlp.w3"] = F * D; need[p + "mlp.b3"] = F;
+      if (cfg->cond_mode == DIT_COND_JOINT2) { need[p + "txt.mlp.w3"] = F * D; need[p + "txt.mlp.b3"] = F; }
+    }
     if (cfg->cond_mode == DIT_COND_JOINT2) {
       need[p + "txt.mod.w"] = 6 * D * D; need[p + "txt.mod.b"] = 6 * D;
       need[p + "txt.attn.wqkv"] = 3 * D * D; need[p + "txt.attn.bqkv"] = 3 * D;
@@ -691,6 +720,7 @@ dit_status dit_init(const dit_config* cfg, const dit_weight* weights, int32_t n_
     b.mod_w = G(p + "mod.w"); b.mod_b = G(p + "mod.b"); b.wqkv = G(p + "attn.wqkv"); b.bqkv = G(p + "attn.bqkv");
     b.gq = G(p + "attn.gq"); b.gk = G(p + "attn.gk"); b.wo = G(p + "attn.wo"); b.bo = G(p + "attn.bo");
     b.w1 = G(p + "mlp.w1"); b.b1 = G(p + "mlp.b1"); b.w2 = G(p + "mlp.w2"); b.b2 = G(p + "mlp.b2");
+    b.w3 = G(p + "mlp.w3"); b.b3 = G(p + "mlp.b3"); b.t_w3 = G(p + "txt.mlp.w3"); b.t_b3 = G(p + "txt.mlp.b3");
     b.cwq = G(p + "cross.wq"); b.cbq = G(p + "cross.bq"); b.cwkv = G(p + "cross.wkv"); b.cbkv = G(p + "cross.bkv");
     b.cgq = G(p + "cross.gq"); b.cgk = G(p + "cross.gk"); b.cwo = G(p + "cross.wo"); b.cbo = G(p + "cross.bo");
     b.t_mod_w = G(p + "txt.mod.w"); b.t_mod_b = G(p + "txt.mod.b"); b.t_wqkv = G(p + "txt.attn.wqkv"); b.t_bqkv = G(p + "txt.attn.bqkv");

@@ -574,6 +574,33 @@ static dit_status launch_merge_t(const MergePtrs& ptrs, int P, int64_t n_rh, int
   return DIT_OK;
 }
 
+// Gated MLP on the FFMA (fp32) path (R40): u <- SiLU(u) (.) u3, elementwise; the tcgen05 path fuses this in the GEMM.
+template <typename T>
+__global__ void __launch_bounds__(256) silu_mul_kernel(T* __restrict__ u, const T* __restrict__ u3, int64_t n8) {
+  pdl_trigger();
+  pdl_wait();
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n8; i += (int64_t)gridDim.x * blockDim.x) {
+    float a[8], b[8];
+    ld8<T>(u + i * 8, a);
+    ld8<T>(u3 + i * 8, b);
+#pragma unroll
+    for (int e = 0; e < 8; ++e) a[e] = a[e] / (1.0f + expf(-a[e])) * b[e];
+    st8<T>(u + i * 8, a);
+  }
+}
+
+dit_status launch_silu_mul(int dtype, void* u, const void* u3, int64_t n, cudaStream_t st) {
+  if (n == 0) return DIT_OK;
+  DIT_REQUIRE(n % 8 == 0, DIT_ERR_UNSUPPORTED, "silu_mul: %lld elements, not a multiple of 8", (long long)n);
+  ProfScope _prof(DIT_KC_MISC, st);
+  const int64_t n8 = n / 8;
+  const int grid = (int)std::min<int64_t>((n8 + 255) / 256, 148 * 8);
+  if (dtype == DIT_F32) DIT_CUDA_OK(launch_pdl(silu_mul_kernel<float>, dim3(grid), dim3(256), 0, st, 1, (float*)u, (const float*)u3, n8));
+  else DIT_CUDA_OK(launch_pdl(silu_mul_kernel<bf16>, dim3(grid), dim3(256), 0, st, 1, (bf16*)u, (const bf16*)u3, n8));
+  DIT_LAUNCH_CHECK();
+  return DIT_OK;
+}
+
 dit_status launch_merge(int dtype, const void* const* o_parts, const float* const* lses, int P, int64_t n_rh, int d,
                         void* o, float* lse_out, cudaStream_t st) {
   if (n_rh == 0) return DIT_OK;

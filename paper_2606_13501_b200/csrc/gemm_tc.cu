@@ -77,7 +77,12 @@ constexpr int A_BYTES = BM * BK * 2;
 constexpr int stage_bytes(int bn) { return A_BYTES + (bn / 2) * BK * 2; }   // own A rows + own HALF of the W tile
 constexpr int GEMM_THREADS = 192;
 constexpr int EPI_THREADS = 128;
-enum { EPI_GATE_RESID = 3, EPI_QKV_NORM_ROPE = 4, EPI_BIAS_SPLIT = 5 };
+enum { EPI_GATE_RESID = 3, EPI_QKV_NORM_ROPE = 4, EPI_BIAS_SPLIT = 5, EPI_SWIGLU = 6 };
+// EPI_SWIGLU (gated MLP, R40): out[row, n] = SiLU(A W1^T + b1)[n] * (A W3^T + b3)[n], n < N.  One 256-wide
+// accumulator tile holds 128 columns of each product: the pair's leader CTA stages 128 rows of W1 (tensor map B), its peer
+// the same 128 rows of W3 (tensor map X) — each CTA supplies half of the MMA's N extent anyway — so accumulator columns
+// [0, 128) are the SiLU branch and [128, 256) the linear branch of output columns 128 nn .. 128 nn + 127.  Neither
+// product is ever written to memory.
 // EPI_BIAS_SPLIT: out[row, n] = hi = bf16(acc + bias), out[row, N + n] = lo = bf16((acc + bias) - hi): the result as an
 // unevaluated sum of two bf16 numbers (~16 significand bits).  A consumer GEMM reads [hi | lo] as ONE A operand of
 // width 2N against W wrapped along K (k_wrap): hi W^T + lo W^T in the fp32 accumulator — for the small operands whose
@@ -94,6 +99,7 @@ constexpr int smem_bytes(int bn, int epi) {
 
 struct EpiArgs {
   const bf16* bias;       // [N] or nullptr
+  const bf16* bias2;      // EPI_SWIGLU: b3 [N] or nullptr
   void* out;              // bf16 or fp32 [M, ldo]
   int64_t ldo;
   const float* gate;      // EPI_GATE_RESID: fp32 [R, gate_stride], nullptr = 1
@@ -142,7 +148,9 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   // 128 B/clk shared-memory port.
   const int rank = (int)cluster_ctarank();
   const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
-  const int mt = (M + BM - 1) / BM, mt2 = (mt + 1) >> 1, nt = (N + BN - 1) / BN, n_tiles = mt2 * nt;   // tile PAIRS
+  // EPI_SWIGLU: a 256-wide accumulator tile is 128 output columns
+  constexpr int BN_OUT = EPI == EPI_SWIGLU ? BN / 2 : BN;
+  const int mt = (M + BM - 1) / BM, mt2 = (mt + 1) >> 1, nt = (N + BN_OUT - 1) / BN_OUT, n_tiles = mt2 * nt;   // tile PAIRS
   const int nkb = (K + BK - 1) / BK;
   // Tile order: groups of GM row-tile pairs; inside a group the column tile is the slow index.  A wave of 74 CTA
   // pairs then covers ~74 / GM column tiles of the same GM row-tile pairs, whose A panels (GM x 256 x K) are sized
@@ -159,7 +167,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&tmA);
     tma_prefetch_desc(&tmB);
-    if (EPI == EPI_GATE_RESID) tma_prefetch_desc(&tmX);
+    if (EPI == EPI_GATE_RESID || EPI == EPI_SWIGLU) tma_prefetch_desc(&tmX);
   }
   if (warp == 1 && lane == 0) {
     for (int s = 0; s < STAGES; ++s) {
@@ -190,7 +198,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     for (int t = pair; t < n_tiles; t += n_pairs) {
       int mp, nn;
       tile_mn(t, mp, nn);
-      const int m0 = (mp * 2 + rank) * BM, n0 = nn * BN + rank * (BN / 2);
+      const int m0 = (mp * 2 + rank) * BM, n0 = EPI == EPI_SWIGLU ? nn * (BN / 2) : nn * BN + rank * (BN / 2);
+      const CUtensorMap* const tmW = (EPI == EPI_SWIGLU && rank != 0) ? &tmX : &tmB;
       for (int kb = 0; kb < nkb; ++kb) {
         mbar_wait_poll(empty_bar(s), ph ^ 1);
         if (elect_one()) {
@@ -198,7 +207,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
           if (rank == 0) mbar_expect_tx(full_bar(s), 2 * STAGE_BYTES);
           tma_load_2d_pair(smem0 + s * STAGE_BYTES, &tmA, kb * BK, m0, fb);
           // k_wrap > 0: A is [hi | lo] (two bf16 parts side by side) and W repeats along K every k_wrap blocks
-          tma_load_2d_pair(smem0 + s * STAGE_BYTES + A_BYTES, &tmB, (k_wrap > 0 ? kb % k_wrap : kb) * BK, n0, fb);
+          tma_load_2d_pair(smem0 + s * STAGE_BYTES + A_BYTES, tmW, (k_wrap > 0 ? kb % k_wrap : kb) * BK, n0, fb);
         }
         __syncwarp();
         if (++s == STAGES) { s = 0; ph ^= 1; }
@@ -247,7 +256,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       const uint32_t aph = (it >> 1) & 1;
       int mp, nn;
       tile_mn(t, mp, nn);
-      const int m0 = (mp * 2 + rank) * BM, n0 = nn * BN;
+      const int m0 = (mp * 2 + rank) * BM, n0 = nn * BN_OUT;
       const int row = m0 + quad * 32 + lane;
       const bool row_ok = row < M;
       float* const s_bias = s_vec + as * 2 * BN_MAX;
@@ -272,6 +281,13 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
           s_gate[i] = g != nullptr ? __bfloat162float(g[i & 127]) : 1.f;
         }
       }
+      if (EPI == EPI_SWIGLU) {   // s_bias[0..127] = b1, [128..255] = b3 of the tile's 128 output columns
+        for (int i = et; i < BN; i += EPI_THREADS) {
+          const bf16* const bsrc = i < BN / 2 ? ep.bias : ep.bias2;
+          const int n = n0 + (i & (BN / 2 - 1));
+          s_bias[i] = (bsrc != nullptr && n < N) ? __bfloat162float(bsrc[n]) : 0.f;
+        }
+      } else
 #pragma unroll
       for (int i = et; i < BN; i += EPI_THREADS)
         s_bias[i] = (ep.bias != nullptr && n0 + i < N) ? __bfloat162float(ep.bias[n0 + i]) : 0.f;
@@ -348,6 +364,28 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
 #pragma unroll
               for (int g = 0; g < 4; ++g) st8<bf16>(orow + hh * 128 + c4 * 32 + g * 8, &v[g * 8]);
             }
+          }
+        }
+      } else if (EPI == EPI_SWIGLU) {
+        bf16* const orow = reinterpret_cast<bf16*>(ep.out) + (int64_t)(row_ok ? row : 0) * ep.ldo + n0;
+#pragma unroll 1
+        for (int c = 0; c < BN / 64; ++c) {
+          if (n0 + c * 32 >= N) break;  // warp-uniform
+          uint32_t r1[32], r3[32];
+          tmem_ld32(t_addr + c * 32, r1);
+          tmem_ld32(t_addr + BN / 2 + c * 32, r3);
+          tmem_ld_wait();
+          float v[32];
+#pragma unroll
+          for (int e = 0; e < 32; ++e) {
+            const float a = __uint_as_float(r1[e]) + s_bias[c * 32 + e];
+            const float b = __uint_as_float(r3[e]) + s_bias[BN / 2 + c * 32 + e];
+            v[e] = __fdividef(a, 1.0f + __expf(-a)) * b;
+          }
+          if (row_ok) {
+#pragma unroll
+            for (int g = 0; g < 4; ++g)
+              if (n0 + c * 32 + g * 8 < N) st8<bf16>(orow + c * 32 + g * 8, &v[g * 8]);
           }
         }
       } else
@@ -468,7 +506,7 @@ dit_status launch_t(const CUtensorMap& ta, const CUtensorMap& tb, const CUtensor
                                      smem_bytes(BN, EPI)));
     attr_set = true;
   }
-  const int pairs = cdiv(cdiv(M, BM), 2) * cdiv(N, BN);
+  const int pairs = cdiv(cdiv(M, BM), 2) * cdiv(N, EPI == EPI_SWIGLU ? BN / 2 : BN);
   const int max_pairs = sm_count() / 2;
   DIT_CUDA_OK(launch_pdl(gemm_tc_kernel<EPI, BN>, dim3(2 * (pairs < max_pairs ? pairs : max_pairs)), dim3(GEMM_THREADS),
                          smem_bytes(BN, EPI), st, 2, ta, tb, tx, ep, M, N, K, group_rows(M, K), k_wrap));
@@ -524,7 +562,7 @@ dit_status launch_gemm_tc_ex(int epi, const void* A, int64_t lda, const void* W,
   const int Ka = a_split ? 2 * K : K;
   DIT_REQUIRE(make_tmap_2d_bf16(&ta, A, M, Ka, lda, BM, BK) && make_tmap_2d_bf16(&tb, W, N, K, K, bn / 2, BK), DIT_ERR_CUDA,
               "gemm_tc: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d lda=%lld)", M, N, K, (long long)lda);
-  EpiArgs ep{(const bf16*)bias, out, ldo, gate, gate_stride, cu, R, nullptr, nullptr, nullptr, nullptr, 0.f, 0, 0};
+  EpiArgs ep{(const bf16*)bias, nullptr, out, ldo, gate, gate_stride, cu, R, nullptr, nullptr, nullptr, nullptr, 0.f, 0, 0};
   ProfScope _prof(DIT_KC_GEMM, st);
   switch (epi) {
     case DIT_EPI_BIAS: return launch_bn<DIT_EPI_BIAS>(bn, ta, tb, ta, ep, M, N, Ka, st, k_wrap);
@@ -555,9 +593,22 @@ dit_status launch_gemm_tc_qkv(const void* A, int64_t lda, const void* W, const v
   CUtensorMap ta, tb;
   DIT_REQUIRE(make_tmap_2d_bf16(&ta, A, M, Ka, lda, BM, BK) && make_tmap_2d_bf16(&tb, W, N, K, K, 128, BK), DIT_ERR_CUDA,
               "gemm_tc_qkv: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d)", M, N, K);
-  EpiArgs ep{(const bf16*)bias, out, ldo, nullptr, 0, nullptr, 1, (const bf16*)gq, (const bf16*)gk, rc, rs, rms_eps, q_end, k_end};
+  EpiArgs ep{(const bf16*)bias, nullptr, out, ldo, nullptr, 0, nullptr, 1, (const bf16*)gq, (const bf16*)gk, rc, rs, rms_eps, q_end, k_end};
   ProfScope _prof(DIT_KC_GEMM, st);
   return launch_t<EPI_QKV_NORM_ROPE, 256>(ta, tb, ta, ep, M, N, Ka, st, k_wrap);
+}
+
+// Gated-MLP up-projection (R40): out bf16 [M, ldo] <- SiLU(A W1^T + b1) (.) (A W3^T + b3); W1, W3 [N, K], b1, b3 [N].
+dit_status launch_gemm_tc_swiglu(const void* A, int64_t lda, const void* W1, const void* b1, const void* W3, const void* b3,
+                                 void* out, int64_t ldo, int M, int N, int K, cudaStream_t st) {
+  if (M == 0 || N == 0) return DIT_OK;
+  CUtensorMap ta, tb, tx;
+  DIT_REQUIRE(make_tmap_2d_bf16(&ta, A, M, K, lda, BM, BK) && make_tmap_2d_bf16(&tb, W1, N, K, K, 128, BK) &&
+                  make_tmap_2d_bf16(&tx, W3, N, K, K, 128, BK),
+              DIT_ERR_CUDA, "gemm_tc_swiglu: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d)", M, N, K);
+  EpiArgs ep{(const bf16*)b1, (const bf16*)b3, out, ldo, nullptr, 0, nullptr, 1, nullptr, nullptr, nullptr, nullptr, 0.f, 0, 0};
+  ProfScope _prof(DIT_KC_GEMM, st);
+  return launch_t<EPI_SWIGLU, 256>(ta, tb, tx, ep, M, N, K, st, 0);
 }
 
 dit_status launch_gemm_tc(int epi, const void* A, int64_t lda, const void* W, const void* bias, void* out, int64_t ldo,

@@ -189,6 +189,8 @@ def weight_shapes(s: DiTShape) -> dict:
             w[p + "cross.wo"] = (D, D); w[p + "cross.bo"] = (D,)
         w[p + "mlp.w1"] = (F, D); w[p + "mlp.b1"] = (F,)
         w[p + "mlp.w2"] = (D, F); w[p + "mlp.b2"] = (D,)
+        if s.extras.get("mlp_gated"):    # gated MLP (SwiGLU): the second up-projection
+            w[p + "mlp.w3"] = (F, D); w[p + "mlp.b3"] = (F,)
         if s.cond_mode == "joint2":      # dual-stream blocks: the text stream's own copy of every per-block tensor
             for k in [k for k in w if k.startswith(p) and not k.startswith(p + "txt.")]:
                 w[p + "txt." + k[len(p):]] = w[k]

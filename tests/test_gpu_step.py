@@ -271,6 +271,52 @@ def test_dual_stream_step_and_taps(lib, dtype, P):
     m.dit_debug_stop_after(-1, 0)
 
 
+@pytest.mark.parametrize("dtype,mode,F", [("f32", "joint", 1024), ("f32", "joint2", 1000), ("bf16", "joint", 2048),
+                                          ("bf16", "cross", 1992), ("bf16", "joint2", 1096)])
+def test_gated_mlp_step_and_taps(lib, dtype, mode, F):
+    """mlp_gated (SwiGLU, R40): u = SiLU(W1 y + b1) (.) (W3 y + b3) — on the bf16 path one tcgen05 kernel whose CTA pair
+    stages W1 | W3 halves (F = 1992 / 1096: ragged last 128-column tile), on the fp32 path two GEMMs + a product.  Output,
+    u of every block and the residual stream after the MLP against the oracle."""
+    if dtype == "f32":
+        s = synth.cfg1(cond_mode=mode, mlp_dim=F, extras={"t": 500.0, "mlp_gated": True})
+    else:
+        s = _small_bf16(cond_mode=mode, mlp_dim=F, extras={"mlp_gated": True})
+    taps = {}
+    n0 = B.dit_fallback_launches()
+    out, ref, m, (lat, temb, cond) = _run_both(s, taps=taps)
+    dt = s.torch_dtype
+    check(out, ref, dt, f"gated MLP {dtype} {mode}")
+    T, D = s.n_tokens + (s.n_cond if mode in ("joint", "joint2") else 0), s.hidden
+    tight = dict(rel=2e-6, maxabs=5e-5) if dt == torch.float32 else {}
+    for l in range(s.n_blocks):
+        m.dit_debug_stop_after(l, "fc1")
+        m.dit_step(lat, temb, cond)
+        u_ref = torch.cat([taps[f"b{l}.txt.u"], taps[f"b{l}.img.u"]], 0) if mode == "joint2" else taps[f"b{l}.u"]
+        u_got = m.dit_get_tap("u", (T, F), dt)
+        if dt == torch.float32:
+            check(u_got, u_ref, dt, f"gated MLP u block {l}", **tight)
+        else:
+            # u is a product of two near-Gaussian factors: heavy-tailed (max ~ 20 RMS), so the bf16 rounding of the stored
+            # value alone (<= 2^-9 |u|) exceeds 3e-2 RMS at the largest elements.  rel-L2 keeps the usual bar; the
+            # element-wise bar is the usual 3e-2 RMS plus a term relative to the element, 2^-7 |u| (its own rounding and
+            # the input rounding of one factor scaled by a large other factor).
+            e_rel, _ = errors(u_got, u_ref)
+            assert e_rel <= 5e-3, f"gated MLP u block {l}: rel-L2 {e_rel:.3e}"
+            diff = (u_got.double().cpu() - u_ref).abs()
+            bound = u_ref.abs() * 2.0 ** -7 + 3e-2 * u_ref.pow(2).mean().sqrt()
+            assert bool((diff <= bound).all()), f"gated MLP u block {l}: worst excess {float((diff - bound).max()):.3e}"
+        m.dit_debug_stop_after(l, "fc2")
+        m.dit_step(lat, temb, cond)
+        check(m.dit_get_tap("x", (T, D), torch.float32), taps[f"b{l}.x_mlp"], dt, f"gated MLP x block {l}", **tight)
+    m.dit_debug_stop_after(-1, 0)
+    assert B.dit_fallback_launches() == n0
+    # a handle built without w3 / b3 for a gated config is refused
+    W = synth.make_weights(s)
+    W.pop("blocks.0.mlp.w3")
+    with pytest.raises(B.DitError):
+        B.Dit(B.make_config(s), W, DEV)
+
+
 def test_dual_stream_varlen_and_empty_text(lib):
     """Packed dual-stream batch: heterogeneous grids and text lengths (one request without text), per-request timesteps;
     each request against the oracle's step on that request alone."""

@@ -535,6 +535,37 @@ def test_dual_stream_block_by_hand():
     assert float((t2["b0.x_mlp"][:Lc] - want[:Lc]).abs().max()) > 1e-3
 
 
+def test_gated_mlp_block_by_hand_and_special_case():
+    """Gated MLP (R40): x += gate2 (.) (W2 (SiLU(W1 y + b1) (.) (W3 y + b3)) + b2), against torch library routines; with
+    W3 = 0, b3 = 1 the second factor is 1 and the branch is W2 SiLU(W1 y + b1) + b2."""
+    s = _tiny(n_blocks=1, cond_mode="none", extras={"mlp_gated": True})
+    W, I = synth.make_weights(s), synth.make_inputs(s)
+    assert "blocks.0.mlp.w3" in W and O.cfg_from_shape(s)["mlp_gated"]
+    taps = {}
+    O.dit_step(O.cfg_from_shape(s), W, I["latents"], I["temb"], None, taps=taps)
+    Fn = torch.nn.functional
+    Wd = {k: v.double() for k, v in W.items()}
+    D = 32
+    c = Fn.linear(Fn.silu(Fn.linear(I["temb"].double(), Wd["t_mlp.w1"], Wd["t_mlp.b1"])), Wd["t_mlp.w2"], Wd["t_mlp.b2"])
+    m = Fn.linear(Fn.silu(c), Wd["blocks.0.mod.w"], Wd["blocks.0.mod.b"]).reshape(6, D)
+    xa = taps["b0.x_attn"]
+    y = Fn.layer_norm(xa, (D,), eps=1e-6) * (1 + m[4]) + m[3]
+    u = Fn.silu(Fn.linear(y, Wd["blocks.0.mlp.w1"], Wd["blocks.0.mlp.b1"])) * Fn.linear(y, Wd["blocks.0.mlp.w3"], Wd["blocks.0.mlp.b3"])
+    want = xa + m[5] * Fn.linear(u, Wd["blocks.0.mlp.w2"], Wd["blocks.0.mlp.b2"])
+    assert torch.allclose(taps["b0.u"], u, rtol=1e-11, atol=1e-13)
+    assert torch.allclose(taps["b0.x_mlp"], want, rtol=1e-10, atol=1e-12)
+    W1 = dict(W)
+    W1["blocks.0.mlp.w3"] = torch.zeros_like(W["blocks.0.mlp.w3"]); W1["blocks.0.mlp.b3"] = torch.ones_like(W["blocks.0.mlp.b3"])
+    t1 = {}
+    O.dit_step(O.cfg_from_shape(s), W1, I["latents"], I["temb"], None, taps=t1)
+    assert torch.allclose(t1["b0.u"], Fn.silu(Fn.linear(t1["b0.y2"], Wd["blocks.0.mlp.w1"], Wd["blocks.0.mlp.b1"])), rtol=1e-12, atol=1e-14)
+    # and it is not the GELU block
+    s0 = _tiny(n_blocks=1, cond_mode="none")
+    t0 = {}
+    O.dit_step(O.cfg_from_shape(s0), {k: v for k, v in W.items() if "w3" not in k and "b3" not in k}, I["latents"], I["temb"], None, taps=t0)
+    assert float((t0["b0.u"] - taps["b0.u"]).abs().max()) > 1e-3
+
+
 def test_varlen_is_per_request_and_block_rows():
     s = _tiny(cond_mode="joint", rope_dims=(0, 8, 8), qk_rmsnorm=True)
     W = synth.make_weights(s)
