@@ -241,6 +241,31 @@ typedef enum {
 dit_status dit_linear(int32_t dtype, int32_t epilogue, const void* A, int64_t lda, const void* W, const void* bias,
                       void* out, int64_t ldo, int32_t M, int32_t N, int32_t K, void* stream);
 
+/* Gated-MLP up-projection (SwiGLU; dit_config.mlp_gated, R40):
+ *   out[M, N] = SiLU(A W1^T + b1) (.) (A W3^T + b3);  W1, W3 contiguous [N, K]; b1, b3 [N] or NULL; A, W, b, out in dtype.
+ * bf16: ONE tcgen05 kernel (the CTA pair stages W1 | W3 halves of a 256-column accumulator tile, the epilogue gates);
+ * tmp is ignored.  fp32: two FFMA GEMMs + an elementwise product; tmp dev fp32 [M, N] is required, out contiguous. */
+dit_status dit_linear_swiglu(int32_t dtype, const void* A, int64_t lda, const void* W1, const void* b1, const void* W3,
+                             const void* b3, void* out, int64_t ldo, void* tmp, int32_t M, int32_t N, int32_t K, void* stream);
+
+/* fp8 (E4M3) linear layer — SURVEY.md §8(f) item 2 ("fp8 ... GEMMs with the same oracle"); reading R42.  Kernel-level
+ * only: a bf16 dit_step never uses it (e4m3 operands miss BASELINE.json's 5e-3 tolerance by ~7x).
+ *
+ * dit_quantize_fp8: per row of x [M, K] (dev, dtype DIT_BF16 or DIT_F32, row stride ldx elements):
+ *     amax = max_k |x[m,k]|;  scale[m] = amax / 448,  inv = 448 / amax (fp32 divisions; both 1 for an all-zero row);
+ *     q[m,k] = e4m3(x[m,k] * inv): one fp32 multiplication, round-to-nearest-even, saturating at +-448.  q dev uint8 [M, ldq] (e4m3 "fn" codes: S.EEEE.MMM, bias 7, no inf),
+ *   scale dev fp32 [M].  K, ldx, ldq multiples of 8; x 16-byte, q 8-byte aligned.
+ * dit_linear_fp8:  out[M, N] = epilogue( a_scale[m] * w_scale[n] * sum_k val(Aq[m,k]) val(Wq[n,k]) + bias[n] )
+ *   Aq dev uint8 [M, lda], Wq dev uint8 [N, K] contiguous, a_scale [M] / w_scale [N] dev fp32, bias dev bf16 [N] or NULL,
+ *   out dev bf16 [M, ldo] (DIT_EPI_BIAS, DIT_EPI_BIAS_GELU) or fp32 (DIT_EPI_BIAS_F32).  tcgen05 kind::f8f6f4 MMAs, fp32
+ *   accumulation.  K and lda multiples of 16, N and ldo of 8, 16-byte aligned pointers; DIT_ERR_UNSUPPORTED otherwise
+ *   (there is no FFMA substitute). */
+dit_status dit_quantize_fp8(int32_t dtype, const void* x, int64_t ldx, int32_t M, int32_t K, void* q, int64_t ldq,
+                            float* scale, void* stream);
+dit_status dit_linear_fp8(int32_t epilogue, const void* Aq, int64_t lda, const float* a_scale, const void* Wq,
+                          const float* w_scale, const void* bias, void* out, int64_t ldo, int32_t M, int32_t N, int32_t K,
+                          void* stream);
+
 /* Residual-stream producer with the gate fused in the GEMM epilogue (north_star subsystem 3, "gate epilogues";
  * the out-projection and fc2 of every block):   x[M, N] <- x + gate[req(row)] (.) (A[M, K] W[N, K]^T + bias[N])
  *   x dev fp32 [M, ldx] in/out;  A, W, bias in dtype;  gate dev fp32 [n_requests, gate_stride] (NULL = 1), row ->

@@ -6,8 +6,9 @@ describe an fp8 path; the format is the OCP 8-bit floating point E4M3 ("e4m3fn":
 bits, no infinities, S.1111.111 = NaN, largest finite value 448), written out here from its definition:
     value(code) = (-1)^s * 2^(e-7) * (1 + m/8)   for e in 1..15   (e = 15, m = 7 is NaN)
                 = (-1)^s * 2^-6   * (m/8)        for e = 0        (subnormals)
-Quantisation of a row x (R42): amax = max|x| in fp32; scale = amax / 448 in fp32 (1 when amax = 0); r = x / scale in fp32;
-code = the e4m3 value nearest to r, ties to the even code, saturating at +-448.  The decision is taken in fp32 on both sides
+Quantisation of a row x (R42): amax = max|x| in fp32; inv = 448 / amax and scale = amax / 448, both fp32 divisions (1 when
+amax = 0); r = x * inv, one fp32 multiplication; code = the e4m3 value nearest to r, ties to the even code, saturating at
++-448; `scale` is what the consumer multiplies back.  The decision is taken in fp32 on both sides
 (the rule for "floating point decides an integer"); everything after it is exact: decode(code) in fp64.
     linear_fp8:  out[m, n] = a_scale[m] * w_scale[n] * sum_k decode(Aq[m, k]) decode(Wq[n, k]) + bias[n]     (fp64)
 
@@ -60,8 +61,10 @@ def quantize_rows(x: torch.Tensor):
     """x [M, K] (any float dtype; used as fp32) -> (codes uint8 [M, K], scale fp32 [M]) by the rule in the header."""
     xf = x.to(torch.float32)
     amax = xf.abs().amax(dim=1)
-    scale = torch.where(amax > 0, amax / torch.tensor(E4M3_MAX, dtype=torch.float32), torch.ones_like(amax))
-    r = xf / scale[:, None]                          # fp32 division (IEEE, round to nearest)
+    m = torch.tensor(E4M3_MAX, dtype=torch.float32)
+    scale = torch.where(amax > 0, amax / m, torch.ones_like(amax))       # fp32 divisions (IEEE, round to nearest)
+    inv = torch.where(amax > 0, m / amax, torch.ones_like(amax))
+    r = xf * inv[:, None]                                                # one fp32 multiplication per element
     return round_to_e4m3(r), scale
 
 

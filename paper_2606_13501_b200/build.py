@@ -30,7 +30,7 @@ def _sources():
 
 def _digest():
     h = hashlib.sha256()
-    for f in sorted(os.listdir(CSRC)) + ["../../include/dit.h"]:
+    for f in sorted(os.listdir(CSRC)) + ["../../include/dit.h", "../../include/dit_sim.h"]:
         with open(os.path.join(CSRC, f), "rb") as fh:
             h.update(f.encode() + fh.read())
     h.update(" ".join(FLAGS).encode())

@@ -987,6 +987,27 @@ dit_status dit_linear_qkv(int32_t dtype, const void* A, int64_t lda, const void*
                             3 * hidden, K, (cudaStream_t)stream);
 }
 
+dit_status dit_linear_swiglu(int32_t dtype, const void* A, int64_t lda, const void* W1, const void* b1, const void* W3,
+                             const void* b3, void* out, int64_t ldo, void* tmp, int32_t M, int32_t N, int32_t K, void* stream) {
+  DIT_REQUIRE(dtype == DIT_F32 || dtype == DIT_BF16, DIT_ERR_INVALID_ARG, "dtype %d", dtype);
+  DIT_REQUIRE(M >= 0 && N > 0 && K > 0 && lda >= K && ldo >= N, DIT_ERR_INVALID_ARG, "bad GEMM shape M=%d N=%d K=%d lda=%lld ldo=%lld",
+              M, N, K, (long long)lda, (long long)ldo);
+  DIT_REQUIRE(M == 0 || (A && W1 && W3 && out), DIT_ERR_INVALID_ARG, "NULL argument");
+  cudaStream_t st = (cudaStream_t)stream;
+  if (M == 0) return DIT_OK;
+  if (dtype == DIT_BF16) {
+    DIT_REQUIRE(gemm_tc_supported(DIT_EPI_BIAS, A, lda, W1, out, ldo, M, N, K) && !((uintptr_t)W3 & 15), DIT_ERR_UNSUPPORTED,
+                "dit_linear_swiglu (bf16): K, N, lda, ldo multiples of 8, 16-byte aligned pointers, sm_100 only");
+    return launch_gemm_tc_swiglu(A, lda, W1, b1, W3, b3, out, ldo, M, N, K, st);
+  }
+  DIT_REQUIRE(tmp != nullptr && ldo == N, DIT_ERR_INVALID_ARG, "dit_linear_swiglu (fp32): tmp [M, N] is required and out must be contiguous");
+  dit_status s = gemm(dtype, DIT_EPI_BIAS, A, lda, W1, b1, out, ldo, M, N, K, st);
+  if (s != DIT_OK) return s;
+  s = gemm(dtype, DIT_EPI_BIAS, A, lda, W3, b3, tmp, N, M, N, K, st);
+  if (s != DIT_OK) return s;
+  return launch_silu_mul(dtype, out, tmp, (int64_t)M * N, st);
+}
+
 dit_status dit_adaln(int32_t dtype, float* x, const void* h, const float* gate, const float* shift, const float* scale,
                      int64_t mod_stride, const int32_t* cu_seqlens_dev, int32_t n_requests, void* y, int32_t T, int32_t D,
                      float eps, void* stream) {

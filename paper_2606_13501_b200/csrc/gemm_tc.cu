@@ -52,6 +52,18 @@ bool make_tmap_2d_bf16(CUtensorMap* out, const void* base, uint64_t rows, uint64
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+bool make_tmap_2d_u8(CUtensorMap* out, const void* base, uint64_t rows, uint64_t cols, uint64_t ld, uint32_t box_rows) {
+  EncodeTiledFn fn = encode_tiled_fn();
+  if (!fn) return false;
+  cuuint64_t dims[2] = {cols, rows};
+  cuuint64_t strides[1] = {ld};
+  cuuint32_t box[2] = {128, box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  return fn(out, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(base), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 bool make_tmap_2d_f32(CUtensorMap* out, const void* base, uint64_t rows, uint64_t cols, uint64_t ld, uint32_t box_rows) {
   EncodeTiledFn fn = encode_tiled_fn();
   if (!fn) return false;
@@ -77,7 +89,11 @@ constexpr int A_BYTES = BM * BK * 2;
 constexpr int stage_bytes(int bn) { return A_BYTES + (bn / 2) * BK * 2; }   // own A rows + own HALF of the W tile
 constexpr int GEMM_THREADS = 192;
 constexpr int EPI_THREADS = 128;
-enum { EPI_GATE_RESID = 3, EPI_QKV_NORM_ROPE = 4, EPI_BIAS_SPLIT = 5, EPI_SWIGLU = 6 };
+enum { EPI_GATE_RESID = 3, EPI_QKV_NORM_ROPE = 4, EPI_BIAS_SPLIT = 5, EPI_SWIGLU = 6, EPI_F8 = 7 /* + 0 / 1 / 2 */ };
+// EPI_F8 + e (e = DIT_EPI_BIAS / _GELU / _F32): both operands are e4m3 bytes (R42), kind::f8f6f4 MMAs with K = 32;
+// a k-block is still 128 bytes of every operand row (128 elements instead of 64), so stages, descriptors and the
+// instruction count per byte are those of the bf16 kernel at twice the flops.  The epilogue applies the row scales:
+// out = e(acc * a_scale[row] * w_scale[col] + bias).
 // EPI_SWIGLU (gated MLP, R40): out[row, n] = SiLU(A W1^T + b1)[n] * (A W3^T + b3)[n], n < N.  One 256-wide
 // accumulator tile holds 128 columns of each product: the pair's leader CTA stages 128 rows of W1 (tensor map B), its peer
 // the same 128 rows of W3 (tensor map X) — each CTA supplies half of the MMA's N extent anyway — so accumulator columns
@@ -113,6 +129,7 @@ struct EpiArgs {
   const float* rc; const float* rs; // RoPE tables [M, 64] (nullptr: no RoPE)
   float rms_eps;
   int q_end, k_end;
+  const float* a_scale; const float* w_scale;   // EPI_F8: fp32 row scales of A [M] and W [N]
 };
 
 __device__ __forceinline__ float gelu_tanh_fast(float z) {
@@ -150,8 +167,11 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
   // EPI_SWIGLU: a 256-wide accumulator tile is 128 output columns
   constexpr int BN_OUT = EPI == EPI_SWIGLU ? BN / 2 : BN;
+  constexpr bool F8 = EPI >= EPI_F8;
+  constexpr int EPB = F8 ? EPI - EPI_F8 : EPI;   // the epilogue proper
+  constexpr int BKE = F8 ? 2 * BK : BK;          // elements per 128-byte k-block
   const int mt = (M + BM - 1) / BM, mt2 = (mt + 1) >> 1, nt = (N + BN_OUT - 1) / BN_OUT, n_tiles = mt2 * nt;   // tile PAIRS
-  const int nkb = (K + BK - 1) / BK;
+  const int nkb = (K + BKE - 1) / BKE;
   // Tile order: groups of GM row-tile pairs; inside a group the column tile is the slow index.  A wave of 74 CTA
   // pairs then covers ~74 / GM column tiles of the same GM row-tile pairs, whose A panels (GM x 256 x K) are sized
   // by the host to stay in L2 while the group sweeps over all column tiles: A is read from DRAM about once instead
@@ -205,9 +225,9 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         if (elect_one()) {
           const uint32_t fb = mapa_cluster(full_bar(s), 0);
           if (rank == 0) mbar_expect_tx(full_bar(s), 2 * STAGE_BYTES);
-          tma_load_2d_pair(smem0 + s * STAGE_BYTES, &tmA, kb * BK, m0, fb);
+          tma_load_2d_pair(smem0 + s * STAGE_BYTES, &tmA, kb * BKE, m0, fb);
           // k_wrap > 0: A is [hi | lo] (two bf16 parts side by side) and W repeats along K every k_wrap blocks
-          tma_load_2d_pair(smem0 + s * STAGE_BYTES + A_BYTES, tmW, (k_wrap > 0 ? kb % k_wrap : kb) * BK, n0, fb);
+          tma_load_2d_pair(smem0 + s * STAGE_BYTES + A_BYTES, tmW, (k_wrap > 0 ? kb % k_wrap : kb) * BKE, n0, fb);
         }
         __syncwarp();
         if (++s == STAGES) { s = 0; ph ^= 1; }
@@ -217,7 +237,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     // the peer CTA's warp 1 has nothing to issue: the leader drives both tensor cores
   } else if (warp == 1) {
     // ===================================================== leader CTA: MMA issuer for the pair
-    constexpr uint32_t idesc = idesc_bf16(2 * BM, BN, 0, 0);
+    constexpr uint32_t idesc = F8 ? idesc_e4m3(2 * BM, BN) : idesc_bf16(2 * BM, BN, 0, 0);
     int s = 0;
     uint32_t ph = 0;
     int it = 0;
@@ -234,7 +254,10 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
           const uint64_t ad = desc_kmajor_sw128(smem0 + s * STAGE_BYTES);
           const uint64_t bd = desc_kmajor_sw128(smem0 + s * STAGE_BYTES + A_BYTES);
 #pragma unroll
-          for (int k = 0; k < BK / 16; ++k) umma_ss_pair(d_tmem, ad + 2 * k, bd + 2 * k, idesc, (kb | k) != 0);
+          for (int k = 0; k < BK / 16; ++k) {   // 32 bytes of K per instruction in both kinds
+            if (F8) umma_ss_pair_f8(d_tmem, ad + 2 * k, bd + 2 * k, idesc, (kb | k) != 0);
+            else umma_ss_pair(d_tmem, ad + 2 * k, bd + 2 * k, idesc, (kb | k) != 0);
+          }
           umma_commit_pair(empty_bar(s), (uint16_t)3);
           if (kb == nkb - 1) umma_commit_pair(tfull_bar(as), (uint16_t)3);
         }
@@ -280,6 +303,11 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
           const bf16* g = i < 128 ? ep.gq : ep.gk;
           s_gate[i] = g != nullptr ? __bfloat162float(g[i & 127]) : 1.f;
         }
+      }
+      float a_scale = 1.0f;
+      if (F8) {   // s_gate = the tile's W row scales; this thread's A row scale
+        for (int i = et; i < BN; i += EPI_THREADS) s_gate[i] = (n0 + i < N) ? ep.w_scale[n0 + i] : 0.f;
+        a_scale = row_ok ? ep.a_scale[row] : 0.f;
       }
       if (EPI == EPI_SWIGLU) {   // s_bias[0..127] = b1, [128..255] = b3 of the tile's 128 output columns
         for (int i = et; i < BN; i += EPI_THREADS) {
@@ -436,8 +464,11 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
           float v[8], b[8];
           ld8<float>(s_bias + c * 32 + g * 8, b);
 #pragma unroll
-          for (int e = 0; e < 8; ++e) v[e] = __uint_as_float(r[g * 8 + e]) + b[e];
-          if (EPI == DIT_EPI_BIAS_GELU) {
+          for (int e = 0; e < 8; ++e) {
+            if (F8) v[e] = fmaf(__uint_as_float(r[g * 8 + e]), a_scale * s_gate[c * 32 + g * 8 + e], b[e]);
+            else v[e] = __uint_as_float(r[g * 8 + e]) + b[e];
+          }
+          if (EPB == DIT_EPI_BIAS_GELU) {
 #pragma unroll
             for (int e = 0; e < 8; ++e) v[e] = gelu_tanh_fast(v[e]);
           }
@@ -449,9 +480,9 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
             for (int e = 0; e < 8; ++e) lo[e] = v[e] - __bfloat162float(__float2bfloat16_rn(v[e]));
             st8<bf16>(o, v);
             st8<bf16>(o + N, lo);
-          } else if (EPI == DIT_EPI_BIAS || EPI == DIT_EPI_BIAS_GELU) {
+          } else if (EPB == DIT_EPI_BIAS || EPB == DIT_EPI_BIAS_GELU) {
             st8<bf16>(reinterpret_cast<bf16*>(ep.out) + (int64_t)row * ep.ldo + ng, v);
-          } else if (EPI == DIT_EPI_BIAS_F32) {
+          } else if (EPB == DIT_EPI_BIAS_F32) {
             st8<float>(reinterpret_cast<float*>(ep.out) + (int64_t)row * ep.ldo + ng, v);
           }
         }
@@ -562,7 +593,7 @@ dit_status launch_gemm_tc_ex(int epi, const void* A, int64_t lda, const void* W,
   const int Ka = a_split ? 2 * K : K;
   DIT_REQUIRE(make_tmap_2d_bf16(&ta, A, M, Ka, lda, BM, BK) && make_tmap_2d_bf16(&tb, W, N, K, K, bn / 2, BK), DIT_ERR_CUDA,
               "gemm_tc: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d lda=%lld)", M, N, K, (long long)lda);
-  EpiArgs ep{(const bf16*)bias, nullptr, out, ldo, gate, gate_stride, cu, R, nullptr, nullptr, nullptr, nullptr, 0.f, 0, 0};
+  EpiArgs ep{(const bf16*)bias, nullptr, out, ldo, gate, gate_stride, cu, R, nullptr, nullptr, nullptr, nullptr, 0.f, 0, 0, nullptr, nullptr};
   ProfScope _prof(DIT_KC_GEMM, st);
   switch (epi) {
     case DIT_EPI_BIAS: return launch_bn<DIT_EPI_BIAS>(bn, ta, tb, ta, ep, M, N, Ka, st, k_wrap);
@@ -593,7 +624,7 @@ dit_status launch_gemm_tc_qkv(const void* A, int64_t lda, const void* W, const v
   CUtensorMap ta, tb;
   DIT_REQUIRE(make_tmap_2d_bf16(&ta, A, M, Ka, lda, BM, BK) && make_tmap_2d_bf16(&tb, W, N, K, K, 128, BK), DIT_ERR_CUDA,
               "gemm_tc_qkv: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d)", M, N, K);
-  EpiArgs ep{(const bf16*)bias, nullptr, out, ldo, nullptr, 0, nullptr, 1, (const bf16*)gq, (const bf16*)gk, rc, rs, rms_eps, q_end, k_end};
+  EpiArgs ep{(const bf16*)bias, nullptr, out, ldo, nullptr, 0, nullptr, 1, (const bf16*)gq, (const bf16*)gk, rc, rs, rms_eps, q_end, k_end, nullptr, nullptr};
   ProfScope _prof(DIT_KC_GEMM, st);
   return launch_t<EPI_QKV_NORM_ROPE, 256>(ta, tb, ta, ep, M, N, Ka, st, k_wrap);
 }
@@ -606,9 +637,32 @@ dit_status launch_gemm_tc_swiglu(const void* A, int64_t lda, const void* W1, con
   DIT_REQUIRE(make_tmap_2d_bf16(&ta, A, M, K, lda, BM, BK) && make_tmap_2d_bf16(&tb, W1, N, K, K, 128, BK) &&
                   make_tmap_2d_bf16(&tx, W3, N, K, K, 128, BK),
               DIT_ERR_CUDA, "gemm_tc_swiglu: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d)", M, N, K);
-  EpiArgs ep{(const bf16*)b1, (const bf16*)b3, out, ldo, nullptr, 0, nullptr, 1, nullptr, nullptr, nullptr, nullptr, 0.f, 0, 0};
+  EpiArgs ep{(const bf16*)b1, (const bf16*)b3, out, ldo, nullptr, 0, nullptr, 1, nullptr, nullptr, nullptr, nullptr, 0.f, 0, 0, nullptr, nullptr};
   ProfScope _prof(DIT_KC_GEMM, st);
   return launch_t<EPI_SWIGLU, 256>(ta, tb, tx, ep, M, N, K, st, 0);
+}
+
+// fp8 linear layer (R42): out = e(decode(Aq) decode(Wq)^T (.) a_scale w_scale^T + bias); Aq [M, lda bytes], Wq [N, K] e4m3
+// bytes, scales fp32, bias bf16 (or nullptr), out bf16 (e = BIAS, BIAS_GELU) or fp32 (BIAS_F32).
+dit_status launch_gemm_tc_fp8(int epi, const void* Aq, int64_t lda, const float* a_scale, const void* Wq, const float* w_scale,
+                              const void* bias, void* out, int64_t ldo, int M, int N, int K, cudaStream_t st) {
+  if (M == 0 || N == 0) return DIT_OK;
+  DIT_REQUIRE(K > 0 && K % 16 == 0 && lda % 16 == 0 && N % 8 == 0 && ldo % 8 == 0, DIT_ERR_UNSUPPORTED,
+              "gemm_tc_fp8: K (%d) and lda (%lld) must be multiples of 16, N (%d) and ldo (%lld) of 8", K, (long long)lda, N, (long long)ldo);
+  DIT_REQUIRE(!(((uintptr_t)Aq | (uintptr_t)Wq | (uintptr_t)out) & 15), DIT_ERR_UNSUPPORTED, "gemm_tc_fp8: pointers must be 16-byte aligned");
+  DIT_REQUIRE(a_scale != nullptr && w_scale != nullptr, DIT_ERR_INVALID_ARG, "gemm_tc_fp8: scales are NULL");
+  CUtensorMap ta, tb;
+  const int bn = pick_bn(M, N);
+  DIT_REQUIRE(make_tmap_2d_u8(&ta, Aq, M, K, lda, BM) && make_tmap_2d_u8(&tb, Wq, N, K, K, bn / 2), DIT_ERR_CUDA,
+              "gemm_tc_fp8: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d lda=%lld)", M, N, K, (long long)lda);
+  EpiArgs ep{(const bf16*)bias, nullptr, out, ldo, nullptr, 0, nullptr, 1, nullptr, nullptr, nullptr, nullptr, 0.f, 0, 0, a_scale, w_scale};
+  ProfScope _prof(DIT_KC_GEMM, st);
+  switch (epi) {
+    case DIT_EPI_BIAS: return launch_bn<EPI_F8 + DIT_EPI_BIAS>(bn, ta, tb, ta, ep, M, N, K, st, 0);
+    case DIT_EPI_BIAS_GELU: return launch_bn<EPI_F8 + DIT_EPI_BIAS_GELU>(bn, ta, tb, ta, ep, M, N, K, st, 0);
+    case DIT_EPI_BIAS_F32: return launch_bn<EPI_F8 + DIT_EPI_BIAS_F32>(bn, ta, tb, ta, ep, M, N, K, st, 0);
+    default: DIT_REQUIRE(false, DIT_ERR_INVALID_ARG, "gemm_tc_fp8: epilogue %d", epi);
+  }
 }
 
 dit_status launch_gemm_tc(int epi, const void* A, int64_t lda, const void* W, const void* bias, void* out, int64_t ldo,

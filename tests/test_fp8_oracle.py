@@ -65,11 +65,19 @@ def test_quantize_rows_scale_rule():
     q, s = F.quantize_rows(x)
     assert s.dtype == torch.float32 and q.dtype == torch.uint8
     assert s.tolist() == [float(torch.tensor(2.0) / torch.tensor(448.0)), 1.0, 1.0]
-    # row 0: x / scale = 112, -448, 224, 0 -> all representable
+    # row 0: inv = 448 / 2 = 224 exactly; x * inv = 112, -448, 224, 0 -> all representable
     assert torch.equal(F.decode(q[0]), torch.tensor([112.0, -448.0, 224.0, 0.0], dtype=torch.float64))
     assert q[1].tolist() == [0, 0, 0, 0]
-    # row 2 (scale 1): 3 -> 3, 448 -> 448, -7 -> -7, 1e-4 -> 0 (below half the smallest subnormal 2^-10)
+    # row 2 (amax = 448: inv = scale = 1): 3 -> 3, 448 -> 448, -7 -> -7, 1e-4 -> 0 (below half the smallest subnormal 2^-10)
     assert torch.equal(F.decode(q[2]), torch.tensor([3.0, 448.0, -7.0, 0.0], dtype=torch.float64))
+    # a row whose scale is not a power of two: inv = fp32(448 / 3), codes of x * inv by hand
+    q3, s3 = F.quantize_rows(torch.tensor([[3.0, 1.0, -0.01, 2.0]]))
+    inv3 = float(torch.tensor(448.0) / torch.tensor(3.0))                       # 149.33333...
+    assert s3.tolist() == [float(torch.tensor(3.0) / torch.tensor(448.0))]
+    # 3 * inv = 448 -> 448; 1 * inv = 149.33 -> between 144 and 160: 144; -0.01 * inv = -1.4933 -> between 1.375 and 1.5: -1.5;
+    # 2 * inv = 298.67 -> between 288 and 320: 288
+    assert 447.9 < 3 * inv3 < 448.1
+    assert F.decode(q3[0]).tolist() == [448.0, 144.0, -1.5, 288.0]
     # the row maximum always lands on +-448
     g = torch.Generator().manual_seed(9)
     y = torch.randn(64, 96, generator=g).to(torch.bfloat16)

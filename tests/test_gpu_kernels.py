@@ -119,6 +119,31 @@ GEMM_SHAPES = [(1, 64, 64), (100, 72, 16), (288, 768, 256), (257, 1024, 320), (1
 
 
 @pytest.mark.parametrize("dtype", DTYPES)
+@pytest.mark.parametrize("M,N,K", [(128, 128, 64), (300, 520, 200), (1000, 1096, 512), (4352, 1992, 3072), (77, 8, 4096)])
+def test_linear_swiglu(lib, dtype, M, N, K):
+    """Gated-MLP up-projection (R40): SiLU(A W1^T + b1) (.) (A W3^T + b3).  bf16: one tcgen05 kernel, W1 | W3 halves of a
+    256-column accumulator tile (N = 520 / 1096 / 1992 / 8: ragged last 128-column tile); fp32: two GEMMs + product."""
+    A = rnd("A", (M, K), dtype)
+    W1, W3 = rnd("W1", (N, K), dtype, std=1.0 / math.sqrt(K)), rnd("W3", (N, K), dtype, std=1.0 / math.sqrt(K))
+    b1, b3 = rnd("b1", (N,), dtype, std=0.5), rnd("b3", (N,), dtype, std=0.5)
+    got = B.dit_linear_swiglu(A, W1, b1, W3, b3)
+    Ad = A.double().cpu()
+    ref = O.silu(O.linear(Ad, W1.cpu(), b1.cpu())) * O.linear(Ad, W3.cpu(), b3.cpu())
+    if dtype == torch.float32:
+        check(got, ref, dtype, f"swiglu {M}x{N}x{K}", rel=2e-6, maxabs=1e-4)
+    else:
+        # heavy-tailed product (max ~ 40 RMS): the bf16 rounding of the largest elements alone exceeds any bar relative to
+        # the RMS, so the element-wise bound below (2^-8 |ref| + 2e-3 RMS) replaces max-abs / RMS
+        check(got, ref, dtype, f"swiglu {M}x{N}x{K}", rel=3e-3, maxabs=1.0)
+        check_rounding(got, ref, f"swiglu {M}x{N}x{K}")
+    got0 = B.dit_linear_swiglu(A, W1, None, W3, None)                            # no biases
+    ref0 = O.silu(O.linear(Ad, W1.cpu(), None)) * O.linear(Ad, W3.cpu(), None)
+    check(got0, ref0, dtype, "swiglu no bias", **(dict(rel=2e-6, maxabs=1e-4) if dtype == torch.float32 else dict(rel=3e-3, maxabs=1.0)))
+    if dtype != torch.float32:
+        check_rounding(got0, ref0, "swiglu no bias")
+
+
+@pytest.mark.parametrize("dtype", DTYPES)
 @pytest.mark.parametrize("M,N,K", GEMM_SHAPES)
 @pytest.mark.parametrize("epi", [B.EPI_BIAS, B.EPI_BIAS_GELU, B.EPI_BIAS_F32])
 def test_linear(lib, dtype, M, N, K, epi):
