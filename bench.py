@@ -47,6 +47,13 @@ def _shape(workload: str):
         return synth.cfg2()
     if workload == "cfg3":
         return synth.cfg3()
+    if workload.startswith("cfg2_"):   # block variants of SURVEY 8(f) item 2 at the cfg 2 shape: dual-stream (MMDiT) blocks, gated MLP
+        kw = {}
+        if "dual" in workload:
+            kw["cond_mode"] = "joint2"
+        if "gated" in workload:
+            kw["extras"] = {"mlp_gated": True}
+        return synth.cfg2(name="cfg2_image_bf16_" + workload[5:], **kw)
     raise SystemExit(f"unknown workload {workload}")
 
 
@@ -55,6 +62,10 @@ CFG4_NAME = ("BASELINE.json configs[3]: packed varlen batch bf16, cfg2 block sha
 
 
 def _workload_name(s) -> str:
+    if s.name.startswith("cfg2_image_bf16_"):
+        return ("cfg 2 shape (image DiT bf16, 8 blocks, D=3072, 24x128, 4096+256 joint tokens) with " +
+                " + ".join((["dual-stream (MMDiT) joint blocks"] if s.cond_mode == "joint2" else []) +
+                           (["gated (SwiGLU) MLP"] if s.extras.get("mlp_gated") else [])) + " — a block variant, not a BASELINE.json config")
     return {"cfg2_image_bf16": "BASELINE.json configs[1]: image DiT bf16, 8 blocks, D=3072, 24x128, 4096+256 joint tokens",
             "cfg3_video_bf16": "BASELINE.json configs[2]: video DiT bf16, 4 blocks, D=5120, 40x128, 32760 tokens, cross-attn 512"}[s.name]
 
@@ -73,10 +84,11 @@ def step_flops(s, seq_lens=None) -> dict:
     seq_lens: per-request sequence lengths of a packed batch (attention is block-diagonal)."""
     D, F, H, d, L = s.hidden, s.mlp_dim, s.n_heads, s.head_dim, s.n_blocks
     N = s.n_tokens
-    T = N + (s.n_cond if s.cond_mode == "joint" else 0)
+    T = N + (s.n_cond if s.cond_mode in ("joint", "joint2") else 0)
     if seq_lens is not None:
         T = sum(seq_lens)
-    gemm = L * (2 * T * D * 3 * D + 2 * T * D * D + 2 * 2 * T * D * F)
+    n_up = 3 if s.extras.get("mlp_gated") else 2     # fc1 (+ the gate's second up-projection) + fc2
+    gemm = L * (2 * T * D * 3 * D + 2 * T * D * D + 2 * n_up * T * D * F)
     attn = L * 4 * (T * T if seq_lens is None else sum(t * t for t in seq_lens)) * d * H
     n_gemm = 4 * L
     if s.cond_mode == "cross":
@@ -179,14 +191,15 @@ class OracleSample:
     def __init__(self, s):
         from oracle import dit_oracle as O
         self.O, self.s = O, s
-        one = synth.cfg2(n_blocks=1) if s.name.startswith("cfg2") else synth.cfg3(n_blocks=1)
+        import dataclasses
+        one = dataclasses.replace(s, n_blocks=1)
         self.cfg1b = O.cfg_from_shape(one)
         self.cfg0b = dict(self.cfg1b, n_blocks=0)
         self.W = synth.make_weights(one)
         self.I = synth.make_inputs(s)
         self.t0 = None
         self.sample = (f"oracle dit_step (torch CPU float64) on the workload's inputs with 1 of {s.n_blocks} blocks, all "
-                       f"{s.n_tokens + (s.n_cond if s.cond_mode == 'joint' else 0)} tokens; step time extrapolated t0 + "
+                       f"{s.n_tokens + (s.n_cond if s.cond_mode in ('joint', 'joint2') else 0)} tokens; step time extrapolated t0 + "
                        f"{s.n_blocks}*(t1 - t0), t0 = zero-block call")
 
     def _run(self, cfg):
@@ -680,7 +693,7 @@ def main():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "kernels", "traj", "sim"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "kernels", "traj", "sim", "cfg2_dual", "cfg2_gated", "cfg2_dual_gated"])
     ap.add_argument("--traj-steps", type=int, default=20, help="--workload traj: denoising steps per trajectory")
     ap.add_argument("--split-p", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")

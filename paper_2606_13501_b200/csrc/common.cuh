@@ -246,6 +246,28 @@ dit_status launch_gemm_tc_ex(int epi, const void* A, int64_t lda, const void* W,
 dit_status launch_gemm_tc_qkv(const void* A, int64_t lda, const void* W, const void* bias, void* out, int64_t ldo,
                               const void* gq, const void* gk, float rms_eps, const float* rc, const float* rs, int q_end,
                               int k_end, int M, int N, int K, cudaStream_t st, int a_split = 0);
+// Row-segmented ("grouped") tcgen05 GEMM for the dual-stream blocks (R37): A and out are ONE packed [M, .] buffer whose rows
+// fall into segments (a request's text rows, its image rows); a segment uses weight set `which` (0 = image, 1 = text) and
+// the gate row of request `req`.  One launch covers every segment: a 256-row tile pair never straddles a segment.
+constexpr int GEMM_MAX_SEGS = 128;
+struct GemmSegs {
+  int n;                              // 0: not segmented
+  int tile0[GEMM_MAX_SEGS + 1];       // first row-tile pair of segment i (prefix sum of ceil(rows / 256))
+  int row0[GEMM_MAX_SEGS];
+  int rows[GEMM_MAX_SEGS];            // > 0
+  uint8_t which[GEMM_MAX_SEGS];
+  uint8_t req[GEMM_MAX_SEGS];
+};
+struct SegGemm {
+  int kind;                           // 0 bias, 1 bias + GELU, 3 gated residual, 4 QKV (+ norm / RoPE), 6 SwiGLU
+  const void* A; int64_t lda; void* out; int64_t ldo; int M, N, K;
+  const GemmSegs* segs;
+  const void* W[2]; const void* bias[2];        // per weight set
+  const void* W3[2]; const void* b3[2];         // SwiGLU
+  const void* gq[2]; const void* gk[2]; float rms_eps; const float* rc; const float* rs;   // QKV (rc / rs: [M, 64] of the packed rows)
+  const float* gate; int64_t gate_stride; int64_t gate_set_off;   // gated residual: gate row = gate + req * stride + which * set_off
+};
+dit_status launch_gemm_tc_segs(const SegGemm& g, cudaStream_t st);
 // Gated-MLP up-projection (R40): out bf16 [M, ldo] <- SiLU(A W1^T + b1) (.) (A W3^T + b3), one kernel (tcgen05)
 dit_status launch_gemm_tc_swiglu(const void* A, int64_t lda, const void* W1, const void* b1, const void* W3, const void* b3,
                                  void* out, int64_t ldo, int M, int N, int K, cudaStream_t st);

@@ -425,6 +425,18 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
       if (Lc > 0) segs.push_back({g.cu[r], Lc, r, true});
       if (g.cu[r + 1] - g.cu[r] - Lc > 0) segs.push_back({g.cu[r] + Lc, g.cu[r + 1] - g.cu[r] - Lc, r, false});
     }
+  // bf16: ONE segmented tcgen05 launch per projection covers every segment of both streams (GemmSegs); fp32: per segment
+  GemmSegs gsegs;
+  gsegs.n = 0;
+  const bool grouped = dual && dt == DIT_BF16 && (int)segs.size() <= GEMM_MAX_SEGS;
+  if (grouped) {
+    gsegs.tile0[0] = 0;
+    for (const Seg& sg : segs) {
+      const int i = gsegs.n++;
+      gsegs.row0[i] = sg.row0; gsegs.rows[i] = sg.rows; gsegs.which[i] = sg.txt ? 1 : 0; gsegs.req[i] = (uint8_t)sg.r;
+      gsegs.tile0[i + 1] = gsegs.tile0[i] + (sg.rows + 255) / 256;
+    }
+  }
   for (int l = 0; l < L; ++l) {
     const BlockW& b = hd->blocks[l];
     if (dual) {
@@ -437,6 +449,19 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
         RUN(launch_adaln(dt, w.x + (size_t)sg.row0 * D, nullptr, nullptr, mod_of(sg), mod_of(sg) + D, 0, nullptr, 1, rows_of(w.y, sg, D),
                          sg.rows, D, c.ln_eps, st));
       if (stop(l, DIT_STAGE_Y1)) return DIT_OK;
+      SegGemm sgm{};   // the fields every segmented launch of this block shares
+      sgm.segs = &gsegs; sgm.M = T; sgm.rms_eps = c.rms_eps;
+      sgm.gate = w.mod + (size_t)l * 6 * D; sgm.gate_stride = mod_stride; sgm.gate_set_off = mod_img;
+      if (grouped) {
+        DIT_REQUIRE(gemm_tc_supported(DIT_EPI_BIAS, w.y, D, sw_img.wqkv, w.qkv, 3 * D, T, 3 * D, D), DIT_ERR_UNSUPPORTED,
+                    "bf16 dual-stream step: the tcgen05 GEMM is unavailable");
+        SegGemm q = sgm;
+        q.kind = 4; q.A = w.y; q.lda = D; q.out = w.qkv; q.ldo = 3 * D; q.N = 3 * D; q.K = D;
+        q.W[0] = sw_img.wqkv; q.W[1] = sw_txt.wqkv; q.bias[0] = sw_img.bqkv; q.bias[1] = sw_txt.bqkv;
+        if (c.qk_rmsnorm) { q.gq[0] = sw_img.gq; q.gq[1] = sw_txt.gq; q.gk[0] = sw_img.gk; q.gk[1] = sw_txt.gk; }
+        q.rc = rope ? w.rope_c : nullptr; q.rs = rope ? w.rope_s : nullptr;
+        RUN(launch_gemm_tc_segs(q, st));
+      } else
       for (const Seg& sg : segs) {
         const SW& sw = sg.txt ? sw_txt : sw_img;
         const float* rc = rope ? w.rope_c + (size_t)sg.row0 * (d / 2) : nullptr;
@@ -477,6 +502,13 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
         }
       }
       if (stop(l, DIT_STAGE_ATTN)) return DIT_OK;
+      if (grouped) {
+        SegGemm q = sgm;
+        q.kind = 3; q.A = w.o; q.lda = D; q.out = w.x; q.ldo = D; q.N = D; q.K = D;
+        q.W[0] = sw_img.wo; q.W[1] = sw_txt.wo; q.bias[0] = sw_img.bo; q.bias[1] = sw_txt.bo;
+        q.gate += 2 * D;
+        RUN(launch_gemm_tc_segs(q, st));
+      } else
       for (const Seg& sg : segs) {
         const SW& sw = sg.txt ? sw_txt : sw_img;
         RUN(gemm_residual(dt, rows_of(w.o, sg, D), D, sw.wo, sw.bo, w.x + (size_t)sg.row0 * D, D, mod_of(sg) + 2 * D, 0, nullptr, 1,
@@ -487,12 +519,26 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
         RUN(launch_adaln(dt, w.x + (size_t)sg.row0 * D, nullptr, nullptr, mod_of(sg) + 3 * D, mod_of(sg) + 4 * D, 0, nullptr, 1,
                          rows_of(w.y, sg, D), sg.rows, D, c.ln_eps, st));
       if (stop(l, DIT_STAGE_Y2)) return DIT_OK;
+      if (grouped) {
+        SegGemm q = sgm;
+        q.kind = sw_img.w3 != nullptr ? 6 : 1; q.A = w.y; q.lda = D; q.out = w.u; q.ldo = F; q.N = F; q.K = D;
+        q.W[0] = sw_img.w1; q.W[1] = sw_txt.w1; q.bias[0] = sw_img.b1; q.bias[1] = sw_txt.b1;
+        q.W3[0] = sw_img.w3; q.W3[1] = sw_txt.w3; q.b3[0] = sw_img.b3; q.b3[1] = sw_txt.b3;
+        RUN(launch_gemm_tc_segs(q, st));
+      } else
       for (const Seg& sg : segs) {
         const SW& sw = sg.txt ? sw_txt : sw_img;
         RUN(gemm_mlp_up(dt, rows_of(w.y, sg, D), sw.w1, sw.b1, sw.w3, sw.b3, rows_of(w.u, sg, F),
                         w.u3 != nullptr ? rows_of(w.u3, sg, F) : nullptr, sg.rows, F, D, st));
       }
       if (stop(l, DIT_STAGE_FC1)) return DIT_OK;
+      if (grouped) {
+        SegGemm q = sgm;
+        q.kind = 3; q.A = w.u; q.lda = F; q.out = w.x; q.ldo = D; q.N = D; q.K = F;
+        q.W[0] = sw_img.w2; q.W[1] = sw_txt.w2; q.bias[0] = sw_img.b2; q.bias[1] = sw_txt.b2;
+        q.gate += 5 * D;
+        RUN(launch_gemm_tc_segs(q, st));
+      } else
       for (const Seg& sg : segs) {
         const SW& sw = sg.txt ? sw_txt : sw_img;
         RUN(gemm_residual(dt, rows_of(w.u, sg, F), F, sw.w2, sw.b2, w.x + (size_t)sg.row0 * D, D, mod_of(sg) + 5 * D, 0, nullptr, 1,

@@ -130,6 +130,9 @@ struct EpiArgs {
   float rms_eps;
   int q_end, k_end;
   const float* a_scale; const float* w_scale;   // EPI_F8: fp32 row scales of A [M] and W [N]
+  // segmented launches (GemmSegs): the second weight set's vectors, and the offset of its gate rows
+  const bf16* bias_b; const bf16* bias2_b; const bf16* gq_b; const bf16* gk_b;
+  int64_t gate_set_off;
 };
 
 __device__ __forceinline__ float gelu_tanh_fast(float z) {
@@ -141,7 +144,9 @@ __device__ __forceinline__ float gelu_tanh_fast(float z) {
 template <int EPI, int BN>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
-               const __grid_constant__ CUtensorMap tmX, EpiArgs ep, int M, int N, int K, int GM, int k_wrap) {
+               const __grid_constant__ CUtensorMap tmX, const __grid_constant__ CUtensorMap tmB2,
+               const __grid_constant__ CUtensorMap tmX2, EpiArgs ep, const __grid_constant__ GemmSegs segs, int M, int N, int K,
+               int GM, int k_wrap) {
   pdl_trigger();
   constexpr int STAGES = stages_for(EPI);
   extern __shared__ uint8_t smem_raw[];
@@ -170,7 +175,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   constexpr bool F8 = EPI >= EPI_F8;
   constexpr int EPB = F8 ? EPI - EPI_F8 : EPI;   // the epilogue proper
   constexpr int BKE = F8 ? 2 * BK : BK;          // elements per 128-byte k-block
-  const int mt = (M + BM - 1) / BM, mt2 = (mt + 1) >> 1, nt = (N + BN_OUT - 1) / BN_OUT, n_tiles = mt2 * nt;   // tile PAIRS
+  const int mt = (M + BM - 1) / BM, mt2 = segs.n > 0 ? segs.tile0[segs.n] : (mt + 1) >> 1;
+  const int nt = (N + BN_OUT - 1) / BN_OUT, n_tiles = mt2 * nt;   // tile PAIRS
   const int nkb = (K + BKE - 1) / BKE;
   // Tile order: groups of GM row-tile pairs; inside a group the column tile is the slow index.  A wave of 74 CTA
   // pairs then covers ~74 / GM column tiles of the same GM row-tile pairs, whose A panels (GM x 256 x K) are sized
@@ -182,6 +188,25 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     const int gsize = (mt2 - g * GM) < GM ? (mt2 - g * GM) : GM;
     n = r / gsize;
     mp = g * GM + (r - n * gsize);
+  };
+
+  // Segmented launch: row-tile pair mp belongs to the last segment whose first pair is <= mp; its rows start at the segment's
+  // first row and end at the segment's end (the tile may reach past it: those rows are loaded but never stored).
+  auto seg_of = [&](int mp, int& m_base, int& m_end, int& which, int& req) {
+    if (segs.n == 0) {
+      m_base = mp * 2 * BM; m_end = M; which = 0; req = -1;
+      return;
+    }
+    int lo = 0, hi = segs.n - 1;
+    while (lo < hi) {
+      const int mid = (lo + hi + 1) >> 1;
+      if (segs.tile0[mid] <= mp) lo = mid;
+      else hi = mid - 1;
+    }
+    m_base = segs.row0[lo] + (mp - segs.tile0[lo]) * 2 * BM;
+    m_end = segs.row0[lo] + segs.rows[lo];
+    which = segs.which[lo];
+    req = segs.req[lo];
   };
 
   if (warp == 0 && lane == 0) {
@@ -218,8 +243,10 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     for (int t = pair; t < n_tiles; t += n_pairs) {
       int mp, nn;
       tile_mn(t, mp, nn);
-      const int m0 = (mp * 2 + rank) * BM, n0 = EPI == EPI_SWIGLU ? nn * (BN / 2) : nn * BN + rank * (BN / 2);
-      const CUtensorMap* const tmW = (EPI == EPI_SWIGLU && rank != 0) ? &tmX : &tmB;
+      int m_base, m_end, wset, req;
+      seg_of(mp, m_base, m_end, wset, req);
+      const int m0 = m_base + rank * BM, n0 = EPI == EPI_SWIGLU ? nn * (BN / 2) : nn * BN + rank * (BN / 2);
+      const CUtensorMap* const tmW = (EPI == EPI_SWIGLU && rank != 0) ? (wset ? &tmX2 : &tmX) : (wset ? &tmB2 : &tmB);
       for (int kb = 0; kb < nkb; ++kb) {
         mbar_wait_poll(empty_bar(s), ph ^ 1);
         if (elect_one()) {
@@ -279,28 +306,35 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       const uint32_t aph = (it >> 1) & 1;
       int mp, nn;
       tile_mn(t, mp, nn);
-      const int m0 = (mp * 2 + rank) * BM, n0 = nn * BN_OUT;
+      int m_base, m_end, wset, seg_req;
+      seg_of(mp, m_base, m_end, wset, seg_req);
+      const int m0 = m_base + rank * BM, n0 = nn * BN_OUT;
       const int row = m0 + quad * 32 + lane;
-      const bool row_ok = row < M;
+      const bool row_ok = row < m_end;
+      const bf16* const bias_p = wset ? ep.bias_b : ep.bias;
+      const bf16* const bias2_p = wset ? ep.bias2_b : ep.bias2;
       float* const s_bias = s_vec + as * 2 * BN_MAX;
       float* const s_gate = s_bias + BN_MAX;
       bool gate_smem = true;          // this thread's row takes the staged gate row
       const float* gate_row = nullptr;
       if (EPI == EPI_GATE_RESID && ep.gate != nullptr) {
         int req0 = 0, req = 0;
-        if (ep.cu != nullptr && ep.R > 1) {
+        if (seg_req >= 0) {   // segmented: the whole tile is one request's rows
+          req0 = req = seg_req;
+        } else if (ep.cu != nullptr && ep.R > 1) {
           req0 = find_request(ep.cu, ep.R, m0);
           req = find_request(ep.cu, ep.R, row_ok ? row : M - 1);
         }
         gate_smem = req == req0;
-        gate_row = ep.gate + (int64_t)req * ep.gate_stride;
-        const float* g0 = ep.gate + (int64_t)req0 * ep.gate_stride;
+        const int64_t set_off = wset ? ep.gate_set_off : 0;
+        gate_row = ep.gate + (int64_t)req * ep.gate_stride + set_off;
+        const float* g0 = ep.gate + (int64_t)req0 * ep.gate_stride + set_off;
 #pragma unroll
         for (int i = et; i < BN; i += EPI_THREADS) s_gate[i] = (n0 + i < N) ? g0[n0 + i] : 0.f;
       }
       if (EPI == EPI_QKV_NORM_ROPE) {   // the two gain vectors: s_gate[0..127] = g_q, s_gate[128..255] = g_k
         for (int i = et; i < 256; i += EPI_THREADS) {
-          const bf16* g = i < 128 ? ep.gq : ep.gk;
+          const bf16* g = i < 128 ? (wset ? ep.gq_b : ep.gq) : (wset ? ep.gk_b : ep.gk);
           s_gate[i] = g != nullptr ? __bfloat162float(g[i & 127]) : 1.f;
         }
       }
@@ -311,14 +345,14 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       }
       if (EPI == EPI_SWIGLU) {   // s_bias[0..127] = b1, [128..255] = b3 of the tile's 128 output columns
         for (int i = et; i < BN; i += EPI_THREADS) {
-          const bf16* const bsrc = i < BN / 2 ? ep.bias : ep.bias2;
+          const bf16* const bsrc = i < BN / 2 ? bias_p : bias2_p;
           const int n = n0 + (i & (BN / 2 - 1));
           s_bias[i] = (bsrc != nullptr && n < N) ? __bfloat162float(bsrc[n]) : 0.f;
         }
       } else
 #pragma unroll
       for (int i = et; i < BN; i += EPI_THREADS)
-        s_bias[i] = (ep.bias != nullptr && n0 + i < N) ? __bfloat162float(ep.bias[n0 + i]) : 0.f;
+        s_bias[i] = (bias_p != nullptr && n0 + i < N) ? __bfloat162float(bias_p[n0 + i]) : 0.f;
       asm volatile("bar.sync 1, 128;" ::: "memory");  // staged rows visible to the 4 epilogue warps
       // Gated residual (x <- x + gate (.) (acc + bias)): the thread's 32-column chunk of gate (.) (acc + bias) goes to
       // a swizzled shared-memory buffer of its warp (32 rows x 128 bytes) and ONE TMA reduce-add per warp and chunk
@@ -340,7 +374,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
           const int nh = n0 + hh * 128;
           if (nh >= N) break;  // warp-uniform
           const int which = nh < ep.q_end ? 0 : (nh < ep.k_end ? 1 : 2);   // 0 = q, 1 = k, 2 = v
-          const bool norm = which < 2 && (which == 0 ? ep.gq : ep.gk) != nullptr;
+          const bool norm = which < 2 && (which == 0 ? ep.gq : ep.gk) != nullptr;   // both weight sets norm or neither
           const bool rope = which < 2 && rcr != nullptr;
           const float* const sg = s_gate + (which == 1 ? 128 : 0);
           float rinv = 1.0f;
@@ -433,7 +467,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
             const int ng = n + g * 8;
             float v[8], b[8], gv[8];
             ld8<float>(s_bias + c * 32 + g * 8, b);
-            const bool live = ng < N && c * 32 + g * 8 < BN;   // columns past the tile belong to the next tile: add 0
+            // columns past the tile belong to the next tile, rows past the segment to the next segment: add 0
+            const bool live = row_ok && ng < N && c * 32 + g * 8 < BN;
             if (gate_row != nullptr && live) {
               if (gate_smem) ld8<float>(s_gate + c * 32 + g * 8, gv);
               else ld8<float>(gate_row + ng, gv);
@@ -528,32 +563,43 @@ int sm_count() {
   return n;
 }
 
+const GemmSegs& no_segs() {
+  static const GemmSegs z = {};
+  return z;
+}
+
+// segmented launches pass the segment table and the second weight set's tensor maps (tb2: W, tx2: W3 of the SwiGLU form)
+struct SegLaunch { const GemmSegs* segs; const CUtensorMap* tb2; const CUtensorMap* tx2; };
+
 template <int EPI, int BN>
 dit_status launch_t(const CUtensorMap& ta, const CUtensorMap& tb, const CUtensorMap& tx, const EpiArgs& ep, int M, int N, int K,
-                    cudaStream_t st, int k_wrap = 0) {
+                    cudaStream_t st, int k_wrap = 0, const SegLaunch* sl = nullptr) {
   static std::atomic<bool> attr_set{false};
   if (!attr_set) {
     DIT_CUDA_OK(cudaFuncSetAttribute(gemm_tc_kernel<EPI, BN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                      smem_bytes(BN, EPI)));
     attr_set = true;
   }
-  const int pairs = cdiv(cdiv(M, BM), 2) * cdiv(N, EPI == EPI_SWIGLU ? BN / 2 : BN);
+  const int mt2 = sl != nullptr ? sl->segs->tile0[sl->segs->n] : cdiv(cdiv(M, BM), 2);
+  const int pairs = mt2 * cdiv(N, EPI == EPI_SWIGLU ? BN / 2 : BN);
   const int max_pairs = sm_count() / 2;
   DIT_CUDA_OK(launch_pdl(gemm_tc_kernel<EPI, BN>, dim3(2 * (pairs < max_pairs ? pairs : max_pairs)), dim3(GEMM_THREADS),
-                         smem_bytes(BN, EPI), st, 2, ta, tb, tx, ep, M, N, K, group_rows(M, K), k_wrap));
+                         smem_bytes(BN, EPI), st, 2, ta, tb, tx, sl != nullptr ? *sl->tb2 : tb, sl != nullptr ? *sl->tx2 : tx, ep,
+                         sl != nullptr ? *sl->segs : no_segs(), M, N, K, group_rows(mt2 * 2 * BM, K), k_wrap));
   DIT_LAUNCH_CHECK();
   return DIT_OK;
 }
 
 // Tile width that minimises waves x width on this many SMs (wave quantisation: M = 4352 gives 34 M-tiles, and
 // 34 x {36, 48, 12} tiles of 256 columns leave the last wave 3-27 % full; 240- or 192-wide tiles fill it).
-int pick_bn(int M, int N) {
+int pick_bn(int M, int N, int mt2 = -1) {
   const int cand[3] = {256, 240, 192};
   int best = 256;
   int64_t best_cost = INT64_MAX;
+  if (mt2 < 0) mt2 = cdiv(cdiv(M, BM), 2);
   for (int i = 0; i < 3; ++i) {
     const int bn = cand[i];
-    const int64_t tiles = (int64_t)cdiv(cdiv(M, BM), 2) * cdiv(N, bn);   // tile pairs on CTA pairs
+    const int64_t tiles = (int64_t)mt2 * cdiv(N, bn);   // tile pairs on CTA pairs
     const int64_t cost = cdiv(tiles, (int64_t)(sm_count() / 2)) * bn;
     if (cost < best_cost - best_cost / 64) {   // a narrower tile must win by > 1.5 %
       best_cost = cost;
@@ -565,10 +611,10 @@ int pick_bn(int M, int N) {
 
 template <int EPI>
 dit_status launch_bn(int bn, const CUtensorMap& ta, const CUtensorMap& tb, const CUtensorMap& tx, const EpiArgs& ep, int M,
-                     int N, int K, cudaStream_t st, int k_wrap = 0) {
-  if (bn == 192) return launch_t<EPI, 192>(ta, tb, tx, ep, M, N, K, st, k_wrap);
-  if (bn == 240) return launch_t<EPI, 240>(ta, tb, tx, ep, M, N, K, st, k_wrap);
-  return launch_t<EPI, 256>(ta, tb, tx, ep, M, N, K, st, k_wrap);
+                     int N, int K, cudaStream_t st, int k_wrap = 0, const SegLaunch* sl = nullptr) {
+  if (bn == 192) return launch_t<EPI, 192>(ta, tb, tx, ep, M, N, K, st, k_wrap, sl);
+  if (bn == 240) return launch_t<EPI, 240>(ta, tb, tx, ep, M, N, K, st, k_wrap, sl);
+  return launch_t<EPI, 256>(ta, tb, tx, ep, M, N, K, st, k_wrap, sl);
 }
 
 }  // namespace
@@ -593,7 +639,7 @@ dit_status launch_gemm_tc_ex(int epi, const void* A, int64_t lda, const void* W,
   const int Ka = a_split ? 2 * K : K;
   DIT_REQUIRE(make_tmap_2d_bf16(&ta, A, M, Ka, lda, BM, BK) && make_tmap_2d_bf16(&tb, W, N, K, K, bn / 2, BK), DIT_ERR_CUDA,
               "gemm_tc: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d lda=%lld)", M, N, K, (long long)lda);
-  EpiArgs ep{(const bf16*)bias, nullptr, out, ldo, gate, gate_stride, cu, R, nullptr, nullptr, nullptr, nullptr, 0.f, 0, 0, nullptr, nullptr};
+  EpiArgs ep{(const bf16*)bias, nullptr, out, ldo, gate, gate_stride, cu, R, nullptr, nullptr, nullptr, nullptr, 0.f, 0, 0, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 0};
   ProfScope _prof(DIT_KC_GEMM, st);
   switch (epi) {
     case DIT_EPI_BIAS: return launch_bn<DIT_EPI_BIAS>(bn, ta, tb, ta, ep, M, N, Ka, st, k_wrap);
@@ -624,7 +670,7 @@ dit_status launch_gemm_tc_qkv(const void* A, int64_t lda, const void* W, const v
   CUtensorMap ta, tb;
   DIT_REQUIRE(make_tmap_2d_bf16(&ta, A, M, Ka, lda, BM, BK) && make_tmap_2d_bf16(&tb, W, N, K, K, 128, BK), DIT_ERR_CUDA,
               "gemm_tc_qkv: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d)", M, N, K);
-  EpiArgs ep{(const bf16*)bias, nullptr, out, ldo, nullptr, 0, nullptr, 1, (const bf16*)gq, (const bf16*)gk, rc, rs, rms_eps, q_end, k_end, nullptr, nullptr};
+  EpiArgs ep{(const bf16*)bias, nullptr, out, ldo, nullptr, 0, nullptr, 1, (const bf16*)gq, (const bf16*)gk, rc, rs, rms_eps, q_end, k_end, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 0};
   ProfScope _prof(DIT_KC_GEMM, st);
   return launch_t<EPI_QKV_NORM_ROPE, 256>(ta, tb, ta, ep, M, N, Ka, st, k_wrap);
 }
@@ -637,9 +683,49 @@ dit_status launch_gemm_tc_swiglu(const void* A, int64_t lda, const void* W1, con
   DIT_REQUIRE(make_tmap_2d_bf16(&ta, A, M, K, lda, BM, BK) && make_tmap_2d_bf16(&tb, W1, N, K, K, 128, BK) &&
                   make_tmap_2d_bf16(&tx, W3, N, K, K, 128, BK),
               DIT_ERR_CUDA, "gemm_tc_swiglu: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d)", M, N, K);
-  EpiArgs ep{(const bf16*)b1, (const bf16*)b3, out, ldo, nullptr, 0, nullptr, 1, nullptr, nullptr, nullptr, nullptr, 0.f, 0, 0, nullptr, nullptr};
+  EpiArgs ep{(const bf16*)b1, (const bf16*)b3, out, ldo, nullptr, 0, nullptr, 1, nullptr, nullptr, nullptr, nullptr, 0.f, 0, 0, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 0};
   ProfScope _prof(DIT_KC_GEMM, st);
   return launch_t<EPI_SWIGLU, 256>(ta, tb, tx, ep, M, N, K, st, 0);
+}
+
+// One launch over every row segment of a packed buffer, two weight sets (dual-stream blocks, R37); see GemmSegs / SegGemm.
+dit_status launch_gemm_tc_segs(const SegGemm& g, cudaStream_t st) {
+  if (g.M == 0 || g.N == 0 || g.segs == nullptr || g.segs->n == 0) return DIT_OK;
+  const GemmSegs& sg = *g.segs;
+  const int mt2 = sg.tile0[sg.n];
+  const bool wide = g.kind == EPI_QKV_NORM_ROPE || g.kind == EPI_SWIGLU;    // 256-wide tiles only
+  const int bn = wide ? 256 : pick_bn(g.M, g.N, mt2);
+  const int wbox = wide ? 128 : bn / 2;
+  const void* W0 = g.W[0];
+  const void* W1 = g.W[1] != nullptr ? g.W[1] : g.W[0];
+  CUtensorMap ta, tb, tb2, tx, tx2;
+  DIT_REQUIRE(make_tmap_2d_bf16(&ta, g.A, g.M, g.K, g.lda, BM, BK) && make_tmap_2d_bf16(&tb, W0, g.N, g.K, g.K, wbox, BK) &&
+                  make_tmap_2d_bf16(&tb2, W1, g.N, g.K, g.K, wbox, BK),
+              DIT_ERR_CUDA, "gemm_tc_segs: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d)", g.M, g.N, g.K);
+  tx = ta; tx2 = ta;
+  if (g.kind == EPI_SWIGLU) {
+    DIT_REQUIRE(make_tmap_2d_bf16(&tx, g.W3[0], g.N, g.K, g.K, 128, BK) &&
+                    make_tmap_2d_bf16(&tx2, g.W3[1] != nullptr ? g.W3[1] : g.W3[0], g.N, g.K, g.K, 128, BK),
+                DIT_ERR_CUDA, "gemm_tc_segs: cuTensorMapEncodeTiled (W3) failed");
+  } else if (g.kind == EPI_GATE_RESID) {
+    DIT_REQUIRE(make_tmap_2d_f32(&tx, g.out, g.M, g.N, g.ldo, 32), DIT_ERR_CUDA, "gemm_tc_segs: cuTensorMapEncodeTiled (x) failed");
+    tx2 = tx;
+  }
+  EpiArgs ep{(const bf16*)g.bias[0], (const bf16*)g.b3[0], g.out, g.ldo, g.gate, g.gate_stride, nullptr, 1,
+             (const bf16*)g.gq[0], (const bf16*)g.gk[0], g.rc, g.rs, g.rms_eps, g.N / 3, 2 * (g.N / 3), nullptr, nullptr,
+             (const bf16*)g.bias[1], (const bf16*)g.b3[1], (const bf16*)g.gq[1], (const bf16*)g.gk[1], g.gate_set_off};
+  const SegLaunch sl{g.segs, &tb2, &tx2};
+  ProfScope _prof(DIT_KC_GEMM, st);
+  switch (g.kind) {
+    case DIT_EPI_BIAS: return launch_bn<DIT_EPI_BIAS>(bn, ta, tb, tx, ep, g.M, g.N, g.K, st, 0, &sl);
+    case DIT_EPI_BIAS_GELU: return launch_bn<DIT_EPI_BIAS_GELU>(bn, ta, tb, tx, ep, g.M, g.N, g.K, st, 0, &sl);
+    case EPI_GATE_RESID: return launch_bn<EPI_GATE_RESID>(bn, ta, tb, tx, ep, g.M, g.N, g.K, st, 0, &sl);
+    case EPI_QKV_NORM_ROPE:
+      DIT_REQUIRE(g.N % 384 == 0, DIT_ERR_INVALID_ARG, "gemm_tc_segs: QKV needs N = 3 D, D %% 128 == 0 (N=%d)", g.N);
+      return launch_t<EPI_QKV_NORM_ROPE, 256>(ta, tb, tx, ep, g.M, g.N, g.K, st, 0, &sl);
+    case EPI_SWIGLU: return launch_t<EPI_SWIGLU, 256>(ta, tb, tx, ep, g.M, g.N, g.K, st, 0, &sl);
+    default: DIT_REQUIRE(false, DIT_ERR_INVALID_ARG, "gemm_tc_segs: kind %d", g.kind);
+  }
 }
 
 // fp8 linear layer (R42): out = e(decode(Aq) decode(Wq)^T (.) a_scale w_scale^T + bias); Aq [M, lda bytes], Wq [N, K] e4m3
@@ -655,7 +741,7 @@ dit_status launch_gemm_tc_fp8(int epi, const void* Aq, int64_t lda, const float*
   const int bn = pick_bn(M, N);
   DIT_REQUIRE(make_tmap_2d_u8(&ta, Aq, M, K, lda, BM) && make_tmap_2d_u8(&tb, Wq, N, K, K, bn / 2), DIT_ERR_CUDA,
               "gemm_tc_fp8: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d lda=%lld)", M, N, K, (long long)lda);
-  EpiArgs ep{(const bf16*)bias, nullptr, out, ldo, nullptr, 0, nullptr, 1, nullptr, nullptr, nullptr, nullptr, 0.f, 0, 0, a_scale, w_scale};
+  EpiArgs ep{(const bf16*)bias, nullptr, out, ldo, nullptr, 0, nullptr, 1, nullptr, nullptr, nullptr, nullptr, 0.f, 0, 0, a_scale, w_scale, nullptr, nullptr, nullptr, nullptr, 0};
   ProfScope _prof(DIT_KC_GEMM, st);
   switch (epi) {
     case DIT_EPI_BIAS: return launch_bn<EPI_F8 + DIT_EPI_BIAS>(bn, ta, tb, ta, ep, M, N, K, st, 0);
