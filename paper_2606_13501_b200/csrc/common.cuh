@@ -206,7 +206,7 @@ dit_status launch_gemv(int dtype, const float* in, const GemvBatch* batches_dev,
 // split != 0 (bf16 only): y is [T, 2D] = [hi | lo], y = hi + lo to ~16 bits (the final layer's input, R36)
 dit_status launch_adaln(int dtype, float* x, const void* h, const float* gate, const float* shift, const float* scale,
                         int64_t mod_stride, const int32_t* cu, int R, void* y, int T, int D, float eps, cudaStream_t st,
-                        int split = 0);
+                        int split = 0, int64_t set_off = 0);   // set_off != 0: cu = R row segments, text | image alternating (R37)
 dit_status launch_qknorm_rope(int dtype, void* qkv, int64_t row_stride, int T, int H, int d, int n_tensors,
                               const void* gq, const void* gk, float eps, const float* rc, const float* rs,
                               cudaStream_t st);

@@ -91,6 +91,7 @@ struct Workspace {
   float* lse_part; // [P, Tm, H]
   int32_t* cu_dev;     // [Rm+1]
   int32_t* cu_cond_dev;// [Rm+1]
+  int32_t* cu_seg_dev; // [2 Rm + 1]: dual-stream blocks, row segments text | image of every request
   SeqMeta* meta_dev;   // [Rm]
   GemvBatch* gemv_tab; // [L + 1 + 2]
   void* stage_in;  // host-call staging: latents | temb | cond
@@ -156,6 +157,7 @@ static bool carve(const dit_config& c, char* base, Workspace* w) {
   w->lse_part = (float*)take(c.split_p > 1 ? (size_t)c.split_p * Tm * c.n_heads * 4 : 0);
   w->cu_dev = (int32_t*)take((Rm + 1) * 4);
   w->cu_cond_dev = (int32_t*)take((Rm + 1) * 4);
+  w->cu_seg_dev = (int32_t*)take(c.cond_mode == DIT_COND_JOINT2 ? (2 * Rm + 1) * 4 : 0);
   w->meta_dev = (SeqMeta*)take(Rm * sizeof(SeqMeta));
   w->gemv_tab = (GemvBatch*)take((2 * L + 4) * sizeof(GemvBatch));
   w->stage_in = take(Tm * pvC * es + Rm * c.temb_dim * 4 + Lcm * c.cond_dim * es + 1024);
@@ -331,6 +333,12 @@ static dit_status upload_geom(dit_handle hd, const StepGeom& g, cudaStream_t st)
   DIT_CUDA_OK(cudaMemcpyAsync(w.cu_dev, g.cu.data(), (R + 1) * 4, cudaMemcpyHostToDevice, st));
   DIT_CUDA_OK(cudaMemcpyAsync(w.cu_cond_dev, g.cu_cond.data(), (R + 1) * 4, cudaMemcpyHostToDevice, st));
   DIT_CUDA_OK(cudaMemcpyAsync(w.meta_dev, meta.data(), R * sizeof(SeqMeta), cudaMemcpyHostToDevice, st));
+  if (c.cond_mode == DIT_COND_JOINT2) {   // segment starts: text of request r at cu[r], its image rows at cu[r] + n_cond[r]
+    std::vector<int32_t> seg(2 * R + 1);
+    for (int r = 0; r < R; ++r) { seg[2 * r] = g.cu[r]; seg[2 * r + 1] = g.cu[r] + g.ncond[r]; }
+    seg[2 * R] = T;
+    DIT_CUDA_OK(cudaMemcpyAsync(w.cu_seg_dev, seg.data(), (2 * R + 1) * 4, cudaMemcpyHostToDevice, st));
+  }
   if (rope) {
     dit_status s = launch_rope_table(w.meta_dev, R, T, d, c.rope_dims, c.rope_theta, w.rope_c, w.rope_s, st);
     if (s != DIT_OK) return s;
@@ -445,9 +453,9 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
       const SW sw_txt{b.t_wqkv, b.t_bqkv, b.t_gq, b.t_gk, b.t_wo, b.t_bo, b.t_w1, b.t_b1, b.t_w2, b.t_b2, b.t_w3, b.t_b3};
       auto mod_of = [&](const Seg& sg) { return w.mod + (size_t)sg.r * mod_stride + (sg.txt ? mod_img : 0) + (size_t)l * 6 * D; };
       auto rows_of = [&](void* base, const Seg& sg, int64_t ld) { return (void*)((char*)base + (size_t)sg.row0 * ld * es); };
-      for (const Seg& sg : segs)
-        RUN(launch_adaln(dt, w.x + (size_t)sg.row0 * D, nullptr, nullptr, mod_of(sg), mod_of(sg) + D, 0, nullptr, 1, rows_of(w.y, sg, D),
-                         sg.rows, D, c.ln_eps, st));
+      // adaLN: one launch over all segments (row -> segment -> request and stream through cu_seg_dev)
+      const float* mblk = w.mod + (size_t)l * 6 * D;
+      RUN(launch_adaln(dt, w.x, nullptr, nullptr, mblk, mblk + D, mod_stride, w.cu_seg_dev, 2 * R, w.y, T, D, c.ln_eps, st, 0, mod_img));
       if (stop(l, DIT_STAGE_Y1)) return DIT_OK;
       SegGemm sgm{};   // the fields every segmented launch of this block shares
       sgm.segs = &gsegs; sgm.M = T; sgm.rms_eps = c.rms_eps;
@@ -515,9 +523,8 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
                           sg.rows, D, D, st));
       }
       if (stop(l, DIT_STAGE_OPROJ)) return DIT_OK;
-      for (const Seg& sg : segs)
-        RUN(launch_adaln(dt, w.x + (size_t)sg.row0 * D, nullptr, nullptr, mod_of(sg) + 3 * D, mod_of(sg) + 4 * D, 0, nullptr, 1,
-                         rows_of(w.y, sg, D), sg.rows, D, c.ln_eps, st));
+      RUN(launch_adaln(dt, w.x, nullptr, nullptr, mblk + 3 * D, mblk + 4 * D, mod_stride, w.cu_seg_dev, 2 * R, w.y, T, D, c.ln_eps, st, 0,
+                       mod_img));
       if (stop(l, DIT_STAGE_Y2)) return DIT_OK;
       if (grouped) {
         SegGemm q = sgm;

@@ -150,7 +150,7 @@ __global__ void __launch_bounds__(128) adaln_kernel(float* __restrict__ x, const
                                                     const float* __restrict__ gate, const float* __restrict__ shift,
                                                     const float* __restrict__ scale, int64_t mod_stride,
                                                     const int32_t* __restrict__ cu, int R, T* __restrict__ y, int T_rows,
-                                                    float eps, int split) {
+                                                    float eps, int split, int64_t set_off) {
   pdl_trigger();
   pdl_wait();
   constexpr int D = NCW * WPR * 256;
@@ -161,7 +161,10 @@ __global__ void __launch_bounds__(128) adaln_kernel(float* __restrict__ x, const
   const int row_raw = blockIdx.x * RPB + warp / WPR;
   const bool row_ok = row_raw < T_rows;
   const int row = row_ok ? row_raw : T_rows - 1;     // out-of-range warps redo the last row and store nothing
-  const int req = (cu != nullptr && R > 1) ? find_request(cu, R, row) : 0;
+  // set_off != 0 (dual-stream blocks, R37): `cu` holds the R row SEGMENTS [text of request 0 | image of request 0 | text of
+  // request 1 | ...]; an even (text) segment takes the modulation row at + set_off
+  const int seg = (cu != nullptr && R > 1) ? find_request(cu, R, row) : 0;
+  const int64_t moff = set_off != 0 ? (int64_t)(seg >> 1) * mod_stride + ((seg & 1) ? 0 : set_off) : (int64_t)seg * mod_stride;
   const int col0 = sub * (NCW * 256) + lane * 8;     // chunk c of this lane starts at col0 + c * 256
   float* xr = x + (int64_t)row * D + col0;
   float v[NCW][8];
@@ -169,7 +172,7 @@ __global__ void __launch_bounds__(128) adaln_kernel(float* __restrict__ x, const
   for (int c = 0; c < NCW; ++c) ld8<float>(xr + c * 256, v[c]);
   if (h != nullptr) {
     const T* hr = h + (int64_t)row * D + col0;
-    const float* g = gate ? gate + (int64_t)req * mod_stride + col0 : nullptr;
+    const float* g = gate ? gate + moff + col0 : nullptr;
 #pragma unroll
     for (int c = 0; c < NCW; ++c) {
       float hv[8], gv[8];
@@ -211,8 +214,8 @@ __global__ void __launch_bounds__(128) adaln_kernel(float* __restrict__ x, const
     for (int i = 0; i < WPR; ++i) q += red[1][(warp / WPR) * WPR + i];
   }
   const float rstd = rsqrtf(q * (1.0f / D) + eps);
-  const float* sh = shift ? shift + (int64_t)req * mod_stride + col0 : nullptr;
-  const float* sc = scale ? scale + (int64_t)req * mod_stride + col0 : nullptr;
+  const float* sh = shift ? shift + moff + col0 : nullptr;
+  const float* sc = scale ? scale + moff + col0 : nullptr;
   T* yr = y + (int64_t)row * (split ? 2 * D : D) + col0;   // split: row = [hi (D) | lo (D)]
 #pragma unroll
   for (int c = 0; c < NCW; ++c) {
@@ -239,14 +242,14 @@ __global__ void __launch_bounds__(128) adaln_kernel(float* __restrict__ x, const
 template <typename T>
 static dit_status launch_adaln_t(float* x, const T* h, const float* gate, const float* shift, const float* scale,
                                  int64_t mod_stride, const int32_t* cu, int R, T* y, int T_rows, int D, float eps,
-                                 cudaStream_t st, int split) {
+                                 cudaStream_t st, int split, int64_t set_off) {
   if (T_rows == 0) return DIT_OK;
   DIT_REQUIRE(D % 256 == 0 && D <= 6144, DIT_ERR_UNSUPPORTED, "adaln: D=%d must be a multiple of 256 (<= 6144)", D);
   ProfScope _prof(DIT_KC_ADALN, st);
 #define ADALN_CASE(NCV, NCW, WPR)                                                                           \
   case NCV:                                                                                                 \
     DIT_CUDA_OK(launch_pdl(adaln_kernel<T, NCW, WPR>, dim3(cdiv(T_rows, 4 / WPR)), dim3(128), 0, st, 1, x, h, gate, \
-                           shift, scale, mod_stride, cu, R, y, T_rows, eps, split));                         \
+                           shift, scale, mod_stride, cu, R, y, T_rows, eps, split, set_off));                \
     break;
   switch (D / 256) {   // D / 256 chunks per row = NCW per warp x WPR warps
     ADALN_CASE(1, 1, 1) ADALN_CASE(2, 2, 1) ADALN_CASE(3, 3, 1) ADALN_CASE(4, 4, 1) ADALN_CASE(5, 5, 1)
@@ -262,10 +265,10 @@ static dit_status launch_adaln_t(float* x, const T* h, const float* gate, const 
 
 dit_status launch_adaln(int dtype, float* x, const void* h, const float* gate, const float* shift, const float* scale,
                         int64_t mod_stride, const int32_t* cu, int R, void* y, int T, int D, float eps, cudaStream_t st,
-                        int split) {
+                        int split, int64_t set_off) {
   if (dtype == DIT_F32)
-    return launch_adaln_t<float>(x, (const float*)h, gate, shift, scale, mod_stride, cu, R, (float*)y, T, D, eps, st, 0);
-  return launch_adaln_t<bf16>(x, (const bf16*)h, gate, shift, scale, mod_stride, cu, R, (bf16*)y, T, D, eps, st, split);
+    return launch_adaln_t<float>(x, (const float*)h, gate, shift, scale, mod_stride, cu, R, (float*)y, T, D, eps, st, 0, set_off);
+  return launch_adaln_t<bf16>(x, (const bf16*)h, gate, shift, scale, mod_stride, cu, R, (bf16*)y, T, D, eps, st, split, set_off);
 }
 
 // =================================================================================================
