@@ -166,6 +166,33 @@ def test_cfg2_full_size_end_to_end(lib):
          x_after_block_max_abs_over_rms=[c[1] for c in curve], oracle_s=round(t_or, 1))
 
 
+def test_cfg2_shape_dual_stream_gated_end_to_end(lib):
+    """The block variants bench.py times as cfg2_dual_gated, at the cfg 2 SHAPE (4096 + 256 rows, D = 3072, F = 12288) with two
+    blocks: dual-stream joint blocks (one segmented tcgen05 launch per projection over the text and image segments, 17 row-tile
+    pairs, 240- / 256-wide tiles) with the gated MLP — whole tensors against the oracle's whole step: `out` and the residual
+    stream after each block."""
+    if _host_gb() < 24:
+        pytest.skip("the oracle's fp64 intermediates need ~16 GB of host memory")
+    s = synth.cfg2(name="cfg2_dual_gated_2", cond_mode="joint2", n_blocks=2, extras={"mlp_gated": True})
+    W = synth.make_weights(s, device=DEV)
+    I = synth.make_inputs(s, device=DEV)
+    m = B.Dit(B.make_config(s), W, DEV)
+    lat, temb, cond = I["latents"], I["temb"][0].contiguous(), I["cond"]
+    D, L, T = s.hidden, s.n_blocks, s.n_tokens + s.n_cond
+    n0 = B.dit_fallback_launches()
+    out = m.dit_step(lat, temb, cond)
+    xs = _x_taps(m, lambda: m.dit_step(lat, temb, cond), T, D, L, "fc2")
+    assert B.dit_fallback_launches() == n0
+    taps = KeepTaps([f"b{l}.x_mlp" for l in range(L)])
+    t0 = time.time()
+    ref = O.dit_step(O.cfg_from_shape(s), {k: v.cpu() for k, v in W.items()}, lat.cpu(), I["temb"].cpu(), cond.cpu(), taps=taps)
+    t_or = time.time() - t0
+    curve = [check(xs[l], taps[f"b{l}.x_mlp"], torch.bfloat16, f"cfg2 dual + gated: x after block {l}") for l in range(L)]
+    e_out = check(out, ref, torch.bfloat16, "cfg2 dual + gated: out")
+    _log(test="cfg2 shape, dual-stream + gated MLP, 2 blocks, end to end", out_rel_l2=e_out[0], out_max_abs_over_rms=e_out[1],
+         x_after_block_rel_l2=[c[0] for c in curve], oracle_s=round(t_or, 1))
+
+
 def test_cfg2_full_size_blocks_teacher_forced(lib):
     s = synth.cfg2()
     W = synth.make_weights(s, device=DEV)
