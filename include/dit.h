@@ -149,16 +149,19 @@ dit_status dit_sample(dit_handle h, const void* latents, const float* timestep_e
                       float guidance_scale, const int32_t latent_grid[3], int32_t n_steps, int32_t use_graph, void* out,
                       void* stream);
 
-/* Same computation with HOST buffers (pageable or pinned): H2D copies of latents / timestep_emb / cond,
- * the step, and the D2H copy of `out` are all enqueued on `stream`; staging lives in the workspace.
+/* Same computation with HOST buffers (pageable or pinned): H2D copies of latents / timestep_emb / cond, the step, and the
+ * D2H copy of `out`; staging lives in the workspace.  Everything is ordered with respect to `stream`: the latent / cond
+ * uploads run on a copy stream of the handle that first waits for all work already enqueued on `stream` and is joined back
+ * before patch-embed (they overlap the timestep MLP and the modulation GEMV, which need only timestep_emb); the caller
+ * synchronises `stream` before reading out_host or reusing the host input buffers.
  * This is the end-to-end call bench.py times ("e2e"). */
 dit_status dit_step_host(dit_handle h, const void* latents_host, const float* timestep_emb_host,
                          const void* cond_tokens_host, int32_t n_cond, const int32_t latent_grid[3],
                          void* out_host, void* stream);
 
 /* dit_step_varlen with HOST buffers (pageable or pinned): latents_packed / timestep_emb / cond_packed are copied to the
- * workspace's staging area, the packed step runs, and out_packed is copied back, all enqueued on `stream`; the caller
- * synchronises the stream before reading out_packed_host.  Arguments as dit_step_varlen below. */
+ * workspace's staging area, the packed step runs, and out_packed is copied back, ordered with respect to `stream` as in
+ * dit_step_host; the caller synchronises the stream before reading out_packed_host.  Arguments as dit_step_varlen below. */
 dit_status dit_step_varlen_host(dit_handle h, const void* latents_packed_host, const float* timestep_emb_host,
                                 const void* cond_packed_host, const int32_t* cu_seqlens, const int32_t* n_cond,
                                 const int32_t* latent_grids, int32_t n_requests, void* out_packed_host, void* stream);
