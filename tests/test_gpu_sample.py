@@ -25,7 +25,7 @@ def _traj(s, n_steps, n_unc=None):
 
 def _packed_caps(s, n_unc):
     """Handle capacities that let dit_sample run a guided step as ONE packed pass of two requests (include/dit.h)."""
-    joint = s.cond_mode == "joint"
+    joint = s.cond_mode in ("joint", "joint2")
     return dict(max_requests=2, max_tokens=2 * s.n_tokens + (s.n_cond + n_unc if joint else 0), max_cond_tokens=s.n_cond + n_unc)
 
 
@@ -72,6 +72,26 @@ def test_bf16_guided_trajectory(lib, use_graph, packed):
                    latent_channels=16, rope_dims=(0, 64, 64), qk_rmsnorm=True, n_blocks=3)
     out, ref, *_, I = _both(s, 4, n_unc=32, g=3.0, use_graph=use_graph, packed=packed)
     _check_traj(out, ref, I, torch.bfloat16, f"bf16 guided 4 steps packed={packed}", 2e-2)
+
+
+@pytest.mark.parametrize("dtype,packed,use_graph", [("bf16", False, False), ("bf16", True, True), ("f32", True, False)])
+def test_dual_stream_gated_guided_trajectory(lib, dtype, packed, use_graph):
+    """Dual-stream blocks with the gated MLP through dit_sample: two passes per step, or ONE packed pass of two requests that
+    share a modulation row (row stride 0) while each request has its own text / image segments (segmented GEMM launches, one
+    adaLN launch over the four segments); n_uncond != n_cond."""
+    if dtype == "bf16":
+        s = synth.cfg1(name="traj_dual", dtype="bf16", cond_mode="joint2", hidden=512, n_heads=4, head_dim=128, mlp_dim=1096,
+                       cond_dim=512, latent_channels=16, rope_dims=(0, 64, 64), qk_rmsnorm=True, n_blocks=2,
+                       extras={"t": 500.0, "mlp_gated": True})
+        bar = 2e-2
+    else:
+        s = synth.cfg1(cond_mode="joint2", rope_dims=(0, 32, 32), qk_rmsnorm=True, extras={"t": 500.0, "mlp_gated": True})
+        bar = 5e-5
+    n0 = B.dit_fallback_launches()
+    out, ref, *_, I = _both(s, 3, n_unc=20, g=3.0, use_graph=use_graph, packed=packed)
+    _check_traj(out, ref, I, s.torch_dtype, f"dual-stream gated guided {dtype} packed={packed}", bar)
+    if dtype == "bf16":
+        assert B.dit_fallback_launches() == n0
 
 
 def test_packed_guidance_needs_room_for_both_requests(lib):
