@@ -540,12 +540,14 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   }
 }
 
-// Row-tile pairs per raster group: their A panels (256 rows x K bf16 each) should take about 48 MB of the 126 MB L2.
+// Row-tile pairs per raster group: their A panels (256 rows x K bf16 each) should take about 36 MB of the 126 MB L2 (DRAM reads
+// of the cfg 3 QKV GEMM by ncu at 12 / 24 / 36 / 48 / 72 MB: 7.49 / 4.61 / 3.66 / 4.69 / 7.06 GB, 3.58 / 3.41 / 3.31 / 3.39 / 3.56 ms;
+// the step times are flat between 30 and 48 MB: profiles/r02_gemm_cfg3_traffic.md).
 int group_rows(int M, int K) {
   const int mt2 = cdiv(cdiv(M, BM), 2);
-  static const double budget = []() {   // DIT_GEMM_L2_MB overrides the 48 MB default (tuning knob)
+  static const double budget = []() {   // DIT_GEMM_L2_MB overrides the 36 MB default (tuning knob)
     const char* e = getenv("DIT_GEMM_L2_MB");
-    return (e != nullptr && atof(e) > 0 ? atof(e) : 48.0) * 1.0e6;
+    return (e != nullptr && atof(e) > 0 ? atof(e) : 36.0) * 1.0e6;
   }();
   int gm = (int)(budget / (512.0 * K) + 0.5);
   if (gm < 4) gm = 4;
