@@ -133,6 +133,9 @@ struct EpiArgs {
   // segmented launches (GemmSegs): the second weight set's vectors, and the offset of its gate rows
   const bf16* bias_b; const bf16* bias2_b; const bf16* gq_b; const bf16* gk_b;
   int64_t gate_set_off;
+  // EPI_QKV_NORM_ROPE: tiles from this index on (the last, less than half full wave) are HALF tiles of one head (128 columns,
+  // N = 128 MMAs, 64 W rows per CTA through tensor map X / X2): the tail wave takes half a tile time.  -1: none.
+  int narrow_from;
 };
 
 __device__ __forceinline__ float gelu_tanh_fast(float z) {
@@ -176,7 +179,9 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   constexpr int EPB = F8 ? EPI - EPI_F8 : EPI;   // the epilogue proper
   constexpr int BKE = F8 ? 2 * BK : BK;          // elements per 128-byte k-block
   const int mt = (M + BM - 1) / BM, mt2 = segs.n > 0 ? segs.tile0[segs.n] : (mt + 1) >> 1;
-  const int nt = (N + BN_OUT - 1) / BN_OUT, n_tiles = mt2 * nt;   // tile PAIRS
+  const int nt = (N + BN_OUT - 1) / BN_OUT, n_wide = mt2 * nt;   // tile PAIRS
+  const int narrow_from = (EPI == EPI_QKV_NORM_ROPE && ep.narrow_from >= 0) ? ep.narrow_from : n_wide;
+  const int n_tiles = narrow_from + 2 * (n_wide - narrow_from);
   const int nkb = (K + BKE - 1) / BKE;
   // Tile order: groups of GM row-tile pairs; inside a group the column tile is the slow index.  A wave of 74 CTA
   // pairs then covers ~74 / GM column tiles of the same GM row-tile pairs, whose A panels (GM x 256 x K) are sized
@@ -188,6 +193,18 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     const int gsize = (mt2 - g * GM) < GM ? (mt2 - g * GM) : GM;
     n = r / gsize;
     mp = g * GM + (r - n * gsize);
+  };
+
+  // tile t -> row-tile pair, column tile, and for the half tiles of the tail wave which half (else -1)
+  auto tile_of = [&](int t, int& mp, int& n, int& half) {
+    if (t < narrow_from) {
+      tile_mn(t, mp, n);
+      half = -1;
+    } else {
+      const int u = t - narrow_from;
+      tile_mn(narrow_from + (u >> 1), mp, n);
+      half = u & 1;
+    }
   };
 
   // Segmented launch: row-tile pair mp belongs to the last segment whose first pair is <= mp; its rows start at the segment's
@@ -241,17 +258,21 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     int s = 0;
     uint32_t ph = 0;
     for (int t = pair; t < n_tiles; t += n_pairs) {
-      int mp, nn;
-      tile_mn(t, mp, nn);
+      int mp, nn, half;
+      tile_of(t, mp, nn, half);
       int m_base, m_end, wset, req;
       seg_of(mp, m_base, m_end, wset, req);
-      const int m0 = m_base + rank * BM, n0 = EPI == EPI_SWIGLU ? nn * (BN / 2) : nn * BN + rank * (BN / 2);
-      const CUtensorMap* const tmW = (EPI == EPI_SWIGLU && rank != 0) ? (wset ? &tmX2 : &tmX) : (wset ? &tmB2 : &tmB);
+      const bool narrow = EPI == EPI_QKV_NORM_ROPE && half >= 0;
+      const int m0 = m_base + rank * BM;
+      const int n0 = EPI == EPI_SWIGLU ? nn * (BN / 2) : (narrow ? nn * BN + half * 128 + rank * 64 : nn * BN + rank * (BN / 2));
+      const CUtensorMap* const tmW =
+          ((EPI == EPI_SWIGLU && rank != 0) || narrow) ? (wset ? &tmX2 : &tmX) : (wset ? &tmB2 : &tmB);
+      const uint32_t stage_tx = narrow ? 2 * (A_BYTES + 64 * BK * 2) : 2 * STAGE_BYTES;
       for (int kb = 0; kb < nkb; ++kb) {
         mbar_wait_poll(empty_bar(s), ph ^ 1);
         if (elect_one()) {
           const uint32_t fb = mapa_cluster(full_bar(s), 0);
-          if (rank == 0) mbar_expect_tx(full_bar(s), 2 * STAGE_BYTES);
+          if (rank == 0) mbar_expect_tx(full_bar(s), stage_tx);
           tma_load_2d_pair(smem0 + s * STAGE_BYTES, &tmA, kb * BKE, m0, fb);
           // k_wrap > 0: A is [hi | lo] (two bf16 parts side by side) and W repeats along K every k_wrap blocks
           tma_load_2d_pair(smem0 + s * STAGE_BYTES + A_BYTES, tmW, (k_wrap > 0 ? kb % k_wrap : kb) * BKE, n0, fb);
@@ -274,6 +295,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       mbar_wait_poll(tempty_bar(as), aph ^ 1);
       tc_fence_after();
       const uint32_t d_tmem = tmem_base + as * BN_MAX;
+      const uint32_t idesc_t = (EPI == EPI_QKV_NORM_ROPE && t >= narrow_from) ? idesc_bf16(2 * BM, 128, 0, 0) : idesc;
       for (int kb = 0; kb < nkb; ++kb) {
         mbar_wait_poll(full_bar(s), ph);
         tc_fence_after();
@@ -283,7 +305,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
 #pragma unroll
           for (int k = 0; k < BK / 16; ++k) {   // 32 bytes of K per instruction in both kinds
             if (F8) umma_ss_pair_f8(d_tmem, ad + 2 * k, bd + 2 * k, idesc, (kb | k) != 0);
-            else umma_ss_pair(d_tmem, ad + 2 * k, bd + 2 * k, idesc, (kb | k) != 0);
+            else umma_ss_pair(d_tmem, ad + 2 * k, bd + 2 * k, idesc_t, (kb | k) != 0);
           }
           umma_commit_pair(empty_bar(s), (uint16_t)3);
           if (kb == nkb - 1) umma_commit_pair(tfull_bar(as), (uint16_t)3);
@@ -304,11 +326,12 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     for (int t = pair; t < n_tiles; t += n_pairs, ++it) {
       const int as = it & 1;
       const uint32_t aph = (it >> 1) & 1;
-      int mp, nn;
-      tile_mn(t, mp, nn);
+      int mp, nn, half;
+      tile_of(t, mp, nn, half);
       int m_base, m_end, wset, seg_req;
       seg_of(mp, m_base, m_end, wset, seg_req);
-      const int m0 = m_base + rank * BM, n0 = nn * BN_OUT;
+      const int m0 = m_base + rank * BM, n0 = nn * BN_OUT + ((EPI == EPI_QKV_NORM_ROPE && half > 0) ? 128 : 0);
+      const int heads_in_tile = (EPI == EPI_QKV_NORM_ROPE && half >= 0) ? 1 : BN / 128;
       const int row = m0 + quad * 32 + lane;
       const bool row_ok = row < m_end;
       const bf16* const bias_p = wset ? ep.bias_b : ep.bias;
@@ -370,7 +393,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         const float* const rcr = ep.rc != nullptr ? ep.rc + (int64_t)(row_ok ? row : 0) * 64 : nullptr;
         const float* const rsr = ep.rs != nullptr ? ep.rs + (int64_t)(row_ok ? row : 0) * 64 : nullptr;
 #pragma unroll 1
-        for (int hh = 0; hh < BN / 128; ++hh) {
+        for (int hh = 0; hh < heads_in_tile; ++hh) {
           const int nh = n0 + hh * 128;
           if (nh >= N) break;  // warp-uniform
           const int which = nh < ep.q_end ? 0 : (nh < ep.k_end ? 1 : 2);   // 0 = q, 1 = k, 2 = v
@@ -573,6 +596,14 @@ const GemmSegs& no_segs() {
 // segmented launches pass the segment table and the second weight set's tensor maps (tb2: W, tx2: W3 of the SwiGLU form)
 struct SegLaunch { const GemmSegs* segs; const CUtensorMap* tb2; const CUtensorMap* tx2; };
 
+// First tile of the tail wave when that wave would be less than half full (then it is run as half-width tiles), else -1
+int narrow_tail_from(int n_wide) {
+  static const bool off = []() { const char* e = getenv("DIT_GEMM_NO_NARROW_TAIL"); return e != nullptr && e[0] == '1'; }();
+  const int max_pairs = sm_count() / 2;
+  const int full = (n_wide / max_pairs) * max_pairs, rem = n_wide - full;
+  return (!off && rem > 0 && 2 * rem <= max_pairs) ? full : -1;
+}
+
 template <int EPI, int BN>
 dit_status launch_t(const CUtensorMap& ta, const CUtensorMap& tb, const CUtensorMap& tx, const EpiArgs& ep, int M, int N, int K,
                     cudaStream_t st, int k_wrap = 0, const SegLaunch* sl = nullptr) {
@@ -583,7 +614,8 @@ dit_status launch_t(const CUtensorMap& ta, const CUtensorMap& tb, const CUtensor
     attr_set = true;
   }
   const int mt2 = sl != nullptr ? sl->segs->tile0[sl->segs->n] : cdiv(cdiv(M, BM), 2);
-  const int pairs = mt2 * cdiv(N, EPI == EPI_SWIGLU ? BN / 2 : BN);
+  const int n_wide = mt2 * cdiv(N, EPI == EPI_SWIGLU ? BN / 2 : BN);
+  const int pairs = (EPI == EPI_QKV_NORM_ROPE && ep.narrow_from >= 0) ? ep.narrow_from + 2 * (n_wide - ep.narrow_from) : n_wide;
   const int max_pairs = sm_count() / 2;
   DIT_CUDA_OK(launch_pdl(gemm_tc_kernel<EPI, BN>, dim3(2 * (pairs < max_pairs ? pairs : max_pairs)), dim3(GEMM_THREADS),
                          smem_bytes(BN, EPI), st, 2, ta, tb, tx, sl != nullptr ? *sl->tb2 : tb, sl != nullptr ? *sl->tx2 : tx, ep,
@@ -641,7 +673,7 @@ dit_status launch_gemm_tc_ex(int epi, const void* A, int64_t lda, const void* W,
   const int Ka = a_split ? 2 * K : K;
   DIT_REQUIRE(make_tmap_2d_bf16(&ta, A, M, Ka, lda, BM, BK) && make_tmap_2d_bf16(&tb, W, N, K, K, bn / 2, BK), DIT_ERR_CUDA,
               "gemm_tc: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d lda=%lld)", M, N, K, (long long)lda);
-  EpiArgs ep{(const bf16*)bias, nullptr, out, ldo, gate, gate_stride, cu, R, nullptr, nullptr, nullptr, nullptr, 0.f, 0, 0, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 0};
+  EpiArgs ep{(const bf16*)bias, nullptr, out, ldo, gate, gate_stride, cu, R, nullptr, nullptr, nullptr, nullptr, 0.f, 0, 0, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 0, -1};
   ProfScope _prof(DIT_KC_GEMM, st);
   switch (epi) {
     case DIT_EPI_BIAS: return launch_bn<DIT_EPI_BIAS>(bn, ta, tb, ta, ep, M, N, Ka, st, k_wrap);
@@ -672,9 +704,12 @@ dit_status launch_gemm_tc_qkv(const void* A, int64_t lda, const void* W, const v
   CUtensorMap ta, tb;
   DIT_REQUIRE(make_tmap_2d_bf16(&ta, A, M, Ka, lda, BM, BK) && make_tmap_2d_bf16(&tb, W, N, K, K, 128, BK), DIT_ERR_CUDA,
               "gemm_tc_qkv: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d)", M, N, K);
-  EpiArgs ep{(const bf16*)bias, nullptr, out, ldo, nullptr, 0, nullptr, 1, (const bf16*)gq, (const bf16*)gk, rc, rs, rms_eps, q_end, k_end, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 0};
+  EpiArgs ep{(const bf16*)bias, nullptr, out, ldo, nullptr, 0, nullptr, 1, (const bf16*)gq, (const bf16*)gk, rc, rs, rms_eps, q_end, k_end, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 0, -1};
   ProfScope _prof(DIT_KC_GEMM, st);
-  return launch_t<EPI_QKV_NORM_ROPE, 256>(ta, tb, ta, ep, M, N, Ka, st, k_wrap);
+  CUtensorMap tn;   // W as 64-row boxes: the half tiles of the tail wave
+  DIT_REQUIRE(make_tmap_2d_bf16(&tn, W, N, K, K, 64, BK), DIT_ERR_CUDA, "gemm_tc_qkv: cuTensorMapEncodeTiled (narrow W) failed");
+  ep.narrow_from = narrow_tail_from(cdiv(cdiv(M, BM), 2) * cdiv(N, 256));
+  return launch_t<EPI_QKV_NORM_ROPE, 256>(ta, tb, tn, ep, M, N, Ka, st, k_wrap);
 }
 
 // Gated-MLP up-projection (R40): out bf16 [M, ldo] <- SiLU(A W1^T + b1) (.) (A W3^T + b3); W1, W3 [N, K], b1, b3 [N].
@@ -685,7 +720,7 @@ dit_status launch_gemm_tc_swiglu(const void* A, int64_t lda, const void* W1, con
   DIT_REQUIRE(make_tmap_2d_bf16(&ta, A, M, K, lda, BM, BK) && make_tmap_2d_bf16(&tb, W1, N, K, K, 128, BK) &&
                   make_tmap_2d_bf16(&tx, W3, N, K, K, 128, BK),
               DIT_ERR_CUDA, "gemm_tc_swiglu: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d)", M, N, K);
-  EpiArgs ep{(const bf16*)b1, (const bf16*)b3, out, ldo, nullptr, 0, nullptr, 1, nullptr, nullptr, nullptr, nullptr, 0.f, 0, 0, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 0};
+  EpiArgs ep{(const bf16*)b1, (const bf16*)b3, out, ldo, nullptr, 0, nullptr, 1, nullptr, nullptr, nullptr, nullptr, 0.f, 0, 0, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 0, -1};
   ProfScope _prof(DIT_KC_GEMM, st);
   return launch_t<EPI_SWIGLU, 256>(ta, tb, tx, ep, M, N, K, st, 0);
 }
@@ -715,7 +750,7 @@ dit_status launch_gemm_tc_segs(const SegGemm& g, cudaStream_t st) {
   }
   EpiArgs ep{(const bf16*)g.bias[0], (const bf16*)g.b3[0], g.out, g.ldo, g.gate, g.gate_stride, nullptr, 1,
              (const bf16*)g.gq[0], (const bf16*)g.gk[0], g.rc, g.rs, g.rms_eps, g.N / 3, 2 * (g.N / 3), nullptr, nullptr,
-             (const bf16*)g.bias[1], (const bf16*)g.b3[1], (const bf16*)g.gq[1], (const bf16*)g.gk[1], g.gate_set_off};
+             (const bf16*)g.bias[1], (const bf16*)g.b3[1], (const bf16*)g.gq[1], (const bf16*)g.gk[1], g.gate_set_off, -1};
   const SegLaunch sl{g.segs, &tb2, &tx2};
   ProfScope _prof(DIT_KC_GEMM, st);
   switch (g.kind) {
@@ -724,6 +759,9 @@ dit_status launch_gemm_tc_segs(const SegGemm& g, cudaStream_t st) {
     case EPI_GATE_RESID: return launch_bn<EPI_GATE_RESID>(bn, ta, tb, tx, ep, g.M, g.N, g.K, st, 0, &sl);
     case EPI_QKV_NORM_ROPE:
       DIT_REQUIRE(g.N % 384 == 0, DIT_ERR_INVALID_ARG, "gemm_tc_segs: QKV needs N = 3 D, D %% 128 == 0 (N=%d)", g.N);
+      DIT_REQUIRE(make_tmap_2d_bf16(&tx, W0, g.N, g.K, g.K, 64, BK) && make_tmap_2d_bf16(&tx2, W1, g.N, g.K, g.K, 64, BK), DIT_ERR_CUDA,
+                  "gemm_tc_segs: cuTensorMapEncodeTiled (narrow W) failed");
+      ep.narrow_from = narrow_tail_from(mt2 * cdiv(g.N, 256));
       return launch_t<EPI_QKV_NORM_ROPE, 256>(ta, tb, tx, ep, g.M, g.N, g.K, st, 0, &sl);
     case EPI_SWIGLU: return launch_t<EPI_SWIGLU, 256>(ta, tb, tx, ep, g.M, g.N, g.K, st, 0, &sl);
     default: DIT_REQUIRE(false, DIT_ERR_INVALID_ARG, "gemm_tc_segs: kind %d", g.kind);
@@ -743,7 +781,7 @@ dit_status launch_gemm_tc_fp8(int epi, const void* Aq, int64_t lda, const float*
   const int bn = pick_bn(M, N);
   DIT_REQUIRE(make_tmap_2d_u8(&ta, Aq, M, K, lda, BM) && make_tmap_2d_u8(&tb, Wq, N, K, K, bn / 2), DIT_ERR_CUDA,
               "gemm_tc_fp8: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d lda=%lld)", M, N, K, (long long)lda);
-  EpiArgs ep{(const bf16*)bias, nullptr, out, ldo, nullptr, 0, nullptr, 1, nullptr, nullptr, nullptr, nullptr, 0.f, 0, 0, a_scale, w_scale, nullptr, nullptr, nullptr, nullptr, 0};
+  EpiArgs ep{(const bf16*)bias, nullptr, out, ldo, nullptr, 0, nullptr, 1, nullptr, nullptr, nullptr, nullptr, 0.f, 0, 0, a_scale, w_scale, nullptr, nullptr, nullptr, nullptr, 0, -1};
   ProfScope _prof(DIT_KC_GEMM, st);
   switch (epi) {
     case DIT_EPI_BIAS: return launch_bn<EPI_F8 + DIT_EPI_BIAS>(bn, ta, tb, ta, ep, M, N, K, st, 0);
