@@ -1156,7 +1156,15 @@ dit_status launch_attn_tc(const AttnArgs& a, cudaStream_t st) {
     p.n_items = n_items;
     int sms = 148;
     { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); }
-    dim3 pgrid(2 * min(n_items, sms / 2), 1, 1);
+    // Equal items (one request): the fewest pairs that still finish in the same number of rounds — cfg 2: 408 items are 6 rounds on
+    // 74 pairs (5.51) and also on 68; the idle SMs' power goes to the clock of the busy ones (the step is power capped).
+    int n_pairs = min(n_items, sms / 2);
+    static const bool trim = []() { const char* e = getenv("DIT_ATTN_NO_TRIM"); return !(e != nullptr && e[0] == '1'); }();
+    if (trim && p.R == 1 && n_pairs > 0) {
+      const int rounds = cdiv(n_items, n_pairs);
+      n_pairs = cdiv(n_items, rounds);
+    }
+    dim3 pgrid(2 * n_pairs, 1, 1);
     DIT_CUDA_OK(launch_pdl(attn_pair_kernel, pgrid, dim3(ATTN_THREADS), PAIR_SMEM, st, 2, tq, tk, tv, p));
     DIT_LAUNCH_CHECK();
     return DIT_OK;
