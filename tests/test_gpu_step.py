@@ -340,6 +340,28 @@ def test_dual_stream_varlen_and_empty_text(lib):
     assert B.dit_fallback_launches() == n0
 
 
+@pytest.mark.parametrize("mode", ["joint2", "joint"])
+def test_sixty_four_tiny_requests_packed(lib, mode):
+    """max_requests = 64 (the capacity limit): 64 tiny requests in one packed step — in dual-stream mode 128 row segments, the
+    size of the segmented GEMM's table, each far smaller than a 256-row tile pair; every request against the oracle alone."""
+    R = 64
+    grids = [(1, 4 + 4 * (r % 3), 4 + 4 * (r % 2)) for r in range(R)]
+    nconds = [1 + (r * 5) % 7 for r in range(R)]
+    shapes = [_small_bf16(cond_mode=mode, latent_grid=g, n_cond=n, n_blocks=1) for g, n in zip(grids, nconds)]
+    W = synth.make_weights(shapes[0])
+    Is = [synth.make_inputs(sh, tag=f"t{r}", t=20.0 + 15 * r) for r, sh in enumerate(shapes)]
+    T_total = sum(sh.n_tokens + n for sh, n in zip(shapes, nconds))
+    m = B.Dit(B.make_config(shapes[0], max_tokens=T_total, max_requests=R, max_cond_tokens=sum(nconds)), W, DEV)
+    n0 = B.dit_fallback_launches()
+    outs = m.dit_step_varlen([i["latents"].to(DEV) for i in Is], torch.cat([i["temb"] for i in Is]).to(DEV),
+                             [i["cond"].to(DEV) for i in Is])
+    torch.cuda.synchronize()
+    assert B.dit_fallback_launches() == n0
+    for r in (0, 1, 2, 17, 40, 63):
+        ref = O.dit_step(O.cfg_from_shape(shapes[r]), W, Is[r]["latents"], Is[r]["temb"], Is[r]["cond"])
+        check(outs[r], ref, torch.bfloat16, f"64 packed requests ({mode}), request {r}")
+
+
 def test_argument_validation_on_gpu(lib):
     s = synth.cfg1()
     W, I = synth.make_weights(s), synth.make_inputs(s)
