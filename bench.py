@@ -443,6 +443,24 @@ def run_ours(args, rank: int, local_rank: int, world: int):
             sec = smp.step_seconds()
             line["cpu_baseline"] = {"value": 1.0 / sec, "unit": UNIT, "cores": torch.get_num_threads(), "kind": "oracle",
                                     "sample": smp.sample}
+        if world == 1 and not args.no_cpu_baseline and args.workload == "cfg4":
+            # The packed batch is DEFINED as its requests one by one (DESIGN.md section 3 step 8): the oracle is timed on the
+            # two smallest distinct requests (1024 and 4096 image tokens), one block each, and the others are extrapolated
+            # with t(T) = a T + b T^2 (per-token work + attention) fitted to the two.
+            torch.set_num_threads(os.cpu_count() or 1)
+            reqs = synth.cfg4_requests()
+            Ts = [sh.n_tokens + sh.n_cond for sh in reqs]
+            t_of = {}
+            for sh in (reqs[0], reqs[2]):
+                t_of[sh.n_tokens + sh.n_cond] = OracleSample(sh).step_seconds()
+            (T1, t1), (T2, t2) = sorted(t_of.items())
+            b_ = (t2 / T2 - t1 / T1) / (T2 - T1)
+            a_ = t1 / T1 - b_ * T1
+            sec = sum(a_ * T + b_ * T * T for T in Ts)
+            line["cpu_baseline"] = {"value": 1.0 / sec, "unit": UNIT, "cores": torch.get_num_threads(), "kind": "oracle",
+                                    "sample": f"oracle dit_step (torch CPU float64) on requests 0 and 2 alone ({T1} and {T2} tokens, 1 of "
+                                              f"{s.n_blocks} blocks each, extrapolated to the step as in the other workloads: {t1:.1f} s and "
+                                              f"{t2:.1f} s); the six requests' times from t(T) = a T + b T^2 fitted to the two, summed"}
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
