@@ -51,3 +51,28 @@ def test_reference_arm_runs_on_rank0_only():
     import bench
     args = argparse.Namespace(workload="cfg2", steps=1, warmup=0, gpus=2)
     assert bench.run_reference(args, rank=1) is None         # returns before touching the oracle
+
+
+def test_step_flops_and_workload_shapes():
+    """The algorithmic flop counts behind bench.py's roofline lines, written out by hand, and the
+    block-variant workloads' shapes."""
+    import bench
+    from paper_2606_13501_b200 import synth
+    s = bench._shape("cfg2")
+    T, D, F, L = 4096 + 256, 3072, 12288, 8
+    fl = bench.step_flops(s)
+    assert fl["gemm"] == L * (2 * T * D * 3 * D + 2 * T * D * D + 2 * 2 * T * D * F) and fl["T"] == T
+    assert fl["attn"] == L * 4 * T * T * 128 * 24
+    assert abs(fl["gemm"] / 1e12 - 7.886) < 1e-3 and abs(fl["attn"] / 1e12 - 1.862) < 1e-3      # DESIGN.md section 6
+    g = bench._shape("cfg2_dual_gated")
+    assert g.cond_mode == "joint2" and g.extras.get("mlp_gated") and g.hidden == D and g.n_blocks == L
+    fg = bench.step_flops(g)
+    assert fg["gemm"] - fl["gemm"] == L * 2 * T * D * F          # the gate's second up-projection; the two streams share T
+    assert fg["attn"] == fl["attn"]
+    assert "blocks.0.txt.mlp.w3" in synth.weight_shapes(g) and "blocks.0.mlp.w3" not in synth.weight_shapes(s)
+    c3 = bench.step_flops(bench._shape("cfg3"))
+    assert abs(c3["gemm"] / 1e12 - 78.54) < 0.01 and abs(c3["attn"] / 1e12 - 89.29) < 0.01
+    seq = [sh.n_tokens + sh.n_cond for sh in synth.cfg4_requests()]
+    c4 = bench.step_flops(bench._shape("cfg4"), seq)
+    assert sum(seq) == 37376 and abs(c4["gemm"] / 1e12 - 67.72) < 0.01 and abs(c4["attn"] / 1e12 - 40.09) < 0.01
+    assert "dual-stream" in bench._workload_name(g) and "BASELINE.json configs[1]" in bench._workload_name(s)
