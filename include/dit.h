@@ -229,6 +229,21 @@ int32_t dit_relayout_plan(int64_t n_rows, int32_t p_src, int32_t p_dst, dit_tran
 dit_status dit_relayout(const dit_transfer* entries, int32_t n_entries, const void* const* src_shards,
                         void* const* dst_shards, int64_t row_bytes, void* stream);
 
+/* Split-KV attention + LSE merge that ALLOCATES NOTHING (for callers that cannot call cudaMalloc: code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid it).  Same result as dit_attn_partial on the split_p contiguous KV
+ * shards of ceil(n_k / split_p) keys (R20) followed by dit_attn_merge, but the partial outputs and their log-sum-exps live
+ * in a static device array inside the library instead of caller memory: dit_static_scratch_bytes() = 8 MiB, held by every
+ * GPU that loads the library until the process exits.  Arguments as dit_attn_partial; o dev [n_q, H, d] in dtype, lse_out
+ * dev fp32 [n_q, H] or NULL.  split_p in 1..8.  Returns DIT_ERR_WORKSPACE (message via dit_last_error(NULL)) when
+ * split_p * (align256(n_q * H * d * sizeof(dtype)) + align256(n_q * H * 4)) exceeds the array.  No cudaMalloc, cudaFree or
+ * allocating library routine is called.  All calls on a device share the one array (it keeps the last call's contents;
+ * nothing needs to start at zero: every partial row is written before the merge reads it): calls that OVERLAP on the GPU
+ * (two streams, two host threads on one device) race and must be serialised by the caller. */
+size_t dit_static_scratch_bytes(void);
+dit_status dit_attn_split_static(int32_t dtype, const void* q, const void* k, const void* v, int32_t n_q, int32_t n_k,
+                                 int32_t n_heads, int32_t head_dim, int64_t q_row_stride, int64_t kv_row_stride,
+                                 float softmax_scale, int32_t split_p, void* o, float* lse_out, void* stream);
+
 /* ---- kernel-level entry points (the building blocks of dit_step; used by the parity tests and by
  *      bench.py's per-kernel roofline lines) ------------------------------------------------------ */
 

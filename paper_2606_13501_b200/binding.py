@@ -19,7 +19,7 @@ TAP = dict(x=0, y=1, qkv=2, o=3, u=5, c=6, mod=7, tok=8)
 STAGE = dict(y1=0, qkv=1, attn=2, oproj=3, cross=4, y2=5, fc1=6, fc2=7)
 
 SYMBOLS = ["dit_workspace_bytes", "dit_init", "dit_step", "dit_step_host", "dit_step_varlen", "dit_step_varlen_host", "dit_sample", "dit_attn_partial",
-           "dit_attn_merge", "dit_relayout_plan", "dit_relayout", "dit_linear", "dit_linear_swiglu", "dit_quantize_fp8", "dit_linear_fp8", "dit_linear_residual", "dit_linear_qkv", "dit_adaln", "dit_gemv", "dit_qknorm_rope", "dit_debug_stop_after",
+           "dit_attn_merge", "dit_static_scratch_bytes", "dit_attn_split_static", "dit_relayout_plan", "dit_relayout", "dit_linear", "dit_linear_swiglu", "dit_quantize_fp8", "dit_linear_fp8", "dit_linear_residual", "dit_linear_qkv", "dit_adaln", "dit_gemv", "dit_qknorm_rope", "dit_debug_stop_after",
            "dit_get_tap", "dit_profile_begin", "dit_profile_end", "dit_last_error", "dit_kernel_launches", "dit_fallback_launches", "dit_sim_run",
            "dit_free"]
 
@@ -91,6 +91,8 @@ def load(path: str = LIB_PATH):
     lib.dit_kernel_launches.restype = C.c_int32
     lib.dit_fallback_launches.restype = C.c_int32
     lib.dit_relayout_plan.restype = C.c_int32
+    lib.dit_static_scratch_bytes.restype = C.c_size_t
+    lib.dit_static_scratch_bytes.argtypes = []
     lib.dit_free.restype = None
     lib.dit_free.argtypes = [C.c_void_p]
     vp, i32, i64, f32 = C.c_void_p, C.c_int32, C.c_int64, C.c_float
@@ -104,6 +106,7 @@ def load(path: str = LIB_PATH):
         "dit_sample": [vp, vp, vp, C.POINTER(C.c_float), vp, i32, vp, i32, f32, pi32, i32, i32, vp, vp],
         "dit_attn_partial": [i32, vp, vp, vp, i32, i32, i32, i32, i64, i64, f32, vp, vp, vp],
         "dit_attn_merge": [i32, C.POINTER(vp), C.POINTER(vp), i32, i32, i32, i32, vp, vp, vp],
+        "dit_attn_split_static": [i32, vp, vp, vp, i32, i32, i32, i32, i64, i64, f32, i32, vp, vp, vp],
         "dit_relayout_plan": [i64, i32, i32, C.POINTER(dit_transfer), i32],
         "dit_relayout": [C.POINTER(dit_transfer), i32, C.POINTER(vp), C.POINTER(vp), i64, vp],
         "dit_linear": [i32, i32, vp, i64, vp, vp, vp, i64, i32, i32, i32, vp],
@@ -300,6 +303,23 @@ def dit_attn_partial(q, k, v, softmax_scale=None, want_lse=True, stream=None):
     _check(lib.dit_attn_partial(_dt(q), _ptr(q), _ptr(k), _ptr(v), nq, nk, H, d, q.stride(0) if nq else H * d,
                                 k.stride(0) if nk else H * d, scale, _ptr(o), _ptr(lse), _stream(stream)),
            "dit_attn_partial")
+    return o, lse
+
+
+def dit_static_scratch_bytes() -> int:
+    return int(load().dit_static_scratch_bytes())
+
+
+def dit_attn_split_static(q, k, v, split_p, o, lse=None, softmax_scale=None, stream=None):
+    """Split-KV attention + merge with the partials in the library's static device array: allocates nothing (the caller
+    passes the outputs o [Nq,H,d] and, optionally, lse [Nq,H] fp32)."""
+    lib = load()
+    nq, H, d = q.shape
+    nk = k.shape[0]
+    scale = d ** -0.5 if softmax_scale is None else softmax_scale
+    _check(lib.dit_attn_split_static(_dt(q), _ptr(q), _ptr(k), _ptr(v), nq, nk, H, d, q.stride(0) if nq else H * d,
+                                     k.stride(0) if nk else H * d, scale, split_p, _ptr(o), _ptr(lse), _stream(stream)),
+           "dit_attn_split_static")
     return o, lse
 
 
