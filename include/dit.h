@@ -284,6 +284,23 @@ dit_status dit_linear_fp8(int32_t epilogue, const void* Aq, int64_t lda, const f
                           const float* w_scale, const void* bias, void* out, int64_t ldo, int32_t M, int32_t N, int32_t K,
                           void* stream);
 
+/* Block-scaled MXFP8 linear layer (OCP Microscaling format) — SURVEY.md §8(f) item 2 ("block-scaled ... mxf8 GEMMs with the same
+ * oracle"); reading R43.  Kernel level only, like the fp8 layer above.
+ *
+ * dit_quantize_mxfp8: per block of 32 consecutive elements along K of x [M, K] (dev, DIT_BF16 or DIT_F32, row stride ldx):
+ *     amax = max |v|;  shared_exp = clamp(floor(log2(amax)) - 8, -127, 127)  (0 for a zero block);
+ *     scales[m, b] = shared_exp + 127  (E8M0: X = 2^(code - 127));   q[m, k] = e4m3(v / X)  (RN-even, saturating at +-448)
+ *   q dev uint8 [M, ldq], scales dev uint8 [M, K / 32] contiguous.  K % 32 == 0, ldx % 8 == 0, ldq % 16 == 0, 16-byte aligned.
+ * dit_linear_mxfp8:  out[M, N] = epilogue( sum_b Xa[m, b] Xw[n, b] sum_{k in b} val(Aq[m, k]) val(Wq[n, k]) + bias[n] )
+ *   Aq dev uint8 [M, lda], a_scales dev uint8 [M, K / 32]; Wq dev uint8 [N, K] contiguous, w_scales dev uint8 [N, K / 32]; bias dev
+ *   bf16 [N] or NULL; out dev bf16 [M, ldo] (DIT_EPI_BIAS, DIT_EPI_BIAS_GELU) or fp32 (DIT_EPI_BIAS_F32).  tcgen05
+ *   kind::mxf8f6f4.block_scale MMAs (the tensor core applies the block scales), fp32 accumulation.  K % 128 == 0, lda % 16 == 0,
+ *   N and ldo multiples of 8, operands 16-byte and scales 4-byte aligned; DIT_ERR_UNSUPPORTED otherwise. */
+dit_status dit_quantize_mxfp8(int32_t dtype, const void* x, int64_t ldx, int32_t M, int32_t K, void* q, int64_t ldq, void* scales,
+                              void* stream);
+dit_status dit_linear_mxfp8(int32_t epilogue, const void* Aq, int64_t lda, const void* a_scales, const void* Wq, const void* w_scales,
+                            const void* bias, void* out, int64_t ldo, int32_t M, int32_t N, int32_t K, void* stream);
+
 /* Residual-stream producer with the gate fused in the GEMM epilogue (north_star subsystem 3, "gate epilogues";
  * the out-projection and fc2 of every block):   x[M, N] <- x + gate[req(row)] (.) (A[M, K] W[N, K]^T + bias[N])
  *   x dev fp32 [M, ldx] in/out;  A, W, bias in dtype;  gate dev fp32 [n_requests, gate_stride] (NULL = 1), row ->

@@ -19,7 +19,7 @@ TAP = dict(x=0, y=1, qkv=2, o=3, u=5, c=6, mod=7, tok=8)
 STAGE = dict(y1=0, qkv=1, attn=2, oproj=3, cross=4, y2=5, fc1=6, fc2=7)
 
 SYMBOLS = ["dit_workspace_bytes", "dit_init", "dit_step", "dit_step_host", "dit_step_varlen", "dit_step_varlen_host", "dit_sample", "dit_attn_partial",
-           "dit_attn_merge", "dit_static_scratch_bytes", "dit_attn_split_static", "dit_relayout_plan", "dit_relayout", "dit_linear", "dit_linear_swiglu", "dit_quantize_fp8", "dit_linear_fp8", "dit_linear_residual", "dit_linear_qkv", "dit_adaln", "dit_gemv", "dit_qknorm_rope", "dit_debug_stop_after",
+           "dit_attn_merge", "dit_static_scratch_bytes", "dit_attn_split_static", "dit_relayout_plan", "dit_relayout", "dit_linear", "dit_linear_swiglu", "dit_quantize_fp8", "dit_linear_fp8", "dit_quantize_mxfp8", "dit_linear_mxfp8", "dit_linear_residual", "dit_linear_qkv", "dit_adaln", "dit_gemv", "dit_qknorm_rope", "dit_debug_stop_after",
            "dit_get_tap", "dit_profile_begin", "dit_profile_end", "dit_last_error", "dit_kernel_launches", "dit_fallback_launches", "dit_sim_run",
            "dit_free"]
 
@@ -113,6 +113,8 @@ def load(path: str = LIB_PATH):
         "dit_linear_swiglu": [i32, vp, i64, vp, vp, vp, vp, vp, i64, vp, i32, i32, i32, vp],
         "dit_quantize_fp8": [i32, vp, i64, i32, i32, vp, i64, vp, vp],
         "dit_linear_fp8": [i32, vp, i64, vp, vp, vp, vp, vp, i64, i32, i32, i32, vp],
+        "dit_quantize_mxfp8": [i32, vp, i64, i32, i32, vp, i64, vp, vp],
+        "dit_linear_mxfp8": [i32, vp, i64, vp, vp, vp, vp, vp, i64, i32, i32, i32, vp],
         "dit_linear_residual": [i32, vp, i64, vp, vp, vp, i64, vp, i64, vp, i32, i32, i32, i32, vp],
         "dit_linear_qkv": [i32, vp, i64, vp, vp, vp, i64, vp, vp, f32, vp, vp, i32, i32, i32, vp],
         "dit_adaln": [i32, vp, vp, vp, vp, vp, i64, vp, i32, vp, i32, i32, f32, vp],
@@ -413,6 +415,29 @@ def dit_linear_fp8(Aq, a_scale, Wq, w_scale, bias=None, epilogue=EPI_BIAS, out=N
         out = torch.empty((M, N), dtype=torch.float32 if epilogue == EPI_BIAS_F32 else torch.bfloat16, device=Aq.device)
     _check(lib.dit_linear_fp8(epilogue, _ptr(Aq), Aq.stride(0), _ptr(a_scale), _ptr(Wq), _ptr(w_scale), _ptr(bias), _ptr(out),
                               out.stride(0), M, N, K, _stream(stream)), "dit_linear_fp8")
+    return out
+
+
+def dit_quantize_mxfp8(x, stream=None):
+    """Rows of x [M, K] (bf16 / fp32) -> (e4m3 codes uint8 [M, K], E8M0 block scales uint8 [M, K / 32])."""
+    lib = load()
+    M, K = x.shape
+    q = torch.empty((M, K), dtype=torch.uint8, device=x.device)
+    sc = torch.empty((M, K // 32), dtype=torch.uint8, device=x.device)
+    _check(lib.dit_quantize_mxfp8(_dt(x), _ptr(x), x.stride(0), M, K, _ptr(q), q.stride(0), _ptr(sc), _stream(stream)),
+           "dit_quantize_mxfp8")
+    return q, sc
+
+
+def dit_linear_mxfp8(Aq, a_scales, Wq, w_scales, bias=None, epilogue=EPI_BIAS, out=None, stream=None):
+    """Block-scaled MXFP8 product: out [M, N] = epilogue(sum over 32-blocks of Xa Xw (val(Aq) val(Wq)^T) + bias)."""
+    lib = load()
+    M, K = Aq.shape
+    N = Wq.shape[0]
+    if out is None:
+        out = torch.empty((M, N), dtype=torch.float32 if epilogue == EPI_BIAS_F32 else torch.bfloat16, device=Aq.device)
+    _check(lib.dit_linear_mxfp8(epilogue, _ptr(Aq), Aq.stride(0), _ptr(a_scales), _ptr(Wq), _ptr(w_scales), _ptr(bias), _ptr(out),
+                                out.stride(0), M, N, K, _stream(stream)), "dit_linear_mxfp8")
     return out
 
 
