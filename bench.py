@@ -621,7 +621,15 @@ def run_kernels(args):
             Wq, sw = B.dit_quantize_fp8(Wt)
             del A, Wt
             tensor(f"gemm fp8 {nm} {M}x{N}x{K}", 2 * M * N * K, lambda: B.dit_linear_fp8(Aq, sa, Wq, sw, b, epi, out=o), fp8=True)
-            del Aq, Wq, o
+            del Aq, Wq
+            # block-scaled MXFP8 (R43): E8M0 scale per 32 elements, applied by the tensor core
+            A2, W2 = rn("A", (M, K), bf), rn("W", (N, K), bf, 0.02)
+            hbm(f"quantize mxfp8 {nm} {M}x{K}", 3 * M * K + M * K // 32, lambda: B.dit_quantize_mxfp8(A2))
+            Am, sam = B.dit_quantize_mxfp8(A2)
+            Wm, swm = B.dit_quantize_mxfp8(W2)
+            del A2, W2
+            tensor(f"gemm mxfp8 {nm} {M}x{N}x{K}", 2 * M * N * K, lambda: B.dit_linear_mxfp8(Am, sam, Wm, swm, b, epi, out=o), fp8=True)
+            del Am, Wm, o
         # gated-MLP up-projection (R40): W1 | W3 in one kernel, 2 x 2 T F D flops
         y = rn("y", (T, D), bf)
         w1, w3 = rn("w1", (F_, D), bf, 0.02), rn("w3", (F_, D), bf, 0.02)

@@ -274,6 +274,9 @@ dit_status launch_gemm_tc_swiglu(const void* A, int64_t lda, const void* W1, con
 // fp8 (e4m3) linear layer with fp32 row scales on both operands (R42)
 dit_status launch_gemm_tc_fp8(int epi, const void* Aq, int64_t lda, const float* a_scale, const void* Wq, const float* w_scale,
                               const void* bias, void* out, int64_t ldo, int M, int N, int K, cudaStream_t st);
+// block-scaled MXFP8 layer on the pair kernel (R43)
+dit_status launch_gemm_tc_mx(int epi, const void* Aq, int64_t lda, const void* sfa, const void* Wq, const void* sfw, const void* bias,
+                             void* out, int64_t ldo, int M, int N, int K, cudaStream_t st);
 // rows of x [M, K] (ldx elements) -> e4m3 codes [M, ldq bytes] + fp32 row scales (R42: scale = amax / 448, RN-even, saturating)
 dit_status launch_quantize_fp8(int dtype, const void* x, int64_t ldx, int M, int K, void* q, int64_t ldq, float* scale, cudaStream_t st);
 dit_status launch_silu_mul(int dtype, void* u, const void* u3, int64_t n, cudaStream_t st);   // u <- SiLU(u) (.) u3 (FFMA path)

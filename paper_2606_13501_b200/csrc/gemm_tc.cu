@@ -89,7 +89,14 @@ constexpr int A_BYTES = BM * BK * 2;
 constexpr int stage_bytes(int bn) { return A_BYTES + (bn / 2) * BK * 2; }   // own A rows + own HALF of the W tile
 constexpr int GEMM_THREADS = 192;
 constexpr int EPI_THREADS = 128;
-enum { EPI_GATE_RESID = 3, EPI_QKV_NORM_ROPE = 4, EPI_BIAS_SPLIT = 5, EPI_SWIGLU = 6, EPI_F8 = 7 /* + 0 / 1 / 2 */ };
+enum { EPI_GATE_RESID = 3, EPI_QKV_NORM_ROPE = 4, EPI_BIAS_SPLIT = 5, EPI_SWIGLU = 6, EPI_F8 = 7 /* + 0 / 1 / 2 */,
+       EPI_MX = 10 /* + 0 / 1 / 2 */ };
+// EPI_MX + e: block-scaled MXFP8 (R43): e4m3 operands as in EPI_F8, but `kind::mxf8f6f4.block_scale` MMAs read one
+// E8M0 scale per row and 32-element K slice from TENSOR MEMORY.  Four extra warps per CTA (6-9, one per TMEM lane quadrant) write
+// them there for every k-block, in the layout `tcgen05.cp ... 32x128b.warpx4` would produce: lane l of every quadrant, column
+// c0 + j, byte k = scale of row l + 32 j, K slice k.  Each CTA holds the scales of its own 128 A rows and of ALL BN W rows.
+// Tile width 224: two accumulator stages (2 x 224 columns) + 4 scale stages of 12 columns fit the 512 TMEM columns.
+constexpr int MX_THREADS = 320, MX_SF_STAGES = 4, MX_SF_COLS = 12;
 // EPI_F8 + e (e = DIT_EPI_BIAS / _GELU / _F32): both operands are e4m3 bytes (R42), kind::f8f6f4 MMAs with K = 32;
 // a k-block is still 128 bytes of every operand row (128 elements instead of 64), so stages, descriptors and the
 // instruction count per byte are those of the bf16 kernel at twice the flops.  The epilogue applies the row scales:
@@ -136,6 +143,7 @@ struct EpiArgs {
   // EPI_QKV_NORM_ROPE: tiles from this index on (the last, less than half full wave) are HALF tiles of one head (128 columns,
   // N = 128 MMAs, 64 W rows per CTA through tensor map X / X2): the tail wave takes half a tile time.  -1: none.
   int narrow_from;
+  const uint8_t* mx_sfa; const uint8_t* mx_sfw;   // EPI_MX: E8M0 block scales [M, K / 32], [N, K / 32]
 };
 
 __device__ __forceinline__ float gelu_tanh_fast(float z) {
@@ -144,8 +152,25 @@ __device__ __forceinline__ float gelu_tanh_fast(float z) {
   return __fdividef(z, 1.0f + __expf(-u2));
 }
 
+__device__ __forceinline__ void umma_mx_pair(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t sfa,
+                                             uint32_t sfb, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::2.kind::mxf8f6f4.block_scale [%0], %1, %2, %3, [%5], [%6], p;\n\t}" ::"r"(d_tmem),
+      "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate), "r"(sfa), "r"(sfb)
+      : "memory");
+}
+// block-scaled instruction descriptor: E4M3 x E4M3, E8M0 scales, K-major, K = 32; sf = scale byte (K slice) for A and B
+__device__ __forceinline__ uint32_t idesc_mx(int M, int N, uint32_t sf) {
+  return (sf << 4) | ((uint32_t)(N >> 3) << 17) | (1u << 23) | ((uint32_t)(M >> 4) << 24) | (sf << 29);
+}
+__device__ __forceinline__ void tmem_st4(uint32_t taddr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(taddr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+
 template <int EPI, int BN>
-__global__ void __launch_bounds__(GEMM_THREADS, 1)
+__global__ void __launch_bounds__(EPI >= EPI_MX ? MX_THREADS : GEMM_THREADS, 1)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                const __grid_constant__ CUtensorMap tmX, const __grid_constant__ CUtensorMap tmB2,
                const __grid_constant__ CUtensorMap tmX2, EpiArgs ep, const __grid_constant__ GemmSegs segs, int M, int N, int K,
@@ -164,6 +189,9 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   auto tfull_bar = [&](int s) { return bar0 + 8u * (2 * STAGES + s); };
   auto tempty_bar = [&](int s) { return bar0 + 8u * (2 * STAGES + 2 + s); };
   const uint32_t tmem_slot = bar0 + 8u * (2 * STAGES + 4);
+  auto sf_full = [&](int s) { return bar0 + 8u * (2 * STAGES + 5 + s); };                    // EPI_MX (leader only)
+  auto sf_empty = [&](int s) { return bar0 + 8u * (2 * STAGES + 5 + MX_SF_STAGES + s); };    // EPI_MX (both CTAs)
+  static_assert(8 * (2 * STAGES + 5 + 2 * MX_SF_STAGES) <= 256, "barrier area");
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   // CTA pairs (cluster of 2, cta_group::2): the pair computes a 256 x BN tile with ONE M = 256 MMA stream issued by
@@ -176,7 +204,11 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   // EPI_SWIGLU: a 256-wide accumulator tile is 128 output columns
   constexpr int BN_OUT = EPI == EPI_SWIGLU ? BN / 2 : BN;
   constexpr bool F8 = EPI >= EPI_F8;
-  constexpr int EPB = F8 ? EPI - EPI_F8 : EPI;   // the epilogue proper
+  constexpr bool MX = EPI >= EPI_MX;
+  constexpr int EPB = MX ? EPI - EPI_MX : (F8 ? EPI - EPI_F8 : EPI);   // the epilogue proper
+  constexpr int ACC_STRIDE = MX ? BN : BN_MAX;                         // TMEM columns between the two accumulator stages
+  constexpr uint32_t TM_SF = 2 * ACC_STRIDE;                           // EPI_MX: first scale column
+  static_assert(!MX || (BN % 32 == 0 && BN / 32 <= 8 && 2 * BN + MX_SF_STAGES * MX_SF_COLS <= 512), "MX tile width");
   constexpr int BKE = F8 ? 2 * BK : BK;          // elements per 128-byte k-block
   const int mt = (M + BM - 1) / BM, mt2 = segs.n > 0 ? segs.tile0[segs.n] : (mt + 1) >> 1;
   const int nt = (N + BN_OUT - 1) / BN_OUT, n_wide = mt2 * nt;   // tile PAIRS
@@ -240,6 +272,11 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       mbar_init(tfull_bar(s), 1);       // the leader's commit, multicast
       mbar_init(tempty_bar(s), 8);      // (leader only) 4 epilogue warps of each CTA
     }
+    if (MX)
+      for (int s = 0; s < MX_SF_STAGES; ++s) {
+        mbar_init(sf_full(s), 8);       // (leader only) 4 scale-writer warps of each CTA
+        mbar_init(sf_empty(s), 1);      // the leader's commit, multicast
+      }
     fence_barrier_init();
   }
   if (warp == 2) tmem_alloc_pair<512>(tmem_slot);
@@ -294,24 +331,85 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       const uint32_t aph = (it >> 1) & 1;
       mbar_wait_poll(tempty_bar(as), aph ^ 1);
       tc_fence_after();
-      const uint32_t d_tmem = tmem_base + as * BN_MAX;
+      const uint32_t d_tmem = tmem_base + as * ACC_STRIDE;
       const uint32_t idesc_t = (EPI == EPI_QKV_NORM_ROPE && t >= narrow_from) ? idesc_bf16(2 * BM, 128, 0, 0) : idesc;
       for (int kb = 0; kb < nkb; ++kb) {
         mbar_wait_poll(full_bar(s), ph);
+        const int gk = it * nkb + kb, ss = gk % MX_SF_STAGES;    // EPI_MX: scale stage of this k-block
+        if (MX) mbar_wait_poll(sf_full(ss), (uint32_t)(gk / MX_SF_STAGES) & 1u);
         tc_fence_after();
         if (elect_one()) {
           const uint64_t ad = desc_kmajor_sw128(smem0 + s * STAGE_BYTES);
           const uint64_t bd = desc_kmajor_sw128(smem0 + s * STAGE_BYTES + A_BYTES);
 #pragma unroll
           for (int k = 0; k < BK / 16; ++k) {   // 32 bytes of K per instruction in both kinds
-            if (F8) umma_ss_pair_f8(d_tmem, ad + 2 * k, bd + 2 * k, idesc, (kb | k) != 0);
+            if (MX) umma_mx_pair(d_tmem, ad + 2 * k, bd + 2 * k, idesc_mx(2 * BM, BN, (uint32_t)k), tmem_base + TM_SF + ss * MX_SF_COLS,
+                                 tmem_base + TM_SF + ss * MX_SF_COLS + 4, (kb | k) != 0);
+            else if (F8) umma_ss_pair_f8(d_tmem, ad + 2 * k, bd + 2 * k, idesc, (kb | k) != 0);
             else umma_ss_pair(d_tmem, ad + 2 * k, bd + 2 * k, idesc_t, (kb | k) != 0);
           }
           umma_commit_pair(empty_bar(s), (uint16_t)3);
+          if (MX) umma_commit_pair(sf_empty(ss), (uint16_t)3);
           if (kb == nkb - 1) umma_commit_pair(tfull_bar(as), (uint16_t)3);
         }
         __syncwarp();
         if (++s == STAGES) { s = 0; ph ^= 1; }
+      }
+    }
+  } else if (MX && warp >= 6) {
+    // ===================================================== EPI_MX: scale writers (TMEM lane quadrant = warp % 4)
+    const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
+    const int sf_ld = K / 32;
+    const uint32_t a_full = mapa_cluster(sf_full(0), 0);
+    int gk = 0;
+    for (int t = pair; t < n_tiles; t += n_pairs) {
+      int mp, nn, half;
+      tile_of(t, mp, nn, half);
+      const int m0 = mp * 2 * BM + rank * BM, n0 = nn * BN;
+      // One 16-byte load per row covers the scales of FOUR k-blocks; the next group's loads are in flight while this group's
+      // words go to tensor memory (a load per k-block put ~700 cycles of L2 latency on every 448-cycle k-block: 0.8 PFLOP/s).
+      constexpr int NB = BN / 32;
+      auto load_group = [&](int g, uint4 (&ra)[4], uint4 (&rb)[NB]) {
+        const uint4 one = make_uint4(0x7f7f7f7fu, 0x7f7f7f7fu, 0x7f7f7f7fu, 0x7f7f7f7fu);   // scale 1: rows past the matrix (codes 0)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const int r = m0 + lane + 32 * j;
+          ra[j] = r < M ? __ldg(reinterpret_cast<const uint4*>(ep.mx_sfa + (int64_t)r * sf_ld + g * 16)) : one;
+        }
+#pragma unroll
+        for (int j = 0; j < NB; ++j) {
+          const int r = n0 + lane + 32 * j;
+          rb[j] = r < N ? __ldg(reinterpret_cast<const uint4*>(ep.mx_sfw + (int64_t)r * sf_ld + g * 16)) : one;
+        }
+      };
+      auto word = [](const uint4& v, int q) { return q == 0 ? v.x : (q == 1 ? v.y : (q == 2 ? v.z : v.w)); };
+      uint4 ca[4], cb[NB], na[4], nb[NB];
+      load_group(0, ca, cb);
+      for (int kb0 = 0; kb0 < nkb; kb0 += 4) {
+        const bool more = kb0 + 4 < nkb;
+        if (more) load_group(kb0 / 4 + 1, na, nb);
+#pragma unroll
+        for (int q = 0; q < 4; ++q, ++gk) {
+          const int ss = gk % MX_SF_STAGES;
+          mbar_wait_poll(sf_empty(ss), (uint32_t)((gk / MX_SF_STAGES) & 1) ^ 1u);
+          tc_fence_after();
+          const uint32_t ta = tmem_base + TM_SF + ss * MX_SF_COLS + lane_off;
+          tmem_st4(ta, word(ca[0], q), word(ca[1], q), word(ca[2], q), word(ca[3], q));
+          tmem_st4(ta + 4u, word(cb[0], q), word(cb[1], q), word(cb[2], q), word(cb[3], q));
+          tmem_st4(ta + 8u, NB > 4 ? word(cb[NB > 4 ? 4 : 0], q) : 0u, NB > 5 ? word(cb[NB > 5 ? 5 : 0], q) : 0u,
+                   NB > 6 ? word(cb[NB > 6 ? 6 : 0], q) : 0u, NB > 7 ? word(cb[NB > 7 ? 7 : 0], q) : 0u);
+          tmem_st_wait();
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0)   // tensor-memory writes are ordered by wait::st + the fence: the barrier carries the event only
+            asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(a_full + 8u * ss) : "memory");
+        }
+        if (more) {
+#pragma unroll
+          for (int j = 0; j < 4; ++j) ca[j] = na[j];
+#pragma unroll
+          for (int j = 0; j < NB; ++j) cb[j] = nb[j];
+        }
       }
     }
   } else {
@@ -362,7 +460,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         }
       }
       float a_scale = 1.0f;
-      if (F8) {   // s_gate = the tile's W row scales; this thread's A row scale
+      if (F8 && !MX) {   // s_gate = the tile's W row scales; this thread's A row scale
         for (int i = et; i < BN; i += EPI_THREADS) s_gate[i] = (n0 + i < N) ? ep.w_scale[n0 + i] : 0.f;
         a_scale = row_ok ? ep.a_scale[row] : 0.f;
       }
@@ -384,7 +482,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       const uint32_t stg = stg0 + (uint32_t)quad * STG_WARP_BYTES;
       mbar_wait_poll(tfull_bar(as), aph);
       tc_fence_after();
-      const uint32_t t_addr = tmem_base + as * BN_MAX + ((uint32_t)(quad * 32) << 16);
+      const uint32_t t_addr = tmem_base + as * ACC_STRIDE + ((uint32_t)(quad * 32) << 16);
       if (EPI == EPI_QKV_NORM_ROPE) {
         // QKV projection with QK-RMSNorm (R5) and RoPE (R6) applied to the fp32 accumulators before the one and
         // only bf16 rounding: per 128-column head, pass 1 reads the accumulator row for sum(q^2), pass 2 reads it
@@ -523,7 +621,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
           ld8<float>(s_bias + c * 32 + g * 8, b);
 #pragma unroll
           for (int e = 0; e < 8; ++e) {
-            if (F8) v[e] = fmaf(__uint_as_float(r[g * 8 + e]), a_scale * s_gate[c * 32 + g * 8 + e], b[e]);
+            if (F8 && !MX) v[e] = fmaf(__uint_as_float(r[g * 8 + e]), a_scale * s_gate[c * 32 + g * 8 + e], b[e]);
             else v[e] = __uint_as_float(r[g * 8 + e]) + b[e];
           }
           if (EPB == DIT_EPI_BIAS_GELU) {
@@ -617,7 +715,8 @@ dit_status launch_t(const CUtensorMap& ta, const CUtensorMap& tb, const CUtensor
   const int n_wide = mt2 * cdiv(N, EPI == EPI_SWIGLU ? BN / 2 : BN);
   const int pairs = (EPI == EPI_QKV_NORM_ROPE && ep.narrow_from >= 0) ? ep.narrow_from + 2 * (n_wide - ep.narrow_from) : n_wide;
   const int max_pairs = sm_count() / 2;
-  DIT_CUDA_OK(launch_pdl(gemm_tc_kernel<EPI, BN>, dim3(2 * (pairs < max_pairs ? pairs : max_pairs)), dim3(GEMM_THREADS),
+  DIT_CUDA_OK(launch_pdl(gemm_tc_kernel<EPI, BN>, dim3(2 * (pairs < max_pairs ? pairs : max_pairs)),
+                         dim3(EPI >= EPI_MX ? MX_THREADS : GEMM_THREADS),
                          smem_bytes(BN, EPI), st, 2, ta, tb, tx, sl != nullptr ? *sl->tb2 : tb, sl != nullptr ? *sl->tx2 : tx, ep,
                          sl != nullptr ? *sl->segs : no_segs(), M, N, K, group_rows(mt2 * 2 * BM, K), k_wrap));
   DIT_LAUNCH_CHECK();
@@ -788,6 +887,28 @@ dit_status launch_gemm_tc_fp8(int epi, const void* Aq, int64_t lda, const float*
     case DIT_EPI_BIAS_GELU: return launch_bn<EPI_F8 + DIT_EPI_BIAS_GELU>(bn, ta, tb, ta, ep, M, N, K, st, 0);
     case DIT_EPI_BIAS_F32: return launch_bn<EPI_F8 + DIT_EPI_BIAS_F32>(bn, ta, tb, ta, ep, M, N, K, st, 0);
     default: DIT_REQUIRE(false, DIT_ERR_INVALID_ARG, "gemm_tc_fp8: epilogue %d", epi);
+  }
+}
+
+// Block-scaled MXFP8 layer on the pair kernel (R43): Aq [M, lda], Wq [N, K] e4m3 bytes; sfa [M, K / 32], sfw [N, K / 32] E8M0.
+dit_status launch_gemm_tc_mx(int epi, const void* Aq, int64_t lda, const void* sfa, const void* Wq, const void* sfw, const void* bias,
+                             void* out, int64_t ldo, int M, int N, int K, cudaStream_t st) {
+  if (M == 0 || N == 0) return DIT_OK;
+  DIT_REQUIRE(K > 0 && K % 512 == 0 && lda % 16 == 0 && N % 8 == 0 && ldo % 8 == 0, DIT_ERR_UNSUPPORTED,
+              "gemm_tc_mx: K (%d) must be a multiple of 512, lda (%lld) of 16, N (%d) and ldo (%lld) of 8", K, (long long)lda, N, (long long)ldo);
+  constexpr int BNX = 224;
+  CUtensorMap ta, tb;
+  DIT_REQUIRE(make_tmap_2d_u8(&ta, Aq, M, K, lda, BM) && make_tmap_2d_u8(&tb, Wq, N, K, K, BNX / 2), DIT_ERR_CUDA,
+              "gemm_tc_mx: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d lda=%lld)", M, N, K, (long long)lda);
+  EpiArgs ep{};
+  ep.bias = (const bf16*)bias; ep.out = out; ep.ldo = ldo; ep.R = 1; ep.narrow_from = -1;
+  ep.mx_sfa = (const uint8_t*)sfa; ep.mx_sfw = (const uint8_t*)sfw;
+  ProfScope _prof(DIT_KC_GEMM, st);
+  switch (epi) {
+    case DIT_EPI_BIAS: return launch_t<EPI_MX + DIT_EPI_BIAS, BNX>(ta, tb, ta, ep, M, N, K, st, 0);
+    case DIT_EPI_BIAS_GELU: return launch_t<EPI_MX + DIT_EPI_BIAS_GELU, BNX>(ta, tb, ta, ep, M, N, K, st, 0);
+    case DIT_EPI_BIAS_F32: return launch_t<EPI_MX + DIT_EPI_BIAS_F32, BNX>(ta, tb, ta, ep, M, N, K, st, 0);
+    default: DIT_REQUIRE(false, DIT_ERR_INVALID_ARG, "gemm_tc_mx: epilogue %d", epi);
   }
 }
 

@@ -278,6 +278,11 @@ dit_status dit_linear_mxfp8(int32_t epilogue, const void* Aq, int64_t lda, const
   DIT_REQUIRE(!(((uintptr_t)Aq | (uintptr_t)Wq | (uintptr_t)out) & 15) && !(((uintptr_t)a_scales | (uintptr_t)w_scales) & 3), DIT_ERR_UNSUPPORTED,
               "dit_linear_mxfp8: operands 16-byte, scales 4-byte aligned");
   DIT_REQUIRE(encode_tiled_fn() != nullptr, DIT_ERR_UNSUPPORTED, "dit_linear_mxfp8: cuTensorMapEncodeTiled unavailable");
+  // default: the persistent CTA-pair kernel of gemm_tc.cu (EPI_MX); DIT_MX_KERNEL=simple selects the 1-CTA kernel of this file
+  static const bool simple = []() { const char* e = getenv("DIT_MX_KERNEL"); return e != nullptr && e[0] == 's'; }();
+  // (the pair kernel loads the scales of four k-blocks with one 16-byte load: K % 512 == 0 and 16-byte aligned scale rows)
+  if (!simple && K % 512 == 0 && !(((uintptr_t)a_scales | (uintptr_t)w_scales) & 15))
+    return launch_gemm_tc_mx(epilogue, Aq, lda, a_scales, Wq, w_scales, bias, out, ldo, M, N, K, (cudaStream_t)stream);
   CUtensorMap ta, tb;
   DIT_REQUIRE(make_tmap_2d_u8(&ta, Aq, M, K, lda, MT) && make_tmap_2d_u8(&tb, Wq, N, K, K, NT), DIT_ERR_CUDA,
               "dit_linear_mxfp8: cuTensorMapEncodeTiled failed (M=%d N=%d K=%d)", M, N, K);

@@ -68,10 +68,10 @@ def test_linear_mx_against_oracle_on_the_same_codes(lib, M, N, K, epi):
         check_rounding(got, ref, f"linear_mx {M}x{N}x{K}")
 
 
-def test_linear_mx_scales_are_applied_per_block_and_per_row(lib):
+@pytest.mark.parametrize("M,N,K", [(256, 256, 512), (300, 520, 384), (600, 456, 1024)])   # K % 512 == 0: the CTA-pair kernel
+def test_linear_mx_scales_are_applied_per_block_and_per_row(lib, M, N, K):
     """A wrong scale layout in tensor memory (row group, K slice or operand swapped) cannot pass: every (row, block) of A and of
     W gets its own power-of-two scale while all codes are the SAME constant, so out[m, n] = c^2 32 sum_b Xa[m, b] Xw[n, b]."""
-    M, N, K = 256, 256, 512
     code_one = 0x38                                                      # e4m3 1.0
     Aq = torch.full((M, K), code_one, dtype=torch.uint8, device=DEV)
     Wq = torch.full((N, K), code_one, dtype=torch.uint8, device=DEV)
