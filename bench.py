@@ -145,6 +145,15 @@ class ClockSampler:
                 "reasons": sorted(reasons)}
 
 
+def _driver_version(gpu_index: int):
+    try:
+        r = subprocess.run(["nvidia-smi", "-i", str(gpu_index), "--query-gpu=driver_version", "--format=csv,noheader"],
+                           capture_output=True, text=True, timeout=10)
+        return r.stdout.strip().splitlines()[0] if r.returncode == 0 and r.stdout.strip() else None
+    except (OSError, subprocess.TimeoutExpired):
+        return None
+
+
 def _gpu_index(local_rank: int) -> int:
     vis = os.environ.get("CUDA_VISIBLE_DEVICES")
     if vis:
@@ -420,7 +429,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
             "config": bench_config(s, wl_name, args.split_p, req_per_gpu, world),
             "clocks": clocks,
             "device": {"name": torch.cuda.get_device_name(dev), "sms": torch.cuda.get_device_properties(dev).multi_processor_count,
-                       "torch": torch.__version__, "cuda": torch.version.cuda, "peaks": pk,
+                       "torch": torch.__version__, "cuda": torch.version.cuda, "driver": _driver_version(_gpu_index(local_rank)), "peaks": pk,
                        "timing": f"{K} back-to-back steps after {Wm} warm-ups, CUDA events, no per-launch instrumentation"},
             "e2e": {"value": job_throughput(world, K, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "call": "dit_step_varlen_host" if args.workload == "cfg4" else "dit_step_host"},
