@@ -524,9 +524,26 @@ def run_traj(args):
                      "model_passes_per_s": (2 if u is not None else 1) * n / (ms * 1e-3),
                      "host_enqueue_ms_per_trajectory": t_enq / K * 1e3,
                      "library_launch_calls_per_trajectory": (B.dit_kernel_launches() - n0) / K})
+    # ONE step per C-ABI call (what the headline bench times), launched kernel by kernel and replayed from the graph the
+    # handle caches (dit_step_graph): device time per step and what the call costs the calling thread
+    single = []
+    for name, fn in (("dit_step", m1.dit_step), ("dit_step_graph", m1.dit_step_graph)):
+        for _ in range(3):
+            fn(lat, tembs[0], cond, out=out)
+        torch.cuda.synchronize()
+        reps = 8                                          # 8 x 65 launches stay below the driver's launch queue depth: no back-pressure in the host time
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0 = time.perf_counter()
+        e0.record()
+        for _ in range(reps):
+            fn(lat, tembs[0], cond, out=out)
+        t_enq = time.perf_counter() - t0
+        e1.record()
+        torch.cuda.synchronize()
+        single.append({"call": name, "ms_per_step": e0.elapsed_time(e1) / reps, "host_enqueue_us_per_step": t_enq / reps * 1e6})
     print(json.dumps({"metric": "trajectory denoising steps/s", "unit": UNIT, "n_gpus": 1, "trajectories": K, "warmup": Wm,
                       "config": {"workload": _workload_name(s), "traj_steps": n, "split_p": args.split_p}, "dtype": "bf16",
-                      "data": "synthetic", "rows": rows}), flush=True)
+                      "data": "synthetic", "rows": rows, "single_step": single}), flush=True)
 
 
 # --------------------------------------------------------------------------------------------------------

@@ -149,6 +149,18 @@ dit_status dit_sample(dit_handle h, const void* latents, const float* timestep_e
                       float guidance_scale, const int32_t latent_grid[3], int32_t n_steps, int32_t use_graph, void* out,
                       void* stream);
 
+/* dit_step / dit_step_varlen replayed from a CUDA graph: ONE cudaGraphLaunch instead of 65+ kernel launches (host cost of a
+ * step ~0.4 ms -> ~10 us; the paper's control plane dispatches a request one denoising step at a time).  Same
+ * arguments and result (bit-identical).  The graph holds every pointer and the geometry: a call whose arguments equal those
+ * of a cached graph replays it (the CONTENTS of the buffers may have changed), any other call captures a new one; a handle
+ * keeps the 8 most recently used graphs.  Falls back to plain launches while dit_profile_begin or a debug stop is active.
+ * The first call for a set of arguments costs a capture + instantiation (milliseconds). */
+dit_status dit_step_graph(dit_handle h, const void* latents, const float* timestep_emb, const void* cond_tokens, int32_t n_cond,
+                          const int32_t latent_grid[3], void* out, void* stream);
+dit_status dit_step_varlen_graph(dit_handle h, const void* latents_packed, const float* timestep_emb, const void* cond_packed,
+                                 const int32_t* cu_seqlens, const int32_t* n_cond, const int32_t* latent_grids, int32_t n_requests,
+                                 void* out_packed, void* stream);
+
 /* Same computation with HOST buffers (pageable or pinned): H2D copies of latents / timestep_emb / cond, the step, and the
  * D2H copy of `out`; staging lives in the workspace.  Everything is ordered with respect to `stream`: the latent / cond
  * uploads run on a copy stream of the handle that first waits for all work already enqueued on `stream` and is joined back

@@ -18,7 +18,7 @@ EPI_BIAS, EPI_BIAS_GELU, EPI_BIAS_F32 = 0, 1, 2
 TAP = dict(x=0, y=1, qkv=2, o=3, u=5, c=6, mod=7, tok=8)
 STAGE = dict(y1=0, qkv=1, attn=2, oproj=3, cross=4, y2=5, fc1=6, fc2=7)
 
-SYMBOLS = ["dit_workspace_bytes", "dit_init", "dit_step", "dit_step_host", "dit_step_varlen", "dit_step_varlen_host", "dit_sample", "dit_attn_partial",
+SYMBOLS = ["dit_workspace_bytes", "dit_init", "dit_step", "dit_step_host", "dit_step_varlen", "dit_step_varlen_host", "dit_step_graph", "dit_step_varlen_graph", "dit_sample", "dit_attn_partial",
            "dit_attn_merge", "dit_static_scratch_bytes", "dit_attn_split_static", "dit_relayout_plan", "dit_relayout", "dit_linear", "dit_linear_swiglu", "dit_quantize_fp8", "dit_linear_fp8", "dit_quantize_mxfp8", "dit_linear_mxfp8", "dit_linear_residual", "dit_linear_qkv", "dit_adaln", "dit_gemv", "dit_qknorm_rope", "dit_debug_stop_after",
            "dit_get_tap", "dit_profile_begin", "dit_profile_end", "dit_last_error", "dit_kernel_launches", "dit_fallback_launches", "dit_sim_run",
            "dit_free"]
@@ -101,6 +101,8 @@ def load(path: str = LIB_PATH):
         "dit_init": [C.POINTER(dit_config), C.POINTER(dit_weight), i32, vp, C.c_size_t, C.POINTER(vp)],
         "dit_step": [vp, vp, vp, vp, i32, pi32, vp, vp],
         "dit_step_host": [vp, vp, vp, vp, i32, pi32, vp, vp],
+        "dit_step_graph": [vp, vp, vp, vp, i32, pi32, vp, vp],
+        "dit_step_varlen_graph": [vp, vp, vp, vp, pi32, pi32, pi32, i32, vp, vp],
         "dit_step_varlen": [vp, vp, vp, vp, pi32, pi32, pi32, i32, vp, vp],
         "dit_step_varlen_host": [vp, vp, vp, vp, pi32, pi32, pi32, i32, vp, vp],
         "dit_sample": [vp, vp, vp, C.POINTER(C.c_float), vp, i32, vp, i32, f32, pi32, i32, i32, vp, vp],
@@ -215,6 +217,23 @@ class Dit:
         n_cond = 0 if cond is None else cond.shape[0]
         _check(self.lib.dit_step(self.handle, _ptr(latents), _ptr(temb), _ptr(cond), n_cond, grid, _ptr(out),
                                  _stream(stream)), "dit_step")
+        return out
+
+    def dit_step_graph(self, latents, temb, cond=None, out=None, stream=None):
+        """dit_step replayed from a CUDA graph cached in the handle (key: the pointers and the geometry)."""
+        out = torch.empty_like(latents) if out is None else out
+        grid = _i32arr(latents.shape[1:])
+        n_cond = 0 if cond is None else cond.shape[0]
+        _check(self.lib.dit_step_graph(self.handle, _ptr(latents), _ptr(temb), _ptr(cond), n_cond, grid, _ptr(out),
+                                       _stream(stream)), "dit_step_graph")
+        return out
+
+    def dit_step_varlen_graph(self, packed, shapes, temb, cond, n_cond, out, stream=None):
+        """Packed step replayed from a CUDA graph: packed = the R latents back to back (1-D, device), shapes their
+        [C,F_r,H_r,W_r] shapes, temb [R, temb_dim], cond [sum n_cond, cond_dim] or None, out like packed."""
+        cu, grids = self._varlen_geom(shapes, n_cond)
+        _check(self.lib.dit_step_varlen_graph(self.handle, _ptr(packed), _ptr(temb), _ptr(cond), _i32arr(cu), _i32arr(n_cond),
+                                              _i32arr(grids), len(shapes), _ptr(out), _stream(stream)), "dit_step_varlen_graph")
         return out
 
     def dit_sample(self, latents, tembs, sigmas, cond=None, uncond=None, guidance_scale=1.0, use_graph=False, out=None,

@@ -115,7 +115,11 @@ struct dit_handle_s {
   // geometry resident on the device (cu_seqlens, cond offsets, per-request meta, RoPE tables): uploads are skipped
   // when a call's geometry equals it in EVERY field
   std::vector<int32_t> last_geom;
-  bool capturing = false;              // inside dit_sample's stream capture: no host -> device copy may be enqueued
+  bool capturing = false;              // inside a stream capture: no host -> device copy may be enqueued
+  // dit_step_graph / dit_step_varlen_graph: up to 8 captured steps, least recently used replaced
+  struct StepGraph { std::vector<uint64_t> key; cudaGraphExec_t exec; uint64_t used; };
+  std::vector<StepGraph> step_graphs;
+  uint64_t step_graph_clock = 0;
   // dit_sample: one cached trajectory graph, valid while every argument (and sigma) it was captured with is unchanged
   cudaGraphExec_t graph_exec = nullptr;
   // dit_step_host / dit_step_varlen_host: the latent / cond uploads run on this stream while the caller's stream computes the
@@ -820,6 +824,70 @@ dit_status dit_step(dit_handle h, const void* latents, const float* timestep_emb
   return dit_step_varlen(h, latents, timestep_emb, cond_tokens, nullptr, &n_cond, latent_grid, 1, out, stream);
 }
 
+// The step as ONE cudaGraphLaunch: the paper's control plane dispatches a request one denoising step at a time,
+// and a step is 65+ kernel launches (~0.4 ms of host time at 6 us each; a 512^2 request's step is 2.4 ms of GPU time).  The
+// captured graph holds every pointer and the geometry: it is replayed while the call's arguments are the same (buffer CONTENTS
+// may change), else captured again; the handle keeps the 8 most recently used graphs.
+dit_status dit_step_varlen_graph(dit_handle h, const void* latents_packed, const float* timestep_emb, const void* cond_packed,
+                                 const int32_t* cu_seqlens, const int32_t* n_cond, const int32_t* latent_grids, int32_t n_requests,
+                                 void* out_packed, void* stream) {
+  DIT_REQUIRE(h != nullptr, DIT_ERR_INVALID_ARG, "handle is NULL");
+  DIT_REQUIRE(latents_packed && timestep_emb && latent_grids && out_packed, DIT_ERR_INVALID_ARG, "NULL tensor argument");
+  StepGeom g;
+  dit_status s = build_geom(h, n_requests, cu_seqlens, n_cond, latent_grids, &g);
+  if (s != DIT_OK) return s;
+  DIT_REQUIRE(g.cu_cond[n_requests] == 0 || cond_packed != nullptr, DIT_ERR_INVALID_ARG, "cond tokens announced but cond pointer is NULL");
+  cudaStream_t st = (cudaStream_t)stream;
+  // no graph while per-class profiling is on (event records are not captured) or a debug stop is set
+  if (g_prof_mask.load() != 0 || h->stop_block >= 0) return run_step(h, g, latents_packed, timestep_emb, cond_packed, out_packed, st);
+  std::vector<uint64_t> key = {(uint64_t)(uintptr_t)latents_packed, (uint64_t)(uintptr_t)timestep_emb, (uint64_t)(uintptr_t)cond_packed,
+                               (uint64_t)(uintptr_t)out_packed, (uint64_t)n_requests};
+  for (int r = 0; r < n_requests; ++r) {
+    key.push_back((uint64_t)g.cu[r + 1]);
+    key.push_back((uint64_t)g.ncond[r]);
+    for (int a = 0; a < 3; ++a) key.push_back((uint64_t)latent_grids[3 * r + a]);
+  }
+  // geometry copies and the RoPE table are not part of the graph: enqueued ahead of the capture or the replay whenever another
+  // call has left a different geometry on the device (else a no-op)
+  s = upload_geom(h, g, st);
+  if (s != DIT_OK) return s;
+  dit_handle_s::StepGraph* hit = nullptr;
+  for (auto& sg : h->step_graphs)
+    if (sg.key == key) hit = &sg;
+  if (hit == nullptr) {
+    if (h->cap_stream == nullptr) DIT_CUDA_OK(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
+    DIT_CUDA_OK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeRelaxed));
+    h->capturing = true;
+    s = run_step(h, g, latents_packed, timestep_emb, cond_packed, out_packed, h->cap_stream);
+    h->capturing = false;
+    cudaGraph_t graph = nullptr;
+    cudaError_t ce = cudaStreamEndCapture(h->cap_stream, &graph);
+    if (s != DIT_OK) { if (graph) cudaGraphDestroy(graph); return s; }
+    DIT_REQUIRE(ce == cudaSuccess && graph != nullptr, DIT_ERR_CUDA, "dit_step_graph: stream capture failed: %s", cudaGetErrorString(ce));
+    cudaGraphExec_t exec = nullptr;
+    ce = cudaGraphInstantiate(&exec, graph, 0);
+    cudaGraphDestroy(graph);
+    DIT_REQUIRE(ce == cudaSuccess, DIT_ERR_CUDA, "dit_step_graph: cudaGraphInstantiate failed: %s", cudaGetErrorString(ce));
+    if (h->step_graphs.size() >= 8) {   // replace the least recently used graph
+      size_t lru = 0;
+      for (size_t i = 1; i < h->step_graphs.size(); ++i)
+        if (h->step_graphs[i].used < h->step_graphs[lru].used) lru = i;
+      cudaGraphExecDestroy(h->step_graphs[lru].exec);
+      h->step_graphs.erase(h->step_graphs.begin() + lru);
+    }
+    h->step_graphs.push_back({key, exec, 0});
+    hit = &h->step_graphs.back();
+  }
+  hit->used = ++h->step_graph_clock;
+  DIT_CUDA_OK(cudaGraphLaunch(hit->exec, st));
+  return DIT_OK;
+}
+
+dit_status dit_step_graph(dit_handle h, const void* latents, const float* timestep_emb, const void* cond_tokens, int32_t n_cond,
+                          const int32_t latent_grid[3], void* out, void* stream) {
+  return dit_step_varlen_graph(h, latents, timestep_emb, cond_tokens, nullptr, &n_cond, latent_grid, 1, out, stream);
+}
+
 }  // extern "C"
 
 // Host-buffer steps: temb goes up on the caller's stream; latents and cond tokens go up on the handle's copy stream, which
@@ -1181,6 +1249,7 @@ int32_t dit_fallback_launches(void) { return g_fallback_launches.load(); }
 void dit_free(dit_handle h) {
   if (!h) return;
   if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
+  for (auto& sg : h->step_graphs) cudaGraphExecDestroy(sg.exec);
   if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
   if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
   if (h->ev_fork) cudaEventDestroy(h->ev_fork);

@@ -362,6 +362,73 @@ def test_sixty_four_tiny_requests_packed(lib, mode):
         check(outs[r], ref, torch.bfloat16, f"64 packed requests ({mode}), request {r}")
 
 
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+def test_step_graph_replay_is_bit_identical(lib, dtype):
+    """dit_step_graph: one cudaGraphLaunch per step.  Bit-identical to dit_step; a replay sees NEW buffer contents (the graph
+    holds pointers, not values); other pointers / geometry capture another graph; more than 8 argument sets evict the least
+    recently used graph and everything still matches."""
+    s = synth.cfg1(cond_mode="joint", rope_dims=(0, 32, 32), qk_rmsnorm=True) if dtype == "f32" else _small_bf16(cond_mode="joint")
+    W, I = synth.make_weights(s), synth.make_inputs(s)
+    m = B.Dit(B.make_config(s), W, DEV)
+    lat, temb, cond = _gpu_inputs(s, I)
+    ref = m.dit_step(lat, temb, cond).clone()
+    out = torch.empty_like(lat)
+    n0 = B.dit_kernel_launches()
+    m.dit_step_graph(lat, temb, cond, out)                      # capture + launch
+    torch.cuda.synchronize()
+    assert torch.equal(out, ref)
+    out.zero_()
+    m.dit_step_graph(lat, temb, cond, out)                      # replay
+    torch.cuda.synchronize()
+    assert torch.equal(out, ref)
+    # new contents in the same buffers
+    I2 = synth.make_inputs(s, tag="other", t=123.0)
+    lat.copy_(I2["latents"].to(DEV)); temb.copy_(I2["temb"][0].to(DEV)); cond.copy_(I2["cond"].to(DEV))
+    ref2 = m.dit_step(lat, temb, cond).clone()
+    m.dit_step_graph(lat, temb, cond, out)
+    torch.cuda.synchronize()
+    assert torch.equal(out, ref2) and not torch.equal(ref2, ref)
+    # other geometry (fewer cond tokens) and ten different output buffers: captures, evictions, replays
+    refc = m.dit_step(lat, temb, cond[:7]).clone()
+    outs = [torch.empty_like(lat) for _ in range(10)]
+    for rep in range(2):
+        for o in outs:
+            o.zero_()
+            m.dit_step_graph(lat, temb, cond[:7], o)
+        torch.cuda.synchronize()
+        assert all(torch.equal(o, refc) for o in outs)
+    m.dit_step_graph(lat, temb, cond, out)
+    torch.cuda.synchronize()
+    assert torch.equal(out, ref2)
+    # a debug stop bypasses the graph
+    m.dit_debug_stop_after(0, "y1")
+    m.dit_step_graph(lat, temb, cond, out)
+    m.dit_debug_stop_after(-1, 0)
+    m.dit_step_graph(lat, temb, cond, out)
+    torch.cuda.synchronize()
+    assert torch.equal(out, ref2)
+
+
+def test_step_varlen_graph_matches_varlen(lib):
+    grids, nconds = [(1, 12, 20), (1, 36, 44), (1, 4, 4)], [9, 70, 3]
+    shapes = [_small_bf16(cond_mode="joint", latent_grid=g, n_cond=n) for g, n in zip(grids, nconds)]
+    W = synth.make_weights(shapes[0])
+    Is = [synth.make_inputs(sh, tag=f"g{r}", t=150.0 + 250 * r) for r, sh in enumerate(shapes)]
+    T_total = sum(sh.n_tokens + n for sh, n in zip(shapes, nconds))
+    m = B.Dit(B.make_config(shapes[0], max_tokens=T_total, max_requests=3, max_cond_tokens=sum(nconds)), W, DEV)
+    lats = [i["latents"].to(DEV) for i in Is]
+    temb = torch.cat([i["temb"] for i in Is]).to(DEV)
+    conds = [i["cond"].to(DEV) for i in Is]
+    want = torch.cat([o.reshape(-1) for o in m.dit_step_varlen(lats, temb, conds)])
+    packed, cond = torch.cat([l.reshape(-1) for l in lats]), torch.cat(conds)
+    out = torch.empty_like(packed)
+    for _ in range(3):
+        out.zero_()
+        m.dit_step_varlen_graph(packed, [tuple(l.shape) for l in lats], temb, cond, nconds, out)
+        torch.cuda.synchronize()
+        assert torch.equal(out, want)
+
+
 def test_argument_validation_on_gpu(lib):
     s = synth.cfg1()
     W, I = synth.make_weights(s), synth.make_inputs(s)
