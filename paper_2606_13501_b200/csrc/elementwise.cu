@@ -1,7 +1,12 @@
 // elementwise.cu — the HBM-bound kernels of the DiT step: weight-streaming GEMV (t-MLP, modulation),
 // adaLN-Zero modulation (LayerNorm + shift/scale + gated residual), QK-RMSNorm + RoPE, RoPE tables,
 // patchify / unpatchify, LSE merge.  All 128-bit coalesced global access, warp-shuffle reductions.
+#include <algorithm>
+#include <cstdlib>
+#include <cstring>
+
 #include "common.cuh"
+#include "tc.cuh"   // mbarrier helpers (adaln_stream_kernel)
 
 namespace dit {
 
@@ -239,6 +244,156 @@ __global__ void __launch_bounds__(128) adaln_kernel(float* __restrict__ x, const
   }
 }
 
+// -------------------------------------------------------------------------------------------------
+// The same operation (without the h / gate residual) for launches of a few waves: a PERSISTENT grid (resident CTAs only),
+// every CTA walks rows b, b + G, b + 2G ... and keeps STAGES rows in flight in shared memory with 1-D bulk copies
+// (cp.async.bulk + mbarrier): the bytes in flight per SM no longer depend on registers or on how many CTAs have been
+// launched yet, and there is no wave tail — at cfg 2 (4352 rows of 12 KB) the one-row-per-CTA kernel above is 3.3 waves of
+// load -> reduce -> load modulation -> store chains.  128 threads per row, NCT = D / 1024 chunks of 8 per thread; the
+// modulation rows stay in registers and are reloaded only when the request (segment) changes.
+// -------------------------------------------------------------------------------------------------
+constexpr int ADALN_STAGES = 3;
+
+__device__ __forceinline__ void bulk_load_1d(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src),
+               "r"(bytes), "r"(bar)
+               : "memory");
+}
+
+template <typename T, int NCT>
+__global__ void __launch_bounds__(128) adaln_stream_kernel(const float* __restrict__ x, const float* __restrict__ shift,
+                                                           const float* __restrict__ scale, int64_t mod_stride,
+                                                           const int32_t* __restrict__ cu, int R, T* __restrict__ y,
+                                                           int T_rows, float eps, int split, int64_t set_off) {
+  constexpr int D = NCT * 1024;
+  extern __shared__ __align__(128) unsigned char adaln_smem[];
+  float* stage = reinterpret_cast<float*>(adaln_smem);                       // [STAGES][D]
+  __shared__ __align__(8) uint64_t full[ADALN_STAGES];
+  __shared__ float red[2][4];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int G = gridDim.x, b = blockIdx.x;
+  const int n_my = b < T_rows ? (T_rows - b + G - 1) / G : 0;
+  if (tid == 0) {
+    for (int s = 0; s < ADALN_STAGES; ++s) tc::mbar_init(tc::smem_u32(&full[s]), 1);
+    tc::fence_barrier_init();
+  }
+  pdl_trigger();
+  pdl_wait();                                                                 // x and the modulation rows come from earlier kernels
+  if (tid == 0) {
+    for (int s = 0; s < ADALN_STAGES && s < n_my; ++s) {
+      tc::mbar_expect_tx(tc::smem_u32(&full[s]), D * 4);
+      bulk_load_1d(tc::smem_u32(stage + (size_t)s * D), x + (int64_t)(b + s * G) * D, D * 4, tc::smem_u32(&full[s]));
+    }
+  }
+  __syncthreads();                                                            // barrier init visible to the waiting threads
+  const int col0 = tid * 8;                                                   // chunk c of this thread starts at col0 + c * 1024
+  float a[NCT][8], sft[NCT][8];
+  int64_t cur = -1;
+  for (int i = 0; i < n_my; ++i) {
+    const int s = i % ADALN_STAGES;
+    const uint32_t ph = (uint32_t)(i / ADALN_STAGES) & 1u;
+    const int row = b + i * G;
+    const int seg = (cu != nullptr && R > 1) ? find_request(cu, R, row) : 0;
+    const int64_t moff = set_off != 0 ? (int64_t)(seg >> 1) * mod_stride + ((seg & 1) ? 0 : set_off) : (int64_t)seg * mod_stride;
+    if (moff != cur) {                                                        // uniform over the CTA
+      cur = moff;
+#pragma unroll
+      for (int c = 0; c < NCT; ++c) {
+        if (scale) ld8<float>(scale + moff + col0 + c * 1024, a[c]);
+        if (shift) ld8<float>(shift + moff + col0 + c * 1024, sft[c]);
+      }
+    }
+    tc::mbar_wait(tc::smem_u32(&full[s]), ph);
+    const float* xs = stage + (size_t)s * D + col0;
+    float v[NCT][8];
+#pragma unroll
+    for (int c = 0; c < NCT; ++c) {
+      const float4 lo = *reinterpret_cast<const float4*>(xs + c * 1024), hi = *reinterpret_cast<const float4*>(xs + c * 1024 + 4);
+      v[c][0] = lo.x; v[c][1] = lo.y; v[c][2] = lo.z; v[c][3] = lo.w;
+      v[c][4] = hi.x; v[c][5] = hi.y; v[c][6] = hi.z; v[c][7] = hi.w;
+    }
+    float sum = 0.f;
+#pragma unroll
+    for (int c = 0; c < NCT; ++c)
+#pragma unroll
+      for (int e = 0; e < 8; ++e) sum += v[c][e];
+    sum = warp_sum(sum);
+    if (lane == 0) red[0][warp] = sum;
+    __syncthreads();                                                          // also: every thread has read stage s
+    if (tid == 0 && i + ADALN_STAGES < n_my) {
+      tc::mbar_expect_tx(tc::smem_u32(&full[s]), D * 4);
+      bulk_load_1d(tc::smem_u32(stage + (size_t)s * D), x + (int64_t)(b + (i + ADALN_STAGES) * G) * D, D * 4,
+                   tc::smem_u32(&full[s]));
+    }
+    const float mean = (red[0][0] + red[0][1] + red[0][2] + red[0][3]) * (1.0f / D);
+    float q = 0.f;
+#pragma unroll
+    for (int c = 0; c < NCT; ++c)
+#pragma unroll
+      for (int e = 0; e < 8; ++e) {
+        float dlt = v[c][e] - mean;
+        q = fmaf(dlt, dlt, q);
+      }
+    q = warp_sum(q);
+    if (lane == 0) red[1][warp] = q;
+    __syncthreads();
+    const float rstd = rsqrtf((red[1][0] + red[1][1] + red[1][2] + red[1][3]) * (1.0f / D) + eps);
+    T* yr = y + (int64_t)row * (split ? 2 * D : D) + col0;
+#pragma unroll
+    for (int c = 0; c < NCT; ++c) {
+      float o[8];
+#pragma unroll
+      for (int e = 0; e < 8; ++e) {
+        float n = (v[c][e] - mean) * rstd;
+        if (scale) n = fmaf(n, a[c][e], n);
+        if (shift) n += sft[c][e];
+        o[e] = n;
+      }
+      st8<T>(yr + c * 1024, o);
+      if (split) {
+        float lo[8];
+#pragma unroll
+        for (int e = 0; e < 8; ++e) lo[e] = o[e] - to_f<T>(from_f<T>(o[e]));
+        st8<T>(yr + D + c * 1024, lo);
+      }
+    }
+  }
+}
+
+template <typename T, int NCT>
+static cudaError_t launch_adaln_stream(const float* x, const float* shift, const float* scale, int64_t mod_stride,
+                                       const int32_t* cu, int R, T* y, int T_rows, float eps, cudaStream_t st, int split,
+                                       int64_t set_off) {
+  constexpr int smem = ADALN_STAGES * NCT * 1024 * 4;
+  static int ctas_per_sm[16] = {0};                 // per device: resident CTAs of this instantiation x SMs (0 = not asked yet)
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev >= 16) return cudaErrorInvalidDevice;
+  if (ctas_per_sm[dev] == 0) {
+    e = cudaFuncSetAttribute(adaln_stream_kernel<T, NCT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    int n = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, adaln_stream_kernel<T, NCT>, 128, smem);
+    if (e != cudaSuccess) return e;
+    int sms = 148;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return e;
+    ctas_per_sm[dev] = (n > 0 ? n : 1) * sms;
+  }
+  const int grid = std::min(T_rows, ctas_per_sm[dev]);
+  return launch_pdl(adaln_stream_kernel<T, NCT>, dim3(grid), dim3(128), smem, st, 1, x, shift, scale, mod_stride, cu, R, y,
+                    T_rows, eps, split, set_off);
+}
+
+static bool adaln_stream_enabled() {
+  static const bool on = [] {
+    const char* e = std::getenv("DIT_ADALN_KERNEL");
+    return !(e && std::strcmp(e, "rows") == 0);
+  }();
+  return on;
+}
+
 template <typename T>
 static dit_status launch_adaln_t(float* x, const T* h, const float* gate, const float* shift, const float* scale,
                                  int64_t mod_stride, const int32_t* cu, int R, T* y, int T_rows, int D, float eps,
@@ -246,6 +401,21 @@ static dit_status launch_adaln_t(float* x, const T* h, const float* gate, const 
   if (T_rows == 0) return DIT_OK;
   DIT_REQUIRE(D % 256 == 0 && D <= 6144, DIT_ERR_UNSUPPORTED, "adaln: D=%d must be a multiple of 256 (<= 6144)", D);
   ProfScope _prof(DIT_KC_ADALN, st);
+  // few-wave launches without the residual: the persistent bulk-copy kernel (rows of whole KB; x rows 16-byte aligned)
+  if (h == nullptr && D % 1024 == 0 && D / 1024 <= 6 && T_rows >= 592 && adaln_stream_enabled()) {
+    cudaError_t e = cudaSuccess;
+    switch (D / 1024) {
+      case 1: e = launch_adaln_stream<T, 1>(x, shift, scale, mod_stride, cu, R, y, T_rows, eps, st, split, set_off); break;
+      case 2: e = launch_adaln_stream<T, 2>(x, shift, scale, mod_stride, cu, R, y, T_rows, eps, st, split, set_off); break;
+      case 3: e = launch_adaln_stream<T, 3>(x, shift, scale, mod_stride, cu, R, y, T_rows, eps, st, split, set_off); break;
+      case 4: e = launch_adaln_stream<T, 4>(x, shift, scale, mod_stride, cu, R, y, T_rows, eps, st, split, set_off); break;
+      case 5: e = launch_adaln_stream<T, 5>(x, shift, scale, mod_stride, cu, R, y, T_rows, eps, st, split, set_off); break;
+      default: e = launch_adaln_stream<T, 6>(x, shift, scale, mod_stride, cu, R, y, T_rows, eps, st, split, set_off); break;
+    }
+    DIT_CUDA_OK(e);
+    DIT_LAUNCH_CHECK();
+    return DIT_OK;
+  }
 #define ADALN_CASE(NCV, NCW, WPR)                                                                           \
   case NCV:                                                                                                 \
     DIT_CUDA_OK(launch_pdl(adaln_kernel<T, NCW, WPR>, dim3(cdiv(T_rows, 4 / WPR)), dim3(128), 0, st, 1, x, h, gate, \

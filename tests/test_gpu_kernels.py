@@ -83,6 +83,31 @@ def test_adaln_varlen_requests_and_null_modulation(lib, dtype):
     check(yc, m[0, :D].expand(4, D), dtype, "constant row", **tol)
 
 
+@pytest.mark.parametrize("dtype", DTYPES)
+@pytest.mark.parametrize("T,D,R", [(592, 1024, 1), (1000, 3072, 3), (4352, 3072, 1), (777, 5120, 2), (2000, 2048, 5), (650, 6144, 1)])
+def test_adaln_persistent_rows_kernel(lib, dtype, T, D, R):
+    """T >= 592 rows without the residual take the persistent bulk-copy kernel (CTAs walk rows with a stride, modulation
+    rows held in registers and reloaded when the request changes): ragged request boundaries, every D / 1024."""
+    bounds = sorted({0, T} | {(T * (2 * r + 1)) // (2 * R) + r for r in range(R - 1)})
+    assert len(bounds) == R + 1
+    cu = torch.tensor(bounds, dtype=torch.int32, device=DEV)
+    x = rnd("xp", (T, D), torch.float32, std=2.0, mean=-0.2)
+    mod = rnd("modp", (R, 2 * D), torch.float32, std=0.3)
+    y = B.dit_adaln(x, dtype, shift=mod[:, :D], scale=mod[:, D:], mod_stride=2 * D, cu_seqlens=cu if R > 1 else None, n_requests=R)
+    m = mod.double().cpu()
+    req = torch.repeat_interleave(torch.arange(R), torch.tensor([bounds[r + 1] - bounds[r] for r in range(R)]))
+    ref = O.layer_norm(x.double().cpu(), 1e-6) * (1 + m[req][:, D:]) + m[req][:, :D]
+    if dtype == torch.float32:
+        check(y, ref, dtype, "adaln persistent", rel=2e-6, maxabs=2e-5)
+    else:
+        check(y, ref, dtype, "adaln persistent", rel=3e-3, maxabs=6e-2)
+        check_rounding(y, ref, "adaln persistent")
+    # plain LN (no modulation) on the same kernel
+    y0 = B.dit_adaln(x, dtype)
+    check(y0, O.layer_norm(x.double().cpu(), 1e-6), dtype, "adaln persistent, plain LN",
+          **(dict(rel=2e-6, maxabs=2e-5) if dtype == torch.float32 else dict(rel=3e-3, maxabs=6e-2)))
+
+
 # ------------------------------------------------------------------------------ QK-RMSNorm + RoPE
 @pytest.mark.parametrize("dtype", DTYPES)
 @pytest.mark.parametrize("T,H,d", [(33, 4, 64), (130, 24, 128), (7, 3, 128)])
