@@ -365,12 +365,13 @@ static cudaError_t launch_adaln_stream(const float* x, const float* shift, const
                                        const int32_t* cu, int R, T* y, int T_rows, float eps, cudaStream_t st, int split,
                                        int64_t set_off) {
   constexpr int smem = ADALN_STAGES * NCT * 1024 * 4;
-  static int ctas_per_sm[16] = {0};                 // per device: resident CTAs of this instantiation x SMs (0 = not asked yet)
+  // per device: resident CTAs of this instantiation x SMs (0 = not asked yet; racing first calls compute the same value)
+  static std::atomic<int> ctas_per_sm[16];
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return e;
   if (dev >= 16) return cudaErrorInvalidDevice;
-  if (ctas_per_sm[dev] == 0) {
+  if (ctas_per_sm[dev].load(std::memory_order_acquire) == 0) {
     e = cudaFuncSetAttribute(adaln_stream_kernel<T, NCT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     int n = 0;
@@ -379,9 +380,9 @@ static cudaError_t launch_adaln_stream(const float* x, const float* shift, const
     int sms = 148;
     e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     if (e != cudaSuccess) return e;
-    ctas_per_sm[dev] = (n > 0 ? n : 1) * sms;
+    ctas_per_sm[dev].store((n > 0 ? n : 1) * sms, std::memory_order_release);
   }
-  const int grid = std::min(T_rows, ctas_per_sm[dev]);
+  const int grid = std::min(T_rows, ctas_per_sm[dev].load(std::memory_order_relaxed));
   return launch_pdl(adaln_stream_kernel<T, NCT>, dim3(grid), dim3(128), smem, st, 1, x, shift, scale, mod_stride, cu, R, y,
                     T_rows, eps, split, set_off);
 }
