@@ -496,6 +496,10 @@ def run_traj(args):
     m1 = B.Dit(B.make_config(s, split_p=args.split_p), W, dev)
     m2 = B.Dit(B.make_config(s, split_p=args.split_p, max_requests=2, max_tokens=2 * (s.n_tokens + s.n_cond),
                              max_cond_tokens=2 * s.n_cond), W, dev)
+    # the same two handles with room for the whole trajectory's modulation vectors (dit_config.max_sample_steps)
+    m1a = B.Dit(B.make_config(s, split_p=args.split_p, max_sample_steps=n), W, dev)
+    m2a = B.Dit(B.make_config(s, split_p=args.split_p, max_requests=2, max_tokens=2 * (s.n_tokens + s.n_cond),
+                              max_cond_tokens=2 * s.n_cond, max_sample_steps=n), W, dev)
     I = synth.make_inputs(s, device=dev)
     lat, cond = I["latents"], I["cond"]
     unc = synth.normal(s.seed, "uncond", tuple(cond.shape), dtype=s.torch_dtype, device=dev)
@@ -506,7 +510,10 @@ def run_traj(args):
     rows = []
     for name, m, u, graph in (("stream launches", m1, None, False), ("cuda graph", m1, None, True),
                               ("guided (2 passes/step), cuda graph", m1, unc, True),
-                              ("guided (1 packed pass of 2 requests/step), cuda graph", m2, unc, True)):
+                              ("guided (1 packed pass of 2 requests/step), cuda graph", m2, unc, True),
+                              ("cuda graph, modulation of all steps computed ahead", m1a, None, True),
+                              ("guided (2 passes/step), cuda graph, modulation ahead", m1a, unc, True),
+                              ("guided (1 packed pass/step), cuda graph, modulation ahead", m2a, unc, True)):
         for _ in range(Wm):
             m.dit_sample(lat, tembs, sigmas, cond, u, 4.0, use_graph=graph, out=out)
         torch.cuda.synchronize()

@@ -89,6 +89,12 @@ typedef struct {
   int32_t max_cond_tokens; /* capacity: max total conditioning tokens per call */
   int32_t mlp_gated;       /* 0: MLP = W2 GELU_tanh(W1 y + b1) + b2 (R3).  1: gated MLP (SwiGLU; SURVEY.md §8(f) item 2,
                               DESIGN.md R40): W2 (SiLU(W1 y + b1) (.) (W3 y + b3)) + b2 with extra weights mlp.w3, mlp.b3 */
+  int32_t max_sample_steps; /* dit_sample only (0..4096; 0 = off): room in the workspace for the timestep-MLP outputs and
+                              modulation vectors of this many denoising steps.  They depend on the timestep embedding alone,
+                              so dit_sample computes them for (chunks of) this many steps AHEAD of the steps, 8 rows per pass
+                              of the modulation weights: the weights (0.9 GB at BASELINE configs[1]) are streamed once per 8
+                              steps instead of once per step (twice per guided step in the two-pass mode).  Results are
+                              bit-identical to max_sample_steps = 0. */
 } dit_config;
 
 /* One named weight tensor (device pointer, caller-owned, config dtype).  Names:

@@ -30,7 +30,8 @@ class dit_config(C.Structure):
                 ("patch", C.c_int32 * 3), ("temb_dim", C.c_int32), ("cond_dim", C.c_int32), ("cond_mode", C.c_int32),
                 ("rope_dims", C.c_int32 * 3), ("rope_theta", C.c_float), ("ln_eps", C.c_float), ("rms_eps", C.c_float),
                 ("qk_rmsnorm", C.c_int32), ("split_p", C.c_int32), ("max_tokens", C.c_int32),
-                ("max_requests", C.c_int32), ("max_cond_tokens", C.c_int32), ("mlp_gated", C.c_int32)]
+                ("max_requests", C.c_int32), ("max_cond_tokens", C.c_int32), ("mlp_gated", C.c_int32),
+                ("max_sample_steps", C.c_int32)]
 
 
 class dit_weight(C.Structure):
@@ -165,7 +166,7 @@ def _i32arr(vals):
     return (C.c_int32 * len(vals))(*vals)
 
 
-def make_config(shape, split_p=1, max_tokens=None, max_requests=1, max_cond_tokens=None) -> dit_config:
+def make_config(shape, split_p=1, max_tokens=None, max_requests=1, max_cond_tokens=None, max_sample_steps=0) -> dit_config:
     """dit_config from a synth.DiTShape-like object (duck typed)."""
     c = dit_config()
     c.struct_size = C.sizeof(dit_config)
@@ -182,6 +183,7 @@ def make_config(shape, split_p=1, max_tokens=None, max_requests=1, max_cond_toke
     c.max_requests = max_requests
     c.max_cond_tokens = int(max_cond_tokens if max_cond_tokens is not None else (shape.n_cond if shape.cond_mode != "none" else 0))
     c.mlp_gated = int(bool(shape.extras.get("mlp_gated", False)))
+    c.max_sample_steps = int(max_sample_steps)
     return c
 
 

@@ -98,6 +98,7 @@ struct Workspace {
   void* stage_out;
   float* sample_x; // dit_sample: fp32 trajectory state [Tm * C*pv]
   float* sample_v; // dit_sample: unconditional velocity of a guided step, fp32
+  float* traj;     // dit_sample: [S, D] c1 | [S, D] c | [S, mod_len] modulation of S = max_sample_steps steps computed ahead
   size_t total;
 };
 
@@ -173,6 +174,7 @@ static bool carve(const dit_config& c, char* base, Workspace* w) {
   w->stage_out = take(Tm * pvC * es);
   w->sample_x = (float*)take(Tm * pvC * 4);
   w->sample_v = (float*)take(Tm * pvC * 4);
+  w->traj = (float*)take((size_t)c.max_sample_steps * (2 * D + L * (c.cond_mode == DIT_COND_JOINT2 ? 12 : 6) * D + 2 * D) * 4);
   w->total = off;
   return true;
 }
@@ -183,6 +185,8 @@ static dit_status validate(const dit_config* c) {
               c->struct_size, (int)sizeof(dit_config));
   DIT_REQUIRE(c->dtype == DIT_F32 || c->dtype == DIT_BF16, DIT_ERR_INVALID_ARG, "dtype %d", c->dtype);
   DIT_REQUIRE(c->n_blocks >= 0 && c->n_blocks <= 256, DIT_ERR_INVALID_ARG, "n_blocks %d", c->n_blocks);
+  DIT_REQUIRE(c->max_sample_steps >= 0 && c->max_sample_steps <= 4096, DIT_ERR_INVALID_ARG, "max_sample_steps %d not in 0..4096",
+              c->max_sample_steps);
   DIT_REQUIRE(c->head_dim == 64 || c->head_dim == 128, DIT_ERR_UNSUPPORTED, "head_dim %d not in {64,128}", c->head_dim);
   DIT_REQUIRE(c->n_heads > 0 && c->hidden == c->n_heads * c->head_dim, DIT_ERR_INVALID_ARG,
               "hidden %d != n_heads %d * head_dim %d", c->hidden, c->n_heads, c->head_dim);
@@ -360,8 +364,10 @@ static dit_status upload_geom(dit_handle hd, const StepGeom& g, cudaStream_t st)
 // of the same latents at the same timestep — one t-MLP / modulation row serves both (row stride 0), each request has its
 // own cond pointer and its own unpatchify epilogue.
 struct GuidedPair { const void* cond[2]; const SampleEpi* epi[2]; };
+// mod_pre != nullptr: this step's modulation row was computed ahead (dit_sample, max_sample_steps): no timestep MLP / GEMV here
 static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents, const float* temb, const void* cond,
-                           void* out, cudaStream_t st, const SampleEpi* epi = nullptr, const GuidedPair* pair = nullptr) {
+                           void* out, cudaStream_t st, const SampleEpi* epi = nullptr, const GuidedPair* pair = nullptr,
+                           const float* mod_pre = nullptr) {
   const dit_config& c = hd->cfg;
   Workspace& w = hd->ws;
   const int dt = c.dtype;
@@ -395,9 +401,12 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
   } while (0)
 
   // ---- steps 1-2: c = W2 SiLU(W1 temb + b1) + b2;  mod = Wmod SiLU(c) + bmod for ALL blocks in one launch
-  RUN(launch_gemv(dt, temb, w.gemv_tab + 0, nullptr, 1, D, w.c1, D, Rt, c.temb_dim, 0, st));
-  RUN(launch_gemv(dt, w.c1, w.gemv_tab + 1, nullptr, 1, D, w.c, D, Rt, D, 1, st));
-  RUN(launch_gemv(dt, w.c, w.gemv_tab + 2, nullptr, dual ? 2 * L + 1 : L + 1, (int)mod_len, w.mod, mod_len, Rt, D, 1, st));
+  const float* const mod = mod_pre != nullptr ? mod_pre : w.mod;
+  if (mod_pre == nullptr) {
+    RUN(launch_gemv(dt, temb, w.gemv_tab + 0, nullptr, 1, D, w.c1, D, Rt, c.temb_dim, 0, st));
+    RUN(launch_gemv(dt, w.c1, w.gemv_tab + 1, nullptr, 1, D, w.c, D, Rt, D, 1, st));
+    RUN(launch_gemv(dt, w.c, w.gemv_tab + 2, nullptr, dual ? 2 * L + 1 : L + 1, (int)mod_len, w.mod, mod_len, Rt, D, 1, st));
+  }
 
   if (hd->wait_before_embed != nullptr) DIT_CUDA_OK(cudaStreamWaitEvent(st, hd->wait_before_embed, 0));   // inputs uploaded
   // ---- steps 3-4: patch-embed and cond projection write the fp32 residual stream
@@ -461,15 +470,15 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
       struct SW { const void *wqkv, *bqkv, *gq, *gk, *wo, *bo, *w1, *b1, *w2, *b2, *w3, *b3; };
       const SW sw_img{b.wqkv, b.bqkv, b.gq, b.gk, b.wo, b.bo, b.w1, b.b1, b.w2, b.b2, b.w3, b.b3};
       const SW sw_txt{b.t_wqkv, b.t_bqkv, b.t_gq, b.t_gk, b.t_wo, b.t_bo, b.t_w1, b.t_b1, b.t_w2, b.t_b2, b.t_w3, b.t_b3};
-      auto mod_of = [&](const Seg& sg) { return w.mod + (size_t)sg.r * mod_stride + (sg.txt ? mod_img : 0) + (size_t)l * 6 * D; };
+      auto mod_of = [&](const Seg& sg) { return mod + (size_t)sg.r * mod_stride + (sg.txt ? mod_img : 0) + (size_t)l * 6 * D; };
       auto rows_of = [&](void* base, const Seg& sg, int64_t ld) { return (void*)((char*)base + (size_t)sg.row0 * ld * es); };
       // adaLN: one launch over all segments (row -> segment -> request and stream through cu_seg_dev)
-      const float* mblk = w.mod + (size_t)l * 6 * D;
+      const float* mblk = mod + (size_t)l * 6 * D;
       RUN(launch_adaln(dt, w.x, nullptr, nullptr, mblk, mblk + D, mod_stride, w.cu_seg_dev, 2 * R, w.y, T, D, c.ln_eps, st, 0, mod_img));
       if (stop(l, DIT_STAGE_Y1)) return DIT_OK;
       SegGemm sgm{};   // the fields every segmented launch of this block shares
       sgm.segs = &gsegs; sgm.M = T; sgm.rms_eps = c.rms_eps;
-      sgm.gate = w.mod + (size_t)l * 6 * D; sgm.gate_stride = mod_stride; sgm.gate_set_off = mod_img;
+      sgm.gate = mod + (size_t)l * 6 * D; sgm.gate_stride = mod_stride; sgm.gate_set_off = mod_img;
       if (grouped) {
         DIT_REQUIRE(gemm_tc_supported(DIT_EPI_BIAS, w.y, D, sw_img.wqkv, w.qkv, 3 * D, T, 3 * D, D), DIT_ERR_UNSUPPORTED,
                     "bf16 dual-stream step: the tcgen05 GEMM is unavailable");
@@ -564,7 +573,7 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
       if (stop(l, DIT_STAGE_FC2)) return DIT_OK;
       continue;
     }
-    const float* m = w.mod + (size_t)l * 6 * D;
+    const float* m = mod + (size_t)l * 6 * D;
     RUN(launch_adaln(dt, w.x, nullptr, nullptr, m + 0 * D, m + 1 * D, mod_stride, cu_dev, R, w.y, T, D, c.ln_eps, st));
     if (stop(l, DIT_STAGE_Y1)) return DIT_OK;
     if (dt == DIT_BF16 && d == 128 && (c.qk_rmsnorm || rope) &&
@@ -645,7 +654,7 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
     if (stop(l, DIT_STAGE_FC2)) return DIT_OK;
   }
   // ---- step 6: final adaLN (folds the last gated residual), Linear D -> C*pv, unpatchify (image tokens only)
-  const float* mf = w.mod + (size_t)L * 6 * D;
+  const float* mf = mod + (size_t)L * 6 * D;
   RUN(launch_adaln(dt, w.x, nullptr, nullptr, mf, mf + D, mod_stride, cu_dev, R, w.y, T, D, c.ln_eps, st, split ? 1 : 0));
   const int y_ld = split ? 2 * D : D;
   for (int r = 0; r < R; ++r) {
@@ -1014,25 +1023,47 @@ dit_status dit_sample(dit_handle h, const void* latents, const float* timestep_e
   auto enqueue = [&](cudaStream_t st) -> dit_status {
     dit_status e = launch_sample_init(c.dtype, latents, w.sample_x, n, st);
     if (e != DIT_OK) return e;
+    // timestep MLP + modulation of up to max_sample_steps steps ahead of the steps (they need the embeddings only): the
+    // GEMV kernels take 8 rows per pass over the weights, so the modulation weights are streamed once per 8 steps
+    const int S = (h->stop_block < 0) ? c.max_sample_steps : 0;
+    const int D = c.hidden, L = c.n_blocks;
+    const bool dual = c.cond_mode == DIT_COND_JOINT2;
+    const int64_t mod_len = (int64_t)L * (dual ? 12 : 6) * D + 2 * D;
+    float* const tc1 = w.traj;
+    float* const tcc = w.traj + (size_t)S * D;
+    float* const tmod = w.traj + (size_t)2 * S * D;
     for (int i = 0; i < n_steps; ++i) {
       const void* x_in = i == 0 ? latents : out;   // x_i rounded to the config dtype was staged in `out` by step i - 1
       const float* temb = timestep_embs + (size_t)i * c.temb_dim;
+      const float* mod_pre = nullptr;
+      if (S > 0) {
+        if (i % S == 0) {
+          const int rows = n_steps - i < S ? n_steps - i : S;
+          e = launch_gemv(c.dtype, temb, w.gemv_tab + 0, nullptr, 1, D, tc1, D, rows, c.temb_dim, 0, st);
+          if (e != DIT_OK) return e;
+          e = launch_gemv(c.dtype, tc1, w.gemv_tab + 1, nullptr, 1, D, tcc, D, rows, D, 1, st);
+          if (e != DIT_OK) return e;
+          e = launch_gemv(c.dtype, tcc, w.gemv_tab + 2, nullptr, dual ? 2 * L + 1 : L + 1, (int)mod_len, tmod, mod_len, rows, D, 1, st);
+          if (e != DIT_OK) return e;
+        }
+        mod_pre = tmod + (size_t)(i % S) * mod_len;
+      }
       SampleEpi epi{2, w.sample_x, nullptr, sigmas_host[i + 1] - sigmas_host[i], guidance_scale};
       if (packed) {
         SampleEpi hold{1, nullptr, w.sample_v, 0.f, 0.f};
         epi.v_hold = w.sample_v;
         GuidedPair gp{{uncond_tokens, cond_tokens}, {&hold, &epi}};
-        e = run_step(h, g2, x_in, temb, nullptr, out, st, nullptr, &gp);
+        e = run_step(h, g2, x_in, temb, nullptr, out, st, nullptr, &gp, mod_pre);
         if (e != DIT_OK) return e;
         continue;
       }
       if (guided) {
         SampleEpi hold{1, nullptr, w.sample_v, 0.f, 0.f};
-        e = run_step(h, gu, x_in, temb, uncond_tokens, out, st, &hold);
+        e = run_step(h, gu, x_in, temb, uncond_tokens, out, st, &hold, nullptr, mod_pre);
         if (e != DIT_OK) return e;
         epi.v_hold = w.sample_v;
       }
-      e = run_step(h, gc, x_in, temb, cond_tokens, out, st, &epi);
+      e = run_step(h, gc, x_in, temb, cond_tokens, out, st, &epi, nullptr, mod_pre);
       if (e != DIT_OK) return e;
     }
     if (n_steps == 0) return launch_sample_final(c.dtype, w.sample_x, out, n, st);

@@ -138,6 +138,41 @@ def test_graph_replay_is_bit_identical_and_recaptures_on_change(lib):
     assert torch.equal(v, v2)
 
 
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+@pytest.mark.parametrize("mode", ["plain", "two_pass", "packed"])
+def test_modulation_computed_ahead_is_bit_identical(lib, dtype, mode):
+    """dit_config.max_sample_steps: the timestep MLP and the modulation GEMV of (chunks of) the trajectory's steps run ahead
+    of the steps, 8 rows per pass over the weights.  11 steps with room for 1, 4 (chunks 4 4 3), 11 and 16 steps (a 9-row
+    launch = an 8-row and a 1-row pass), stream launches and graph: every result equals max_sample_steps = 0 bit for bit."""
+    if dtype == "f32":
+        s = synth.cfg1(cond_mode="joint", rope_dims=(0, 32, 32), qk_rmsnorm=True)
+    else:
+        s = synth.cfg1(name="traj_bf16", dtype="bf16", hidden=512, n_heads=4, head_dim=128, mlp_dim=2048, cond_dim=512,
+                       latent_channels=16, rope_dims=(0, 64, 64), qk_rmsnorm=True, cond_mode="joint2" if mode == "packed" else "joint")
+    n_steps, n_unc = 11, 24
+    W = synth.make_weights(s)
+    I, tembs, sigmas, unc = _traj(s, n_steps, n_unc)
+    caps = _packed_caps(s, n_unc) if mode == "packed" else {}
+    dev = lambda t: None if t is None else t.to(DEV)
+    args = (dev(I["latents"]), dev(tembs), sigmas, dev(I["cond"]), dev(unc) if mode != "plain" else None, 3.0 if mode != "plain" else 1.0)
+    base = B.Dit(B.make_config(s, **caps), W, DEV).dit_sample(*args)
+    torch.cuda.synchronize()
+    for S in (1, 4, 11, 16):
+        m = B.Dit(B.make_config(s, max_sample_steps=S, **caps), W, DEV)
+        for use_graph in (False, True, True):
+            out = m.dit_sample(*args, use_graph=use_graph)
+            torch.cuda.synchronize()
+            assert torch.equal(out, base), f"max_sample_steps={S} graph={use_graph}"
+        # the single step of the same handle is untouched by the trajectory buffers
+        v = m.dit_step(args[0], args[1][0], args[3])
+        v0 = B.Dit(B.make_config(s, **caps), W, DEV).dit_step(args[0], args[1][0], args[3])
+        torch.cuda.synchronize()
+        assert torch.equal(v, v0)
+    bad = B.make_config(s, max_sample_steps=5000)
+    with pytest.raises(B.DitError):
+        B.Dit(bad, W, DEV)
+
+
 def test_packed_guided_cross_graph_with_changing_uncond_count(lib):
     """Cross-attention, packed guided step (R = 2), CUDA-graph replay: a second trajectory on the SAME handle with the
     same latents but another number of unconditional tokens changes only the cond-token offsets (cu_cond) — the resident
