@@ -403,7 +403,7 @@ static dit_status launch_adaln_t(float* x, const T* h, const float* gate, const 
   DIT_REQUIRE(D % 256 == 0 && D <= 6144, DIT_ERR_UNSUPPORTED, "adaln: D=%d must be a multiple of 256 (<= 6144)", D);
   ProfScope _prof(DIT_KC_ADALN, st);
   // few-wave launches without the residual: the persistent bulk-copy kernel (rows of whole KB; x rows 16-byte aligned)
-  if (h == nullptr && D % 1024 == 0 && D / 1024 <= 6 && T_rows >= 592 && adaln_stream_enabled()) {
+  if (h == nullptr && D % 1024 == 0 && D / 1024 <= 6 && T_rows >= 592 && ((uintptr_t)x & 15) == 0 && adaln_stream_enabled()) {
     cudaError_t e = cudaSuccess;
     switch (D / 1024) {
       case 1: e = launch_adaln_stream<T, 1>(x, shift, scale, mod_stride, cu, R, y, T_rows, eps, st, split, set_off); break;
