@@ -253,8 +253,14 @@ def test_zero_gates_make_blocks_identity_bit_exact():
     assert torch.equal(taps["b1.x_mlp"], taps["x0"])                                  # bit exact identity
     s0 = _tiny(n_blocks=0)
     W0 = {k: v for k, v in W.items() if not k.startswith("blocks.")}
-    out0, _, _ = _run(s0, W0)
+    out0, I, _ = _run(s0, W0)[0], synth.make_inputs(s0), None
     assert torch.equal(out, out0)
+    # joint mode, identity blocks: the final layer reads the IMAGE rows x[Lc:] only (step 6), so the output neither depends
+    # on the cond tokens nor differs from the same model without conditioning
+    other = dict(I, cond=I["cond"] * -3.0 + 1.0)
+    assert torch.equal(_run(s0, W0, other)[0], out0)
+    sn = _tiny(n_blocks=0, cond_mode="none")
+    assert torch.equal(O.dit_step(O.cfg_from_shape(sn), W0, I["latents"], I["temb"], None), out0)
 
 
 def test_step_split_p_invariance_and_modes():

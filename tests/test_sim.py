@@ -82,6 +82,45 @@ def test_edf_orders_ready_tasks_by_deadline():
     assert res[0]["finish_s"] == pytest.approx(6 * 0.05)
 
 
+def test_edf_deadline_beats_arrival_and_migration_enters_the_degree_choice():
+    # the earlier DEADLINE wins although the request arrived later (R39: order by (deadline, arrival, index))
+    reqs = [_req(1, 2, 0.0, 50.0), _req(1, 2, 0.01, 0.5)]
+    tr = []
+    S.simulate(_cfg(S.EDF, n_ranks=1), TABLE, reqs, trace=tr)
+    assert [t[0] for t in tr] == [0, 1, 1, 0]
+    # the predicted finish of a candidate degree includes the migration it would cause: with a slow
+    # re-layout (16 MB at 0.16 GB/s = 0.1 s) leaving degree 2 for degree 1 never meets 3.6 (3 + 0.027 i + 0.1 + 0.05 (20 - i)
+    # <= 3.6 needs i >= 21.7), so the request stays on its two ranks: 20 x 0.027, no migration, deadline met.  (Without the
+    # migration term it would switch after 18 steps and finish at 3.686.)
+    res, _ = S.simulate(_cfg(S.EDF, relayout_gbps=0.16), TABLE, [_req(1, 20, 3.0, 3.6)])
+    assert res[0]["n_migrations"] == 0 and res[0]["max_degree"] == 2 and res[0]["met_deadline"] == 1
+    assert res[0]["finish_s"] == pytest.approx(3.0 + 20 * 0.027, abs=1e-12)
+    # a change of rank set is counted as a migration even when it costs no time (no re-layout bandwidth given): degree 1 meets
+    # the deadline once 3 + 0.027 i + 0.05 (20 - i) <= 3.6, i.e. from i = 18
+    res, _ = S.simulate(_cfg(S.EDF, relayout_gbps=0.0), TABLE, [_req(1, 20, 3.0, 3.6)])
+    assert res[0]["n_migrations"] == 1 and res[0]["finish_s"] == pytest.approx(3.0 + 18 * 0.027 + 2 * 0.05, abs=1e-12)
+
+
+def test_summary_statistics_and_timeouts_by_hand():
+    # 20 requests of 1..20 steps, one rank each (SRTF places a new request on the least-loaded rank): latency_i = 0.01 i
+    reqs = [_req(0, i + 1, 0.0, 0.01 * (i + 1) + (1e-9 if i % 2 == 0 else -1e-3)) for i in range(20)]
+    res, summ = S.simulate(_cfg(S.SRTF, n_ranks=20), TABLE, reqs)
+    for i, r in enumerate(res):
+        assert r["finish_s"] == pytest.approx(0.01 * (i + 1), abs=1e-12) and r["failed"] == 0
+        assert r["met_deadline"] == (1 if i % 2 == 0 else 0)
+    assert summ["p95_latency_s"] == pytest.approx(0.19, abs=1e-12)          # 19th of 20 sorted latencies (ceil(0.95 n))
+    assert summ["mean_latency_s"] == pytest.approx(0.105, abs=1e-12)
+    assert summ["makespan_s"] == pytest.approx(0.20, abs=1e-12) and summ["throughput_rps"] == pytest.approx(100.0)
+    assert summ["slo_attainment"] == pytest.approx(0.5)
+    assert summ["utilisation"] == pytest.approx(sum(0.01 * (i + 1) for i in range(20)) / (20 * 0.20))
+    # a timeout of 0.155 s fails the five requests of 16..20 steps: they leave the latency statistics and miss their SLO
+    res, summ = S.simulate(_cfg(S.SRTF, n_ranks=20, timeout_s=0.155), TABLE, reqs)
+    assert [r["failed"] for r in res] == [0] * 15 + [1] * 5
+    assert summ["p95_latency_s"] == pytest.approx(0.15, abs=1e-12) and summ["mean_latency_s"] == pytest.approx(0.08, abs=1e-12)
+    assert summ["slo_attainment"] == pytest.approx(8 / 20)                   # the even-indexed ones among the first 15
+    assert summ["throughput_rps"] == pytest.approx(15 / 0.20)
+
+
 def _random_trace(seed, n, classes=3, rate=40.0):
     u = synth.uniform01(seed, "sim.trace", 4 * n).tolist()
     t, reqs = 0.0, []
@@ -137,6 +176,22 @@ def test_library_simulator_matches_oracle(lib, policy, seed, n, ranks, group, ra
         assert a == b, (a, b)                                  # finish times etc. bit for bit
     for k in so:
         assert sl[k] == so[k] or sl[k] == pytest.approx(so[k], rel=1e-15), k
+
+
+def test_library_simulator_on_the_hand_made_scenarios(lib):
+    """The scenarios the oracle is pinned on by hand, through the library: slow / absent re-layout bandwidth in EDF's degree
+    choice, deadline-before-arrival order, timeouts in the summary."""
+    cases = [(_cfg(S.EDF, n_ranks=1), [_req(1, 2, 0.0, 50.0), _req(1, 2, 0.01, 0.5)]),
+             (_cfg(S.EDF, relayout_gbps=0.16), [_req(1, 20, 3.0, 3.6)]),
+             (_cfg(S.EDF, relayout_gbps=0.0), [_req(1, 20, 3.0, 3.6)]),
+             (_cfg(S.EDF), [_req(1, 20, 3.0, 3.6)]),
+             (_cfg(S.SRTF, n_ranks=20, timeout_s=0.155), [_req(0, i + 1, 0.0, 0.01 * (i + 1) + (1e-9 if i % 2 == 0 else -1e-3)) for i in range(20)])]
+    for cfg, reqs in cases:
+        ro, so = S.simulate(cfg, TABLE, reqs)
+        rl, sl = B.dit_sim_run(cfg, TABLE, reqs)
+        assert ro == rl
+        for k in so:
+            assert sl[k] == so[k] or sl[k] == pytest.approx(so[k], rel=1e-15), k
 
 
 def test_library_simulator_rejects_bad_input(lib):
