@@ -3,8 +3,8 @@
 Every entry is ONE plausible mistake in oracle/*.py — a sign, an index, an operand order, a dropped term, a constant.  The script
 copies oracle/ and tests/ to a temporary directory, applies one mutant at a time and runs the CPU suite there
 (`pytest -m "not gpu"`; set MUT_ARGS='-k not(library)' to leave out the library-against-oracle comparisons and see the
-independent pins alone).  A mutant that no test fails is printed as SURVIVED.  State at the end of round 2: 64 mutants,
-62 killed; the two survivors are equivalent programs (clamping |r| at 480 instead of 448 before the nearest-code search
+independent pins alone).  A mutant that no test fails is printed as SURVIVED.  State at the end of round 2: 80 mutants,
+78 killed; the two survivors are equivalent programs (clamping |r| at 480 instead of 448 before the nearest-code search
 saturates to the same code; 1 / (amax / 448) against 448 / amax differs by an ulp on inputs the pins do not contain — the rule
 itself is reading R42).  Nothing here is imported by the product or by a test."""
 import os, shutil, subprocess, sys, tempfile
@@ -79,6 +79,24 @@ MORE += [
  ("oracle/sim_oracle.py", "sim p95", "p95_latency_s=lats[max(0, math.ceil(0.95 * len(lats)) - 1)] if lats else 0.0,", "p95_latency_s=lats[max(0, math.ceil(0.95 * len(lats)) - 2)] if lats else 0.0,"),
  ("oracle/sim_oracle.py", "sim failed", "failed = bool(timeout > 0 and lat > timeout)", "failed = bool(timeout > 0 and lat >= 0)"),
  ("oracle/sim_oracle.py", "sim mig count", "if mig > 0.0 or (last_set[r] is not None and last_set[r] != set_id):", "if mig > 0.0:"),
+]
+MORE += [
+ ("oracle/dit_oracle.py", "rms eps outside", "return x / torch.sqrt(ms + eps) * g", "return x / (torch.sqrt(ms) + eps) * g"),
+ ("oracle/dit_oracle.py", "rms sum", "ms = (x ** 2).mean(dim=-1, keepdim=True)", "ms = (x ** 2).sum(dim=-1, keepdim=True)"),
+ ("oracle/dit_oracle.py", "ln unbiased", "var = ((x - mu) ** 2).mean(dim=-1, keepdim=True)", "var = ((x - mu) ** 2).sum(dim=-1, keepdim=True) / (x.shape[-1] - 1)"),
+ ("oracle/dit_oracle.py", "linear transpose", "y = x @ _d(w).t()", "y = x @ _d(w)[:, :x.shape[-1]].t() if w.shape[0] != w.shape[1] else x @ _d(w)"),
+ ("oracle/dit_oracle.py", "rope on v", "q, k = apply_rope(q, ang), apply_rope(k, ang)\n    if taps is not None:\n        taps[f\"b{l}.q\"]", "q, k, v = apply_rope(q, ang), apply_rope(k, ang), apply_rope(v, ang)\n    if taps is not None:\n        taps[f\"b{l}.q\"]"),
+ ("oracle/dit_oracle.py", "softmax axis", "z = e.sum(dim=-1, keepdim=True)\n        p = e / z", "z = e.sum(dim=-1, keepdim=True)\n        p = e / e.sum(dim=0, keepdim=True)"),
+ ("oracle/dit_oracle.py", "cross kv from x", "kv = linear(ctx, W[p + \"wkv\"], W[p + \"bkv\"])\n            kc, vc", "kv = linear(ctx * 1.0001, W[p + \"wkv\"], W[p + \"bkv\"])\n            kc, vc"),
+ ("oracle/dit_oracle.py", "cross sign", "x = x + linear(oc.reshape(-1, D), W[p + \"wo\"], W[p + \"bo\"])\n            if taps", "x = x - linear(oc.reshape(-1, D), W[p + \"wo\"], W[p + \"bo\"])\n            if taps"),
+ ("oracle/dit_oracle.py", "modf order", "modf = linear(sc, W[\"final.mod.w\"], W[\"final.mod.b\"]).reshape(2, -1)", "modf = linear(sc, W[\"final.mod.w\"], W[\"final.mod.b\"]).reshape(-1, 2).t()"),
+ ("oracle/dit_oracle.py", "mods reshape", "mods = [linear(sc, W[f\"blocks.{l}.mod.w\"], W[f\"blocks.{l}.mod.b\"]).reshape(6, -1) for l in range(cfg[\"n_blocks\"])]", "mods = [linear(sc, W[f\"blocks.{l}.mod.w\"], W[f\"blocks.{l}.mod.b\"]).reshape(-1, 6).t() for l in range(cfg[\"n_blocks\"])]"),
+ ("oracle/dit_oracle.py", "mlp second modulate", "y2 = modulate(x, sh2, sc2, eps)\n        u, hm = mlp(cfg, W, f\"blocks.{l}.\", y2)", "y2 = modulate(x, sh1, sc1, eps)\n        u, hm = mlp(cfg, W, f\"blocks.{l}.\", y2)"),
+ ("oracle/dit_oracle.py", "qkv split", "q, k, v = (qkv[:, i * D:(i + 1) * D].reshape(T, H, d) for i in range(3))", "k, q, v = (qkv[:, i * D:(i + 1) * D].reshape(T, H, d) for i in range(3))"),
+ ("oracle/dit_oracle.py", "heads layout", "q, k, v = (qkv[:, i * D:(i + 1) * D].reshape(T, H, d) for i in range(3))", "q, k, v = (qkv[:, i * D:(i + 1) * D].reshape(T, d, H).transpose(1, 2) for i in range(3))"),
+ ("oracle/dit_oracle.py", "varlen shares temb", "return [dit_step(cfg, W, lat, te, co, split_p) for lat, te, co in zip(latents_list, temb_list, cond_list)]", "return [dit_step(cfg, W, lat, temb_list[0], co, split_p) for lat, te, co in zip(latents_list, temb_list, cond_list)]"),
+ ("oracle/dit_oracle.py", "merge lse", "lse = m_safe + torch.log(z)                                    # log(0) = -inf when all shards are empty", "lse = m_safe + z"),
+ ("oracle/dit_oracle.py", "dual qk gains", "k = rms_norm_heads(k, _d(W[pre + \"attn.gk\"]), cfg[\"rms_eps\"])\n        qs.append(q)", "k = rms_norm_heads(k, _d(W[pre + \"attn.gq\"]), cfg[\"rms_eps\"])\n        qs.append(q)"),
 ]
 def setup():
     shutil.copytree(os.path.join(ROOT, "oracle"), os.path.join(MUT, "oracle"))
