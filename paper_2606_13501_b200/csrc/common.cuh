@@ -212,6 +212,10 @@ dit_status launch_qknorm_rope(int dtype, void* qkv, int64_t row_stride, int T, i
                               cudaStream_t st);
 dit_status launch_rope_table(const SeqMeta* meta, int R, int T, int d, const int32_t rope_dims[3], float theta,
                              float* rc, float* rs, cudaStream_t st);
+dit_status launch_patchify_varlen(int dtype, const void* lat, void* patches, const SeqMeta* meta_dev, int R, int64_t max_elems,
+                                  int C, const int32_t patch[3], cudaStream_t st);
+dit_status launch_unpatchify_varlen(int dtype, const float* tok, void* out, const SeqMeta* meta_dev, int R, int64_t max_elems,
+                                    int C, const int32_t patch[3], cudaStream_t st);
 dit_status launch_patchify(int dtype, const void* lat, void* patches, int C, int F, int H, int W, const int32_t patch[3],
                            cudaStream_t st);
 // Sampler epilogue of the unpatchify kernel (dit_sample).  mode 0: out = v.  mode 1: v_hold = v (fp32, no out).

@@ -410,14 +410,29 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
 
   if (hd->wait_before_embed != nullptr) DIT_CUDA_OK(cudaStreamWaitEvent(st, hd->wait_before_embed, 0));   // inputs uploaded
   // ---- steps 3-4: patch-embed and cond projection write the fp32 residual stream
+  // A packed step of R > 1 requests: ONE patchify launch over all requests (geometry from the device table), ONE patch-embed
+  // GEMM over all T rows — patches live in sequence rows, the cond rows of a joint sequence hold whatever the buffer held and
+  // their x rows are overwritten by the cond projection right after — and at the end ONE final GEMM and ONE unpatchify:
+  // 4 launches instead of 4 R.  (Row-wise GEMM results do not depend on how rows are tiled: bit-identical to the per-request
+  // form, which DIT_VARLEN_PER_REQUEST=1 brings back.)
+  static const bool per_request_env = [] { const char* e = getenv("DIT_VARLEN_PER_REQUEST"); return e != nullptr && e[0] == '1'; }();
+  const bool batched_ends = R > 1 && pair == nullptr && epi == nullptr && !per_request_env;
+  int64_t max_elems = 0;
+  for (int r = 0; r < R; ++r) max_elems = std::max<int64_t>(max_elems, g.lat_off[r + 1] - g.lat_off[r]);
+  if (batched_ends) {
+    RUN(launch_patchify_varlen(dt, latents, w.patches, w.meta_dev, R, max_elems, c.latent_channels, c.patch, st));
+    RUN(gemm(dt, DIT_EPI_BIAS_F32, w.patches, pvC, hd->pe_w, hd->pe_b, w.x, D, T, D, pvC, st, DIT_KC_MISC));
+  }
   for (int r = 0; r < R; ++r) {
     const int Fr = g.grids[3 * r], Hr = g.grids[3 * r + 1], Wr = g.grids[3 * r + 2];
     const int Nr = (Fr / c.patch[0]) * (Hr / c.patch[1]) * (Wr / c.patch[2]);
     const int Lc = joint ? g.ncond[r] : 0;
     const int row0 = g.cu[r] + Lc;
     char* pr = (char*)w.patches + (size_t)row0 * pvC * es;
-    RUN(launch_patchify(dt, (const char*)latents + g.lat_off[r] * es, pr, c.latent_channels, Fr, Hr, Wr, c.patch, st));
-    RUN(gemm(dt, DIT_EPI_BIAS_F32, pr, pvC, hd->pe_w, hd->pe_b, w.x + (size_t)row0 * D, D, Nr, D, pvC, st, DIT_KC_MISC));
+    if (!batched_ends) {
+      RUN(launch_patchify(dt, (const char*)latents + g.lat_off[r] * es, pr, c.latent_channels, Fr, Hr, Wr, c.patch, st));
+      RUN(gemm(dt, DIT_EPI_BIAS_F32, pr, pvC, hd->pe_w, hd->pe_b, w.x + (size_t)row0 * D, D, Nr, D, pvC, st, DIT_KC_MISC));
+    }
     if (joint && Lc > 0)
       RUN(gemm(dt, DIT_EPI_BIAS_F32, cond_of(r), c.cond_dim, hd->cp_w, hd->cp_b, w.x + (size_t)g.cu[r] * D, D, Lc, D,
                c.cond_dim, st, DIT_KC_MISC));
@@ -657,7 +672,11 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
   const float* mf = mod + (size_t)L * 6 * D;
   RUN(launch_adaln(dt, w.x, nullptr, nullptr, mf, mf + D, mod_stride, cu_dev, R, w.y, T, D, c.ln_eps, st, split ? 1 : 0));
   const int y_ld = split ? 2 * D : D;
-  for (int r = 0; r < R; ++r) {
+  if (batched_ends) {   // all rows at once (the cond rows' tokens are computed and never read)
+    RUN(gemm(dt, DIT_EPI_BIAS_F32, w.y, y_ld, hd->f_w, hd->f_b, w.tok, pvC, T, pvC, D, st, DIT_KC_MISC, split ? 1 : 0));
+    RUN(launch_unpatchify_varlen(dt, w.tok, out, w.meta_dev, R, max_elems, c.latent_channels, c.patch, st));
+  }
+  for (int r = 0; r < R && !batched_ends; ++r) {
     const int Fr = g.grids[3 * r], Hr = g.grids[3 * r + 1], Wr = g.grids[3 * r + 2];
     const int Nr = (Fr / c.patch[0]) * (Hr / c.patch[1]) * (Wr / c.patch[2]);
     const int row0 = g.cu[r] + (joint ? g.ncond[r] : 0);

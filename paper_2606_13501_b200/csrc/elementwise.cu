@@ -626,6 +626,43 @@ __global__ void unpatchify_kernel(const float* __restrict__ tok, T* __restrict__
   out[idx] = from_f<T>(v);
 }
 
+// Packed forms (R > 1 requests in one step): blockIdx.y = request, its geometry from the device-resident SeqMeta table; rows are
+// written to / read from the request's image rows of the packed sequence (seq_start + n_cond).  Same index arithmetic as above.
+template <typename T>
+__global__ void patchify_varlen_kernel(const T* __restrict__ lat, T* __restrict__ patches, const SeqMeta* __restrict__ meta,
+                                       int C, int pf, int ph, int pw) {
+  const SeqMeta m = meta[blockIdx.y];
+  const int Fp = m.gf, Hp = m.gh, Wp = m.gw, pv = pf * ph * pw;
+  const int F = Fp * pf, H = Hp * ph, W = Wp * pw;
+  const int64_t total = (int64_t)Fp * Hp * Wp * C * pv;
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= total) return;
+  const int64_t lat_off = ((int64_t)(uint32_t)m.lat_off_lo) | ((int64_t)m.lat_off_hi << 32);
+  const int feat = (int)(idx % (C * pv));
+  const int n = (int)(idx / (C * pv));
+  const int k = feat % pw, j = (feat / pw) % ph, i = (feat / (pw * ph)) % pf, c = feat / pv;
+  const int w_ = n % Wp, h_ = (n / Wp) % Hp, f_ = n / (Wp * Hp);
+  patches[(int64_t)(m.seq_start + m.n_cond) * (C * pv) + idx] =
+      lat[lat_off + (((int64_t)c * F + f_ * pf + i) * H + h_ * ph + j) * W + w_ * pw + k];
+}
+
+template <typename T>
+__global__ void unpatchify_varlen_kernel(const float* __restrict__ tok, T* __restrict__ out, const SeqMeta* __restrict__ meta,
+                                         int C, int pf, int ph, int pw) {
+  const SeqMeta m = meta[blockIdx.y];
+  const int Hp = m.gh, Wp = m.gw, pv = pf * ph * pw;
+  const int F = m.gf * pf, H = Hp * ph, W = Wp * pw;
+  const int64_t total = (int64_t)C * F * H * W;
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= total) return;
+  const int64_t lat_off = ((int64_t)(uint32_t)m.lat_off_lo) | ((int64_t)m.lat_off_hi << 32);
+  const int w = (int)(idx % W), hh = (int)((idx / W) % H), f = (int)((idx / ((int64_t)W * H)) % F);
+  const int c = (int)(idx / ((int64_t)W * H * F));
+  const int n = ((f / pf) * Hp + hh / ph) * Wp + w / pw;
+  const int feat = ((c * pf + f % pf) * ph + hh % ph) * pw + w % pw;
+  out[lat_off + idx] = from_f<T>(tok[(int64_t)(m.seq_start + m.n_cond + n) * (C * pv) + feat]);
+}
+
 template <typename T>
 __global__ void sample_init_kernel(const T* __restrict__ lat, float* __restrict__ state, int64_t n) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -662,6 +699,33 @@ dit_status launch_unpatchify(int dtype, const float* tok, void* out, int C, int 
     unpatchify_kernel<float><<<cdiv(total, 256), 256, 0, st>>>(tok, (float*)out, C, F, H, W, patch[0], patch[1], patch[2], e);
   else
     unpatchify_kernel<bf16><<<cdiv(total, 256), 256, 0, st>>>(tok, (bf16*)out, C, F, H, W, patch[0], patch[1], patch[2], e);
+  DIT_LAUNCH_CHECK();
+  return DIT_OK;
+}
+
+// max_elems = the largest request's C*F*H*W (grid x); lat / out = the PACKED latents, patches / tok = [T, C*pv] in sequence rows
+dit_status launch_patchify_varlen(int dtype, const void* lat, void* patches, const SeqMeta* meta_dev, int R, int64_t max_elems,
+                                  int C, const int32_t patch[3], cudaStream_t st) {
+  if (R == 0 || max_elems == 0) return DIT_OK;
+  ProfScope _prof(DIT_KC_MISC, st);
+  const dim3 grid((unsigned)cdiv(max_elems, 256), (unsigned)R);
+  if (dtype == DIT_F32)
+    patchify_varlen_kernel<float><<<grid, 256, 0, st>>>((const float*)lat, (float*)patches, meta_dev, C, patch[0], patch[1], patch[2]);
+  else
+    patchify_varlen_kernel<bf16><<<grid, 256, 0, st>>>((const bf16*)lat, (bf16*)patches, meta_dev, C, patch[0], patch[1], patch[2]);
+  DIT_LAUNCH_CHECK();
+  return DIT_OK;
+}
+
+dit_status launch_unpatchify_varlen(int dtype, const float* tok, void* out, const SeqMeta* meta_dev, int R, int64_t max_elems,
+                                    int C, const int32_t patch[3], cudaStream_t st) {
+  if (R == 0 || max_elems == 0) return DIT_OK;
+  ProfScope _prof(DIT_KC_MISC, st);
+  const dim3 grid((unsigned)cdiv(max_elems, 256), (unsigned)R);
+  if (dtype == DIT_F32)
+    unpatchify_varlen_kernel<float><<<grid, 256, 0, st>>>(tok, (float*)out, meta_dev, C, patch[0], patch[1], patch[2]);
+  else
+    unpatchify_varlen_kernel<bf16><<<grid, 256, 0, st>>>(tok, (bf16*)out, meta_dev, C, patch[0], patch[1], patch[2]);
   DIT_LAUNCH_CHECK();
   return DIT_OK;
 }
