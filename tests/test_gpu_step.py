@@ -445,3 +445,56 @@ def test_argument_validation_on_gpu(lib):
         B.Dit(B.make_config(s), Wbad, DEV)
     m.dit_step(lat, temb, cond)
     assert B.dit_kernel_launches() > n0
+
+
+_PACKED_ENDS = r'''
+import sys, torch
+from paper_2606_13501_b200 import binding as B, synth
+B.load()
+dev = torch.device("cuda", 0)
+res = {}
+for mode, dtype in (("joint", "bf16"), ("cross", "bf16"), ("joint2", "bf16"), ("joint", "f32"), ("none", "f32")):
+    if dtype == "bf16":
+        s = synth.cfg1(name="x", dtype="bf16", hidden=512, n_heads=4, head_dim=128, mlp_dim=2048, cond_dim=512, latent_channels=16,
+                       rope_dims=(0, 64, 64), qk_rmsnorm=True, cond_mode=mode)
+    else:
+        s = synth.cfg1(cond_mode=mode, rope_dims=(0, 32, 32), qk_rmsnorm=True)
+    W = synth.make_weights(s, device=dev)
+    grids = [(1, 32, 32), (1, 16, 48), (1, 8, 8), (1, 64, 32), (1, 2, 2)]
+    ncs = [0 if mode == "none" else n for n in (32, 7, 0, 19, 32)]
+    R = len(grids)
+    T = sum((g[1] // 2) * (g[2] // 2) + (nc if mode in ("joint", "joint2") else 0) for g, nc in zip(grids, ncs))
+    m = B.Dit(B.make_config(s, max_requests=R, max_tokens=T, max_cond_tokens=max(1, sum(ncs))), W, dev)
+    lats = [synth.normal(5, f"l{r}", (s.latent_channels,) + g, dtype=s.torch_dtype, device=dev) for r, g in enumerate(grids)]
+    conds = None if mode == "none" else [synth.normal(5, f"c{r}", (nc, s.cond_dim), dtype=s.torch_dtype, device=dev) if nc else None
+                                         for r, nc in enumerate(ncs)]
+    temb = synth.timestep_embedding([100.0 * (r + 1) for r in range(R)], s.temb_dim, device=dev).contiguous()
+    n0 = B.dit_kernel_launches()
+    outs = m.dit_step_varlen(lats, temb, conds)
+    torch.cuda.synchronize()
+    res[f"{mode}-{dtype}"] = ([o.cpu() for o in outs], B.dit_kernel_launches() - n0)
+torch.save(res, sys.argv[1])
+'''
+
+
+def test_packed_step_ends_launched_once_are_bit_identical_to_per_request_launches(lib, tmp_path):
+    """A packed step launches patchify, the patch-embed GEMM, the final GEMM and unpatchify ONCE for all requests;
+    DIT_VARLEN_PER_REQUEST=1 (read once per process, hence the two subprocesses) launches them per request.  Five requests of
+    unequal grids and cond counts (one without cond tokens, one of a single token), every cond mode: same bits, 4 (R - 1) = 16
+    launches fewer."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    got = {}
+    for knob in ("0", "1"):
+        path = tmp_path / f"ends{knob}.pt"
+        env = dict(os.environ, DIT_VARLEN_PER_REQUEST=knob, PYTHONPATH=root + os.pathsep + os.environ.get("PYTHONPATH", ""))
+        r = subprocess.run([sys.executable, "-c", _PACKED_ENDS, str(path)], env=env, capture_output=True, text=True, timeout=600)
+        assert r.returncode == 0, r.stderr[-2000:]
+        got[knob] = torch.load(path)
+    for key, (outs, n_launch) in got["0"].items():
+        ref, n_ref = got["1"][key]
+        assert all(torch.isfinite(o.float()).all() for o in outs)
+        assert all(torch.equal(a, b) for a, b in zip(outs, ref)), key
+        assert n_ref - n_launch == 16, (key, n_launch, n_ref)
