@@ -419,6 +419,8 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
   const bool batched_ends = R > 1 && pair == nullptr && epi == nullptr && !per_request_env;
   int64_t max_elems = 0;
   for (int r = 0; r < R; ++r) max_elems = std::max<int64_t>(max_elems, g.lat_off[r + 1] - g.lat_off[r]);
+  // (joint modes) the cond projection too, when its fp32 result fits the MLP scratch it borrows
+  const bool cond_once = batched_ends && joint && g.cu_cond[R] > 0 && (size_t)g.cu_cond[R] * D * 4 <= (size_t)c.max_tokens * F * es;
   if (batched_ends) {
     RUN(launch_patchify_varlen(dt, latents, w.patches, w.meta_dev, R, max_elems, c.latent_channels, c.patch, st));
     RUN(gemm(dt, DIT_EPI_BIAS_F32, w.patches, pvC, hd->pe_w, hd->pe_b, w.x, D, T, D, pvC, st, DIT_KC_MISC));
@@ -433,9 +435,14 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
       RUN(launch_patchify(dt, (const char*)latents + g.lat_off[r] * es, pr, c.latent_channels, Fr, Hr, Wr, c.patch, st));
       RUN(gemm(dt, DIT_EPI_BIAS_F32, pr, pvC, hd->pe_w, hd->pe_b, w.x + (size_t)row0 * D, D, Nr, D, pvC, st, DIT_KC_MISC));
     }
-    if (joint && Lc > 0)
+    if (joint && Lc > 0 && !cond_once)
       RUN(gemm(dt, DIT_EPI_BIAS_F32, cond_of(r), c.cond_dim, hd->cp_w, hd->cp_b, w.x + (size_t)g.cu[r] * D, D, Lc, D,
                c.cond_dim, st, DIT_KC_MISC));
+  }
+  if (cond_once) {   // ONE cond projection over the packed cond tokens into scratch (w.u is free until the first MLP), then
+                     // one row scatter to the heads of the requests' segments: an exact fp32 copy
+    RUN(gemm(dt, DIT_EPI_BIAS_F32, cond, c.cond_dim, hd->cp_w, hd->cp_b, w.u, D, g.cu_cond[R], D, c.cond_dim, st, DIT_KC_MISC));
+    RUN(launch_scatter_cond_rows((const float*)w.u, w.x, w.cu_dev, w.cu_cond_dev, R, g.cu_cond[R], D, st));
   }
   const int Lc_total = g.cu_cond[R];
   // R36: in a bf16 step the cross-attention context and the final layer's input are kept as an unevaluated sum of two

@@ -703,6 +703,31 @@ dit_status launch_unpatchify(int dtype, const float* tok, void* out, int C, int 
   return DIT_OK;
 }
 
+// Rows of a [Lc_total, D] fp32 matrix packed by request -> the cond rows at the head of every request's segment of x
+// (row cu_cond[r] + i -> row cu[r] + i).  One thread per 4 elements.
+__global__ void scatter_cond_rows_kernel(const float* __restrict__ src, float* __restrict__ x, const int32_t* __restrict__ cu,
+                                         const int32_t* __restrict__ cu_cond, int R, int Lc_total, int D4) {
+  pdl_trigger();
+  pdl_wait();
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (int64_t)Lc_total * D4) return;
+  const int row = (int)(idx / D4), col = (int)(idx % D4);
+  const int r = find_request(cu_cond, R, row);
+  const int dst = cu[r] + (row - cu_cond[r]);
+  reinterpret_cast<float4*>(x)[(int64_t)dst * D4 + col] = reinterpret_cast<const float4*>(src)[idx];
+}
+
+dit_status launch_scatter_cond_rows(const float* src, float* x, const int32_t* cu_dev, const int32_t* cu_cond_dev, int R,
+                                    int Lc_total, int D, cudaStream_t st) {
+  if (Lc_total == 0) return DIT_OK;
+  ProfScope _prof(DIT_KC_MISC, st);
+  const int64_t n = (int64_t)Lc_total * (D / 4);
+  DIT_CUDA_OK(launch_pdl(scatter_cond_rows_kernel, dim3((unsigned)cdiv(n, 256)), dim3(256), 0, st, 1, src, x, cu_dev, cu_cond_dev, R,
+                         Lc_total, D / 4));
+  DIT_LAUNCH_CHECK();
+  return DIT_OK;
+}
+
 // max_elems = the largest request's C*F*H*W (grid x); lat / out = the PACKED latents, patches / tok = [T, C*pv] in sequence rows
 dit_status launch_patchify_varlen(int dtype, const void* lat, void* patches, const SeqMeta* meta_dev, int R, int64_t max_elems,
                                   int C, const int32_t patch[3], cudaStream_t st) {
