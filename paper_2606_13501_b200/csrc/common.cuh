@@ -212,6 +212,7 @@ dit_status launch_qknorm_rope(int dtype, void* qkv, int64_t row_stride, int T, i
                               cudaStream_t st);
 dit_status launch_rope_table(const SeqMeta* meta, int R, int T, int d, const int32_t rope_dims[3], float theta,
                              float* rc, float* rs, cudaStream_t st);
+dit_status launch_silu_split(const float* c, void* out, int R, int D, cudaStream_t st);
 dit_status launch_scatter_cond_rows(const float* src, float* x, const int32_t* cu_dev, const int32_t* cu_cond_dev, int R,
                                     int Lc_total, int D, cudaStream_t st);
 dit_status launch_patchify_varlen(int dtype, const void* lat, void* patches, const SeqMeta* meta_dev, int R, int64_t max_elems,

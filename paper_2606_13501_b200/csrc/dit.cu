@@ -405,7 +405,27 @@ static dit_status run_step(dit_handle hd, const StepGeom& g, const void* latents
   if (mod_pre == nullptr) {
     RUN(launch_gemv(dt, temb, w.gemv_tab + 0, nullptr, 1, D, w.c1, D, Rt, c.temb_dim, 0, st));
     RUN(launch_gemv(dt, w.c1, w.gemv_tab + 1, nullptr, 1, D, w.c, D, Rt, D, 1, st));
-    RUN(launch_gemv(dt, w.c, w.gemv_tab + 2, nullptr, dual ? 2 * L + 1 : L + 1, (int)mod_len, w.mod, mod_len, Rt, D, 1, st));
+    // The GEMV kernels take 8 input rows per pass over the weights.  A packed bf16 step of MORE than 8 requests runs the
+    // modulation as tensor-core GEMMs instead — SiLU(c) as an unevaluated [hi | lo] pair of bf16 rows (R36: ~16 significand
+    // bits), one M = R GEMM per modulation matrix, fp32 out: the weights are streamed once, not ceil(R / 8) times by passes that
+    // are FMA-bound at 8 rows (64 requests at the cfg 2 model: 3.4 ms of GEMV passes -> 0.3 ms).
+    static const bool mod_gemv_env = [] { const char* e = getenv("DIT_MOD_GEMV"); return e != nullptr && e[0] == '1'; }();
+    const bool mod_tc = dt == DIT_BF16 && Rt > 8 && !mod_gemv_env && D % 64 == 0 &&
+                        gemm_tc_supported(DIT_EPI_BIAS_F32, w.y, 2 * D, hd->fm_w, w.mod, mod_len, Rt, 2 * D, 2 * D);
+    if (mod_tc) {
+      RUN(launch_silu_split(w.c, w.y, Rt, D, st));   // w.y is free until the first adaLN
+      struct Override { int prev; Override() : prev(g_prof_class_override) { g_prof_class_override = DIT_KC_GEMV; }
+                        ~Override() { g_prof_class_override = prev; } } ov;
+      auto one = [&](const void* Wm, const void* bm, int N, int64_t off) -> dit_status {
+        return launch_gemm_tc(DIT_EPI_BIAS_F32, w.y, 2 * D, Wm, bm, w.mod + off, mod_len, Rt, N, D, st, 1);
+      };
+      for (int l = 0; l < L; ++l) RUN(one(hd->blocks[l].mod_w, hd->blocks[l].mod_b, 6 * D, (int64_t)l * 6 * D));
+      RUN(one(hd->fm_w, hd->fm_b, 2 * D, (int64_t)L * 6 * D));
+      if (dual)
+        for (int l = 0; l < L; ++l) RUN(one(hd->blocks[l].t_mod_w, hd->blocks[l].t_mod_b, 6 * D, mod_img + (int64_t)l * 6 * D));
+    } else {
+      RUN(launch_gemv(dt, w.c, w.gemv_tab + 2, nullptr, dual ? 2 * L + 1 : L + 1, (int)mod_len, w.mod, mod_len, Rt, D, 1, st));
+    }
   }
 
   if (hd->wait_before_embed != nullptr) DIT_CUDA_OK(cudaStreamWaitEvent(st, hd->wait_before_embed, 0));   // inputs uploaded

@@ -703,6 +703,28 @@ dit_status launch_unpatchify(int dtype, const float* tok, void* out, int C, int 
   return DIT_OK;
 }
 
+// out[r, 0..D) = bf16(SiLU(c[r, :])), out[r, D..2D) = bf16(SiLU(c) - hi): the [hi | lo] operand (R36) of the modulation GEMMs of a
+// packed step with more than 8 requests (dit.cu).  One thread per element.
+__global__ void silu_split_kernel(const float* __restrict__ c, bf16* __restrict__ out, int R, int D) {
+  pdl_trigger();
+  pdl_wait();
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= R * D) return;
+  const int r = idx / D, k = idx % D;
+  const float v = silu_f(c[idx]);
+  const bf16 hi = __float2bfloat16_rn(v);
+  out[(size_t)r * 2 * D + k] = hi;
+  out[(size_t)r * 2 * D + D + k] = __float2bfloat16_rn(v - __bfloat162float(hi));
+}
+
+dit_status launch_silu_split(const float* c, void* out, int R, int D, cudaStream_t st) {
+  if (R == 0) return DIT_OK;
+  ProfScope _prof(DIT_KC_GEMV, st);
+  DIT_CUDA_OK(launch_pdl(silu_split_kernel, dim3((unsigned)cdiv(R * D, 256)), dim3(256), 0, st, 1, c, (bf16*)out, R, D));
+  DIT_LAUNCH_CHECK();
+  return DIT_OK;
+}
+
 // Rows of a [Lc_total, D] fp32 matrix packed by request -> the cond rows at the head of every request's segment of x
 // (row cu_cond[r] + i -> row cu[r] + i).  One thread per 4 elements.
 __global__ void scatter_cond_rows_kernel(const float* __restrict__ src, float* __restrict__ x, const int32_t* __restrict__ cu,

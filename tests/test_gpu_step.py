@@ -357,6 +357,21 @@ def test_sixty_four_tiny_requests_packed(lib, mode):
                              [i["cond"].to(DEV) for i in Is])
     torch.cuda.synchronize()
     assert B.dit_fallback_launches() == n0
+    # more than 8 requests: the modulation runs as tensor-core GEMMs on a [hi | lo] bf16 pair of SiLU(c) (dit.cu) — the fp32
+    # modulation rows must still be the oracle's to ~2^-16 (the GEMV form, fp32 inputs, holds 2e-6)
+    sh0 = shapes[0]
+    n_img = sh0.n_blocks * 6 * sh0.hidden + 2 * sh0.hidden
+    mod_len = n_img + (sh0.n_blocks * 6 * sh0.hidden if mode == "joint2" else 0)
+    mod = m.dit_get_tap("mod", (R, mod_len), torch.float32)
+    torch.cuda.synchronize()
+    for r in (0, 9, 63):
+        cfg_r = O.cfg_from_shape(shapes[r])
+        c, mods, modf = O.conditioning(cfg_r, W, Is[r]["temb"])
+        want = torch.cat([torch.stack(mods, 0).reshape(-1), modf.reshape(-1)])
+        check(mod[r, :n_img], want, torch.float32, f"modulation rows of request {r} ({mode})", rel=2e-5, maxabs=2e-4)
+        if mode == "joint2":
+            want_t = torch.stack(O.conditioning_txt(cfg_r, W, c), 0).reshape(-1)
+            check(mod[r, n_img:], want_t, torch.float32, f"text-stream modulation rows of request {r}", rel=2e-5, maxabs=2e-4)
     for r in (0, 1, 2, 17, 40, 63):
         ref = O.dit_step(O.cfg_from_shape(shapes[r]), W, Is[r]["latents"], Is[r]["temb"], Is[r]["cond"])
         check(outs[r], ref, torch.bfloat16, f"64 packed requests ({mode}), request {r}")
