@@ -246,7 +246,7 @@ __global__ void __launch_bounds__(128) adaln_kernel(float* __restrict__ x, const
 
 // -------------------------------------------------------------------------------------------------
 // The same operation (without the h / gate residual) for launches of a few waves: a PERSISTENT grid (resident CTAs only),
-// every CTA walks rows b, b + G, b + 2G ... and keeps STAGES rows in flight in shared memory with 1-D bulk copies
+// every CTA walks its rows (strided or contiguous, see below) and keeps STAGES rows in flight in shared memory with 1-D bulk copies
 // (cp.async.bulk + mbarrier): the bytes in flight per SM no longer depend on registers or on how many CTAs have been
 // launched yet, and there is no wave tail — at cfg 2 (4352 rows of 12 KB) the one-row-per-CTA kernel above is 3.3 waves of
 // load -> reduce -> load modulation -> store chains.  128 threads per row, NCT = D / 1024 chunks of 8 per thread; the
@@ -271,8 +271,15 @@ __global__ void __launch_bounds__(128) adaln_stream_kernel(const float* __restri
   __shared__ __align__(8) uint64_t full[ADALN_STAGES];
   __shared__ float red[2][4];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  // One request: CTA b walks rows b, b + G, b + 2G ... (the CTAs read one moving window of the matrix).  Several requests: CTA b owns
+  // the CONTIGUOUS rows [b T / G, (b + 1) T / G) — it crosses a request boundary at most a few times, so the modulation rows are
+  // reloaded and the request looked up rarely (the strided walk changed request at every row of a many-request batch: 2.4x slower
+  // at 64 requests, 15 % at cfg 4's six)
   const int G = gridDim.x, b = blockIdx.x;
-  const int n_my = b < T_rows ? (T_rows - b + G - 1) / G : 0;
+  const bool multi = cu != nullptr && R > 1;
+  const int row_begin = multi ? (int)((int64_t)b * T_rows / G) : b;
+  const int row_step = multi ? 1 : G;
+  const int n_my = multi ? (int)((int64_t)(b + 1) * T_rows / G) - row_begin : (b < T_rows ? (T_rows - b + G - 1) / G : 0);
   if (tid == 0) {
     for (int s = 0; s < ADALN_STAGES; ++s) tc::mbar_init(tc::smem_u32(&full[s]), 1);
     tc::fence_barrier_init();
@@ -282,18 +289,20 @@ __global__ void __launch_bounds__(128) adaln_stream_kernel(const float* __restri
   if (tid == 0) {
     for (int s = 0; s < ADALN_STAGES && s < n_my; ++s) {
       tc::mbar_expect_tx(tc::smem_u32(&full[s]), D * 4);
-      bulk_load_1d(tc::smem_u32(stage + (size_t)s * D), x + (int64_t)(b + s * G) * D, D * 4, tc::smem_u32(&full[s]));
+      bulk_load_1d(tc::smem_u32(stage + (size_t)s * D), x + (int64_t)(row_begin + s * row_step) * D, D * 4, tc::smem_u32(&full[s]));
     }
   }
   __syncthreads();                                                            // barrier init visible to the waiting threads
   const int col0 = tid * 8;                                                   // chunk c of this thread starts at col0 + c * 1024
   float a[NCT][8], sft[NCT][8];
   int64_t cur = -1;
+  int seg = multi ? find_request(cu, R, row_begin) : 0;
   for (int i = 0; i < n_my; ++i) {
     const int s = i % ADALN_STAGES;
     const uint32_t ph = (uint32_t)(i / ADALN_STAGES) & 1u;
-    const int row = b + i * G;
-    const int seg = (cu != nullptr && R > 1) ? find_request(cu, R, row) : 0;
+    const int row = row_begin + i * row_step;
+    if (multi)
+      while (seg + 1 < R && row >= cu[seg + 1]) ++seg;
     const int64_t moff = set_off != 0 ? (int64_t)(seg >> 1) * mod_stride + ((seg & 1) ? 0 : set_off) : (int64_t)seg * mod_stride;
     if (moff != cur) {                                                        // uniform over the CTA
       cur = moff;
@@ -322,7 +331,7 @@ __global__ void __launch_bounds__(128) adaln_stream_kernel(const float* __restri
     __syncthreads();                                                          // also: every thread has read stage s
     if (tid == 0 && i + ADALN_STAGES < n_my) {
       tc::mbar_expect_tx(tc::smem_u32(&full[s]), D * 4);
-      bulk_load_1d(tc::smem_u32(stage + (size_t)s * D), x + (int64_t)(b + (i + ADALN_STAGES) * G) * D, D * 4,
+      bulk_load_1d(tc::smem_u32(stage + (size_t)s * D), x + (int64_t)(row + ADALN_STAGES * row_step) * D, D * 4,
                    tc::smem_u32(&full[s]));
     }
     const float mean = (red[0][0] + red[0][1] + red[0][2] + red[0][3]) * (1.0f / D);
